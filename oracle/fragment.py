@@ -1,0 +1,418 @@
+"""Fragment-encoding oracle: Algorithm 1 layout, the HConv operation graph, planner counts, AAC.
+TEST INFRASTRUCTURE ONLY -- see oracle/__init__.py.
+
+Follows PAPER.md:166-178 (Algorithm 1), PAPER.md:84-91 (Eq. 2, inner / outer rotations),
+PAPER.md:198-246 (Eq. 3-8), PAPER.md:252-276 (AAC), PAPER.md:284 (stride by dropping
+ciphertexts), with the readings R2.9-R2.11 / A3-A6, A13-A19 of DESIGN.md section 4.
+
+The graph is written once, over an abstract "backend" with rot / pmult_acc / add / finish, and
+run (i) on plain slot vectors, where a rotation is a cyclic shift -- the oracle-of-the-oracle
+pin against direct convolution -- and (ii) on oracle ciphertexts (oracle/ckks.py).
+"""
+import math
+from fractions import Fraction
+
+import numpy as np
+
+
+def next_pow2(x: int) -> int:
+    return 1 << max(0, (x - 1).bit_length())
+
+
+# --------------------------------------------------------------------------- Algorithm 1 (R2.9)
+class Layout:
+    """Layout(n, M, S, BS, C): ciphertext (u, v, g, bg) holds at slot(cpos, k, b) the value
+    X_pad[bg*B + b, g*ch + cpos, bi*S + u, bj*S + v], k = bi*m + bj  (PAPER.md:170-176 read
+    0-based with floors, A3; "filled first with other samples then other channels")."""
+
+    def __init__(self, n, M, S, BS, C):
+        assert M % S == 0
+        self.n, self.M, self.S, self.BS, self.C = n, M, S, BS, C
+        self.m = M // S
+        m2 = self.m * self.m
+        assert m2 <= n and n % m2 == 0, "m^2 must divide the slot count"
+        self.B = min(next_pow2(BS), n // m2)
+        self.ch = n // (self.B * m2)
+        self.cs = self.B * m2
+        self.G = -(-C // self.ch)
+        self.BG = -(-BS // self.B)
+
+    def slot(self, cpos, k, b):
+        return cpos * self.cs + k * self.B + b
+
+    def ct_keys(self):
+        return [(u, v, g, bg) for bg in range(self.BG) for g in range(self.G) for u in range(self.S) for v in range(self.S)]
+
+    def gather(self, X, u, v, g, bg):
+        """Slot vector of ciphertext (u, v, g, bg) for X[BS, C, H, W] (zero outside the tensor)."""
+        BS, C, H, W = X.shape
+        vec = np.zeros(self.n, dtype=np.float64)
+        for cpos in range(self.ch):
+            c = g * self.ch + cpos
+            if c >= C:
+                continue
+            for b in range(self.B):
+                bb = bg * self.B + b
+                if bb >= BS:
+                    continue
+                for bi in range(self.m):
+                    h = bi * self.S + u
+                    if h >= H:
+                        continue
+                    for bj in range(self.m):
+                        w = bj * self.S + v
+                        if w < W:
+                            vec[self.slot(cpos, bi * self.m + bj, b)] = X[bb, c, h, w]
+        return vec
+
+    def scatter(self, Y, vec, u, v, g, bg):
+        """Inverse of gather: write this ciphertext's entries into Y[BS, C, H, W]."""
+        BS, C, H, W = Y.shape
+        for cpos in range(self.ch):
+            c = g * self.ch + cpos
+            if c >= C:
+                continue
+            for b in range(self.B):
+                bb = bg * self.B + b
+                if bb >= BS:
+                    continue
+                for bi in range(self.m):
+                    h = bi * self.S + u
+                    if h >= H:
+                        continue
+                    for bj in range(self.m):
+                        w = bj * self.S + v
+                        if w < W:
+                            Y[bb, c, h, w] = vec[self.slot(cpos, bi * self.m + bj, b)]
+
+
+class ConvDesc:
+    def __init__(self, BS, C_in, H, W, C_out, K, stride=1, pad=0, depthwise=False, S=0, M=0):
+        self.BS, self.C_in, self.H, self.W, self.C_out, self.K = BS, C_in, H, W, C_out, K
+        self.stride, self.pad, self.depthwise, self.S, self.M = stride, pad, depthwise, S, M
+        self.H_out = (H + 2 * pad - K) // stride + 1
+        self.W_out = (W + 2 * pad - K) // stride + 1
+
+
+def direct_conv(desc: ConvDesc, X, Kw):
+    """Eq. 2 with stride and zero padding, fp64, plain loops over taps."""
+    BS, Ci, H, W = X.shape
+    Y = np.zeros((BS, desc.C_out, desc.H_out, desc.W_out), dtype=np.float64)
+    Xp = np.zeros((BS, Ci, H + 2 * desc.pad, W + 2 * desc.pad), dtype=np.float64)
+    Xp[:, :, desc.pad:desc.pad + H, desc.pad:desc.pad + W] = X
+    s = desc.stride
+    for o in range(desc.C_out):
+        for c in ([o] if desc.depthwise else range(Ci)):
+            for i in range(desc.K):
+                for j in range(desc.K):
+                    w = Kw[o, 0 if desc.depthwise else c, i, j]
+                    Y[:, o] += w * Xp[:, c, i:i + s * desc.H_out:s, j:j + s * desc.W_out:s]
+    return Y
+
+
+# --------------------------------------------------------------------------- the HConv graph (R2.9)
+class ConvGraph:
+    """Static operation graph of one fragment-encoded conv layer for one batch group.
+
+    terms[(u_o, v_o, g_out)][d] = list of (src_key (u', v', g_in), amt, wkey (u_o, v_o, g_out, g_in, d, i, j));
+    inner = sorted set of (src_key, amt != 0); outer[(u_o, v_o, g_out)] = existing diagonals d."""
+
+    def __init__(self, desc: ConvDesc, n: int):
+        d = desc
+        self.desc, self.n = d, n
+        self.M = d.M if d.M else next_pow2(max(d.H, d.W))
+        self.S = d.S
+        assert self.S >= 1 and self.S % d.stride == 0, "stride must divide S"
+        self.lin = Layout(n, self.M, self.S, d.BS, d.C_in)
+        self.S_out = self.S // d.stride
+        self.lout = Layout(n, self.M // d.stride, self.S_out, d.BS, d.C_out)
+        assert (self.lout.m, self.lout.B, self.lout.ch) == (self.lin.m, self.lin.B, self.lin.ch)
+        self._wcache = {}
+        self.terms, inner = {}, set()
+        L = self.lin
+        for uo in range(self.S_out):
+            for vo in range(self.S_out):
+                for go in range(self.lout.G):
+                    diags = {}
+                    for dd in range(L.ch):
+                        lst = []
+                        for gi in range(L.G):
+                            for i in range(d.K):
+                                for j in range(d.K):
+                                    wkey = (uo, vo, go, gi, dd, i, j)
+                                    if not self.weight_nonzero_pattern(wkey):
+                                        continue
+                                    ti = d.stride * uo + i - d.pad
+                                    tj = d.stride * vo + j - d.pad
+                                    up, di = ti % self.S, ti // self.S  # floor division, may be negative
+                                    vp, dj = tj % self.S, tj // self.S
+                                    amt = ((di * L.m + dj) * L.B) % n
+                                    lst.append(((up, vp, gi), amt, wkey))
+                                    if amt:
+                                        inner.add(((up, vp, gi), amt))
+                        if lst:
+                            diags[dd] = lst
+                    self.terms[(uo, vo, go)] = diags
+        self.inner = sorted(inner)
+
+    # Which entries of weight plaintext wkey can be non-zero (independent of the values).  The validity
+    # conditions of R2.9 step 2 factorise: channel positions (c < C_in, o < C_out, depthwise o == c),
+    # block rows (h_o < H_o, 0 <= h_i < H) and block columns (w_o < W_o, 0 <= w_i < W).
+    def _valid_cpos(self, go, gi, dd):
+        key = ("c", go, gi, dd)
+        if key not in self._wcache:
+            d, L = self.desc, self.lin
+            out = []
+            for cpos in range(L.ch):
+                c = gi * L.ch + cpos
+                o = go * L.ch + ((cpos - dd) % L.ch)
+                if c < d.C_in and o < d.C_out and (not d.depthwise or o == c):
+                    out.append((cpos, o, c))
+            self._wcache[key] = out
+        return self._wcache[key]
+
+    def _valid_blocks(self, frag_o, tap, size_in, size_out):
+        """Block indices bi with h_o = bi*S_o + frag_o < size_out and 0 <= stride*h_o + tap - pad < size_in."""
+        key = ("b", frag_o, tap, size_in, size_out)
+        if key not in self._wcache:
+            d = self.desc
+            out = []
+            for bi in range(self.lin.m):
+                ho = bi * self.S_out + frag_o
+                hi = d.stride * ho + tap - d.pad
+                if ho < size_out and 0 <= hi < size_in:
+                    out.append(bi)
+            self._wcache[key] = out
+        return self._wcache[key]
+
+    def _weight_factors(self, wkey):
+        uo, vo, go, gi, dd, i, j = wkey
+        d = self.desc
+        return (self._valid_cpos(go, gi, dd), self._valid_blocks(uo, i, d.H, d.H_out), self._valid_blocks(vo, j, d.W, d.W_out))
+
+    def weight_nonzero_pattern(self, wkey):
+        cp, rows, cols = self._weight_factors(wkey)
+        return bool(cp) and bool(rows) and bool(cols)
+
+    def weight_slots(self, wkey, Kw):
+        """Slot vector W(u_o, v_o, g_out, g_in, d, i, j) (R2.9 step 2); all b alike."""
+        _, _, _, _, _, i, j = wkey
+        L = self.lin
+        cp, rows, cols = self._weight_factors(wkey)
+        vec = np.zeros(self.n, dtype=np.float64)
+        for cpos, o, c in cp:
+            val = Kw[o, 0 if self.desc.depthwise else c, i, j]
+            for bi in rows:
+                for bj in cols:
+                    base = L.slot(cpos, bi * L.m + bj, 0)
+                    vec[base:base + L.B] = val
+        return vec
+
+    # ---- exact counts of this graph (per batch group; multiply by BG for the layer)
+    def counts(self):
+        n_outer = 0
+        n_pmult = 0
+        for diags in self.terms.values():
+            n_outer += len([x for x in diags if x != 0])  # every existing diagonal d != 0 is rotated once
+            n_pmult += sum(len(v) for v in diags.values())
+        bg = self.lin.BG
+        steps = sorted({amt for _, amt in self.inner} | {dd * self.lin.cs % self.n for diags in self.terms.values() for dd in diags if dd})
+        return dict(n_in_ct=self.S * self.S * self.lin.G * bg, n_out_ct=self.S_out ** 2 * self.lout.G * bg,
+                    n_inner_rot=len(self.inner) * bg, n_outer_rot=n_outer * bg, n_pmult=n_pmult * bg,
+                    n_distinct_pt=n_pmult, rot_steps=steps)
+
+    # ---- run the graph on a backend (R2.9 steps 1, 3, 4; rescale / finish is the caller's)
+    def run(self, be, inputs, weights):
+        """inputs: {(u, v, g_in): x}; weights: {wkey: w}.  Returns {(u_o, v_o, g_out): y}."""
+        R = {}
+        for src, amt in self.inner:
+            R[(src, amt)] = be.rot(inputs[src], amt)  # always from the original input, never chained
+        out = {}
+        for okey, diags in self.terms.items():
+            y = None
+            for dd in sorted(diags):
+                acc = be.zero()
+                for src, amt, wkey in diags[dd]:
+                    be.pmult_acc(acc, R[(src, amt)] if amt else inputs[src], weights[wkey])
+                pd = be.wrap(acc)
+                if dd:
+                    pd = be.rot(pd, dd * self.lin.cs % self.n)
+                y = pd if y is None else be.add(y, pd)
+            out[okey] = y
+        return out
+
+
+class SlotBackend:
+    """Plain slot vectors: rotation = cyclic left shift, PMult = slot-wise product."""
+
+    def __init__(self, n):
+        self.n = n
+
+    def rot(self, x, r):
+        return np.roll(x, -r)
+
+    def zero(self):
+        return np.zeros(self.n)
+
+    def pmult_acc(self, acc, x, w):
+        acc += x * w
+
+    def wrap(self, acc):
+        return acc
+
+    def add(self, x, y):
+        return x + y
+
+
+def hconv_slots(desc: ConvDesc, n: int, X, Kw):
+    """The graph on plain slot vectors -> Y[BS, C_out, H_out, W_out]."""
+    g = ConvGraph(desc, n)
+    be = SlotBackend(n)
+    W = {wk: g.weight_slots(wk, Kw) for diags in g.terms.values() for lst in diags.values() for _, _, wk in lst}
+    Y = np.zeros((desc.BS, desc.C_out, desc.H_out, desc.W_out))
+    for bg in range(g.lin.BG):
+        ins = {(u, v, gi): g.lin.gather(X, u, v, gi, bg) for u in range(g.S) for v in range(g.S) for gi in range(g.lin.G)}
+        outs = g.run(be, ins, W)
+        for (uo, vo, go), y in outs.items():
+            if y is not None:
+                g.lout.scatter(Y, y, uo, vo, go, bg)
+    return Y
+
+
+# --------------------------------------------------------------------------- planner (R2.10, Eq. 3-8)
+def alpha_ch(n, M):
+    """Channels per ciphertext at S = 1, BS = 1 as a rational: n / M^2 (A16)."""
+    return Fraction(n, M * M)
+
+
+def paper_inner_per_ct(S, K, M):
+    """Eq. 3 per input ciphertext, with Table IX's evident 0 for K <= S (A6)."""
+    if S >= M or K <= S:
+        return 0
+    return (-(-K // S)) ** 2 - 1
+
+
+def paper_rot_count(desc: ConvDesc, n, S):
+    """#Rot as Table IX prints it: n_in * I(S, K) + n_out * (ch - 1), with
+    n_in = N_in*BS/alpha, n_out = N_out*BS/alpha (A18), ch = alpha*S^2/BS (Eq. 4)."""
+    M = desc.M if desc.M else next_pow2(max(desc.H, desc.W))
+    a = alpha_ch(n, M)
+    n_in = Fraction(desc.C_in * desc.BS) / a
+    n_out = Fraction(desc.C_out * desc.BS) / a
+    ch = a * S * S / desc.BS
+    tot = n_in * paper_inner_per_ct(S, desc.K, M) + n_out * (ch - 1)
+    return tot
+
+
+def s_star_real(desc: ConvDesc, n):
+    """Eq. 8 with the BS factor restored (A5): (K^2 N_in BS / (alpha N_out))^(1/4)."""
+    M = desc.M if desc.M else next_pow2(max(desc.H, desc.W))
+    return (desc.K ** 2 * desc.C_in * desc.BS / (float(alpha_ch(n, M)) * desc.C_out)) ** 0.25
+
+
+def candidates(desc: ConvDesc, n):
+    """Feasible block sizes: powers of two with S | M, stride | S, m^2 <= n, and Eq. 7
+    S <= sqrt(BS N_in / alpha) unless that leaves none (then the smallest feasible)."""
+    M = desc.M if desc.M else next_pow2(max(desc.H, desc.W))
+    feas = [S for S in (1 << k for k in range(0, 12)) if S <= M and M % S == 0 and S % desc.stride == 0 and (M // S) ** 2 <= n]
+    bound = math.sqrt(desc.BS * desc.C_in / float(alpha_ch(n, M)))
+    ok = [S for S in feas if S <= bound]
+    return ok if ok else feas[:1]
+
+
+def with_S(desc: ConvDesc, S):
+    return ConvDesc(desc.BS, desc.C_in, desc.H, desc.W, desc.C_out, desc.K, desc.stride, desc.pad, desc.depthwise, S, desc.M)
+
+
+def select_S(desc: ConvDesc, n):
+    """Conv-aware selection: arg-min of the exact rotation count over the candidates, ties -> smaller S."""
+    best = None
+    for S in candidates(desc, n):
+        c = ConvGraph(with_S(desc, S), n).counts()
+        tot = c["n_inner_rot"] + c["n_outer_rot"]
+        if best is None or tot < best[0]:
+            best = (tot, S)
+    return best[1]
+
+
+# --------------------------------------------------------------------------- encrypted HConv (R2.9)
+class CtBackend:
+    def __init__(self, ck, params, keys, L, scale_in, scale_w):
+        self.ck, self.params, self.keys, self.L = ck, params, keys, L
+        self.scale_in, self.scale_w = Fraction(scale_in), Fraction(scale_w)
+
+    def rot(self, x, r):
+        return self.ck.rotate(self.params, self.keys, x, r)
+
+    def zero(self):
+        return np.zeros((2, self.L, self.params.N), dtype=np.uint64)
+
+    def pmult_acc(self, acc, x, w):
+        assert x.scale == self.scale_in and w.scale == self.scale_w
+        self.ck.pmult_acc(self.params, acc, x, w)
+
+    def wrap(self, acc):
+        return self.ck.Ciphertext(acc, self.L, self.scale_in * self.scale_w)
+
+    def add(self, x, y):
+        return self.ck.add(self.params, x, y)
+
+
+def encode_weights(ck, params, graph: ConvGraph, Kw, L, scale_w=None):
+    """Every non-zero weight plaintext of the graph, encoded at s_w (default q_{L-1}, A14) on L limbs."""
+    sw = Fraction(params.q[L - 1]) if scale_w is None else Fraction(scale_w)
+    W = {}
+    for diags in graph.terms.values():
+        for lst in diags.values():
+            for _, _, wk in lst:
+                if wk not in W:
+                    W[wk] = ck.encode(params, graph.weight_slots(wk, Kw), L, sw)
+    return W
+
+
+def hconv(ck, params, keys, graph: ConvGraph, inputs, weights, do_rescale=True):
+    """inputs {(u, v, g_in): Ciphertext} of ONE batch group -> {(u_o, v_o, g_out): Ciphertext};
+    one rescale per output ciphertext after the outer-rotation sum (A13)."""
+    any_in = next(iter(inputs.values()))
+    any_w = next(iter(weights.values()))
+    be = CtBackend(ck, params, keys, any_in.L, any_in.scale, any_w.scale)
+    outs = graph.run(be, inputs, weights)
+    if do_rescale:
+        outs = {k: (ck.rescale(params, y) if y is not None else None) for k, y in outs.items()}
+    return outs
+
+
+# --------------------------------------------------------------------------- AAC compress (R2.11)
+def compress_plan(n, ch, cs, v, n_src):
+    """Canonical batch-group compaction: sources hold valid channel positions [0, v), v | ch, v < ch;
+    output t gathers sources i in [t*ch/v, (t+1)*ch/v) with r = (n - (i mod (ch/v)) * v * cs) mod n
+    (a right shift by whole v-position segments).  Returns [[(src, r), ...], ...]."""
+    assert ch % v == 0 and v < ch
+    per = ch // v
+    plan = []
+    for t in range(-(-n_src // per)):
+        plan.append([(i, (n - (i % per) * v * cs) % n) for i in range(t * per, min((t + 1) * per, n_src))])
+    return plan
+
+
+def compress_mask(n, cs, v):
+    """0/1 slot vector keeping channel positions [0, v) (constant over k and b)."""
+    m = np.zeros(n)
+    m[: v * cs] = 1.0
+    return m
+
+
+def compress(ck, params, keys, plan, srcs, mask_pt=None, do_rescale=False):
+    """out_t = sum over terms Rot(mask (*) src, r).  Maskless: no level consumed.  Masked split-scale
+    (PAPER.md:276): sources at scale s_ct*Delta1 (conv rescale skipped), mask at Delta2, one rescale after."""
+    outs = []
+    for terms in plan:
+        y = None
+        for i, r in terms:
+            x = srcs[i]
+            if mask_pt is not None:
+                x = ck.pmult(params, x, mask_pt)
+            x = ck.rotate(params, keys, x, r)
+            y = x if y is None else ck.add(params, y, x)
+        outs.append(ck.rescale(params, y) if do_rescale else y)
+    return outs

@@ -1,0 +1,222 @@
+"""Pins for oracle/fragment.py (CPU only): the paper's printed values (tests/golden/), its worked
+examples, special cases, and direct fp64 convolution (Eq. 2)."""
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+from oracle import ckks as ck
+from oracle import fragment as fr
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _table_ix():
+    rows = []
+    for line in open(os.path.join(GOLD, "table_ix_rot.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        rows.append(tuple(int(x) for x in line.split()))
+    return rows
+
+
+def _paper_values():
+    out = {}
+    for line in open(os.path.join(GOLD, "paper_values.txt")):
+        line = line.split("#")[0].split()
+        if line:
+            out[line[0]] = [float(x) for x in line[1:]]
+    return out
+
+
+# ------------------------------------------------------------------ Table IX
+def test_table_ix_closed_form_all_15_rows():
+    n = 1 << 14  # N = 2^15
+    for cin, cout, K, BS, H, W, S, rot in _table_ix():
+        d = fr.ConvDesc(BS, cin, H, W, cout, K, 1, (K - 1) // 2, S=S)
+        assert fr.paper_rot_count(d, n, S) == rot
+
+
+def test_table_ix_exact_graph_counts():
+    """The exact graph count equals the printed value when K > S, S | (K-1) and C_out >= ch (A6, A19);
+    elsewhere it exceeds it by the edge term / the sparse-output term."""
+    n = 1 << 14
+    equal, differ = 0, 0
+    for cin, cout, K, BS, H, W, S, rot in _table_ix():
+        d = fr.ConvDesc(BS, cin, H, W, cout, K, 1, (K - 1) // 2, S=S)
+        g = fr.ConvGraph(d, n)
+        c = g.counts()
+        tot = c["n_inner_rot"] + c["n_outer_rot"]
+        if K > S and (K - 1) % S == 0 and cout >= g.lin.ch:
+            assert tot == rot
+            equal += 1
+        else:
+            assert tot >= rot
+            differ += 1
+        # exact closed forms of this graph (R2.9): inner per group of S^2 fragments = (K-1)(2S+K-1)
+        assert c["n_inner_rot"] == (K - 1) * (2 * S + K - 1) * g.lin.G * g.lin.BG
+        assert c["n_in_ct"] == cin * BS * 32 * 32 // n
+    assert equal == 10 and differ == 5
+
+
+def test_s_star_matches_printed_example():
+    d = fr.ConvDesc(8, 128, 32, 32, 32, 9, 1, 4)
+    assert abs(fr.s_star_real(d, 1 << 14) - _paper_values()["s_star_conv128_32_9_bs8"][0]) < 0.005
+    # the measured optimum in Table IX for this shape is S = 4; so is the exact-count arg-min over its three sizes
+    tot = {}
+    for S in (2, 4, 8):
+        c = fr.ConvGraph(fr.with_S(d, S), 1 << 14).counts()
+        tot[S] = c["n_inner_rot"] + c["n_outer_rot"]
+    assert min(tot, key=tot.get) == 4
+
+
+# ------------------------------------------------------------------ Fig. 4 toy
+def test_fig4_toy_rotation_profile():
+    n = int(_paper_values()["fig4_slots"][0])
+    prof = {}
+    for S in (1, 2, 4):
+        g = fr.ConvGraph(fr.ConvDesc(1, 16, 4, 4, 16, 3, 1, 1, S=S), n)
+        c = g.counts()
+        prof[S] = (c["n_inner_rot"], c["n_outer_rot"])
+        assert g.lin.B * g.lin.ch * g.lin.m ** 2 == n and c["n_in_ct"] == 16  # fully packed, 16 ciphertexts
+    assert prof[1][1] == 0 and prof[1][0] == 16 * 8       # S=1: no outer rotations, K^2-1 inner per ct
+    assert prof[4][0] == 0 and prof[4][1] == 16 * 15      # S=M: no inner, maximal outer
+    assert sum(prof[2]) < sum(prof[1]) and sum(prof[2]) < sum(prof[4])  # S=2 optimal
+    assert fr.select_S(fr.ConvDesc(1, 16, 4, 4, 16, 3, 1, 1), n) == 2
+
+
+# ------------------------------------------------------------------ Algorithm 1 layout
+def test_layout_4x4_example():
+    pv = _paper_values()
+    X = np.arange(16, dtype=np.float64).reshape(1, 1, 4, 4) + 1
+    l2 = fr.Layout(4, 4, 2, 1, 1)
+    assert len(l2.ct_keys()) == pv["map4x4_S2_cts"][0]
+    for (u, v, g, bg) in l2.ct_keys():
+        vec = l2.gather(X, u, v, g, bg)
+        assert np.count_nonzero(vec) == 4  # dense: 4 slots, 4 pixels
+        assert list(vec) == [X[0, 0, bi * 2 + u, bj * 2 + v] for bi in range(2) for bj in range(2)]
+    l4 = fr.Layout(4, 4, 4, 1, 1)
+    assert len(l4.ct_keys()) == pv["map4x4_S4_cts"][0]
+    assert all(np.count_nonzero(l4.gather(X, u, v, 0, 0)) == 1 for u in range(4) for v in range(4))  # 25 %
+
+
+def test_layout_special_cases_and_round_trip():
+    rng = np.random.default_rng(0)
+    X = rng.uniform(-1, 1, (1, 4, 8, 8))
+    # S = 1, BS = 1: row-major, channel after channel
+    l1 = fr.Layout(256, 8, 1, 1, 4)
+    assert np.array_equal(l1.gather(X, 0, 0, 0, 0), X.reshape(-1))
+    # S = M: one pixel per ciphertext, channels along the slots
+    lm = fr.Layout(4, 8, 8, 1, 4)
+    assert np.array_equal(lm.gather(X, 3, 5, 0, 0), X[0, :, 3, 5])
+    # batch first, then channels: slot index = cpos*cs + k*B + b
+    Xb = rng.uniform(-1, 1, (3, 5, 6, 7))
+    lb = fr.Layout(128, 8, 2, 3, 5)
+    assert (lb.B, lb.ch, lb.G, lb.BG) == (4, 2, 3, 1)
+    Y = np.zeros_like(Xb)
+    for key in lb.ct_keys():
+        lb.scatter(Y, lb.gather(Xb, *key), *key)
+    assert np.array_equal(Y, Xb)
+    v = lb.gather(Xb, 1, 0, 1, 0)
+    assert v[lb.slot(1, 2 * 4 + 3, 2)] == Xb[2, 3, 2 * 2 + 1, 3 * 2 + 0]
+
+
+# ------------------------------------------------------------------ the graph on plain slots vs Eq. 2
+SHAPES = [
+    # BS Cin H W Cout K s p dw S n
+    (1, 16, 4, 4, 16, 3, 1, 1, False, 1, 16), (1, 16, 4, 4, 16, 3, 1, 1, False, 2, 16), (1, 16, 4, 4, 16, 3, 1, 1, False, 4, 16),
+    (2, 4, 8, 8, 8, 3, 2, 1, False, 2, 64), (2, 4, 8, 8, 8, 3, 2, 1, False, 4, 64),
+    (1, 8, 8, 8, 8, 3, 1, 1, True, 2, 128), (3, 8, 8, 8, 8, 3, 2, 1, True, 2, 128),
+    (1, 8, 8, 8, 4, 1, 1, 0, False, 1, 128), (1, 2, 12, 12, 3, 5, 1, 0, False, 2, 256),
+    (1, 1, 28, 28, 6, 5, 1, 2, False, 1, 4096), (1, 1, 28, 28, 6, 5, 1, 2, False, 2, 4096),
+    (5, 3, 7, 6, 5, 3, 1, 1, False, 4, 32), (2, 6, 8, 8, 6, 2, 2, 0, True, 2, 64),
+]
+
+
+@pytest.mark.parametrize("shape", SHAPES)
+def test_graph_on_slots_equals_direct_conv(shape):
+    BS, Ci, H, W, Co, K, s, p, dw, S, n = shape
+    rng = np.random.default_rng(hash(shape) % 2 ** 32)
+    d = fr.ConvDesc(BS, Ci, H, W, Co, K, s, p, dw, S=S)
+    X = rng.uniform(-1, 1, (BS, Ci, H, W))
+    Kw = rng.normal(0, 0.1, (Co, 1 if dw else Ci, K, K))
+    assert np.abs(fr.hconv_slots(d, n, X, Kw) - fr.direct_conv(d, X, Kw)).max() < 1e-12
+
+
+def test_direct_conv_against_hand_example():
+    # 1x1x3x3 input, 2x2 kernel, no padding: 4 outputs computed by hand
+    X = np.arange(9, dtype=np.float64).reshape(1, 1, 3, 3)
+    Kw = np.array([[[[1.0, 2.0], [3.0, 4.0]]]])
+    Y = fr.direct_conv(fr.ConvDesc(1, 1, 3, 3, 1, 2), X, Kw)
+    assert Y.reshape(-1).tolist() == [0 + 2 + 9 + 16, 1 + 4 + 12 + 20, 3 + 8 + 18 + 28, 4 + 10 + 21 + 32]
+
+
+def test_lenet_conv1_counts_config1():
+    d = fr.ConvDesc(1, 1, 28, 28, 6, 5, 1, 2)
+    assert fr.select_S(d, 4096) == 1  # Eq. 7: sqrt(BS*C_in/alpha) = 0.5 < 1 -> smallest feasible
+    c = fr.ConvGraph(fr.with_S(d, 1), 4096).counts()
+    assert (c["n_in_ct"], c["n_out_ct"], c["n_inner_rot"], c["n_outer_rot"], c["n_pmult"]) == (1, 2, 24, 4, 150)
+    assert len(c["rot_steps"]) == 27
+
+
+# ------------------------------------------------------------------ encrypted HConv on the Fig. 4 toy (N = 32)
+@pytest.fixture(scope="module")
+def toy32():
+    P = ck.Params(5, 3, 36, 1, 40, 3, 30)  # 16 slots, dlen = 1
+    return P
+
+
+@pytest.mark.parametrize("S", [1, 2, 4])
+def test_encrypted_hconv_fig4(toy32, S):
+    P = toy32
+    rng = np.random.default_rng(S)
+    d = fr.ConvDesc(1, 16, 4, 4, 16, 3, 1, 1, S=S)
+    g = fr.ConvGraph(d, P.n)
+    X = rng.uniform(-1, 1, (1, 16, 4, 4))
+    Kw = rng.normal(0, 0.3, (16, 16, 3, 3))
+    keys = ck.keygen(P, 5, g.counts()["rot_steps"])
+    W = fr.encode_weights(ck, P, g, Kw, P.nq)
+    ins = {}
+    for i, (u, v, gi, bg) in enumerate(g.lin.ct_keys()):
+        ins[(u, v, gi)] = ck.encrypt(P, keys, ck.encode(P, g.lin.gather(X, u, v, gi, bg), P.nq), 100 + i)
+    outs = fr.hconv(ck, P, keys, g, ins, W)
+    Y = np.zeros((1, 16, 4, 4))
+    for (uo, vo, go), y in outs.items():
+        assert y.L == P.nq - 1 and y.scale == P.scale
+        g.lout.scatter(Y, ck.decrypt_decode(P, keys, y).real, uo, vo, go, 0)
+    assert np.abs(Y - fr.direct_conv(d, X, Kw)).max() < 1e-3
+
+
+# ------------------------------------------------------------------ AAC (Fig. 5)
+def test_compress_fig5_shape(toy32):
+    """8 -> 2 -> 8 bottleneck: 4 sources at 25 % (2 of 8 channel positions) -> 1 dense ciphertext;
+    maskless adds no level; masked split-scale costs exactly the one rescale."""
+    P = toy32
+    n, ch, v = P.n, 8, 2
+    cs = n // ch
+    n_src = int(_paper_values()["fig5_sources"][0])
+    plan = fr.compress_plan(n, ch, cs, v, n_src)
+    assert len(plan) == 1 and len(plan[0]) == 4
+    keys = ck.keygen(P, 9, [r for _, r in plan[0]])
+    rng = np.random.default_rng(1)
+    zs = []
+    for i in range(n_src):
+        z = np.zeros(n)
+        z[: v * cs] = rng.uniform(-1, 1, v * cs)
+        zs.append(z)
+    exp = np.concatenate([z[: v * cs] for z in zs])  # segmented layout: seg*(v*cs) + cpos*cs + k*B + b
+    srcs = [ck.encrypt(P, keys, ck.encode(P, z, P.nq), 50 + i) for i, z in enumerate(zs)]
+    out = fr.compress(ck, P, keys, plan, srcs)[0]
+    assert out.L == P.nq and out.scale == P.scale
+    assert np.abs(ck.decrypt_decode(P, keys, out).real - exp).max() < 1e-4
+    # masked: sources carry garbage outside the kept positions and sit at scale s*Delta1; mask at Delta2
+    q = P.q[P.nq - 1]
+    d1 = Fraction(2) ** ((q.bit_length() + 1) // 2)
+    d2 = Fraction(q) / d1
+    dirty = [z + np.concatenate([np.zeros(v * cs), rng.uniform(-1, 1, n - v * cs)]) for z in zs]
+    srcs = [ck.encrypt(P, keys, ck.encode(P, z, P.nq, P.scale * d1), 60 + i) for i, z in enumerate(dirty)]
+    mpt = ck.encode(P, fr.compress_mask(n, cs, v), P.nq, d2)
+    out = fr.compress(ck, P, keys, plan, srcs, mask_pt=mpt, do_rescale=True)[0]
+    assert out.L == P.nq - 1 and out.scale == P.scale
+    assert np.abs(ck.decrypt_decode(P, keys, out).real - exp).max() < 1e-3
