@@ -1,0 +1,200 @@
+/*
+ * fenc.h -- C ABI of libfenc: the B200-native (sm_100a) hot path of FEnc^2 (arxiv/paper_2606_16359):
+ * a CKKS homomorphic convolution layer over fragment-encoded ciphertexts.
+ *
+ * Citations are "PAPER.md:<line>" (the paper) or "DESIGN.md R2.x / A-n" (the readings this build takes
+ * where the paper is silent; the paper only names the CKKS primitives).
+ *
+ * Conventions
+ *  - Plain C, no exceptions cross the boundary.  Every function returns fenc_status (0 = OK); outputs are
+ *    written only on success.  fenc_last_error(ctx) returns a text for the last failure on that context.
+ *  - "host" pointers are ordinary CPU memory owned by the caller; the library copies what it needs before
+ *    returning.  "device" pointers are CUDA global memory on the context's device.
+ *  - Handles (fenc_ctx, fenc_keys, fenc_pt, fenc_ct, fenc_wts) are opaque, created by the library and
+ *    destroyed by the matching *_free (NULL-safe).  A handle must be freed before its context.
+ *  - Device memory comes from the allocator callbacks in fenc_params_desc (the Python binding backs them
+ *    with torch tensors); if they are NULL the library uses cudaMalloc / cudaFree.
+ *  - All GPU work is enqueued on the stream given at init (torch's current stream in the binding) and is
+ *    asynchronous; calls that return host-visible data synchronise that stream internally.
+ *  - There is NO CPU fallback: without a CUDA device of compute capability 10.x init fails (FENC_ERR_DEVICE).
+ *  - Device layout of a ciphertext at L limbs: uint64 [2][L][N], limb-major, NTT ("evaluation") domain,
+ *    canonical residues in [0, q_i).  The NTT ordering is private; every export is coefficient domain.
+ */
+#ifndef FENC_H
+#define FENC_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  FENC_OK = 0,
+  FENC_ERR_INVALID_ARG = 1,
+  FENC_ERR_PARAMS = 2,   /* prime not = 1 mod 2N, not enough primes, P < max digit product, ... */
+  FENC_ERR_LAYOUT = 3,   /* S does not divide M, m^2 > N/2, stride does not divide S, ...        */
+  FENC_ERR_NO_KEY = 4,   /* rotation amount / relinearisation key not generated                */
+  FENC_ERR_LEVEL = 5,    /* not enough limbs left for the requested rescale                    */
+  FENC_ERR_MISMATCH = 6, /* operands differ in level / scale / layout                          */
+  FENC_ERR_OOM = 7,
+  FENC_ERR_DEVICE = 8,
+  FENC_ERR_CUDA = 9
+} fenc_status;
+
+typedef struct fenc_ctx fenc_ctx;
+typedef struct fenc_keys fenc_keys;
+typedef struct fenc_pt fenc_pt;
+typedef struct fenc_ct fenc_ct;
+typedef struct fenc_wts fenc_wts;
+
+/* Parameter set (Table I: N, Q = {q_0..q_L}, Delta; BASELINE.json configs; R1).
+ * Ciphertext primes: the n_q largest primes = 1 (mod 2N) below 2^q_bits, descending (q_0 largest);
+ * special primes likewise below 2^p_bits.  dlen = ceil(n_q / dnum) limbs per key-switch digit unless
+ * dlen_override != 0.  init fails with FENC_ERR_PARAMS when P = prod(p_i) < max digit product unless
+ * allow_noisy_ks != 0 (A1: BASELINE config 1's literal dnum=1 is bit-exact-only). */
+typedef struct {
+  uint32_t log2N;            /* 4..16 */
+  uint32_t n_q, q_bits;      /* q_bits <= 60 */
+  uint32_t n_p, p_bits;      /* p_bits <= 60 */
+  uint32_t dnum;
+  uint32_t dlen_override;    /* 0 = derive from dnum */
+  uint32_t allow_noisy_ks;
+  double log2_scale;         /* default scale Delta = 2^log2_scale */
+  const uint64_t *q_override; /* host, n_q entries, or NULL */
+  const uint64_t *p_override; /* host, n_p entries, or NULL */
+  void *(*dev_alloc)(size_t bytes, void *user); /* returns a device pointer (256-byte aligned) or NULL */
+  void (*dev_free)(void *dev_ptr, void *user);
+  void *user;
+  void *cuda_stream;         /* cudaStream_t; NULL = legacy default stream */
+  int device;                /* CUDA device ordinal */
+} fenc_params_desc;
+
+/* Convolution shape, Eq. 2 + Algorithm 1. */
+typedef struct {
+  uint32_t BS, C_in, H, W, C_out, K, stride, pad;
+  int32_t depthwise;
+  uint32_t S; /* fragment (block) size; 0 = Conv-aware selection (R2.10) */
+  uint32_t M; /* square padded frame; 0 = next power of two >= max(H, W) (A4)             */
+} fenc_conv_desc;
+
+/* Filled by fenc_layout_plan.  All counts are exact for the operation graph of DESIGN.md R2.9. */
+typedef struct {
+  uint32_t S, S_out, M, M_out, m, B, ch, cs, G_in, G_out, BG, H_out, W_out;
+  uint32_t n_in_ct, n_out_ct, n_inner_rot, n_outer_rot, n_pmult, n_distinct_pt, n_rot_keys;
+  double S_star_real;                /* (K^2 C_in BS / (alpha C_out))^(1/4): Eq. 8 with BS restored (A5) */
+  double paper_rot_count;            /* #Rot as Table IX prints it (A6, A18)           */
+  int32_t rot_steps[512];            /* the n_rot_keys distinct rotation amounts the layer needs          */
+} fenc_layout;
+
+#define FENC_RELIN_KEY_ID (1ll << 40)
+
+/* ------------------------------------------------------------------ context */
+fenc_status fenc_params_init(const fenc_params_desc *desc, fenc_ctx **out);
+void fenc_ctx_free(fenc_ctx *ctx);
+const char *fenc_last_error(fenc_ctx *ctx);
+/* host q[n_q], p[n_p]; dlen_out / beta_max_out may be NULL */
+fenc_status fenc_get_primes(fenc_ctx *ctx, uint64_t *q, uint64_t *p, uint32_t *dlen_out, uint32_t *beta_max_out);
+fenc_status fenc_sync(fenc_ctx *ctx); /* synchronise the context's stream */
+
+/* ------------------------------------------------------------------ planner (host only) */
+fenc_status fenc_layout_plan(fenc_ctx *ctx, const fenc_conv_desc *conv, fenc_layout *out);
+
+/* ------------------------------------------------------------------ keys (R2.3, R2.4)
+ * Secret: uniform ternary; errors: discrete Gaussian sigma = 3.2; all from the counter-based generator of
+ * DESIGN.md R2.3 keyed by `seed` (evaluated on the device; bit-identical to any host evaluation).
+ * rot_steps: host array of n_rot rotation amounts (reduced mod N/2; 0 ignored).  Evaluation keys stay on
+ * the device in NTT form. */
+fenc_status fenc_keygen(fenc_ctx *ctx, uint64_t seed, const int32_t *rot_steps, size_t n_rot, int want_relin,
+                        fenc_keys **out);
+void fenc_keys_free(fenc_keys *keys);
+/* host s[N]: the secret's coefficients in {-1,0,1} */
+fenc_status fenc_secret_export(fenc_ctx *ctx, const fenc_keys *keys, int64_t *s);
+/* key_id = rotation amount in [1, N/2) or FENC_RELIN_KEY_ID.  host b, a: uint64 [beta_max][n_q+n_p][N],
+ * coefficient domain, canonical residues (the parity view of a switching key, R2.4). */
+fenc_status fenc_evk_export(fenc_ctx *ctx, const fenc_keys *keys, int64_t key_id, uint64_t *b, uint64_t *a);
+
+/* ------------------------------------------------------------------ plaintexts (R2.2, R2.9) */
+/* Algorithm 1: gather fragment ciphertext (u, v, group, batch_group) of host x[BS][C][H][W] (fp64) per
+ * `layout` (input side of the conv the layout was planned for), then encode at `scale` on n_limbs limbs.
+ * scale <= 0 means the context default. */
+fenc_status fenc_encode_fragment(fenc_ctx *ctx, const fenc_conv_desc *conv, const fenc_layout *layout,
+                                 const double *x, uint32_t u, uint32_t v, uint32_t group, uint32_t batch_group,
+                                 uint32_t n_limbs, double scale, fenc_pt **out);
+/* host re[N/2], im[N/2] (im may be NULL): m_t = round((2 s / N) Re(sum_j z_j conj(zeta_j)^t)) (R2.2) */
+fenc_status fenc_encode_slots(fenc_ctx *ctx, const double *re, const double *im, uint32_t n_limbs, double scale,
+                              fenc_pt **out);
+/* host centred integer coefficients [N]: where bit-exact parity starts (A7) */
+fenc_status fenc_pt_from_coeffs(fenc_ctx *ctx, const int64_t *coeffs, uint32_t n_limbs, double scale, fenc_pt **out);
+fenc_status fenc_pt_coeffs(fenc_ctx *ctx, const fenc_pt *pt, int64_t *coeffs /* host [N] */);
+void fenc_pt_free(fenc_pt *pt);
+
+/* ------------------------------------------------------------------ ciphertexts (R2.5) */
+/* Symmetric encryption: c1 = a uniform per limb, c0 = -a s + e + m; randomness from enc_seed (R2.3). */
+fenc_status fenc_encrypt(fenc_ctx *ctx, const fenc_keys *keys, const fenc_pt *pt, uint64_t enc_seed, fenc_ct **out);
+/* host re[N/2], im[N/2] (im may be NULL): decode(c0 + c1 s) at the ciphertext's scale */
+fenc_status fenc_decrypt_slots(fenc_ctx *ctx, const fenc_keys *keys, const fenc_ct *ct, double *re, double *im);
+/* decrypt, decode and scatter (inverse of Algorithm 1, output side of `conv`): writes only this ciphertext's
+ * entries of host y[BS][C_out][H_out][W_out].  which = 0: input-side layout ([BS][C_in][H][W]), 1: output side. */
+fenc_status fenc_decrypt_decode(fenc_ctx *ctx, const fenc_keys *keys, const fenc_ct *ct, const fenc_conv_desc *conv,
+                                const fenc_layout *layout, int which, uint32_t u, uint32_t v, uint32_t group,
+                                uint32_t batch_group, double *y);
+/* host limbs: uint64 [2][L][N], coefficient domain, canonical residues in [0, q_i) */
+fenc_status fenc_ct_export(fenc_ctx *ctx, const fenc_ct *ct, uint64_t *limbs);
+fenc_status fenc_ct_import(fenc_ctx *ctx, const uint64_t *limbs, uint32_t L, double scale, fenc_ct **out);
+fenc_status fenc_ct_info(fenc_ctx *ctx, const fenc_ct *ct, uint32_t *L, double *scale, void **device_ptr);
+void fenc_ct_free(fenc_ct *ct);
+
+/* ------------------------------------------------------------------ primitives (R2.6-R2.8) */
+/* Rot(in[i], steps[i]) for i < n in ONE batched pass (automorphism + hybrid key switch: ModUp, evk inner
+ * product, ModDown; Eq. 1).  All inputs must share the level.  steps: host array. */
+fenc_status fenc_rotate(fenc_ctx *ctx, const fenc_keys *keys, fenc_ct *const *in, const int32_t *steps, size_t n,
+                        fenc_ct **out);
+/* drop the last limb of each input, floor rounding on the canonical representative (A10) */
+fenc_status fenc_rescale(fenc_ctx *ctx, fenc_ct *const *in, size_t n, fenc_ct **out);
+fenc_status fenc_add(fenc_ctx *ctx, const fenc_ct *a, const fenc_ct *b, fenc_ct **out);
+/* out = sum_i in[i] (*) pt[i], one lazy 128-bit accumulation per coefficient (a7); scale multiplies */
+fenc_status fenc_pmult_sum(fenc_ctx *ctx, fenc_ct *const *in, fenc_pt *const *pt, size_t n, fenc_ct **out);
+/* (c0,c1)^2 relinearised and rescaled: x -> x^2 (R2.12) */
+fenc_status fenc_square_relin(fenc_ctx *ctx, const fenc_keys *keys, const fenc_ct *in, fenc_ct **out);
+
+/* ------------------------------------------------------------------ HConv (R2.9) */
+/* Number of distinct non-zero weight plaintexts of the layer and their keys (u_o, v_o, g_out, g_in, d, i, j). */
+fenc_status fenc_wts_keys(fenc_ctx *ctx, const fenc_conv_desc *conv, const fenc_layout *layout, uint32_t *keys7,
+                          size_t capacity, size_t *n);
+/* Encode every non-zero weight plaintext from host w[C_out][C_in or 1][K][K] at `scale` (<= 0: q_{L-1}, A14). */
+fenc_status fenc_conv_weights(fenc_ctx *ctx, const fenc_conv_desc *conv, const fenc_layout *layout, const double *w,
+                              uint32_t n_limbs, double scale, fenc_wts **out);
+/* Same from pre-encoded centred integer coefficients, host coeffs[n][N] in fenc_wts_keys order (A7). */
+fenc_status fenc_conv_weights_from_coeffs(fenc_ctx *ctx, const fenc_conv_desc *conv, const fenc_layout *layout,
+                                          const int64_t *coeffs, size_t n, uint32_t n_limbs, double scale,
+                                          fenc_wts **out);
+void fenc_wts_free(fenc_wts *w);
+/* One fragment-encoded conv layer over ALL batch groups.  in: n_in = S^2 G_in BG ciphertexts ordered
+ * [bg][g][u][v]; out: n_out = S_out^2 G_out BG ciphertexts ordered [bg][g_out][u_o][v_o].  Inner rotations
+ * (batched), MAC, outer rotations (batched), one rescale per output ciphertext when do_rescale != 0 (A13). */
+fenc_status fenc_hconv(fenc_ctx *ctx, const fenc_keys *keys, const fenc_conv_desc *conv, const fenc_layout *layout,
+                       const fenc_wts *wts, fenc_ct *const *in, size_t n_in, int do_rescale, fenc_ct **out,
+                       size_t n_out_capacity, size_t *n_out);
+
+/* ------------------------------------------------------------------ AAC compress (R2.11) */
+/* out[t] = sum over the terms with term_out[i] == t of Rot(mask (*) in[term_src[i]], term_rot[i]).
+ * mask may be NULL (maskless mode, no level consumed); with a mask and do_rescale != 0 this is the paper's
+ * split-scale mode (one late rescale).  term_*: host arrays of n_terms entries. */
+fenc_status fenc_compress(fenc_ctx *ctx, const fenc_keys *keys, fenc_ct *const *in, size_t n_in, const fenc_pt *mask,
+                          const uint32_t *term_out, const uint32_t *term_src, const int32_t *term_rot, size_t n_terms,
+                          int do_rescale, fenc_ct **out, size_t n_out);
+
+/* ------------------------------------------------------------------ measurement helpers */
+/* Raw batched negacyclic NTT / iNTT (a1) in place on device memory: rows uint64 [n_rows][N]; mod_idx: host
+ * array, row r uses modulus mod_idx[r] (0..n_q-1 ciphertext primes, n_q.. special primes). */
+fenc_status fenc_ntt_rows(fenc_ctx *ctx, void *device_rows, const int32_t *mod_idx, size_t n_rows, int inverse);
+/* counters since context creation: kernels launched by this library; optional reset */
+uint64_t fenc_launch_count(fenc_ctx *ctx, int reset);
+/* bytes currently held through the allocator */
+uint64_t fenc_device_bytes(fenc_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FENC_H */

@@ -1,0 +1,412 @@
+"""Thin ctypes binding of libfenc (include/fenc.h): argument marshalling only -- every step of the hot path
+runs in the library's CUDA kernels.  PyTorch supplies device memory (allocator callbacks) and the stream.
+
+There is no CPU fallback: importing works without a GPU (so that the symbol checks can run), but creating a
+Context without a CUDA device raises."""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+RELIN_KEY_ID = 1 << 40
+
+STATUS = {0: "OK", 1: "INVALID_ARG", 2: "PARAMS", 3: "LAYOUT", 4: "NO_KEY", 5: "LEVEL", 6: "MISMATCH", 7: "OOM",
+          8: "DEVICE", 9: "CUDA"}
+
+ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
+FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+
+
+class ParamsDesc(C.Structure):
+    _fields_ = [("log2N", C.c_uint32), ("n_q", C.c_uint32), ("q_bits", C.c_uint32), ("n_p", C.c_uint32),
+                ("p_bits", C.c_uint32), ("dnum", C.c_uint32), ("dlen_override", C.c_uint32),
+                ("allow_noisy_ks", C.c_uint32), ("log2_scale", C.c_double),
+                ("q_override", C.POINTER(C.c_uint64)), ("p_override", C.POINTER(C.c_uint64)),
+                ("dev_alloc", ALLOC_FN), ("dev_free", FREE_FN), ("user", C.c_void_p),
+                ("cuda_stream", C.c_void_p), ("device", C.c_int)]
+
+
+class ConvDesc(C.Structure):
+    _fields_ = [("BS", C.c_uint32), ("C_in", C.c_uint32), ("H", C.c_uint32), ("W", C.c_uint32), ("C_out", C.c_uint32),
+                ("K", C.c_uint32), ("stride", C.c_uint32), ("pad", C.c_uint32), ("depthwise", C.c_int32),
+                ("S", C.c_uint32), ("M", C.c_uint32)]
+
+
+class Layout(C.Structure):
+    _fields_ = [(k, C.c_uint32) for k in ("S", "S_out", "M", "M_out", "m", "B", "ch", "cs", "G_in", "G_out", "BG",
+                                          "H_out", "W_out", "n_in_ct", "n_out_ct", "n_inner_rot", "n_outer_rot",
+                                          "n_pmult", "n_distinct_pt", "n_rot_keys")] + \
+               [("S_star_real", C.c_double), ("paper_rot_count", C.c_double), ("rot_steps", C.c_int32 * 512)]
+
+    def steps(self):
+        return [int(self.rot_steps[i]) for i in range(self.n_rot_keys)]
+
+
+# every symbol include/fenc.h declares (checked by tests/test_abi.py against the header text)
+SYMBOLS = ["fenc_params_init", "fenc_ctx_free", "fenc_last_error", "fenc_get_primes", "fenc_sync", "fenc_layout_plan",
+           "fenc_keygen", "fenc_keys_free", "fenc_secret_export", "fenc_evk_export", "fenc_encode_fragment",
+           "fenc_encode_slots", "fenc_pt_from_coeffs", "fenc_pt_coeffs", "fenc_pt_free", "fenc_encrypt",
+           "fenc_decrypt_slots", "fenc_decrypt_decode", "fenc_ct_export", "fenc_ct_import", "fenc_ct_info",
+           "fenc_ct_free", "fenc_rotate", "fenc_rescale", "fenc_add", "fenc_pmult_sum", "fenc_square_relin",
+           "fenc_wts_keys", "fenc_conv_weights", "fenc_conv_weights_from_coeffs", "fenc_wts_free", "fenc_hconv",
+           "fenc_compress", "fenc_ntt_rows", "fenc_launch_count", "fenc_device_bytes"]
+
+_lib = None
+
+
+def load_library(path=None):
+    """dlopen libfenc.so (building it first if the sources are newer) and set the argument types."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    lib = C.CDLL(path or _build.build())
+    vp, u64p, i64p, dp, i32p, u32p = C.c_void_p, C.POINTER(C.c_uint64), C.POINTER(C.c_int64), C.POINTER(C.c_double), \
+        C.POINTER(C.c_int32), C.POINTER(C.c_uint32)
+    vpp = C.POINTER(C.c_void_p)
+    sig = {
+        "fenc_params_init": [C.POINTER(ParamsDesc), vpp],
+        "fenc_get_primes": [vp, u64p, u64p, u32p, u32p],
+        "fenc_sync": [vp],
+        "fenc_layout_plan": [vp, C.POINTER(ConvDesc), C.POINTER(Layout)],
+        "fenc_keygen": [vp, C.c_uint64, i32p, C.c_size_t, C.c_int, vpp],
+        "fenc_secret_export": [vp, vp, i64p],
+        "fenc_evk_export": [vp, vp, C.c_int64, u64p, u64p],
+        "fenc_encode_fragment": [vp, C.POINTER(ConvDesc), C.POINTER(Layout), dp, C.c_uint32, C.c_uint32, C.c_uint32,
+                                 C.c_uint32, C.c_uint32, C.c_double, vpp],
+        "fenc_encode_slots": [vp, dp, dp, C.c_uint32, C.c_double, vpp],
+        "fenc_pt_from_coeffs": [vp, i64p, C.c_uint32, C.c_double, vpp],
+        "fenc_pt_coeffs": [vp, vp, i64p],
+        "fenc_encrypt": [vp, vp, vp, C.c_uint64, vpp],
+        "fenc_decrypt_slots": [vp, vp, vp, dp, dp],
+        "fenc_decrypt_decode": [vp, vp, vp, C.POINTER(ConvDesc), C.POINTER(Layout), C.c_int, C.c_uint32, C.c_uint32,
+                                C.c_uint32, C.c_uint32, dp],
+        "fenc_ct_export": [vp, vp, u64p],
+        "fenc_ct_import": [vp, u64p, C.c_uint32, C.c_double, vpp],
+        "fenc_ct_info": [vp, vp, u32p, dp, vpp],
+        "fenc_rotate": [vp, vp, vpp, i32p, C.c_size_t, vpp],
+        "fenc_rescale": [vp, vpp, C.c_size_t, vpp],
+        "fenc_add": [vp, vp, vp, vpp],
+        "fenc_pmult_sum": [vp, vpp, vpp, C.c_size_t, vpp],
+        "fenc_square_relin": [vp, vp, vp, vpp],
+        "fenc_wts_keys": [vp, C.POINTER(ConvDesc), C.POINTER(Layout), u32p, C.c_size_t, C.POINTER(C.c_size_t)],
+        "fenc_conv_weights": [vp, C.POINTER(ConvDesc), C.POINTER(Layout), dp, C.c_uint32, C.c_double, vpp],
+        "fenc_conv_weights_from_coeffs": [vp, C.POINTER(ConvDesc), C.POINTER(Layout), i64p, C.c_size_t, C.c_uint32,
+                                          C.c_double, vpp],
+        "fenc_hconv": [vp, vp, C.POINTER(ConvDesc), C.POINTER(Layout), vp, vpp, C.c_size_t, C.c_int, vpp, C.c_size_t,
+                       C.POINTER(C.c_size_t)],
+        "fenc_compress": [vp, vp, vpp, C.c_size_t, vp, u32p, u32p, i32p, C.c_size_t, C.c_int, vpp, C.c_size_t],
+        "fenc_ntt_rows": [vp, vp, i32p, C.c_size_t, C.c_int],
+    }
+    for name, args in sig.items():
+        f = getattr(lib, name)
+        f.argtypes, f.restype = args, C.c_int
+    for name in ("fenc_ctx_free", "fenc_keys_free", "fenc_pt_free", "fenc_ct_free", "fenc_wts_free"):
+        getattr(lib, name).argtypes, getattr(lib, name).restype = [vp], None
+    lib.fenc_last_error.argtypes, lib.fenc_last_error.restype = [vp], C.c_char_p
+    lib.fenc_launch_count.argtypes, lib.fenc_launch_count.restype = [vp, C.c_int], C.c_uint64
+    lib.fenc_device_bytes.argtypes, lib.fenc_device_bytes.restype = [vp], C.c_uint64
+    if path is None:
+        _lib = lib
+    return lib
+
+
+class FencError(RuntimeError):
+    pass
+
+
+def _ptr(a, ty):
+    return a.ctypes.data_as(C.POINTER(ty))
+
+
+class _Handle:
+    _free = None
+
+    def __init__(self, ctx, h):
+        self.ctx, self.h = ctx, h
+
+    def free(self):
+        if self.h:
+            getattr(self.ctx.lib, self._free)(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            if self.ctx.h:
+                self.free()
+        except Exception:
+            pass
+
+
+class Keys(_Handle):
+    _free = "fenc_keys_free"
+
+
+class Plaintext(_Handle):
+    _free = "fenc_pt_free"
+
+
+class Weights(_Handle):
+    _free = "fenc_wts_free"
+
+
+class Ciphertext(_Handle):
+    _free = "fenc_ct_free"
+
+    def info(self):
+        L, s, p = C.c_uint32(), C.c_double(), C.c_void_p()
+        self.ctx._ck(self.ctx.lib.fenc_ct_info(self.ctx.h, self.h, C.byref(L), C.byref(s), C.byref(p)))
+        return L.value, s.value, p.value
+
+    @property
+    def L(self):
+        return self.info()[0]
+
+    @property
+    def scale(self):
+        return self.info()[1]
+
+
+class Context:
+    """fenc_params_init + the calls of include/fenc.h with numpy marshalling."""
+
+    def __init__(self, log2N, n_q, q_bits, n_p, p_bits, dnum=1, log2_scale=40, dlen=0, allow_noisy_ks=False,
+                 q_override=None, p_override=None, device=0):
+        import torch
+        self.lib = load_library()
+        self.h = None
+        if not torch.cuda.is_available():
+            raise FencError("libfenc needs a CUDA device (sm_100a); there is no CPU fallback")
+        self._torch = torch
+        self._blocks = {}
+        dev = torch.device("cuda", device)
+
+        def _alloc(nbytes, _user):
+            try:
+                t = torch.empty(int(nbytes), dtype=torch.uint8, device=dev)
+            except Exception:
+                return None
+            self._blocks[t.data_ptr()] = t
+            return t.data_ptr()
+
+        def _free(p, _user):
+            self._blocks.pop(p, None)
+
+        self._alloc_cb, self._free_cb = ALLOC_FN(_alloc), FREE_FN(_free)
+        d = ParamsDesc()
+        d.log2N, d.n_q, d.q_bits, d.n_p, d.p_bits, d.dnum = log2N, n_q, q_bits, n_p, p_bits, dnum
+        d.dlen_override, d.allow_noisy_ks, d.log2_scale = dlen, int(allow_noisy_ks), float(log2_scale)
+        self._qo = np.asarray(q_override, dtype=np.uint64) if q_override is not None else None
+        self._po = np.asarray(p_override, dtype=np.uint64) if p_override is not None else None
+        d.q_override = _ptr(self._qo, C.c_uint64) if self._qo is not None else None
+        d.p_override = _ptr(self._po, C.c_uint64) if self._po is not None else None
+        d.dev_alloc, d.dev_free, d.user = self._alloc_cb, self._free_cb, None
+        with torch.cuda.device(dev):
+            d.cuda_stream = torch.cuda.current_stream().cuda_stream
+        d.device = device
+        h = C.c_void_p()
+        st = self.lib.fenc_params_init(C.byref(d), C.byref(h))
+        if st != 0:
+            raise FencError("fenc_params_init: " + STATUS.get(st, str(st)))
+        self.h = h
+        self.log2N, self.N, self.n, self.n_q, self.n_p = log2N, 1 << log2N, 1 << (log2N - 1), n_q, n_p
+        q = np.zeros(n_q, dtype=np.uint64)
+        p = np.zeros(n_p, dtype=np.uint64)
+        dl, bm = C.c_uint32(), C.c_uint32()
+        self._ck(self.lib.fenc_get_primes(self.h, _ptr(q, C.c_uint64), _ptr(p, C.c_uint64), C.byref(dl), C.byref(bm)))
+        self.q, self.p, self.dlen, self.beta_max = [int(x) for x in q], [int(x) for x in p], dl.value, bm.value
+
+    def _ck(self, st):
+        if st != 0:
+            raise FencError("%s: %s" % (STATUS.get(st, str(st)), self.lib.fenc_last_error(self.h).decode()))
+
+    def close(self):
+        if self.h:
+            self.lib.fenc_ctx_free(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def sync(self):
+        self._ck(self.lib.fenc_sync(self.h))
+
+    def launch_count(self, reset=False):
+        return int(self.lib.fenc_launch_count(self.h, int(reset)))
+
+    def device_bytes(self):
+        return int(self.lib.fenc_device_bytes(self.h))
+
+    # ---- planner
+    def conv_desc(self, BS, C_in, H, W, C_out, K, stride=1, pad=0, depthwise=False, S=0, M=0):
+        return ConvDesc(BS, C_in, H, W, C_out, K, stride, pad, int(depthwise), S, M)
+
+    def layout_plan(self, conv):
+        lay = Layout()
+        self._ck(self.lib.fenc_layout_plan(self.h, C.byref(conv), C.byref(lay)))
+        return lay
+
+    # ---- keys
+    def keygen(self, seed, rot_steps=(), want_relin=False):
+        steps = np.asarray(list(rot_steps), dtype=np.int32)
+        h = C.c_void_p()
+        self._ck(self.lib.fenc_keygen(self.h, C.c_uint64(seed), _ptr(steps, C.c_int32), len(steps), int(want_relin), C.byref(h)))
+        return Keys(self, h)
+
+    def secret_export(self, keys):
+        s = np.zeros(self.N, dtype=np.int64)
+        self._ck(self.lib.fenc_secret_export(self.h, keys.h, _ptr(s, C.c_int64)))
+        return s
+
+    def evk_export(self, keys, key_id):
+        A = self.n_q + self.n_p
+        b = np.zeros((self.beta_max, A, self.N), dtype=np.uint64)
+        a = np.zeros_like(b)
+        self._ck(self.lib.fenc_evk_export(self.h, keys.h, C.c_int64(key_id), _ptr(b, C.c_uint64), _ptr(a, C.c_uint64)))
+        return b, a
+
+    # ---- plaintexts
+    def encode_fragment(self, conv, lay, x, u, v, g, bg, n_limbs, scale=0.0):
+        x = np.ascontiguousarray(x, dtype=np.float64)
+        assert x.shape == (conv.BS, conv.C_in, conv.H, conv.W)
+        h = C.c_void_p()
+        self._ck(self.lib.fenc_encode_fragment(self.h, C.byref(conv), C.byref(lay), _ptr(x, C.c_double), u, v, g, bg, n_limbs,
+                                               float(scale), C.byref(h)))
+        return Plaintext(self, h)
+
+    def encode_slots(self, z, n_limbs, scale=0.0):
+        z = np.asarray(z)
+        re = np.ascontiguousarray(z.real, dtype=np.float64)
+        im = np.ascontiguousarray(z.imag, dtype=np.float64) if np.iscomplexobj(z) else None
+        assert re.shape == (self.n,)
+        h = C.c_void_p()
+        self._ck(self.lib.fenc_encode_slots(self.h, _ptr(re, C.c_double), _ptr(im, C.c_double) if im is not None else None,
+                                            n_limbs, float(scale), C.byref(h)))
+        return Plaintext(self, h)
+
+    def pt_from_coeffs(self, coeffs, n_limbs, scale=0.0):
+        c = np.ascontiguousarray(coeffs, dtype=np.int64)
+        assert c.shape == (self.N,)
+        h = C.c_void_p()
+        self._ck(self.lib.fenc_pt_from_coeffs(self.h, _ptr(c, C.c_int64), n_limbs, float(scale), C.byref(h)))
+        return Plaintext(self, h)
+
+    def pt_coeffs(self, pt):
+        c = np.zeros(self.N, dtype=np.int64)
+        self._ck(self.lib.fenc_pt_coeffs(self.h, pt.h, _ptr(c, C.c_int64)))
+        return c
+
+    # ---- ciphertexts
+    def encrypt(self, keys, pt, enc_seed):
+        h = C.c_void_p()
+        self._ck(self.lib.fenc_encrypt(self.h, keys.h, pt.h, C.c_uint64(enc_seed), C.byref(h)))
+        return Ciphertext(self, h)
+
+    def decrypt_slots(self, keys, ct):
+        re = np.zeros(self.n, dtype=np.float64)
+        im = np.zeros(self.n, dtype=np.float64)
+        self._ck(self.lib.fenc_decrypt_slots(self.h, keys.h, ct.h, _ptr(re, C.c_double), _ptr(im, C.c_double)))
+        return re + 1j * im
+
+    def decrypt_decode(self, keys, ct, conv, lay, which, u, v, g, bg, y):
+        assert y.dtype == np.float64 and y.flags["C_CONTIGUOUS"]
+        self._ck(self.lib.fenc_decrypt_decode(self.h, keys.h, ct.h, C.byref(conv), C.byref(lay), which, u, v, g, bg,
+                                              _ptr(y, C.c_double)))
+
+    def ct_export(self, ct):
+        L = ct.L
+        out = np.zeros((2, L, self.N), dtype=np.uint64)
+        self._ck(self.lib.fenc_ct_export(self.h, ct.h, _ptr(out, C.c_uint64)))
+        return out
+
+    def ct_import(self, limbs, scale=0.0):
+        a = np.ascontiguousarray(limbs, dtype=np.uint64)
+        assert a.ndim == 3 and a.shape[0] == 2 and a.shape[2] == self.N
+        h = C.c_void_p()
+        self._ck(self.lib.fenc_ct_import(self.h, _ptr(a, C.c_uint64), a.shape[1], float(scale), C.byref(h)))
+        return Ciphertext(self, h)
+
+    def _harr(self, handles):
+        return (C.c_void_p * len(handles))(*[x.h.value for x in handles])
+
+    # ---- primitives
+    def rotate(self, keys, cts, steps):
+        n = len(cts)
+        st = np.asarray(list(steps), dtype=np.int32)
+        assert st.shape == (n,)
+        out = (C.c_void_p * n)()
+        self._ck(self.lib.fenc_rotate(self.h, keys.h, self._harr(cts), _ptr(st, C.c_int32), n, out))
+        return [Ciphertext(self, C.c_void_p(out[i])) for i in range(n)]
+
+    def rescale(self, cts):
+        n = len(cts)
+        out = (C.c_void_p * n)()
+        self._ck(self.lib.fenc_rescale(self.h, self._harr(cts), n, out))
+        return [Ciphertext(self, C.c_void_p(out[i])) for i in range(n)]
+
+    def add(self, a, b):
+        h = C.c_void_p()
+        self._ck(self.lib.fenc_add(self.h, a.h, b.h, C.byref(h)))
+        return Ciphertext(self, h)
+
+    def pmult_sum(self, cts, pts):
+        h = C.c_void_p()
+        self._ck(self.lib.fenc_pmult_sum(self.h, self._harr(cts), self._harr(pts), len(cts), C.byref(h)))
+        return Ciphertext(self, h)
+
+    def square_relin(self, keys, ct):
+        h = C.c_void_p()
+        self._ck(self.lib.fenc_square_relin(self.h, keys.h, ct.h, C.byref(h)))
+        return Ciphertext(self, h)
+
+    # ---- HConv
+    def wts_keys(self, conv, lay):
+        n = C.c_size_t()
+        self._ck(self.lib.fenc_wts_keys(self.h, C.byref(conv), C.byref(lay), None, 0, C.byref(n)))
+        k = np.zeros((n.value, 7), dtype=np.uint32)
+        self._ck(self.lib.fenc_wts_keys(self.h, C.byref(conv), C.byref(lay), _ptr(k, C.c_uint32), n.value, C.byref(n)))
+        return k
+
+    def conv_weights(self, conv, lay, w, n_limbs, scale=0.0):
+        w = np.ascontiguousarray(w, dtype=np.float64)
+        h = C.c_void_p()
+        self._ck(self.lib.fenc_conv_weights(self.h, C.byref(conv), C.byref(lay), _ptr(w, C.c_double), n_limbs, float(scale), C.byref(h)))
+        return Weights(self, h)
+
+    def conv_weights_from_coeffs(self, conv, lay, coeffs, n_limbs, scale=0.0):
+        c = np.ascontiguousarray(coeffs, dtype=np.int64)
+        assert c.ndim == 2 and c.shape[1] == self.N
+        h = C.c_void_p()
+        self._ck(self.lib.fenc_conv_weights_from_coeffs(self.h, C.byref(conv), C.byref(lay), _ptr(c, C.c_int64), c.shape[0],
+                                                        n_limbs, float(scale), C.byref(h)))
+        return Weights(self, h)
+
+    def hconv(self, keys, conv, lay, wts, cts, do_rescale=True):
+        cap = int(lay.n_out_ct)
+        out = (C.c_void_p * cap)()
+        n = C.c_size_t()
+        self._ck(self.lib.fenc_hconv(self.h, keys.h, C.byref(conv), C.byref(lay), wts.h, self._harr(cts), len(cts),
+                                     int(do_rescale), out, cap, C.byref(n)))
+        return [Ciphertext(self, C.c_void_p(out[i])) for i in range(n.value)]
+
+    def compress(self, keys, cts, terms, n_out, mask=None, do_rescale=False):
+        """terms: list of (out index, source index, rotation amount)."""
+        to = np.asarray([t[0] for t in terms], dtype=np.uint32)
+        ts = np.asarray([t[1] for t in terms], dtype=np.uint32)
+        tr = np.asarray([t[2] for t in terms], dtype=np.int32)
+        out = (C.c_void_p * n_out)()
+        self._ck(self.lib.fenc_compress(self.h, keys.h, self._harr(cts), len(cts), mask.h if mask is not None else None,
+                                        _ptr(to, C.c_uint32), _ptr(ts, C.c_uint32), _ptr(tr, C.c_int32), len(terms),
+                                        int(do_rescale), out, n_out))
+        return [Ciphertext(self, C.c_void_p(out[i])) for i in range(n_out)]
+
+    # ---- raw NTT on a torch tensor of uint64 rows (viewed as int64 by torch)
+    def ntt_rows(self, tensor, mod_idx, inverse=False):
+        m = np.asarray(list(mod_idx), dtype=np.int32)
+        assert tensor.is_cuda and tensor.is_contiguous() and tensor.numel() == len(m) * self.N
+        self._ck(self.lib.fenc_ntt_rows(self.h, C.c_void_p(tensor.data_ptr()), _ptr(m, C.c_int32), len(m), int(inverse)))

@@ -1,0 +1,537 @@
+// fenc_conv.cu -- fragment layout (Algorithm 1), Conv-aware planner, the HConv
+// operation graph and its batched execution (R2.9), and AAC compress.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <set>
+
+#include "fenc_ctx.h"
+
+static u32 next_pow2(u32 x) {
+  u32 p = 1;
+  while (p < x) p <<= 1;
+  return p;
+}
+
+struct Term {
+  int src;  // input ciphertext within a batch group: (g_in * S + u') * S + v'
+  int amt;  // inner rotation amount (0 = the input itself)
+  int w;    // weight plaintext index (fenc_wts_keys order)
+};
+struct OutCt {
+  std::vector<int> diags;                // existing channel diagonals d, ascending
+  std::vector<std::vector<Term>> terms;  // per existing diagonal
+};
+struct ConvGraph {
+  fenc_conv_desc d;
+  int n, M, S, S_out, m, B, ch, cs, G_in, G_out, BG, H_out, W_out;
+  std::vector<OutCt> outs;                    // index (g_out * S_out + u_o) * S_out + v_o
+  std::vector<std::pair<int, int>> inner;     // distinct (src, amt != 0), sorted
+  std::map<std::pair<int, int>, int> inner_index;
+  std::vector<std::array<u32, 7>> wkeys;      // (u_o, v_o, g_out, g_in, d, i, j) per weight plaintext
+  std::vector<int> rot_steps;                 // distinct rotation amounts (inner and outer), ascending
+  size_t n_outer = 0, n_pmult = 0;
+  // R2.9 step 2: the validity conditions factorise into channel positions, block rows and block columns
+  std::vector<std::array<int, 3>> valid_cpos(int go, int gi, int dd) const {
+    std::vector<std::array<int, 3>> v;
+    for (int cpos = 0; cpos < ch; cpos++) {
+      int c = gi * ch + cpos, o = go * ch + (((cpos - dd) % ch + ch) % ch);
+      if (c < (int)d.C_in && o < (int)d.C_out && (!d.depthwise || o == c)) v.push_back({cpos, o, c});
+    }
+    return v;
+  }
+  std::vector<int> valid_blocks(int frag_o, int tap, int size_in, int size_out) const {
+    std::vector<int> v;
+    for (int bi = 0; bi < m; bi++) {
+      int ho = bi * S_out + frag_o, hi = (int)d.stride * ho + tap - (int)d.pad;
+      if (ho < size_out && hi >= 0 && hi < size_in) v.push_back(bi);
+    }
+    return v;
+  }
+  // slot vector of weight plaintext wk for kernel tensor w[C_out][C_in or 1][K][K]
+  void weight_slots(const std::array<u32, 7> &wk, const double *w, std::vector<double> &vec) const {
+    vec.assign(n, 0.0);
+    const int uo = wk[0], vo = wk[1], go = wk[2], gi = wk[3], dd = wk[4], i = wk[5], j = wk[6];
+    const int K = d.K, Cw = d.depthwise ? 1 : (int)d.C_in;
+    auto cp = valid_cpos(go, gi, dd);
+    auto rows = valid_blocks(uo, i, d.H, H_out), cols = valid_blocks(vo, j, d.W, W_out);
+    for (auto &t : cp) {
+      const double val = w[(((size_t)t[1] * Cw + (d.depthwise ? 0 : t[2])) * K + i) * K + j];
+      for (int bi : rows)
+        for (int bj : cols) {
+          size_t base = (size_t)t[0] * cs + (size_t)(bi * m + bj) * B;
+          for (int b = 0; b < B; b++) vec[base + b] = val;
+        }
+    }
+  }
+};
+
+static fenc_status build_graph(fenc_ctx *ctx, const fenc_conv_desc *cd, int S, std::shared_ptr<ConvGraph> &out) {
+  char keybuf[256];
+  snprintf(keybuf, sizeof keybuf, "%u,%u,%u,%u,%u,%u,%u,%u,%d,%d,%u", cd->BS, cd->C_in, cd->H, cd->W, cd->C_out, cd->K,
+           cd->stride, cd->pad, cd->depthwise, S, cd->M);
+  auto it = ctx->graphs.find(keybuf);
+  if (it != ctx->graphs.end()) {
+    out = it->second;
+    return FENC_OK;
+  }
+  if (cd->BS < 1 || cd->C_in < 1 || cd->C_out < 1 || cd->K < 1 || cd->stride < 1 || cd->H + 2 * cd->pad < cd->K || cd->W + 2 * cd->pad < cd->K)
+    return fail(ctx, FENC_ERR_INVALID_ARG, "bad convolution shape");
+  if (cd->depthwise && cd->C_in != cd->C_out) return fail(ctx, FENC_ERR_INVALID_ARG, "depthwise needs C_in == C_out");
+  auto g = std::make_shared<ConvGraph>();
+  g->d = *cd;
+  g->n = ctx->n;
+  g->M = cd->M ? cd->M : next_pow2(std::max(cd->H, cd->W));
+  g->S = S;
+  if (S < 1 || g->M % S || S % (int)cd->stride || (u32)g->M < std::max(cd->H, cd->W))
+    return fail(ctx, FENC_ERR_LAYOUT, "S=%d must divide M=%d and be a multiple of the stride", S, g->M);
+  g->m = g->M / S;
+  const long m2 = (long)g->m * g->m;
+  if (m2 > g->n || g->n % m2) return fail(ctx, FENC_ERR_LAYOUT, "m^2=%ld does not fit %d slots", m2, g->n);
+  g->B = (int)std::min<long>(next_pow2(cd->BS), g->n / m2);
+  g->ch = (int)(g->n / (g->B * m2));
+  g->cs = (int)(g->B * m2);
+  g->G_in = (cd->C_in + g->ch - 1) / g->ch;
+  g->G_out = (cd->C_out + g->ch - 1) / g->ch;
+  g->BG = (cd->BS + g->B - 1) / g->B;
+  g->S_out = S / cd->stride;
+  g->H_out = (cd->H + 2 * cd->pad - cd->K) / cd->stride + 1;
+  g->W_out = (cd->W + 2 * cd->pad - cd->K) / cd->stride + 1;
+  const int K = cd->K, So = g->S_out, ch = g->ch;
+  std::set<std::pair<int, int>> inner;
+  std::set<int> steps;
+  g->outs.resize((size_t)g->G_out * So * So);
+  for (int uo = 0; uo < So; uo++)
+    for (int vo = 0; vo < So; vo++)
+      for (int go = 0; go < g->G_out; go++) {
+        OutCt &oc = g->outs[((size_t)go * So + uo) * So + vo];
+        for (int dd = 0; dd < ch; dd++) {
+          std::vector<Term> lst;
+          for (int gi = 0; gi < g->G_in; gi++) {
+            if (g->valid_cpos(go, gi, dd).empty()) continue;
+            for (int i = 0; i < K; i++) {
+              if (g->valid_blocks(uo, i, cd->H, g->H_out).empty()) continue;
+              for (int j = 0; j < K; j++) {
+                if (g->valid_blocks(vo, j, cd->W, g->W_out).empty()) continue;
+                const int ti = (int)cd->stride * uo + i - (int)cd->pad, tj = (int)cd->stride * vo + j - (int)cd->pad;
+                const int up = ((ti % S) + S) % S, di = (ti - up) / S;  // floor division
+                const int vp = ((tj % S) + S) % S, dj = (tj - vp) / S;
+                const long a = ((long)(di * g->m + dj) * g->B) % g->n;
+                const int amt = (int)((a + g->n) % g->n);
+                const int src = (gi * S + up) * S + vp;
+                lst.push_back(Term{src, amt, (int)g->wkeys.size()});
+                g->wkeys.push_back({(u32)uo, (u32)vo, (u32)go, (u32)gi, (u32)dd, (u32)i, (u32)j});
+                if (amt) inner.insert({src, amt}), steps.insert(amt);
+              }
+            }
+          }
+          if (!lst.empty()) {
+            oc.diags.push_back(dd);
+            oc.terms.push_back(std::move(lst));
+            g->n_pmult += oc.terms.back().size();
+            if (dd) g->n_outer++, steps.insert((int)(((long)dd * g->cs) % g->n));
+          }
+        }
+      }
+  g->inner.assign(inner.begin(), inner.end());
+  for (size_t i = 0; i < g->inner.size(); i++) g->inner_index[g->inner[i]] = (int)i;
+  g->rot_steps.assign(steps.begin(), steps.end());
+  ctx->graphs[keybuf] = g;
+  out = g;
+  return FENC_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ planner (R2.10)
+static double paper_rot_count(const fenc_conv_desc *cd, int n, int M, int S) {
+  // Table IX: n_in I(S,K) + n_out (ch - 1), I = ceil(K/S)^2 - 1 for K > S else 0 (A6, A18)
+  const double alpha = (double)n / ((double)M * M);
+  const double n_in = cd->C_in * cd->BS / alpha, n_out = cd->C_out * cd->BS / alpha, ch = alpha * S * S / cd->BS;
+  const int c = (cd->K + S - 1) / S;
+  const double inner = (S >= M || (int)cd->K <= S) ? 0.0 : (double)(c * c - 1);
+  return n_in * inner + n_out * (ch - 1.0);
+}
+
+extern "C" fenc_status fenc_layout_plan(fenc_ctx *ctx, const fenc_conv_desc *cd, fenc_layout *out) {
+  if (!ctx || !cd || !out) return FENC_ERR_INVALID_ARG;
+  const int M = cd->M ? cd->M : next_pow2(std::max(cd->H, cd->W));
+  const double alpha = (double)ctx->n / ((double)M * M);
+  int S = cd->S;
+  std::shared_ptr<ConvGraph> g;
+  if (S == 0) {
+    // Conv-aware selection: feasible powers of two under Eq. 7, arg-min of the exact rotation count
+    std::vector<int> feas, ok;
+    for (int s = 1; s <= M; s <<= 1)
+      if (M % s == 0 && s % (int)cd->stride == 0 && (long)(M / s) * (M / s) <= ctx->n) feas.push_back(s);
+    if (feas.empty()) return fail(ctx, FENC_ERR_LAYOUT, "no feasible block size");
+    const double bound = std::sqrt(cd->BS * cd->C_in / alpha);
+    for (int s : feas)
+      if (s <= bound) ok.push_back(s);
+    if (ok.empty()) ok.push_back(feas[0]);
+    size_t best = ~(size_t)0;
+    for (int s : ok) {
+      std::shared_ptr<ConvGraph> gs;
+      fenc_status st = build_graph(ctx, cd, s, gs);
+      if (st != FENC_OK) return st;
+      size_t tot = (gs->inner.size() + gs->n_outer) * gs->BG;
+      if (tot < best) best = tot, S = s, g = gs;
+    }
+  } else {
+    fenc_status st = build_graph(ctx, cd, S, g);
+    if (st != FENC_OK) return st;
+  }
+  memset(out, 0, sizeof *out);
+  out->S = g->S, out->S_out = g->S_out, out->M = g->M, out->M_out = g->M / cd->stride, out->m = g->m, out->B = g->B;
+  out->ch = g->ch, out->cs = g->cs, out->G_in = g->G_in, out->G_out = g->G_out, out->BG = g->BG;
+  out->H_out = g->H_out, out->W_out = g->W_out;
+  out->n_in_ct = g->S * g->S * g->G_in * g->BG;
+  out->n_out_ct = g->S_out * g->S_out * g->G_out * g->BG;
+  out->n_inner_rot = (u32)(g->inner.size() * g->BG);
+  out->n_outer_rot = (u32)(g->n_outer * g->BG);
+  out->n_pmult = (u32)(g->n_pmult * g->BG);
+  out->n_distinct_pt = (u32)g->wkeys.size();
+  out->n_rot_keys = (u32)g->rot_steps.size();
+  if (g->rot_steps.size() > 512) return fail(ctx, FENC_ERR_LAYOUT, "more than 512 rotation amounts");
+  for (size_t i = 0; i < g->rot_steps.size(); i++) out->rot_steps[i] = g->rot_steps[i];
+  out->S_star_real = std::pow((double)cd->K * cd->K * cd->C_in * cd->BS / (alpha * cd->C_out), 0.25);
+  out->paper_rot_count = paper_rot_count(cd, ctx->n, M, g->S);
+  return FENC_OK;
+}
+
+static fenc_status graph_for(fenc_ctx *ctx, const fenc_conv_desc *cd, const fenc_layout *lay, std::shared_ptr<ConvGraph> &g) {
+  if (!lay || lay->S == 0) return fail(ctx, FENC_ERR_INVALID_ARG, "layout not planned");
+  return build_graph(ctx, cd, (int)lay->S, g);
+}
+
+// ------------------------------------------------------------------------------------------------ Algorithm 1
+// ciphertext (u, v, g, bg) holds at slot cpos*cs + (bi*m+bj)*B + b the value X[bg*B+b][g*ch+cpos][bi*S+u][bj*S+v]
+extern "C" fenc_status fenc_encode_fragment(fenc_ctx *ctx, const fenc_conv_desc *cd, const fenc_layout *lay, const double *x,
+                                            uint32_t u, uint32_t v, uint32_t group, uint32_t bgi, uint32_t n_limbs, double scale,
+                                            fenc_pt **out) {
+  if (!ctx || !cd || !lay || !x || !out) return FENC_ERR_INVALID_ARG;
+  if (u >= lay->S || v >= lay->S || group >= lay->G_in || bgi >= lay->BG) return fail(ctx, FENC_ERR_LAYOUT, "fragment index out of range");
+  std::vector<double> vec(ctx->n, 0.0);
+  const int m = lay->m, B = lay->B, S = lay->S;
+  for (u32 cpos = 0; cpos < lay->ch; cpos++) {
+    u32 c = group * lay->ch + cpos;
+    if (c >= cd->C_in) continue;
+    for (int b = 0; b < B; b++) {
+      u32 bb = bgi * B + b;
+      if (bb >= cd->BS) continue;
+      for (int bi = 0; bi < m; bi++) {
+        u32 h = bi * S + u;
+        if (h >= cd->H) continue;
+        for (int bj = 0; bj < m; bj++) {
+          u32 w = bj * S + v;
+          if (w < cd->W) vec[(size_t)cpos * lay->cs + (size_t)(bi * m + bj) * B + b] = x[(((size_t)bb * cd->C_in + c) * cd->H + h) * cd->W + w];
+        }
+      }
+    }
+  }
+  return fenc_encode_slots(ctx, vec.data(), nullptr, n_limbs, scale, out);
+}
+
+extern "C" fenc_status fenc_decrypt_decode(fenc_ctx *ctx, const fenc_keys *K, const fenc_ct *ct, const fenc_conv_desc *cd,
+                                           const fenc_layout *lay, int which, uint32_t u, uint32_t v, uint32_t group, uint32_t bgi,
+                                           double *y) {
+  if (!ctx || !K || !ct || !cd || !lay || !y) return FENC_ERR_INVALID_ARG;
+  const u32 S = which ? lay->S_out : lay->S, C = which ? cd->C_out : cd->C_in, H = which ? lay->H_out : cd->H,
+            W = which ? lay->W_out : cd->W, G = which ? lay->G_out : lay->G_in;
+  if (u >= S || v >= S || group >= G || bgi >= lay->BG) return fail(ctx, FENC_ERR_LAYOUT, "fragment index out of range");
+  std::vector<double> vec(ctx->n);
+  fenc_status st = fenc_decrypt_slots(ctx, K, ct, vec.data(), nullptr);
+  if (st != FENC_OK) return st;
+  const int m = lay->m, B = lay->B;
+  for (u32 cpos = 0; cpos < lay->ch; cpos++) {
+    u32 c = group * lay->ch + cpos;
+    if (c >= C) continue;
+    for (int b = 0; b < B; b++) {
+      u32 bb = bgi * B + b;
+      if (bb >= cd->BS) continue;
+      for (int bi = 0; bi < m; bi++) {
+        u32 h = bi * S + u;
+        if (h >= H) continue;
+        for (int bj = 0; bj < m; bj++) {
+          u32 w = bj * S + v;
+          if (w < W) y[(((size_t)bb * C + c) * H + h) * W + w] = vec[(size_t)cpos * lay->cs + (size_t)(bi * m + bj) * B + b];
+        }
+      }
+    }
+  }
+  return FENC_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ weights
+extern "C" fenc_status fenc_wts_keys(fenc_ctx *ctx, const fenc_conv_desc *cd, const fenc_layout *lay, uint32_t *keys7,
+                                     size_t capacity, size_t *n) {
+  if (!ctx || !cd || !n) return FENC_ERR_INVALID_ARG;
+  std::shared_ptr<ConvGraph> g;
+  fenc_status st = graph_for(ctx, cd, lay, g);
+  if (st != FENC_OK) return st;
+  *n = g->wkeys.size();
+  if (keys7) {
+    if (capacity < g->wkeys.size()) return fail(ctx, FENC_ERR_INVALID_ARG, "capacity %zu < %zu weight plaintexts", capacity, g->wkeys.size());
+    for (size_t i = 0; i < g->wkeys.size(); i++) memcpy(keys7 + 7 * i, g->wkeys[i].data(), 7 * sizeof(u32));
+  }
+  return FENC_OK;
+}
+
+static fenc_status make_wts(fenc_ctx *ctx, const ConvGraph &g, const double *w, const int64_t *coeffs, uint32_t n_limbs,
+                            double scale, fenc_wts **out) {
+  if (n_limbs < 1 || (int)n_limbs > ctx->nq) return FENC_ERR_INVALID_ARG;
+  const int L = n_limbs;
+  const size_t N = ctx->N, n = g.wkeys.size();
+  fenc_wts *W = new fenc_wts{ctx, L, scale > 0 ? scale : (double)ctx->mod[L - 1], n, nullptr, ""};  // A14: s_w = q_{L-1}
+  W->d_all = dalloc_t<u64>(ctx, n * L * N);
+  if (!W->d_all) {
+    delete W;
+    return fail(ctx, FENC_ERR_OOM, "weight plaintexts (%zu x %d limbs)", n, L);
+  }
+  std::vector<double> vec;
+  std::vector<int64_t> c(N);
+  for (size_t i = 0; i < n; i++) {
+    const int64_t *src = coeffs ? coeffs + i * N : c.data();
+    if (!coeffs) {
+      g.weight_slots(g.wkeys[i], w, vec);
+      fh::encode_slots(ctx->logN, vec.data(), nullptr, W->scale, c.data());
+    }
+    fenc_status st = coeffs_to_mont(ctx, src, L, W->d_all + i * L * N);
+    if (st != FENC_OK) return st;
+    if (!coeffs && cudaStreamSynchronize(ctx->stream) != cudaSuccess) return FENC_ERR_CUDA;  // c is reused
+  }
+  if (cudaStreamSynchronize(ctx->stream) != cudaSuccess) return FENC_ERR_CUDA;
+  *out = W;
+  return FENC_OK;
+}
+extern "C" fenc_status fenc_conv_weights(fenc_ctx *ctx, const fenc_conv_desc *cd, const fenc_layout *lay, const double *w,
+                                         uint32_t n_limbs, double scale, fenc_wts **out) {
+  if (!ctx || !cd || !w || !out) return FENC_ERR_INVALID_ARG;
+  std::shared_ptr<ConvGraph> g;
+  fenc_status st = graph_for(ctx, cd, lay, g);
+  return st != FENC_OK ? st : make_wts(ctx, *g, w, nullptr, n_limbs, scale, out);
+}
+extern "C" fenc_status fenc_conv_weights_from_coeffs(fenc_ctx *ctx, const fenc_conv_desc *cd, const fenc_layout *lay,
+                                                     const int64_t *coeffs, size_t n, uint32_t n_limbs, double scale,
+                                                     fenc_wts **out) {
+  if (!ctx || !cd || !coeffs || !out) return FENC_ERR_INVALID_ARG;
+  std::shared_ptr<ConvGraph> g;
+  fenc_status st = graph_for(ctx, cd, lay, g);
+  if (st != FENC_OK) return st;
+  if (n != g->wkeys.size()) return fail(ctx, FENC_ERR_MISMATCH, "expected %zu weight plaintexts, got %zu", g->wkeys.size(), n);
+  return make_wts(ctx, *g, nullptr, coeffs, n_limbs, scale, out);
+}
+extern "C" void fenc_wts_free(fenc_wts *W) {
+  if (!W) return;
+  cudaStreamSynchronize(W->ctx->stream);
+  dfree(W->ctx, W->d_all);
+  delete W;
+}
+
+// ------------------------------------------------------------------------------------------------ HConv (R2.9)
+// 1. inner rotations: every distinct (input ciphertext, amount) once, always from the original input, ONE batch
+// 2. MAC: P_d = sum over (g_in, taps) of R (*) W per existing channel diagonal d, one launch for all (bg, output, d)
+// 3. outer rotations: Rot(P_d, d cs) for d != 0, ONE batch;  4. Y = P_0 + sum of those;  5. one rescale per output (A13)
+extern "C" fenc_status fenc_hconv(fenc_ctx *ctx, const fenc_keys *K, const fenc_conv_desc *cd, const fenc_layout *lay,
+                                  const fenc_wts *W, fenc_ct *const *in, size_t n_in, int do_rescale, fenc_ct **out,
+                                  size_t cap, size_t *n_out) {
+  if (!ctx || !K || !cd || !lay || !W || !in || !out || !n_out) return FENC_ERR_INVALID_ARG;
+  std::shared_ptr<ConvGraph> gp;
+  fenc_status st = graph_for(ctx, cd, lay, gp);
+  if (st != FENC_OK) return st;
+  const ConvGraph &g = *gp;
+  const size_t nin_bg = (size_t)g.S * g.S * g.G_in, nout_bg = g.outs.size(), BG = g.BG;
+  if (n_in != nin_bg * BG) return fail(ctx, FENC_ERR_MISMATCH, "expected %zu input ciphertexts, got %zu", nin_bg * BG, n_in);
+  if (cap < nout_bg * BG) return fail(ctx, FENC_ERR_INVALID_ARG, "output capacity %zu < %zu", cap, nout_bg * BG);
+  if (W->n != g.wkeys.size()) return fail(ctx, FENC_ERR_MISMATCH, "weights belong to another layer");
+  const int L = in[0]->L;
+  const double s_in = in[0]->scale;
+  for (size_t i = 0; i < n_in; i++)
+    if (in[i]->L != L || std::fabs(in[i]->scale - s_in) > 1e-9 * s_in) return fail(ctx, FENC_ERR_MISMATCH, "inputs differ in level or scale");
+  if (W->L != L) return fail(ctx, FENC_ERR_MISMATCH, "weights at %d limbs, inputs at %d", W->L, L);
+  if (do_rescale && L < 2) return fail(ctx, FENC_ERR_LEVEL, "no level left to rescale");
+  for (auto &oc : g.outs)
+    if (oc.diags.empty()) return fail(ctx, FENC_ERR_LAYOUT, "an output ciphertext receives no term");
+  const size_t N = ctx->N, CT = (size_t)2 * L * N;
+  const size_t n_inner = g.inner.size();
+  // ---- 1. inner rotations
+  u64 *Rbuf = n_inner ? dalloc_t<u64>(ctx, n_inner * BG * CT) : nullptr;
+  if (n_inner && !Rbuf) return fail(ctx, FENC_ERR_OOM, "inner-rotation results (%zu ciphertexts)", n_inner * BG);
+  {
+    std::vector<const u64 *> vin;
+    std::vector<u64 *> vout;
+    std::vector<int> vs;
+    for (size_t bg = 0; bg < BG; bg++)
+      for (size_t r = 0; r < n_inner; r++) {
+        vin.push_back(in[bg * nin_bg + g.inner[r].first]->d);
+        vs.push_back(g.inner[r].second);
+        vout.push_back(Rbuf + (bg * n_inner + r) * CT);
+      }
+    st = rotate_raw(ctx, K, L, vin, vs, vout);
+    if (st != FENC_OK) return st;
+  }
+  // ---- 2. MAC over every (bg, output, diagonal)
+  size_t n_P = 0, n_rot_out = 0;
+  for (auto &oc : g.outs) {
+    n_P += oc.diags.size();
+    for (int d : oc.diags) n_rot_out += d != 0;
+  }
+  std::vector<fenc_ct *> res(nout_bg * BG, nullptr);
+  const double s_acc = s_in * W->scale;
+  u64 *Ybuf = do_rescale ? dalloc_t<u64>(ctx, nout_bg * BG * CT) : nullptr;  // pre-rescale sums
+  u64 *Pbuf = dalloc_t<u64>(ctx, n_P * BG * CT);                               // diagonal partial sums (worst case)
+  u64 *Obuf = n_rot_out ? dalloc_t<u64>(ctx, n_rot_out * BG * CT) : nullptr;   // outer-rotation results
+  if ((do_rescale && !Ybuf) || !Pbuf || (n_rot_out && !Obuf)) return fail(ctx, FENC_ERR_OOM, "hconv partial sums");
+  for (size_t i = 0; i < res.size(); i++) {
+    res[i] = new_ct(ctx, do_rescale ? L - 1 : L, do_rescale ? s_acc / (double)ctx->mod[L - 1] : s_acc);
+    if (!res[i]) return fail(ctx, FENC_ERR_OOM, "hconv outputs");
+  }
+  std::vector<const u64 *> term_ct, term_pt;
+  std::vector<int> start{0};
+  std::vector<u64 *> mac_out;
+  std::vector<const u64 *> rot_in, sum_terms;
+  std::vector<u64 *> rot_out, sum_out;
+  std::vector<int> rot_step, sum_start{0};
+  size_t pi = 0, oi = 0;
+  for (size_t bg = 0; bg < BG; bg++)
+    for (size_t o = 0; o < nout_bg; o++) {
+      const OutCt &oc = g.outs[o];
+      u64 *Y = do_rescale ? Ybuf + (bg * nout_bg + o) * CT : res[bg * nout_bg + o]->d;
+      const bool single = oc.diags.size() == 1 && oc.diags[0] == 0;
+      for (size_t k = 0; k < oc.diags.size(); k++) {
+        u64 *P = single ? Y : Pbuf + (pi++) * CT;
+        for (const Term &t : oc.terms[k]) {
+          term_ct.push_back(t.amt ? Rbuf + (bg * n_inner + g.inner_index.at({t.src, t.amt})) * CT : in[bg * nin_bg + t.src]->d);
+          term_pt.push_back(W->d_all + (size_t)t.w * L * N);
+        }
+        start.push_back((int)term_ct.size());
+        mac_out.push_back(P);
+        if (single) continue;
+        if (oc.diags[k] == 0) sum_terms.push_back(P);
+        else {
+          u64 *R = Obuf + (oi++) * CT;
+          rot_in.push_back(P), rot_out.push_back(R), rot_step.push_back((int)(((long)oc.diags[k] * g.cs) % g.n));
+          sum_terms.push_back(R);
+        }
+      }
+      if (!single) sum_start.push_back((int)sum_terms.size()), sum_out.push_back(Y);
+    }
+  {
+    DescStage ds(ctx);
+    size_t o0 = ds.add(term_ct), o1 = ds.add(term_pt), o2 = ds.add(start), o3 = ds.add(mac_out);
+    char *base = ds.commit();
+    if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
+    CUDA_OK(ctx, k_mac(ctx->k, (const u64 *const *)(base + o0), (const u64 *const *)(base + o1), (const int *)(base + o2),
+                       (u64 *const *)(base + o3), (int)mac_out.size(), L, ctx->max_lazy));
+  }
+  // ---- 3. outer rotations, 4. sums
+  st = rotate_raw(ctx, K, L, rot_in, rot_step, rot_out);
+  if (st != FENC_OK) return st;
+  if (!sum_out.empty()) {
+    DescStage ds(ctx);
+    size_t o0 = ds.add(sum_terms), o1 = ds.add(sum_start), o2 = ds.add(sum_out);
+    char *base = ds.commit();
+    if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
+    CUDA_OK(ctx, k_add_many(ctx->k, (const u64 *const *)(base + o0), (const int *)(base + o1), (u64 *const *)(base + o2), (int)sum_out.size(), L));
+  }
+  // ---- 5. rescale
+  if (do_rescale) {
+    std::vector<BatchItem> items(res.size());
+    for (size_t i = 0; i < res.size(); i++) {
+      items[i] = BatchItem{};
+      items[i].sub_in = Ybuf + i * CT, items[i].out = res[i]->d;
+    }
+    st = rescale_batch(ctx, L, items);
+    if (st != FENC_OK) return st;
+  }
+  dfree(ctx, Rbuf), dfree(ctx, Ybuf), dfree(ctx, Pbuf), dfree(ctx, Obuf);
+  for (size_t i = 0; i < res.size(); i++) out[i] = res[i];
+  *n_out = res.size();
+  return FENC_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ AAC compress (R2.11)
+extern "C" fenc_status fenc_compress(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const *in, size_t n_in, const fenc_pt *mask_c,
+                                     const uint32_t *term_out, const uint32_t *term_src, const int32_t *term_rot, size_t n_terms,
+                                     int do_rescale, fenc_ct **out, size_t n_out) {
+  if (!ctx || !K || !in || !term_out || !term_src || !term_rot || !out || n_in == 0 || n_out == 0) return FENC_ERR_INVALID_ARG;
+  fenc_pt *mask = const_cast<fenc_pt *>(mask_c);
+  const int L = in[0]->L;
+  const double s_in = in[0]->scale;
+  for (size_t i = 0; i < n_in; i++)
+    if (in[i]->L != L || std::fabs(in[i]->scale - s_in) > 1e-9 * s_in) return fail(ctx, FENC_ERR_MISMATCH, "sources differ in level or scale");
+  if (mask && mask->L != L) return fail(ctx, FENC_ERR_MISMATCH, "mask level");
+  if (do_rescale && L < 2) return fail(ctx, FENC_ERR_LEVEL, "no level left to rescale");
+  const size_t N = ctx->N, CT = (size_t)2 * L * N;
+  std::vector<int> cnt(n_out, 0);
+  for (size_t i = 0; i < n_terms; i++) {
+    if (term_out[i] >= n_out || term_src[i] >= n_in) return fail(ctx, FENC_ERR_INVALID_ARG, "compress term out of range");
+    cnt[term_out[i]]++;
+  }
+  for (size_t t = 0; t < n_out; t++)
+    if (!cnt[t]) return fail(ctx, FENC_ERR_INVALID_ARG, "compress output %zu has no term", t);
+  double s_mid = s_in;
+  u64 *Mbuf = nullptr;
+  if (mask) {  // masked sources: one PMult each (split-scale mode)
+
+    fenc_status st = pt_device(ctx, mask);
+    if (st != FENC_OK) return st;
+    s_mid = s_in * mask->scale;
+    Mbuf = dalloc_t<u64>(ctx, n_in * CT);
+    if (!Mbuf) return fail(ctx, FENC_ERR_OOM, "compress masked sources");
+    std::vector<const u64 *> tc(n_in), tp(n_in, mask->d_mont);
+    std::vector<int> start(n_in + 1);
+    std::vector<u64 *> outs(n_in);
+    for (size_t i = 0; i < n_in; i++) tc[i] = in[i]->d, start[i] = (int)i, outs[i] = Mbuf + i * CT;
+    start[n_in] = (int)n_in;
+    DescStage ds(ctx);
+    size_t o0 = ds.add(tc), o1 = ds.add(tp), o2 = ds.add(start), o3 = ds.add(outs);
+    char *base = ds.commit();
+    if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
+    CUDA_OK(ctx, k_mac(ctx->k, (const u64 *const *)(base + o0), (const u64 *const *)(base + o1), (const int *)(base + o2),
+                       (u64 *const *)(base + o3), (int)n_in, L, ctx->max_lazy));
+  }
+  u64 *Rbuf = dalloc_t<u64>(ctx, n_terms * CT);
+  u64 *Ybuf = do_rescale ? dalloc_t<u64>(ctx, n_out * CT) : nullptr;
+  if (!Rbuf || (do_rescale && !Ybuf)) return fail(ctx, FENC_ERR_OOM, "compress workspace");
+  std::vector<fenc_ct *> res(n_out);
+  for (size_t t = 0; t < n_out; t++) {
+    res[t] = new_ct(ctx, do_rescale ? L - 1 : L, do_rescale ? s_mid / (double)ctx->mod[L - 1] : s_mid);
+    if (!res[t]) return fail(ctx, FENC_ERR_OOM, "compress outputs");
+  }
+  std::vector<const u64 *> vin(n_terms);
+  std::vector<u64 *> vout(n_terms);
+  std::vector<int> vs(n_terms);
+  for (size_t i = 0; i < n_terms; i++) {
+    vin[i] = mask ? Mbuf + term_src[i] * CT : in[term_src[i]]->d;
+    vout[i] = Rbuf + i * CT, vs[i] = term_rot[i];
+  }
+  fenc_status st = rotate_raw(ctx, K, L, vin, vs, vout);
+  if (st != FENC_OK) return st;
+  std::vector<const u64 *> sum_terms;
+  std::vector<int> sum_start{0};
+  std::vector<u64 *> sum_out;
+  for (size_t t = 0; t < n_out; t++) {
+    for (size_t i = 0; i < n_terms; i++)
+      if (term_out[i] == t) sum_terms.push_back(vout[i]);
+    sum_start.push_back((int)sum_terms.size());
+    sum_out.push_back(do_rescale ? Ybuf + t * CT : res[t]->d);
+  }
+  {
+    DescStage ds(ctx);
+    size_t o0 = ds.add(sum_terms), o1 = ds.add(sum_start), o2 = ds.add(sum_out);
+    char *base = ds.commit();
+    if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
+    CUDA_OK(ctx, k_add_many(ctx->k, (const u64 *const *)(base + o0), (const int *)(base + o1), (u64 *const *)(base + o2), (int)n_out, L));
+  }
+  if (do_rescale) {
+    std::vector<BatchItem> items(n_out);
+    for (size_t t = 0; t < n_out; t++) {
+      items[t] = BatchItem{};
+      items[t].sub_in = Ybuf + t * CT, items[t].out = res[t]->d;
+    }
+    st = rescale_batch(ctx, L, items);
+    if (st != FENC_OK) return st;
+  }
+  dfree(ctx, Mbuf), dfree(ctx, Rbuf), dfree(ctx, Ybuf);
+  for (size_t t = 0; t < n_out; t++) out[t] = res[t];
+  return FENC_OK;
+}

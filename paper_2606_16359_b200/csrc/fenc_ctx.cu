@@ -1,0 +1,410 @@
+// fenc_ctx.cu -- context, per-level key-switch tables, workspace, and the batched key-switch / rescale drivers.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+
+#include "fenc_ctx.h"
+
+fenc_status fail(fenc_ctx *ctx, fenc_status st, const char *fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  if (ctx) ctx->err = buf;
+  return st;
+}
+
+void *dalloc(fenc_ctx *ctx, size_t bytes) {
+  if (bytes == 0) bytes = 256;
+  void *p = nullptr;
+  if (ctx->dev_alloc) p = ctx->dev_alloc(bytes, ctx->user);
+  else if (cudaMalloc(&p, bytes) != cudaSuccess) p = nullptr;
+  if (p) {
+    ctx->live[p] = bytes;
+    ctx->dev_bytes += bytes;
+  } else {
+    (void)cudaGetLastError();
+  }
+  return p;
+}
+void dfree(fenc_ctx *ctx, void *p) {
+  if (!p) return;
+  auto it = ctx->live.find(p);
+  if (it != ctx->live.end()) {
+    ctx->dev_bytes -= it->second;
+    ctx->live.erase(it);
+  }
+  if (ctx->dev_free) ctx->dev_free(p, ctx->user);
+  else cudaFree(p);
+}
+void *workspace(fenc_ctx *ctx, size_t bytes) {
+  if (bytes > ctx->ws_bytes) {
+    dfree(ctx, ctx->ws);
+    ctx->ws_bytes = 0;
+    ctx->ws = dalloc(ctx, bytes);
+    if (ctx->ws) ctx->ws_bytes = bytes;
+  }
+  return ctx->ws;
+}
+char *DescStage::commit() {
+  size_t need = (host.size() + 255) & ~(size_t)255;
+  if (need > ctx->desc_bytes) {
+    dfree(ctx, ctx->desc_buf);
+    size_t cap = need < (1u << 20) ? (1u << 20) : need * 2;
+    ctx->desc_buf = dalloc(ctx, cap);
+    ctx->desc_bytes = ctx->desc_buf ? cap : 0;
+    if (!ctx->desc_buf) return nullptr;
+  }
+  if (!host.empty() &&
+      cudaMemcpyAsync(ctx->desc_buf, host.data(), host.size(), cudaMemcpyHostToDevice, ctx->stream) != cudaSuccess)
+    return nullptr;
+  return (char *)ctx->desc_buf;
+}
+fenc_ct *new_ct(fenc_ctx *ctx, int L, double scale) {
+  u64 *d = dalloc_t<u64>(ctx, (size_t)2 * L * ctx->N);
+  if (!d) return nullptr;
+  return new fenc_ct{ctx, L, scale, d};
+}
+u32 galois_elt(const fenc_ctx *ctx, int step) {
+  int r = ((step % ctx->n) + ctx->n) % ctx->n;
+  return (u32)fh::powmod(5, (u64)r, 2ull * ctx->N);
+}
+
+// ------------------------------------------------------------------------------------------------ context
+extern "C" fenc_status fenc_params_init(const fenc_params_desc *d, fenc_ctx **out) {
+  if (!d || !out) return FENC_ERR_INVALID_ARG;
+  std::unique_ptr<fenc_ctx> c(new fenc_ctx());
+  fenc_ctx *ctx = c.get();
+  if (d->log2N < 4 || d->log2N > 16 || d->n_q < 1 || d->n_p < 1 || d->n_q + d->n_p > FENC_MAX_MOD || d->q_bits > 60 ||
+      d->p_bits > 60 || (d->dnum < 1 && !d->dlen_override))
+    return FENC_ERR_PARAMS;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || d->device < 0 || d->device >= ndev) {
+    (void)cudaGetLastError();
+    return FENC_ERR_DEVICE;  // no CPU fallback
+  }
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, d->device) != cudaSuccess || prop.major != 10) return FENC_ERR_DEVICE;
+  if (cudaSetDevice(d->device) != cudaSuccess) return FENC_ERR_DEVICE;
+  ctx->device = d->device;
+  ctx->stream = (cudaStream_t)d->cuda_stream;
+  ctx->dev_alloc = d->dev_alloc, ctx->dev_free = d->dev_free, ctx->user = d->user;
+  ctx->logN = d->log2N, ctx->N = 1 << d->log2N, ctx->n = ctx->N / 2;
+  ctx->nq = d->n_q, ctx->np = d->n_p, ctx->A = ctx->nq + ctx->np;
+  std::vector<u64> q, p;
+  if (d->q_override) q.assign(d->q_override, d->q_override + d->n_q);
+  else if (!fh::find_primes(ctx->logN, d->q_bits, d->n_q, q)) return FENC_ERR_PARAMS;
+  if (d->p_override) p.assign(d->p_override, d->p_override + d->n_p);
+  else if (!fh::find_primes(ctx->logN, d->p_bits, d->n_p, p)) return FENC_ERR_PARAMS;
+  ctx->mod = q;
+  ctx->mod.insert(ctx->mod.end(), p.begin(), p.end());
+  for (size_t i = 0; i < ctx->mod.size(); i++) {
+    u64 m = ctx->mod[i];
+    if (m >= (1ull << 61) || m % (2ull * ctx->N) != 1 || !fh::is_prime(m)) return FENC_ERR_PARAMS;
+    for (size_t k = 0; k < i; k++)
+      if (ctx->mod[k] == m) return FENC_ERR_PARAMS;
+  }
+  ctx->dlen = d->dlen_override ? (int)d->dlen_override : (ctx->nq + (int)d->dnum - 1) / (int)d->dnum;
+  if (ctx->dlen < 1 || ctx->dlen > ctx->nq) return FENC_ERR_PARAMS;
+  ctx->beta_max = (ctx->nq + ctx->dlen - 1) / ctx->dlen;
+  // key-switch noise condition P >= max_j Q_j (A1)
+  long double logP = 0, logQj = 0;
+  for (u64 m : p) logP += log2l((long double)m);
+  for (int i = 0; i < ctx->dlen; i++) logQj += log2l((long double)q[i]);
+  if (logP < logQj && !d->allow_noisy_ks) return FENC_ERR_PARAMS;
+  // lazy 128-bit accumulation bounds (fenc_device.cuh): sums must stay below t 2^64
+  u64 qmax = 0, pmax = 0;
+  for (u64 m : q) qmax = m > qmax ? m : qmax;
+  for (u64 m : p) pmax = m > pmax ? m : pmax;
+  u64 allmax = qmax > pmax ? qmax : pmax;
+  if ((u64)ctx->dlen > ~0ull / qmax || (u64)ctx->np > ~0ull / pmax || (u64)ctx->beta_max > ~0ull / allmax) return FENC_ERR_PARAMS;
+  u64 ml = ~0ull / qmax;
+  ctx->max_lazy = ml > (1u << 20) ? (1 << 20) : (int)ml;
+  ctx->default_scale = std::ldexp(1.0, (int)d->log2_scale);
+  // device tables
+  const int A = ctx->A, N = ctx->N;
+  std::vector<ModConst> mods(A);
+  std::vector<ShoupC> fwd((size_t)A * N), inv((size_t)A * N), ninv(A);
+  std::vector<RowDesc> ident(A);
+  std::vector<int> imod(2 * A);
+  ctx->psi.resize(A);
+  for (int i = 0; i < A; i++) {
+    u64 m = ctx->mod[i];
+    ctx->psi[i] = fh::find_psi(m, N);
+    int bits = 64 - __builtin_clzll(m - 1);
+    mods[i] = ModConst{m, fh::neg_qinv(m), fh::to_mont(fh::to_mont(1, m), m), (bits >= 64 ? ~0ull : (1ull << bits) - 1)};
+    fh::build_twiddles(m, ctx->psi[i], ctx->logN, &fwd[(size_t)i * N], &inv[(size_t)i * N]);
+    u64 ni = fh::invmod((u64)N % m, m);
+    ninv[i] = ShoupC{ni, fh::shoup(ni, m)};
+    ident[i] = RowDesc{i, i, i, 0, 0, {0, 0, 0}};
+    imod[i] = imod[A + i] = i;
+  }
+  ctx->d_mods = dalloc_t<ModConst>(ctx, A);
+  ctx->d_tw_fwd = dalloc_t<ShoupC>(ctx, (size_t)A * N);
+  ctx->d_tw_inv = dalloc_t<ShoupC>(ctx, (size_t)A * N);
+  ctx->d_ident_rows = dalloc_t<RowDesc>(ctx, A);
+  ctx->d_ninv = dalloc_t<ShoupC>(ctx, A);
+  ctx->d_ident_mod = dalloc_t<int>(ctx, 2 * A);
+  if (!ctx->d_mods || !ctx->d_tw_fwd || !ctx->d_tw_inv || !ctx->d_ident_rows || !ctx->d_ninv || !ctx->d_ident_mod) return FENC_ERR_OOM;
+  cudaMemcpy(ctx->d_mods, mods.data(), A * sizeof(ModConst), cudaMemcpyHostToDevice);
+  cudaMemcpy(ctx->d_tw_fwd, fwd.data(), fwd.size() * sizeof(ShoupC), cudaMemcpyHostToDevice);
+  cudaMemcpy(ctx->d_tw_inv, inv.data(), inv.size() * sizeof(ShoupC), cudaMemcpyHostToDevice);
+  cudaMemcpy(ctx->d_ident_rows, ident.data(), A * sizeof(RowDesc), cudaMemcpyHostToDevice);
+  cudaMemcpy(ctx->d_ninv, ninv.data(), A * sizeof(ShoupC), cudaMemcpyHostToDevice);
+  if (cudaMemcpy(ctx->d_ident_mod, imod.data(), 2 * A * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess) return FENC_ERR_CUDA;
+  // 2-pass NTT geometry
+  NttGeom g{};
+  g.logN = ctx->logN;
+  if (ctx->logN <= 11) {
+    g.brow = ctx->logN, g.bcol = 0, g.lt_row = ctx->logN, g.lt_col = ctx->logN, g.lc_col = ctx->logN;
+  } else {
+    g.brow = 8, g.bcol = ctx->logN - 8, g.lt_row = 11, g.lc_col = 4, g.lt_col = g.bcol + 4;
+  }
+  ctx->k = KCtx{(void *)ctx->stream, g, ctx->d_mods, ctx->d_tw_fwd, ctx->d_tw_inv, &ctx->launches, N, ctx->nq, ctx->np};
+  *out = c.release();
+  return FENC_OK;
+}
+
+extern "C" void fenc_ctx_free(fenc_ctx *ctx) {
+  if (!ctx) return;
+  cudaStreamSynchronize(ctx->stream);
+  for (auto &kv : ctx->plans)
+    for (void *p : kv.second->owned) dfree(ctx, p);
+  dfree(ctx, ctx->ws), dfree(ctx, ctx->desc_buf);
+  dfree(ctx, ctx->d_mods), dfree(ctx, ctx->d_tw_fwd), dfree(ctx, ctx->d_tw_inv);
+  dfree(ctx, ctx->d_ident_rows), dfree(ctx, ctx->d_ninv), dfree(ctx, ctx->d_ident_mod);
+  delete ctx;
+}
+extern "C" const char *fenc_last_error(fenc_ctx *ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+extern "C" fenc_status fenc_get_primes(fenc_ctx *ctx, uint64_t *q, uint64_t *p, uint32_t *dlen, uint32_t *beta_max) {
+  if (!ctx) return FENC_ERR_INVALID_ARG;
+  if (q) memcpy(q, ctx->mod.data(), ctx->nq * sizeof(u64));
+  if (p) memcpy(p, ctx->mod.data() + ctx->nq, ctx->np * sizeof(u64));
+  if (dlen) *dlen = ctx->dlen;
+  if (beta_max) *beta_max = ctx->beta_max;
+  return FENC_OK;
+}
+extern "C" fenc_status fenc_sync(fenc_ctx *ctx) {
+  if (!ctx) return FENC_ERR_INVALID_ARG;
+  CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+  return FENC_OK;
+}
+extern "C" uint64_t fenc_launch_count(fenc_ctx *ctx, int reset) {
+  if (!ctx) return 0;
+  u64 v = ctx->launches;
+  if (reset) ctx->launches = 0;
+  return v;
+}
+extern "C" uint64_t fenc_device_bytes(fenc_ctx *ctx) { return ctx ? ctx->dev_bytes : 0; }
+
+// ------------------------------------------------------------------------------------------------ per-level tables
+// DESIGN.md R2.6: digit j = limbs [j dlen, min((j+1) dlen, L)), Q_j its product;
+//   ModUp:   y_i = d[q_i] [(Q_j/q_i)^-1]_{q_i},   up_j[t] = sum_i y_i ((Q_j/q_i) mod t)          (no correction)
+//   ModDown: y_i = acc[p_i] [(P/p_i)^-1]_{p_i},   out[t] = (acc[t] - sum_i y_i ((P/p_i) mod t)) [P^-1]_t
+// DESIGN.md R2.8: rescale c'[t] = (c[t] - (c[q_{L-1}] mod t)) [q_{L-1}^-1]_t.
+LevelPlan *get_plan(fenc_ctx *ctx, int L) {
+  auto it = ctx->plans.find(L);
+  if (it != ctx->plans.end()) return it->second.get();
+  std::unique_ptr<LevelPlan> pl(new LevelPlan());
+  LevelPlan &P = *pl;
+  const int np = ctx->np, nq = ctx->nq, dlen = ctx->dlen, A = ctx->A;
+  const std::vector<u64> &mod = ctx->mod;
+  P.L = L, P.E = L + np, P.beta = (L + dlen - 1) / dlen;
+  const int E = P.E;
+  auto emod = [&](int row) { return row < L ? row : nq + (row - L); };
+  auto shoupc = [&](u64 c, u64 m) { return ShoupC{c, fh::shoup(c, m)}; };
+  std::vector<RowDesc> rows_in(L), rows_up, rows_p(2 * np), rows_down(2 * L), rows_div(2 * L), rows_ct(2 * L);
+  std::vector<ShoupC> scale_in(L), scale_p(2 * np), mul_pinv(A, ShoupC{0, 0}), scale_ct(2 * L);
+  std::vector<u64> bc_up, bc_down((size_t)L * np);
+  std::vector<int> tmp_index((size_t)P.beta * E, -1);
+  for (int j = 0; j < P.beta; j++) {
+    const int lo = j * dlen, hi = std::min(lo + dlen, L);
+    for (int i = lo; i < hi; i++) {
+      u64 qi = mod[i], qhat = 1;
+      for (int i2 = lo; i2 < hi; i2++)
+        if (i2 != i) qhat = fh::mulmod(qhat, mod[i2] % qi, qi);
+      u64 ninv = fh::invmod((u64)ctx->N % qi, qi);
+      rows_in[i] = RowDesc{i, i, i, 0, 0, {0, 0, 0}};
+      scale_in[i] = shoupc(fh::mulmod(ninv, fh::invmod(qhat, qi), qi), qi);
+    }
+    for (int t = 0; t < E; t++) {
+      if (t >= lo && t < hi) continue;
+      const u64 T = mod[emod(t)];
+      RowDesc rd{emod(t), lo, (int)rows_up.size(), hi - lo, (int)bc_up.size(), {0, 0, 0}};
+      for (int i = lo; i < hi; i++) {
+        u64 c = 1;
+        for (int i2 = lo; i2 < hi; i2++)
+          if (i2 != i) c = fh::mulmod(c, mod[i2] % T, T);
+        bc_up.push_back(fh::to_mont(c, T));
+      }
+      tmp_index[(size_t)j * E + t] = rd.dst_row;
+      rows_up.push_back(rd);
+    }
+  }
+  P.n_up = (int)rows_up.size();
+  for (int c = 0; c < 2; c++)
+    for (int i = 0; i < np; i++) {
+      u64 pi = mod[nq + i], phat = 1;
+      for (int i2 = 0; i2 < np; i2++)
+        if (i2 != i) phat = fh::mulmod(phat, mod[nq + i2] % pi, pi);
+      u64 ninv = fh::invmod((u64)ctx->N % pi, pi);
+      rows_p[c * np + i] = RowDesc{nq + i, c * E + L + i, c * np + i, 0, 0, {0, 0, 0}};
+      scale_p[c * np + i] = shoupc(fh::mulmod(ninv, fh::invmod(phat, pi), pi), pi);
+    }
+  for (int t = 0; t < L; t++) {
+    const u64 T = mod[t];
+    u64 Pm = 1;
+    for (int i = 0; i < np; i++) {
+      Pm = fh::mulmod(Pm, mod[nq + i] % T, T);
+      u64 c = 1;
+      for (int i2 = 0; i2 < np; i2++)
+        if (i2 != i) c = fh::mulmod(c, mod[nq + i2] % T, T);
+      bc_down[(size_t)t * np + i] = fh::to_mont(c, T);
+    }
+    mul_pinv[t] = shoupc(fh::invmod(Pm, T), T);
+    u64 ninv = fh::invmod((u64)ctx->N % T, T);
+    for (int c = 0; c < 2; c++) {
+      rows_down[c * L + t] = RowDesc{t, c * np, c * L + t, np, t * np, {0, 0, 0}};
+      rows_div[c * L + t] = RowDesc{t, c * L + t, c * L + t, c, c * E + t, {0, 0, 0}};
+      rows_ct[c * L + t] = RowDesc{t, c * L + t, c * L + t, 0, 0, {0, 0, 0}};
+      scale_ct[c * L + t] = shoupc(ninv, T);
+    }
+  }
+  P.d_rows_in = upload_owned(ctx, P.owned, rows_in);
+  P.d_scale_in = upload_owned(ctx, P.owned, scale_in);
+  P.d_rows_up = upload_owned(ctx, P.owned, rows_up);
+  P.d_bc_up = upload_owned(ctx, P.owned, bc_up);
+  P.d_tmp_index = upload_owned(ctx, P.owned, tmp_index);
+  P.d_rows_p = upload_owned(ctx, P.owned, rows_p);
+  P.d_scale_p = upload_owned(ctx, P.owned, scale_p);
+  P.d_rows_down = upload_owned(ctx, P.owned, rows_down);
+  P.d_bc_down = upload_owned(ctx, P.owned, bc_down);
+  P.d_rows_div = upload_owned(ctx, P.owned, rows_div);
+  P.d_mul_pinv = upload_owned(ctx, P.owned, mul_pinv);
+  P.d_rows_ct = upload_owned(ctx, P.owned, rows_ct);
+  P.d_scale_ct = upload_owned(ctx, P.owned, scale_ct);
+  // rescale tables
+  const int L1 = L - 1;
+  std::vector<RowDesc> rs_in(2), rs_up, rs_div;
+  std::vector<ShoupC> rs_scale(2), mul_ql(A, ShoupC{0, 0});
+  std::vector<u64> bc_rs;
+  if (L >= 2) {
+    const u64 ql = mod[L1];
+    u64 ninv = fh::invmod((u64)ctx->N % ql, ql);
+    for (int c = 0; c < 2; c++) {
+      rs_in[c] = RowDesc{L1, c * L + L1, c, 0, 0, {0, 0, 0}};
+      rs_scale[c] = shoupc(ninv, ql);
+    }
+    for (int t = 0; t < L1; t++) {
+      bc_rs.push_back(fh::to_mont(1, mod[t]));
+      mul_ql[t] = shoupc(fh::invmod(ql % mod[t], mod[t]), mod[t]);
+    }
+    for (int c = 0; c < 2; c++)
+      for (int t = 0; t < L1; t++) {
+        rs_up.push_back(RowDesc{t, c, c * L1 + t, 1, t, {0, 0, 0}});
+        rs_div.push_back(RowDesc{t, c * L1 + t, c * L1 + t, c, c * L + t, {0, 0, 0}});
+      }
+  }
+  P.d_rows_rs_in = upload_owned(ctx, P.owned, rs_in);
+  P.d_scale_rs = upload_owned(ctx, P.owned, rs_scale);
+  P.d_rows_rs_up = upload_owned(ctx, P.owned, rs_up);
+  P.d_bc_rs = upload_owned(ctx, P.owned, bc_rs);
+  P.d_rows_rs_div = upload_owned(ctx, P.owned, rs_div);
+  P.d_mul_qlinv = upload_owned(ctx, P.owned, mul_ql);
+  cudaStreamSynchronize(ctx->stream);  // host vectors go out of scope
+  for (void *p : P.owned)
+    if (!p) return nullptr;
+  LevelPlan *ret = pl.get();
+  ctx->plans[L] = std::move(pl);
+  return ret;
+}
+
+// ------------------------------------------------------------------------------------------------ batched key switch
+static const size_t WS_CAP = (size_t)6 << 30;  // workspace budget for one chunk of a batch
+
+fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items) {
+  if (items.empty()) return FENC_OK;
+  LevelPlan *P = get_plan(ctx, L);
+  if (!P) return fail(ctx, FENC_ERR_OOM, "level plan");
+  const size_t N = ctx->N;
+  const int E = P->E, np = ctx->np;
+  const size_t per = ((size_t)L + P->n_up + 2 * E + 2 * np + 2 * L) * N;  // u64 per item
+  size_t chunk = WS_CAP / (per * 8);
+  if (chunk < 1) chunk = 1;
+  if (chunk > items.size()) chunk = items.size();
+  u64 *ws = (u64 *)workspace(ctx, chunk * per * 8);
+  if (!ws) return fail(ctx, FENC_ERR_OOM, "key-switch workspace (%zu bytes)", chunk * per * 8);
+  u64 *y = ws, *tmp = y + chunk * L * N, *acc = tmp + chunk * P->n_up * N, *yP = acc + chunk * 2 * E * N,
+      *tmp2 = yP + chunk * 2 * np * N;
+  const KCtx &k = ctx->k;
+  for (size_t at = 0; at < items.size(); at += chunk) {
+    const int nb = (int)std::min(chunk, items.size() - at);
+    DescStage st(ctx);
+    std::vector<BatchItem> part(items.begin() + at, items.begin() + at + nb);
+    st.add(part);
+    const BatchItem *d_items = (const BatchItem *)st.commit();
+    if (!d_items) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
+    // a2 + a1: iNTT of sigma_g(d), pre-scaled for ModUp
+    CUDA_OK(ctx, k_intt(k, d_items, nullptr, 0, true, y, (size_t)L * N, P->d_rows_in, L, P->d_scale_in, nb));
+    // a3 + a1 (pass 1): ModUp fused into the first NTT pass
+    CUDA_OK(ctx, k_ntt_cols_bconv(k, y, (size_t)L * N, P->d_bc_up, tmp, (size_t)P->n_up * N, P->d_rows_up, P->n_up, nb));
+    // a1 (pass 2) + a4: evk inner product
+    CUDA_OK(ctx, k_ntt_rows_keymac(k, d_items, L, E, P->beta, P->d_tmp_index, tmp, (size_t)P->n_up * N, acc, (size_t)2 * E * N, nb));
+    // a5: ModDown = iNTT of the special limbs, conversion fused into pass 1, divide epilogue fused into pass 2
+    CUDA_OK(ctx, k_intt(k, nullptr, acc, (size_t)2 * E * N, false, yP, (size_t)2 * np * N, P->d_rows_p, 2 * np, P->d_scale_p, nb));
+    CUDA_OK(ctx, k_ntt_cols_bconv(k, yP, (size_t)2 * np * N, P->d_bc_down, tmp2, (size_t)2 * L * N, P->d_rows_down, 2 * L, nb));
+    CUDA_OK(ctx, k_ntt_rows_divide(k, d_items, tmp2, (size_t)2 * L * N, acc, (size_t)2 * E * N, false, P->d_mul_pinv, P->d_rows_div, 2 * L, nb));
+  }
+  return FENC_OK;
+}
+
+fenc_status rescale_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items) {
+  if (items.empty()) return FENC_OK;
+  if (L < 2) return fail(ctx, FENC_ERR_LEVEL, "rescale needs at least 2 limbs");
+  LevelPlan *P = get_plan(ctx, L);
+  if (!P) return fail(ctx, FENC_ERR_OOM, "level plan");
+  const size_t N = ctx->N;
+  const int L1 = L - 1;
+  const size_t per = ((size_t)2 + 2 * L1) * N;
+  size_t chunk = std::min(items.size(), std::max<size_t>(1, WS_CAP / (per * 8)));
+  u64 *ws = (u64 *)workspace(ctx, chunk * per * 8);
+  if (!ws) return fail(ctx, FENC_ERR_OOM, "rescale workspace");
+  u64 *yR = ws, *tmp2 = yR + chunk * 2 * N;
+  const KCtx &k = ctx->k;
+  for (size_t at = 0; at < items.size(); at += chunk) {
+    const int nb = (int)std::min(chunk, items.size() - at);
+    DescStage st(ctx);
+    std::vector<BatchItem> part(items.begin() + at, items.begin() + at + nb);
+    for (auto &it : part) it.ks_in = it.sub_in, it.add0 = it.add1 = nullptr, it.g = 1;
+    st.add(part);
+    const BatchItem *d_items = (const BatchItem *)st.commit();
+    if (!d_items) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
+    CUDA_OK(ctx, k_intt(k, d_items, nullptr, 0, false, yR, 2 * N, P->d_rows_rs_in, 2, P->d_scale_rs, nb));
+    CUDA_OK(ctx, k_ntt_cols_bconv(k, yR, 2 * N, P->d_bc_rs, tmp2, (size_t)2 * L1 * N, P->d_rows_rs_up, 2 * L1, nb));
+    CUDA_OK(ctx, k_ntt_rows_divide(k, d_items, tmp2, (size_t)2 * L1 * N, nullptr, 0, true, P->d_mul_qlinv, P->d_rows_rs_div, 2 * L1, nb));
+  }
+  return FENC_OK;
+}
+
+// Rot(in[i], steps[i]) -> out[i]; all at level L (Eq. 1; R2.7: automorphism first)
+fenc_status rotate_raw(fenc_ctx *ctx, const fenc_keys *keys, int L, const std::vector<const u64 *> &in,
+                       const std::vector<int> &steps, const std::vector<u64 *> &out) {
+  std::vector<BatchItem> items;
+  const size_t LN = (size_t)L * ctx->N;
+  for (size_t i = 0; i < in.size(); i++) {
+    int r = ((steps[i] % ctx->n) + ctx->n) % ctx->n;
+    if (r == 0) {
+      CUDA_OK(ctx, cudaMemcpyAsync(out[i], in[i], 2 * LN * 8, cudaMemcpyDeviceToDevice, ctx->stream));
+      continue;
+    }
+    auto it = keys->evk.find(r);
+    if (it == keys->evk.end()) return fail(ctx, FENC_ERR_NO_KEY, "no rotation key for step %d", r);
+    BatchItem b{};
+    b.ks_in = in[i] + LN, b.sub_in = nullptr, b.out = out[i], b.evk = it->second, b.add0 = in[i], b.add1 = nullptr;
+    b.g = galois_elt(ctx, r);
+    items.push_back(b);
+  }
+  return ks_batch(ctx, L, items);
+}

@@ -1,0 +1,150 @@
+// fenc_ctx.h -- host-side objects behind the opaque handles of include/fenc.h (library private).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <array>
+#include <map>
+#include <memory>
+#include <string>
+#include <vector>
+
+#include "fenc_internal.h"
+
+// Per-level (number of ciphertext limbs L) tables of the hybrid key switch and of the rescale (R2.6, R2.8).
+struct LevelPlan {
+  int L, E, beta, n_up;      // E = L + np target rows; n_up = rows of the ModUp temp = beta*E - L
+  // key switch
+  RowDesc *d_rows_in;        // [L] iNTT of the polynomial to switch (row t, modulus t)
+  ShoupC *d_scale_in;        // [L] N^-1 * Qhat_{j,t}^-1 mod q_t (the ModUp pre-scaling folded into the iNTT)
+  RowDesc *d_rows_up;        // [n_up] ModUp + forward pass 1 job rows
+  u64 *d_bc_up;              // Montgomery-form (Q_j / q_i mod t) constants, indexed by RowDesc.aux2 + s
+  int *d_tmp_index;          // [beta*E] -> row of the ModUp temp or -1
+  RowDesc *d_rows_p;         // [2 np] iNTT of the special limbs of both accumulators
+  ShoupC *d_scale_p;         // [2 np] N^-1 * Phat_i^-1 mod p_i
+  RowDesc *d_rows_down;      // [2L] ModDown conversion + forward pass 1
+  u64 *d_bc_down;            // [L*np] (P / p_i mod q_t) Montgomery form
+  RowDesc *d_rows_div;       // [2L] forward pass 2 + divide epilogue
+  ShoupC *d_mul_pinv;        // [A] P^-1 mod q_t
+  // rescale (drop limb L-1)
+  RowDesc *d_rows_rs_in;     // [2]
+  ShoupC *d_scale_rs;        // [2] N^-1 mod q_{L-1}
+  RowDesc *d_rows_rs_up;     // [2(L-1)]
+  u64 *d_bc_rs;              // [L-1] 2^64 mod q_t (i.e. "mod t")
+  RowDesc *d_rows_rs_div;    // [2(L-1)]
+  ShoupC *d_mul_qlinv;       // [A] q_{L-1}^-1 mod q_t
+  // plain transforms of a whole ciphertext [2][L][N]
+  RowDesc *d_rows_ct;        // [2L]
+  ShoupC *d_scale_ct;        // [2L] N^-1 mod q_t
+  std::vector<void *> owned;
+};
+
+struct ConvGraph;  // fenc_conv.cu
+
+struct fenc_ctx {
+  int logN = 0, N = 0, n = 0, nq = 0, np = 0, A = 0, dlen = 0, beta_max = 0;
+  std::vector<u64> mod, psi;  // q_0..q_{nq-1}, p_0..p_{np-1}
+  double default_scale = 0;
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  void *(*dev_alloc)(size_t, void *) = nullptr;
+  void (*dev_free)(void *, void *) = nullptr;
+  void *user = nullptr;
+  ModConst *d_mods = nullptr;
+  ShoupC *d_tw_fwd = nullptr, *d_tw_inv = nullptr;
+  RowDesc *d_ident_rows = nullptr;  // [A] row r <-> modulus r
+  ShoupC *d_ninv = nullptr;         // [A] N^-1 mod each modulus
+  int *d_ident_mod = nullptr;       // [2A] 0..A-1, 0..A-1
+  KCtx k{};
+  u64 launches = 0, dev_bytes = 0;
+  int max_lazy = 1;                 // floor(2^64 / max modulus): terms per lazy 128-bit accumulation
+  std::string err;
+  std::map<int, std::unique_ptr<LevelPlan>> plans;
+  std::map<void *, size_t> live;    // device pointer -> bytes (accounting)
+  void *ws = nullptr;               // grow-only key-switch workspace
+  size_t ws_bytes = 0;
+  void *desc_buf = nullptr;         // device staging for per-call descriptor arrays
+  size_t desc_bytes = 0;
+  std::map<std::string, std::shared_ptr<ConvGraph>> graphs;
+};
+
+struct fenc_keys {
+  fenc_ctx *ctx;
+  u64 seed;
+  std::vector<int64_t> s;        // secret coefficients
+  u64 *d_s_mont = nullptr;       // [A][N] NTT domain, Montgomery form
+  std::map<int64_t, u64 *> evk;  // key id -> [beta_max][2][A][N] NTT domain, Montgomery form
+};
+
+struct fenc_pt {
+  fenc_ctx *ctx;
+  int L;
+  double scale;
+  std::vector<int64_t> coeffs;  // centred integer coefficients (A7: parity starts here)
+  u64 *d_mont = nullptr;        // [L][N] NTT domain, Montgomery form (built on first use)
+};
+
+struct fenc_ct {
+  fenc_ctx *ctx;
+  int L;
+  double scale;
+  u64 *d;  // [2][L][N] NTT domain, canonical
+};
+
+struct fenc_wts {
+  fenc_ctx *ctx;
+  int L;
+  double scale;
+  size_t n;
+  u64 *d_all = nullptr;  // [n][L][N] NTT domain, Montgomery form, fenc_wts_keys order
+  std::string graph_key;
+};
+
+// ---------------------------------------------------------------- helpers (fenc_ctx.cu)
+fenc_status fail(fenc_ctx *ctx, fenc_status st, const char *fmt, ...);
+#define CUDA_OK(ctx, expr)                                                                              \
+  do {                                                                                                  \
+    cudaError_t e__ = (cudaError_t)(expr);                                                              \
+    if (e__ != cudaSuccess) return fail(ctx, FENC_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e__)); \
+  } while (0)
+void *dalloc(fenc_ctx *ctx, size_t bytes);
+void dfree(fenc_ctx *ctx, void *p);
+template <class T>
+T *dalloc_t(fenc_ctx *ctx, size_t count) { return (T *)dalloc(ctx, count * sizeof(T)); }
+// upload a host vector into plan-owned device memory
+template <class T>
+T *upload_owned(fenc_ctx *ctx, std::vector<void *> &owned, const std::vector<T> &v) {
+  T *d = dalloc_t<T>(ctx, v.size() ? v.size() : 1);
+  if (!d) return nullptr;
+  if (!v.empty()) cudaMemcpyAsync(d, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, ctx->stream);
+  owned.push_back(d);
+  return d;
+}
+LevelPlan *get_plan(fenc_ctx *ctx, int L);
+void *workspace(fenc_ctx *ctx, size_t bytes);
+// stage small host arrays into the context's descriptor buffer (one region per call site per batch)
+struct DescStage {
+  fenc_ctx *ctx;
+  size_t off = 0;
+  std::vector<char> host;
+  explicit DescStage(fenc_ctx *c) : ctx(c) {}
+  template <class T>
+  size_t add(const std::vector<T> &v) {
+    size_t o = (host.size() + 255) & ~(size_t)255;
+    host.resize(o + v.size() * sizeof(T));
+    if (!v.empty()) memcpy(host.data() + o, v.data(), v.size() * sizeof(T));
+    return o;
+  }
+  // uploads; returns device base or nullptr
+  char *commit();
+};
+fenc_ct *new_ct(fenc_ctx *ctx, int L, double scale);
+// batched key switch over items (all at level L): out = (ModDown(acc_0) + add0, ModDown(acc_1) + add1)
+fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items);
+// batched rescale: items[i].sub_in = input ct [2][L][N], items[i].out = [2][L-1][N]
+fenc_status rescale_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items);
+// rotation items for (in, step) pairs; step 0 handled by a device copy
+fenc_status rotate_raw(fenc_ctx *ctx, const fenc_keys *keys, int L, const std::vector<const u64 *> &in,
+                       const std::vector<int> &steps, const std::vector<u64 *> &out);
+u32 galois_elt(const fenc_ctx *ctx, int step);
+fenc_status pt_device(fenc_ctx *ctx, fenc_pt *pt);  // ensure pt->d_mont
+fenc_status coeffs_to_mont(fenc_ctx *ctx, const int64_t *coeffs_host, int L, u64 *d_out);

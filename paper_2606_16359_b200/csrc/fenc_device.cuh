@@ -1,0 +1,127 @@
+// fenc_device.cuh -- device-side modular arithmetic and the shared-memory NTT tile engine (sm_100a).
+//
+// Arithmetic: 64-bit words on the 32-bit integer pipes (IMAD.WIDE on the fma pipe, IADD3/LOP3 on the alu pipe).
+//  - constant operands (twiddles, scaling constants): Shoup multiplication with a precomputed floor(c 2^64 / q),
+//    Harvey lazy butterflies with values in [0,4q) (forward) / [0,2q) (inverse); needs q < 2^62.
+//  - variable x variable sums (evk inner product, plaintext MAC, base conversion): 128-bit lazy accumulation of
+//    x * y_mont products followed by ONE Montgomery reduction (y stored as y 2^64 mod q).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "fenc_internal.h"
+
+#define DEVI __device__ __forceinline__
+
+DEVI u64 csub(u64 x, u64 q) { return x >= q ? x - q : x; }
+
+// x * c mod q in [0, 2q) for any x < 2^64 (cs = floor(c 2^64 / q), c < q)
+DEVI u64 shoup_lazy(u64 x, u64 c, u64 cs, u64 q) {
+  u64 hi = __umul64hi(x, cs);
+  return x * c - hi * q;
+}
+DEVI u64 shoup_mul(u64 x, u64 c, u64 cs, u64 q) { return csub(shoup_lazy(x, c, cs, q), q); }
+
+// (hi:lo) += a * b
+DEVI void mac128(u64 &lo, u64 &hi, u64 a, u64 b) {
+  asm("mad.lo.cc.u64 %0, %2, %3, %0;\n\tmadc.hi.u64 %1, %2, %3, %1;" : "+l"(lo), "+l"(hi) : "l"(a), "l"(b));
+}
+// Montgomery reduction: (hi:lo) 2^-64 mod q, canonical; requires (hi:lo) < q 2^64
+DEVI u64 mont_redc(u64 lo, u64 hi, u64 q, u64 qinv_neg) {
+  u64 m = lo * qinv_neg;
+  u64 t = hi + __umul64hi(m, q) + (lo != 0 ? 1ull : 0ull);
+  return csub(t, q);
+}
+// a * b_mont 2^-64 mod q  (= a*b mod q when b_mont = b 2^64 mod q)
+DEVI u64 mont_mul(u64 a, u64 b, u64 q, u64 qinv_neg) {
+  u64 lo = a * b, hi = __umul64hi(a, b);
+  return mont_redc(lo, hi, q, qinv_neg);
+}
+DEVI u64 addmod(u64 a, u64 b, u64 q) { return csub(a + b, q); }
+DEVI u64 submod(u64 a, u64 b, u64 q) { return a >= b ? a - b : a + q - b; }
+
+// NTT-domain index map of the Galois automorphism sigma_g (R2.7): position p of the transform holds the
+// evaluation at psi^(2 brev(p) + 1); sigma_g(a) evaluated there is a evaluated at psi^((2 brev(p) + 1) g).
+DEVI u32 galois_src(u32 p, u32 g, int logN) {
+  u32 e = __brev(p) >> (32 - logN);
+  u32 r = ((g * (2u * e + 1u)) >> 1) & ((1u << logN) - 1u);
+  return __brev(r) >> (32 - logN);
+}
+
+// shared-memory swizzle: XOR of low index bits with bits 4..6 so that the radix-8 register rounds at window
+// positions 0, 2, 3 and >= 5 as well as linear accesses are bank-conflict free for 64-bit words.
+DEVI int swz(int e) { return e ^ (((e >> 4) & 1) << 1) ^ (((e >> 5) & 1) << 2) ^ (((e >> 6) & 1) * 9); }
+
+// Tile geometry: tile element e (0 <= e < 2^lt) is global coefficient
+//   j = ((e >> lc) << sh) | (tile << lc) | (e & (2^lc - 1)).
+// Row pass: lc = lt (contiguous tile).  Column pass: lc = log2(columns per tile), sh = brow.
+struct TileGeo {
+  int lt, lc, sh, logN;
+  u32 tile;
+  DEVI u32 gidx(int e) const { return ((u32)(e >> lc) << sh) | (tile << lc) | ((u32)e & ((1u << lc) - 1u)); }
+  DEVI int gbit(int pb) const { return pb < lc ? pb : pb - lc + sh; }  // global bit of tile bit pb
+};
+
+// One radix-8 register round over tile bits [pw, pw+3); only window bits s in [s_lo, s_hi) are transformed.
+// FWD: Cooley-Tukey, high bit first, values in [0,4q).  INV: Gentleman-Sande, low bit first, values in [0,2q).
+template <bool FWD>
+DEVI void tile_round(u64 *sm, const TileGeo &G, int pw, int s_lo, int s_hi, const ShoupC *tw, u64 q, u64 q2, int tid) {
+  const int ebase = ((tid >> pw) << (pw + 3)) | (tid & ((1 << pw) - 1));
+  u64 x[8];
+#pragma unroll
+  for (int k = 0; k < 8; k++) x[k] = sm[swz(ebase | (k << pw))];
+  const u32 N = 1u << G.logN;
+#pragma unroll
+  for (int ss = 0; ss < 3; ss++) {
+    const int s = FWD ? 2 - ss : ss;
+    if (s < s_lo || s >= s_hi) continue;
+    const int g1 = G.gbit(pw + s) + 1;
+#pragma unroll
+    for (int k = 0; k < 8; k++) {
+      if (k & (1 << s)) continue;
+      const int k2 = k | (1 << s);
+      const u32 j = G.gidx(ebase | (k << pw));
+      const ShoupC w = tw[(N + j) >> g1];
+      if (FWD) {
+        u64 X = csub(x[k], q2);
+        u64 T = shoup_lazy(x[k2], w.c, w.cs, q);
+        x[k] = X + T;
+        x[k2] = X - T + q2;
+      } else {
+        u64 U = x[k], V = x[k2];
+        x[k] = csub(U + V, q2);
+        x[k2] = shoup_lazy(U - V + q2, w.c, w.cs, q);
+      }
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < 8; k++) sm[swz(ebase | (k << pw))] = x[k];
+}
+
+// All rounds of one pass over active tile bits [lo, lo+nb).  Every thread of the block must call this
+// (it synchronises); threads with tid >= 2^(lt-3) only take part in the barriers.
+template <bool FWD>
+DEVI void tile_transform(u64 *sm, const TileGeo &G, int lo, int nb, const ShoupC *tw, u64 q, int tid) {
+  const u64 q2 = q + q;
+  const bool active = tid < (1 << (G.lt - 3));
+  if (FWD) {
+    int cur = lo + nb;
+    while (cur > lo) {
+      int take = cur - lo < 3 ? cur - lo : 3;
+      int p = cur - take;
+      int pw = p < G.lt - 3 ? p : G.lt - 3;
+      if (active) tile_round<true>(sm, G, pw, p - pw, cur - pw, tw, q, q2, tid);
+      __syncthreads();
+      cur = p;
+    }
+  } else {
+    int cur = lo;
+    while (cur < lo + nb) {
+      int take = lo + nb - cur < 3 ? lo + nb - cur : 3;
+      int pw = cur < G.lt - 3 ? cur : G.lt - 3;
+      if (active) tile_round<false>(sm, G, pw, cur - pw, cur + take - pw, tw, q, q2, tid);
+      __syncthreads();
+      cur += take;
+    }
+  }
+}

@@ -1,0 +1,227 @@
+// fenc_elem.cu -- element-wise kernels of the hot path: plaintext MAC (a7), ciphertext sums, encrypt / decrypt
+// combines, the counter-based samplers (R2.3) and Montgomery-form conversions.  sm_100a.
+// All are HBM-bound streaming kernels: 16-byte vector accesses, limb-major, one pass.
+#include "fenc_device.cuh"
+
+#define LAUNCH_CHECK(k)                         \
+  do {                                          \
+    (*(k).launches)++;                          \
+    cudaError_t e__ = cudaGetLastError();       \
+    if (e__ != cudaSuccess) return (int)e__;    \
+  } while (0)
+
+static inline cudaStream_t S(const KCtx &k) { return (cudaStream_t)k.stream; }
+
+// ------------------------------------------------------------------------------------------------ MAC (a7)
+// outs[o][c][l][n] = sum_t ct_t[c][l][n] * pt_t[l][n]; products accumulate in 128 bits and are reduced once per
+// max_lazy terms (max_lazy = floor(2^64 / q_max) keeps the accumulator below q 2^64).
+struct MacP {
+  const u64 *const *term_ct; const u64 *const *term_pt; const int *start; u64 *const *outs; const ModConst *mods;
+  int L, logN, max_lazy;
+};
+__global__ void __launch_bounds__(256) mac_kernel(MacP p) {
+  const size_t LN = (size_t)p.L << p.logN;
+  const size_t idx = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) * 2;
+  if (idx >= LN) return;
+  const int o = blockIdx.y;
+  const ModConst mc = p.mods[idx >> p.logN];
+  const int t0 = p.start[o], t1 = p.start[o + 1];
+  u64 r00 = 0, r01 = 0, r10 = 0, r11 = 0;  // reduced running sums [comp][elem]
+  u64 l00 = 0, h00 = 0, l01 = 0, h01 = 0, l10 = 0, h10 = 0, l11 = 0, h11 = 0;
+  int lazy = 0;
+  for (int t = t0; t < t1; t++) {
+    const u64 *c = p.term_ct[t];
+    const ulonglong2 w = __ldg(reinterpret_cast<const ulonglong2 *>(p.term_pt[t] + idx));
+    const ulonglong2 x0 = __ldg(reinterpret_cast<const ulonglong2 *>(c + idx));
+    const ulonglong2 x1 = __ldg(reinterpret_cast<const ulonglong2 *>(c + LN + idx));
+    mac128(l00, h00, x0.x, w.x); mac128(l01, h01, x0.y, w.y);
+    mac128(l10, h10, x1.x, w.x); mac128(l11, h11, x1.y, w.y);
+    if (++lazy == p.max_lazy) {
+      r00 = addmod(r00, mont_redc(l00, h00, mc.q, mc.qinv_neg), mc.q); r01 = addmod(r01, mont_redc(l01, h01, mc.q, mc.qinv_neg), mc.q);
+      r10 = addmod(r10, mont_redc(l10, h10, mc.q, mc.qinv_neg), mc.q); r11 = addmod(r11, mont_redc(l11, h11, mc.q, mc.qinv_neg), mc.q);
+      l00 = h00 = l01 = h01 = l10 = h10 = l11 = h11 = 0; lazy = 0;
+    }
+  }
+  r00 = addmod(r00, mont_redc(l00, h00, mc.q, mc.qinv_neg), mc.q); r01 = addmod(r01, mont_redc(l01, h01, mc.q, mc.qinv_neg), mc.q);
+  r10 = addmod(r10, mont_redc(l10, h10, mc.q, mc.qinv_neg), mc.q); r11 = addmod(r11, mont_redc(l11, h11, mc.q, mc.qinv_neg), mc.q);
+  u64 *out = p.outs[o];
+  *reinterpret_cast<ulonglong2 *>(out + idx) = make_ulonglong2(r00, r01);
+  *reinterpret_cast<ulonglong2 *>(out + LN + idx) = make_ulonglong2(r10, r11);
+}
+int k_mac(const KCtx &k, const u64 *const *term_ct, const u64 *const *term_pt, const int *start, u64 *const *outs, int n_out,
+          int L, int max_lazy) {
+  if (n_out == 0) return 0;
+  MacP p{term_ct, term_pt, start, outs, k.d_mods, L, k.geom.logN, max_lazy};
+  size_t pairs = ((size_t)L * k.N) / 2;
+  dim3 grid((unsigned)((pairs + 255) / 256), n_out);
+  mac_kernel<<<grid, 256, 0, S(k)>>>(p);
+  LAUNCH_CHECK(k);
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------------ sum of ciphertexts
+struct AddManyP { const u64 *const *term; const int *start; u64 *const *outs; const ModConst *mods; int L, logN; };
+__global__ void __launch_bounds__(256) add_many_kernel(AddManyP p) {
+  const size_t LN = (size_t)p.L << p.logN;
+  const size_t idx = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) * 2;  // over [2][L][N]
+  if (idx >= 2 * LN) return;
+  const int o = blockIdx.y;
+  const u64 q = p.mods[(idx % LN) >> p.logN].q;
+  u64 a = 0, b = 0;
+  for (int t = p.start[o]; t < p.start[o + 1]; t++) {
+    const ulonglong2 x = __ldg(reinterpret_cast<const ulonglong2 *>(p.term[t] + idx));
+    a = addmod(a, x.x, q); b = addmod(b, x.y, q);
+  }
+  *reinterpret_cast<ulonglong2 *>(p.outs[o] + idx) = make_ulonglong2(a, b);
+}
+int k_add_many(const KCtx &k, const u64 *const *term, const int *start, u64 *const *outs, int n_out, int L) {
+  if (n_out == 0) return 0;
+  AddManyP p{term, start, outs, k.d_mods, L, k.geom.logN};
+  size_t pairs = (size_t)L * k.N;
+  dim3 grid((unsigned)((pairs + 255) / 256), n_out);
+  add_many_kernel<<<grid, 256, 0, S(k)>>>(p);
+  LAUNCH_CHECK(k);
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------------ generic row kernels
+// grid (N/256, n_rows); row r uses modulus row_mod[r]
+enum RowOp { OP_X_MINUS_AS, OP_TO_MONT, OP_FROM_MONT, OP_ADD_F_SP, OP_MUL, OP_ADD, OP_ADD_TWICE, OP_REDUCE_SIGNED };
+struct RowP {
+  const u64 *a; const u64 *b; const u64 *s; u64 *out; const int *row_mod; const ModConst *mods; const u64 *f;
+  const i64 *coeffs; int logN; u32 g;
+};
+template <int OP>
+__global__ void __launch_bounds__(256) row_kernel(RowP p) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x, r = blockIdx.y, N = 1 << p.logN;
+  if (n >= N) return;
+  const int mod = p.row_mod[r];
+  const ModConst mc = p.mods[mod];
+  const size_t i = (size_t)r * N + n;
+  u64 v;
+  if (OP == OP_X_MINUS_AS) v = submod(p.b[i], mont_mul(p.a[i], p.s[(size_t)mod * N + n], mc.q, mc.qinv_neg), mc.q);
+  else if (OP == OP_TO_MONT) v = mont_mul(p.a[i], mc.r2, mc.q, mc.qinv_neg);
+  else if (OP == OP_FROM_MONT) v = mont_redc(p.a[i], 0, mc.q, mc.qinv_neg);
+  else if (OP == OP_ADD_F_SP) {
+    const u64 sp = p.s[(size_t)mod * N + galois_src(n, p.g, p.logN)];  // sigma_g(s) in the NTT domain, Montgomery form
+    v = addmod(p.a[i], mont_mul(p.f[mod], sp, mc.q, mc.qinv_neg), mc.q);
+  } else if (OP == OP_MUL) v = mont_mul(p.a[i], mont_mul(p.b[i], mc.r2, mc.q, mc.qinv_neg), mc.q, mc.qinv_neg);
+  else if (OP == OP_ADD) v = addmod(p.a[i], p.b[i], mc.q);
+  else if (OP == OP_ADD_TWICE) v = addmod(addmod(p.a[i], p.b[i], mc.q), p.b[i], mc.q);
+  else {  // OP_REDUCE_SIGNED: centred integer -> residue (negative -> q - |m| mod q)
+    const i64 m = p.coeffs[n];
+    const u64 mag = (u64)(m < 0 ? -m : m) % mc.q;
+    v = (m < 0 && mag) ? mc.q - mag : mag;
+  }
+  p.out[i] = v;
+}
+template <int OP>
+static int launch_row(const KCtx &k, RowP p, int n_rows) {
+  if (n_rows == 0) return 0;
+  p.mods = k.d_mods; p.logN = k.geom.logN;
+  dim3 grid((k.N + 255) / 256, n_rows);
+  row_kernel<OP><<<grid, 256, 0, S(k)>>>(p);
+  LAUNCH_CHECK(k);
+  return 0;
+}
+int k_x_minus_as(const KCtx &k, const u64 *a, const u64 *x, const u64 *s_mont, u64 *out, const int *row_mod, int n_rows) {
+  RowP p{}; p.a = a; p.b = x; p.s = s_mont; p.out = out; p.row_mod = row_mod;
+  return launch_row<OP_X_MINUS_AS>(k, p, n_rows);
+}
+int k_mont_convert(const KCtx &k, const u64 *src, u64 *dst, const int *row_mod, int n_rows, bool to_mont) {
+  RowP p{}; p.a = src; p.out = dst; p.row_mod = row_mod;
+  return to_mont ? launch_row<OP_TO_MONT>(k, p, n_rows) : launch_row<OP_FROM_MONT>(k, p, n_rows);
+}
+int k_add_f_sprime(const KCtx &k, const u64 *x, const u64 *sp_mont, u32 g, const u64 *f, u64 *out, const int *row_mod,
+                   int n_rows) {
+  RowP p{}; p.a = x; p.s = sp_mont; p.g = g; p.f = f; p.out = out; p.row_mod = row_mod;
+  return launch_row<OP_ADD_F_SP>(k, p, n_rows);
+}
+int k_mul_rows(const KCtx &k, const u64 *a, const u64 *b, u64 *out, const int *row_mod, int n_rows) {
+  RowP p{}; p.a = a; p.b = b; p.out = out; p.row_mod = row_mod;
+  return launch_row<OP_MUL>(k, p, n_rows);
+}
+int k_add_rows(const KCtx &k, const u64 *a, const u64 *b, u64 *out, const int *row_mod, int n_rows, bool twice) {
+  RowP p{}; p.a = a; p.b = b; p.out = out; p.row_mod = row_mod;
+  return twice ? launch_row<OP_ADD_TWICE>(k, p, n_rows) : launch_row<OP_ADD>(k, p, n_rows);
+}
+int k_reduce_signed(const KCtx &k, const i64 *coeffs, const int *row_mod, u64 *dst, int n_rows) {
+  RowP p{}; p.coeffs = coeffs; p.out = dst; p.row_mod = row_mod;
+  return launch_row<OP_REDUCE_SIGNED>(k, p, n_rows);
+}
+
+// out[t] = c0[t] + c1[t] * s[t]  (decrypt, R2.5)
+__global__ void __launch_bounds__(256) dec_combine_kernel(const u64 *ct, const u64 *s_mont, u64 *out, const ModConst *mods, int L, int logN) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x, t = blockIdx.y, N = 1 << logN;
+  if (n >= N) return;
+  const ModConst mc = mods[t];
+  const size_t i = (size_t)t * N + n;
+  out[i] = addmod(ct[i], mont_mul(ct[(size_t)L * N + i], s_mont[i], mc.q, mc.qinv_neg), mc.q);
+}
+int k_dec_combine(const KCtx &k, const u64 *ct, const u64 *s_mont, u64 *out, int L) {
+  dim3 grid((k.N + 255) / 256, L);
+  dec_combine_kernel<<<grid, 256, 0, S(k)>>>(ct, s_mont, out, k.d_mods, L, k.geom.logN);
+  LAUNCH_CHECK(k);
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------------ samplers (R2.3)
+// draw(key, n) = mix64(key + (n+1) GAMMA); coefficient i owns counters i*64 .. i*64+63.
+#define FENC_GAMMA 0x9E3779B97F4A7C15ull
+DEVI u64 d_mix64(u64 z) {
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+DEVI u64 d_draw(u64 key, u64 n) { return d_mix64(key + (n + 1) * FENC_GAMMA); }
+
+// C[x] = floor(2^64 Pr(|X| <= x)), X discrete Gaussian sigma = 3.2 cut at |x| <= 19 (R2.3 table)
+__constant__ u64 c_gauss_cdt[19] = {
+    0x1fea56814b22fe3aull, 0x5cb44ba97e1c801cull, 0x9135c4d2ab6097acull, 0xba57841ec437e30aull, 0xd790d29879901fe9ull,
+    0xea65b1358d74fb9dull, 0xf5672d96e886cf31ull, 0xfb3c9d22cc87d60full, 0xfe0a92b033d640a2ull, 0xff439d38007352aeull,
+    0xffbf67e425d189d1ull, 0xffebcdf3a4629f98ull, 0xfffa3f2f78880d45ull, 0xfffe81f40111a23bull, 0xffffa5d06bc38afbull,
+    0xffffeca4870dfe3cull, 0xfffffc3b68ed3b4aull, 0xffffff58143b9611ull, 0xffffffe850ce70a6ull};
+
+__global__ void __launch_bounds__(256) sample_uniform_kernel(const u64 *keys, const int *row_mod, u64 *dst, const ModConst *mods, int logN) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x, r = blockIdx.y, N = 1 << logN;
+  if (n >= N) return;
+  const ModConst mc = mods[row_mod[r]];
+  const u64 key = keys[r];
+  u64 x = 0;
+  bool ok = false;
+  for (int a = 0; a < 64 && !ok; a++) {
+    x = d_draw(key, (u64)n * 64 + a) & mc.mask;
+    ok = x < mc.q;
+  }
+  if (!ok) x %= mc.q;
+  dst[(size_t)r * N + n] = x;
+}
+int k_sample_uniform(const KCtx &k, const u64 *keys, const int *row_mod, u64 *dst, int n_rows) {
+  if (n_rows == 0) return 0;
+  dim3 grid((k.N + 255) / 256, n_rows);
+  sample_uniform_kernel<<<grid, 256, 0, S(k)>>>(keys, row_mod, dst, k.d_mods, k.geom.logN);
+  LAUNCH_CHECK(k);
+  return 0;
+}
+
+__global__ void __launch_bounds__(256) sample_gauss_kernel(u64 key, const i64 *addend, const int *row_mod, u64 *dst, const ModConst *mods,
+                                                           int logN, int n_rows) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x, N = 1 << logN;
+  if (n >= N) return;
+  const u64 u = d_draw(key, (u64)n * 64);
+  int mag = 0;
+  for (int x = 0; x < 19; x++) mag += (c_gauss_cdt[x] <= u) ? 1 : 0;  // least x with u < C[x]
+  i64 v = (d_draw(key, (u64)n * 64 + 1) & 1) ? -(i64)mag : (i64)mag;
+  if (addend) v += addend[n];
+  for (int r = 0; r < n_rows; r++) {
+    const u64 q = mods[row_mod[r]].q;
+    const u64 m = (u64)(v < 0 ? -v : v) % q;
+    dst[(size_t)r * N + n] = (v < 0 && m) ? q - m : m;
+  }
+}
+int k_sample_gauss(const KCtx &k, u64 key, const i64 *addend, const int *row_mod, u64 *dst, int n_rows) {
+  if (n_rows == 0) return 0;
+  sample_gauss_kernel<<<(k.N + 255) / 256, 256, 0, S(k)>>>(key, addend, row_mod, dst, k.d_mods, k.geom.logN, n_rows);
+  LAUNCH_CHECK(k);
+  return 0;
+}

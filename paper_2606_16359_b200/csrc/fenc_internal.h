@@ -1,0 +1,141 @@
+// fenc_internal.h -- shared declarations of libfenc's translation units (not part of the public ABI).
+// Nothing here is shared with oracle/ (the CPU oracle is an independent program).
+#pragma once
+#include <stddef.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "../../include/fenc.h"
+
+typedef uint64_t u64;
+typedef uint32_t u32;
+typedef unsigned __int128 u128;
+typedef long long i64;
+
+#define FENC_MAX_MOD 64  // moduli per context (n_q + n_p)
+
+// ---------------------------------------------------------------- device-visible tables
+struct ModConst {  // one per modulus, device global memory
+  u64 q;           // prime, < 2^61
+  u64 qinv_neg;    // -q^{-1} mod 2^64 (Montgomery)
+  u64 r2;          // 2^128 mod q: mont_mul(x, r2) = x 2^64 mod q
+  u64 mask;        // 2^ceil(log2 q) - 1 (uniform rejection sampler)
+};
+
+struct ShoupC {  // constant c with its Shoup companion floor(c 2^64 / q)
+  u64 c, cs;
+};
+
+// one job row of a batched NTT launch
+struct RowDesc {
+  int mod;      // modulus index
+  int src_row;  // row in the source tensor (first source row for a base conversion)
+  int dst_row;  // row in the destination tensor
+  int aux;      // base conversion: number of source rows; divide epilogue: component (0/1)
+  int aux2;     // base conversion: offset of this row's constants; divide epilogue: row in the minuend tensor
+  int pad[3];
+};
+
+// one element of a batch of key switches (rotations, relinearisations, rescales)
+struct BatchItem {
+  const u64 *ks_in;  // polynomial to switch [L][N] (NTT domain); rotation: c1 of the input
+  const u64 *sub_in; // rescale: the input ciphertext [2][L][N] (minuend of the divide epilogue)
+  u64 *out;          // output ciphertext [2][L_out][N]
+  const u64 *evk;    // switching key [beta_max][2][A][N] (NTT domain, Montgomery form)
+  const u64 *add0;   // epilogue addend for component 0 ([L][N], read through the Galois gather) or NULL
+  const u64 *add1;   // epilogue addend for component 1 or NULL
+  u32 g;             // Galois element (1 = identity)
+  u32 pad;
+};
+
+// geometry of the 2-pass NTT for one ring degree
+struct NttGeom {
+  int logN;
+  int brow;    // stages done by the row pass (contiguous sub-transforms of 2^brow points)
+  int bcol;    // stages done by the column pass (stride 2^brow)
+  int lt_row;  // log2 tile elements of the row pass
+  int lt_col;  // log2 tile elements of the column pass
+  int lc_col;  // log2 columns per tile of the column pass
+};
+
+struct KCtx {  // what kernels need from a context
+  void *stream;  // cudaStream_t
+  NttGeom geom;
+  const ModConst *d_mods;
+  const ShoupC *d_tw_fwd;  // [nmod][N] forward twiddles psi^bitrev(k)
+  const ShoupC *d_tw_inv;  // [nmod][N] inverse twiddles
+  u64 *launches;           // host counter of kernel launches
+  int N, nq, np;
+};
+
+// ---------------------------------------------------------------- launchers (fenc_kernels.cu); return cudaError_t
+// inverse NTT (both passes).  Source row r of batch b: (items ? items[b].ks_in : src + b*src_bstride) +
+// rows[r].src_row*N, read through the Galois gather of items[b].g when gather.  Result: coefficient domain,
+// canonical, times scale[r], at dst + b*dst_bstride + rows[r].dst_row*N.
+int k_intt(const KCtx &k, const BatchItem *items, const u64 *src, size_t src_bstride, bool gather, u64 *dst,
+           size_t dst_bstride, const RowDesc *rows, int n_rows, const ShoupC *scale, int n_batch);
+// forward NTT of plain rows: src + b*src_bstride + rows[r].src_row*N -> dst + b*dst_bstride + rows[r].dst_row*N
+int k_ntt(const KCtx &k, const u64 *src, size_t src_bstride, u64 *dst, size_t dst_bstride, const RowDesc *rows, int n_rows,
+          int n_batch);
+// forward pass 1 (column stages) with fused base conversion (ModUp a3 / ModDown's Conv / rescale's mod):
+// value = sum_{s < rows[r].aux} y[b][rows[r].src_row + s][.] * bc[rows[r].aux2 + s] (Montgomery constants)
+int k_ntt_cols_bconv(const KCtx &k, const u64 *y, size_t y_bstride, const u64 *bc, u64 *tmp, size_t tmp_bstride,
+                     const RowDesc *rows, int n_rows, int n_batch);
+// forward pass 2 (row stages) fused with the evaluation-key inner product (a4) over E = L + np target rows.
+// tmp_index[j*E + t] = row of tmp holding digit j / target t, or -1 when t lies in digit j (then the row is
+// items[b].ks_in[t] itself, read through the Galois gather).  acc[b][c][t][N] canonical.
+int k_ntt_rows_keymac(const KCtx &k, const BatchItem *items, int L, int E, int beta, const int *tmp_index, const u64 *tmp,
+                      size_t tmp_bstride, u64 *acc, size_t acc_bstride, int n_batch);
+// forward pass 2 fused with the divide epilogue (ModDown a5 / rescale a8):
+// out[dst_row] = (minuend[aux2] - X) * mul[mod] (+ addend_c[mod] through the gather)
+// minuend = from_items ? items[b].sub_in : acc + b*acc_bstride
+int k_ntt_rows_divide(const KCtx &k, const BatchItem *items, const u64 *tmp, size_t tmp_bstride, const u64 *acc,
+                      size_t acc_bstride, bool minuend_from_items, const ShoupC *mul, const RowDesc *rows, int n_rows,
+                      int n_batch);
+// MAC (a7): outs[o] = sum_{t in [start[o], start[o+1])} ct[t] (*) pt[t]; ct [2][L][N], pt [L][N] Montgomery form
+int k_mac(const KCtx &k, const u64 *const *term_ct, const u64 *const *term_pt, const int *start, u64 *const *outs, int n_out,
+          int L, int max_lazy);
+// outs[o] = sum of listed [2][L][N] arrays
+int k_add_many(const KCtx &k, const u64 *const *term, const int *start, u64 *const *outs, int n_out, int L);
+// rows kernels: row r uses modulus row_mod[r] (device array)
+// out = x - a * s_mont[mod]   (s_mont: [nmod][N] Montgomery form)
+int k_x_minus_as(const KCtx &k, const u64 *a, const u64 *x, const u64 *s_mont, u64 *out, const int *row_mod, int n_rows);
+// out[t] = c0[t] + c1[t] * s_mont[t], t < L
+int k_dec_combine(const KCtx &k, const u64 *ct, const u64 *s_mont, u64 *out, int L);
+// samplers of the counter-based generator (R2.3); coefficient domain, one row per key
+int k_sample_uniform(const KCtx &k, const u64 *keys, const int *row_mod, u64 *dst, int n_rows);
+// dst[r][n] = (gauss(key)[n] + addend[n]) mod q_{row_mod[r]}; addend may be NULL
+int k_sample_gauss(const KCtx &k, u64 key, const i64 *addend, const int *row_mod, u64 *dst, int n_rows);
+int k_reduce_signed(const KCtx &k, const i64 *coeffs, const int *row_mod, u64 *dst, int n_rows);
+// dst = to ? src 2^64 mod q : src 2^-64 mod q
+int k_mont_convert(const KCtx &k, const u64 *src, u64 *dst, const int *row_mod, int n_rows, bool to_mont);
+// b = x + f[mod] * sp[mod][gather_g(.)]   (sp Montgomery-form secret; f normal form): evk's "+ f s'" term
+int k_add_f_sprime(const KCtx &k, const u64 *x, const u64 *sp_mont, u32 g, const u64 *f, u64 *out, const int *row_mod,
+                   int n_rows);
+// out[r] = a[r] * b[r] mod q (both normal form, NTT domain)
+int k_mul_rows(const KCtx &k, const u64 *a, const u64 *b, u64 *out, const int *row_mod, int n_rows);
+// out[r] = a[r] + b[r] (+ b[r] again when twice)
+int k_add_rows(const KCtx &k, const u64 *a, const u64 *b, u64 *out, const int *row_mod, int n_rows, bool twice);
+
+// ---------------------------------------------------------------- host math (fenc_host.cpp)
+namespace fh {
+u64 mulmod(u64 a, u64 b, u64 q);
+u64 powmod(u64 a, u64 e, u64 q);
+u64 invmod(u64 a, u64 q);
+bool is_prime(u64 n);
+bool find_primes(int logN, int bits, int count, std::vector<u64> &out);
+u64 find_psi(u64 q, u64 N);
+u64 shoup(u64 c, u64 q);    // floor(c 2^64 / q)
+u64 to_mont(u64 c, u64 q);  // c 2^64 mod q
+u64 neg_qinv(u64 q);        // -q^{-1} mod 2^64
+void build_twiddles(u64 q, u64 psi, int logN, ShoupC *fwd, ShoupC *inv);
+u64 mix64(u64 z);
+u64 stream_key(u64 seed, u64 purpose, u64 a, u64 b, u64 c);
+void sample_ternary(u64 key, int N, int64_t *out);
+// encode / decode (R2.2): fp64 FFT over the 2N-th roots of unity
+void encode_slots(int logN, const double *re, const double *im, double scale, int64_t *coeffs);
+void decode_coeffs(int logN, const long double *m_over_scale, double *re, double *im);
+// Garner mixed-radix lift of [L][N] residues to centred values divided by scale
+void crt_centre_scaled(const u64 *q, int L, int N, const u64 *res, long double scale, long double *out);
+}  // namespace fh

@@ -1,0 +1,280 @@
+// fenc_ntt.cu -- batched negacyclic NTT / iNTT kernels (a1) and the key-switch kernels fused around them
+// (a2 automorphism gather, a3 ModUp, a4 evk inner product, a5 ModDown, a8 rescale).  sm_100a.
+//
+// Transform (R2.1 and section 6): merged-twiddle Cooley-Tukey forward (natural in, bit-reversed out) and
+// Gentleman-Sande inverse, split in two passes so that each pass works on a shared-memory tile:
+//   forward = column pass (the bcol high stages, stride 2^brow) then row pass (the brow low stages, contiguous);
+//   inverse = row pass then column pass.
+// Each pass: coalesced tile load -> radix-8 register rounds through swizzled shared memory -> coalesced store.
+// The first touch of a forward transform and the last touch of either direction carry the fused work.
+#include "fenc_device.cuh"
+
+static inline int nthreads_for(int lt) { int t = 1 << (lt - 3); return t < 32 ? 32 : t; }
+#define LAUNCH_CHECK(k)                         \
+  do {                                          \
+    (*(k).launches)++;                          \
+    cudaError_t e__ = cudaGetLastError();       \
+    if (e__ != cudaSuccess) return (int)e__;    \
+  } while (0)
+
+// ------------------------------------------------------------------------------------------------ inverse, pass A
+struct InttRowP {
+  const BatchItem *items; const u64 *src; size_t src_bstride; u64 *dst; size_t dst_bstride;
+  const RowDesc *rows; const ModConst *mods; const ShoupC *tw; NttGeom g;
+};
+template <bool GATHER>
+__global__ void __launch_bounds__(256) intt_rowpass_kernel(InttRowP p) {
+  extern __shared__ u64 sm[];
+  const int tid = threadIdx.x, b = blockIdx.z;
+  const RowDesc rd = p.rows[blockIdx.y];
+  const int N = 1 << p.g.logN, T = 1 << p.g.lt_row;
+  TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, blockIdx.x};
+  const u64 *src = (p.items ? p.items[b].ks_in : p.src + (size_t)b * p.src_bstride) + (size_t)rd.src_row * N;
+  const u32 gal = GATHER ? p.items[b].g : 1u;
+  for (int e = tid; e < T; e += blockDim.x) {
+    u32 j = G.gidx(e);
+    sm[swz(e)] = __ldg(src + (GATHER ? galois_src(j, gal, p.g.logN) : j));
+  }
+  __syncthreads();
+  const u64 q = p.mods[rd.mod].q;
+  tile_transform<false>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid);
+  u64 *dst = p.dst + (size_t)b * p.dst_bstride + (size_t)rd.dst_row * N;
+  for (int e = tid; e < T; e += blockDim.x) dst[G.gidx(e)] = sm[swz(e)];
+}
+
+// ------------------------------------------------------------------------------------------------ inverse, pass B
+struct InttColP {
+  u64 *dst; size_t dst_bstride; const RowDesc *rows; const ShoupC *scale; const ModConst *mods; const ShoupC *tw; NttGeom g;
+};
+__global__ void __launch_bounds__(512) intt_colpass_kernel(InttColP p) {
+  extern __shared__ u64 sm[];
+  const int tid = threadIdx.x, b = blockIdx.z;
+  const RowDesc rd = p.rows[blockIdx.y];
+  const int N = 1 << p.g.logN, T = 1 << p.g.lt_col;
+  TileGeo G{p.g.lt_col, p.g.lc_col, p.g.brow, p.g.logN, blockIdx.x};
+  u64 *dst = p.dst + (size_t)b * p.dst_bstride + (size_t)rd.dst_row * N;
+  for (int e = tid; e < T; e += blockDim.x) sm[swz(e)] = dst[G.gidx(e)];
+  __syncthreads();
+  const u64 q = p.mods[rd.mod].q;
+  tile_transform<false>(sm, G, p.g.lc_col, p.g.bcol, p.tw + (size_t)rd.mod * N, q, tid);
+  const ShoupC sc = p.scale[blockIdx.y];
+  for (int e = tid; e < T; e += blockDim.x) dst[G.gidx(e)] = shoup_mul(sm[swz(e)], sc.c, sc.cs, q);
+}
+
+int k_intt(const KCtx &k, const BatchItem *items, const u64 *src, size_t src_bstride, bool gather, u64 *dst,
+           size_t dst_bstride, const RowDesc *rows, int n_rows, const ShoupC *scale, int n_batch) {
+  if (n_rows == 0 || n_batch == 0) return 0;
+  cudaStream_t st = (cudaStream_t)k.stream;
+  const NttGeom &g = k.geom;
+  InttRowP a{items, src, src_bstride, dst, dst_bstride, rows, k.d_mods, k.d_tw_inv, g};
+  dim3 gridA(k.N >> g.lt_row, n_rows, n_batch);
+  if (gather) intt_rowpass_kernel<true><<<gridA, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(a);
+  else intt_rowpass_kernel<false><<<gridA, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(a);
+  LAUNCH_CHECK(k);
+  InttColP c{dst, dst_bstride, rows, scale, k.d_mods, k.d_tw_inv, g};
+  dim3 gridB(k.N >> g.lt_col, n_rows, n_batch);
+  intt_colpass_kernel<<<gridB, nthreads_for(g.lt_col), sizeof(u64) << g.lt_col, st>>>(c);
+  LAUNCH_CHECK(k);
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------------ forward, pass 1
+struct NttColP {
+  const u64 *src; size_t src_bstride; const u64 *bc; u64 *dst; size_t dst_bstride;
+  const RowDesc *rows; const ModConst *mods; const ShoupC *tw; NttGeom g;
+};
+template <bool BCONV>
+__global__ void __launch_bounds__(512) ntt_colpass_kernel(NttColP p) {
+  extern __shared__ u64 sm[];
+  const int tid = threadIdx.x, b = blockIdx.z;
+  const RowDesc rd = p.rows[blockIdx.y];
+  const int N = 1 << p.g.logN, T = 1 << p.g.lt_col;
+  TileGeo G{p.g.lt_col, p.g.lc_col, p.g.brow, p.g.logN, blockIdx.x};
+  const ModConst mc = p.mods[rd.mod];
+  const u64 *src = p.src + (size_t)b * p.src_bstride + (size_t)rd.src_row * N;
+  if (BCONV) {
+    // fused base conversion (R2.6): sum_s y_s * (Qhat_s mod t), one Montgomery reduction
+    const u64 *bc = p.bc + rd.aux2;
+    const int ns = rd.aux;
+    for (int e = tid; e < T; e += blockDim.x) {
+      u32 j = G.gidx(e);
+      u64 lo = 0, hi = 0;
+      for (int s = 0; s < ns; s++) mac128(lo, hi, __ldg(src + (size_t)s * N + j), __ldg(bc + s));
+      sm[swz(e)] = mont_redc(lo, hi, mc.q, mc.qinv_neg);
+    }
+  } else {
+    for (int e = tid; e < T; e += blockDim.x) sm[swz(e)] = __ldg(src + G.gidx(e));
+  }
+  __syncthreads();
+  tile_transform<true>(sm, G, p.g.lc_col, p.g.bcol, p.tw + (size_t)rd.mod * N, mc.q, tid);
+  u64 *dst = p.dst + (size_t)b * p.dst_bstride + (size_t)rd.dst_row * N;
+  for (int e = tid; e < T; e += blockDim.x) dst[G.gidx(e)] = sm[swz(e)];  // lazy, in [0,4q)
+}
+
+// ------------------------------------------------------------------------------------------------ forward, pass 2 (plain)
+struct NttRowP {
+  const u64 *src; size_t src_bstride; u64 *dst; size_t dst_bstride; const RowDesc *rows; const ModConst *mods;
+  const ShoupC *tw; NttGeom g; int src_is_dst_row;
+};
+__global__ void __launch_bounds__(256) ntt_rowpass_kernel(NttRowP p) {
+  extern __shared__ u64 sm[];
+  const int tid = threadIdx.x, b = blockIdx.z;
+  const RowDesc rd = p.rows[blockIdx.y];
+  const int N = 1 << p.g.logN, T = 1 << p.g.lt_row;
+  TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, blockIdx.x};
+  const u64 *src = p.src + (size_t)b * p.src_bstride + (size_t)(p.src_is_dst_row ? rd.dst_row : rd.src_row) * N;
+  for (int e = tid; e < T; e += blockDim.x) sm[swz(e)] = src[G.gidx(e)];
+  __syncthreads();
+  const u64 q = p.mods[rd.mod].q;
+  tile_transform<true>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid);
+  u64 *dst = p.dst + (size_t)b * p.dst_bstride + (size_t)rd.dst_row * N;
+  for (int e = tid; e < T; e += blockDim.x) dst[G.gidx(e)] = csub(csub(sm[swz(e)], q + q), q);
+}
+
+int k_ntt(const KCtx &k, const u64 *src, size_t src_bstride, u64 *dst, size_t dst_bstride, const RowDesc *rows, int n_rows,
+          int n_batch) {
+  if (n_rows == 0 || n_batch == 0) return 0;
+  cudaStream_t st = (cudaStream_t)k.stream;
+  const NttGeom &g = k.geom;
+  NttColP a{src, src_bstride, nullptr, dst, dst_bstride, rows, k.d_mods, k.d_tw_fwd, g};
+  dim3 grid1(k.N >> g.lt_col, n_rows, n_batch);
+  ntt_colpass_kernel<false><<<grid1, nthreads_for(g.lt_col), sizeof(u64) << g.lt_col, st>>>(a);
+  LAUNCH_CHECK(k);
+  NttRowP r{dst, dst_bstride, dst, dst_bstride, rows, k.d_mods, k.d_tw_fwd, g, 1};
+  dim3 grid2(k.N >> g.lt_row, n_rows, n_batch);
+  ntt_rowpass_kernel<<<grid2, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(r);
+  LAUNCH_CHECK(k);
+  return 0;
+}
+
+int k_ntt_cols_bconv(const KCtx &k, const u64 *y, size_t y_bstride, const u64 *bc, u64 *tmp, size_t tmp_bstride,
+                     const RowDesc *rows, int n_rows, int n_batch) {
+  if (n_rows == 0 || n_batch == 0) return 0;
+  const NttGeom &g = k.geom;
+  NttColP a{y, y_bstride, bc, tmp, tmp_bstride, rows, k.d_mods, k.d_tw_fwd, g};
+  dim3 grid1(k.N >> g.lt_col, n_rows, n_batch);
+  ntt_colpass_kernel<true><<<grid1, nthreads_for(g.lt_col), sizeof(u64) << g.lt_col, (cudaStream_t)k.stream>>>(a);
+  LAUNCH_CHECK(k);
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------------ forward pass 2 + evk inner product (a4)
+// One block = one tile of one target row t for one batch item; it loops over the beta digits, finishing the NTT of
+// ModUp_j(d)[t] in shared memory and accumulating x * evk_j.{b,a}[t] in 128-bit registers: the extended digits never
+// exist in NTT form in HBM, and each evk element is read exactly once per batch item (blocks of one tile that differ
+// only in the batch index are adjacent in launch order, so the key tile is served from L2 after its first read).
+struct KeyMacP {
+  const BatchItem *items; const int *tmp_index; const u64 *tmp; size_t tmp_bstride; u64 *acc; size_t acc_bstride;
+  const ModConst *mods; const ShoupC *tw; NttGeom g; int L, E, beta, A, nq, n_batch;
+};
+template <int EPT>  // elements per thread
+__global__ void __launch_bounds__(256) ntt_rows_keymac_kernel(KeyMacP p) {
+  extern __shared__ u64 sm[];
+  const int tid = threadIdx.x;
+  // batch index fastest: blockIdx.x = tile * n_batch + b
+  const int nb = p.n_batch, b = blockIdx.x % nb, tile = blockIdx.x / nb, t = blockIdx.y;
+  const int N = 1 << p.g.logN, T = 1 << p.g.lt_row;
+  TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, (u32)tile};
+  const int mod = t < p.L ? t : p.nq + (t - p.L);
+  const ModConst mc = p.mods[mod];
+  const BatchItem it = p.items[b];
+  u64 a0l[EPT], a0h[EPT], a1l[EPT], a1h[EPT];
+#pragma unroll
+  for (int i = 0; i < EPT; i++) a0l[i] = a0h[i] = a1l[i] = a1h[i] = 0;
+  const int nth = blockDim.x;
+  for (int j = 0; j < p.beta; j++) {
+    const int ti = p.tmp_index[j * p.E + t];
+    const u64 *kb = it.evk + ((size_t)(j * 2 + 0) * p.A + mod) * N;
+    const u64 *ka = it.evk + ((size_t)(j * 2 + 1) * p.A + mod) * N;
+    if (ti >= 0) {
+      const u64 *src = p.tmp + (size_t)b * p.tmp_bstride + (size_t)ti * N;
+      for (int e = tid; e < T; e += nth) sm[swz(e)] = src[G.gidx(e)];
+      __syncthreads();
+      tile_transform<true>(sm, G, 0, p.g.brow, p.tw + (size_t)mod * N, mc.q, tid);
+    }
+#pragma unroll
+    for (int i = 0; i < EPT; i++) {
+      const int e = tid + i * nth;
+      if (e < T) {
+        const u32 jj = G.gidx(e);
+        u64 x;
+        if (ti >= 0) x = csub(csub(sm[swz(e)], mc.q + mc.q), mc.q);
+        else x = __ldg(it.ks_in + (size_t)t * N + galois_src(jj, it.g, p.g.logN));
+        mac128(a0l[i], a0h[i], x, __ldg(kb + jj));
+        mac128(a1l[i], a1h[i], x, __ldg(ka + jj));
+      }
+    }
+    __syncthreads();
+  }
+  u64 *o0 = p.acc + (size_t)b * p.acc_bstride + (size_t)t * N;
+  u64 *o1 = o0 + (size_t)p.E * N;
+#pragma unroll
+  for (int i = 0; i < EPT; i++) {
+    const int e = tid + i * nth;
+    if (e < T) {
+      const u32 jj = G.gidx(e);
+      o0[jj] = mont_redc(a0l[i], a0h[i], mc.q, mc.qinv_neg);
+      o1[jj] = mont_redc(a1l[i], a1h[i], mc.q, mc.qinv_neg);
+    }
+  }
+}
+
+int k_ntt_rows_keymac(const KCtx &k, const BatchItem *items, int L, int E, int beta, const int *tmp_index, const u64 *tmp,
+                      size_t tmp_bstride, u64 *acc, size_t acc_bstride, int n_batch) {
+  if (n_batch == 0) return 0;
+  const NttGeom &g = k.geom;
+  KeyMacP p{items, tmp_index, tmp, tmp_bstride, acc, acc_bstride, k.d_mods, k.d_tw_fwd, g, L, E, beta, k.nq + k.np, k.nq,
+            n_batch};
+  const int nth = nthreads_for(g.lt_row);
+  dim3 grid((k.N >> g.lt_row) * n_batch, E, 1);
+  const int ept = ((1 << g.lt_row) + nth - 1) / nth;
+  if (ept <= 1) ntt_rows_keymac_kernel<1><<<grid, nth, sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
+  else if (ept <= 4) ntt_rows_keymac_kernel<4><<<grid, nth, sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
+  else ntt_rows_keymac_kernel<8><<<grid, nth, sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
+  LAUNCH_CHECK(k);
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------------ forward pass 2 + divide epilogue (a5, a8)
+// X = NTT(Conv_{dropped -> t}(.)) finished here; out = (minuend - X) * mul[t] (+ addend through the Galois gather).
+struct DivideP {
+  const BatchItem *items; const u64 *tmp; size_t tmp_bstride; const u64 *acc; size_t acc_bstride; const ShoupC *mul;
+  const RowDesc *rows; const ModConst *mods; const ShoupC *tw; NttGeom g; int from_items;
+};
+__global__ void __launch_bounds__(256) ntt_rows_divide_kernel(DivideP p) {
+  extern __shared__ u64 sm[];
+  const int tid = threadIdx.x, b = blockIdx.z;
+  const RowDesc rd = p.rows[blockIdx.y];
+  const int N = 1 << p.g.logN, T = 1 << p.g.lt_row;
+  TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, blockIdx.x};
+  const u64 *src = p.tmp + (size_t)b * p.tmp_bstride + (size_t)rd.src_row * N;
+  for (int e = tid; e < T; e += blockDim.x) sm[swz(e)] = src[G.gidx(e)];
+  __syncthreads();
+  const u64 q = p.mods[rd.mod].q;
+  tile_transform<true>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid);
+  const BatchItem it = p.items[b];
+  const u64 *minuend = (p.from_items ? it.sub_in : p.acc + (size_t)b * p.acc_bstride) + (size_t)rd.aux2 * N;
+  const u64 *addend = rd.aux == 0 ? it.add0 : it.add1;
+  if (addend) addend += (size_t)rd.mod * N;
+  const ShoupC mc = p.mul[rd.mod];
+  u64 *dst = it.out + (size_t)rd.dst_row * N;
+  for (int e = tid; e < T; e += blockDim.x) {
+    const u32 j = G.gidx(e);
+    const u64 x = csub(csub(sm[swz(e)], q + q), q);
+    u64 v = shoup_mul(submod(__ldg(minuend + j), x, q), mc.c, mc.cs, q);
+    if (addend) v = addmod(v, __ldg(addend + galois_src(j, it.g, p.g.logN)), q);
+    dst[j] = v;
+  }
+}
+
+int k_ntt_rows_divide(const KCtx &k, const BatchItem *items, const u64 *tmp, size_t tmp_bstride, const u64 *acc,
+                      size_t acc_bstride, bool minuend_from_items, const ShoupC *mul, const RowDesc *rows, int n_rows,
+                      int n_batch) {
+  if (n_rows == 0 || n_batch == 0) return 0;
+  const NttGeom &g = k.geom;
+  DivideP p{items, tmp, tmp_bstride, acc, acc_bstride, mul, rows, k.d_mods, k.d_tw_fwd, g, minuend_from_items ? 1 : 0};
+  dim3 grid(k.N >> g.lt_row, n_rows, n_batch);
+  ntt_rows_divide_kernel<<<grid, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
+  LAUNCH_CHECK(k);
+  return 0;
+}

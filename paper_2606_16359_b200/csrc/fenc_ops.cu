@@ -1,0 +1,392 @@
+// fenc_ops.cu -- keys, plaintexts, encryption / decryption and the ciphertext primitives of the C ABI.
+#include <cmath>
+#include <cstring>
+
+#include "fenc_ctx.h"
+
+enum { PURPOSE_SECRET = 1, PURPOSE_EVK_A = 2, PURPOSE_EVK_E = 3, PURPOSE_ENC_A = 4, PURPOSE_ENC_E = 5 };
+
+static bool scale_close(double a, double b) { return std::fabs(a - b) <= 1e-9 * std::fabs(b); }
+
+// centred integer coefficients (host) -> [L][N] NTT domain, Montgomery form
+fenc_status coeffs_to_mont(fenc_ctx *ctx, const int64_t *coeffs, int L, u64 *d_out) {
+  const size_t N = ctx->N;
+  i64 *d_c = dalloc_t<i64>(ctx, N);
+  if (!d_c) return fail(ctx, FENC_ERR_OOM, "coefficient staging");
+  CUDA_OK(ctx, cudaMemcpyAsync(d_c, coeffs, N * 8, cudaMemcpyHostToDevice, ctx->stream));
+  CUDA_OK(ctx, k_reduce_signed(ctx->k, d_c, ctx->d_ident_mod, d_out, L));
+  CUDA_OK(ctx, k_ntt(ctx->k, d_out, 0, d_out, 0, ctx->d_ident_rows, L, 1));
+  CUDA_OK(ctx, k_mont_convert(ctx->k, d_out, d_out, ctx->d_ident_mod, L, true));
+  dfree(ctx, d_c);
+  return FENC_OK;
+}
+fenc_status pt_device(fenc_ctx *ctx, fenc_pt *pt) {
+  if (pt->d_mont) return FENC_OK;
+  pt->d_mont = dalloc_t<u64>(ctx, (size_t)pt->L * ctx->N);
+  if (!pt->d_mont) return fail(ctx, FENC_ERR_OOM, "plaintext");
+  return coeffs_to_mont(ctx, pt->coeffs.data(), pt->L, pt->d_mont);
+}
+
+// ------------------------------------------------------------------------------------------------ keys (R2.4)
+// For every digit j over ALL nq+np limbs t: a_j[t] uniform, b_j[t] = -a_j[t] s + e_j + f_{j,t} s' (mod t),
+// f_{j,t} = P mod t if t in D_j else 0.  Stored in NTT domain, Montgomery form: [beta_max][{b,a}][A][N].
+static fenc_status make_switch_key(fenc_ctx *ctx, fenc_keys *K, int64_t key_id, const u64 *d_sp_mont, u32 g, u64 **out) {
+  const int A = ctx->A, N = ctx->N, nq = ctx->nq;
+  const size_t AN = (size_t)A * N;
+  u64 *evk = dalloc_t<u64>(ctx, (size_t)ctx->beta_max * 2 * AN);
+  u64 *d_a = dalloc_t<u64>(ctx, AN), *d_e = dalloc_t<u64>(ctx, AN);
+  u64 *d_keys = dalloc_t<u64>(ctx, A), *d_f = dalloc_t<u64>(ctx, A);
+  if (!evk || !d_a || !d_e || !d_keys || !d_f) return fail(ctx, FENC_ERR_OOM, "evaluation key");
+  u64 Pmod[FENC_MAX_MOD];
+  for (int t = 0; t < A; t++) {
+    u64 m = ctx->mod[t], x = 1;
+    for (int i = 0; i < ctx->np; i++) x = fh::mulmod(x, ctx->mod[nq + i] % m, m);
+    Pmod[t] = x;
+  }
+  for (int j = 0; j < ctx->beta_max; j++) {
+    std::vector<u64> hk(A), hf(A, 0);
+    for (int t = 0; t < A; t++) hk[t] = fh::stream_key(K->seed, PURPOSE_EVK_A, (u64)key_id, (u64)j, (u64)t);
+    for (int t = j * ctx->dlen; t < std::min((j + 1) * ctx->dlen, nq); t++) hf[t] = Pmod[t];
+    CUDA_OK(ctx, cudaMemcpyAsync(d_keys, hk.data(), A * 8, cudaMemcpyHostToDevice, ctx->stream));
+    CUDA_OK(ctx, cudaMemcpyAsync(d_f, hf.data(), A * 8, cudaMemcpyHostToDevice, ctx->stream));
+    CUDA_OK(ctx, k_sample_uniform(ctx->k, d_keys, ctx->d_ident_mod, d_a, A));
+    CUDA_OK(ctx, k_sample_gauss(ctx->k, fh::stream_key(K->seed, PURPOSE_EVK_E, (u64)key_id, (u64)j, 0), nullptr, ctx->d_ident_mod, d_e, A));
+    CUDA_OK(ctx, k_ntt(ctx->k, d_a, 0, d_a, 0, ctx->d_ident_rows, A, 1));
+    CUDA_OK(ctx, k_ntt(ctx->k, d_e, 0, d_e, 0, ctx->d_ident_rows, A, 1));
+    u64 *kb = evk + (size_t)(j * 2 + 0) * AN, *ka = evk + (size_t)(j * 2 + 1) * AN;
+    CUDA_OK(ctx, k_x_minus_as(ctx->k, d_a, d_e, K->d_s_mont, kb, ctx->d_ident_mod, A));
+    CUDA_OK(ctx, k_add_f_sprime(ctx->k, kb, d_sp_mont, g, d_f, kb, ctx->d_ident_mod, A));
+    CUDA_OK(ctx, k_mont_convert(ctx->k, kb, kb, ctx->d_ident_mod, A, true));
+    CUDA_OK(ctx, k_mont_convert(ctx->k, d_a, ka, ctx->d_ident_mod, A, true));
+    CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));  // hk / hf go out of scope
+  }
+  dfree(ctx, d_a), dfree(ctx, d_e), dfree(ctx, d_keys), dfree(ctx, d_f);
+  *out = evk;
+  return FENC_OK;
+}
+
+extern "C" fenc_status fenc_keygen(fenc_ctx *ctx, uint64_t seed, const int32_t *rot_steps, size_t n_rot, int want_relin,
+                                   fenc_keys **out) {
+  if (!ctx || !out || (n_rot && !rot_steps)) return FENC_ERR_INVALID_ARG;
+  std::unique_ptr<fenc_keys> K(new fenc_keys{ctx, seed, {}, nullptr, {}});
+  const int A = ctx->A, N = ctx->N;
+  K->s.resize(N);
+  fh::sample_ternary(fh::stream_key(seed, PURPOSE_SECRET, 0, 0, 0), N, K->s.data());
+  K->d_s_mont = dalloc_t<u64>(ctx, (size_t)A * N);
+  i64 *d_c = dalloc_t<i64>(ctx, N);
+  if (!K->d_s_mont || !d_c) return fail(ctx, FENC_ERR_OOM, "secret key");
+  CUDA_OK(ctx, cudaMemcpyAsync(d_c, K->s.data(), (size_t)N * 8, cudaMemcpyHostToDevice, ctx->stream));
+  CUDA_OK(ctx, k_reduce_signed(ctx->k, d_c, ctx->d_ident_mod, K->d_s_mont, A));
+  CUDA_OK(ctx, k_ntt(ctx->k, K->d_s_mont, 0, K->d_s_mont, 0, ctx->d_ident_rows, A, 1));
+  CUDA_OK(ctx, k_mont_convert(ctx->k, K->d_s_mont, K->d_s_mont, ctx->d_ident_mod, A, true));
+  CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+  dfree(ctx, d_c);
+  for (size_t i = 0; i < n_rot; i++) {
+    int r = ((rot_steps[i] % ctx->n) + ctx->n) % ctx->n;
+    if (r == 0 || K->evk.count(r)) continue;
+    u64 *evk = nullptr;
+    // s' = sigma_g(s): in the NTT domain the automorphism is the index gather (done inside k_add_f_sprime)
+    fenc_status st = make_switch_key(ctx, K.get(), r, K->d_s_mont, galois_elt(ctx, r), &evk);
+    if (st != FENC_OK) return st;
+    K->evk[r] = evk;
+  }
+  if (want_relin) {
+    // s' = s * s: from Montgomery form, mont_mul(s 2^64, s 2^64) = s^2 2^64 directly
+    u64 *d_s2 = dalloc_t<u64>(ctx, (size_t)A * N), *d_sn = dalloc_t<u64>(ctx, (size_t)A * N);
+    if (!d_s2 || !d_sn) return fail(ctx, FENC_ERR_OOM, "relinearisation key");
+    CUDA_OK(ctx, k_mont_convert(ctx->k, K->d_s_mont, d_sn, ctx->d_ident_mod, A, false));
+    CUDA_OK(ctx, k_mul_rows(ctx->k, d_sn, d_sn, d_s2, ctx->d_ident_mod, A));
+    CUDA_OK(ctx, k_mont_convert(ctx->k, d_s2, d_s2, ctx->d_ident_mod, A, true));
+    u64 *evk = nullptr;
+    fenc_status st = make_switch_key(ctx, K.get(), FENC_RELIN_KEY_ID, d_s2, 1, &evk);
+    dfree(ctx, d_s2), dfree(ctx, d_sn);
+    if (st != FENC_OK) return st;
+    K->evk[FENC_RELIN_KEY_ID] = evk;
+  }
+  *out = K.release();
+  return FENC_OK;
+}
+extern "C" void fenc_keys_free(fenc_keys *K) {
+  if (!K) return;
+  cudaStreamSynchronize(K->ctx->stream);
+  dfree(K->ctx, K->d_s_mont);
+  for (auto &kv : K->evk) dfree(K->ctx, kv.second);
+  delete K;
+}
+extern "C" fenc_status fenc_secret_export(fenc_ctx *ctx, const fenc_keys *K, int64_t *s) {
+  if (!ctx || !K || !s) return FENC_ERR_INVALID_ARG;
+  memcpy(s, K->s.data(), K->s.size() * 8);
+  return FENC_OK;
+}
+extern "C" fenc_status fenc_evk_export(fenc_ctx *ctx, const fenc_keys *K, int64_t key_id, uint64_t *b, uint64_t *a) {
+  if (!ctx || !K || !b || !a) return FENC_ERR_INVALID_ARG;
+  auto it = K->evk.find(key_id);
+  if (it == K->evk.end()) return fail(ctx, FENC_ERR_NO_KEY, "no key %lld", (long long)key_id);
+  const int A = ctx->A, N = ctx->N;
+  const size_t AN = (size_t)A * N;
+  u64 *tmp = dalloc_t<u64>(ctx, AN);
+  if (!tmp) return fail(ctx, FENC_ERR_OOM, "export staging");
+  for (int j = 0; j < ctx->beta_max; j++)
+    for (int c = 0; c < 2; c++) {
+      CUDA_OK(ctx, k_mont_convert(ctx->k, it->second + (size_t)(j * 2 + c) * AN, tmp, ctx->d_ident_mod, A, false));
+      CUDA_OK(ctx, k_intt(ctx->k, nullptr, tmp, 0, false, tmp, 0, ctx->d_ident_rows, A, ctx->d_ninv, 1));
+      CUDA_OK(ctx, cudaMemcpyAsync((c == 0 ? b : a) + (size_t)j * AN, tmp, AN * 8, cudaMemcpyDeviceToHost, ctx->stream));
+    }
+  CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+  dfree(ctx, tmp);
+  return FENC_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ plaintexts
+extern "C" fenc_status fenc_pt_from_coeffs(fenc_ctx *ctx, const int64_t *coeffs, uint32_t n_limbs, double scale, fenc_pt **out) {
+  if (!ctx || !coeffs || !out || n_limbs < 1 || (int)n_limbs > ctx->nq) return FENC_ERR_INVALID_ARG;
+  fenc_pt *pt = new fenc_pt{ctx, (int)n_limbs, scale > 0 ? scale : ctx->default_scale, {}, nullptr};
+  pt->coeffs.assign(coeffs, coeffs + ctx->N);
+  *out = pt;
+  return FENC_OK;
+}
+extern "C" fenc_status fenc_encode_slots(fenc_ctx *ctx, const double *re, const double *im, uint32_t n_limbs, double scale,
+                                         fenc_pt **out) {
+  if (!ctx || !re || !out || n_limbs < 1 || (int)n_limbs > ctx->nq) return FENC_ERR_INVALID_ARG;
+  fenc_pt *pt = new fenc_pt{ctx, (int)n_limbs, scale > 0 ? scale : ctx->default_scale, {}, nullptr};
+  pt->coeffs.resize(ctx->N);
+  fh::encode_slots(ctx->logN, re, im, pt->scale, pt->coeffs.data());
+  *out = pt;
+  return FENC_OK;
+}
+extern "C" fenc_status fenc_pt_coeffs(fenc_ctx *ctx, const fenc_pt *pt, int64_t *coeffs) {
+  if (!ctx || !pt || !coeffs) return FENC_ERR_INVALID_ARG;
+  memcpy(coeffs, pt->coeffs.data(), pt->coeffs.size() * 8);
+  return FENC_OK;
+}
+extern "C" void fenc_pt_free(fenc_pt *pt) {
+  if (!pt) return;
+  if (pt->d_mont) {
+    cudaStreamSynchronize(pt->ctx->stream);
+    dfree(pt->ctx, pt->d_mont);
+  }
+  delete pt;
+}
+
+// ------------------------------------------------------------------------------------------------ encrypt / decrypt (R2.5)
+extern "C" fenc_status fenc_encrypt(fenc_ctx *ctx, const fenc_keys *K, const fenc_pt *pt, uint64_t enc_seed, fenc_ct **out) {
+  if (!ctx || !K || !pt || !out) return FENC_ERR_INVALID_ARG;
+  const int L = pt->L, N = ctx->N;
+  fenc_ct *ct = new_ct(ctx, L, pt->scale);
+  i64 *d_m = dalloc_t<i64>(ctx, N);
+  u64 *d_x = dalloc_t<u64>(ctx, (size_t)L * N), *d_keys = dalloc_t<u64>(ctx, L);
+  if (!ct || !d_m || !d_x || !d_keys) return fail(ctx, FENC_ERR_OOM, "encrypt");
+  std::vector<u64> hk(L);
+  for (int t = 0; t < L; t++) hk[t] = fh::stream_key(enc_seed, PURPOSE_ENC_A, (u64)t, 0, 0);
+  CUDA_OK(ctx, cudaMemcpyAsync(d_m, pt->coeffs.data(), (size_t)N * 8, cudaMemcpyHostToDevice, ctx->stream));
+  CUDA_OK(ctx, cudaMemcpyAsync(d_keys, hk.data(), (size_t)L * 8, cudaMemcpyHostToDevice, ctx->stream));
+  u64 *c0 = ct->d, *c1 = ct->d + (size_t)L * N;
+  CUDA_OK(ctx, k_sample_gauss(ctx->k, fh::stream_key(enc_seed, PURPOSE_ENC_E, 0, 0, 0), d_m, ctx->d_ident_mod, d_x, L));  // e + m
+  CUDA_OK(ctx, k_sample_uniform(ctx->k, d_keys, ctx->d_ident_mod, c1, L));                                                // a
+  CUDA_OK(ctx, k_ntt(ctx->k, d_x, 0, d_x, 0, ctx->d_ident_rows, L, 1));
+  CUDA_OK(ctx, k_ntt(ctx->k, c1, 0, c1, 0, ctx->d_ident_rows, L, 1));
+  CUDA_OK(ctx, k_x_minus_as(ctx->k, c1, d_x, K->d_s_mont, c0, ctx->d_ident_mod, L));  // c0 = (e + m) - a s
+  CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+  dfree(ctx, d_m), dfree(ctx, d_x), dfree(ctx, d_keys);
+  *out = ct;
+  return FENC_OK;
+}
+
+extern "C" fenc_status fenc_decrypt_slots(fenc_ctx *ctx, const fenc_keys *K, const fenc_ct *ct, double *re, double *im) {
+  if (!ctx || !K || !ct || !re) return FENC_ERR_INVALID_ARG;
+  const int L = ct->L, N = ctx->N;
+  u64 *d_mu = dalloc_t<u64>(ctx, (size_t)L * N);
+  if (!d_mu) return fail(ctx, FENC_ERR_OOM, "decrypt");
+  CUDA_OK(ctx, k_dec_combine(ctx->k, ct->d, K->d_s_mont, d_mu, L));
+  CUDA_OK(ctx, k_intt(ctx->k, nullptr, d_mu, 0, false, d_mu, 0, ctx->d_ident_rows, L, ctx->d_ninv, 1));
+  std::vector<u64> mu((size_t)L * N);
+  CUDA_OK(ctx, cudaMemcpyAsync(mu.data(), d_mu, mu.size() * 8, cudaMemcpyDeviceToHost, ctx->stream));
+  CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+  dfree(ctx, d_mu);
+  std::vector<long double> m(N);
+  fh::crt_centre_scaled(ctx->mod.data(), L, N, mu.data(), (long double)ct->scale, m.data());
+  fh::decode_coeffs(ctx->logN, m.data(), re, im);
+  return FENC_OK;
+}
+
+extern "C" fenc_status fenc_ct_export(fenc_ctx *ctx, const fenc_ct *ct, uint64_t *limbs) {
+  if (!ctx || !ct || !limbs) return FENC_ERR_INVALID_ARG;
+  LevelPlan *P = get_plan(ctx, ct->L);
+  const size_t n = (size_t)2 * ct->L * ctx->N;
+  u64 *tmp = dalloc_t<u64>(ctx, n);
+  if (!P || !tmp) return fail(ctx, FENC_ERR_OOM, "export");
+  CUDA_OK(ctx, k_intt(ctx->k, nullptr, ct->d, 0, false, tmp, 0, P->d_rows_ct, 2 * ct->L, P->d_scale_ct, 1));
+  CUDA_OK(ctx, cudaMemcpyAsync(limbs, tmp, n * 8, cudaMemcpyDeviceToHost, ctx->stream));
+  CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+  dfree(ctx, tmp);
+  return FENC_OK;
+}
+extern "C" fenc_status fenc_ct_import(fenc_ctx *ctx, const uint64_t *limbs, uint32_t L, double scale, fenc_ct **out) {
+  if (!ctx || !limbs || !out || L < 1 || (int)L > ctx->nq) return FENC_ERR_INVALID_ARG;
+  LevelPlan *P = get_plan(ctx, (int)L);
+  fenc_ct *ct = new_ct(ctx, (int)L, scale > 0 ? scale : ctx->default_scale);
+  if (!P || !ct) return fail(ctx, FENC_ERR_OOM, "import");
+  const size_t n = (size_t)2 * L * ctx->N;
+  CUDA_OK(ctx, cudaMemcpyAsync(ct->d, limbs, n * 8, cudaMemcpyHostToDevice, ctx->stream));
+  CUDA_OK(ctx, k_ntt(ctx->k, ct->d, 0, ct->d, 0, P->d_rows_ct, 2 * (int)L, 1));
+  CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+  *out = ct;
+  return FENC_OK;
+}
+extern "C" fenc_status fenc_ct_info(fenc_ctx *ctx, const fenc_ct *ct, uint32_t *L, double *scale, void **device_ptr) {
+  if (!ctx || !ct) return FENC_ERR_INVALID_ARG;
+  if (L) *L = ct->L;
+  if (scale) *scale = ct->scale;
+  if (device_ptr) *device_ptr = ct->d;
+  return FENC_OK;
+}
+extern "C" void fenc_ct_free(fenc_ct *ct) {
+  if (!ct) return;
+  dfree(ct->ctx, ct->d);
+  delete ct;
+}
+
+// ------------------------------------------------------------------------------------------------ primitives
+extern "C" fenc_status fenc_rotate(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const *in, const int32_t *steps, size_t n,
+                                   fenc_ct **out) {
+  if (!ctx || !K || !in || !steps || !out) return FENC_ERR_INVALID_ARG;
+  if (n == 0) return FENC_OK;
+  const int L = in[0]->L;
+  std::vector<const u64 *> vin(n);
+  std::vector<u64 *> vout(n);
+  std::vector<int> vs(steps, steps + n);
+  std::vector<fenc_ct *> made(n, nullptr);
+  for (size_t i = 0; i < n; i++) {
+    if (in[i]->L != L) return fail(ctx, FENC_ERR_MISMATCH, "rotate: inputs differ in level");
+    made[i] = new_ct(ctx, L, in[i]->scale);
+    if (!made[i]) {
+      for (auto *c : made) fenc_ct_free(c);
+      return fail(ctx, FENC_ERR_OOM, "rotate output");
+    }
+    vin[i] = in[i]->d, vout[i] = made[i]->d;
+  }
+  fenc_status st = rotate_raw(ctx, K, L, vin, vs, vout);
+  if (st != FENC_OK) {
+    for (auto *c : made) fenc_ct_free(c);
+    return st;
+  }
+  for (size_t i = 0; i < n; i++) out[i] = made[i];
+  return FENC_OK;
+}
+
+extern "C" fenc_status fenc_rescale(fenc_ctx *ctx, fenc_ct *const *in, size_t n, fenc_ct **out) {
+  if (!ctx || !in || !out) return FENC_ERR_INVALID_ARG;
+  if (n == 0) return FENC_OK;
+  const int L = in[0]->L;
+  if (L < 2) return fail(ctx, FENC_ERR_LEVEL, "rescale at the last level");
+  std::vector<BatchItem> items(n);
+  std::vector<fenc_ct *> made(n, nullptr);
+  for (size_t i = 0; i < n; i++) {
+    if (in[i]->L != L) return fail(ctx, FENC_ERR_MISMATCH, "rescale: inputs differ in level");
+    made[i] = new_ct(ctx, L - 1, in[i]->scale / (double)ctx->mod[L - 1]);
+    if (!made[i]) return fail(ctx, FENC_ERR_OOM, "rescale output");
+    items[i] = BatchItem{};
+    items[i].sub_in = in[i]->d, items[i].out = made[i]->d;
+  }
+  fenc_status st = rescale_batch(ctx, L, items);
+  if (st != FENC_OK) return st;
+  for (size_t i = 0; i < n; i++) out[i] = made[i];
+  return FENC_OK;
+}
+
+extern "C" fenc_status fenc_add(fenc_ctx *ctx, const fenc_ct *a, const fenc_ct *b, fenc_ct **out) {
+  if (!ctx || !a || !b || !out) return FENC_ERR_INVALID_ARG;
+  if (a->L != b->L || !scale_close(a->scale, b->scale)) return fail(ctx, FENC_ERR_MISMATCH, "add: level or scale differ");
+  fenc_ct *c = new_ct(ctx, a->L, a->scale);
+  if (!c) return fail(ctx, FENC_ERR_OOM, "add");
+  std::vector<const u64 *> terms{a->d, b->d};
+  std::vector<int> start{0, 2};
+  std::vector<u64 *> outs{c->d};
+  DescStage st(ctx);
+  size_t o1 = st.add(terms), o2 = st.add(start), o3 = st.add(outs);
+  char *base = st.commit();
+  if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
+  CUDA_OK(ctx, k_add_many(ctx->k, (const u64 *const *)(base + o1), (const int *)(base + o2), (u64 *const *)(base + o3), 1, a->L));
+  *out = c;
+  return FENC_OK;
+}
+
+extern "C" fenc_status fenc_pmult_sum(fenc_ctx *ctx, fenc_ct *const *in, fenc_pt *const *pt, size_t n, fenc_ct **out) {
+  if (!ctx || !in || !pt || !out || n == 0) return FENC_ERR_INVALID_ARG;
+  const int L = in[0]->L;
+  std::vector<const u64 *> tc(n), tp(n);
+  for (size_t i = 0; i < n; i++) {
+    if (in[i]->L != L || pt[i]->L != L) return fail(ctx, FENC_ERR_MISMATCH, "pmult: level differs");
+    if (!scale_close(in[i]->scale * pt[i]->scale, in[0]->scale * pt[0]->scale)) return fail(ctx, FENC_ERR_MISMATCH, "pmult: scales differ");
+    fenc_status s = pt_device(ctx, pt[i]);
+    if (s != FENC_OK) return s;
+    tc[i] = in[i]->d, tp[i] = pt[i]->d_mont;
+  }
+  fenc_ct *c = new_ct(ctx, L, in[0]->scale * pt[0]->scale);
+  if (!c) return fail(ctx, FENC_ERR_OOM, "pmult");
+  std::vector<int> start{0, (int)n};
+  std::vector<u64 *> outs{c->d};
+  DescStage st(ctx);
+  size_t o0 = st.add(tc), o1 = st.add(tp), o2 = st.add(start), o3 = st.add(outs);
+  char *base = st.commit();
+  if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
+  CUDA_OK(ctx, k_mac(ctx->k, (const u64 *const *)(base + o0), (const u64 *const *)(base + o1), (const int *)(base + o2),
+                     (u64 *const *)(base + o3), 1, L, ctx->max_lazy));
+  *out = c;
+  return FENC_OK;
+}
+
+// x -> x^2 (R2.12): d0 = c0 c0, d1 = 2 c0 c1, d2 = c1 c1; (d0, d1) + KS(d2; relin); rescale
+extern "C" fenc_status fenc_square_relin(fenc_ctx *ctx, const fenc_keys *K, const fenc_ct *in, fenc_ct **out) {
+  if (!ctx || !K || !in || !out) return FENC_ERR_INVALID_ARG;
+  auto it = K->evk.find(FENC_RELIN_KEY_ID);
+  if (it == K->evk.end()) return fail(ctx, FENC_ERR_NO_KEY, "no relinearisation key");
+  const int L = in->L;
+  if (L < 2) return fail(ctx, FENC_ERR_LEVEL, "square needs a level to rescale into");
+  const size_t LN = (size_t)L * ctx->N;
+  u64 *d = dalloc_t<u64>(ctx, 3 * LN), *mid = dalloc_t<u64>(ctx, 2 * LN);
+  if (!d || !mid) return fail(ctx, FENC_ERR_OOM, "square");
+  const u64 *c0 = in->d, *c1 = in->d + LN;
+  CUDA_OK(ctx, k_mul_rows(ctx->k, c0, c0, d, ctx->d_ident_mod, L));
+  CUDA_OK(ctx, k_mul_rows(ctx->k, c0, c1, d + LN, ctx->d_ident_mod, L));
+  CUDA_OK(ctx, k_add_rows(ctx->k, d + LN, d + LN, d + LN, ctx->d_ident_mod, L, false));
+  CUDA_OK(ctx, k_mul_rows(ctx->k, c1, c1, d + 2 * LN, ctx->d_ident_mod, L));
+  std::vector<BatchItem> items(1);
+  items[0] = BatchItem{};
+  items[0].ks_in = d + 2 * LN, items[0].out = mid, items[0].evk = it->second, items[0].add0 = d, items[0].add1 = d + LN, items[0].g = 1;
+  fenc_status st = ks_batch(ctx, L, items);
+  if (st != FENC_OK) return st;
+  fenc_ct *c = new_ct(ctx, L - 1, in->scale * in->scale / (double)ctx->mod[L - 1]);
+  if (!c) return fail(ctx, FENC_ERR_OOM, "square output");
+  std::vector<BatchItem> rs(1);
+  rs[0] = BatchItem{};
+  rs[0].sub_in = mid, rs[0].out = c->d;
+  st = rescale_batch(ctx, L, rs);
+  if (st != FENC_OK) return st;
+  CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+  dfree(ctx, d), dfree(ctx, mid);
+  *out = c;
+  return FENC_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ raw NTT (a1)
+extern "C" fenc_status fenc_ntt_rows(fenc_ctx *ctx, void *device_rows, const int32_t *mod_idx, size_t n_rows, int inverse) {
+  if (!ctx || !device_rows || !mod_idx) return FENC_ERR_INVALID_ARG;
+  std::vector<RowDesc> rows(n_rows);
+  std::vector<ShoupC> sc(n_rows);
+  for (size_t r = 0; r < n_rows; r++) {
+    if (mod_idx[r] < 0 || mod_idx[r] >= ctx->A) return FENC_ERR_INVALID_ARG;
+    u64 m = ctx->mod[mod_idx[r]];
+    u64 ni = fh::invmod((u64)ctx->N % m, m);
+    rows[r] = RowDesc{mod_idx[r], (int)r, (int)r, 0, 0, {0, 0, 0}};
+    sc[r] = ShoupC{ni, fh::shoup(ni, m)};
+  }
+  DescStage st(ctx);
+  size_t o0 = st.add(rows), o1 = st.add(sc);
+  char *base = st.commit();
+  if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
+  u64 *p = (u64 *)device_rows;
+  if (inverse) CUDA_OK(ctx, k_intt(ctx->k, nullptr, p, 0, false, p, 0, (const RowDesc *)(base + o0), (int)n_rows, (const ShoupC *)(base + o1), 1));
+  else CUDA_OK(ctx, k_ntt(ctx->k, p, 0, p, 0, (const RowDesc *)(base + o0), (int)n_rows, 1));
+  return FENC_OK;
+}
