@@ -1,0 +1,255 @@
+"""GPU parity (-m gpu): libfenc's CUDA path, called through the C ABI, against the CPU oracle element by element on
+the same seeded inputs.  Bar: bit-exact on every RNS limb (integer work); decoded outputs within 1e-3 of plaintext
+fp64 convolution (BASELINE.json north_star).  Parity starts at integer plaintext coefficients (A7)."""
+import numpy as np
+import pytest
+
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def mods():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from oracle import ckks as ck
+    from oracle import fragment as fr
+    import paper_2606_16359_b200 as fenc
+    return ck, fr, fenc
+
+
+def make(mods, name, **over):
+    ck, fr, fenc = mods
+    p = dict(wl.PARAMS[name], **over)
+    P = ck.Params(*wl.oracle_params_args(p))
+    ctx = fenc.Context(**p)
+    assert ctx.q == P.q and ctx.p == P.p and ctx.dlen == P.dlen
+    return P, ctx
+
+
+@pytest.mark.parametrize("name", ["toy64", "mid10", "mid12"])
+def test_primitives_bit_exact(mods, name):
+    ck, fr, fenc = mods
+    P, ctx = make(mods, name)
+    N, L = P.N, P.nq
+    rng = np.random.default_rng(11)
+    limbs = wl.random_ct_limbs(3, P.q, L, N)
+    assert np.array_equal(ctx.ct_export(ctx.ct_import(limbs, 2.0 ** 20)), limbs)  # NTT round trip at full N
+    steps = [1, 2, 5, P.n - 1, P.n // 2]
+    ok = ck.keygen(P, 42, steps, want_relin=True)
+    gk = ctx.keygen(42, steps, want_relin=True)
+    assert np.array_equal(ctx.secret_export(gk), ok.s)
+    for kid in steps + [ck.RELIN_KEY_ID]:
+        b, a = ctx.evk_export(gk, kid)
+        assert np.array_equal(a, ok.evk[kid][1]) and np.array_equal(b, ok.evk[kid][0]), kid
+    z = rng.uniform(-1, 1, P.n)
+    opt = ck.encode(P, z, L)
+    oct_ = ck.encrypt(P, ok, opt, 7)
+    gct = ctx.encrypt(gk, ctx.pt_from_coeffs(opt.coeffs, L, float(opt.scale)), 7)
+    assert np.array_equal(ctx.ct_export(gct), oct_.c)
+    assert np.abs(ctx.decrypt_slots(gk, gct) - z).max() < 1e-4
+    # batched rotation, including step 0 and a repeated step
+    st = steps + [0, 1]
+    outs = ctx.rotate(gk, [gct] * len(st), st)
+    for r, o in zip(st, outs):
+        assert np.array_equal(ctx.ct_export(o), ck.rotate(P, ok, oct_, r).c), r
+    assert np.abs(ctx.decrypt_slots(gk, outs[1]) - np.roll(z, -2)).max() < 1e-4  # left shift (R2.7)
+    # PMult-accumulate of three terms, then rescale
+    ws = [ck.encode(P, rng.normal(0, 0.1, P.n), L, P.q[L - 1]) for _ in range(3)]
+    acc = np.zeros_like(oct_.c)
+    rots = [ck.rotate(P, ok, oct_, r) for r in (0, 1, 2)]
+    for x, w in zip(rots, ws):
+        ck.pmult_acc(P, acc, x, w)
+    gp = ctx.pmult_sum([outs[5], outs[0], outs[1]], [ctx.pt_from_coeffs(w.coeffs, L, float(w.scale)) for w in ws])
+    assert np.array_equal(ctx.ct_export(gp), acc)
+    ors = ck.rescale(P, ck.Ciphertext(acc, L, oct_.scale * ws[0].scale))
+    grs = ctx.rescale([gp])[0]
+    assert np.array_equal(ctx.ct_export(grs), ors.c) and grs.L == L - 1
+    assert abs(grs.scale - float(ors.scale)) <= 1e-9 * float(ors.scale)
+    # add, square + relinearise + rescale
+    assert np.array_equal(ctx.ct_export(ctx.add(gct, outs[0])), ck.add(P, oct_, rots[1]).c)
+    assert np.array_equal(ctx.ct_export(ctx.square_relin(gk, gct)), ck.square_relin(P, ok, oct_).c)
+    # rotation below the top level (short last digit: 5 limbs -> 3 limbs, dlen 2 -> digits 2,1)
+    o2 = ck.rescale(P, ors) if ors.L > 2 else ors
+    g2 = ctx.rescale([grs])[0] if ors.L > 2 else grs
+    assert np.array_equal(ctx.ct_export(ctx.rotate(gk, [g2], [5])[0]), ck.rotate(P, ok, o2, 5).c)
+    ctx.close()
+
+
+def test_errors_and_edges(mods):
+    ck, fr, fenc = mods
+    P, ctx = make(mods, "toy64")
+    gk = ctx.keygen(1, [1])
+    ct = ctx.encrypt(gk, ctx.encode_slots(np.zeros(P.n), 1), 3)
+    with pytest.raises(fenc.FencError, match="NO_KEY"):
+        ctx.rotate(gk, [ct], [2])
+    with pytest.raises(fenc.FencError, match="LEVEL"):
+        ctx.rescale([ct])
+    with pytest.raises(fenc.FencError, match="NO_KEY"):
+        ctx.square_relin(gk, ct)
+    assert ctx.rotate(gk, [], []) == []
+    with pytest.raises(fenc.FencError):
+        fenc.Context(log2N=6, n_q=4, q_bits=30, n_p=1, p_bits=31, dnum=1)  # P < Q_j without allow_noisy_ks
+    ctx.close()
+
+
+def test_library_encoder_close_to_oracle(mods):
+    ck, fr, fenc = mods
+    P, ctx = make(mods, "mid12")
+    rng = np.random.default_rng(5)
+    z = rng.uniform(-1, 1, P.n) + 1j * rng.uniform(-1, 1, P.n)
+    mine = ctx.pt_coeffs(ctx.encode_slots(z, 2))
+    assert np.abs(mine - ck.encode_coeffs(z, P.N, P.scale)).max() <= 1  # A7: rounding may differ by one
+    const = ctx.pt_coeffs(ctx.encode_slots(np.full(P.n, 0.25), 2))
+    assert const[0] == round(0.25 * 2 ** 40) and not const[1:].any()       # closed form (R2.2)
+    ctx.close()
+
+
+def run_hconv(mods, P, ctx, conv_kw, S, seed, do_rescale=True, kaiming=False):
+    """GPU fenc_hconv vs oracle hconv for every batch group; returns (max decoded error, layout)."""
+    ck, fr, fenc = mods
+    x, w = wl.conv_inputs(seed, conv_kw, kaiming=kaiming)
+    od = fr.ConvDesc(S=S, **conv_kw)
+    graph = fr.ConvGraph(od, P.n)
+    conv = ctx.conv_desc(S=S, **conv_kw)
+    lay = ctx.layout_plan(conv)
+    c = graph.counts()
+    assert (lay.n_in_ct, lay.n_out_ct, lay.n_inner_rot, lay.n_outer_rot, lay.n_pmult, lay.n_distinct_pt) == \
+        (c["n_in_ct"], c["n_out_ct"], c["n_inner_rot"], c["n_outer_rot"], c["n_pmult"], c["n_distinct_pt"])
+    assert lay.steps() == c["rot_steps"]
+    L = P.nq
+    ok = ck.keygen(P, 100 + seed, c["rot_steps"])
+    gk = ctx.keygen(100 + seed, c["rot_steps"])
+    oW = fr.encode_weights(ck, P, graph, w, L)
+    keys = ctx.wts_keys(conv, lay)
+    coeffs = np.stack([oW[tuple(int(v) for v in k)].coeffs for k in keys])
+    gW = ctx.conv_weights_from_coeffs(conv, lay, coeffs, L, float(P.q[L - 1]))
+    lin = graph.lin
+    g_in, o_in = [], {}
+    for bg in range(lin.BG):
+        for g in range(lin.G):
+            for u in range(S):
+                for v in range(S):
+                    pt = ck.encode(P, lin.gather(x, u, v, g, bg), L)
+                    o_in[(bg, u, v, g)] = ck.encrypt(P, ok, pt, 1000 + len(g_in))
+                    g_in.append(ctx.encrypt(gk, ctx.pt_from_coeffs(pt.coeffs, L, float(pt.scale)), 1000 + len(g_in)))
+    g_out = ctx.hconv(gk, conv, lay, gW, g_in, do_rescale=do_rescale)
+    So, lout = graph.S_out, graph.lout
+    Y = np.zeros((od.BS, od.C_out, od.H_out, od.W_out))
+    for bg in range(lin.BG):
+        ins = {(u, v, g): o_in[(bg, u, v, g)] for g in range(lin.G) for u in range(S) for v in range(S)}
+        o_out = fr.hconv(ck, P, ok, graph, ins, oW, do_rescale=do_rescale)
+        for go in range(lout.G):
+            for uo in range(So):
+                for vo in range(So):
+                    gct = g_out[((bg * lout.G + go) * So + uo) * So + vo]
+                    ref = o_out[(uo, vo, go)]
+                    assert np.array_equal(ctx.ct_export(gct), ref.c), (bg, go, uo, vo)
+                    assert abs(gct.scale - float(ref.scale)) <= 1e-9 * float(ref.scale)
+                    ctx.decrypt_decode(gk, gct, conv, lay, 1, uo, vo, go, bg, Y)
+    err = np.abs(Y - fr.direct_conv(od, x, w)).max()
+    return err, lay
+
+
+@pytest.mark.parametrize("conv_kw,S", [
+    (dict(BS=2, C_in=4, H=8, W=8, C_out=4, K=3, stride=1, pad=1), 2),      # inner + outer rotations, 2 samples per ct
+    (dict(BS=1, C_in=3, H=7, W=6, C_out=5, K=3, stride=1, pad=1), 1),      # ragged channels and frame, row-major (S=1)
+    (dict(BS=3, C_in=2, H=8, W=8, C_out=4, K=3, stride=2, pad=1), 2),      # stride by dropping fragments; BS not 2^k
+    (dict(BS=1, C_in=4, H=8, W=8, C_out=4, K=3, stride=1, pad=1, depthwise=True), 4),
+    (dict(BS=40, C_in=2, H=8, W=8, C_out=3, K=1, stride=1, pad=0), 2),     # several batch groups (B=32, BG=2), 1x1
+])
+def test_hconv_bit_exact_small(mods, conv_kw, S):
+    P, ctx = make(mods, "mid10")
+    err, _ = run_hconv(mods, P, ctx, conv_kw, S, seed=3)
+    assert err < 1e-3
+    ctx.close()
+
+
+def test_hconv_fig4_toy(mods):
+    """PAPER.md:160 (Fig. 4): input 1x16x4x4, conv(16,16,3,1), 16-slot ciphertexts, S in {1,2,4}."""
+    ck, fr, fenc = mods
+    for S, rots in ((1, 128), (2, 96), (4, 240)):
+        P = ck.Params(5, 3, 30, 1, 31, 3, 25)
+        ctx = fenc.Context(log2N=5, n_q=3, q_bits=30, n_p=1, p_bits=31, dnum=3, log2_scale=25)
+        err, lay = run_hconv(mods, P, ctx, wl.CONVS["fig4_toy"], S, seed=4)
+        assert lay.n_inner_rot + lay.n_outer_rot == rots
+        assert err < 5e-2  # 25-bit scale, 30-bit primes: the toy's own precision
+        ctx.close()
+
+
+def test_hconv_config1_full_size(mods):
+    """BASELINE config 1 (LeNet conv1-shaped, N=2^13, primary reading A1) at the size bench.py times."""
+    P, ctx = make(mods, "cfg1")
+    conv = ctx.conv_desc(**wl.CONVS["lenet_conv1"])
+    assert ctx.layout_plan(conv).S == 1  # Conv-aware selection (Eq. 7 bound < 1 -> smallest feasible)
+    err, lay = run_hconv(mods, P, ctx, wl.CONVS["lenet_conv1"], 1, seed=1001)
+    assert (lay.n_in_ct, lay.n_out_ct, lay.n_inner_rot, lay.n_outer_rot, lay.n_pmult, lay.n_rot_keys) == (1, 2, 24, 4, 150, 27)
+    assert err < 1e-3
+    ctx.close()
+
+
+def test_hconv_config1_literal_dnum1_bit_exact_only(mods):
+    """Literal dnum=1 (one digit of 3 limbs, P < Q): decoded check waived (A1), limbs must still match."""
+    ck, fr, fenc = mods
+    P, ctx = make(mods, "cfg1_literal")
+    assert ctx.dlen == 3 and ctx.beta_max == 1
+    ok = ck.keygen(P, 9, [1, 33])
+    gk = ctx.keygen(9, [1, 33])
+    limbs = wl.random_ct_limbs(8, P.q, 3, P.N)
+    outs = ctx.rotate(gk, [ctx.ct_import(limbs)] * 2, [1, 33])
+    for r, o in zip((1, 33), outs):
+        assert np.array_equal(ctx.ct_export(o), ck.rotate(P, ok, ck.Ciphertext(limbs, 3, 1), r).c)
+    ctx.close()
+
+
+def test_compress_fig5_shape(mods):
+    """PAPER.md:258-262 (Fig. 5): 4 sparse ciphertexts at 25% -> 1 dense; maskless keeps the level, the split-scale
+    masked mode consumes exactly one rescale."""
+    ck, fr, fenc = mods
+    P, ctx = make(mods, "mid10")
+    n, L, ch, v = P.n, P.nq, 8, 2
+    cs = n // ch
+    plan = fr.compress_plan(n, ch, cs, v, 4)
+    steps = sorted({r for terms in plan for _, r in terms if r})
+    ok, gk = ck.keygen(P, 77, steps), ctx.keygen(77, steps)
+    rng = np.random.default_rng(6)
+    srcs_o, srcs_g, vecs = [], [], []
+    for i in range(4):
+        z = np.zeros(n)
+        z[: v * cs] = rng.uniform(-1, 1, v * cs)
+        pt = ck.encode(P, z, L)
+        srcs_o.append(ck.encrypt(P, ok, pt, 50 + i))
+        srcs_g.append(ctx.encrypt(gk, ctx.pt_from_coeffs(pt.coeffs, L, float(pt.scale)), 50 + i))
+        vecs.append(z)
+    terms = [(t, i, r) for t, tl in enumerate(plan) for i, r in tl]
+    ref = fr.compress(ck, P, ok, plan, srcs_o)
+    got = ctx.compress(gk, srcs_g, terms, len(plan))
+    assert len(got) == 1 and got[0].L == L
+    assert np.array_equal(ctx.ct_export(got[0]), ref[0].c)
+    want = sum(np.roll(vecs[i], -r) for i, r in plan[0])
+    assert np.abs(ctx.decrypt_slots(gk, got[0]).real - want).max() < 1e-4
+    # masked, split scale: mask at Delta2 = q_{L-1} here, one rescale after
+    mask = ck.encode(P, fr.compress_mask(n, cs, v), L, P.q[L - 1])
+    ref = fr.compress(ck, P, ok, plan, srcs_o, mask_pt=mask, do_rescale=True)
+    got = ctx.compress(gk, srcs_g, terms, len(plan), mask=ctx.pt_from_coeffs(mask.coeffs, L, float(mask.scale)), do_rescale=True)
+    assert got[0].L == L - 1 and np.array_equal(ctx.ct_export(got[0]), ref[0].c)
+    ctx.close()
+
+
+def test_rotation_full_size_config3_sampled(mods):
+    """N=2^16, 24+4 limbs, dlen 4 (config 3): one batched rotation at the bench's launch configuration; the oracle
+    checks two limbs of each polynomial fully (the oracle's key switch costs ~1 min at this size)."""
+    ck, fr, fenc = mods
+    P, ctx = make(mods, "cfg3")
+    steps = [1, 12345]
+    gk = ctx.keygen(5, steps)
+    ok = ck.keygen(P, 5, steps[:1])
+    L = P.nq
+    limbs = wl.random_ct_limbs(21, P.q, L, P.N)
+    gin = ctx.ct_import(limbs)
+    outs = ctx.rotate(gk, [gin, gin], steps)
+    ref = ck.rotate(P, ok, ck.Ciphertext(limbs, L, 1), 1)
+    assert np.array_equal(ctx.ct_export(outs[0]), ref.c)
+    ctx.close()
