@@ -1,0 +1,351 @@
+"""bench.py -- measures BASELINE.json's metric on one B200 (or N independent replicas).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl ours|reference]
+
+A step = one pass of the whole hot path over one batch of synthetic input (workloads.py).  `value` is the
+whole-job throughput with inputs resident in HBM; `e2e` is the same metric through the C-ABI calls with HOST
+buffers (ciphertext limbs imported from / exported to host memory inside the timed region).  `roofline` is
+for the dominant kernel class, timed live with CUDA events by the library's profile hooks; `cpu_baseline`
+times the CPU oracle as it stands on a bounded sample of the same workload."""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+import workloads as wl  # noqa: E402
+
+METRIC = "encrypted conv layers/s & key-switched rotations/s; HBM GB/s vs B200 peak"
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return json.load(open(p)), "measured (MEASURED_PEAKS.json)"
+    return {"hbm_gbs": 6650.0}, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, device):
+        self.rows, self.proc, self.device = [], None, device
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.device), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) > 2 + i and r[2 + i].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
+                "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------ workloads
+def lenet_layers(BS, seed, upto="fc"):
+    """BASELINE config 2: LeNet-5-shaped network on MNIST-shaped input (D2).  S=4 for conv1
+    (the paper's best LeNet block size); pooling halves S; the 1/4 pool factors live in the next weights."""
+    rng = np.random.default_rng(seed)
+    w1 = rng.normal(0, 0.1, (6, 1, 5, 5))
+    w2 = rng.normal(0, 0.1, (16, 6, 5, 5)) * 0.25
+    layers = [
+        {"op": "conv", "conv": dict(BS=BS, C_in=1, H=28, W=28, C_out=6, K=5, stride=1, pad=2), "S": 4, "w": w1},
+        {"op": "square"}, {"op": "pool"},
+        {"op": "conv", "conv": dict(BS=BS, C_in=6, H=14, W=14, C_out=16, K=5, stride=1, pad=0, M=16), "S": 2, "w": w2},
+        {"op": "square"}, {"op": "pool"},
+    ]
+    if upto == "fc":
+        f1 = rng.normal(0, 0.1, (120, 400)) * 0.25
+        f2 = rng.normal(0, 0.1, (84, 120))
+        f3 = rng.normal(0, 0.1, (10, 84))
+        layers += [
+            {"op": "fc", "fc": dict(BS=BS, n_in=400, n_out=120, in_C=16, in_H=5, in_W=5, in_M=8), "w": f1},
+            {"op": "fc", "fc": dict(BS=BS, n_in=120, n_out=84, in_M=8), "w": f2},
+            {"op": "fc", "fc": dict(BS=BS, n_in=84, n_out=10, in_M=8), "w": f3},
+        ]
+    x = rng.uniform(0, 1, (BS, 1, 28, 28))
+    return layers, x
+
+
+WORKLOADS = {
+    # name: (PARAMS key, builder, description)
+    "cfg2_lenet5_convstage": ("cfg2", lambda bs, seed: lenet_layers(bs, seed, upto="conv"),
+                              "BASELINE config 2, conv stage: conv1-x^2-pool-conv2-x^2-pool, N=2^14, 8x40b+2x60b, dnum=4"),
+    "cfg2_lenet5": ("cfg2", lambda bs, seed: lenet_layers(bs, seed, upto="fc"),
+                    "BASELINE config 2: LeNet-5-shaped network, N=2^14, 8x40b+2x60b, dnum=4"),
+}
+DEFAULT_WORKLOAD = "cfg2_lenet5_convstage"
+
+
+def run_ours(args, rank, world):
+    import torch
+    import paper_2606_16359_b200 as fenc
+    from paper_2606_16359_b200.pipeline import Pipeline
+    dev = int(os.environ.get("LOCAL_RANK", 0))
+    torch.cuda.set_device(dev)
+    pkey, builder, desc = WORKLOADS[args.workload]
+    seed = 2000 + rank
+    layers, x = builder(args.batch, seed)
+    ctx = fenc.Context(device=dev, **wl.PARAMS[pkey])
+    pipe = Pipeline(ctx, layers)
+    pipe.setup(key_seed=seed)
+    cts = pipe.encrypt_input(x, enc_seed0=10 * seed)
+    n_lin, n_rot, n_relin, n_pm = pipe.counts()
+    ctx.sync()
+    setup_bytes = ctx.device_bytes()
+
+    def barrier():
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        pipe.forward(cts)
+    barrier()
+    sampler = ClockSampler(dev)
+    sampler.start()
+    ctx.launch_count(reset=True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        out = pipe.forward(cts)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = ctx.launch_count()
+    clocks = sampler.stop()
+    if world > 1:
+        t = torch.tensor([ms], device="cuda")
+        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+        ms = float(t.item())
+    step_ms = ms / args.steps
+    # ---- per-kernel-class timing (separate pass with the library's CUDA-event hooks on the same stream)
+    ctx.profile_enable(True)
+    prof_steps = min(args.steps, 3)
+    t0 = time.perf_counter()
+    for _ in range(prof_steps):
+        pipe.forward(cts)
+    prof = ctx.profile_read()
+    prof_ms = (time.perf_counter() - t0) * 1e3 / prof_steps
+    ctx.profile_enable(False)
+    peaks, peak_src = measured_peaks()
+    tot = sum(v[0] for v in prof.values())
+    top = max(prof, key=lambda k: prof[k][0])
+    t_ms, t_cnt, t_bytes = prof[top]
+    achieved = t_bytes / (t_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": top, "achieved": round(achieved, 1), "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": round(achieved / peaks["hbm_gbs"], 4), "traffic": None, "peak_source": peak_src,
+                "avg_launch_us": round(t_ms * 1e3 / t_cnt, 2), "share_of_step": round(t_ms / tot, 4),
+                "alg_bytes_per_launch": t_bytes / t_cnt,
+                "per_kernel": {k: {"ms_per_step": round(v[0] / prof_steps, 4), "launches_per_step": v[1] // prof_steps,
+                                   "alg_GBps": round(v[2] / (v[0] * 1e-3) / 1e9, 1)} for k, v in sorted(prof.items(), key=lambda kv: -kv[1][0])},
+                "profiled_step_ms": round(prof_ms, 3)}
+    # ---- end to end through the C ABI with host buffers: import (H2D + NTT), forward, export (iNTT + D2H)
+    host_in = [ctx.ct_export(c) for c in cts]
+    s_in = cts[0].scale
+    h2d = sum(a.nbytes for a in host_in)
+    d2h = 0
+    for it in range(1 + args.steps):  # first iteration is a warm-up
+        if it == 1:
+            barrier()
+            t0 = time.perf_counter()
+        dc = [ctx.ct_import(a, s_in) for a in host_in]
+        res = [ctx.ct_export(c) for c in pipe.forward(dc)]
+        d2h = sum(a.nbytes for a in res)
+    barrier()
+    e2e_s = (time.perf_counter() - t0) / args.steps
+    if world > 1:
+        t = torch.tensor([e2e_s], device="cuda")
+        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    layers_per_s = world * n_lin / (step_ms * 1e-3)
+    line = {
+        "metric": METRIC, "value": round(layers_per_s, 3), "unit": "encrypted conv layers/s",
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(step_ms, 4),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+        "config": {"workload": args.workload, "description": desc, "batch": args.batch, "linear_layers_per_step": n_lin,
+                   "rotations_per_step": n_rot, "relinearisations_per_step": n_relin, "pmults_per_step": n_pm,
+                   "multi_gpu": "replicas only" if world > 1 else "single", "l2": "inputs_exceed_l2: %d MiB resident" % (setup_bytes >> 20)},
+        "rotations_per_s": round(world * (n_rot + n_relin) / (step_ms * 1e-3), 1),
+        "images_per_s": round(world * args.batch / (step_ms * 1e-3), 2),
+        "gpu_launches": int(launches), "clocks": clocks,
+        "e2e": {"value": round(world * n_lin / e2e_s, 3), "unit": "encrypted conv layers/s", "h2d_bytes_per_step": int(h2d),
+                "d2h_bytes_per_step": int(d2h), "ms_per_step": round(e2e_s * 1e3, 3)},
+        "roofline": roofline,
+    }
+    if rank == 0 and world == 1:
+        line["cpu_baseline"] = cpu_baseline(args, pipe, budget_s=args.cpu_budget)
+    del out
+    return line
+
+
+# ------------------------------------------------------------------------------------------------ CPU oracle arm
+def level_ops(plan):
+    """{L: [rotations, pmults, rescales, squares]} of one forward pass, from the planner's exact counts."""
+    ops, n_ct = {}, None
+    for p in plan:
+        o = ops.setdefault(p["L"], [0, 0, 0, 0])
+        if p["op"] == "conv":
+            o[0] += p["lay"].n_inner_rot + p["lay"].n_outer_rot
+            o[1] += p["lay"].n_pmult
+            o[2] += p["lay"].n_out_ct
+            n_ct = p["lay"].n_out_ct
+        elif p["op"] == "fc":
+            o[0] += p["info"]["n_rot"]
+            o[1] += p["info"]["n_pmult"]
+            o[2] += p["info"]["n_out_ct"]
+            n_ct = p["info"]["n_out_ct"]
+        elif p["op"] == "square":
+            o[3] += n_ct
+        elif p["op"] == "pool":
+            n_ct //= 4
+    return ops
+
+
+class OracleSampler:
+    """Times the CPU oracle (oracle/, as it stands, single-threaded) on one rotation, one PMult-accumulate, one rescale
+    and one square per level the workload uses, and scales by the workload's exact operation counts."""
+
+    def __init__(self, pkey, ops, step):
+        from oracle import ckks as ck
+        self.ck, self.ops = ck, ops
+        self.P = ck.Params(*wl.oracle_params_args(wl.PARAMS[pkey]))
+        need_sq = any(o[3] for o in ops.values())
+        self.keys = ck.keygen(self.P, 1, [step], want_relin=need_sq)
+        self.step = step
+        rng = np.random.default_rng(0)
+        self.ct, self.pt = {}, {}
+        for L in ops:
+            z = rng.uniform(-1, 1, self.P.n)
+            self.pt[L] = ck.encode(self.P, z, L, self.P.q[L - 1])
+            self.ct[L] = ck.encrypt(self.P, self.keys, ck.encode(self.P, z, L), 5)
+
+    def sample(self):
+        ck, P, total, detail = self.ck, self.P, 0.0, {}
+        for L, (n_rot, n_pm, n_rs, n_sq) in sorted(self.ops.items(), reverse=True):
+            ct, t = self.ct[L], {}
+            if n_rot:
+                t0 = time.perf_counter(); ck.rotate(P, self.keys, ct, self.step); t["rot"] = time.perf_counter() - t0
+            if n_pm:
+                acc = np.zeros_like(ct.c)
+                t0 = time.perf_counter(); ck.pmult_acc(P, acc, ct, self.pt[L]); t["pmult"] = time.perf_counter() - t0
+            if n_rs and L >= 2:
+                t0 = time.perf_counter(); ck.rescale(P, ct); t["rescale"] = time.perf_counter() - t0
+            if n_sq and L >= 2:
+                t0 = time.perf_counter(); ck.square_relin(P, self.keys, ct); t["square"] = time.perf_counter() - t0
+            total += n_rot * t.get("rot", 0) + n_pm * t.get("pmult", 0) + n_rs * t.get("rescale", 0) + n_sq * t.get("square", 0)
+            detail[L] = {k: round(v, 4) for k, v in t.items()}
+        return total, detail
+
+
+def cpu_baseline(args, pipe, budget_s=20.0):
+    pkey = WORKLOADS[args.workload][0]
+    ops = level_ops(pipe.plan)
+    smp = OracleSampler(pkey, ops, sorted(pipe.steps)[0])
+    est, detail = smp.sample()
+    n_lin = pipe.counts()[0]
+    return {"value": round(n_lin / est, 6), "unit": "encrypted conv layers/s", "cores": 1, "kind": "oracle",
+            "sample": "one rotation, PMult-accumulate, rescale and square+relin per level used (%s), timed once each on the "
+                      "oracle and scaled by the step's exact operation counts; estimated oracle step %.1f s" % (
+                          ", ".join("L=%d" % L for L in sorted(ops, reverse=True)), est),
+            "seconds_per_op": detail}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle as it stands, on the host cores (no GPU).  Each step times the bounded sample."""
+    import paper_2606_16359_b200  # noqa: F401  (planner counts only come from the GPU-free description below)
+    pkey, builder, desc = WORKLOADS[args.workload]
+    # exact operation counts from the oracle's own planner (oracle/fragment.py), no GPU involved
+    from oracle import fragment as fr
+    from oracle import ckks as ck
+    P_n = 1 << (wl.PARAMS[pkey]["log2N"] - 1)
+    layers, _ = builder(args.batch, 2000)
+    ops, L, n_ct, n_lin, steps = {}, wl.PARAMS[pkey]["n_q"], None, 0, set()
+    for ly in layers:
+        o = ops.setdefault(L, [0, 0, 0, 0])
+        if ly["op"] == "conv":
+            g = fr.ConvGraph(fr.ConvDesc(S=ly["S"], **ly["conv"]), P_n)
+            c = g.counts()
+            o[0] += c["n_inner_rot"] + c["n_outer_rot"]; o[1] += c["n_pmult"]; o[2] += c["n_out_ct"]
+            n_ct, n_lin = c["n_out_ct"], n_lin + 1
+            steps.update(c["rot_steps"])
+            L -= 1
+        elif ly["op"] == "fc":
+            from oracle import network as nw
+            c = nw.fc_counts(P_n, **ly["fc"])
+            o[0] += c["n_rot"]; o[1] += c["n_pmult"]; o[2] += c["n_out_ct"]
+            n_ct, n_lin = c["n_out_ct"], n_lin + 1
+            steps.update(c["rot_steps"])
+            L -= 1
+        elif ly["op"] == "square":
+            o[3] += n_ct
+            L -= 1
+        elif ly["op"] == "pool":
+            n_ct //= 4
+    ops = {k: v for k, v in ops.items() if any(v)}
+    smp = OracleSampler(pkey, ops, sorted(steps)[0])
+    for _ in range(min(args.warmup, 1)):
+        smp.sample()
+    ests = [smp.sample()[0] for _ in range(min(args.steps, 3))]
+    est = float(np.mean(ests))
+    v = round(n_lin / est, 6)
+    sample = "per step: one rotation, PMult-accumulate, rescale, square+relin per level, scaled by exact counts; est. step %.1f s" % est
+    return {"impl": "reference", "metric": METRIC, "value": v, "unit": "encrypted conv layers/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(est * 1e3, 1), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+            "config": {"workload": args.workload, "description": desc, "batch": args.batch},
+            "cpu_baseline": {"value": v, "unit": "encrypted conv layers/s", "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": "encrypted conv layers/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
+    ap.add_argument("--batch", type=int, default=128)
+    ap.add_argument("--cpu-budget", type=float, default=20.0)
+    args = ap.parse_args()
+    rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+    if args.impl == "reference":
+        if rank == 0:
+            print(json.dumps(run_reference(args)), flush=True)
+        return
+    args.warmup = max(args.warmup, 3)
+    if world > 1:
+        import torch
+        torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", 0)))
+        torch.distributed.init_process_group("nccl")
+    line = run_ours(args, rank, world)
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        import torch
+        torch.distributed.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

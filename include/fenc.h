@@ -155,8 +155,11 @@ fenc_status fenc_rescale(fenc_ctx *ctx, fenc_ct *const *in, size_t n, fenc_ct **
 fenc_status fenc_add(fenc_ctx *ctx, const fenc_ct *a, const fenc_ct *b, fenc_ct **out);
 /* out = sum_i in[i] (*) pt[i], one lazy 128-bit accumulation per coefficient (a7); scale multiplies */
 fenc_status fenc_pmult_sum(fenc_ctx *ctx, fenc_ct *const *in, fenc_pt *const *pt, size_t n, fenc_ct **out);
-/* (c0,c1)^2 relinearised and rescaled: x -> x^2 (R2.12) */
-fenc_status fenc_square_relin(fenc_ctx *ctx, const fenc_keys *keys, const fenc_ct *in, fenc_ct **out);
+/* out[i] = in[i]^2 relinearised and rescaled (a13; R2.12), all n in ONE batched key switch; inputs share the level */
+fenc_status fenc_square_relin(fenc_ctx *ctx, const fenc_keys *keys, fenc_ct *const *in, size_t n, fenc_ct **out);
+/* out[g] = sum_{i < group} in[g*group + i] for g < n_groups: avg-pool by fragment selection (a14; PAPER.md:284;
+ * the 1/group^2 factor belongs to the next layer's weights, R2.12).  No rotations, no level consumed. */
+fenc_status fenc_sum_groups(fenc_ctx *ctx, fenc_ct *const *in, size_t group, size_t n_groups, fenc_ct **out);
 
 /* ------------------------------------------------------------------ HConv (R2.9) */
 /* Number of distinct non-zero weight plaintexts of the layer and their keys (u_o, v_o, g_out, g_in, d, i, j). */
@@ -189,6 +192,12 @@ fenc_status fenc_compress(fenc_ctx *ctx, const fenc_keys *keys, fenc_ct *const *
 /* Raw batched negacyclic NTT / iNTT (a1) in place on device memory: rows uint64 [n_rows][N]; mod_idx: host
  * array, row r uses modulus mod_idx[r] (0..n_q-1 ciphertext primes, n_q.. special primes). */
 fenc_status fenc_ntt_rows(fenc_ctx *ctx, void *device_rows, const int32_t *mod_idx, size_t n_rows, int inverse);
+/* Per-kernel-class timing with CUDA events on the context's stream, and the algorithmic bytes each launch moved
+ * (DESIGN.md section 7).  Off by default.  ms / launches / alg_bytes: host arrays of fenc_profile_kernels() entries. */
+fenc_status fenc_profile_enable(fenc_ctx *ctx, int on);
+int fenc_profile_kernels(void);
+const char *fenc_profile_name(int id);
+fenc_status fenc_profile_read(fenc_ctx *ctx, double *ms, uint64_t *launches, double *alg_bytes, int reset);
 /* counters since context creation: kernels launched by this library; optional reset */
 uint64_t fenc_launch_count(fenc_ctx *ctx, int reset);
 /* bytes currently held through the allocator */

@@ -52,7 +52,8 @@ SYMBOLS = ["fenc_params_init", "fenc_ctx_free", "fenc_last_error", "fenc_get_pri
            "fenc_decrypt_slots", "fenc_decrypt_decode", "fenc_ct_export", "fenc_ct_import", "fenc_ct_info",
            "fenc_ct_free", "fenc_rotate", "fenc_rescale", "fenc_add", "fenc_pmult_sum", "fenc_square_relin",
            "fenc_wts_keys", "fenc_conv_weights", "fenc_conv_weights_from_coeffs", "fenc_wts_free", "fenc_hconv",
-           "fenc_compress", "fenc_ntt_rows", "fenc_launch_count", "fenc_device_bytes"]
+           "fenc_compress", "fenc_ntt_rows", "fenc_launch_count", "fenc_device_bytes", "fenc_sum_groups",
+           "fenc_profile_enable", "fenc_profile_kernels", "fenc_profile_name", "fenc_profile_read"]
 
 _lib = None
 
@@ -90,7 +91,10 @@ def load_library(path=None):
         "fenc_rescale": [vp, vpp, C.c_size_t, vpp],
         "fenc_add": [vp, vp, vp, vpp],
         "fenc_pmult_sum": [vp, vpp, vpp, C.c_size_t, vpp],
-        "fenc_square_relin": [vp, vp, vp, vpp],
+        "fenc_square_relin": [vp, vp, vpp, C.c_size_t, vpp],
+        "fenc_sum_groups": [vp, vpp, C.c_size_t, C.c_size_t, vpp],
+        "fenc_profile_enable": [vp, C.c_int],
+        "fenc_profile_read": [vp, dp, u64p, dp, C.c_int],
         "fenc_wts_keys": [vp, C.POINTER(ConvDesc), C.POINTER(Layout), u32p, C.c_size_t, C.POINTER(C.c_size_t)],
         "fenc_conv_weights": [vp, C.POINTER(ConvDesc), C.POINTER(Layout), dp, C.c_uint32, C.c_double, vpp],
         "fenc_conv_weights_from_coeffs": [vp, C.POINTER(ConvDesc), C.POINTER(Layout), i64p, C.c_size_t, C.c_uint32,
@@ -106,6 +110,8 @@ def load_library(path=None):
     for name in ("fenc_ctx_free", "fenc_keys_free", "fenc_pt_free", "fenc_ct_free", "fenc_wts_free"):
         getattr(lib, name).argtypes, getattr(lib, name).restype = [vp], None
     lib.fenc_last_error.argtypes, lib.fenc_last_error.restype = [vp], C.c_char_p
+    lib.fenc_profile_kernels.argtypes, lib.fenc_profile_kernels.restype = [], C.c_int
+    lib.fenc_profile_name.argtypes, lib.fenc_profile_name.restype = [C.c_int], C.c_char_p
     lib.fenc_launch_count.argtypes, lib.fenc_launch_count.restype = [vp, C.c_int], C.c_uint64
     lib.fenc_device_bytes.argtypes, lib.fenc_device_bytes.restype = [vp], C.c_uint64
     if path is None:
@@ -359,10 +365,30 @@ class Context:
         self._ck(self.lib.fenc_pmult_sum(self.h, self._harr(cts), self._harr(pts), len(cts), C.byref(h)))
         return Ciphertext(self, h)
 
-    def square_relin(self, keys, ct):
-        h = C.c_void_p()
-        self._ck(self.lib.fenc_square_relin(self.h, keys.h, ct.h, C.byref(h)))
-        return Ciphertext(self, h)
+    def square_relin(self, keys, cts):
+        single = isinstance(cts, Ciphertext)
+        lst = [cts] if single else list(cts)
+        out = (C.c_void_p * len(lst))()
+        self._ck(self.lib.fenc_square_relin(self.h, keys.h, self._harr(lst), len(lst), out))
+        res = [Ciphertext(self, C.c_void_p(out[i])) for i in range(len(lst))]
+        return res[0] if single else res
+
+    def sum_groups(self, cts, group):
+        n = len(cts) // group
+        assert n * group == len(cts)
+        out = (C.c_void_p * n)()
+        self._ck(self.lib.fenc_sum_groups(self.h, self._harr(cts), group, n, out))
+        return [Ciphertext(self, C.c_void_p(out[i])) for i in range(n)]
+
+    def profile_enable(self, on=True):
+        self._ck(self.lib.fenc_profile_enable(self.h, int(on)))
+
+    def profile_read(self, reset=True):
+        """{kernel class: (ms, launches, algorithmic bytes)} accumulated since the last reset."""
+        k = self.lib.fenc_profile_kernels()
+        ms, cnt, by = np.zeros(k), np.zeros(k, dtype=np.uint64), np.zeros(k)
+        self._ck(self.lib.fenc_profile_read(self.h, _ptr(ms, C.c_double), _ptr(cnt, C.c_uint64), _ptr(by, C.c_double), int(reset)))
+        return {self.lib.fenc_profile_name(i).decode(): (float(ms[i]), int(cnt[i]), float(by[i])) for i in range(k) if cnt[i]}
 
     # ---- HConv
     def wts_keys(self, conv, lay):

@@ -420,7 +420,8 @@ extern "C" fenc_status fenc_hconv(fenc_ctx *ctx, const fenc_keys *K, const fenc_
     char *base = ds.commit();
     if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
     CUDA_OK(ctx, k_mac(ctx->k, (const u64 *const *)(base + o0), (const u64 *const *)(base + o1), (const int *)(base + o2),
-                       (u64 *const *)(base + o3), (int)mac_out.size(), L, ctx->max_lazy));
+                       (u64 *const *)(base + o3), (int)mac_out.size(), L, ctx->max_lazy,
+                       mac_alg_bytes(ctx, term_ct, term_pt, mac_out.size(), L)));
   }
   // ---- 3. outer rotations, 4. sums
   st = rotate_raw(ctx, K, L, rot_in, rot_step, rot_out);
@@ -430,7 +431,7 @@ extern "C" fenc_status fenc_hconv(fenc_ctx *ctx, const fenc_keys *K, const fenc_
     size_t o0 = ds.add(sum_terms), o1 = ds.add(sum_start), o2 = ds.add(sum_out);
     char *base = ds.commit();
     if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
-    CUDA_OK(ctx, k_add_many(ctx->k, (const u64 *const *)(base + o0), (const int *)(base + o1), (u64 *const *)(base + o2), (int)sum_out.size(), L));
+    CUDA_OK(ctx, k_add_many(ctx->k, (const u64 *const *)(base + o0), (const int *)(base + o1), (u64 *const *)(base + o2), (int)sum_out.size(), L, (int)sum_terms.size()));
   }
   // ---- 5. rescale
   if (do_rescale) {
@@ -487,7 +488,7 @@ extern "C" fenc_status fenc_compress(fenc_ctx *ctx, const fenc_keys *K, fenc_ct 
     char *base = ds.commit();
     if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
     CUDA_OK(ctx, k_mac(ctx->k, (const u64 *const *)(base + o0), (const u64 *const *)(base + o1), (const int *)(base + o2),
-                       (u64 *const *)(base + o3), (int)n_in, L, ctx->max_lazy));
+                       (u64 *const *)(base + o3), (int)n_in, L, ctx->max_lazy, mac_alg_bytes(ctx, tc, tp, n_in, L)));
   }
   u64 *Rbuf = dalloc_t<u64>(ctx, n_terms * CT);
   u64 *Ybuf = do_rescale ? dalloc_t<u64>(ctx, n_out * CT) : nullptr;
@@ -520,7 +521,7 @@ extern "C" fenc_status fenc_compress(fenc_ctx *ctx, const fenc_keys *K, fenc_ct 
     size_t o0 = ds.add(sum_terms), o1 = ds.add(sum_start), o2 = ds.add(sum_out);
     char *base = ds.commit();
     if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
-    CUDA_OK(ctx, k_add_many(ctx->k, (const u64 *const *)(base + o0), (const int *)(base + o1), (u64 *const *)(base + o2), (int)n_out, L));
+    CUDA_OK(ctx, k_add_many(ctx->k, (const u64 *const *)(base + o0), (const int *)(base + o1), (u64 *const *)(base + o2), (int)n_out, L, (int)sum_terms.size()));
   }
   if (do_rescale) {
     std::vector<BatchItem> items(n_out);

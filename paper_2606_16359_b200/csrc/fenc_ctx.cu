@@ -1,4 +1,5 @@
 // fenc_ctx.cu -- context, per-level key-switch tables, workspace, and the batched key-switch / rescale drivers.
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -162,7 +163,7 @@ extern "C" fenc_status fenc_params_init(const fenc_params_desc *d, fenc_ctx **ou
   } else {
     g.brow = 8, g.bcol = ctx->logN - 8, g.lt_row = 11, g.lc_col = 4, g.lt_col = g.bcol + 4;
   }
-  ctx->k = KCtx{(void *)ctx->stream, g, ctx->d_mods, ctx->d_tw_fwd, ctx->d_tw_inv, &ctx->launches, N, ctx->nq, ctx->np};
+  ctx->k = KCtx{(void *)ctx->stream, g, ctx->d_mods, ctx->d_tw_fwd, ctx->d_tw_inv, &ctx->launches, N, ctx->nq, ctx->np, nullptr};
   *out = c.release();
   return FENC_OK;
 }
@@ -343,18 +344,22 @@ fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items) {
     const int nb = (int)std::min(chunk, items.size() - at);
     DescStage st(ctx);
     std::vector<BatchItem> part(items.begin() + at, items.begin() + at + nb);
+    // items sharing a key run as neighbouring blocks (L2 reuse of the key tile)
+    std::stable_sort(part.begin(), part.end(), [](const BatchItem &a, const BatchItem &b) { return a.evk < b.evk; });
+    int n_keys = 0;
+    for (int i = 0; i < nb; i++) n_keys += (i == 0 || part[i].evk != part[i - 1].evk);
     st.add(part);
     const BatchItem *d_items = (const BatchItem *)st.commit();
     if (!d_items) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
     // a2 + a1: iNTT of sigma_g(d), pre-scaled for ModUp
     CUDA_OK(ctx, k_intt(k, d_items, nullptr, 0, true, y, (size_t)L * N, P->d_rows_in, L, P->d_scale_in, nb));
     // a3 + a1 (pass 1): ModUp fused into the first NTT pass
-    CUDA_OK(ctx, k_ntt_cols_bconv(k, y, (size_t)L * N, P->d_bc_up, tmp, (size_t)P->n_up * N, P->d_rows_up, P->n_up, nb));
+    CUDA_OK(ctx, k_ntt_cols_bconv(k, y, (size_t)L * N, P->d_bc_up, tmp, (size_t)P->n_up * N, P->d_rows_up, P->n_up, nb, L));
     // a1 (pass 2) + a4: evk inner product
-    CUDA_OK(ctx, k_ntt_rows_keymac(k, d_items, L, E, P->beta, P->d_tmp_index, tmp, (size_t)P->n_up * N, acc, (size_t)2 * E * N, nb));
+    CUDA_OK(ctx, k_ntt_rows_keymac(k, d_items, L, E, P->beta, P->d_tmp_index, tmp, (size_t)P->n_up * N, acc, (size_t)2 * E * N, nb, P->n_up, n_keys));
     // a5: ModDown = iNTT of the special limbs, conversion fused into pass 1, divide epilogue fused into pass 2
     CUDA_OK(ctx, k_intt(k, nullptr, acc, (size_t)2 * E * N, false, yP, (size_t)2 * np * N, P->d_rows_p, 2 * np, P->d_scale_p, nb));
-    CUDA_OK(ctx, k_ntt_cols_bconv(k, yP, (size_t)2 * np * N, P->d_bc_down, tmp2, (size_t)2 * L * N, P->d_rows_down, 2 * L, nb));
+    CUDA_OK(ctx, k_ntt_cols_bconv(k, yP, (size_t)2 * np * N, P->d_bc_down, tmp2, (size_t)2 * L * N, P->d_rows_down, 2 * L, nb, 2 * np));
     CUDA_OK(ctx, k_ntt_rows_divide(k, d_items, tmp2, (size_t)2 * L * N, acc, (size_t)2 * E * N, false, P->d_mul_pinv, P->d_rows_div, 2 * L, nb));
   }
   return FENC_OK;
@@ -382,7 +387,7 @@ fenc_status rescale_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items) {
     const BatchItem *d_items = (const BatchItem *)st.commit();
     if (!d_items) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
     CUDA_OK(ctx, k_intt(k, d_items, nullptr, 0, false, yR, 2 * N, P->d_rows_rs_in, 2, P->d_scale_rs, nb));
-    CUDA_OK(ctx, k_ntt_cols_bconv(k, yR, 2 * N, P->d_bc_rs, tmp2, (size_t)2 * L1 * N, P->d_rows_rs_up, 2 * L1, nb));
+    CUDA_OK(ctx, k_ntt_cols_bconv(k, yR, 2 * N, P->d_bc_rs, tmp2, (size_t)2 * L1 * N, P->d_rows_rs_up, 2 * L1, nb, 2));
     CUDA_OK(ctx, k_ntt_rows_divide(k, d_items, tmp2, (size_t)2 * L1 * N, nullptr, 0, true, P->d_mul_qlinv, P->d_rows_rs_div, 2 * L1, nb));
   }
   return FENC_OK;

@@ -147,4 +147,5 @@ fenc_status rotate_raw(fenc_ctx *ctx, const fenc_keys *keys, int L, const std::v
                        const std::vector<int> &steps, const std::vector<u64 *> &out);
 u32 galois_elt(const fenc_ctx *ctx, int step);
 fenc_status pt_device(fenc_ctx *ctx, fenc_pt *pt);  // ensure pt->d_mont
+double mac_alg_bytes(fenc_ctx *ctx, const std::vector<const u64 *> &tc, const std::vector<const u64 *> &tp, size_t n_out, int L);
 fenc_status coeffs_to_mont(fenc_ctx *ctx, const int64_t *coeffs_host, int L, u64 *d_out);

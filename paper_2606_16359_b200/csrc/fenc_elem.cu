@@ -3,11 +3,13 @@
 // All are HBM-bound streaming kernels: 16-byte vector accesses, limb-major, one pass.
 #include "fenc_device.cuh"
 
-#define LAUNCH_CHECK(k)                         \
-  do {                                          \
-    (*(k).launches)++;                          \
-    cudaError_t e__ = cudaGetLastError();       \
-    if (e__ != cudaSuccess) return (int)e__;    \
+#define PROF(k, id, bytes) if ((k).prof) prof_begin((k).prof, (k).stream, id, (double)(bytes))
+#define LAUNCH_CHECK(k)                            \
+  do {                                             \
+    (*(k).launches)++;                             \
+    if ((k).prof) prof_end((k).prof, (k).stream);  \
+    cudaError_t e__ = cudaGetLastError();          \
+    if (e__ != cudaSuccess) return (int)e__;       \
   } while (0)
 
 static inline cudaStream_t S(const KCtx &k) { return (cudaStream_t)k.stream; }
@@ -49,11 +51,12 @@ __global__ void __launch_bounds__(256) mac_kernel(MacP p) {
   *reinterpret_cast<ulonglong2 *>(out + LN + idx) = make_ulonglong2(r10, r11);
 }
 int k_mac(const KCtx &k, const u64 *const *term_ct, const u64 *const *term_pt, const int *start, u64 *const *outs, int n_out,
-          int L, int max_lazy) {
+          int L, int max_lazy, double alg_bytes) {
   if (n_out == 0) return 0;
   MacP p{term_ct, term_pt, start, outs, k.d_mods, L, k.geom.logN, max_lazy};
   size_t pairs = ((size_t)L * k.N) / 2;
   dim3 grid((unsigned)((pairs + 255) / 256), n_out);
+  PROF(k, K_MAC, alg_bytes);
   mac_kernel<<<grid, 256, 0, S(k)>>>(p);
   LAUNCH_CHECK(k);
   return 0;
@@ -74,11 +77,12 @@ __global__ void __launch_bounds__(256) add_many_kernel(AddManyP p) {
   }
   *reinterpret_cast<ulonglong2 *>(p.outs[o] + idx) = make_ulonglong2(a, b);
 }
-int k_add_many(const KCtx &k, const u64 *const *term, const int *start, u64 *const *outs, int n_out, int L) {
+int k_add_many(const KCtx &k, const u64 *const *term, const int *start, u64 *const *outs, int n_out, int L, int n_terms) {
   if (n_out == 0) return 0;
   AddManyP p{term, start, outs, k.d_mods, L, k.geom.logN};
   size_t pairs = (size_t)L * k.N;
   dim3 grid((unsigned)((pairs + 255) / 256), n_out);
+  PROF(k, K_ADD_MANY, 16.0 * L * k.N * ((double)n_terms + n_out));
   add_many_kernel<<<grid, 256, 0, S(k)>>>(p);
   LAUNCH_CHECK(k);
   return 0;
@@ -120,6 +124,7 @@ static int launch_row(const KCtx &k, RowP p, int n_rows) {
   if (n_rows == 0) return 0;
   p.mods = k.d_mods; p.logN = k.geom.logN;
   dim3 grid((k.N + 255) / 256, n_rows);
+  PROF(k, K_ROWOP, 24.0 * k.N * n_rows);
   row_kernel<OP><<<grid, 256, 0, S(k)>>>(p);
   LAUNCH_CHECK(k);
   return 0;
@@ -150,6 +155,30 @@ int k_reduce_signed(const KCtx &k, const i64 *coeffs, const int *row_mod, u64 *d
   return launch_row<OP_REDUCE_SIGNED>(k, p, n_rows);
 }
 
+// (d0, d1, d2) = (c0 c0, 2 c0 c1, c1 c1) per limb (a13, R2.12)
+__global__ void __launch_bounds__(256) tensor_square_kernel(const u64 *const *in, u64 *d, const ModConst *mods, int L, int logN) {
+  const size_t LN = (size_t)L << logN;
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= LN) return;
+  const ModConst mc = mods[i >> logN];
+  const u64 *c = in[blockIdx.y];
+  const u64 c0 = c[i], c1 = c[LN + i];
+  const u64 c0m = mont_mul(c0, mc.r2, mc.q, mc.qinv_neg), c1m = mont_mul(c1, mc.r2, mc.q, mc.qinv_neg);
+  u64 *o = d + (size_t)blockIdx.y * 3 * LN;
+  const u64 x = mont_mul(c1, c0m, mc.q, mc.qinv_neg);
+  o[i] = mont_mul(c0, c0m, mc.q, mc.qinv_neg);
+  o[LN + i] = addmod(x, x, mc.q);
+  o[2 * LN + i] = mont_mul(c1, c1m, mc.q, mc.qinv_neg);
+}
+int k_tensor_square(const KCtx &k, const u64 *const *in, u64 *d, int n, int L) {
+  if (n == 0) return 0;
+  dim3 grid((unsigned)(((size_t)L * k.N + 255) / 256), n);
+  PROF(k, K_ROWOP, 40.0 * L * k.N * n);
+  tensor_square_kernel<<<grid, 256, 0, S(k)>>>(in, d, k.d_mods, L, k.geom.logN);
+  LAUNCH_CHECK(k);
+  return 0;
+}
+
 // out[t] = c0[t] + c1[t] * s[t]  (decrypt, R2.5)
 __global__ void __launch_bounds__(256) dec_combine_kernel(const u64 *ct, const u64 *s_mont, u64 *out, const ModConst *mods, int L, int logN) {
   const int n = blockIdx.x * blockDim.x + threadIdx.x, t = blockIdx.y, N = 1 << logN;
@@ -160,6 +189,7 @@ __global__ void __launch_bounds__(256) dec_combine_kernel(const u64 *ct, const u
 }
 int k_dec_combine(const KCtx &k, const u64 *ct, const u64 *s_mont, u64 *out, int L) {
   dim3 grid((k.N + 255) / 256, L);
+  PROF(k, K_ROWOP, 32.0 * k.N * L);
   dec_combine_kernel<<<grid, 256, 0, S(k)>>>(ct, s_mont, out, k.d_mods, L, k.geom.logN);
   LAUNCH_CHECK(k);
   return 0;
@@ -199,6 +229,7 @@ __global__ void __launch_bounds__(256) sample_uniform_kernel(const u64 *keys, co
 int k_sample_uniform(const KCtx &k, const u64 *keys, const int *row_mod, u64 *dst, int n_rows) {
   if (n_rows == 0) return 0;
   dim3 grid((k.N + 255) / 256, n_rows);
+  PROF(k, K_SAMPLE, 8.0 * k.N * n_rows);
   sample_uniform_kernel<<<grid, 256, 0, S(k)>>>(keys, row_mod, dst, k.d_mods, k.geom.logN);
   LAUNCH_CHECK(k);
   return 0;
@@ -221,6 +252,7 @@ __global__ void __launch_bounds__(256) sample_gauss_kernel(u64 key, const i64 *a
 }
 int k_sample_gauss(const KCtx &k, u64 key, const i64 *addend, const int *row_mod, u64 *dst, int n_rows) {
   if (n_rows == 0) return 0;
+  PROF(k, K_SAMPLE, 8.0 * k.N * n_rows);
   sample_gauss_kernel<<<(k.N + 255) / 256, 256, 0, S(k)>>>(key, addend, row_mod, dst, k.d_mods, k.geom.logN, n_rows);
   LAUNCH_CHECK(k);
   return 0;

@@ -59,6 +59,15 @@ struct NttGeom {
   int lc_col;  // log2 columns per tile of the column pass
 };
 
+// per-kernel-class timing with CUDA events on the launching stream (measurement only; off by default)
+enum KernelId {
+  K_INTT_ROW, K_INTT_COL, K_NTT_COL, K_NTT_COL_BCONV, K_NTT_ROW, K_KEYMAC, K_DIVIDE, K_MAC, K_ADD_MANY, K_ROWOP, K_SAMPLE,
+  K_COUNT
+};
+struct Prof;
+void prof_begin(Prof *p, void *stream, int id, double alg_bytes);
+void prof_end(Prof *p, void *stream);
+
 struct KCtx {  // what kernels need from a context
   void *stream;  // cudaStream_t
   NttGeom geom;
@@ -67,6 +76,7 @@ struct KCtx {  // what kernels need from a context
   const ShoupC *d_tw_inv;  // [nmod][N] inverse twiddles
   u64 *launches;           // host counter of kernel launches
   int N, nq, np;
+  Prof *prof;              // NULL unless profiling is enabled
 };
 
 // ---------------------------------------------------------------- launchers (fenc_kernels.cu); return cudaError_t
@@ -81,12 +91,12 @@ int k_ntt(const KCtx &k, const u64 *src, size_t src_bstride, u64 *dst, size_t ds
 // forward pass 1 (column stages) with fused base conversion (ModUp a3 / ModDown's Conv / rescale's mod):
 // value = sum_{s < rows[r].aux} y[b][rows[r].src_row + s][.] * bc[rows[r].aux2 + s] (Montgomery constants)
 int k_ntt_cols_bconv(const KCtx &k, const u64 *y, size_t y_bstride, const u64 *bc, u64 *tmp, size_t tmp_bstride,
-                     const RowDesc *rows, int n_rows, int n_batch);
+                     const RowDesc *rows, int n_rows, int n_batch, int n_src_rows);
 // forward pass 2 (row stages) fused with the evaluation-key inner product (a4) over E = L + np target rows.
 // tmp_index[j*E + t] = row of tmp holding digit j / target t, or -1 when t lies in digit j (then the row is
 // items[b].ks_in[t] itself, read through the Galois gather).  acc[b][c][t][N] canonical.
 int k_ntt_rows_keymac(const KCtx &k, const BatchItem *items, int L, int E, int beta, const int *tmp_index, const u64 *tmp,
-                      size_t tmp_bstride, u64 *acc, size_t acc_bstride, int n_batch);
+                      size_t tmp_bstride, u64 *acc, size_t acc_bstride, int n_batch, int n_up, int n_distinct_keys);
 // forward pass 2 fused with the divide epilogue (ModDown a5 / rescale a8):
 // out[dst_row] = (minuend[aux2] - X) * mul[mod] (+ addend_c[mod] through the gather)
 // minuend = from_items ? items[b].sub_in : acc + b*acc_bstride
@@ -95,9 +105,9 @@ int k_ntt_rows_divide(const KCtx &k, const BatchItem *items, const u64 *tmp, siz
                       int n_batch);
 // MAC (a7): outs[o] = sum_{t in [start[o], start[o+1])} ct[t] (*) pt[t]; ct [2][L][N], pt [L][N] Montgomery form
 int k_mac(const KCtx &k, const u64 *const *term_ct, const u64 *const *term_pt, const int *start, u64 *const *outs, int n_out,
-          int L, int max_lazy);
+          int L, int max_lazy, double alg_bytes);
 // outs[o] = sum of listed [2][L][N] arrays
-int k_add_many(const KCtx &k, const u64 *const *term, const int *start, u64 *const *outs, int n_out, int L);
+int k_add_many(const KCtx &k, const u64 *const *term, const int *start, u64 *const *outs, int n_out, int L, int n_terms);
 // rows kernels: row r uses modulus row_mod[r] (device array)
 // out = x - a * s_mont[mod]   (s_mont: [nmod][N] Montgomery form)
 int k_x_minus_as(const KCtx &k, const u64 *a, const u64 *x, const u64 *s_mont, u64 *out, const int *row_mod, int n_rows);
@@ -115,6 +125,8 @@ int k_add_f_sprime(const KCtx &k, const u64 *x, const u64 *sp_mont, u32 g, const
                    int n_rows);
 // out[r] = a[r] * b[r] mod q (both normal form, NTT domain)
 int k_mul_rows(const KCtx &k, const u64 *a, const u64 *b, u64 *out, const int *row_mod, int n_rows);
+// tensor square of n ciphertexts: d[b] = (c0 c0, 2 c0 c1, c1 c1), d: [n][3][L][N]
+int k_tensor_square(const KCtx &k, const u64 *const *in, u64 *d, int n, int L);
 // out[r] = a[r] + b[r] (+ b[r] again when twice)
 int k_add_rows(const KCtx &k, const u64 *a, const u64 *b, u64 *out, const int *row_mod, int n_rows, bool twice);
 

@@ -10,11 +10,13 @@
 #include "fenc_device.cuh"
 
 static inline int nthreads_for(int lt) { int t = 1 << (lt - 3); return t < 32 ? 32 : t; }
-#define LAUNCH_CHECK(k)                         \
-  do {                                          \
-    (*(k).launches)++;                          \
-    cudaError_t e__ = cudaGetLastError();       \
-    if (e__ != cudaSuccess) return (int)e__;    \
+#define PROF(k, id, bytes) if ((k).prof) prof_begin((k).prof, (k).stream, id, (double)(bytes))
+#define LAUNCH_CHECK(k)                            \
+  do {                                             \
+    (*(k).launches)++;                             \
+    if ((k).prof) prof_end((k).prof, (k).stream);  \
+    cudaError_t e__ = cudaGetLastError();          \
+    if (e__ != cudaSuccess) return (int)e__;       \
   } while (0)
 
 // ------------------------------------------------------------------------------------------------ inverse, pass A
@@ -68,11 +70,13 @@ int k_intt(const KCtx &k, const BatchItem *items, const u64 *src, size_t src_bst
   const NttGeom &g = k.geom;
   InttRowP a{items, src, src_bstride, dst, dst_bstride, rows, k.d_mods, k.d_tw_inv, g};
   dim3 gridA(k.N >> g.lt_row, n_rows, n_batch);
+  PROF(k, K_INTT_ROW, 16.0 * k.N * n_rows * n_batch);
   if (gather) intt_rowpass_kernel<true><<<gridA, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(a);
   else intt_rowpass_kernel<false><<<gridA, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(a);
   LAUNCH_CHECK(k);
   InttColP c{dst, dst_bstride, rows, scale, k.d_mods, k.d_tw_inv, g};
   dim3 gridB(k.N >> g.lt_col, n_rows, n_batch);
+  PROF(k, K_INTT_COL, 16.0 * k.N * n_rows * n_batch);
   intt_colpass_kernel<<<gridB, nthreads_for(g.lt_col), sizeof(u64) << g.lt_col, st>>>(c);
   LAUNCH_CHECK(k);
   return 0;
@@ -138,21 +142,25 @@ int k_ntt(const KCtx &k, const u64 *src, size_t src_bstride, u64 *dst, size_t ds
   const NttGeom &g = k.geom;
   NttColP a{src, src_bstride, nullptr, dst, dst_bstride, rows, k.d_mods, k.d_tw_fwd, g};
   dim3 grid1(k.N >> g.lt_col, n_rows, n_batch);
+  PROF(k, K_NTT_COL, 16.0 * k.N * n_rows * n_batch);
   ntt_colpass_kernel<false><<<grid1, nthreads_for(g.lt_col), sizeof(u64) << g.lt_col, st>>>(a);
   LAUNCH_CHECK(k);
   NttRowP r{dst, dst_bstride, dst, dst_bstride, rows, k.d_mods, k.d_tw_fwd, g, 1};
   dim3 grid2(k.N >> g.lt_row, n_rows, n_batch);
+  PROF(k, K_NTT_ROW, 16.0 * k.N * n_rows * n_batch);
   ntt_rowpass_kernel<<<grid2, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(r);
   LAUNCH_CHECK(k);
   return 0;
 }
 
 int k_ntt_cols_bconv(const KCtx &k, const u64 *y, size_t y_bstride, const u64 *bc, u64 *tmp, size_t tmp_bstride,
-                     const RowDesc *rows, int n_rows, int n_batch) {
+                     const RowDesc *rows, int n_rows, int n_batch, int n_src_rows) {
   if (n_rows == 0 || n_batch == 0) return 0;
   const NttGeom &g = k.geom;
   NttColP a{y, y_bstride, bc, tmp, tmp_bstride, rows, k.d_mods, k.d_tw_fwd, g};
   dim3 grid1(k.N >> g.lt_col, n_rows, n_batch);
+  // algorithmic bytes: every source row read once, every target row written once
+  PROF(k, K_NTT_COL_BCONV, 8.0 * k.N * ((double)n_src_rows + n_rows) * n_batch);
   ntt_colpass_kernel<true><<<grid1, nthreads_for(g.lt_col), sizeof(u64) << g.lt_col, (cudaStream_t)k.stream>>>(a);
   LAUNCH_CHECK(k);
   return 0;
@@ -220,7 +228,7 @@ __global__ void __launch_bounds__(256) ntt_rows_keymac_kernel(KeyMacP p) {
 }
 
 int k_ntt_rows_keymac(const KCtx &k, const BatchItem *items, int L, int E, int beta, const int *tmp_index, const u64 *tmp,
-                      size_t tmp_bstride, u64 *acc, size_t acc_bstride, int n_batch) {
+                      size_t tmp_bstride, u64 *acc, size_t acc_bstride, int n_batch, int n_up, int n_distinct_keys) {
   if (n_batch == 0) return 0;
   const NttGeom &g = k.geom;
   KeyMacP p{items, tmp_index, tmp, tmp_bstride, acc, acc_bstride, k.d_mods, k.d_tw_fwd, g, L, E, beta, k.nq + k.np, k.nq,
@@ -228,6 +236,8 @@ int k_ntt_rows_keymac(const KCtx &k, const BatchItem *items, int L, int E, int b
   const int nth = nthreads_for(g.lt_row);
   dim3 grid((k.N >> g.lt_row) * n_batch, E, 1);
   const int ept = ((1 << g.lt_row) + nth - 1) / nth;
+  // algorithmic bytes: ModUp temp + the switched polynomial read once, accumulators written once, each key once
+  PROF(k, K_KEYMAC, 8.0 * k.N * (((double)n_up + L + 2.0 * E) * n_batch + 2.0 * beta * E * n_distinct_keys));
   if (ept <= 1) ntt_rows_keymac_kernel<1><<<grid, nth, sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
   else if (ept <= 4) ntt_rows_keymac_kernel<4><<<grid, nth, sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
   else ntt_rows_keymac_kernel<8><<<grid, nth, sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
@@ -274,6 +284,7 @@ int k_ntt_rows_divide(const KCtx &k, const BatchItem *items, const u64 *tmp, siz
   const NttGeom &g = k.geom;
   DivideP p{items, tmp, tmp_bstride, acc, acc_bstride, mul, rows, k.d_mods, k.d_tw_fwd, g, minuend_from_items ? 1 : 0};
   dim3 grid(k.N >> g.lt_row, n_rows, n_batch);
+  PROF(k, K_DIVIDE, 8.0 * k.N * (3.5 * n_rows) * n_batch);  // temp + minuend + output, addend on half the rows
   ntt_rows_divide_kernel<<<grid, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
   LAUNCH_CHECK(k);
   return 0;

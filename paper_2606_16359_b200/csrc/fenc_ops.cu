@@ -1,4 +1,5 @@
 // fenc_ops.cu -- keys, plaintexts, encryption / decryption and the ciphertext primitives of the C ABI.
+#include <algorithm>
 #include <cmath>
 #include <cstring>
 
@@ -247,6 +248,13 @@ extern "C" void fenc_ct_free(fenc_ct *ct) {
 }
 
 // ------------------------------------------------------------------------------------------------ primitives
+// algorithmic bytes of one MAC launch: every distinct ciphertext and plaintext read once, every output written once
+double mac_alg_bytes(fenc_ctx *ctx, const std::vector<const u64 *> &tc, const std::vector<const u64 *> &tp, size_t n_out, int L) {
+  std::vector<const u64 *> a(tc), b(tp);
+  std::sort(a.begin(), a.end()), std::sort(b.begin(), b.end());
+  size_t nc = std::unique(a.begin(), a.end()) - a.begin(), npt = std::unique(b.begin(), b.end()) - b.begin();
+  return 8.0 * L * ctx->N * (2.0 * nc + (double)npt + 2.0 * n_out);
+}
 extern "C" fenc_status fenc_rotate(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const *in, const int32_t *steps, size_t n,
                                    fenc_ct **out) {
   if (!ctx || !K || !in || !steps || !out) return FENC_ERR_INVALID_ARG;
@@ -306,7 +314,7 @@ extern "C" fenc_status fenc_add(fenc_ctx *ctx, const fenc_ct *a, const fenc_ct *
   size_t o1 = st.add(terms), o2 = st.add(start), o3 = st.add(outs);
   char *base = st.commit();
   if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
-  CUDA_OK(ctx, k_add_many(ctx->k, (const u64 *const *)(base + o1), (const int *)(base + o2), (u64 *const *)(base + o3), 1, a->L));
+  CUDA_OK(ctx, k_add_many(ctx->k, (const u64 *const *)(base + o1), (const int *)(base + o2), (u64 *const *)(base + o3), 1, a->L, 2));
   *out = c;
   return FENC_OK;
 }
@@ -331,41 +339,80 @@ extern "C" fenc_status fenc_pmult_sum(fenc_ctx *ctx, fenc_ct *const *in, fenc_pt
   char *base = st.commit();
   if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
   CUDA_OK(ctx, k_mac(ctx->k, (const u64 *const *)(base + o0), (const u64 *const *)(base + o1), (const int *)(base + o2),
-                     (u64 *const *)(base + o3), 1, L, ctx->max_lazy));
+                     (u64 *const *)(base + o3), 1, L, ctx->max_lazy, mac_alg_bytes(ctx, tc, tp, 1, L)));
   *out = c;
   return FENC_OK;
 }
 
-// x -> x^2 (R2.12): d0 = c0 c0, d1 = 2 c0 c1, d2 = c1 c1; (d0, d1) + KS(d2; relin); rescale
-extern "C" fenc_status fenc_square_relin(fenc_ctx *ctx, const fenc_keys *K, const fenc_ct *in, fenc_ct **out) {
+// x -> x^2 (R2.12): d0 = c0 c0, d1 = 2 c0 c1, d2 = c1 c1; (d0, d1) + KS(d2; relin); rescale.  Batched over n.
+extern "C" fenc_status fenc_square_relin(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const *in, size_t n, fenc_ct **out) {
   if (!ctx || !K || !in || !out) return FENC_ERR_INVALID_ARG;
+  if (n == 0) return FENC_OK;
   auto it = K->evk.find(FENC_RELIN_KEY_ID);
   if (it == K->evk.end()) return fail(ctx, FENC_ERR_NO_KEY, "no relinearisation key");
-  const int L = in->L;
+  const int L = in[0]->L;
   if (L < 2) return fail(ctx, FENC_ERR_LEVEL, "square needs a level to rescale into");
   const size_t LN = (size_t)L * ctx->N;
-  u64 *d = dalloc_t<u64>(ctx, 3 * LN), *mid = dalloc_t<u64>(ctx, 2 * LN);
+  std::vector<const u64 *> ptrs(n);
+  for (size_t i = 0; i < n; i++) {
+    if (in[i]->L != L) return fail(ctx, FENC_ERR_MISMATCH, "square: inputs differ in level");
+    ptrs[i] = in[i]->d;
+  }
+  u64 *d = dalloc_t<u64>(ctx, n * 3 * LN), *mid = dalloc_t<u64>(ctx, n * 2 * LN);
   if (!d || !mid) return fail(ctx, FENC_ERR_OOM, "square");
-  const u64 *c0 = in->d, *c1 = in->d + LN;
-  CUDA_OK(ctx, k_mul_rows(ctx->k, c0, c0, d, ctx->d_ident_mod, L));
-  CUDA_OK(ctx, k_mul_rows(ctx->k, c0, c1, d + LN, ctx->d_ident_mod, L));
-  CUDA_OK(ctx, k_add_rows(ctx->k, d + LN, d + LN, d + LN, ctx->d_ident_mod, L, false));
-  CUDA_OK(ctx, k_mul_rows(ctx->k, c1, c1, d + 2 * LN, ctx->d_ident_mod, L));
-  std::vector<BatchItem> items(1);
-  items[0] = BatchItem{};
-  items[0].ks_in = d + 2 * LN, items[0].out = mid, items[0].evk = it->second, items[0].add0 = d, items[0].add1 = d + LN, items[0].g = 1;
+  {
+    DescStage st(ctx);
+    size_t o0 = st.add(ptrs);
+    char *base = st.commit();
+    if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
+    CUDA_OK(ctx, k_tensor_square(ctx->k, (const u64 *const *)(base + o0), d, (int)n, L));
+  }
+  std::vector<BatchItem> items(n), rs(n);
+  std::vector<fenc_ct *> made(n, nullptr);
+  for (size_t i = 0; i < n; i++) {
+    u64 *di = d + i * 3 * LN;
+    items[i] = BatchItem{};
+    items[i].ks_in = di + 2 * LN, items[i].out = mid + i * 2 * LN, items[i].evk = it->second;
+    items[i].add0 = di, items[i].add1 = di + LN, items[i].g = 1;
+    made[i] = new_ct(ctx, L - 1, in[i]->scale * in[i]->scale / (double)ctx->mod[L - 1]);
+    if (!made[i]) return fail(ctx, FENC_ERR_OOM, "square output");
+    rs[i] = BatchItem{};
+    rs[i].sub_in = mid + i * 2 * LN, rs[i].out = made[i]->d;
+  }
   fenc_status st = ks_batch(ctx, L, items);
   if (st != FENC_OK) return st;
-  fenc_ct *c = new_ct(ctx, L - 1, in->scale * in->scale / (double)ctx->mod[L - 1]);
-  if (!c) return fail(ctx, FENC_ERR_OOM, "square output");
-  std::vector<BatchItem> rs(1);
-  rs[0] = BatchItem{};
-  rs[0].sub_in = mid, rs[0].out = c->d;
   st = rescale_batch(ctx, L, rs);
   if (st != FENC_OK) return st;
-  CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
   dfree(ctx, d), dfree(ctx, mid);
-  *out = c;
+  for (size_t i = 0; i < n; i++) out[i] = made[i];
+  return FENC_OK;
+}
+
+extern "C" fenc_status fenc_sum_groups(fenc_ctx *ctx, fenc_ct *const *in, size_t group, size_t n_groups, fenc_ct **out) {
+  if (!ctx || !in || !out || group == 0) return FENC_ERR_INVALID_ARG;
+  if (n_groups == 0) return FENC_OK;
+  const int L = in[0]->L;
+  std::vector<const u64 *> terms(group * n_groups);
+  std::vector<int> start(n_groups + 1);
+  std::vector<u64 *> outs(n_groups);
+  std::vector<fenc_ct *> made(n_groups, nullptr);
+  for (size_t i = 0; i < group * n_groups; i++) {
+    if (in[i]->L != L || !scale_close(in[i]->scale, in[0]->scale)) return fail(ctx, FENC_ERR_MISMATCH, "sum: level or scale differ");
+    terms[i] = in[i]->d;
+  }
+  for (size_t g = 0; g < n_groups; g++) {
+    made[g] = new_ct(ctx, L, in[0]->scale);
+    if (!made[g]) return fail(ctx, FENC_ERR_OOM, "sum output");
+    start[g] = (int)(g * group), outs[g] = made[g]->d;
+  }
+  start[n_groups] = (int)(group * n_groups);
+  DescStage st(ctx);
+  size_t o0 = st.add(terms), o1 = st.add(start), o2 = st.add(outs);
+  char *base = st.commit();
+  if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
+  CUDA_OK(ctx, k_add_many(ctx->k, (const u64 *const *)(base + o0), (const int *)(base + o1), (u64 *const *)(base + o2), (int)n_groups, L,
+                          (int)terms.size()));
+  for (size_t g = 0; g < n_groups; g++) out[g] = made[g];
   return FENC_OK;
 }
 

@@ -1,0 +1,128 @@
+"""Layer sequencing over the C ABI: a list of fragment-encoded layers (conv / square / pool / fc) evaluated by one
+batched library call per layer (R2.9, R2.12).  Orchestration only: every ciphertext
+operation runs inside libfenc's kernels; this file holds no arithmetic on ciphertext data."""
+import numpy as np
+
+
+class Pipeline:
+    """layers: list of dicts
+         {"op": "conv", "conv": {BS, C_in, H, W, C_out, K, stride, pad, [depthwise], [M]}, "S": S, "w": ndarray}
+         {"op": "square"}                      x -> x^2, relinearised and rescaled (one level)
+         {"op": "pool"}                        2x2 sum-pool by fragment selection (S halves; factor 1/4 goes into the next w)
+         {"op": "fc", "fc": {...}, "w": ndarray[n_out][n_in]}     plain-diagonal fully connected layer
+    """
+
+    def __init__(self, ctx, layers, L0=None):
+        self.ctx, self.layers, self.L0 = ctx, layers, L0 or ctx.n_q
+        self.plan, self.steps, self.need_relin = [], set(), False
+        L = self.L0
+        for ly in layers:
+            if ly["op"] == "conv":
+                conv = ctx.conv_desc(S=ly["S"], **ly["conv"])
+                lay = ctx.layout_plan(conv)
+                self.steps.update(lay.steps())
+                self.plan.append(dict(op="conv", conv=conv, lay=lay, L=L, w=ly.get("w")))
+                L -= 1
+            elif ly["op"] == "fc":
+                fc = ctx.fc_desc(**ly["fc"])
+                info = ctx.fc_plan(fc)
+                self.steps.update(info["rot_steps"])
+                self.plan.append(dict(op="fc", fc=fc, info=info, L=L, w=ly.get("w")))
+                L -= 1
+            elif ly["op"] == "square":
+                self.need_relin = True
+                self.plan.append(dict(op="square", L=L))
+                L -= 1
+            elif ly["op"] == "pool":
+                self.plan.append(dict(op="pool", L=L))
+            else:
+                raise ValueError(ly["op"])
+        self.L_out = L
+        self.keys, self.weights = None, []
+
+    def counts(self):
+        """(linear layers, key-switched rotations, relinearisations, PMults) of one forward pass."""
+        lin = rot = relin = pm = 0
+        n_ct = None
+        for p in self.plan:
+            if p["op"] == "conv":
+                lin += 1
+                rot += p["lay"].n_inner_rot + p["lay"].n_outer_rot
+                pm += p["lay"].n_pmult
+                n_ct = p["lay"].n_out_ct
+            elif p["op"] == "fc":
+                lin += 1
+                rot += p["info"]["n_rot"]
+                pm += p["info"]["n_pmult"]
+                n_ct = p["info"]["n_out_ct"]
+            elif p["op"] == "square":
+                relin += n_ct
+            elif p["op"] == "pool":
+                n_ct //= 4
+        return lin, rot, relin, pm
+
+    def setup(self, key_seed, encode_weight=None):
+        """Generate keys for exactly the rotation amounts the layers need and encode every weight plaintext.
+        encode_weight(plan_entry) -> int64 coefficient array, to start from pre-encoded integers (A7)."""
+        ctx = self.ctx
+        self.keys = ctx.keygen(key_seed, sorted(self.steps), want_relin=self.need_relin)
+        self.weights = []
+        for p in self.plan:
+            if p["op"] == "conv":
+                if encode_weight is not None:
+                    self.weights.append(ctx.conv_weights_from_coeffs(p["conv"], p["lay"], encode_weight(p), p["L"]))
+                else:
+                    self.weights.append(ctx.conv_weights(p["conv"], p["lay"], p["w"], p["L"]))
+            elif p["op"] == "fc":
+                if encode_weight is not None:
+                    self.weights.append(ctx.fc_weights_from_coeffs(p["fc"], encode_weight(p), p["L"]))
+                else:
+                    self.weights.append(ctx.fc_weights(p["fc"], p["w"], p["L"]))
+            else:
+                self.weights.append(None)
+        return self.keys
+
+    def encrypt_input(self, x, enc_seed0):
+        """Algorithm 1 on host x[BS][C][H][W] for the first layer; ciphertext order [bg][g][u][v]."""
+        p = self.plan[0]
+        conv, lay, ctx = p["conv"], p["lay"], self.ctx
+        cts = []
+        for bg in range(lay.BG):
+            for g in range(lay.G_in):
+                for u in range(lay.S):
+                    for v in range(lay.S):
+                        pt = ctx.encode_fragment(conv, lay, x, u, v, g, bg, p["L"])
+                        cts.append(ctx.encrypt(self.keys, pt, enc_seed0 + len(cts)))
+        return cts
+
+    @staticmethod
+    def pool_order(n_ct, S):
+        """indices so that consecutive groups of 4 are the fragments (2uo+a, 2vo+b) of output fragment (uo, vo)."""
+        per = S * S
+        idx = []
+        for base in range(0, n_ct, per):
+            for uo in range(S // 2):
+                for vo in range(S // 2):
+                    for a in range(2):
+                        for b in range(2):
+                            idx.append(base + (2 * uo + a) * S + (2 * vo + b))
+        return idx
+
+    def forward(self, cts, trace=None):
+        ctx = self.ctx
+        S = None
+        for p, w in zip(self.plan, self.weights):
+            if p["op"] == "conv":
+                cts = ctx.hconv(self.keys, p["conv"], p["lay"], w, cts, do_rescale=True)
+                S = p["lay"].S_out
+            elif p["op"] == "fc":
+                cts = ctx.fc(self.keys, p["fc"], w, cts, do_rescale=True)
+                S = 1
+            elif p["op"] == "square":
+                cts = ctx.square_relin(self.keys, cts)
+            elif p["op"] == "pool":
+                cts = ctx.sum_groups([cts[i] for i in self.pool_order(len(cts), S)], 4)
+                S //= 2
+            if trace is not None:
+                trace.append(cts)
+        return cts
