@@ -62,26 +62,93 @@ struct TileGeo {
   DEVI int gbit(int pb) const { return pb < lc ? pb : pb - lc + sh; }  // global bit of tile bit pb
 };
 
-// One radix-8 register round over tile bits [pw, pw+3); only window bits s in [s_lo, s_hi) are transformed.
-// FWD: Cooley-Tukey, high bit first, values in [0,4q).  INV: Gentleman-Sande, low bit first, values in [0,2q).
-template <bool FWD>
-DEVI void tile_round(u64 *sm, const TileGeo &G, int pw, int s_lo, int s_hi, const ShoupC *tw, u64 q, u64 q2, int tid) {
-  const int ebase = ((tid >> pw) << (pw + 3)) | (tid & ((1 << pw) - 1));
+// v mod q for any v < 2^64: v - floor(v qbar / 2^64) q lies in [0, 2q) (qbar = floor(2^64 / q)), then one correction
+DEVI u64 fullred(u64 v, u64 q, u64 qbar) { return csub(v - __umul64hi(v, qbar) * q, q); }
+
+// ---------------------------------------------------------------------------------------------- tile engine
+// A pass transforms the active tile bits [lo, lo+nb) in radix-8 register rounds (3 stages per round) through
+// swizzled shared memory.  FWD: Cooley-Tukey, high bit first.  INV: Gentleman-Sande, low bit first, values in [0,2q).
+// Forward laziness: T = shoup_lazy(Y) is < 2q for ANY 64-bit Y, so X' = X + T and Y' = X - T + 2q grow by at most
+// 2q per stage and need no correction while (1 + 2 log2 N) q < 2^64 (LAZY: q < 2^58); otherwise X is brought back
+// below 2q in every butterfly (Harvey), keeping values below 4q.
+// Indexing: a round's window [PW, PW+3) maps to contiguous global bits starting at gpw, so element k is global
+// j0 + (k << gpw), its stage-s twiddle is tw[((N + j0) >> (gpw+s+1)) + (k >> (s+1))], and, swz being XOR-linear, its
+// shared-memory slot is swz(ebase) ^ swz(k << PW): one base computation per thread and round.
+
+// compile-time round: window position and active stages [SLO, SHI) are constants (production geometries)
+template <bool FWD, bool LAZY, int PW, int SLO, int SHI>
+DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid) {
+  const int ebase = ((tid >> PW) << (PW + 3)) | (tid & ((1 << PW) - 1));
+  const int gpw = G.gbit(PW);
+  const u32 nj = (1u << G.logN) + G.gidx(ebase);
+  const ulonglong2 *twv = reinterpret_cast<const ulonglong2 *>(tw);
+  ulonglong2 t2 = make_ulonglong2(0, 0), t1[2], t0[4];
+  // twiddles first: their L2 latency overlaps the shared-memory loads
+  if (2 >= SLO && 2 < SHI) t2 = __ldg(twv + (nj >> (gpw + 3)));
+#pragma unroll
+  for (int i = 0; i < 2; i++) t1[i] = (1 >= SLO && 1 < SHI) ? __ldg(twv + (nj >> (gpw + 2)) + i) : t2;
+#pragma unroll
+  for (int i = 0; i < 4; i++) t0[i] = (0 >= SLO && 0 < SHI) ? __ldg(twv + (nj >> (gpw + 1)) + i) : t2;
+  const int sbase = swz(ebase);
   u64 x[8];
 #pragma unroll
-  for (int k = 0; k < 8; k++) x[k] = sm[swz(ebase | (k << pw))];
-  const u32 N = 1u << G.logN;
+  for (int k = 0; k < 8; k++) x[k] = sm[sbase ^ swz(k << PW)];
 #pragma unroll
   for (int ss = 0; ss < 3; ss++) {
     const int s = FWD ? 2 - ss : ss;
-    if (s < s_lo || s >= s_hi) continue;
-    const int g1 = G.gbit(pw + s) + 1;
+    if (s < SLO || s >= SHI) continue;
 #pragma unroll
     for (int k = 0; k < 8; k++) {
       if (k & (1 << s)) continue;
       const int k2 = k | (1 << s);
-      const u32 j = G.gidx(ebase | (k << pw));
-      const ShoupC w = tw[(N + j) >> g1];
+      const ulonglong2 w = s == 2 ? t2 : (s == 1 ? t1[k >> 2] : t0[k >> 1]);
+      if (FWD) {
+        const u64 X = LAZY ? x[k] : csub(x[k], q2);
+        const u64 T = shoup_lazy(x[k2], w.x, w.y, q);
+        x[k] = X + T;
+        x[k2] = X - T + q2;
+      } else {
+        const u64 U = x[k], V = x[k2];
+        x[k] = csub(U + V, q2);
+        x[k2] = shoup_lazy(U - V + q2, w.x, w.y, q);
+      }
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < 8; k++) sm[sbase ^ swz(k << PW)] = x[k];
+}
+
+template <bool FWD, bool LAZY, int LT, int LO, int NB, int DONE>
+DEVI void tile_rounds_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid) {
+  if constexpr (DONE < NB) {
+    constexpr int take = NB - DONE < 3 ? NB - DONE : 3;
+    constexpr int cur = FWD ? LO + NB - DONE : LO + DONE;         // FWD: exclusive top; INV: inclusive bottom
+    constexpr int p = FWD ? cur - take : cur;
+    constexpr int pw = p < LT - 3 ? p : LT - 3;
+    if (tid < (1 << (LT - 3))) tile_round_ct<FWD, LAZY, pw, p - pw, p - pw + take>(sm, G, tw, q, q2, tid);
+    __syncthreads();
+    tile_rounds_ct<FWD, LAZY, LT, LO, NB, DONE + take>(sm, G, tw, q, q2, tid);
+  }
+}
+
+// runtime round (toy ring degrees and any geometry without a compile-time instance)
+template <bool FWD>
+DEVI void tile_round_rt(u64 *sm, const TileGeo &G, int pw, int s_lo, int s_hi, const ShoupC *tw, u64 q, u64 q2, int tid) {
+  const int ebase = ((tid >> pw) << (pw + 3)) | (tid & ((1 << pw) - 1));
+  u64 x[8];
+#pragma unroll
+  for (int k = 0; k < 8; k++) x[k] = sm[swz(ebase | (k << pw))];
+  const u32 nj = (1u << G.logN) + G.gidx(ebase);
+  const int gpw = G.gbit(pw);
+#pragma unroll
+  for (int ss = 0; ss < 3; ss++) {
+    const int s = FWD ? 2 - ss : ss;
+    if (s < s_lo || s >= s_hi) continue;
+#pragma unroll
+    for (int k = 0; k < 8; k++) {
+      if (k & (1 << s)) continue;
+      const int k2 = k | (1 << s);
+      const ShoupC w = tw[(nj >> (gpw + s + 1)) + (k >> (s + 1))];
       if (FWD) {
         u64 X = csub(x[k], q2);
         u64 T = shoup_lazy(x[k2], w.c, w.cs, q);
@@ -98,30 +165,37 @@ DEVI void tile_round(u64 *sm, const TileGeo &G, int pw, int s_lo, int s_hi, cons
   for (int k = 0; k < 8; k++) sm[swz(ebase | (k << pw))] = x[k];
 }
 
-// All rounds of one pass over active tile bits [lo, lo+nb).  Every thread of the block must call this
-// (it synchronises); threads with tid >= 2^(lt-3) only take part in the barriers.
-template <bool FWD>
+// GEO selects the schedule: 0 = runtime (any lo/nb), 1 = row pass of 2048-element tiles with 8 stages,
+// 4..8 = column pass with GEO stages over tiles of 2^(GEO+4) elements (16 columns).
+// Every thread of the block must call this (it synchronises).  Outputs: forward < 33q (use fullred), inverse < 2q.
+template <bool FWD, int GEO>
 DEVI void tile_transform(u64 *sm, const TileGeo &G, int lo, int nb, const ShoupC *tw, u64 q, int tid) {
   const u64 q2 = q + q;
-  const bool active = tid < (1 << (G.lt - 3));
-  if (FWD) {
-    int cur = lo + nb;
-    while (cur > lo) {
-      int take = cur - lo < 3 ? cur - lo : 3;
-      int p = cur - take;
-      int pw = p < G.lt - 3 ? p : G.lt - 3;
-      if (active) tile_round<true>(sm, G, pw, p - pw, cur - pw, tw, q, q2, tid);
-      __syncthreads();
-      cur = p;
+  if constexpr (GEO == 0) {
+    const bool active = tid < (1 << (G.lt - 3));
+    if (FWD) {
+      int cur = lo + nb;
+      while (cur > lo) {
+        int take = cur - lo < 3 ? cur - lo : 3;
+        int p = cur - take;
+        int pw = p < G.lt - 3 ? p : G.lt - 3;
+        if (active) tile_round_rt<true>(sm, G, pw, p - pw, cur - pw, tw, q, q2, tid);
+        __syncthreads();
+        cur = p;
+      }
+    } else {
+      int cur = lo;
+      while (cur < lo + nb) {
+        int take = lo + nb - cur < 3 ? lo + nb - cur : 3;
+        int pw = cur < G.lt - 3 ? cur : G.lt - 3;
+        if (active) tile_round_rt<false>(sm, G, pw, cur - pw, cur + take - pw, tw, q, q2, tid);
+        __syncthreads();
+        cur += take;
+      }
     }
   } else {
-    int cur = lo;
-    while (cur < lo + nb) {
-      int take = lo + nb - cur < 3 ? lo + nb - cur : 3;
-      int pw = cur < G.lt - 3 ? cur : G.lt - 3;
-      if (active) tile_round<false>(sm, G, pw, cur - pw, cur + take - pw, tw, q, q2, tid);
-      __syncthreads();
-      cur += take;
-    }
+    constexpr int LT = GEO == 1 ? 11 : GEO + 4, LO = GEO == 1 ? 0 : 4, NB = GEO == 1 ? 8 : GEO;
+    if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
+    else tile_rounds_ct<FWD, false, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
   }
 }

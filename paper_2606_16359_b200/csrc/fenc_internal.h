@@ -21,6 +21,8 @@ struct ModConst {  // one per modulus, device global memory
   u64 qinv_neg;    // -q^{-1} mod 2^64 (Montgomery)
   u64 r2;          // 2^128 mod q: mont_mul(x, r2) = x 2^64 mod q
   u64 mask;        // 2^ceil(log2 q) - 1 (uniform rejection sampler)
+  u64 qbar;        // floor(2^64 / q): full reduction of a lazy 64-bit value
+  u64 pad[3];
 };
 
 struct ShoupC {  // constant c with its Shoup companion floor(c 2^64 / q)

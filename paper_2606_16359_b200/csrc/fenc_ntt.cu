@@ -9,6 +9,23 @@
 // The first touch of a forward transform and the last touch of either direction carry the fused work.
 #include "fenc_device.cuh"
 
+// geometry dispatch: row kernels GEO in {0,1}; column kernels GEO in {0,4..8} (fenc_device.cuh tile_transform)
+#define ROW_GEO(g, CALL)            \
+  do {                              \
+    if ((g).logN >= 12) { constexpr int GEO = 1; CALL; } \
+    else { constexpr int GEO = 0; CALL; }                \
+  } while (0)
+#define COL_GEO(g, CALL)                                   \
+  do {                                                     \
+    switch ((g).logN >= 12 ? (g).bcol : 0) {               \
+      case 4: { constexpr int GEO = 4; CALL; } break;      \
+      case 5: { constexpr int GEO = 5; CALL; } break;      \
+      case 6: { constexpr int GEO = 6; CALL; } break;      \
+      case 7: { constexpr int GEO = 7; CALL; } break;      \
+      case 8: { constexpr int GEO = 8; CALL; } break;      \
+      default: { constexpr int GEO = 0; CALL; } break;     \
+    }                                                      \
+  } while (0)
 static inline int nthreads_for(int lt) { int t = 1 << (lt - 3); return t < 32 ? 32 : t; }
 #define PROF(k, id, bytes) if ((k).prof) prof_begin((k).prof, (k).stream, id, (double)(bytes))
 #define LAUNCH_CHECK(k)                            \
@@ -24,7 +41,7 @@ struct InttRowP {
   const BatchItem *items; const u64 *src; size_t src_bstride; u64 *dst; size_t dst_bstride;
   const RowDesc *rows; const ModConst *mods; const ShoupC *tw; NttGeom g;
 };
-template <bool GATHER>
+template <bool GATHER, int GEO>
 __global__ void __launch_bounds__(256) intt_rowpass_kernel(InttRowP p) {
   extern __shared__ u64 sm[];
   const int tid = threadIdx.x, b = blockIdx.z;
@@ -39,7 +56,7 @@ __global__ void __launch_bounds__(256) intt_rowpass_kernel(InttRowP p) {
   }
   __syncthreads();
   const u64 q = p.mods[rd.mod].q;
-  tile_transform<false>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid);
+  tile_transform<false, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid);
   u64 *dst = p.dst + (size_t)b * p.dst_bstride + (size_t)rd.dst_row * N;
   for (int e = tid; e < T; e += blockDim.x) dst[G.gidx(e)] = sm[swz(e)];
 }
@@ -48,6 +65,7 @@ __global__ void __launch_bounds__(256) intt_rowpass_kernel(InttRowP p) {
 struct InttColP {
   u64 *dst; size_t dst_bstride; const RowDesc *rows; const ShoupC *scale; const ModConst *mods; const ShoupC *tw; NttGeom g;
 };
+template <int GEO>
 __global__ void __launch_bounds__(512) intt_colpass_kernel(InttColP p) {
   extern __shared__ u64 sm[];
   const int tid = threadIdx.x, b = blockIdx.z;
@@ -58,7 +76,7 @@ __global__ void __launch_bounds__(512) intt_colpass_kernel(InttColP p) {
   for (int e = tid; e < T; e += blockDim.x) sm[swz(e)] = dst[G.gidx(e)];
   __syncthreads();
   const u64 q = p.mods[rd.mod].q;
-  tile_transform<false>(sm, G, p.g.lc_col, p.g.bcol, p.tw + (size_t)rd.mod * N, q, tid);
+  tile_transform<false, GEO>(sm, G, p.g.lc_col, p.g.bcol, p.tw + (size_t)rd.mod * N, q, tid);
   const ShoupC sc = p.scale[blockIdx.y];
   for (int e = tid; e < T; e += blockDim.x) dst[G.gidx(e)] = shoup_mul(sm[swz(e)], sc.c, sc.cs, q);
 }
@@ -71,13 +89,13 @@ int k_intt(const KCtx &k, const BatchItem *items, const u64 *src, size_t src_bst
   InttRowP a{items, src, src_bstride, dst, dst_bstride, rows, k.d_mods, k.d_tw_inv, g};
   dim3 gridA(k.N >> g.lt_row, n_rows, n_batch);
   PROF(k, K_INTT_ROW, 16.0 * k.N * n_rows * n_batch);
-  if (gather) intt_rowpass_kernel<true><<<gridA, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(a);
-  else intt_rowpass_kernel<false><<<gridA, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(a);
+  if (gather) ROW_GEO(g, (intt_rowpass_kernel<true, GEO><<<gridA, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(a)));
+  else ROW_GEO(g, (intt_rowpass_kernel<false, GEO><<<gridA, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(a)));
   LAUNCH_CHECK(k);
   InttColP c{dst, dst_bstride, rows, scale, k.d_mods, k.d_tw_inv, g};
   dim3 gridB(k.N >> g.lt_col, n_rows, n_batch);
   PROF(k, K_INTT_COL, 16.0 * k.N * n_rows * n_batch);
-  intt_colpass_kernel<<<gridB, nthreads_for(g.lt_col), sizeof(u64) << g.lt_col, st>>>(c);
+  COL_GEO(g, (intt_colpass_kernel<GEO><<<gridB, nthreads_for(g.lt_col), sizeof(u64) << g.lt_col, st>>>(c)));
   LAUNCH_CHECK(k);
   return 0;
 }
@@ -87,7 +105,7 @@ struct NttColP {
   const u64 *src; size_t src_bstride; const u64 *bc; u64 *dst; size_t dst_bstride;
   const RowDesc *rows; const ModConst *mods; const ShoupC *tw; NttGeom g;
 };
-template <bool BCONV>
+template <bool BCONV, int GEO>
 __global__ void __launch_bounds__(512) ntt_colpass_kernel(NttColP p) {
   extern __shared__ u64 sm[];
   const int tid = threadIdx.x, b = blockIdx.z;
@@ -110,7 +128,7 @@ __global__ void __launch_bounds__(512) ntt_colpass_kernel(NttColP p) {
     for (int e = tid; e < T; e += blockDim.x) sm[swz(e)] = __ldg(src + G.gidx(e));
   }
   __syncthreads();
-  tile_transform<true>(sm, G, p.g.lc_col, p.g.bcol, p.tw + (size_t)rd.mod * N, mc.q, tid);
+  tile_transform<true, GEO>(sm, G, p.g.lc_col, p.g.bcol, p.tw + (size_t)rd.mod * N, mc.q, tid);
   u64 *dst = p.dst + (size_t)b * p.dst_bstride + (size_t)rd.dst_row * N;
   for (int e = tid; e < T; e += blockDim.x) dst[G.gidx(e)] = sm[swz(e)];  // lazy, in [0,4q)
 }
@@ -120,6 +138,7 @@ struct NttRowP {
   const u64 *src; size_t src_bstride; u64 *dst; size_t dst_bstride; const RowDesc *rows; const ModConst *mods;
   const ShoupC *tw; NttGeom g; int src_is_dst_row;
 };
+template <int GEO>
 __global__ void __launch_bounds__(256) ntt_rowpass_kernel(NttRowP p) {
   extern __shared__ u64 sm[];
   const int tid = threadIdx.x, b = blockIdx.z;
@@ -129,10 +148,10 @@ __global__ void __launch_bounds__(256) ntt_rowpass_kernel(NttRowP p) {
   const u64 *src = p.src + (size_t)b * p.src_bstride + (size_t)(p.src_is_dst_row ? rd.dst_row : rd.src_row) * N;
   for (int e = tid; e < T; e += blockDim.x) sm[swz(e)] = src[G.gidx(e)];
   __syncthreads();
-  const u64 q = p.mods[rd.mod].q;
-  tile_transform<true>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid);
+  const ModConst mc = p.mods[rd.mod];
+  tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, mc.q, tid);
   u64 *dst = p.dst + (size_t)b * p.dst_bstride + (size_t)rd.dst_row * N;
-  for (int e = tid; e < T; e += blockDim.x) dst[G.gidx(e)] = csub(csub(sm[swz(e)], q + q), q);
+  for (int e = tid; e < T; e += blockDim.x) dst[G.gidx(e)] = fullred(sm[swz(e)], mc.q, mc.qbar);
 }
 
 int k_ntt(const KCtx &k, const u64 *src, size_t src_bstride, u64 *dst, size_t dst_bstride, const RowDesc *rows, int n_rows,
@@ -143,12 +162,12 @@ int k_ntt(const KCtx &k, const u64 *src, size_t src_bstride, u64 *dst, size_t ds
   NttColP a{src, src_bstride, nullptr, dst, dst_bstride, rows, k.d_mods, k.d_tw_fwd, g};
   dim3 grid1(k.N >> g.lt_col, n_rows, n_batch);
   PROF(k, K_NTT_COL, 16.0 * k.N * n_rows * n_batch);
-  ntt_colpass_kernel<false><<<grid1, nthreads_for(g.lt_col), sizeof(u64) << g.lt_col, st>>>(a);
+  COL_GEO(g, (ntt_colpass_kernel<false, GEO><<<grid1, nthreads_for(g.lt_col), sizeof(u64) << g.lt_col, st>>>(a)));
   LAUNCH_CHECK(k);
   NttRowP r{dst, dst_bstride, dst, dst_bstride, rows, k.d_mods, k.d_tw_fwd, g, 1};
   dim3 grid2(k.N >> g.lt_row, n_rows, n_batch);
   PROF(k, K_NTT_ROW, 16.0 * k.N * n_rows * n_batch);
-  ntt_rowpass_kernel<<<grid2, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(r);
+  ROW_GEO(g, (ntt_rowpass_kernel<GEO><<<grid2, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(r)));
   LAUNCH_CHECK(k);
   return 0;
 }
@@ -161,7 +180,7 @@ int k_ntt_cols_bconv(const KCtx &k, const u64 *y, size_t y_bstride, const u64 *b
   dim3 grid1(k.N >> g.lt_col, n_rows, n_batch);
   // algorithmic bytes: every source row read once, every target row written once
   PROF(k, K_NTT_COL_BCONV, 8.0 * k.N * ((double)n_src_rows + n_rows) * n_batch);
-  ntt_colpass_kernel<true><<<grid1, nthreads_for(g.lt_col), sizeof(u64) << g.lt_col, (cudaStream_t)k.stream>>>(a);
+  COL_GEO(g, (ntt_colpass_kernel<true, GEO><<<grid1, nthreads_for(g.lt_col), sizeof(u64) << g.lt_col, (cudaStream_t)k.stream>>>(a)));
   LAUNCH_CHECK(k);
   return 0;
 }
@@ -175,8 +194,8 @@ struct KeyMacP {
   const BatchItem *items; const int *tmp_index; const u64 *tmp; size_t tmp_bstride; u64 *acc; size_t acc_bstride;
   const ModConst *mods; const ShoupC *tw; NttGeom g; int L, E, beta, A, nq, n_batch;
 };
-template <int EPT>  // elements per thread
-__global__ void __launch_bounds__(256) ntt_rows_keymac_kernel(KeyMacP p) {
+template <int EPT, int GEO>  // elements per thread
+__global__ void __launch_bounds__(256, 2) ntt_rows_keymac_kernel(KeyMacP p) {
   extern __shared__ u64 sm[];
   const int tid = threadIdx.x;
   // batch index fastest: blockIdx.x = tile * n_batch + b
@@ -198,7 +217,7 @@ __global__ void __launch_bounds__(256) ntt_rows_keymac_kernel(KeyMacP p) {
       const u64 *src = p.tmp + (size_t)b * p.tmp_bstride + (size_t)ti * N;
       for (int e = tid; e < T; e += nth) sm[swz(e)] = src[G.gidx(e)];
       __syncthreads();
-      tile_transform<true>(sm, G, 0, p.g.brow, p.tw + (size_t)mod * N, mc.q, tid);
+      tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)mod * N, mc.q, tid);
     }
 #pragma unroll
     for (int i = 0; i < EPT; i++) {
@@ -206,7 +225,7 @@ __global__ void __launch_bounds__(256) ntt_rows_keymac_kernel(KeyMacP p) {
       if (e < T) {
         const u32 jj = G.gidx(e);
         u64 x;
-        if (ti >= 0) x = csub(csub(sm[swz(e)], mc.q + mc.q), mc.q);
+        if (ti >= 0) x = fullred(sm[swz(e)], mc.q, mc.qbar);
         else x = __ldg(it.ks_in + (size_t)t * N + galois_src(jj, it.g, p.g.logN));
         mac128(a0l[i], a0h[i], x, __ldg(kb + jj));
         mac128(a1l[i], a1h[i], x, __ldg(ka + jj));
@@ -238,9 +257,10 @@ int k_ntt_rows_keymac(const KCtx &k, const BatchItem *items, int L, int E, int b
   const int ept = ((1 << g.lt_row) + nth - 1) / nth;
   // algorithmic bytes: ModUp temp + the switched polynomial read once, accumulators written once, each key once
   PROF(k, K_KEYMAC, 8.0 * k.N * (((double)n_up + L + 2.0 * E) * n_batch + 2.0 * beta * E * n_distinct_keys));
-  if (ept <= 1) ntt_rows_keymac_kernel<1><<<grid, nth, sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
-  else if (ept <= 4) ntt_rows_keymac_kernel<4><<<grid, nth, sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
-  else ntt_rows_keymac_kernel<8><<<grid, nth, sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
+  if (g.logN >= 12) ntt_rows_keymac_kernel<8, 1><<<grid, nth, sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
+  else if (ept <= 1) ntt_rows_keymac_kernel<1, 0><<<grid, nth, sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
+  else if (ept <= 4) ntt_rows_keymac_kernel<4, 0><<<grid, nth, sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
+  else ntt_rows_keymac_kernel<8, 0><<<grid, nth, sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
   LAUNCH_CHECK(k);
   return 0;
 }
@@ -251,6 +271,7 @@ struct DivideP {
   const BatchItem *items; const u64 *tmp; size_t tmp_bstride; const u64 *acc; size_t acc_bstride; const ShoupC *mul;
   const RowDesc *rows; const ModConst *mods; const ShoupC *tw; NttGeom g; int from_items;
 };
+template <int GEO>
 __global__ void __launch_bounds__(256) ntt_rows_divide_kernel(DivideP p) {
   extern __shared__ u64 sm[];
   const int tid = threadIdx.x, b = blockIdx.z;
@@ -260,8 +281,9 @@ __global__ void __launch_bounds__(256) ntt_rows_divide_kernel(DivideP p) {
   const u64 *src = p.tmp + (size_t)b * p.tmp_bstride + (size_t)rd.src_row * N;
   for (int e = tid; e < T; e += blockDim.x) sm[swz(e)] = src[G.gidx(e)];
   __syncthreads();
-  const u64 q = p.mods[rd.mod].q;
-  tile_transform<true>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid);
+  const ModConst mq = p.mods[rd.mod];
+  const u64 q = mq.q;
+  tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid);
   const BatchItem it = p.items[b];
   const u64 *minuend = (p.from_items ? it.sub_in : p.acc + (size_t)b * p.acc_bstride) + (size_t)rd.aux2 * N;
   const u64 *addend = rd.aux == 0 ? it.add0 : it.add1;
@@ -270,7 +292,7 @@ __global__ void __launch_bounds__(256) ntt_rows_divide_kernel(DivideP p) {
   u64 *dst = it.out + (size_t)rd.dst_row * N;
   for (int e = tid; e < T; e += blockDim.x) {
     const u32 j = G.gidx(e);
-    const u64 x = csub(csub(sm[swz(e)], q + q), q);
+    const u64 x = fullred(sm[swz(e)], q, mq.qbar);
     u64 v = shoup_mul(submod(__ldg(minuend + j), x, q), mc.c, mc.cs, q);
     if (addend) v = addmod(v, __ldg(addend + galois_src(j, it.g, p.g.logN)), q);
     dst[j] = v;
@@ -285,7 +307,7 @@ int k_ntt_rows_divide(const KCtx &k, const BatchItem *items, const u64 *tmp, siz
   DivideP p{items, tmp, tmp_bstride, acc, acc_bstride, mul, rows, k.d_mods, k.d_tw_fwd, g, minuend_from_items ? 1 : 0};
   dim3 grid(k.N >> g.lt_row, n_rows, n_batch);
   PROF(k, K_DIVIDE, 8.0 * k.N * (3.5 * n_rows) * n_batch);  // temp + minuend + output, addend on half the rows
-  ntt_rows_divide_kernel<<<grid, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
+  ROW_GEO(g, (ntt_rows_divide_kernel<GEO><<<grid, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p)));
   LAUNCH_CHECK(k);
   return 0;
 }
