@@ -3,6 +3,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstring>
+#include <functional>
 #include <set>
 
 #include "fenc_ctx.h"
@@ -275,31 +276,49 @@ extern "C" fenc_status fenc_wts_keys(fenc_ctx *ctx, const fenc_conv_desc *cd, co
   return FENC_OK;
 }
 
-static fenc_status make_wts(fenc_ctx *ctx, const ConvGraph &g, const double *w, const int64_t *coeffs, uint32_t n_limbs,
-                            double scale, fenc_wts **out) {
+static u64 fnv64(const void *data, size_t n, u64 h) {
+  const unsigned char *p = (const unsigned char *)data;
+  for (size_t i = 0; i < n; i++) h = (h ^ p[i]) * 0x100000001B3ull;
+  return h;
+}
+// Encodes (or takes pre-encoded) every weight plaintext; plaintexts with identical coefficients are stored once
+// (content deduplication: in the large-batch layouts the same masked constant serves several fragments).
+static fenc_status make_wts(fenc_ctx *ctx, size_t n, const std::function<void(size_t, std::vector<double> &)> &slots,
+                            const int64_t *coeffs, uint32_t n_limbs, double scale, fenc_wts **out) {
   if (n_limbs < 1 || (int)n_limbs > ctx->nq) return FENC_ERR_INVALID_ARG;
   const int L = n_limbs;
-  const size_t N = ctx->N, n = g.wkeys.size();
-  fenc_wts *W = new fenc_wts{ctx, L, scale > 0 ? scale : (double)ctx->mod[L - 1], n, nullptr, ""};  // A14: s_w = q_{L-1}
-  W->d_all = dalloc_t<u64>(ctx, n * L * N);
-  if (!W->d_all) {
-    delete W;
-    return fail(ctx, FENC_ERR_OOM, "weight plaintexts (%zu x %d limbs)", n, L);
-  }
+  const size_t N = ctx->N;
+  std::unique_ptr<fenc_wts> W(new fenc_wts{ctx, L, scale > 0 ? scale : (double)ctx->mod[L - 1], n});  // A14: s_w = q_{L-1}
+  W->slot.resize(n);
+  std::vector<std::vector<int64_t>> uniq;
+  std::map<std::pair<u64, u64>, int> seen;
   std::vector<double> vec;
   std::vector<int64_t> c(N);
   for (size_t i = 0; i < n; i++) {
     const int64_t *src = coeffs ? coeffs + i * N : c.data();
     if (!coeffs) {
-      g.weight_slots(g.wkeys[i], w, vec);
+      slots(i, vec);
       fh::encode_slots(ctx->logN, vec.data(), nullptr, W->scale, c.data());
     }
-    fenc_status st = coeffs_to_mont(ctx, src, L, W->d_all + i * L * N);
+    std::pair<u64, u64> key{fnv64(src, N * 8, 0xcbf29ce484222325ull), fnv64(src, N * 8, 0x9E3779B97F4A7C15ull)};
+    auto it = seen.find(key);
+    if (it != seen.end() && memcmp(uniq[it->second].data(), src, N * 8) == 0) {
+      W->slot[i] = it->second;
+    } else {
+      W->slot[i] = (int)uniq.size();
+      if (it == seen.end()) seen[key] = (int)uniq.size();
+      uniq.emplace_back(src, src + N);
+    }
+  }
+  W->n_unique = uniq.size();
+  W->d_all = dalloc_t<u64>(ctx, W->n_unique * L * N);
+  if (!W->d_all) return fail(ctx, FENC_ERR_OOM, "weight plaintexts (%zu x %d limbs)", W->n_unique, L);
+  for (size_t i = 0; i < uniq.size(); i++) {
+    fenc_status st = coeffs_to_mont(ctx, uniq[i].data(), L, W->d_all + i * L * N);
     if (st != FENC_OK) return st;
-    if (!coeffs && cudaStreamSynchronize(ctx->stream) != cudaSuccess) return FENC_ERR_CUDA;  // c is reused
   }
   if (cudaStreamSynchronize(ctx->stream) != cudaSuccess) return FENC_ERR_CUDA;
-  *out = W;
+  *out = W.release();
   return FENC_OK;
 }
 extern "C" fenc_status fenc_conv_weights(fenc_ctx *ctx, const fenc_conv_desc *cd, const fenc_layout *lay, const double *w,
@@ -307,7 +326,10 @@ extern "C" fenc_status fenc_conv_weights(fenc_ctx *ctx, const fenc_conv_desc *cd
   if (!ctx || !cd || !w || !out) return FENC_ERR_INVALID_ARG;
   std::shared_ptr<ConvGraph> g;
   fenc_status st = graph_for(ctx, cd, lay, g);
-  return st != FENC_OK ? st : make_wts(ctx, *g, w, nullptr, n_limbs, scale, out);
+  if (st != FENC_OK) return st;
+  const ConvGraph *gp = g.get();
+  return make_wts(ctx, gp->wkeys.size(), [gp, w](size_t i, std::vector<double> &v) { gp->weight_slots(gp->wkeys[i], w, v); }, nullptr,
+                  n_limbs, scale, out);
 }
 extern "C" fenc_status fenc_conv_weights_from_coeffs(fenc_ctx *ctx, const fenc_conv_desc *cd, const fenc_layout *lay,
                                                      const int64_t *coeffs, size_t n, uint32_t n_limbs, double scale,
@@ -317,7 +339,7 @@ extern "C" fenc_status fenc_conv_weights_from_coeffs(fenc_ctx *ctx, const fenc_c
   fenc_status st = graph_for(ctx, cd, lay, g);
   if (st != FENC_OK) return st;
   if (n != g->wkeys.size()) return fail(ctx, FENC_ERR_MISMATCH, "expected %zu weight plaintexts, got %zu", g->wkeys.size(), n);
-  return make_wts(ctx, *g, nullptr, coeffs, n_limbs, scale, out);
+  return make_wts(ctx, n, nullptr, coeffs, n_limbs, scale, out);
 }
 extern "C" void fenc_wts_free(fenc_wts *W) {
   if (!W) return;
@@ -384,9 +406,7 @@ extern "C" fenc_status fenc_hconv(fenc_ctx *ctx, const fenc_keys *K, const fenc_
     res[i] = new_ct(ctx, do_rescale ? L - 1 : L, do_rescale ? s_acc / (double)ctx->mod[L - 1] : s_acc);
     if (!res[i]) return fail(ctx, FENC_ERR_OOM, "hconv outputs");
   }
-  std::vector<const u64 *> term_ct, term_pt;
-  std::vector<int> start{0};
-  std::vector<u64 *> mac_out;
+  MacJob job;
   std::vector<const u64 *> rot_in, sum_terms;
   std::vector<u64 *> rot_out, sum_out;
   std::vector<int> rot_step, sum_start{0};
@@ -398,12 +418,11 @@ extern "C" fenc_status fenc_hconv(fenc_ctx *ctx, const fenc_keys *K, const fenc_
       const bool single = oc.diags.size() == 1 && oc.diags[0] == 0;
       for (size_t k = 0; k < oc.diags.size(); k++) {
         u64 *P = single ? Y : Pbuf + (pi++) * CT;
-        for (const Term &t : oc.terms[k]) {
-          term_ct.push_back(t.amt ? Rbuf + (bg * n_inner + g.inner_index.at({t.src, t.amt})) * CT : in[bg * nin_bg + t.src]->d);
-          term_pt.push_back(W->d_all + (size_t)t.w * L * N);
-        }
-        start.push_back((int)term_ct.size());
-        mac_out.push_back(P);
+        job.terms.emplace_back();
+        for (const Term &t : oc.terms[k])
+          job.terms.back().push_back({t.amt ? Rbuf + (bg * n_inner + g.inner_index.at({t.src, t.amt})) * CT : in[bg * nin_bg + t.src]->d,
+                                      W->d_all + (size_t)W->slot[t.w] * L * N});
+        job.outs.push_back(P);
         if (single) continue;
         if (oc.diags[k] == 0) sum_terms.push_back(P);
         else {
@@ -414,15 +433,8 @@ extern "C" fenc_status fenc_hconv(fenc_ctx *ctx, const fenc_keys *K, const fenc_
       }
       if (!single) sum_start.push_back((int)sum_terms.size()), sum_out.push_back(Y);
     }
-  {
-    DescStage ds(ctx);
-    size_t o0 = ds.add(term_ct), o1 = ds.add(term_pt), o2 = ds.add(start), o3 = ds.add(mac_out);
-    char *base = ds.commit();
-    if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
-    CUDA_OK(ctx, k_mac(ctx->k, (const u64 *const *)(base + o0), (const u64 *const *)(base + o1), (const int *)(base + o2),
-                       (u64 *const *)(base + o3), (int)mac_out.size(), L, ctx->max_lazy,
-                       mac_alg_bytes(ctx, term_ct, term_pt, mac_out.size(), L)));
-  }
+  st = run_mac(ctx, job, L);
+  if (st != FENC_OK) return st;
   // ---- 3. outer rotations, 4. sums
   st = rotate_raw(ctx, K, L, rot_in, rot_step, rot_out);
   if (st != FENC_OK) return st;
@@ -478,17 +490,13 @@ extern "C" fenc_status fenc_compress(fenc_ctx *ctx, const fenc_keys *K, fenc_ct 
     s_mid = s_in * mask->scale;
     Mbuf = dalloc_t<u64>(ctx, n_in * CT);
     if (!Mbuf) return fail(ctx, FENC_ERR_OOM, "compress masked sources");
-    std::vector<const u64 *> tc(n_in), tp(n_in, mask->d_mont);
-    std::vector<int> start(n_in + 1);
-    std::vector<u64 *> outs(n_in);
-    for (size_t i = 0; i < n_in; i++) tc[i] = in[i]->d, start[i] = (int)i, outs[i] = Mbuf + i * CT;
-    start[n_in] = (int)n_in;
-    DescStage ds(ctx);
-    size_t o0 = ds.add(tc), o1 = ds.add(tp), o2 = ds.add(start), o3 = ds.add(outs);
-    char *base = ds.commit();
-    if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
-    CUDA_OK(ctx, k_mac(ctx->k, (const u64 *const *)(base + o0), (const u64 *const *)(base + o1), (const int *)(base + o2),
-                       (u64 *const *)(base + o3), (int)n_in, L, ctx->max_lazy, mac_alg_bytes(ctx, tc, tp, n_in, L)));
+    MacJob job;
+    for (size_t i = 0; i < n_in; i++) {
+      job.terms.push_back({{in[i]->d, mask->d_mont}});
+      job.outs.push_back(Mbuf + i * CT);
+    }
+    st = run_mac(ctx, job, L);
+    if (st != FENC_OK) return st;
   }
   u64 *Rbuf = dalloc_t<u64>(ctx, n_terms * CT);
   u64 *Ybuf = do_rescale ? dalloc_t<u64>(ctx, n_out * CT) : nullptr;

@@ -95,8 +95,9 @@ struct fenc_wts {
   int L;
   double scale;
   size_t n;
-  u64 *d_all = nullptr;  // [n][L][N] NTT domain, Montgomery form, fenc_wts_keys order
-  std::string graph_key;
+  size_t n_unique = 0;
+  std::vector<int> slot;  // weight index (fenc_wts_keys order) -> storage slot; identical plaintexts share one
+  u64 *d_all = nullptr;  // [n_unique][L][N] NTT domain, Montgomery form
 };
 
 // ---------------------------------------------------------------- helpers (fenc_ctx.cu)
@@ -147,5 +148,11 @@ fenc_status rotate_raw(fenc_ctx *ctx, const fenc_keys *keys, int L, const std::v
                        const std::vector<int> &steps, const std::vector<u64 *> &out);
 u32 galois_elt(const fenc_ctx *ctx, int step);
 fenc_status pt_device(fenc_ctx *ctx, fenc_pt *pt);  // ensure pt->d_mont
+// Builds the grouped MAC launch from per-output term lists (ct pointer, pt pointer) and enqueues it.
+struct MacJob {
+  std::vector<std::vector<std::pair<const u64 *, const u64 *>>> terms;  // per output
+  std::vector<u64 *> outs;
+};
+fenc_status run_mac(fenc_ctx *ctx, const MacJob &job, int L);
 double mac_alg_bytes(fenc_ctx *ctx, const std::vector<const u64 *> &tc, const std::vector<const u64 *> &tp, size_t n_out, int L);
 fenc_status coeffs_to_mont(fenc_ctx *ctx, const int64_t *coeffs_host, int L, u64 *d_out);

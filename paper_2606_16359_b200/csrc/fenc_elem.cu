@@ -15,49 +15,83 @@
 static inline cudaStream_t S(const KCtx &k) { return (cudaStream_t)k.stream; }
 
 // ------------------------------------------------------------------------------------------------ MAC (a7)
-// outs[o][c][l][n] = sum_t ct_t[c][l][n] * pt_t[l][n]; products accumulate in 128 bits and are reduced once per
-// max_lazy terms (max_lazy = floor(2^64 / q_max) keeps the accumulator below q 2^64).
+// A group = up to G outputs that read the SAME ciphertext sequence with different plaintexts (the output channel
+// groups of one fragment and diagonal): each ciphertext word is loaded once and multiplied into G accumulators
+// (register tiling), each plaintext word is read once.  out[i][c][l][n] = sum_t ct_t[c][l][n] * pt_{i,t}[l][n];
+// products accumulate in 128 bits and are reduced once per max_lazy terms (max_lazy = floor(2^64 / q_max) keeps the
+// accumulator below q 2^64).  Blocks of one coefficient chunk are adjacent across groups (blockIdx.x = group), so
+// plaintexts shared by neighbouring groups (deduplicated weights) are served from L2.
 struct MacP {
-  const u64 *const *term_ct; const u64 *const *term_pt; const int *start; u64 *const *outs; const ModConst *mods;
+  const MacGroup *groups; const u64 *const *term_ct; const u64 *const *term_pt; u64 *const *outs; const ModConst *mods;
   int L, logN, max_lazy;
 };
-__global__ void __launch_bounds__(256) mac_kernel(MacP p) {
+#define MAC_TILE 64  // terms whose pointers are staged in shared memory at a time
+template <int G>
+__global__ void __launch_bounds__(256, 3) mac_kernel(MacP p) {
+  __shared__ const u64 *s_ct[MAC_TILE];
+  __shared__ const u64 *s_pt[G][MAC_TILE];
   const size_t LN = (size_t)p.L << p.logN;
-  const size_t idx = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) * 2;
-  if (idx >= LN) return;
-  const int o = blockIdx.y;
-  const ModConst mc = p.mods[idx >> p.logN];
-  const int t0 = p.start[o], t1 = p.start[o + 1];
-  u64 r00 = 0, r01 = 0, r10 = 0, r11 = 0;  // reduced running sums [comp][elem]
-  u64 l00 = 0, h00 = 0, l01 = 0, h01 = 0, l10 = 0, h10 = 0, l11 = 0, h11 = 0;
+  const size_t idx = (size_t)blockIdx.y * blockDim.x + threadIdx.x;  // LN is a multiple of 256 or the guard below holds
+  const bool live = idx < LN;
+  const MacGroup g = p.groups[blockIdx.x];
+  const ModConst mc = p.mods[(live ? idx : 0) >> p.logN];
+  u64 lo0[G], hi0[G], lo1[G], hi1[G], r0[G], r1[G];
+#pragma unroll
+  for (int i = 0; i < G; i++) lo0[i] = hi0[i] = lo1[i] = hi1[i] = r0[i] = r1[i] = 0;
   int lazy = 0;
-  for (int t = t0; t < t1; t++) {
-    const u64 *c = p.term_ct[t];
-    const ulonglong2 w = __ldg(reinterpret_cast<const ulonglong2 *>(p.term_pt[t] + idx));
-    const ulonglong2 x0 = __ldg(reinterpret_cast<const ulonglong2 *>(c + idx));
-    const ulonglong2 x1 = __ldg(reinterpret_cast<const ulonglong2 *>(c + LN + idx));
-    mac128(l00, h00, x0.x, w.x); mac128(l01, h01, x0.y, w.y);
-    mac128(l10, h10, x1.x, w.x); mac128(l11, h11, x1.y, w.y);
-    if (++lazy == p.max_lazy) {
-      r00 = addmod(r00, mont_redc(l00, h00, mc.q, mc.qinv_neg), mc.q); r01 = addmod(r01, mont_redc(l01, h01, mc.q, mc.qinv_neg), mc.q);
-      r10 = addmod(r10, mont_redc(l10, h10, mc.q, mc.qinv_neg), mc.q); r11 = addmod(r11, mont_redc(l11, h11, mc.q, mc.qinv_neg), mc.q);
-      l00 = h00 = l01 = h01 = l10 = h10 = l11 = h11 = 0; lazy = 0;
+  for (int t0 = 0; t0 < g.n_terms; t0 += MAC_TILE) {
+    const int nt = g.n_terms - t0 < MAC_TILE ? g.n_terms - t0 : MAC_TILE;
+    __syncthreads();
+    for (int j = threadIdx.x; j < nt * (G + 1); j += blockDim.x) {
+      const int i = j / nt, t = j - i * nt;
+      if (i == 0) s_ct[t] = p.term_ct[g.ct_start + t0 + t];
+      else if (i - 1 < g.n_out) s_pt[i - 1][t] = p.term_pt[g.pt_start + (i - 1) * g.n_terms + t0 + t];
+      else s_pt[i - 1][t] = p.term_pt[g.pt_start + t0 + t];  // unused lanes of a short group: any valid pointer
+    }
+    __syncthreads();
+    if (!live) continue;
+#pragma unroll 2
+    for (int t = 0; t < nt; t++) {
+      const u64 *c = s_ct[t];
+      const u64 x0 = __ldg(c + idx), x1 = __ldg(c + LN + idx);
+      u64 w[G];
+#pragma unroll
+      for (int i = 0; i < G; i++) w[i] = __ldg(s_pt[i][t] + idx);
+#pragma unroll
+      for (int i = 0; i < G; i++) {
+        mac128(lo0[i], hi0[i], x0, w[i]);
+        mac128(lo1[i], hi1[i], x1, w[i]);
+      }
+      if (++lazy == p.max_lazy) {
+#pragma unroll
+        for (int i = 0; i < G; i++) {
+          r0[i] = addmod(r0[i], mont_redc(lo0[i], hi0[i], mc.q, mc.qinv_neg), mc.q);
+          r1[i] = addmod(r1[i], mont_redc(lo1[i], hi1[i], mc.q, mc.qinv_neg), mc.q);
+          lo0[i] = hi0[i] = lo1[i] = hi1[i] = 0;
+        }
+        lazy = 0;
+      }
     }
   }
-  r00 = addmod(r00, mont_redc(l00, h00, mc.q, mc.qinv_neg), mc.q); r01 = addmod(r01, mont_redc(l01, h01, mc.q, mc.qinv_neg), mc.q);
-  r10 = addmod(r10, mont_redc(l10, h10, mc.q, mc.qinv_neg), mc.q); r11 = addmod(r11, mont_redc(l11, h11, mc.q, mc.qinv_neg), mc.q);
-  u64 *out = p.outs[o];
-  *reinterpret_cast<ulonglong2 *>(out + idx) = make_ulonglong2(r00, r01);
-  *reinterpret_cast<ulonglong2 *>(out + LN + idx) = make_ulonglong2(r10, r11);
+  if (!live) return;
+#pragma unroll
+  for (int i = 0; i < G; i++) {
+    if (i < g.n_out) {
+      u64 *out = p.outs[g.out_start + i];
+      out[idx] = addmod(r0[i], mont_redc(lo0[i], hi0[i], mc.q, mc.qinv_neg), mc.q);
+      out[LN + idx] = addmod(r1[i], mont_redc(lo1[i], hi1[i], mc.q, mc.qinv_neg), mc.q);
+    }
+  }
 }
-int k_mac(const KCtx &k, const u64 *const *term_ct, const u64 *const *term_pt, const int *start, u64 *const *outs, int n_out,
-          int L, int max_lazy, double alg_bytes) {
-  if (n_out == 0) return 0;
-  MacP p{term_ct, term_pt, start, outs, k.d_mods, L, k.geom.logN, max_lazy};
-  size_t pairs = ((size_t)L * k.N) / 2;
-  dim3 grid((unsigned)((pairs + 255) / 256), n_out);
+int k_mac(const KCtx &k, const MacGroup *groups, int n_groups, int max_group, const u64 *const *term_ct, const u64 *const *term_pt,
+          u64 *const *outs, int L, int max_lazy, double alg_bytes) {
+  if (n_groups == 0) return 0;
+  MacP p{groups, term_ct, term_pt, outs, k.d_mods, L, k.geom.logN, max_lazy};
+  dim3 grid(n_groups, (unsigned)(((size_t)L * k.N + 255) / 256));
   PROF(k, K_MAC, alg_bytes);
-  mac_kernel<<<grid, 256, 0, S(k)>>>(p);
+  if (max_group <= 1) mac_kernel<1><<<grid, 256, 0, S(k)>>>(p);
+  else if (max_group <= 2) mac_kernel<2><<<grid, 256, 0, S(k)>>>(p);
+  else mac_kernel<4><<<grid, 256, 0, S(k)>>>(p);
   LAUNCH_CHECK(k);
   return 0;
 }

@@ -39,6 +39,11 @@ struct RowDesc {
   int pad[3];
 };
 
+#define FENC_MAC_GROUP 4
+struct MacGroup {
+  int n_out, n_terms, ct_start, pt_start, out_start, pad[3];
+};
+
 // one element of a batch of key switches (rotations, relinearisations, rescales)
 struct BatchItem {
   const u64 *ks_in;  // polynomial to switch [L][N] (NTT domain); rotation: c1 of the input
@@ -105,9 +110,10 @@ int k_ntt_rows_keymac(const KCtx &k, const BatchItem *items, int L, int E, int b
 int k_ntt_rows_divide(const KCtx &k, const BatchItem *items, const u64 *tmp, size_t tmp_bstride, const u64 *acc,
                       size_t acc_bstride, bool minuend_from_items, const ShoupC *mul, const RowDesc *rows, int n_rows,
                       int n_batch);
-// MAC (a7): outs[o] = sum_{t in [start[o], start[o+1])} ct[t] (*) pt[t]; ct [2][L][N], pt [L][N] Montgomery form
-int k_mac(const KCtx &k, const u64 *const *term_ct, const u64 *const *term_pt, const int *start, u64 *const *outs, int n_out,
-          int L, int max_lazy, double alg_bytes);
+// MAC (a7) over groups of outputs sharing one ciphertext sequence (register tiling, fenc_elem.cu):
+// out[out_start+i] = sum_{t<n_terms} ct[ct_start+t] (*) pt[pt_start + i*n_terms + t], i < n_out <= FENC_MAC_GROUP
+int k_mac(const KCtx &k, const MacGroup *groups, int n_groups, int max_group, const u64 *const *term_ct, const u64 *const *term_pt,
+          u64 *const *outs, int L, int max_lazy, double alg_bytes);
 // outs[o] = sum of listed [2][L][N] arrays
 int k_add_many(const KCtx &k, const u64 *const *term, const int *start, u64 *const *outs, int n_out, int L, int n_terms);
 // rows kernels: row r uses modulus row_mod[r] (device array)

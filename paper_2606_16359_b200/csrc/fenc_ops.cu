@@ -2,6 +2,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstring>
+#include <map>
 
 #include "fenc_ctx.h"
 
@@ -248,6 +249,46 @@ extern "C" void fenc_ct_free(fenc_ct *ct) {
 }
 
 // ------------------------------------------------------------------------------------------------ primitives
+// Groups outputs with identical ciphertext sequences (up to FENC_MAC_GROUP per group) and launches the MAC.
+fenc_status run_mac(fenc_ctx *ctx, const MacJob &job, int L) {
+  const size_t n = job.outs.size();
+  if (n == 0) return FENC_OK;
+  std::map<std::vector<const u64 *>, std::vector<int>> by_seq;
+  std::vector<std::vector<const u64 *>> order;  // first-appearance order keeps neighbouring fragments adjacent
+  for (size_t o = 0; o < n; o++) {
+    std::vector<const u64 *> seq(job.terms[o].size());
+    for (size_t t = 0; t < seq.size(); t++) seq[t] = job.terms[o][t].first;
+    auto it = by_seq.find(seq);
+    if (it == by_seq.end()) order.push_back(seq), by_seq[seq] = {(int)o};
+    else it->second.push_back((int)o);
+  }
+  std::vector<MacGroup> groups;
+  std::vector<const u64 *> tc, tp, all_c, all_p;
+  std::vector<u64 *> outs;
+  int max_group = 1;
+  for (auto &seq : order) {
+    const std::vector<int> &members = by_seq[seq];
+    for (size_t at = 0; at < members.size(); at += FENC_MAC_GROUP) {
+      const int ng = (int)std::min<size_t>(FENC_MAC_GROUP, members.size() - at);
+      MacGroup g{ng, (int)seq.size(), (int)tc.size(), (int)tp.size(), (int)outs.size(), {0, 0, 0}};
+      tc.insert(tc.end(), seq.begin(), seq.end());
+      for (int i = 0; i < ng; i++) {
+        const auto &tl = job.terms[members[at + i]];
+        for (auto &pr : tl) tp.push_back(pr.second);
+        outs.push_back(job.outs[members[at + i]]);
+      }
+      groups.push_back(g);
+      max_group = std::max(max_group, ng);
+    }
+  }
+  DescStage st(ctx);
+  size_t o0 = st.add(groups), o1 = st.add(tc), o2 = st.add(tp), o3 = st.add(outs);
+  char *base = st.commit();
+  if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
+  CUDA_OK(ctx, k_mac(ctx->k, (const MacGroup *)(base + o0), (int)groups.size(), max_group, (const u64 *const *)(base + o1),
+                     (const u64 *const *)(base + o2), (u64 *const *)(base + o3), L, ctx->max_lazy, mac_alg_bytes(ctx, tc, tp, n, L)));
+  return FENC_OK;
+}
 // algorithmic bytes of one MAC launch: every distinct ciphertext and plaintext read once, every output written once
 double mac_alg_bytes(fenc_ctx *ctx, const std::vector<const u64 *> &tc, const std::vector<const u64 *> &tp, size_t n_out, int L) {
   std::vector<const u64 *> a(tc), b(tp);
@@ -332,14 +373,12 @@ extern "C" fenc_status fenc_pmult_sum(fenc_ctx *ctx, fenc_ct *const *in, fenc_pt
   }
   fenc_ct *c = new_ct(ctx, L, in[0]->scale * pt[0]->scale);
   if (!c) return fail(ctx, FENC_ERR_OOM, "pmult");
-  std::vector<int> start{0, (int)n};
-  std::vector<u64 *> outs{c->d};
-  DescStage st(ctx);
-  size_t o0 = st.add(tc), o1 = st.add(tp), o2 = st.add(start), o3 = st.add(outs);
-  char *base = st.commit();
-  if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
-  CUDA_OK(ctx, k_mac(ctx->k, (const u64 *const *)(base + o0), (const u64 *const *)(base + o1), (const int *)(base + o2),
-                     (u64 *const *)(base + o3), 1, L, ctx->max_lazy, mac_alg_bytes(ctx, tc, tp, 1, L)));
+  MacJob job;
+  job.terms.resize(1);
+  for (size_t i = 0; i < n; i++) job.terms[0].push_back({tc[i], tp[i]});
+  job.outs.push_back(c->d);
+  fenc_status ms = run_mac(ctx, job, L);
+  if (ms != FENC_OK) return ms;
   *out = c;
   return FENC_OK;
 }
