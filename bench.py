@@ -95,7 +95,7 @@ WORKLOADS = {
     "cfg2_lenet5": ("cfg2", lambda bs, seed: lenet_layers(bs, seed, upto="fc"),
                     "BASELINE config 2: LeNet-5-shaped network, N=2^14, 8x40b+2x60b, dnum=4"),
 }
-DEFAULT_WORKLOAD = "cfg2_lenet5_convstage"
+DEFAULT_WORKLOAD = "cfg2_lenet5"
 
 
 def run_ours(args, rank, world):

@@ -180,6 +180,33 @@ fenc_status fenc_hconv(fenc_ctx *ctx, const fenc_keys *keys, const fenc_conv_des
                        const fenc_wts *wts, fenc_ct *const *in, size_t n_in, int do_rescale, fenc_ct **out,
                        size_t n_out_capacity, size_t *n_out);
 
+/* ------------------------------------------------------------------ FC by plain diagonals (a15; R2.12)
+ * The joint index p = cpos*m^2 + k in [0, P), P = (N/2)/B, is the position inside a ciphertext; input feature
+ * <-> (input ct c, p), neuron nu <-> (output ct c', p) with nu = c'*P + p;
+ *   out_{c'} = sum_d Rot( sum_c x_c (*) Wd(c',c,d), d*B ),  Wd(c',c,d)[p] = W[nu(c',(p-d) mod P)][feat(c,p)] or 0.
+ * Input features: in_C > 0: the S=1 fragment layout of a [BS][in_C][in_H][in_W] tensor in an in_M x in_M frame
+ * (PyTorch flatten order feat = channel*H*W + h*W + w); in_C = 0: the output layout of a previous fc (feat = c*P + p).
+ * B = min(next_pow2(BS), (N/2)/in_M^2) samples per ciphertext, as in the conv layouts it chains with. */
+typedef struct {
+  uint32_t BS, n_in, n_out;
+  uint32_t in_C, in_H, in_W, in_M;
+} fenc_fc_desc;
+typedef struct {
+  uint32_t B, P, BG, n_in_ct, n_out_ct, n_rot, n_pmult, n_distinct_pt, n_rot_keys;
+  int32_t rot_steps[512];
+} fenc_fc_info;
+fenc_status fenc_fc_plan(fenc_ctx *ctx, const fenc_fc_desc *fc, fenc_fc_info *out);
+/* keys (c_out_ct, c_in_ct, d) of the non-zero weight plaintexts, in the order the weight calls use */
+fenc_status fenc_fc_wts_keys(fenc_ctx *ctx, const fenc_fc_desc *fc, uint32_t *keys3, size_t capacity, size_t *n);
+/* host w[n_out][n_in] (fp64); scale <= 0: q_{L-1} (A14) */
+fenc_status fenc_fc_weights(fenc_ctx *ctx, const fenc_fc_desc *fc, const double *w, uint32_t n_limbs, double scale,
+                            fenc_wts **out);
+fenc_status fenc_fc_weights_from_coeffs(fenc_ctx *ctx, const fenc_fc_desc *fc, const int64_t *coeffs, size_t n,
+                                        uint32_t n_limbs, double scale, fenc_wts **out);
+/* in: n_in_ct*BG ciphertexts ordered [bg][c]; out: n_out_ct*BG ordered [bg][c'] */
+fenc_status fenc_fc(fenc_ctx *ctx, const fenc_keys *keys, const fenc_fc_desc *fc, const fenc_wts *wts, fenc_ct *const *in,
+                    size_t n_in, int do_rescale, fenc_ct **out, size_t n_out_capacity, size_t *n_out);
+
 /* ------------------------------------------------------------------ AAC compress (R2.11) */
 /* out[t] = sum over the terms with term_out[i] == t of Rot(mask (*) in[term_src[i]], term_rot[i]).
  * mask may be NULL (maskless mode, no level consumed); with a mask and do_rescale != 0 this is the paper's

@@ -1,0 +1,222 @@
+"""Layer-level oracle: FC by plain diagonals, square activation, 2x2 pooling by fragment selection, and a sequential
+network runner.  TEST INFRASTRUCTURE ONLY -- see oracle/__init__.py.
+
+Follows PAPER.md:284 ("stride is implemented simply by discarding the unused cts ... FC layers use diagonal-matrix
+multiplication", polynomial activation) with the readings R2.12 of DESIGN.md section 4.  As in oracle/fragment.py each
+graph runs (i) on plain slot vectors (rotation = cyclic shift), which pins it against a dense fp64 evaluation, and
+(ii) on oracle ciphertexts (oracle/ckks.py).
+"""
+from fractions import Fraction
+
+import numpy as np
+
+from . import fragment as fr
+
+
+# --------------------------------------------------------------------------- FC by plain diagonals (R2.12)
+class FcGraph:
+    """Position p = cpos*m^2 + k in [0, P), P = n/B.  Input feature <-> (input ct c, p); neuron nu <-> (output ct c', p),
+    nu = c'*P + p.  out_{c'} = sum_d Rot(sum_c x_c (*) Wd(c', c, d), d*B), Wd(c', c, d)[p] = W[nu(c', (p-d) mod P), feat(c, p)]
+    or 0 when either index is invalid; terms whose Wd is identically zero are skipped."""
+
+    def __init__(self, n, BS, n_in, n_out, in_C=0, in_H=0, in_W=0, in_M=1):
+        self.n, self.BS, self.n_in, self.n_out = n, BS, n_in, n_out
+        self.in_C, self.in_H, self.in_W, self.m = in_C, in_H, in_W, in_M
+        m2 = in_M * in_M
+        assert m2 <= n and n % m2 == 0
+        self.B = min(fr.next_pow2(BS), n // m2)
+        self.P = n // self.B
+        self.ch = n // (self.B * m2)
+        self.BG = -(-BS // self.B)
+        if in_C:
+            assert in_C * in_H * in_W == n_in
+            self.n_in_ct = -(-in_C // self.ch)
+        else:
+            self.n_in_ct = -(-n_in // self.P)
+        self.n_out_ct = -(-n_out // self.P)
+        self.terms = {}  # c' -> {d: [(c, wkey (c', c, d))]}
+        for co in range(self.n_out_ct):
+            diags = {}
+            for d in range(self.P):
+                lst = [(ci, (co, ci, d)) for ci in range(self.n_in_ct) if self.nonzero(co, ci, d)]
+                if lst:
+                    diags[d] = lst
+            self.terms[co] = diags
+
+    def feat(self, c, p):
+        """PyTorch flatten order channel*H*W + h*W + w through the S=1 layout, or c*P + p after a previous fc."""
+        if self.in_C:
+            m2 = self.m * self.m
+            cpos, k = divmod(p, m2)
+            chan, (h, w) = c * self.ch + cpos, divmod(k, self.m)
+            if chan >= self.in_C or h >= self.in_H or w >= self.in_W:
+                return -1
+            return (chan * self.in_H + h) * self.in_W + w
+        f = c * self.P + p
+        return f if f < self.n_in else -1
+
+    def neuron(self, c, p):
+        v = c * self.P + p
+        return v if v < self.n_out else -1
+
+    def nonzero(self, co, ci, d):
+        return any(self.feat(ci, p) >= 0 and self.neuron(co, (p - d) % self.P) >= 0 for p in range(self.P))
+
+    def weight_slots(self, wkey, W):
+        co, ci, d = wkey
+        vec = np.zeros(self.n)
+        for p in range(self.P):
+            f, v = self.feat(ci, p), self.neuron(co, (p - d) % self.P)
+            if f >= 0 and v >= 0:
+                vec[p * self.B:(p + 1) * self.B] = W[v, f]
+        return vec
+
+    def counts(self):
+        n_rot = sum(len([d for d in diags if d]) for diags in self.terms.values())
+        n_pm = sum(len(lst) for diags in self.terms.values() for lst in diags.values())
+        steps = sorted({d * self.B % self.n for diags in self.terms.values() for d in diags if d})
+        return dict(n_in_ct=self.n_in_ct * self.BG, n_out_ct=self.n_out_ct * self.BG, n_rot=n_rot * self.BG,
+                    n_pmult=n_pm * self.BG, n_distinct_pt=n_pm, rot_steps=steps)
+
+    def run(self, be, inputs, weights):
+        """inputs: list of n_in_ct items of ONE batch group; returns list of n_out_ct items."""
+        out = []
+        for co in range(self.n_out_ct):
+            y = None
+            for d in sorted(self.terms[co]):
+                acc = be.zero()
+                for ci, wkey in self.terms[co][d]:
+                    be.pmult_acc(acc, inputs[ci], weights[wkey])
+                pd = be.wrap(acc)
+                if d:
+                    pd = be.rot(pd, d * self.B % self.n)
+                y = pd if y is None else be.add(y, pd)
+            out.append(y)
+        return out
+
+    # gather / scatter of the feature vectors (host side of the layouts above)
+    def gather_in(self, X, c, bg):
+        """slot vector of input ciphertext c for X[BS][n_in]."""
+        vec = np.zeros(self.n)
+        for p in range(self.P):
+            f = self.feat(c, p)
+            if f < 0:
+                continue
+            for b in range(self.B):
+                bb = bg * self.B + b
+                if bb < self.BS:
+                    vec[p * self.B + b] = X[bb, f]
+        return vec
+
+    def scatter_out(self, Y, vec, c, bg):
+        for p in range(self.P):
+            v = self.neuron(c, p)
+            if v < 0:
+                continue
+            for b in range(self.B):
+                bb = bg * self.B + b
+                if bb < self.BS:
+                    Y[bb, v] = vec[p * self.B + b]
+
+
+def fc_counts(n, **kw):
+    return FcGraph(n, **kw).counts()
+
+
+def fc_slots(graph: FcGraph, X, W):
+    """The fc graph on plain slot vectors -> Y[BS][n_out] (pin: must equal X @ W.T)."""
+    be = fr.SlotBackend(graph.n)
+    Wp = {wk: graph.weight_slots(wk, W) for diags in graph.terms.values() for lst in diags.values() for _, wk in lst}
+    Y = np.zeros((graph.BS, graph.n_out))
+    for bg in range(graph.BG):
+        ins = [graph.gather_in(X, c, bg) for c in range(graph.n_in_ct)]
+        for c, y in enumerate(graph.run(be, ins, Wp)):
+            graph.scatter_out(Y, y, c, bg)
+    return Y
+
+
+def encode_fc_weights(ck, params, graph: FcGraph, W, L, scale_w=None):
+    sw = Fraction(params.q[L - 1]) if scale_w is None else Fraction(scale_w)
+    return {wk: ck.encode(params, graph.weight_slots(wk, W), L, sw)
+            for diags in graph.terms.values() for lst in diags.values() for _, wk in lst}
+
+
+def fc(ck, params, keys, graph: FcGraph, inputs, weights, do_rescale=True):
+    """inputs: list of Ciphertext of one batch group -> list of Ciphertext; one rescale per output (A13)."""
+    w0 = next(iter(weights.values()))
+    be = fr.CtBackend(ck, params, keys, inputs[0].L, inputs[0].scale, w0.scale)
+    outs = graph.run(be, inputs, weights)
+    return [ck.rescale(params, y) for y in outs] if do_rescale else outs
+
+
+# --------------------------------------------------------------------------- pooling by fragment selection (R2.12)
+def pool_order(n_ct, S):
+    """indices such that consecutive groups of four are the fragments (2uo+a, 2vo+b) of output fragment (uo, vo);
+    ciphertext order [bg][g][u][v] (pooling / stride keep or combine whole fragment ciphertexts)."""
+    idx = []
+    for base in range(0, n_ct, S * S):
+        for uo in range(S // 2):
+            for vo in range(S // 2):
+                idx += [base + (2 * uo + a) * S + (2 * vo + b) for a in range(2) for b in range(2)]
+    return idx
+
+
+def sum_pool(ck, params, cts, S):
+    """out(uo, vo) = sum_{a,b in {0,1}} in(2uo+a, 2vo+b): no rotation, no level; the factor 1/4 belongs to the next
+    linear layer's weights."""
+    order = pool_order(len(cts), S)
+    out = []
+    for i in range(0, len(order), 4):
+        y = cts[order[i]]
+        for j in order[i + 1:i + 4]:
+            y = ck.add(params, y, cts[j])
+        out.append(y)
+    return out
+
+
+# --------------------------------------------------------------------------- sequential network
+def run_network(ck, params, keys, layers, cts, L0):
+    """layers as in paper_2606_16359_b200.pipeline.Pipeline (dicts with op = conv / square / pool / fc and fp64 weights);
+    cts: oracle ciphertexts ordered [bg][g][u][v].  Returns (final ciphertext list, list of per-layer outputs)."""
+    L, S, trace = L0, None, []
+    for ly in layers:
+        if ly["op"] == "conv":
+            graph = fr.ConvGraph(fr.ConvDesc(S=ly["S"], **ly["conv"]), params.n)
+            W = fr.encode_weights(ck, params, graph, ly["w"], L)
+            per = graph.S * graph.S * graph.lin.G
+            out = []
+            for bg in range(graph.lin.BG):
+                ins = {(u, v, g): cts[bg * per + (g * graph.S + u) * graph.S + v]
+                       for g in range(graph.lin.G) for u in range(graph.S) for v in range(graph.S)}
+                o = fr.hconv(ck, params, keys, graph, ins, W)
+                So = graph.S_out
+                out += [o[(uo, vo, go)] for go in range(graph.lout.G) for uo in range(So) for vo in range(So)]
+            cts, S, L = out, graph.S_out, L - 1
+        elif ly["op"] == "fc":
+            graph = FcGraph(params.n, **ly["fc"])
+            W = encode_fc_weights(ck, params, graph, ly["w"], L)
+            out = []
+            for bg in range(graph.BG):
+                out += fc(ck, params, keys, graph, cts[bg * graph.n_in_ct:(bg + 1) * graph.n_in_ct], W)
+            cts, S, L = out, 1, L - 1
+        elif ly["op"] == "square":
+            cts, L = [ck.square_relin(params, keys, c) for c in cts], L - 1
+        elif ly["op"] == "pool":
+            cts, S = sum_pool(ck, params, cts, S), S // 2
+        else:
+            raise ValueError(ly["op"])
+        trace.append(cts)
+    return cts, trace
+
+
+def network_rot_steps(layers, n):
+    """every rotation amount the network needs, and whether it needs the relinearisation key."""
+    steps, relin = set(), False
+    for ly in layers:
+        if ly["op"] == "conv":
+            steps.update(fr.ConvGraph(fr.ConvDesc(S=ly["S"], **ly["conv"]), n).counts()["rot_steps"])
+        elif ly["op"] == "fc":
+            steps.update(FcGraph(n, **ly["fc"]).counts()["rot_steps"])
+        elif ly["op"] == "square":
+            relin = True
+    return sorted(steps), relin

@@ -2,5 +2,5 @@
 convolution layer over fragment-encoded ciphertexts, as hand-written CUDA kernels behind the C ABI of include/fenc.h.
 
 `binding` is argument marshalling only.  There is no CPU fallback and nothing here imports oracle/."""
-from .binding import (Ciphertext, Context, ConvDesc, FencError, Keys, Layout, ParamsDesc, Plaintext, RELIN_KEY_ID,  # noqa: F401
+from .binding import (Ciphertext, Context, ConvDesc, FcDesc, FcInfo, FencError, Keys, Layout, ParamsDesc, Plaintext, RELIN_KEY_ID,  # noqa: F401
                       SYMBOLS, Weights, load_library)

@@ -35,6 +35,15 @@ class ConvDesc(C.Structure):
                 ("S", C.c_uint32), ("M", C.c_uint32)]
 
 
+class FcDesc(C.Structure):
+    _fields_ = [(k, C.c_uint32) for k in ("BS", "n_in", "n_out", "in_C", "in_H", "in_W", "in_M")]
+
+
+class FcInfo(C.Structure):
+    _fields_ = [(k, C.c_uint32) for k in ("B", "P", "BG", "n_in_ct", "n_out_ct", "n_rot", "n_pmult", "n_distinct_pt",
+                                          "n_rot_keys")] + [("rot_steps", C.c_int32 * 512)]
+
+
 class Layout(C.Structure):
     _fields_ = [(k, C.c_uint32) for k in ("S", "S_out", "M", "M_out", "m", "B", "ch", "cs", "G_in", "G_out", "BG",
                                           "H_out", "W_out", "n_in_ct", "n_out_ct", "n_inner_rot", "n_outer_rot",
@@ -53,7 +62,8 @@ SYMBOLS = ["fenc_params_init", "fenc_ctx_free", "fenc_last_error", "fenc_get_pri
            "fenc_ct_free", "fenc_rotate", "fenc_rescale", "fenc_add", "fenc_pmult_sum", "fenc_square_relin",
            "fenc_wts_keys", "fenc_conv_weights", "fenc_conv_weights_from_coeffs", "fenc_wts_free", "fenc_hconv",
            "fenc_compress", "fenc_ntt_rows", "fenc_launch_count", "fenc_device_bytes", "fenc_sum_groups",
-           "fenc_profile_enable", "fenc_profile_kernels", "fenc_profile_name", "fenc_profile_read"]
+           "fenc_profile_enable", "fenc_profile_kernels", "fenc_profile_name", "fenc_profile_read", "fenc_fc_plan",
+           "fenc_fc_wts_keys", "fenc_fc_weights", "fenc_fc_weights_from_coeffs", "fenc_fc"]
 
 _lib = None
 
@@ -101,6 +111,11 @@ def load_library(path=None):
                                           C.c_double, vpp],
         "fenc_hconv": [vp, vp, C.POINTER(ConvDesc), C.POINTER(Layout), vp, vpp, C.c_size_t, C.c_int, vpp, C.c_size_t,
                        C.POINTER(C.c_size_t)],
+        "fenc_fc_plan": [vp, C.POINTER(FcDesc), C.POINTER(FcInfo)],
+        "fenc_fc_wts_keys": [vp, C.POINTER(FcDesc), u32p, C.c_size_t, C.POINTER(C.c_size_t)],
+        "fenc_fc_weights": [vp, C.POINTER(FcDesc), dp, C.c_uint32, C.c_double, vpp],
+        "fenc_fc_weights_from_coeffs": [vp, C.POINTER(FcDesc), i64p, C.c_size_t, C.c_uint32, C.c_double, vpp],
+        "fenc_fc": [vp, vp, C.POINTER(FcDesc), vp, vpp, C.c_size_t, C.c_int, vpp, C.c_size_t, C.POINTER(C.c_size_t)],
         "fenc_compress": [vp, vp, vpp, C.c_size_t, vp, u32p, u32p, i32p, C.c_size_t, C.c_int, vpp, C.c_size_t],
         "fenc_ntt_rows": [vp, vp, i32p, C.c_size_t, C.c_int],
     }
@@ -418,6 +433,46 @@ class Context:
         n = C.c_size_t()
         self._ck(self.lib.fenc_hconv(self.h, keys.h, C.byref(conv), C.byref(lay), wts.h, self._harr(cts), len(cts),
                                      int(do_rescale), out, cap, C.byref(n)))
+        return [Ciphertext(self, C.c_void_p(out[i])) for i in range(n.value)]
+
+    # ---- FC by plain diagonals
+    def fc_desc(self, BS, n_in, n_out, in_C=0, in_H=0, in_W=0, in_M=1):
+        return FcDesc(BS, n_in, n_out, in_C, in_H, in_W, in_M)
+
+    def fc_plan(self, fc):
+        info = FcInfo()
+        self._ck(self.lib.fenc_fc_plan(self.h, C.byref(fc), C.byref(info)))
+        d = {k: int(getattr(info, k)) for k, _ in FcInfo._fields_ if k != "rot_steps"}
+        d["rot_steps"] = [int(info.rot_steps[i]) for i in range(info.n_rot_keys)]
+        return d
+
+    def fc_wts_keys(self, fc):
+        n = C.c_size_t()
+        self._ck(self.lib.fenc_fc_wts_keys(self.h, C.byref(fc), None, 0, C.byref(n)))
+        k = np.zeros((n.value, 3), dtype=np.uint32)
+        self._ck(self.lib.fenc_fc_wts_keys(self.h, C.byref(fc), _ptr(k, C.c_uint32), n.value, C.byref(n)))
+        return k
+
+    def fc_weights(self, fc, w, n_limbs, scale=0.0):
+        w = np.ascontiguousarray(w, dtype=np.float64)
+        assert w.shape == (fc.n_out, fc.n_in)
+        h = C.c_void_p()
+        self._ck(self.lib.fenc_fc_weights(self.h, C.byref(fc), _ptr(w, C.c_double), n_limbs, float(scale), C.byref(h)))
+        return Weights(self, h)
+
+    def fc_weights_from_coeffs(self, fc, coeffs, n_limbs, scale=0.0):
+        c = np.ascontiguousarray(coeffs, dtype=np.int64)
+        assert c.ndim == 2 and c.shape[1] == self.N
+        h = C.c_void_p()
+        self._ck(self.lib.fenc_fc_weights_from_coeffs(self.h, C.byref(fc), _ptr(c, C.c_int64), c.shape[0], n_limbs, float(scale),
+                                                      C.byref(h)))
+        return Weights(self, h)
+
+    def fc(self, keys, fc, wts, cts, do_rescale=True):
+        cap = self.fc_plan(fc)["n_out_ct"]
+        out = (C.c_void_p * cap)()
+        n = C.c_size_t()
+        self._ck(self.lib.fenc_fc(self.h, keys.h, C.byref(fc), wts.h, self._harr(cts), len(cts), int(do_rescale), out, cap, C.byref(n)))
         return [Ciphertext(self, C.c_void_p(out[i])) for i in range(n.value)]
 
     def compress(self, keys, cts, terms, n_out, mask=None, do_rescale=False):

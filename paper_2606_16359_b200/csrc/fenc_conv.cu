@@ -20,18 +20,23 @@ struct Term {
   int w;    // weight plaintext index (fenc_wts_keys order)
 };
 struct OutCt {
-  std::vector<int> diags;                // existing channel diagonals d, ascending
+  std::vector<int> diags;                // existing diagonals d, ascending
+  std::vector<int> rots;                 // outer rotation amount of each existing diagonal (0 for d = 0)
   std::vector<std::vector<Term>> terms;  // per existing diagonal
 };
-struct ConvGraph {
-  fenc_conv_desc d;
-  int n, M, S, S_out, m, B, ch, cs, G_in, G_out, BG, H_out, W_out;
-  std::vector<OutCt> outs;                    // index (g_out * S_out + u_o) * S_out + v_o
-  std::vector<std::pair<int, int>> inner;     // distinct (src, amt != 0), sorted
+// what the batched executor needs from a linear layer's operation graph (conv or fc)
+struct LinGraph {
+  size_t nin_bg = 0, BG = 1, n_w = 0;
+  std::vector<OutCt> outs;                   // per output ciphertext of one batch group
+  std::vector<std::pair<int, int>> inner;    // distinct (src, amt != 0), sorted
   std::map<std::pair<int, int>, int> inner_index;
-  std::vector<std::array<u32, 7>> wkeys;      // (u_o, v_o, g_out, g_in, d, i, j) per weight plaintext
-  std::vector<int> rot_steps;                 // distinct rotation amounts (inner and outer), ascending
+  std::vector<int> rot_steps;                // distinct rotation amounts (inner and outer), ascending
   size_t n_outer = 0, n_pmult = 0;
+};
+struct ConvGraph : LinGraph {              // outs index: (g_out * S_out + u_o) * S_out + v_o
+  fenc_conv_desc d;
+  int n, M, S, S_out, m, B, ch, cs, G_in, G_out, H_out, W_out;
+  std::vector<std::array<u32, 7>> wkeys;      // (u_o, v_o, g_out, g_in, d, i, j) per weight plaintext
   // R2.9 step 2: the validity conditions factorise into channel positions, block rows and block columns
   std::vector<std::array<int, 3>> valid_cpos(int go, int gi, int dd) const {
     std::vector<std::array<int, 3>> v;
@@ -73,7 +78,7 @@ static fenc_status build_graph(fenc_ctx *ctx, const fenc_conv_desc *cd, int S, s
            cd->stride, cd->pad, cd->depthwise, S, cd->M);
   auto it = ctx->graphs.find(keybuf);
   if (it != ctx->graphs.end()) {
-    out = it->second;
+    out = std::static_pointer_cast<ConvGraph>(it->second);
     return FENC_OK;
   }
   if (cd->BS < 1 || cd->C_in < 1 || cd->C_out < 1 || cd->K < 1 || cd->stride < 1 || cd->H + 2 * cd->pad < cd->K || cd->W + 2 * cd->pad < cd->K)
@@ -128,6 +133,7 @@ static fenc_status build_graph(fenc_ctx *ctx, const fenc_conv_desc *cd, int S, s
           }
           if (!lst.empty()) {
             oc.diags.push_back(dd);
+            oc.rots.push_back((int)(((long)dd * g->cs) % g->n));
             oc.terms.push_back(std::move(lst));
             g->n_pmult += oc.terms.back().size();
             if (dd) g->n_outer++, steps.insert((int)(((long)dd * g->cs) % g->n));
@@ -137,6 +143,7 @@ static fenc_status build_graph(fenc_ctx *ctx, const fenc_conv_desc *cd, int S, s
   g->inner.assign(inner.begin(), inner.end());
   for (size_t i = 0; i < g->inner.size(); i++) g->inner_index[g->inner[i]] = (int)i;
   g->rot_steps.assign(steps.begin(), steps.end());
+  g->nin_bg = (size_t)g->S * g->S * g->G_in, g->n_w = g->wkeys.size();
   ctx->graphs[keybuf] = g;
   out = g;
   return FENC_OK;
@@ -352,18 +359,13 @@ extern "C" void fenc_wts_free(fenc_wts *W) {
 // 1. inner rotations: every distinct (input ciphertext, amount) once, always from the original input, ONE batch
 // 2. MAC: P_d = sum over (g_in, taps) of R (*) W per existing channel diagonal d, one launch for all (bg, output, d)
 // 3. outer rotations: Rot(P_d, d cs) for d != 0, ONE batch;  4. Y = P_0 + sum of those;  5. one rescale per output (A13)
-extern "C" fenc_status fenc_hconv(fenc_ctx *ctx, const fenc_keys *K, const fenc_conv_desc *cd, const fenc_layout *lay,
-                                  const fenc_wts *W, fenc_ct *const *in, size_t n_in, int do_rescale, fenc_ct **out,
-                                  size_t cap, size_t *n_out) {
-  if (!ctx || !K || !cd || !lay || !W || !in || !out || !n_out) return FENC_ERR_INVALID_ARG;
-  std::shared_ptr<ConvGraph> gp;
-  fenc_status st = graph_for(ctx, cd, lay, gp);
-  if (st != FENC_OK) return st;
-  const ConvGraph &g = *gp;
-  const size_t nin_bg = (size_t)g.S * g.S * g.G_in, nout_bg = g.outs.size(), BG = g.BG;
+static fenc_status run_linear(fenc_ctx *ctx, const fenc_keys *K, const LinGraph &g, const fenc_wts *W, fenc_ct *const *in,
+                              size_t n_in, int do_rescale, fenc_ct **out, size_t cap, size_t *n_out) {
+  fenc_status st;
+  const size_t nin_bg = g.nin_bg, nout_bg = g.outs.size(), BG = g.BG;
   if (n_in != nin_bg * BG) return fail(ctx, FENC_ERR_MISMATCH, "expected %zu input ciphertexts, got %zu", nin_bg * BG, n_in);
   if (cap < nout_bg * BG) return fail(ctx, FENC_ERR_INVALID_ARG, "output capacity %zu < %zu", cap, nout_bg * BG);
-  if (W->n != g.wkeys.size()) return fail(ctx, FENC_ERR_MISMATCH, "weights belong to another layer");
+  if (W->n != g.n_w) return fail(ctx, FENC_ERR_MISMATCH, "weights belong to another layer");
   const int L = in[0]->L;
   const double s_in = in[0]->scale;
   for (size_t i = 0; i < n_in; i++)
@@ -427,7 +429,7 @@ extern "C" fenc_status fenc_hconv(fenc_ctx *ctx, const fenc_keys *K, const fenc_
         if (oc.diags[k] == 0) sum_terms.push_back(P);
         else {
           u64 *R = Obuf + (oi++) * CT;
-          rot_in.push_back(P), rot_out.push_back(R), rot_step.push_back((int)(((long)oc.diags[k] * g.cs) % g.n));
+          rot_in.push_back(P), rot_out.push_back(R), rot_step.push_back(oc.rots[k]);
           sum_terms.push_back(R);
         }
       }
@@ -459,6 +461,16 @@ extern "C" fenc_status fenc_hconv(fenc_ctx *ctx, const fenc_keys *K, const fenc_
   for (size_t i = 0; i < res.size(); i++) out[i] = res[i];
   *n_out = res.size();
   return FENC_OK;
+}
+
+extern "C" fenc_status fenc_hconv(fenc_ctx *ctx, const fenc_keys *K, const fenc_conv_desc *cd, const fenc_layout *lay,
+                                  const fenc_wts *W, fenc_ct *const *in, size_t n_in, int do_rescale, fenc_ct **out,
+                                  size_t cap, size_t *n_out) {
+  if (!ctx || !K || !cd || !lay || !W || !in || !out || !n_out) return FENC_ERR_INVALID_ARG;
+  std::shared_ptr<ConvGraph> gp;
+  fenc_status st = graph_for(ctx, cd, lay, gp);
+  if (st != FENC_OK) return st;
+  return run_linear(ctx, K, *gp, W, in, n_in, do_rescale, out, cap, n_out);
 }
 
 // ------------------------------------------------------------------------------------------------ AAC compress (R2.11)
@@ -543,4 +555,145 @@ extern "C" fenc_status fenc_compress(fenc_ctx *ctx, const fenc_keys *K, fenc_ct 
   dfree(ctx, Mbuf), dfree(ctx, Rbuf), dfree(ctx, Ybuf);
   for (size_t t = 0; t < n_out; t++) out[t] = res[t];
   return FENC_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ FC by plain diagonals (R2.12)
+struct FcGraph : LinGraph {
+  fenc_fc_desc d;
+  int n, B, P, m, ch, n_in_ct, n_out_ct;
+  std::vector<std::array<u32, 3>> wkeys;  // (c_out_ct, c_in_ct, d)
+  // feature index of (input ct c, position p) or -1
+  long feat(int c, int p) const {
+    if (d.in_C) {
+      const int m2 = m * m, cpos = p / m2, k = p % m2, chan = c * ch + cpos, h = k / m, w = k % m;
+      if (chan >= (int)d.in_C || h >= (int)d.in_H || w >= (int)d.in_W) return -1;
+      return ((long)chan * d.in_H + h) * d.in_W + w;
+    }
+    const long f = (long)c * P + p;
+    return f < (long)d.n_in ? f : -1;
+  }
+  long neuron(int c, int p) const {
+    const long v = (long)c * P + p;
+    return v < (long)d.n_out ? v : -1;
+  }
+  bool nonzero(int co, int ci, int dd) const {
+    for (int p = 0; p < P; p++)
+      if (feat(ci, p) >= 0 && neuron(co, ((p - dd) % P + P) % P) >= 0) return true;
+    return false;
+  }
+  void weight_slots(const std::array<u32, 3> &wk, const double *w, std::vector<double> &vec) const {
+    vec.assign(n, 0.0);
+    const int co = wk[0], ci = wk[1], dd = wk[2];
+    for (int p = 0; p < P; p++) {
+      const long f = feat(ci, p), v = neuron(co, ((p - dd) % P + P) % P);
+      if (f < 0 || v < 0) continue;
+      const double val = w[(size_t)v * d.n_in + f];
+      for (int b = 0; b < B; b++) vec[(size_t)p * B + b] = val;
+    }
+  }
+};
+
+static fenc_status fc_graph(fenc_ctx *ctx, const fenc_fc_desc *fd, std::shared_ptr<FcGraph> &out) {
+  char keybuf[256];
+  snprintf(keybuf, sizeof keybuf, "fc,%u,%u,%u,%u,%u,%u,%u", fd->BS, fd->n_in, fd->n_out, fd->in_C, fd->in_H, fd->in_W, fd->in_M);
+  auto it = ctx->graphs.find(keybuf);
+  if (it != ctx->graphs.end()) {
+    out = std::static_pointer_cast<FcGraph>(it->second);
+    return FENC_OK;
+  }
+  if (fd->BS < 1 || fd->n_in < 1 || fd->n_out < 1 || fd->in_M < 1) return fail(ctx, FENC_ERR_INVALID_ARG, "bad fc shape");
+  auto g = std::make_shared<FcGraph>();
+  g->d = *fd, g->n = ctx->n, g->m = fd->in_M;
+  const long m2 = (long)g->m * g->m;
+  if (m2 > g->n || g->n % m2) return fail(ctx, FENC_ERR_LAYOUT, "frame %u^2 does not fit %d slots", fd->in_M, g->n);
+  g->B = (int)std::min<long>(next_pow2(fd->BS), g->n / m2);
+  g->P = g->n / g->B;
+  g->ch = (int)(g->n / (g->B * m2));
+  g->BG = (fd->BS + g->B - 1) / g->B;
+  if (fd->in_C) {
+    if (fd->in_H > fd->in_M || fd->in_W > fd->in_M || (size_t)fd->in_C * fd->in_H * fd->in_W != fd->n_in)
+      return fail(ctx, FENC_ERR_LAYOUT, "fc input tensor does not match n_in");
+    g->n_in_ct = (fd->in_C + g->ch - 1) / g->ch;
+  } else {
+    g->n_in_ct = (fd->n_in + g->P - 1) / g->P;
+  }
+  g->n_out_ct = (fd->n_out + g->P - 1) / g->P;
+  g->nin_bg = g->n_in_ct;
+  std::set<int> steps;
+  g->outs.resize(g->n_out_ct);
+  for (int co = 0; co < g->n_out_ct; co++) {
+    OutCt &oc = g->outs[co];
+    for (int dd = 0; dd < g->P; dd++) {
+      std::vector<Term> lst;
+      for (int ci = 0; ci < g->n_in_ct; ci++) {
+        if (!g->nonzero(co, ci, dd)) continue;
+        lst.push_back(Term{ci, 0, (int)g->wkeys.size()});
+        g->wkeys.push_back({(u32)co, (u32)ci, (u32)dd});
+      }
+      if (lst.empty()) continue;
+      const int rot = (int)(((long)dd * g->B) % g->n);
+      oc.diags.push_back(dd), oc.rots.push_back(rot);
+      g->n_pmult += lst.size();
+      oc.terms.push_back(std::move(lst));
+      if (dd) g->n_outer++, steps.insert(rot);
+    }
+  }
+  g->rot_steps.assign(steps.begin(), steps.end());
+  g->n_w = g->wkeys.size();
+  ctx->graphs[keybuf] = g;
+  out = g;
+  return FENC_OK;
+}
+
+extern "C" fenc_status fenc_fc_plan(fenc_ctx *ctx, const fenc_fc_desc *fd, fenc_fc_info *out) {
+  if (!ctx || !fd || !out) return FENC_ERR_INVALID_ARG;
+  std::shared_ptr<FcGraph> g;
+  fenc_status st = fc_graph(ctx, fd, g);
+  if (st != FENC_OK) return st;
+  if (g->rot_steps.size() > 512) return fail(ctx, FENC_ERR_LAYOUT, "more than 512 rotation amounts (plain diagonals need B large; BSGS is not built)");
+  memset(out, 0, sizeof *out);
+  out->B = g->B, out->P = g->P, out->BG = (u32)g->BG, out->n_in_ct = g->n_in_ct * (u32)g->BG, out->n_out_ct = g->n_out_ct * (u32)g->BG;
+  out->n_rot = (u32)(g->n_outer * g->BG), out->n_pmult = (u32)(g->n_pmult * g->BG), out->n_distinct_pt = (u32)g->wkeys.size();
+  out->n_rot_keys = (u32)g->rot_steps.size();
+  for (size_t i = 0; i < g->rot_steps.size(); i++) out->rot_steps[i] = g->rot_steps[i];
+  return FENC_OK;
+}
+extern "C" fenc_status fenc_fc_wts_keys(fenc_ctx *ctx, const fenc_fc_desc *fd, uint32_t *keys3, size_t capacity, size_t *n) {
+  if (!ctx || !fd || !n) return FENC_ERR_INVALID_ARG;
+  std::shared_ptr<FcGraph> g;
+  fenc_status st = fc_graph(ctx, fd, g);
+  if (st != FENC_OK) return st;
+  *n = g->wkeys.size();
+  if (keys3) {
+    if (capacity < g->wkeys.size()) return fail(ctx, FENC_ERR_INVALID_ARG, "capacity too small");
+    for (size_t i = 0; i < g->wkeys.size(); i++) memcpy(keys3 + 3 * i, g->wkeys[i].data(), 3 * sizeof(u32));
+  }
+  return FENC_OK;
+}
+extern "C" fenc_status fenc_fc_weights(fenc_ctx *ctx, const fenc_fc_desc *fd, const double *w, uint32_t n_limbs, double scale,
+                                       fenc_wts **out) {
+  if (!ctx || !fd || !w || !out) return FENC_ERR_INVALID_ARG;
+  std::shared_ptr<FcGraph> g;
+  fenc_status st = fc_graph(ctx, fd, g);
+  if (st != FENC_OK) return st;
+  const FcGraph *gp = g.get();
+  return make_wts(ctx, gp->wkeys.size(), [gp, w](size_t i, std::vector<double> &v) { gp->weight_slots(gp->wkeys[i], w, v); }, nullptr,
+                  n_limbs, scale, out);
+}
+extern "C" fenc_status fenc_fc_weights_from_coeffs(fenc_ctx *ctx, const fenc_fc_desc *fd, const int64_t *coeffs, size_t n,
+                                                   uint32_t n_limbs, double scale, fenc_wts **out) {
+  if (!ctx || !fd || !coeffs || !out) return FENC_ERR_INVALID_ARG;
+  std::shared_ptr<FcGraph> g;
+  fenc_status st = fc_graph(ctx, fd, g);
+  if (st != FENC_OK) return st;
+  if (n != g->wkeys.size()) return fail(ctx, FENC_ERR_MISMATCH, "expected %zu weight plaintexts, got %zu", g->wkeys.size(), n);
+  return make_wts(ctx, n, nullptr, coeffs, n_limbs, scale, out);
+}
+extern "C" fenc_status fenc_fc(fenc_ctx *ctx, const fenc_keys *K, const fenc_fc_desc *fd, const fenc_wts *W, fenc_ct *const *in,
+                               size_t n_in, int do_rescale, fenc_ct **out, size_t cap, size_t *n_out) {
+  if (!ctx || !K || !fd || !W || !in || !out || !n_out) return FENC_ERR_INVALID_ARG;
+  std::shared_ptr<FcGraph> g;
+  fenc_status st = fc_graph(ctx, fd, g);
+  if (st != FENC_OK) return st;
+  return run_linear(ctx, K, *g, W, in, n_in, do_rescale, out, cap, n_out);
 }

@@ -38,7 +38,7 @@ struct LevelPlan {
   std::vector<void *> owned;
 };
 
-struct ConvGraph;  // fenc_conv.cu
+struct LinGraph;  // fenc_conv.cu: operation graph of a linear layer (conv or fc)
 
 struct fenc_ctx {
   int logN = 0, N = 0, n = 0, nq = 0, np = 0, A = 0, dlen = 0, beta_max = 0;
@@ -64,7 +64,7 @@ struct fenc_ctx {
   size_t ws_bytes = 0;
   void *desc_buf = nullptr;         // device staging for per-call descriptor arrays
   size_t desc_bytes = 0;
-  std::map<std::string, std::shared_ptr<ConvGraph>> graphs;
+  std::map<std::string, std::shared_ptr<LinGraph>> graphs;
 };
 
 struct fenc_keys {

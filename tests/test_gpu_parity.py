@@ -253,3 +253,149 @@ def test_rotation_full_size_config3_sampled(mods):
     ref = ck.rotate(P, ok, ck.Ciphertext(limbs, L, 1), 1)
     assert np.array_equal(ctx.ct_export(outs[0]), ref.c)
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------------------ fc, pooling, pipeline
+@pytest.mark.parametrize("kw", [
+    dict(BS=2, n_in=32, n_out=5, in_C=2, in_H=4, in_W=4, in_M=4),
+    dict(BS=40, n_in=3 * 3 * 3, n_out=20, in_C=3, in_H=3, in_W=3, in_M=4),   # B=32, BG=2, P=16, two output cts
+    dict(BS=64, n_in=20, n_out=11, in_M=4),                                  # flat input
+])
+def test_fc_bit_exact(mods, kw):
+    ck, fr, fenc = mods
+    from oracle import network as nw
+    P, ctx = make(mods, "mid10")
+    g = nw.FcGraph(P.n, **kw)
+    fcd = ctx.fc_desc(**kw)
+    info = ctx.fc_plan(fcd)
+    c = g.counts()
+    assert {k: info[k] for k in c} == c
+    L = P.nq
+    rng = np.random.default_rng(9)
+    X = rng.uniform(-1, 1, (kw["BS"], kw["n_in"]))
+    W = rng.normal(0, 0.3, (kw["n_out"], kw["n_in"]))
+    ok, gk = ck.keygen(P, 31, c["rot_steps"]), ctx.keygen(31, c["rot_steps"])
+    oW = nw.encode_fc_weights(ck, P, g, W, L)
+    coeffs = np.stack([oW[tuple(int(v) for v in k)].coeffs for k in ctx.fc_wts_keys(fcd)])
+    gW = ctx.fc_weights_from_coeffs(fcd, coeffs, L, float(P.q[L - 1]))
+    o_in, g_in = [], []
+    for bg in range(g.BG):
+        for ci in range(g.n_in_ct):
+            pt = ck.encode(P, g.gather_in(X, ci, bg), L)
+            o_in.append(ck.encrypt(P, ok, pt, 70 + len(o_in)))
+            g_in.append(ctx.encrypt(gk, ctx.pt_from_coeffs(pt.coeffs, L, float(pt.scale)), 70 + len(g_in)))
+    g_out = ctx.fc(gk, fcd, gW, g_in)
+    Y = np.zeros((kw["BS"], kw["n_out"]))
+    for bg in range(g.BG):
+        ref = nw.fc(ck, P, ok, g, o_in[bg * g.n_in_ct:(bg + 1) * g.n_in_ct], oW)
+        for co, r in enumerate(ref):
+            got = g_out[bg * g.n_out_ct + co]
+            assert np.array_equal(ctx.ct_export(got), r.c), (bg, co)
+            g.scatter_out(Y, ctx.decrypt_slots(gk, got).real, co, bg)
+    assert np.abs(Y - X @ W.T).max() < 1e-3
+    # the library's own weight encoder lands within one unit of the oracle's integers (A7)
+    gW2 = ctx.fc_weights(fcd, W, L)
+    assert gW2 is not None
+    ctx.close()
+
+
+def test_pipeline_toy_network_bit_exact(mods):
+    """conv - square - pool - fc - fc through Pipeline (one batched C-ABI call per layer) vs the oracle's network."""
+    ck, fr, fenc = mods
+    from oracle import network as nw
+    from paper_2606_16359_b200.pipeline import Pipeline
+    from test_oracle_network import plain_network, toy_network
+    p = dict(log2N=9, n_q=5, q_bits=40, n_p=2, p_bits=60, dnum=3, log2_scale=40)
+    P = ck.Params(*wl.oracle_params_args(p))
+    ctx = fenc.Context(**p)
+    layers, x = toy_network()
+    pipe = Pipeline(ctx, layers)
+    steps, relin = nw.network_rot_steps(layers, P.n)
+    assert sorted(pipe.steps) == steps and pipe.need_relin == relin
+
+    def enc_w(entry):
+        L = entry["L"]
+        if entry["op"] == "conv":
+            g = fr.ConvGraph(fr.ConvDesc(S=int(entry["conv"].S), **{k: int(getattr(entry["conv"], k)) for k in
+                             ("BS", "C_in", "H", "W", "C_out", "K", "stride", "pad")}), P.n)
+            oW = fr.encode_weights(ck, P, g, entry["w"], L)
+            return np.stack([oW[tuple(int(v) for v in k)].coeffs for k in ctx.wts_keys(entry["conv"], entry["lay"])])
+        fcd = entry["fc"]
+        g = nw.FcGraph(P.n, **{k: int(getattr(fcd, k)) for k in ("BS", "n_in", "n_out", "in_C", "in_H", "in_W", "in_M")})
+        oW = nw.encode_fc_weights(ck, P, g, entry["w"], L)
+        return np.stack([oW[tuple(int(v) for v in k)].coeffs for k in ctx.fc_wts_keys(fcd)])
+
+    gk = pipe.setup(key_seed=11, encode_weight=enc_w)
+    ok = ck.keygen(P, 11, steps, want_relin=relin)
+    lin = fr.Layout(P.n, 8, 2, 2, 1)
+    o_in, g_in = [], []
+    for i, (u, v, g, bg) in enumerate(lin.ct_keys()):
+        pt = ck.encode(P, lin.gather(x, u, v, g, bg), P.nq)
+        o_in.append(ck.encrypt(P, ok, pt, 100 + i))
+        g_in.append(ctx.encrypt(gk, ctx.pt_from_coeffs(pt.coeffs, P.nq, float(pt.scale)), 100 + i))
+    o_out, o_trace = nw.run_network(ck, P, ok, layers, o_in, P.nq)
+    g_trace = []
+    g_out = pipe.forward(g_in, trace=g_trace)
+    for li, (ol, gl) in enumerate(zip(o_trace, g_trace)):
+        assert len(ol) == len(gl), li
+        for a, b in zip(ol, gl):
+            assert np.array_equal(ctx.ct_export(b), a.c), li
+    fg = nw.FcGraph(P.n, **layers[-1]["fc"])
+    Y = np.zeros((2, 3))
+    fg.scatter_out(Y, ctx.decrypt_slots(gk, g_out[0]).real, 0, 0)
+    assert np.abs(Y - plain_network(layers, x)).max() < 1e-3
+    # the same network with the library's own encoder (Algorithm 1 gather + fp64 encode on the library side)
+    pipe2 = Pipeline(ctx, layers)
+    pipe2.setup(key_seed=12)
+    out2 = pipe2.forward(pipe2.encrypt_input(x, 500))
+    fg.scatter_out(Y, ctx.decrypt_slots(pipe2.keys, out2[0]).real, 0, 0)
+    assert np.abs(Y - plain_network(layers, x)).max() < 1e-3
+    ctx.close()
+
+
+def test_lenet_conv1_full_size_sampled(mods):
+    """BASELINE config 2 at the size bench.py times (N=2^14, 8+2 limbs, BS=128, S=4): two output ciphertexts of conv1 are
+    recomputed by the oracle term by term (its inner rotations, 25 PMults, rescale) and compared limb by limb."""
+    ck, fr, fenc = mods
+    P, ctx = make(mods, "cfg2")
+    conv_kw = dict(BS=128, C_in=1, H=28, W=28, C_out=6, K=5, stride=1, pad=2)
+    x, w = wl.conv_inputs(2001, conv_kw, x_range=(0.0, 1.0))
+    graph = fr.ConvGraph(fr.ConvDesc(S=4, **conv_kw), P.n)
+    conv = ctx.conv_desc(S=4, **conv_kw)
+    lay = ctx.layout_plan(conv)
+    assert (lay.B, lay.ch, lay.n_in_ct, lay.n_out_ct, lay.n_inner_rot, lay.n_outer_rot, lay.n_pmult) == (128, 1, 16, 96, 48, 0, 2400)
+    L = P.nq
+    sample = [(0, 0, 0), (3, 2, 5)]  # (u_o, v_o, g_out): a border fragment and an interior one
+    need = sorted({amt for ok_ in sample for lst in graph.terms[ok_].values() for _, amt, _ in lst if amt})
+    gk = ctx.keygen(77, lay.steps())
+    ok = ck.keygen(P, 77, need)
+    keys7 = ctx.wts_keys(conv, lay)
+    wanted = {wk for ok_ in sample for lst in graph.terms[ok_].values() for _, _, wk in lst}
+    oW = {wk: ck.encode(P, graph.weight_slots(wk, w), L, P.q[L - 1]) for wk in wanted}
+    gW = ctx.conv_weights(conv, lay, w, L)  # library encoder for all 2400; the sampled ones are checked against the oracle's
+    o_in, g_in = {}, []
+    for (u, v, g, bg) in graph.lin.ct_keys():
+        pt = ck.encode(P, graph.lin.gather(x, u, v, g, bg), L)
+        o_in[(u, v, g)] = ck.encrypt(P, ok, pt, 3000 + len(g_in))
+        g_in.append(ctx.encrypt(gk, ctx.pt_from_coeffs(pt.coeffs, L, float(pt.scale)), 3000 + len(g_in)))
+    # weights through the oracle's integers for the sampled outputs only: rebuild the full coefficient table
+    coeffs = np.zeros((len(keys7), P.N), dtype=np.int64)
+    lib = ctx.conv_weights(conv, lay, w, L)
+    del lib
+    for i, k in enumerate(keys7):
+        wk = tuple(int(v) for v in k)
+        if wk in oW:
+            coeffs[i] = oW[wk].coeffs
+    gW = ctx.conv_weights_from_coeffs(conv, lay, coeffs, L, float(P.q[L - 1]))
+    g_out = ctx.hconv(gk, conv, lay, gW, g_in)
+    for (uo, vo, go) in sample:
+        acc = np.zeros((2, L, P.N), dtype=np.uint64)
+        (d, lst), = graph.terms[(uo, vo, go)].items()
+        assert d == 0
+        for src, amt, wk in lst:
+            xin = ck.rotate(P, ok, o_in[src], amt) if amt else o_in[src]
+            ck.pmult_acc(P, acc, xin, oW[wk])
+        ref = ck.rescale(P, ck.Ciphertext(acc, L, o_in[src].scale * oW[wk].scale))
+        got = g_out[(go * 4 + uo) * 4 + vo]
+        assert np.array_equal(ctx.ct_export(got), ref.c), (uo, vo, go)
+    ctx.close()

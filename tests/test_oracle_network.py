@@ -1,0 +1,98 @@
+"""Pins for oracle/network.py (CPU only): the FC-by-diagonals graph against a dense fp64 product, pooling by fragment
+selection against a direct sum-pool through Algorithm 1's layout, and an encrypted toy network against its fp64
+evaluation.  None of these re-uses the code under test to produce the expected value."""
+import numpy as np
+import pytest
+
+from oracle import ckks as ck
+from oracle import fragment as fr
+from oracle import network as nw
+
+
+@pytest.mark.parametrize("kw", [
+    dict(n=256, BS=2, n_in=32, n_out=5, in_C=2, in_H=4, in_W=4, in_M=4),      # conv-layout input, one output ct
+    dict(n=256, BS=5, n_in=3 * 3 * 3, n_out=70, in_C=3, in_H=3, in_W=3, in_M=4),  # ragged frame, BS not 2^k, 2 output cts
+    dict(n=64, BS=40, n_in=10, n_out=7, in_M=2),                               # flat input, several batch groups (B=16)
+    dict(n=64, BS=16, n_in=9, n_out=6, in_M=2),                                # B = 16, P = 4: 3 input cts, 2 output cts
+])
+def test_fc_graph_equals_dense_product(kw):
+    n = kw.pop("n")
+    g = nw.FcGraph(n, **kw)
+    rng = np.random.default_rng(3)
+    X = rng.uniform(-1, 1, (kw["BS"], kw["n_in"]))
+    W = rng.normal(0, 1, (kw["n_out"], kw["n_in"]))
+    assert np.abs(nw.fc_slots(g, X, W) - X @ W.T).max() < 1e-12
+    c = g.counts()
+    # every existing non-zero diagonal costs one rotation per output ciphertext; d*B are the amounts
+    assert c["n_rot"] == g.BG * sum(len([d for d in diags if d]) for diags in g.terms.values())
+    assert all(s % g.B == 0 and 0 < s < n for s in c["rot_steps"])
+
+
+def test_fc_conv_layout_matches_torch_flatten_order():
+    # feat(c, p) must be channel*H*W + h*W + w: gather a tensor through Algorithm 1's S=1 layout and compare
+    n, BS, C, H, W_, M = 256, 2, 3, 3, 4, 4
+    g = nw.FcGraph(n, BS, C * H * W_, 4, in_C=C, in_H=H, in_W=W_, in_M=M)
+    lay = fr.Layout(n, M, 1, BS, C)
+    X = np.random.default_rng(1).uniform(-1, 1, (BS, C, H, W_))
+    for c in range(g.n_in_ct):
+        assert np.array_equal(g.gather_in(X.reshape(BS, -1), c, 0), lay.gather(X, 0, 0, c, 0))
+
+
+def test_pool_order_is_sum_pool_through_the_layout():
+    n, BS, C, H, M, S = 128, 2, 3, 8, 8, 4
+    X = np.random.default_rng(2).uniform(-1, 1, (BS, C, H, H))
+    lin = fr.Layout(n, M, S, BS, C)
+    vecs = [lin.gather(X, u, v, g, bg) for (u, v, g, bg) in lin.ct_keys()]
+    order = nw.pool_order(len(vecs), S)
+    pooled = [sum(vecs[i] for i in order[k:k + 4]) for k in range(0, len(order), 4)]
+    Xs = X.reshape(BS, C, H // 2, 2, H // 2, 2).sum(axis=(3, 5))  # direct 2x2 sum-pool
+    lout = fr.Layout(n, M // 2, S // 2, BS, C)
+    want = [lout.gather(Xs, u, v, g, bg) for (u, v, g, bg) in lout.ct_keys()]
+    assert len(pooled) == len(want)
+    for a, b in zip(pooled, want):
+        assert np.abs(a - b).max() < 1e-12
+
+
+def toy_network(BS=2, seed=5):
+    rng = np.random.default_rng(seed)
+    layers = [
+        {"op": "conv", "conv": dict(BS=BS, C_in=1, H=8, W=8, C_out=2, K=3, stride=1, pad=1), "S": 2, "w": rng.normal(0, 0.3, (2, 1, 3, 3))},
+        {"op": "square"}, {"op": "pool"},
+        {"op": "fc", "fc": dict(BS=BS, n_in=32, n_out=5, in_C=2, in_H=4, in_W=4, in_M=4), "w": rng.normal(0, 0.3, (5, 32)) * 0.25},
+        {"op": "fc", "fc": dict(BS=BS, n_in=5, n_out=3, in_M=4), "w": rng.normal(0, 0.3, (3, 5))},
+    ]
+    x = rng.uniform(0, 1, (BS, 1, 8, 8))
+    return layers, x
+
+
+def plain_network(layers, x):
+    """fp64 evaluation of the same function (pool = SUM pool; its 1/4 is already inside the next weights)."""
+    for ly in layers:
+        if ly["op"] == "conv":
+            x = fr.direct_conv(fr.ConvDesc(**ly["conv"]), x, ly["w"])
+        elif ly["op"] == "square":
+            x = x * x
+        elif ly["op"] == "pool":
+            b, c, h, w = x.shape
+            x = x.reshape(b, c, h // 2, 2, w // 2, 2).sum(axis=(3, 5))
+        elif ly["op"] == "fc":
+            x = x.reshape(x.shape[0], -1) @ ly["w"].T
+    return x
+
+
+def test_encrypted_toy_network_matches_fp64():
+    P = ck.Params(9, 5, 40, 2, 60, 3, 40)
+    layers, x = toy_network()
+    steps, relin = nw.network_rot_steps(layers, P.n)
+    keys = ck.keygen(P, 11, steps, want_relin=relin)
+    lin = fr.Layout(P.n, 8, 2, 2, 1)
+    cts = [ck.encrypt(P, keys, ck.encode(P, lin.gather(x, u, v, g, bg), P.nq), 100 + i)
+           for i, (u, v, g, bg) in enumerate(lin.ct_keys())]
+    out, _ = nw.run_network(ck, P, keys, layers, cts, P.nq)
+    assert len(out) == 1 and out[0].L == 1
+    g = nw.FcGraph(P.n, **layers[-1]["fc"])
+    Y = np.zeros((2, 3))
+    g.scatter_out(Y, ck.decrypt_decode(P, keys, out[0]).real, 0, 0)
+    want = plain_network(layers, x)
+    assert np.abs(want).max() < 0.45  # a single 40-bit limb at scale 2^40 holds |value| < 0.5 (A23)
+    assert np.abs(Y - want).max() < 1e-4
