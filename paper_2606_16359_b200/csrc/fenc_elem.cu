@@ -26,18 +26,42 @@ struct MacP {
   int L, logN, max_lazy;
 };
 #define MAC_TILE 64  // terms whose pointers are staged in shared memory at a time
-template <int G>
-__global__ void __launch_bounds__(256, 3) mac_kernel(MacP p) {
+// SMALL (every modulus in use < 2^52): operands are split in 26-bit limbs, x = x1 2^26 + x0, and the three partial sums
+// sum x0 w0, sum (x0 w1 + x1 w0), sum x1 w1 are accumulated in plain 64-bit registers by IMAD.WIDE with NO carry
+// handling (each product < 2^52, so 1024 terms fit); they are recombined into a 128-bit value once per flush.  This is
+// 4 IMAD.WIDE + ~1.5 limb-split instructions per multiply-accumulate against ~20 for a carried 64x64->128 MAC.
+struct Acc3 { u64 a0, a1, a2; };
+DEVI void acc3_mac(Acc3 &A, u32 x0, u32 x1, u32 w0, u32 w1) {
+  A.a0 += (u64)x0 * w0;
+  A.a1 += (u64)x0 * w1;
+  A.a1 += (u64)x1 * w0;
+  A.a2 += (u64)x1 * w1;
+}
+DEVI u64 acc3_redc(Acc3 &A, u64 q, u64 qinv_neg) {  // (a0 + a1 2^26 + a2 2^52) 2^-64 mod q, and clears A
+  u64 lo = A.a0, hi = 0, t;
+  t = A.a1 << 26; lo += t; hi += (A.a1 >> 38) + (lo < t ? 1 : 0);
+  t = A.a2 << 52; lo += t; hi += (A.a2 >> 12) + (lo < t ? 1 : 0);
+  A.a0 = A.a1 = A.a2 = 0;
+  return mont_redc(lo, hi, q, qinv_neg);
+}
+template <int G, bool SMALL>
+__global__ void __launch_bounds__(256, 2) mac_kernel(MacP p) {
   __shared__ const u64 *s_ct[MAC_TILE];
   __shared__ const u64 *s_pt[G][MAC_TILE];
   const size_t LN = (size_t)p.L << p.logN;
-  const size_t idx = (size_t)blockIdx.y * blockDim.x + threadIdx.x;  // LN is a multiple of 256 or the guard below holds
+  const size_t idx = (size_t)blockIdx.y * blockDim.x + threadIdx.x;
   const bool live = idx < LN;
   const MacGroup g = p.groups[blockIdx.x];
   const ModConst mc = p.mods[(live ? idx : 0) >> p.logN];
-  u64 lo0[G], hi0[G], lo1[G], hi1[G], r0[G], r1[G];
+  u64 lo0[SMALL ? 1 : G], hi0[SMALL ? 1 : G], lo1[SMALL ? 1 : G], hi1[SMALL ? 1 : G], r0[G], r1[G];
+  Acc3 A0[SMALL ? G : 1], A1[SMALL ? G : 1];
 #pragma unroll
-  for (int i = 0; i < G; i++) lo0[i] = hi0[i] = lo1[i] = hi1[i] = r0[i] = r1[i] = 0;
+  for (int i = 0; i < G; i++) r0[i] = r1[i] = 0;
+#pragma unroll
+  for (int i = 0; i < (SMALL ? 1 : G); i++) lo0[i] = hi0[i] = lo1[i] = hi1[i] = 0;
+#pragma unroll
+  for (int i = 0; i < (SMALL ? G : 1); i++) A0[i] = Acc3{0, 0, 0}, A1[i] = Acc3{0, 0, 0};
+  const int max_lazy = SMALL ? (p.max_lazy < 1024 ? p.max_lazy : 1024) : p.max_lazy;
   int lazy = 0;
   for (int t0 = 0; t0 < g.n_terms; t0 += MAC_TILE) {
     const int nt = g.n_terms - t0 < MAC_TILE ? g.n_terms - t0 : MAC_TILE;
@@ -57,17 +81,33 @@ __global__ void __launch_bounds__(256, 3) mac_kernel(MacP p) {
       u64 w[G];
 #pragma unroll
       for (int i = 0; i < G; i++) w[i] = __ldg(s_pt[i][t] + idx);
-#pragma unroll
-      for (int i = 0; i < G; i++) {
-        mac128(lo0[i], hi0[i], x0, w[i]);
-        mac128(lo1[i], hi1[i], x1, w[i]);
-      }
-      if (++lazy == p.max_lazy) {
+      if (SMALL) {
+        const u32 m26 = (1u << 26) - 1;
+        const u32 x00 = (u32)x0 & m26, x01 = (u32)(x0 >> 26), x10 = (u32)x1 & m26, x11 = (u32)(x1 >> 26);
 #pragma unroll
         for (int i = 0; i < G; i++) {
-          r0[i] = addmod(r0[i], mont_redc(lo0[i], hi0[i], mc.q, mc.qinv_neg), mc.q);
-          r1[i] = addmod(r1[i], mont_redc(lo1[i], hi1[i], mc.q, mc.qinv_neg), mc.q);
-          lo0[i] = hi0[i] = lo1[i] = hi1[i] = 0;
+          const u32 w0 = (u32)w[i] & m26, w1 = (u32)(w[i] >> 26);
+          acc3_mac(A0[i], x00, x01, w0, w1);
+          acc3_mac(A1[i], x10, x11, w0, w1);
+        }
+      } else {
+#pragma unroll
+        for (int i = 0; i < G; i++) {
+          mac128(lo0[i], hi0[i], x0, w[i]);
+          mac128(lo1[i], hi1[i], x1, w[i]);
+        }
+      }
+      if (++lazy == max_lazy) {
+#pragma unroll
+        for (int i = 0; i < G; i++) {
+          if (SMALL) {
+            r0[i] = addmod(r0[i], acc3_redc(A0[i], mc.q, mc.qinv_neg), mc.q);
+            r1[i] = addmod(r1[i], acc3_redc(A1[i], mc.q, mc.qinv_neg), mc.q);
+          } else {
+            r0[i] = addmod(r0[i], mont_redc(lo0[i], hi0[i], mc.q, mc.qinv_neg), mc.q);
+            r1[i] = addmod(r1[i], mont_redc(lo1[i], hi1[i], mc.q, mc.qinv_neg), mc.q);
+            lo0[i] = hi0[i] = lo1[i] = hi1[i] = 0;
+          }
         }
         lazy = 0;
       }
@@ -78,20 +118,31 @@ __global__ void __launch_bounds__(256, 3) mac_kernel(MacP p) {
   for (int i = 0; i < G; i++) {
     if (i < g.n_out) {
       u64 *out = p.outs[g.out_start + i];
-      out[idx] = addmod(r0[i], mont_redc(lo0[i], hi0[i], mc.q, mc.qinv_neg), mc.q);
-      out[LN + idx] = addmod(r1[i], mont_redc(lo1[i], hi1[i], mc.q, mc.qinv_neg), mc.q);
+      if (SMALL) {
+        out[idx] = addmod(r0[i], acc3_redc(A0[i], mc.q, mc.qinv_neg), mc.q);
+        out[LN + idx] = addmod(r1[i], acc3_redc(A1[i], mc.q, mc.qinv_neg), mc.q);
+      } else {
+        out[idx] = addmod(r0[i], mont_redc(lo0[i], hi0[i], mc.q, mc.qinv_neg), mc.q);
+        out[LN + idx] = addmod(r1[i], mont_redc(lo1[i], hi1[i], mc.q, mc.qinv_neg), mc.q);
+      }
     }
   }
 }
 int k_mac(const KCtx &k, const MacGroup *groups, int n_groups, int max_group, const u64 *const *term_ct, const u64 *const *term_pt,
-          u64 *const *outs, int L, int max_lazy, double alg_bytes) {
+          u64 *const *outs, int L, int max_lazy, bool small_moduli, double alg_bytes) {
   if (n_groups == 0) return 0;
   MacP p{groups, term_ct, term_pt, outs, k.d_mods, L, k.geom.logN, max_lazy};
   dim3 grid(n_groups, (unsigned)(((size_t)L * k.N + 255) / 256));
   PROF(k, K_MAC, alg_bytes);
-  if (max_group <= 1) mac_kernel<1><<<grid, 256, 0, S(k)>>>(p);
-  else if (max_group <= 2) mac_kernel<2><<<grid, 256, 0, S(k)>>>(p);
-  else mac_kernel<4><<<grid, 256, 0, S(k)>>>(p);
+  if (small_moduli) {
+    if (max_group <= 1) mac_kernel<1, true><<<grid, 256, 0, S(k)>>>(p);
+    else if (max_group <= 2) mac_kernel<2, true><<<grid, 256, 0, S(k)>>>(p);
+    else mac_kernel<4, true><<<grid, 256, 0, S(k)>>>(p);
+  } else {
+    if (max_group <= 1) mac_kernel<1, false><<<grid, 256, 0, S(k)>>>(p);
+    else if (max_group <= 2) mac_kernel<2, false><<<grid, 256, 0, S(k)>>>(p);
+    else mac_kernel<4, false><<<grid, 256, 0, S(k)>>>(p);
+  }
   LAUNCH_CHECK(k);
   return 0;
 }

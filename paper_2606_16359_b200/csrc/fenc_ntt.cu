@@ -26,6 +26,30 @@
       default: { constexpr int GEO = 0; CALL; } break;     \
     }                                                      \
   } while (0)
+// Tile fill / drain with all of a thread's (<= 8) global accesses independent and in flight together: the loads are issued
+// first, the shared-memory stores after (a rolled loop would serialise one L2/HBM latency per element).
+template <class F>
+DEVI void tile_fill(u64 *sm, int T, int tid, int nth, F f) {
+  u64 v[8];
+#pragma unroll
+  for (int i = 0; i < 8; i++) {
+    const int e = tid + i * nth;
+    if (e < T) v[i] = f(e);
+  }
+#pragma unroll
+  for (int i = 0; i < 8; i++) {
+    const int e = tid + i * nth;
+    if (e < T) sm[swz(e)] = v[i];
+  }
+}
+template <class F>
+DEVI void tile_drain(const u64 *sm, int T, int tid, int nth, F f) {
+#pragma unroll
+  for (int i = 0; i < 8; i++) {
+    const int e = tid + i * nth;
+    if (e < T) f(e, sm[swz(e)]);
+  }
+}
 static inline int nthreads_for(int lt) { int t = 1 << (lt - 3); return t < 32 ? 32 : t; }
 #define PROF(k, id, bytes) if ((k).prof) prof_begin((k).prof, (k).stream, id, (double)(bytes))
 #define LAUNCH_CHECK(k)                            \
@@ -42,7 +66,7 @@ struct InttRowP {
   const RowDesc *rows; const ModConst *mods; const ShoupC *tw; NttGeom g;
 };
 template <bool GATHER, int GEO>
-__global__ void __launch_bounds__(256) intt_rowpass_kernel(InttRowP p) {
+__global__ void __launch_bounds__(256, 4) intt_rowpass_kernel(InttRowP p) {
   extern __shared__ u64 sm[];
   const int tid = threadIdx.x, b = blockIdx.z;
   const RowDesc rd = p.rows[blockIdx.y];
@@ -50,15 +74,16 @@ __global__ void __launch_bounds__(256) intt_rowpass_kernel(InttRowP p) {
   TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, blockIdx.x};
   const u64 *src = (p.items ? p.items[b].ks_in : p.src + (size_t)b * p.src_bstride) + (size_t)rd.src_row * N;
   const u32 gal = GATHER ? p.items[b].g : 1u;
-  for (int e = tid; e < T; e += blockDim.x) {
-    u32 j = G.gidx(e);
-    sm[swz(e)] = __ldg(src + (GATHER ? galois_src(j, gal, p.g.logN) : j));
-  }
+  const int logN = p.g.logN, nth = blockDim.x;
+  tile_fill(sm, T, tid, nth, [&](int e) {
+    const u32 j = G.gidx(e);
+    return __ldg(src + (GATHER ? galois_src(j, gal, logN) : j));
+  });
   __syncthreads();
   const u64 q = p.mods[rd.mod].q;
   tile_transform<false, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid);
   u64 *dst = p.dst + (size_t)b * p.dst_bstride + (size_t)rd.dst_row * N;
-  for (int e = tid; e < T; e += blockDim.x) dst[G.gidx(e)] = sm[swz(e)];
+  tile_drain(sm, T, tid, nth, [&](int e, u64 v) { dst[G.gidx(e)] = v; });
 }
 
 // ------------------------------------------------------------------------------------------------ inverse, pass B
@@ -73,12 +98,13 @@ __global__ void __launch_bounds__(512) intt_colpass_kernel(InttColP p) {
   const int N = 1 << p.g.logN, T = 1 << p.g.lt_col;
   TileGeo G{p.g.lt_col, p.g.lc_col, p.g.brow, p.g.logN, blockIdx.x};
   u64 *dst = p.dst + (size_t)b * p.dst_bstride + (size_t)rd.dst_row * N;
-  for (int e = tid; e < T; e += blockDim.x) sm[swz(e)] = dst[G.gidx(e)];
+  const int nth = blockDim.x;
+  tile_fill(sm, T, tid, nth, [&](int e) { return dst[G.gidx(e)]; });
   __syncthreads();
   const u64 q = p.mods[rd.mod].q;
   tile_transform<false, GEO>(sm, G, p.g.lc_col, p.g.bcol, p.tw + (size_t)rd.mod * N, q, tid);
   const ShoupC sc = p.scale[blockIdx.y];
-  for (int e = tid; e < T; e += blockDim.x) dst[G.gidx(e)] = shoup_mul(sm[swz(e)], sc.c, sc.cs, q);
+  tile_drain(sm, T, tid, nth, [&](int e, u64 v) { dst[G.gidx(e)] = shoup_mul(v, sc.c, sc.cs, q); });
 }
 
 int k_intt(const KCtx &k, const BatchItem *items, const u64 *src, size_t src_bstride, bool gather, u64 *dst,
@@ -106,7 +132,7 @@ struct NttColP {
   const RowDesc *rows; const ModConst *mods; const ShoupC *tw; NttGeom g;
 };
 template <bool BCONV, int GEO>
-__global__ void __launch_bounds__(512) ntt_colpass_kernel(NttColP p) {
+__global__ void __launch_bounds__(512, 2) ntt_colpass_kernel(NttColP p) {
   extern __shared__ u64 sm[];
   const int tid = threadIdx.x, b = blockIdx.z;
   const RowDesc rd = p.rows[blockIdx.y];
@@ -114,23 +140,39 @@ __global__ void __launch_bounds__(512) ntt_colpass_kernel(NttColP p) {
   TileGeo G{p.g.lt_col, p.g.lc_col, p.g.brow, p.g.logN, blockIdx.x};
   const ModConst mc = p.mods[rd.mod];
   const u64 *src = p.src + (size_t)b * p.src_bstride + (size_t)rd.src_row * N;
+  const int nth = blockDim.x;
   if (BCONV) {
     // fused base conversion (R2.6): sum_s y_s * (Qhat_s mod t), one Montgomery reduction
     const u64 *bc = p.bc + rd.aux2;
     const int ns = rd.aux;
-    for (int e = tid; e < T; e += blockDim.x) {
-      u32 j = G.gidx(e);
-      u64 lo = 0, hi = 0;
-      for (int s = 0; s < ns; s++) mac128(lo, hi, __ldg(src + (size_t)s * N + j), __ldg(bc + s));
-      sm[swz(e)] = mont_redc(lo, hi, mc.q, mc.qinv_neg);
+    // source-major in two halves: the 4 elements' loads of one source row are in flight together
+#pragma unroll
+    for (int h = 0; h < 8; h += 4) {
+      u64 lo[4], hi[4];
+      u32 j[4];
+#pragma unroll
+      for (int i = 0; i < 4; i++) lo[i] = hi[i] = 0, j[i] = G.gidx((tid + (h + i) * nth) & (T - 1));
+      for (int s = 0; s < ns; s++) {
+        const u64 c = __ldg(bc + s);
+        u64 y[4];
+#pragma unroll
+        for (int i = 0; i < 4; i++) y[i] = __ldg(src + (size_t)s * N + j[i]);
+#pragma unroll
+        for (int i = 0; i < 4; i++) mac128(lo[i], hi[i], y[i], c);
+      }
+#pragma unroll
+      for (int i = 0; i < 4; i++) {
+        const int e = tid + (h + i) * nth;
+        if (e < T) sm[swz(e)] = mont_redc(lo[i], hi[i], mc.q, mc.qinv_neg);
+      }
     }
   } else {
-    for (int e = tid; e < T; e += blockDim.x) sm[swz(e)] = __ldg(src + G.gidx(e));
+    tile_fill(sm, T, tid, nth, [&](int e) { return __ldg(src + G.gidx(e)); });
   }
   __syncthreads();
   tile_transform<true, GEO>(sm, G, p.g.lc_col, p.g.bcol, p.tw + (size_t)rd.mod * N, mc.q, tid);
   u64 *dst = p.dst + (size_t)b * p.dst_bstride + (size_t)rd.dst_row * N;
-  for (int e = tid; e < T; e += blockDim.x) dst[G.gidx(e)] = sm[swz(e)];  // lazy, in [0,4q)
+  tile_drain(sm, T, tid, nth, [&](int e, u64 v) { dst[G.gidx(e)] = v; });  // lazy, below 33q
 }
 
 // ------------------------------------------------------------------------------------------------ forward, pass 2 (plain)
@@ -139,19 +181,20 @@ struct NttRowP {
   const ShoupC *tw; NttGeom g; int src_is_dst_row;
 };
 template <int GEO>
-__global__ void __launch_bounds__(256) ntt_rowpass_kernel(NttRowP p) {
+__global__ void __launch_bounds__(256, 4) ntt_rowpass_kernel(NttRowP p) {
   extern __shared__ u64 sm[];
   const int tid = threadIdx.x, b = blockIdx.z;
   const RowDesc rd = p.rows[blockIdx.y];
   const int N = 1 << p.g.logN, T = 1 << p.g.lt_row;
   TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, blockIdx.x};
   const u64 *src = p.src + (size_t)b * p.src_bstride + (size_t)(p.src_is_dst_row ? rd.dst_row : rd.src_row) * N;
-  for (int e = tid; e < T; e += blockDim.x) sm[swz(e)] = src[G.gidx(e)];
+  const int nth = blockDim.x;
+  tile_fill(sm, T, tid, nth, [&](int e) { return src[G.gidx(e)]; });
   __syncthreads();
   const ModConst mc = p.mods[rd.mod];
   tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, mc.q, tid);
   u64 *dst = p.dst + (size_t)b * p.dst_bstride + (size_t)rd.dst_row * N;
-  for (int e = tid; e < T; e += blockDim.x) dst[G.gidx(e)] = fullred(sm[swz(e)], mc.q, mc.qbar);
+  tile_drain(sm, T, tid, nth, [&](int e, u64 v) { dst[G.gidx(e)] = fullred(v, mc.q, mc.qbar); });
 }
 
 int k_ntt(const KCtx &k, const u64 *src, size_t src_bstride, u64 *dst, size_t dst_bstride, const RowDesc *rows, int n_rows,
@@ -209,26 +252,38 @@ __global__ void __launch_bounds__(256, 2) ntt_rows_keymac_kernel(KeyMacP p) {
 #pragma unroll
   for (int i = 0; i < EPT; i++) a0l[i] = a0h[i] = a1l[i] = a1h[i] = 0;
   const int nth = blockDim.x;
+  constexpr int HB = EPT < 4 ? EPT : 4;
   for (int j = 0; j < p.beta; j++) {
     const int ti = p.tmp_index[j * p.E + t];
     const u64 *kb = it.evk + ((size_t)(j * 2 + 0) * p.A + mod) * N;
     const u64 *ka = it.evk + ((size_t)(j * 2 + 1) * p.A + mod) * N;
     if (ti >= 0) {
       const u64 *src = p.tmp + (size_t)b * p.tmp_bstride + (size_t)ti * N;
-      for (int e = tid; e < T; e += nth) sm[swz(e)] = src[G.gidx(e)];
+      tile_fill(sm, T, tid, nth, [&](int e) { return src[G.gidx(e)]; });
       __syncthreads();
       tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)mod * N, mc.q, tid);
     }
+    // the key words (and, inside the digit, the permuted input words) of 4 elements are loaded together, then used
 #pragma unroll
-    for (int i = 0; i < EPT; i++) {
-      const int e = tid + i * nth;
-      if (e < T) {
-        const u32 jj = G.gidx(e);
-        u64 x;
-        if (ti >= 0) x = fullred(sm[swz(e)], mc.q, mc.qbar);
-        else x = __ldg(it.ks_in + (size_t)t * N + galois_src(jj, it.g, p.g.logN));
-        mac128(a0l[i], a0h[i], x, __ldg(kb + jj));
-        mac128(a1l[i], a1h[i], x, __ldg(ka + jj));
+    for (int h = 0; h < EPT; h += HB) {
+      u64 x[HB], vb[HB], va[HB];
+      u32 jj[HB];
+#pragma unroll
+      for (int i = 0; i < HB; i++) {
+        const int e = (tid + (h + i) * nth) & (T - 1);
+        jj[i] = G.gidx(e);
+        vb[i] = __ldg(kb + jj[i]);
+        va[i] = __ldg(ka + jj[i]);
+        if (ti >= 0) x[i] = sm[swz(e)];
+        else x[i] = __ldg(it.ks_in + (size_t)t * N + galois_src(jj[i], it.g, p.g.logN));
+      }
+#pragma unroll
+      for (int i = 0; i < HB; i++) {
+        if (tid + (h + i) * nth < T) {
+          const u64 xx = ti >= 0 ? fullred(x[i], mc.q, mc.qbar) : x[i];
+          mac128(a0l[h + i], a0h[h + i], xx, vb[i]);
+          mac128(a1l[h + i], a1h[h + i], xx, va[i]);
+        }
       }
     }
     __syncthreads();
@@ -272,30 +327,42 @@ struct DivideP {
   const RowDesc *rows; const ModConst *mods; const ShoupC *tw; NttGeom g; int from_items;
 };
 template <int GEO>
-__global__ void __launch_bounds__(256) ntt_rows_divide_kernel(DivideP p) {
+__global__ void __launch_bounds__(256, 3) ntt_rows_divide_kernel(DivideP p) {
   extern __shared__ u64 sm[];
   const int tid = threadIdx.x, b = blockIdx.z;
   const RowDesc rd = p.rows[blockIdx.y];
   const int N = 1 << p.g.logN, T = 1 << p.g.lt_row;
   TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, blockIdx.x};
   const u64 *src = p.tmp + (size_t)b * p.tmp_bstride + (size_t)rd.src_row * N;
-  for (int e = tid; e < T; e += blockDim.x) sm[swz(e)] = src[G.gidx(e)];
-  __syncthreads();
-  const ModConst mq = p.mods[rd.mod];
-  const u64 q = mq.q;
-  tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid);
+  const int nth = blockDim.x, logN = p.g.logN;
   const BatchItem it = p.items[b];
   const u64 *minuend = (p.from_items ? it.sub_in : p.acc + (size_t)b * p.acc_bstride) + (size_t)rd.aux2 * N;
   const u64 *addend = rd.aux == 0 ? it.add0 : it.add1;
   if (addend) addend += (size_t)rd.mod * N;
+  // epilogue operands are fetched BEFORE the transform so that their latency hides behind it
+  u64 mi[8], ad[8];
+#pragma unroll
+  for (int i = 0; i < 8; i++) {
+    const u32 j = G.gidx((tid + i * nth) & (T - 1));
+    mi[i] = __ldg(minuend + j);
+    ad[i] = addend ? __ldg(addend + galois_src(j, it.g, logN)) : 0;
+  }
+  tile_fill(sm, T, tid, nth, [&](int e) { return src[G.gidx(e)]; });
+  __syncthreads();
+  const ModConst mq = p.mods[rd.mod];
+  const u64 q = mq.q;
+  tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid);
   const ShoupC mc = p.mul[rd.mod];
   u64 *dst = it.out + (size_t)rd.dst_row * N;
-  for (int e = tid; e < T; e += blockDim.x) {
-    const u32 j = G.gidx(e);
-    const u64 x = fullred(sm[swz(e)], q, mq.qbar);
-    u64 v = shoup_mul(submod(__ldg(minuend + j), x, q), mc.c, mc.cs, q);
-    if (addend) v = addmod(v, __ldg(addend + galois_src(j, it.g, p.g.logN)), q);
-    dst[j] = v;
+#pragma unroll
+  for (int i = 0; i < 8; i++) {
+    const int e = tid + i * nth;
+    if (e < T) {
+      const u64 x = fullred(sm[swz(e)], q, mq.qbar);
+      u64 v = shoup_mul(submod(mi[i], x, q), mc.c, mc.cs, q);
+      v = addmod(v, ad[i], q);
+      dst[G.gidx(e)] = v;
+    }
   }
 }
 
