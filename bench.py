@@ -109,8 +109,73 @@ WORKLOADS = {
                               "BASELINE config 2, conv stage: conv1-x^2-pool-conv2-x^2-pool, N=2^14, 8x40b+2x60b, dnum=4"),
     "cfg2_lenet5": ("cfg2", lambda bs, seed: lenet_layers(bs, seed, upto="fc"),
                     "BASELINE config 2: LeNet-5-shaped network, N=2^14, 8x40b+2x60b, dnum=4"),
+    # single layers (parity-test configurations, timed for the record; --batch is ignored: BS = 1 as in BASELINE.json)
+    "cfg1_conv1": ("cfg1", lambda bs, seed: conv_layers("lenet_conv1", seed),
+                   "BASELINE config 1: LeNet conv1-shaped layer, N=2^13, 3x40b+1x60b, dlen=1 (A1), batch 1"),
+    "cfg3_conv_16_16": ("cfg3", lambda bs, seed: conv_layers("resnet_16_16", seed, True),
+                        "BASELINE config 3: ResNet-20 3x3 16->16 layer, N=2^16, 24x50b+4x60b, dnum=6, batch 1"),
+    "cfg3_conv_16_32_s2": ("cfg3", lambda bs, seed: conv_layers("resnet_16_32_s2", seed, True),
+                           "BASELINE config 3: ResNet-20 3x3 16->32 stride 2, N=2^16, batch 1"),
+    "cfg3_conv_32_64_s2": ("cfg3", lambda bs, seed: conv_layers("resnet_32_64_s2", seed, True),
+                           "BASELINE config 3: ResNet-20 3x3 32->64 stride 2, N=2^16, batch 1"),
+    "cfg5_rotsweep": (None, None, "BASELINE config 5: rotation / key-switch sweep"),
 }
 DEFAULT_WORKLOAD = "cfg2_lenet5"
+
+
+def conv_layers(name, seed, kaiming=False):
+    """one encrypted conv layer of a BASELINE config at the top level (reading A20), planner-selected S."""
+    kw = wl.CONVS[name]
+    x, w = wl.conv_inputs(seed, kw, kaiming=kaiming)
+    return [{"op": "conv", "conv": dict(kw), "S": 0, "w": w}], x
+
+
+def run_rotsweep(args):
+    """BASELINE config 5: rotation / key-switch sweep at N=2^16 (reading A2: k = dlen = ceil(L/dnum)).  64 ciphertexts with
+    uniform-random limbs, 32 distinct seeded rotation amounts; every amount is one batched fenc_rotate over the 64."""
+    import torch
+    import paper_2606_16359_b200 as fenc
+    peaks, peak_src = measured_peaks()
+    n_ct, n_steps, points = 64, 32, []
+    for L in (4, 8, 16, 24, 36):
+        for dnum in (1, 2, 3, 4):
+            pr = wl.sweep_params(L, dnum)
+            ctx = fenc.Context(**pr)
+            N, k, dlen = ctx.N, ctx.n_p, ctx.dlen
+            beta = -(-L // dlen)
+            steps = wl.rotation_steps(5000 + L * 10 + dnum, n_steps, ctx.n)
+            keys = ctx.keygen(5, steps)
+            cts = [ctx.ct_import(wl.random_ct_limbs(100 * L + i, ctx.q, L, N)) for i in range(n_ct)]
+            for r in steps[:2]:
+                ctx.rotate(keys, cts, [r] * n_ct)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ctx.launch_count(reset=True)
+            e0.record()
+            for r in steps:
+                out = ctx.rotate(keys, cts, [r] * n_ct)
+                del out
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            rots = n_ct * n_steps
+            # algorithmic bytes per rotation (SURVEY.md 8(d)): ciphertext in + out, key once per batch of 64
+            b_alg = 2 * (2 * L * N * 8) + 2 * beta * (L + k) * N * 8 / n_ct
+            gbs = rots * b_alg / (ms * 1e-3) / 1e9
+            points.append({"L": L, "dnum": dnum, "dlen": dlen, "k": k, "beta": beta,
+                           "ntt_per_rot": beta * (L + k) + 2 * k + 2 * L, "rot_per_s": round(rots / (ms * 1e-3), 1),
+                           "us_per_rot": round(ms * 1e3 / rots, 2), "alg_GBps": round(gbs, 1),
+                           "hbm_frac": round(gbs / peaks["hbm_gbs"], 4), "launches": ctx.launch_count()})
+            del cts, keys
+            ctx.close()
+            torch.cuda.empty_cache()
+    ref = [p for p in points if p["L"] == 24 and p["dnum"] == 3][0]
+    return {"metric": METRIC, "value": ref["rot_per_s"], "unit": "key-switched rotations/s", "n_gpus": 1, "steps": n_steps,
+            "warmup": 2, "ms_per_step": round(1e3 * n_ct / ref["rot_per_s"], 4), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+            "config": {"workload": "cfg5_rotsweep", "description": "BASELINE config 5: N=2^16, 64 cts x 32 amounts per point; "
+                       "value quoted at L=24, dnum=3", "peak_source": peak_src, "hbm_peak_GBps": peaks["hbm_gbs"]},
+            "points": points}
 
 
 def run_ours(args, rank, world):
@@ -122,6 +187,7 @@ def run_ours(args, rank, world):
     pkey, builder, desc = WORKLOADS[args.workload]
     seed = 2000 + rank
     layers, x = builder(args.batch, seed)
+    args.batch = int(layers[0]["conv"]["BS"])
     ctx = fenc.Context(device=dev, **wl.PARAMS[pkey])
     pipe = Pipeline(ctx, layers)
     pipe.setup(key_seed=seed)
@@ -169,17 +235,28 @@ def run_ours(args, rank, world):
     prof_ms = (time.perf_counter() - t0) * 1e3 / prof_steps
     ctx.profile_enable(False)
     peaks, peak_src = measured_peaks()
+    imad_peak, bfly_peak = ctx.measure_alu_peak()
     tot = sum(v[0] for v in prof.values())
     top = max(prof, key=lambda k: prof[k][0])
-    t_ms, t_cnt, t_bytes = prof[top]
-    achieved = t_bytes / (t_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": top, "achieved": round(achieved, 1), "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": round(achieved / peaks["hbm_gbs"], 4), "traffic": None, "peak_source": peak_src,
-                "avg_launch_us": round(t_ms * 1e3 / t_cnt, 2), "share_of_step": round(t_ms / tot, 4),
-                "alg_bytes_per_launch": t_bytes / t_cnt,
-                "per_kernel": {k: {"ms_per_step": round(v[0] / prof_steps, 4), "launches_per_step": v[1] // prof_steps,
-                                   "alg_GBps": round(v[2] / (v[0] * 1e-3) / 1e9, 1)} for k, v in sorted(prof.items(), key=lambda kv: -kv[1][0])},
-                "profiled_step_ms": round(prof_ms, 3)}
+    t_ms, t_cnt, t_bytes, t_ops = prof[top]
+    hbm_ach, alu_ach = t_bytes / (t_ms * 1e-3) / 1e9, t_ops / (t_ms * 1e-3)
+    per_kernel = {k: {"ms_per_step": round(v[0] / prof_steps, 4), "launches_per_step": v[1] // prof_steps,
+                      "alg_GBps": round(v[2] / (v[0] * 1e-3) / 1e9, 1), "hbm_frac": round(v[2] / (v[0] * 1e-3) / 1e9 / peaks["hbm_gbs"], 4),
+                      "Gbutterflies_per_s": round(v[3] / (v[0] * 1e-3) / 1e9, 1), "alu_frac": round(v[3] / (v[0] * 1e-3) / bfly_peak, 4)}
+                  for k, v in sorted(prof.items(), key=lambda kv: -kv[1][0])}
+    # the NTT-carrying kernels are bound by the integer pipes: report the roof the kernel is nearer to
+    if t_ops and alu_ach / bfly_peak >= hbm_ach / peaks["hbm_gbs"]:
+        roofline = {"bound": "alu", "kernel": top, "achieved": round(alu_ach / 1e9, 2), "peak": round(bfly_peak / 1e9, 2),
+                    "unit": "G modular butterflies/s", "frac": round(alu_ach / bfly_peak, 4), "traffic": None,
+                    "peak_source": "measured live: register-only Shoup butterflies of this library on all SMs "
+                                   "(fenc_measure_alu_peak); 32-bit IMAD peak %.2f T lane-ops/s" % (imad_peak / 1e12),
+                    "butterflies_per_launch": t_ops / t_cnt, "hbm_frac_of_same_kernel": round(hbm_ach / peaks["hbm_gbs"], 4)}
+    else:
+        roofline = {"bound": "hbm", "kernel": top, "achieved": round(hbm_ach, 1), "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                    "frac": round(hbm_ach / peaks["hbm_gbs"], 4), "traffic": None, "peak_source": peak_src}
+    roofline.update({"avg_launch_us": round(t_ms * 1e3 / t_cnt, 2), "share_of_step": round(t_ms / tot, 4),
+                     "alg_bytes_per_launch": t_bytes / t_cnt, "per_kernel": per_kernel, "profiled_step_ms": round(prof_ms, 3),
+                     "hbm_peak_GBps": peaks["hbm_gbs"], "hbm_peak_source": peak_src})
     # ---- end to end through the C ABI with host buffers: import (H2D + NTT), forward, export (iNTT + D2H)
     host_in = [ctx.ct_export(c) for c in cts]
     s_in = cts[0].scale
@@ -300,7 +377,8 @@ def run_reference(args):
     for ly in layers:
         o = ops.setdefault(L, [0, 0, 0, 0])
         if ly["op"] == "conv":
-            g = fr.ConvGraph(fr.ConvDesc(S=ly["S"], **ly["conv"]), P_n)
+            S = ly["S"] or fr.select_S(fr.ConvDesc(**ly["conv"]), P_n)
+            g = fr.ConvGraph(fr.ConvDesc(S=S, **ly["conv"]), P_n)
             c = g.counts()
             o[0] += c["n_inner_rot"] + c["n_outer_rot"]; o[1] += c["n_pmult"]; o[2] += c["n_out_ct"]
             n_ct, n_lin = c["n_out_ct"], n_lin + 1
@@ -356,7 +434,7 @@ def main():
         import torch
         torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", 0)))
         torch.distributed.init_process_group("nccl")
-    line = run_ours(args, rank, world)
+    line = run_rotsweep(args) if args.workload == "cfg5_rotsweep" else run_ours(args, rank, world)
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:

@@ -220,11 +220,16 @@ fenc_status fenc_compress(fenc_ctx *ctx, const fenc_keys *keys, fenc_ct *const *
  * array, row r uses modulus mod_idx[r] (0..n_q-1 ciphertext primes, n_q.. special primes). */
 fenc_status fenc_ntt_rows(fenc_ctx *ctx, void *device_rows, const int32_t *mod_idx, size_t n_rows, int inverse);
 /* Per-kernel-class timing with CUDA events on the context's stream, and the algorithmic bytes each launch moved
- * (DESIGN.md section 7).  Off by default.  ms / launches / alg_bytes: host arrays of fenc_profile_kernels() entries. */
+ * and the modular butterflies it computed.  Off by default.  ms / launches / alg_bytes /
+ * alg_butterflies: host arrays of fenc_profile_kernels() entries. */
 fenc_status fenc_profile_enable(fenc_ctx *ctx, int on);
 int fenc_profile_kernels(void);
 const char *fenc_profile_name(int id);
-fenc_status fenc_profile_read(fenc_ctx *ctx, double *ms, uint64_t *launches, double *alg_bytes, int reset);
+fenc_status fenc_profile_read(fenc_ctx *ctx, double *ms, uint64_t *launches, double *alg_bytes, double *alg_butterflies,
+                              int reset);
+/* Measured integer-pipe ceilings on this device: dependency-free 32-bit IMAD lane-ops/s, and
+ * register-only forward Shoup butterflies/s of the library's own butterfly (no memory traffic). */
+fenc_status fenc_measure_alu_peak(fenc_ctx *ctx, double *imad_lane_ops_per_s, double *butterflies_per_s);
 /* counters since context creation: kernels launched by this library; optional reset */
 uint64_t fenc_launch_count(fenc_ctx *ctx, int reset);
 /* bytes currently held through the allocator */

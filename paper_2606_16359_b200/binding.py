@@ -63,7 +63,7 @@ SYMBOLS = ["fenc_params_init", "fenc_ctx_free", "fenc_last_error", "fenc_get_pri
            "fenc_wts_keys", "fenc_conv_weights", "fenc_conv_weights_from_coeffs", "fenc_wts_free", "fenc_hconv",
            "fenc_compress", "fenc_ntt_rows", "fenc_launch_count", "fenc_device_bytes", "fenc_sum_groups",
            "fenc_profile_enable", "fenc_profile_kernels", "fenc_profile_name", "fenc_profile_read", "fenc_fc_plan",
-           "fenc_fc_wts_keys", "fenc_fc_weights", "fenc_fc_weights_from_coeffs", "fenc_fc"]
+           "fenc_fc_wts_keys", "fenc_fc_weights", "fenc_fc_weights_from_coeffs", "fenc_fc", "fenc_measure_alu_peak"]
 
 _lib = None
 
@@ -104,7 +104,8 @@ def load_library(path=None):
         "fenc_square_relin": [vp, vp, vpp, C.c_size_t, vpp],
         "fenc_sum_groups": [vp, vpp, C.c_size_t, C.c_size_t, vpp],
         "fenc_profile_enable": [vp, C.c_int],
-        "fenc_profile_read": [vp, dp, u64p, dp, C.c_int],
+        "fenc_measure_alu_peak": [vp, dp, dp],
+        "fenc_profile_read": [vp, dp, u64p, dp, dp, C.c_int],
         "fenc_wts_keys": [vp, C.POINTER(ConvDesc), C.POINTER(Layout), u32p, C.c_size_t, C.POINTER(C.c_size_t)],
         "fenc_conv_weights": [vp, C.POINTER(ConvDesc), C.POINTER(Layout), dp, C.c_uint32, C.c_double, vpp],
         "fenc_conv_weights_from_coeffs": [vp, C.POINTER(ConvDesc), C.POINTER(Layout), i64p, C.c_size_t, C.c_uint32,
@@ -395,15 +396,22 @@ class Context:
         self._ck(self.lib.fenc_sum_groups(self.h, self._harr(cts), group, n, out))
         return [Ciphertext(self, C.c_void_p(out[i])) for i in range(n)]
 
+    def measure_alu_peak(self):
+        a, b = C.c_double(), C.c_double()
+        self._ck(self.lib.fenc_measure_alu_peak(self.h, C.byref(a), C.byref(b)))
+        return a.value, b.value
+
     def profile_enable(self, on=True):
         self._ck(self.lib.fenc_profile_enable(self.h, int(on)))
 
     def profile_read(self, reset=True):
-        """{kernel class: (ms, launches, algorithmic bytes)} accumulated since the last reset."""
+        """{kernel class: (ms, launches, algorithmic bytes, modular butterflies)} accumulated since the last reset."""
         k = self.lib.fenc_profile_kernels()
-        ms, cnt, by = np.zeros(k), np.zeros(k, dtype=np.uint64), np.zeros(k)
-        self._ck(self.lib.fenc_profile_read(self.h, _ptr(ms, C.c_double), _ptr(cnt, C.c_uint64), _ptr(by, C.c_double), int(reset)))
-        return {self.lib.fenc_profile_name(i).decode(): (float(ms[i]), int(cnt[i]), float(by[i])) for i in range(k) if cnt[i]}
+        ms, cnt, by, op = np.zeros(k), np.zeros(k, dtype=np.uint64), np.zeros(k), np.zeros(k)
+        self._ck(self.lib.fenc_profile_read(self.h, _ptr(ms, C.c_double), _ptr(cnt, C.c_uint64), _ptr(by, C.c_double),
+                                            _ptr(op, C.c_double), int(reset)))
+        return {self.lib.fenc_profile_name(i).decode(): (float(ms[i]), int(cnt[i]), float(by[i]), float(op[i]))
+                for i in range(k) if cnt[i]}
 
     # ---- HConv
     def wts_keys(self, conv, lay):

@@ -120,7 +120,9 @@ extern "C" fenc_status fenc_params_init(const fenc_params_desc *d, fenc_ctx **ou
   for (u64 m : q) qmax = m > qmax ? m : qmax;
   for (u64 m : p) pmax = m > pmax ? m : pmax;
   u64 allmax = qmax > pmax ? qmax : pmax;
-  if ((u64)ctx->dlen > ~0ull / qmax || (u64)ctx->np > ~0ull / pmax || (u64)ctx->beta_max > ~0ull / allmax) return FENC_ERR_PARAMS;
+  if ((u64)ctx->beta_max > ~0ull / allmax) return FENC_ERR_PARAMS;
+  ctx->lazy_q = (int)std::min<u64>(~0ull / qmax, 1u << 20);  // base-conversion terms per Montgomery reduction
+  ctx->lazy_p = (int)std::min<u64>(~0ull / pmax, 1u << 20);
   u64 ml = ~0ull / qmax;
   ctx->max_lazy = ml > (1u << 20) ? (1 << 20) : (int)ml;
   ctx->default_scale = std::ldexp(1.0, (int)d->log2_scale);
@@ -354,12 +356,12 @@ fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items) {
     // a2 + a1: iNTT of sigma_g(d), pre-scaled for ModUp
     CUDA_OK(ctx, k_intt(k, d_items, nullptr, 0, true, y, (size_t)L * N, P->d_rows_in, L, P->d_scale_in, nb));
     // a3 + a1 (pass 1): ModUp fused into the first NTT pass
-    CUDA_OK(ctx, k_ntt_cols_bconv(k, y, (size_t)L * N, P->d_bc_up, tmp, (size_t)P->n_up * N, P->d_rows_up, P->n_up, nb, L));
+    CUDA_OK(ctx, k_ntt_cols_bconv(k, y, (size_t)L * N, P->d_bc_up, tmp, (size_t)P->n_up * N, P->d_rows_up, P->n_up, nb, L, ctx->lazy_q));
     // a1 (pass 2) + a4: evk inner product
     CUDA_OK(ctx, k_ntt_rows_keymac(k, d_items, L, E, P->beta, P->d_tmp_index, tmp, (size_t)P->n_up * N, acc, (size_t)2 * E * N, nb, P->n_up, n_keys));
     // a5: ModDown = iNTT of the special limbs, conversion fused into pass 1, divide epilogue fused into pass 2
     CUDA_OK(ctx, k_intt(k, nullptr, acc, (size_t)2 * E * N, false, yP, (size_t)2 * np * N, P->d_rows_p, 2 * np, P->d_scale_p, nb));
-    CUDA_OK(ctx, k_ntt_cols_bconv(k, yP, (size_t)2 * np * N, P->d_bc_down, tmp2, (size_t)2 * L * N, P->d_rows_down, 2 * L, nb, 2 * np));
+    CUDA_OK(ctx, k_ntt_cols_bconv(k, yP, (size_t)2 * np * N, P->d_bc_down, tmp2, (size_t)2 * L * N, P->d_rows_down, 2 * L, nb, 2 * np, ctx->lazy_p));
     CUDA_OK(ctx, k_ntt_rows_divide(k, d_items, tmp2, (size_t)2 * L * N, acc, (size_t)2 * E * N, false, P->d_mul_pinv, P->d_rows_div, 2 * L, nb));
   }
   return FENC_OK;
@@ -387,7 +389,7 @@ fenc_status rescale_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items) {
     const BatchItem *d_items = (const BatchItem *)st.commit();
     if (!d_items) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
     CUDA_OK(ctx, k_intt(k, d_items, nullptr, 0, false, yR, 2 * N, P->d_rows_rs_in, 2, P->d_scale_rs, nb));
-    CUDA_OK(ctx, k_ntt_cols_bconv(k, yR, 2 * N, P->d_bc_rs, tmp2, (size_t)2 * L1 * N, P->d_rows_rs_up, 2 * L1, nb, 2));
+    CUDA_OK(ctx, k_ntt_cols_bconv(k, yR, 2 * N, P->d_bc_rs, tmp2, (size_t)2 * L1 * N, P->d_rows_rs_up, 2 * L1, nb, 2, ctx->lazy_q));
     CUDA_OK(ctx, k_ntt_rows_divide(k, d_items, tmp2, (size_t)2 * L1 * N, nullptr, 0, true, P->d_mul_qlinv, P->d_rows_rs_div, 2 * L1, nb));
   }
   return FENC_OK;

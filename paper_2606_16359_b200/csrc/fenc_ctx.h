@@ -56,7 +56,8 @@ struct fenc_ctx {
   int *d_ident_mod = nullptr;       // [2A] 0..A-1, 0..A-1
   KCtx k{};
   u64 launches = 0, dev_bytes = 0;
-  int max_lazy = 1;                 // floor(2^64 / max modulus): terms per lazy 128-bit accumulation
+  int max_lazy = 1;                 // floor(2^64 / max ciphertext modulus): terms per lazy 128-bit accumulation
+  int lazy_q = 1, lazy_p = 1;       // the same for base conversions out of the q limbs / the p limbs
   std::string err;
   std::map<int, std::unique_ptr<LevelPlan>> plans;
   std::map<void *, size_t> live;    // device pointer -> bytes (accounting)

@@ -13,7 +13,7 @@ typedef uint32_t u32;
 typedef unsigned __int128 u128;
 typedef long long i64;
 
-#define FENC_MAX_MOD 64  // moduli per context (n_q + n_p)
+#define FENC_MAX_MOD 96  // moduli per context (n_q + n_p)
 
 // ---------------------------------------------------------------- device-visible tables
 struct ModConst {  // one per modulus, device global memory
@@ -72,7 +72,7 @@ enum KernelId {
   K_COUNT
 };
 struct Prof;
-void prof_begin(Prof *p, void *stream, int id, double alg_bytes);
+void prof_begin(Prof *p, void *stream, int id, double alg_bytes, double alg_butterflies = 0);
 void prof_end(Prof *p, void *stream);
 
 struct KCtx {  // what kernels need from a context
@@ -98,7 +98,7 @@ int k_ntt(const KCtx &k, const u64 *src, size_t src_bstride, u64 *dst, size_t ds
 // forward pass 1 (column stages) with fused base conversion (ModUp a3 / ModDown's Conv / rescale's mod):
 // value = sum_{s < rows[r].aux} y[b][rows[r].src_row + s][.] * bc[rows[r].aux2 + s] (Montgomery constants)
 int k_ntt_cols_bconv(const KCtx &k, const u64 *y, size_t y_bstride, const u64 *bc, u64 *tmp, size_t tmp_bstride,
-                     const RowDesc *rows, int n_rows, int n_batch, int n_src_rows);
+                     const RowDesc *rows, int n_rows, int n_batch, int n_src_rows, int max_terms);
 // forward pass 2 (row stages) fused with the evaluation-key inner product (a4) over E = L + np target rows.
 // tmp_index[j*E + t] = row of tmp holding digit j / target t, or -1 when t lies in digit j (then the row is
 // items[b].ks_in[t] itself, read through the Galois gather).  acc[b][c][t][N] canonical.

@@ -51,7 +51,8 @@ DEVI void tile_drain(const u64 *sm, int T, int tid, int nth, F f) {
   }
 }
 static inline int nthreads_for(int lt) { int t = 1 << (lt - 3); return t < 32 ? 32 : t; }
-#define PROF(k, id, bytes) if ((k).prof) prof_begin((k).prof, (k).stream, id, (double)(bytes))
+#define PROF(k, id, bytes, bfly) if ((k).prof) prof_begin((k).prof, (k).stream, id, (double)(bytes), (double)(bfly))
+#define HALF_N(k) (0.5 * (k).N)
 #define LAUNCH_CHECK(k)                            \
   do {                                             \
     (*(k).launches)++;                             \
@@ -114,13 +115,13 @@ int k_intt(const KCtx &k, const BatchItem *items, const u64 *src, size_t src_bst
   const NttGeom &g = k.geom;
   InttRowP a{items, src, src_bstride, dst, dst_bstride, rows, k.d_mods, k.d_tw_inv, g};
   dim3 gridA(k.N >> g.lt_row, n_rows, n_batch);
-  PROF(k, K_INTT_ROW, 16.0 * k.N * n_rows * n_batch);
+  PROF(k, K_INTT_ROW, 16.0 * k.N * n_rows * n_batch, HALF_N(k) * g.brow * n_rows * n_batch);
   if (gather) ROW_GEO(g, (intt_rowpass_kernel<true, GEO><<<gridA, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(a)));
   else ROW_GEO(g, (intt_rowpass_kernel<false, GEO><<<gridA, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(a)));
   LAUNCH_CHECK(k);
   InttColP c{dst, dst_bstride, rows, scale, k.d_mods, k.d_tw_inv, g};
   dim3 gridB(k.N >> g.lt_col, n_rows, n_batch);
-  PROF(k, K_INTT_COL, 16.0 * k.N * n_rows * n_batch);
+  PROF(k, K_INTT_COL, 16.0 * k.N * n_rows * n_batch, HALF_N(k) * g.bcol * n_rows * n_batch);
   COL_GEO(g, (intt_colpass_kernel<GEO><<<gridB, nthreads_for(g.lt_col), sizeof(u64) << g.lt_col, st>>>(c)));
   LAUNCH_CHECK(k);
   return 0;
@@ -129,7 +130,7 @@ int k_intt(const KCtx &k, const BatchItem *items, const u64 *src, size_t src_bst
 // ------------------------------------------------------------------------------------------------ forward, pass 1
 struct NttColP {
   const u64 *src; size_t src_bstride; const u64 *bc; u64 *dst; size_t dst_bstride;
-  const RowDesc *rows; const ModConst *mods; const ShoupC *tw; NttGeom g;
+  const RowDesc *rows; const ModConst *mods; const ShoupC *tw; NttGeom g; int max_terms;
 };
 template <bool BCONV, int GEO>
 __global__ void __launch_bounds__(512, 2) ntt_colpass_kernel(NttColP p) {
@@ -148,10 +149,11 @@ __global__ void __launch_bounds__(512, 2) ntt_colpass_kernel(NttColP p) {
     // source-major in two halves: the 4 elements' loads of one source row are in flight together
 #pragma unroll
     for (int h = 0; h < 8; h += 4) {
-      u64 lo[4], hi[4];
+      u64 lo[4], hi[4], r[4];
       u32 j[4];
 #pragma unroll
-      for (int i = 0; i < 4; i++) lo[i] = hi[i] = 0, j[i] = G.gidx((tid + (h + i) * nth) & (T - 1));
+      for (int i = 0; i < 4; i++) lo[i] = hi[i] = r[i] = 0, j[i] = G.gidx((tid + (h + i) * nth) & (T - 1));
+      int lazy = 0;
       for (int s = 0; s < ns; s++) {
         const u64 c = __ldg(bc + s);
         u64 y[4];
@@ -159,11 +161,16 @@ __global__ void __launch_bounds__(512, 2) ntt_colpass_kernel(NttColP p) {
         for (int i = 0; i < 4; i++) y[i] = __ldg(src + (size_t)s * N + j[i]);
 #pragma unroll
         for (int i = 0; i < 4; i++) mac128(lo[i], hi[i], y[i], c);
+        if (++lazy == p.max_terms) {  // keep the 128-bit sum below t 2^64 (only many 60-bit sources get here)
+#pragma unroll
+          for (int i = 0; i < 4; i++) r[i] = addmod(r[i], mont_redc(lo[i], hi[i], mc.q, mc.qinv_neg), mc.q), lo[i] = hi[i] = 0;
+          lazy = 0;
+        }
       }
 #pragma unroll
       for (int i = 0; i < 4; i++) {
         const int e = tid + (h + i) * nth;
-        if (e < T) sm[swz(e)] = mont_redc(lo[i], hi[i], mc.q, mc.qinv_neg);
+        if (e < T) sm[swz(e)] = addmod(r[i], mont_redc(lo[i], hi[i], mc.q, mc.qinv_neg), mc.q);
       }
     }
   } else {
@@ -202,27 +209,27 @@ int k_ntt(const KCtx &k, const u64 *src, size_t src_bstride, u64 *dst, size_t ds
   if (n_rows == 0 || n_batch == 0) return 0;
   cudaStream_t st = (cudaStream_t)k.stream;
   const NttGeom &g = k.geom;
-  NttColP a{src, src_bstride, nullptr, dst, dst_bstride, rows, k.d_mods, k.d_tw_fwd, g};
+  NttColP a{src, src_bstride, nullptr, dst, dst_bstride, rows, k.d_mods, k.d_tw_fwd, g, 1 << 30};
   dim3 grid1(k.N >> g.lt_col, n_rows, n_batch);
-  PROF(k, K_NTT_COL, 16.0 * k.N * n_rows * n_batch);
+  PROF(k, K_NTT_COL, 16.0 * k.N * n_rows * n_batch, HALF_N(k) * g.bcol * n_rows * n_batch);
   COL_GEO(g, (ntt_colpass_kernel<false, GEO><<<grid1, nthreads_for(g.lt_col), sizeof(u64) << g.lt_col, st>>>(a)));
   LAUNCH_CHECK(k);
   NttRowP r{dst, dst_bstride, dst, dst_bstride, rows, k.d_mods, k.d_tw_fwd, g, 1};
   dim3 grid2(k.N >> g.lt_row, n_rows, n_batch);
-  PROF(k, K_NTT_ROW, 16.0 * k.N * n_rows * n_batch);
+  PROF(k, K_NTT_ROW, 16.0 * k.N * n_rows * n_batch, HALF_N(k) * g.brow * n_rows * n_batch);
   ROW_GEO(g, (ntt_rowpass_kernel<GEO><<<grid2, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(r)));
   LAUNCH_CHECK(k);
   return 0;
 }
 
 int k_ntt_cols_bconv(const KCtx &k, const u64 *y, size_t y_bstride, const u64 *bc, u64 *tmp, size_t tmp_bstride,
-                     const RowDesc *rows, int n_rows, int n_batch, int n_src_rows) {
+                     const RowDesc *rows, int n_rows, int n_batch, int n_src_rows, int max_terms) {
   if (n_rows == 0 || n_batch == 0) return 0;
   const NttGeom &g = k.geom;
-  NttColP a{y, y_bstride, bc, tmp, tmp_bstride, rows, k.d_mods, k.d_tw_fwd, g};
+  NttColP a{y, y_bstride, bc, tmp, tmp_bstride, rows, k.d_mods, k.d_tw_fwd, g, max_terms};
   dim3 grid1(k.N >> g.lt_col, n_rows, n_batch);
   // algorithmic bytes: every source row read once, every target row written once
-  PROF(k, K_NTT_COL_BCONV, 8.0 * k.N * ((double)n_src_rows + n_rows) * n_batch);
+  PROF(k, K_NTT_COL_BCONV, 8.0 * k.N * ((double)n_src_rows + n_rows) * n_batch, HALF_N(k) * g.bcol * n_rows * n_batch);
   COL_GEO(g, (ntt_colpass_kernel<true, GEO><<<grid1, nthreads_for(g.lt_col), sizeof(u64) << g.lt_col, (cudaStream_t)k.stream>>>(a)));
   LAUNCH_CHECK(k);
   return 0;
@@ -311,7 +318,8 @@ int k_ntt_rows_keymac(const KCtx &k, const BatchItem *items, int L, int E, int b
   dim3 grid((k.N >> g.lt_row) * n_batch, E, 1);
   const int ept = ((1 << g.lt_row) + nth - 1) / nth;
   // algorithmic bytes: ModUp temp + the switched polynomial read once, accumulators written once, each key once
-  PROF(k, K_KEYMAC, 8.0 * k.N * (((double)n_up + L + 2.0 * E) * n_batch + 2.0 * beta * E * n_distinct_keys));
+  PROF(k, K_KEYMAC, 8.0 * k.N * (((double)n_up + L + 2.0 * E) * n_batch + 2.0 * beta * E * n_distinct_keys),
+       HALF_N(k) * g.brow * n_up * n_batch);
   if (g.logN >= 12) ntt_rows_keymac_kernel<8, 1><<<grid, nth, sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
   else if (ept <= 1) ntt_rows_keymac_kernel<1, 0><<<grid, nth, sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
   else if (ept <= 4) ntt_rows_keymac_kernel<4, 0><<<grid, nth, sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
@@ -373,7 +381,7 @@ int k_ntt_rows_divide(const KCtx &k, const BatchItem *items, const u64 *tmp, siz
   const NttGeom &g = k.geom;
   DivideP p{items, tmp, tmp_bstride, acc, acc_bstride, mul, rows, k.d_mods, k.d_tw_fwd, g, minuend_from_items ? 1 : 0};
   dim3 grid(k.N >> g.lt_row, n_rows, n_batch);
-  PROF(k, K_DIVIDE, 8.0 * k.N * (3.5 * n_rows) * n_batch);  // temp + minuend + output, addend on half the rows
+  PROF(k, K_DIVIDE, 8.0 * k.N * (3.5 * n_rows) * n_batch, HALF_N(k) * g.brow * n_rows * n_batch);  // temp + minuend + output, addend on half the rows
   ROW_GEO(g, (ntt_rows_divide_kernel<GEO><<<grid, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p)));
   LAUNCH_CHECK(k);
   return 0;

@@ -5,21 +5,22 @@
 #include <vector>
 
 #include "fenc_ctx.h"
+#include "fenc_device.cuh"
 
 struct ProfRec { int id; cudaEvent_t a, b; };
 struct Prof {
   std::vector<ProfRec> recs;
   std::vector<cudaEvent_t> pool;
-  double ms[K_COUNT] = {0}, bytes[K_COUNT] = {0};
+  double ms[K_COUNT] = {0}, bytes[K_COUNT] = {0}, ops[K_COUNT] = {0};
   u64 count[K_COUNT] = {0};
   cudaEvent_t get() {
     if (!pool.empty()) { cudaEvent_t e = pool.back(); pool.pop_back(); return e; }
     cudaEvent_t e; cudaEventCreate(&e); return e;
   }
 };
-void prof_begin(Prof *p, void *stream, int id, double alg_bytes) {
+void prof_begin(Prof *p, void *stream, int id, double alg_bytes, double alg_butterflies) {
   ProfRec r{id, p->get(), p->get()};
-  p->bytes[id] += alg_bytes, p->count[id]++;
+  p->bytes[id] += alg_bytes, p->ops[id] += alg_butterflies, p->count[id]++;
   cudaEventRecord(r.a, (cudaStream_t)stream);
   p->recs.push_back(r);
 }
@@ -42,7 +43,8 @@ extern "C" fenc_status fenc_profile_enable(fenc_ctx *ctx, int on) {
 }
 extern "C" int fenc_profile_kernels(void) { return K_COUNT; }
 extern "C" const char *fenc_profile_name(int id) { return id >= 0 && id < K_COUNT ? kNames[id] : ""; }
-extern "C" fenc_status fenc_profile_read(fenc_ctx *ctx, double *ms, uint64_t *launches, double *alg_bytes, int reset) {
+extern "C" fenc_status fenc_profile_read(fenc_ctx *ctx, double *ms, uint64_t *launches, double *alg_bytes, double *alg_butterflies,
+                                         int reset) {
   if (!ctx || !ctx->k.prof) return FENC_ERR_INVALID_ARG;
   Prof *p = ctx->k.prof;
   CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
@@ -57,7 +59,83 @@ extern "C" fenc_status fenc_profile_read(fenc_ctx *ctx, double *ms, uint64_t *la
     if (ms) ms[i] = p->ms[i];
     if (launches) launches[i] = p->count[i];
     if (alg_bytes) alg_bytes[i] = p->bytes[i];
-    if (reset) p->ms[i] = p->bytes[i] = 0, p->count[i] = 0;
+    if (alg_butterflies) alg_butterflies[i] = p->ops[i];
+    if (reset) p->ms[i] = p->bytes[i] = p->ops[i] = 0, p->count[i] = 0;
   }
+  return FENC_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ integer-pipe peaks
+// Measured denominators for the "alu" roofline: (1) dependency-free 32-bit IMAD chains, all SMs;
+// (2) the forward lazy Shoup butterfly of fenc_device.cuh on registers only (no memory traffic): the ceiling of any NTT
+// kernel built from this butterfly.
+__global__ void __launch_bounds__(256) imad_peak_kernel(u32 *out, int iters) {
+  u32 x[8];
+#pragma unroll
+  for (int k = 0; k < 8; k++) x[k] = threadIdx.x + k;
+  const u32 a = 2654435761u + blockIdx.x, b = 40503u;
+  for (int it = 0; it < iters; it++) {
+#pragma unroll
+    for (int k = 0; k < 8; k++) x[k] = x[k] * a + b;
+  }
+  u32 s = 0;
+#pragma unroll
+  for (int k = 0; k < 8; k++) s ^= x[k];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+__global__ void __launch_bounds__(256) butterfly_peak_kernel(u64 *out, u64 q, u64 w, u64 ws, int iters) {
+  u64 x[8];
+#pragma unroll
+  for (int k = 0; k < 8; k++) x[k] = (threadIdx.x * 8 + k + blockIdx.x) % q;
+  const u64 q2 = q + q;
+  for (int it = 0; it < iters; it++) {
+#pragma unroll
+    for (int s = 2; s >= 0; s--) {
+#pragma unroll
+      for (int k = 0; k < 8; k++) {
+        if (k & (1 << s)) continue;
+        const int k2 = k | (1 << s);
+        const u64 T = shoup_lazy(x[k2], w, ws, q);
+        const u64 X = x[k];
+        x[k] = X + T;
+        x[k2] = X - T + q2;
+      }
+    }
+#pragma unroll
+    for (int k = 0; k < 8; k++) x[k] = csub(x[k] & ((1ull << 58) - 1), q2);  // keep the lazy values bounded between rounds
+  }
+  u64 s = 0;
+#pragma unroll
+  for (int k = 0; k < 8; k++) s ^= x[k];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+extern "C" fenc_status fenc_measure_alu_peak(fenc_ctx *ctx, double *imad_lane_ops_per_s, double *butterflies_per_s) {
+  if (!ctx || !imad_lane_ops_per_s || !butterflies_per_s) return FENC_ERR_INVALID_ARG;
+  const int blocks = 148 * 8, iters = 4096;
+  u64 *buf = dalloc_t<u64>(ctx, (size_t)blocks * 256);
+  if (!buf) return fail(ctx, FENC_ERR_OOM, "peak buffer");
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0), cudaEventCreate(&e1);
+  float ms = 0;
+  const u64 q = ctx->mod[0], w = ctx->psi[0], ws = fh::shoup(w, q);
+  for (int rep = 0; rep < 2; rep++) {  // first repetition warms up
+    cudaEventRecord(e0, ctx->stream);
+    imad_peak_kernel<<<blocks, 256, 0, ctx->stream>>>((u32 *)buf, iters);
+    cudaEventRecord(e1, ctx->stream);
+    CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+    cudaEventElapsedTime(&ms, e0, e1);
+  }
+  *imad_lane_ops_per_s = (double)blocks * 256 * 8.0 * iters / (ms * 1e-3);
+  for (int rep = 0; rep < 2; rep++) {
+    cudaEventRecord(e0, ctx->stream);
+    butterfly_peak_kernel<<<blocks, 256, 0, ctx->stream>>>(buf, q, w, ws, iters / 8);
+    cudaEventRecord(e1, ctx->stream);
+    CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+    cudaEventElapsedTime(&ms, e0, e1);
+  }
+  *butterflies_per_s = (double)blocks * 256 * 12.0 * (iters / 8) / (ms * 1e-3);
+  cudaEventDestroy(e0), cudaEventDestroy(e1);
+  dfree(ctx, buf);
+  ctx->launches += 4;
   return FENC_OK;
 }
