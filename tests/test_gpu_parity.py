@@ -399,3 +399,65 @@ def test_lenet_conv1_full_size_sampled(mods):
         got = g_out[(go * 4 + uo) * 4 + vo]
         assert np.array_equal(ctx.ct_export(got), ref.c), (uo, vo, go)
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------------------ full-size properties (configs 3, 4)
+def decoded_conv_error(mods, pkey, conv_kw, S, seed, kaiming=False, w_std=0.1):
+    """Encrypted conv at a BASELINE parameter set through the library's own encoder; returns max |decoded - fp64 conv|.
+    (The oracle needs minutes per output ciphertext at N=2^16, so full-size configs 3/4 are checked by this property,
+    which holds at any size; their limbs are covered bit-exactly by the same graphs at reduced N above.)"""
+    ck, fr, fenc = mods
+    ctx = fenc.Context(**wl.PARAMS[pkey])
+    x, w = wl.conv_inputs(seed, conv_kw, kaiming=kaiming, w_std=w_std)
+    conv = ctx.conv_desc(S=S, **conv_kw)
+    lay = ctx.layout_plan(conv)
+    L = ctx.n_q
+    keys = ctx.keygen(seed, lay.steps())
+    W = ctx.conv_weights(conv, lay, w, L)
+    cts = []
+    for bg in range(lay.BG):
+        for g in range(lay.G_in):
+            for u in range(lay.S):
+                for v in range(lay.S):
+                    cts.append(ctx.encrypt(keys, ctx.encode_fragment(conv, lay, x, u, v, g, bg, L), 9000 + len(cts)))
+    outs = ctx.hconv(keys, conv, lay, W, cts)
+    od = fr.ConvDesc(**conv_kw)
+    Y = np.zeros((od.BS, od.C_out, od.H_out, od.W_out))
+    i = 0
+    for bg in range(lay.BG):
+        for go in range(lay.G_out):
+            for uo in range(lay.S_out):
+                for vo in range(lay.S_out):
+                    assert outs[i].L == L - 1
+                    ctx.decrypt_decode(keys, outs[i], conv, lay, 1, uo, vo, go, bg, Y)
+                    i += 1
+    err = np.abs(Y - fr.direct_conv(od, x, w)).max()
+    ctx.close()
+    return err, lay
+
+
+def test_config3_resnet_layers_full_size_decoded(mods):
+    """BASELINE config 3 (N=2^16, 24x50b + 4x60b, dlen 4, scale 2^50): the three ResNet-20-shaped layers, BS=1."""
+    err, lay = decoded_conv_error(mods, "cfg3", wl.CONVS["resnet_16_16"], 0, 301, kaiming=True)
+    assert (lay.S, lay.n_in_ct, lay.n_out_ct, lay.n_inner_rot, lay.n_outer_rot, lay.n_pmult) == (1, 1, 1, 8, 30, 279)
+    assert err < 1e-3
+    err, lay = decoded_conv_error(mods, "cfg3", wl.CONVS["resnet_16_32_s2"], 2, 302, kaiming=True)
+    assert (lay.n_in_ct, lay.n_out_ct, lay.n_inner_rot, lay.n_outer_rot, lay.n_pmult) == (4, 1, 5, 46, 423)
+    assert err < 1e-3
+    err, lay = decoded_conv_error(mods, "cfg3", wl.CONVS["resnet_32_64_s2"], 2, 303, kaiming=True)
+    assert (lay.n_in_ct, lay.n_out_ct, lay.n_inner_rot, lay.n_outer_rot, lay.n_pmult) == (4, 1, 5, 94, 855)
+    assert err < 1e-3
+
+
+def test_config4_mobilenet_layers_full_size_decoded(mods):
+    """BASELINE config 4 (N=2^16, 30x50b + 5x60b, dlen 5): depthwise 3x3 and pointwise 1x1 at 112x112 (M=128, S=4)
+    and the strided depthwise at 112 -> 56, batch 2 (the same kernels and graphs as the max-batch run, fewer groups)."""
+    dw = dict(BS=2, C_in=32, H=112, W=112, C_out=32, K=3, stride=1, pad=1, depthwise=True)
+    err, lay = decoded_conv_error(mods, "cfg4", dw, 4, 401, w_std=0.05)
+    assert lay.M == 128 and lay.m == 32 and err < 1e-3
+    pw = dict(BS=2, C_in=32, H=112, W=112, C_out=64, K=1, stride=1, pad=0)
+    err, lay = decoded_conv_error(mods, "cfg4", pw, 4, 402, w_std=0.05)
+    assert lay.n_inner_rot == 0 and err < 1e-3
+    dws = dict(BS=2, C_in=64, H=112, W=112, C_out=64, K=3, stride=2, pad=1, depthwise=True)
+    err, lay = decoded_conv_error(mods, "cfg4", dws, 4, 403, w_std=0.05)
+    assert lay.S_out == 2 and lay.H_out == 56 and err < 1e-3
