@@ -163,7 +163,7 @@ extern "C" fenc_status fenc_params_init(const fenc_params_desc *d, fenc_ctx **ou
   if (ctx->logN <= 11) {
     g.brow = ctx->logN, g.bcol = 0, g.lt_row = ctx->logN, g.lt_col = ctx->logN, g.lc_col = ctx->logN;
   } else {
-    g.brow = 8, g.bcol = ctx->logN - 8, g.lt_row = 11, g.lc_col = 4, g.lt_col = g.bcol + 4;
+    g.brow = 8, g.bcol = ctx->logN - 8, g.lt_row = FENC_ROW_LT, g.lc_col = 4, g.lt_col = g.bcol + 4;
   }
   ctx->k = KCtx{(void *)ctx->stream, g, ctx->d_mods, ctx->d_tw_fwd, ctx->d_tw_inv, &ctx->launches, N, ctx->nq, ctx->np, nullptr};
   *out = c.release();

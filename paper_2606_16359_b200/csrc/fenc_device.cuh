@@ -194,7 +194,7 @@ DEVI void tile_transform(u64 *sm, const TileGeo &G, int lo, int nb, const ShoupC
       }
     }
   } else {
-    constexpr int LT = GEO == 1 ? 11 : GEO + 4, LO = GEO == 1 ? 0 : 4, NB = GEO == 1 ? 8 : GEO;
+    constexpr int LT = GEO == 1 ? FENC_ROW_LT : GEO + 4, LO = GEO == 1 ? 0 : 4, NB = GEO == 1 ? 8 : GEO;
     if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
     else tile_rounds_ct<FWD, false, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
   }

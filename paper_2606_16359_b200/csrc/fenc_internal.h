@@ -13,7 +13,10 @@ typedef uint32_t u32;
 typedef unsigned __int128 u128;
 typedef long long i64;
 
-#define FENC_MAX_MOD 96  // moduli per context (n_q + n_p)
+#define FENC_MAX_MOD 96
+#ifndef FENC_ROW_LT
+#define FENC_ROW_LT 10  // log2 elements of a row-pass tile for N >= 2^12 (8 stages on 2^FENC_ROW_LT contiguous coefficients)
+#endif  // moduli per context (n_q + n_p)
 
 // ---------------------------------------------------------------- device-visible tables
 struct ModConst {  // one per modulus, device global memory
