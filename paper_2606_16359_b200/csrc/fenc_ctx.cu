@@ -49,18 +49,37 @@ void *workspace(fenc_ctx *ctx, size_t bytes) {
   }
   return ctx->ws;
 }
+// Descriptor arrays go through a ring of pinned host slots: a copy from pageable memory would synchronise the stream
+// before every batch (and stall the host-side enqueue of the next kernels behind all queued GPU work).
+static const size_t DESC_SLOT = (size_t)1 << 20;
+static const int DESC_SLOTS = 8;
 char *DescStage::commit() {
   size_t need = (host.size() + 255) & ~(size_t)255;
   if (need > ctx->desc_bytes) {
     dfree(ctx, ctx->desc_buf);
-    size_t cap = need < (1u << 20) ? (1u << 20) : need * 2;
+    size_t cap = need < DESC_SLOT ? DESC_SLOT : need * 2;
     ctx->desc_buf = dalloc(ctx, cap);
     ctx->desc_bytes = ctx->desc_buf ? cap : 0;
     if (!ctx->desc_buf) return nullptr;
   }
-  if (!host.empty() &&
-      cudaMemcpyAsync(ctx->desc_buf, host.data(), host.size(), cudaMemcpyHostToDevice, ctx->stream) != cudaSuccess)
-    return nullptr;
+  if (host.empty()) return (char *)ctx->desc_buf;
+  if (host.size() <= DESC_SLOT) {
+    if (!ctx->desc_pinned) {
+      if (cudaHostAlloc(&ctx->desc_pinned, DESC_SLOT * DESC_SLOTS, cudaHostAllocDefault) != cudaSuccess) ctx->desc_pinned = nullptr;
+      for (int i = 0; i < DESC_SLOTS && ctx->desc_pinned; i++) cudaEventCreateWithFlags(&ctx->desc_ev[i], cudaEventDisableTiming);
+    }
+    if (ctx->desc_pinned) {
+      const int slot = ctx->desc_next++ % DESC_SLOTS;
+      if (ctx->desc_used[slot]) cudaEventSynchronize(ctx->desc_ev[slot]);  // the copy that last read this slot is done
+      char *h = (char *)ctx->desc_pinned + (size_t)slot * DESC_SLOT;
+      memcpy(h, host.data(), host.size());
+      if (cudaMemcpyAsync(ctx->desc_buf, h, host.size(), cudaMemcpyHostToDevice, ctx->stream) != cudaSuccess) return nullptr;
+      cudaEventRecord(ctx->desc_ev[slot], ctx->stream);
+      ctx->desc_used[slot] = true;
+      return (char *)ctx->desc_buf;
+    }
+  }
+  if (cudaMemcpyAsync(ctx->desc_buf, host.data(), host.size(), cudaMemcpyHostToDevice, ctx->stream) != cudaSuccess) return nullptr;
   return (char *)ctx->desc_buf;
 }
 fenc_ct *new_ct(fenc_ctx *ctx, int L, double scale) {
@@ -176,6 +195,10 @@ extern "C" void fenc_ctx_free(fenc_ctx *ctx) {
   for (auto &kv : ctx->plans)
     for (void *p : kv.second->owned) dfree(ctx, p);
   dfree(ctx, ctx->ws), dfree(ctx, ctx->desc_buf);
+  if (ctx->desc_pinned) {
+    for (int i = 0; i < 8; i++) cudaEventDestroy(ctx->desc_ev[i]);
+    cudaFreeHost(ctx->desc_pinned);
+  }
   dfree(ctx, ctx->d_mods), dfree(ctx, ctx->d_tw_fwd), dfree(ctx, ctx->d_tw_inv);
   dfree(ctx, ctx->d_ident_rows), dfree(ctx, ctx->d_ninv), dfree(ctx, ctx->d_ident_mod);
   delete ctx;

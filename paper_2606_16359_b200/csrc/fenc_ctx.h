@@ -65,6 +65,10 @@ struct fenc_ctx {
   size_t ws_bytes = 0;
   void *desc_buf = nullptr;         // device staging for per-call descriptor arrays
   size_t desc_bytes = 0;
+  void *desc_pinned = nullptr;      // ring of pinned host slots feeding desc_buf
+  cudaEvent_t desc_ev[8] = {};
+  bool desc_used[8] = {};
+  unsigned desc_next = 0;
   std::map<std::string, std::shared_ptr<LinGraph>> graphs;
 };
 
