@@ -67,7 +67,7 @@ struct InttRowP {
   const RowDesc *rows; const ModConst *mods; const ShoupC *tw; NttGeom g;
 };
 template <bool GATHER, int GEO>
-__global__ void __launch_bounds__(256, 4) intt_rowpass_kernel(InttRowP p) {
+__global__ void __launch_bounds__(256, 5) intt_rowpass_kernel(InttRowP p) {
   extern __shared__ u64 sm[];
   const int tid = threadIdx.x, b = blockIdx.z;
   const RowDesc rd = p.rows[blockIdx.y];
@@ -92,7 +92,7 @@ struct InttColP {
   u64 *dst; size_t dst_bstride; const RowDesc *rows; const ShoupC *scale; const ModConst *mods; const ShoupC *tw; NttGeom g;
 };
 template <int GEO>
-__global__ void __launch_bounds__(512) intt_colpass_kernel(InttColP p) {
+__global__ void __launch_bounds__(512, 3) intt_colpass_kernel(InttColP p) {
   extern __shared__ u64 sm[];
   const int tid = threadIdx.x, b = blockIdx.z;
   const RowDesc rd = p.rows[blockIdx.y];
@@ -335,7 +335,7 @@ struct DivideP {
   const RowDesc *rows; const ModConst *mods; const ShoupC *tw; NttGeom g; int from_items;
 };
 template <int GEO>
-__global__ void __launch_bounds__(256, 3) ntt_rows_divide_kernel(DivideP p) {
+__global__ void __launch_bounds__(256, 5) ntt_rows_divide_kernel(DivideP p) {
   extern __shared__ u64 sm[];
   const int tid = threadIdx.x, b = blockIdx.z;
   const RowDesc rd = p.rows[blockIdx.y];
