@@ -157,6 +157,13 @@ fenc_status fenc_add(fenc_ctx *ctx, const fenc_ct *a, const fenc_ct *b, fenc_ct 
 fenc_status fenc_pmult_sum(fenc_ctx *ctx, fenc_ct *const *in, fenc_pt *const *pt, size_t n, fenc_ct **out);
 /* out[i] = in[i]^2 relinearised and rescaled (a13; R2.12), all n in ONE batched key switch; inputs share the level */
 fenc_status fenc_square_relin(fenc_ctx *ctx, const fenc_keys *keys, fenc_ct *const *in, size_t n, fenc_ct **out);
+/* out[i] = a[i] * b[i] relinearised and rescaled (CMult; R2.12); square_relin is the case b = a */
+fenc_status fenc_cmult_relin(fenc_ctx *ctx, const fenc_keys *keys, fenc_ct *const *a, fenc_ct *const *b, size_t n, fenc_ct **out);
+/* PMultConst (R2.8): out[i] = in[i] * k for the integer k given by its residues, host k_res[L] with k_res[t] = k mod q_t
+ * (the caller rounds c*E exactly, R2.8); the scale is multiplied by scale_factor (= E).  No level is consumed. */
+fenc_status fenc_mul_scalar(fenc_ctx *ctx, fenc_ct *const *in, size_t n, const uint64_t *k_res, double scale_factor, fenc_ct **out);
+/* out[i] = in[i] + k: the integer k (residues k_res[L]) added to coefficient 0 of c0, i.e. round(scale*c) for a real constant c */
+fenc_status fenc_add_const(fenc_ctx *ctx, fenc_ct *const *in, size_t n, const uint64_t *k_res, fenc_ct **out);
 /* out[g] = sum_{i < group} in[g*group + i] for g < n_groups: avg-pool by fragment selection (a14; PAPER.md:284;
  * the 1/group^2 factor belongs to the next layer's weights, R2.12).  No rotations, no level consumed. */
 fenc_status fenc_sum_groups(fenc_ctx *ctx, fenc_ct *const *in, size_t group, size_t n_groups, fenc_ct **out);

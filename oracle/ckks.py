@@ -467,3 +467,62 @@ def square_relin(params: Params, keys: Keys, ct: Ciphertext) -> Ciphertext:
         out[0, t] = (d0[t] + k0[t]) % q
         out[1, t] = ((d1[t] + d1[t]) % q + k1[t]) % q
     return rescale(params, Ciphertext(out, L, ct.scale * ct.scale))
+
+
+# --------------------------------------------------------------------------- CMult, PMultConst, degree-3 activation (R2.8, R2.12)
+def cmult_relin(params: Params, keys: Keys, x: Ciphertext, y: Ciphertext) -> Ciphertext:
+    """(d0, d1, d2) = (x0 y0, x0 y1 + x1 y0, x1 y1); (d0, d1) + KS(d2; relin); then rescale (PAPER.md:63 CMult; R2.12)."""
+    assert x.L == y.L
+    L, N = x.L, params.N
+    d0, d1, d1b, d2 = (np.zeros((L, N), dtype=np.uint64) for _ in range(4))
+    _lib.orc_polymul_rns(params._h, L, _p(x.c[0]), _p(y.c[0]), _p(d0))
+    _lib.orc_polymul_rns(params._h, L, _p(x.c[0]), _p(y.c[1]), _p(d1))
+    _lib.orc_polymul_rns(params._h, L, _p(x.c[1]), _p(y.c[0]), _p(d1b))
+    _lib.orc_polymul_rns(params._h, L, _p(x.c[1]), _p(y.c[1]), _p(d2))
+    k0, k1 = keyswitch(params, L, d2, keys.evk[RELIN_KEY_ID])
+    out = np.zeros_like(x.c)
+    for t in range(L):
+        q = np.uint64(params.mod[t])
+        out[0, t] = (d0[t] + k0[t]) % q
+        out[1, t] = ((d1[t] + d1b[t]) % q + k1[t]) % q
+    return rescale(params, Ciphertext(out, L, x.scale * y.scale))
+
+
+def round_half_up(x) -> int:
+    return math.floor(Fraction(x) + Fraction(1, 2))
+
+
+def mul_const(params: Params, ct: Ciphertext, c, E) -> Ciphertext:
+    """PMultConst(ct, c, E): every limb times round_half_up(c E) with c, E exact rationals; scale multiplies by E (R2.8)."""
+    k = round_half_up(Fraction(c) * Fraction(E))
+    kt = np.array([k % q for q in params.q[:ct.L]], dtype=np.uint64)
+    out = np.zeros_like(ct.c)
+    for j in range(2):
+        _lib.orc_mul_scalar(params._h, ct.L, _p(ct.c[j]), _p(kt), _p(out[j]))
+    return Ciphertext(out, ct.L, ct.scale * Fraction(E))
+
+
+def add_const(params: Params, ct: Ciphertext, k: int) -> Ciphertext:
+    """the integer k added to coefficient 0 of c0 (the encoding of the real constant k / scale in every slot, R2.2)."""
+    out = ct.c.copy()
+    for t in range(ct.L):
+        q = params.q[t]
+        out[0, t, 0] = np.uint64((int(out[0, t, 0]) + k) % q)
+    return Ciphertext(out, ct.L, ct.scale)
+
+
+POLY3 = (Fraction(1, 2), Fraction(197, 1000), Fraction(-4, 1000))  # BASELINE config 3: x -> 0.5 + 0.197 x - 0.004 x^3
+
+
+def poly3(params: Params, keys: Keys, x: Ciphertext, coef=POLY3) -> Ciphertext:
+    """Degree-3 activation a0 + a1 x + a3 x^3 in two levels (R2.12): x2 = Rescale(Relin(x x));
+    t = Rescale(PMultConst(x, a3, q_{L-1})); x3 = Rescale(Relin(x2 t)) at scale s3 = s^3/(q_{L-1} q_{L-2});
+    u = Rescale(Rescale(PMultConst(x, a1, s^2))) (same scale); out = x3 + u + round_half_up(a0 s3) on coefficient 0."""
+    a0, a1, a3 = coef
+    L, s = x.L, x.scale
+    x2 = cmult_relin(params, keys, x, x)
+    t = rescale(params, mul_const(params, x, a3, params.q[L - 1]))
+    x3 = cmult_relin(params, keys, x2, t)
+    u = rescale(params, rescale(params, mul_const(params, x, a1, s * s)))
+    assert x3.scale == u.scale == s ** 3 / (params.q[L - 1] * params.q[L - 2])
+    return add_const(params, add(params, x3, u), round_half_up(Fraction(a0) * x3.scale))

@@ -201,6 +201,8 @@ def run_network(ck, params, keys, layers, cts, L0):
             cts, S, L = out, 1, L - 1
         elif ly["op"] == "square":
             cts, L = [ck.square_relin(params, keys, c) for c in cts], L - 1
+        elif ly["op"] == "poly3":
+            cts, L = [ck.poly3(params, keys, c, ly.get("coef", ck.POLY3)) for c in cts], L - 2
         elif ly["op"] == "pool":
             cts, S = sum_pool(ck, params, cts, S), S // 2
         else:
@@ -217,6 +219,6 @@ def network_rot_steps(layers, n):
             steps.update(fr.ConvGraph(fr.ConvDesc(S=ly["S"], **ly["conv"]), n).counts()["rot_steps"])
         elif ly["op"] == "fc":
             steps.update(FcGraph(n, **ly["fc"]).counts()["rot_steps"])
-        elif ly["op"] == "square":
+        elif ly["op"] in ("square", "poly3"):
             relin = True
     return sorted(steps), relin

@@ -63,7 +63,8 @@ SYMBOLS = ["fenc_params_init", "fenc_ctx_free", "fenc_last_error", "fenc_get_pri
            "fenc_wts_keys", "fenc_conv_weights", "fenc_conv_weights_from_coeffs", "fenc_wts_free", "fenc_hconv",
            "fenc_compress", "fenc_ntt_rows", "fenc_launch_count", "fenc_device_bytes", "fenc_sum_groups",
            "fenc_profile_enable", "fenc_profile_kernels", "fenc_profile_name", "fenc_profile_read", "fenc_fc_plan",
-           "fenc_fc_wts_keys", "fenc_fc_weights", "fenc_fc_weights_from_coeffs", "fenc_fc", "fenc_measure_alu_peak"]
+           "fenc_fc_wts_keys", "fenc_fc_weights", "fenc_fc_weights_from_coeffs", "fenc_fc", "fenc_measure_alu_peak",
+           "fenc_cmult_relin", "fenc_mul_scalar", "fenc_add_const"]
 
 _lib = None
 
@@ -103,6 +104,9 @@ def load_library(path=None):
         "fenc_pmult_sum": [vp, vpp, vpp, C.c_size_t, vpp],
         "fenc_square_relin": [vp, vp, vpp, C.c_size_t, vpp],
         "fenc_sum_groups": [vp, vpp, C.c_size_t, C.c_size_t, vpp],
+        "fenc_cmult_relin": [vp, vp, vpp, vpp, C.c_size_t, vpp],
+        "fenc_mul_scalar": [vp, vpp, C.c_size_t, u64p, C.c_double, vpp],
+        "fenc_add_const": [vp, vpp, C.c_size_t, u64p, vpp],
         "fenc_profile_enable": [vp, C.c_int],
         "fenc_measure_alu_peak": [vp, dp, dp],
         "fenc_profile_read": [vp, dp, u64p, dp, dp, C.c_int],
@@ -388,6 +392,28 @@ class Context:
         self._ck(self.lib.fenc_square_relin(self.h, keys.h, self._harr(lst), len(lst), out))
         res = [Ciphertext(self, C.c_void_p(out[i])) for i in range(len(lst))]
         return res[0] if single else res
+
+    def cmult_relin(self, keys, a, b):
+        out = (C.c_void_p * len(a))()
+        self._ck(self.lib.fenc_cmult_relin(self.h, keys.h, self._harr(a), self._harr(b), len(a), out))
+        return [Ciphertext(self, C.c_void_p(out[i])) for i in range(len(a))]
+
+    def _residues(self, k, L):
+        return np.asarray([int(k) % self.q[t] for t in range(L)], dtype=np.uint64)
+
+    def mul_scalar(self, cts, k, scale_factor):
+        """every limb times the (Python) integer k; the scale is multiplied by scale_factor."""
+        r = self._residues(k, cts[0].L)
+        out = (C.c_void_p * len(cts))()
+        self._ck(self.lib.fenc_mul_scalar(self.h, self._harr(cts), len(cts), _ptr(r, C.c_uint64), float(scale_factor), out))
+        return [Ciphertext(self, C.c_void_p(out[i])) for i in range(len(cts))]
+
+    def add_const(self, cts, k):
+        """the (Python) integer k added to coefficient 0 of c0."""
+        r = self._residues(k, cts[0].L)
+        out = (C.c_void_p * len(cts))()
+        self._ck(self.lib.fenc_add_const(self.h, self._harr(cts), len(cts), _ptr(r, C.c_uint64), out))
+        return [Ciphertext(self, C.c_void_p(out[i])) for i in range(len(cts))]
 
     def sum_groups(self, cts, group):
         n = len(cts) // group

@@ -240,26 +240,53 @@ int k_reduce_signed(const KCtx &k, const i64 *coeffs, const int *row_mod, u64 *d
   return launch_row<OP_REDUCE_SIGNED>(k, p, n_rows);
 }
 
-// (d0, d1, d2) = (c0 c0, 2 c0 c1, c1 c1) per limb (a13, R2.12)
-__global__ void __launch_bounds__(256) tensor_square_kernel(const u64 *const *in, u64 *d, const ModConst *mods, int L, int logN) {
+// tensor product per limb (a13, R2.12): (d0, d1, d2) = (a0 b0, a0 b1 + a1 b0, a1 b1); d: [n][3][L][N]
+__global__ void __launch_bounds__(256) tensor_product_kernel(const u64 *const *ina, const u64 *const *inb, u64 *d, const ModConst *mods,
+                                                             int L, int logN) {
   const size_t LN = (size_t)L << logN;
   const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= LN) return;
   const ModConst mc = mods[i >> logN];
-  const u64 *c = in[blockIdx.y];
-  const u64 c0 = c[i], c1 = c[LN + i];
-  const u64 c0m = mont_mul(c0, mc.r2, mc.q, mc.qinv_neg), c1m = mont_mul(c1, mc.r2, mc.q, mc.qinv_neg);
+  const u64 *a = ina[blockIdx.y], *b = inb[blockIdx.y];
+  const u64 a0 = a[i], a1 = a[LN + i], b0 = b[i], b1 = b[LN + i];
+  const u64 b0m = mont_mul(b0, mc.r2, mc.q, mc.qinv_neg), b1m = mont_mul(b1, mc.r2, mc.q, mc.qinv_neg);
   u64 *o = d + (size_t)blockIdx.y * 3 * LN;
-  const u64 x = mont_mul(c1, c0m, mc.q, mc.qinv_neg);
-  o[i] = mont_mul(c0, c0m, mc.q, mc.qinv_neg);
-  o[LN + i] = addmod(x, x, mc.q);
-  o[2 * LN + i] = mont_mul(c1, c1m, mc.q, mc.qinv_neg);
+  o[i] = mont_mul(a0, b0m, mc.q, mc.qinv_neg);
+  o[LN + i] = addmod(mont_mul(a0, b1m, mc.q, mc.qinv_neg), mont_mul(a1, b0m, mc.q, mc.qinv_neg), mc.q);
+  o[2 * LN + i] = mont_mul(a1, b1m, mc.q, mc.qinv_neg);
 }
-int k_tensor_square(const KCtx &k, const u64 *const *in, u64 *d, int n, int L) {
+int k_tensor_product(const KCtx &k, const u64 *const *ina, const u64 *const *inb, u64 *d, int n, int L) {
   if (n == 0) return 0;
   dim3 grid((unsigned)(((size_t)L * k.N + 255) / 256), n);
-  PROF(k, K_ROWOP, 40.0 * L * k.N * n);
-  tensor_square_kernel<<<grid, 256, 0, S(k)>>>(in, d, k.d_mods, L, k.geom.logN);
+  PROF(k, K_ROWOP, 56.0 * L * k.N * n);
+  tensor_product_kernel<<<grid, 256, 0, S(k)>>>(ina, inb, d, k.d_mods, L, k.geom.logN);
+  LAUNCH_CHECK(k);
+  return 0;
+}
+// out[b] = in[b] * k (both polynomials), k given per limb in Montgomery form; add_const: c0 += k (the constant polynomial
+// k is k at every evaluation point), k given per limb as a canonical residue
+__global__ void __launch_bounds__(256) scalar_kernel(const u64 *const *in, u64 *const *out, const u64 *kl, const ModConst *mods, int L,
+                                                     int logN, int add_const) {
+  const size_t LN = (size_t)L << logN;
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= LN) return;
+  const int t = (int)(i >> logN);
+  const ModConst mc = mods[t];
+  const u64 *a = in[blockIdx.y];
+  u64 *o = out[blockIdx.y];
+  if (add_const) {
+    o[i] = addmod(a[i], kl[t], mc.q);
+    o[LN + i] = a[LN + i];
+  } else {
+    o[i] = mont_mul(a[i], kl[t], mc.q, mc.qinv_neg);
+    o[LN + i] = mont_mul(a[LN + i], kl[t], mc.q, mc.qinv_neg);
+  }
+}
+int k_scalar(const KCtx &k, const u64 *const *in, u64 *const *out, const u64 *kl, int n, int L, bool add_const) {
+  if (n == 0) return 0;
+  dim3 grid((unsigned)(((size_t)L * k.N + 255) / 256), n);
+  PROF(k, K_ROWOP, 32.0 * L * k.N * n);
+  scalar_kernel<<<grid, 256, 0, S(k)>>>(in, out, kl, k.d_mods, L, k.geom.logN, add_const ? 1 : 0);
   LAUNCH_CHECK(k);
   return 0;
 }

@@ -383,28 +383,28 @@ extern "C" fenc_status fenc_pmult_sum(fenc_ctx *ctx, fenc_ct *const *in, fenc_pt
   return FENC_OK;
 }
 
-// x -> x^2 (R2.12): d0 = c0 c0, d1 = 2 c0 c1, d2 = c1 c1; (d0, d1) + KS(d2; relin); rescale.  Batched over n.
-extern "C" fenc_status fenc_square_relin(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const *in, size_t n, fenc_ct **out) {
-  if (!ctx || !K || !in || !out) return FENC_ERR_INVALID_ARG;
+// CMult + relinearise + rescale (a13, R2.12): (d0, d1, d2) = (a0 b0, a0 b1 + a1 b0, a1 b1);
+// (d0, d1) + KS(d2; relin); rescale.  Batched over n pairs; x^2 is the case b = a.
+static fenc_status cmult_relin(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const *ina, fenc_ct *const *inb, size_t n, fenc_ct **out) {
   if (n == 0) return FENC_OK;
   auto it = K->evk.find(FENC_RELIN_KEY_ID);
   if (it == K->evk.end()) return fail(ctx, FENC_ERR_NO_KEY, "no relinearisation key");
-  const int L = in[0]->L;
-  if (L < 2) return fail(ctx, FENC_ERR_LEVEL, "square needs a level to rescale into");
+  const int L = ina[0]->L;
+  if (L < 2) return fail(ctx, FENC_ERR_LEVEL, "a product needs a level to rescale into");
   const size_t LN = (size_t)L * ctx->N;
-  std::vector<const u64 *> ptrs(n);
+  std::vector<const u64 *> pa(n), pb(n);
   for (size_t i = 0; i < n; i++) {
-    if (in[i]->L != L) return fail(ctx, FENC_ERR_MISMATCH, "square: inputs differ in level");
-    ptrs[i] = in[i]->d;
+    if (ina[i]->L != L || inb[i]->L != L) return fail(ctx, FENC_ERR_MISMATCH, "product: inputs differ in level");
+    pa[i] = ina[i]->d, pb[i] = inb[i]->d;
   }
   u64 *d = dalloc_t<u64>(ctx, n * 3 * LN), *mid = dalloc_t<u64>(ctx, n * 2 * LN);
-  if (!d || !mid) return fail(ctx, FENC_ERR_OOM, "square");
+  if (!d || !mid) return fail(ctx, FENC_ERR_OOM, "product");
   {
     DescStage st(ctx);
-    size_t o0 = st.add(ptrs);
+    size_t o0 = st.add(pa), o1 = st.add(pb);
     char *base = st.commit();
     if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
-    CUDA_OK(ctx, k_tensor_square(ctx->k, (const u64 *const *)(base + o0), d, (int)n, L));
+    CUDA_OK(ctx, k_tensor_product(ctx->k, (const u64 *const *)(base + o0), (const u64 *const *)(base + o1), d, (int)n, L));
   }
   std::vector<BatchItem> items(n), rs(n);
   std::vector<fenc_ct *> made(n, nullptr);
@@ -413,8 +413,8 @@ extern "C" fenc_status fenc_square_relin(fenc_ctx *ctx, const fenc_keys *K, fenc
     items[i] = BatchItem{};
     items[i].ks_in = di + 2 * LN, items[i].out = mid + i * 2 * LN, items[i].evk = it->second;
     items[i].add0 = di, items[i].add1 = di + LN, items[i].g = 1;
-    made[i] = new_ct(ctx, L - 1, in[i]->scale * in[i]->scale / (double)ctx->mod[L - 1]);
-    if (!made[i]) return fail(ctx, FENC_ERR_OOM, "square output");
+    made[i] = new_ct(ctx, L - 1, ina[i]->scale * inb[i]->scale / (double)ctx->mod[L - 1]);
+    if (!made[i]) return fail(ctx, FENC_ERR_OOM, "product output");
     rs[i] = BatchItem{};
     rs[i].sub_in = mid + i * 2 * LN, rs[i].out = made[i]->d;
   }
@@ -425,6 +425,51 @@ extern "C" fenc_status fenc_square_relin(fenc_ctx *ctx, const fenc_keys *K, fenc
   dfree(ctx, d), dfree(ctx, mid);
   for (size_t i = 0; i < n; i++) out[i] = made[i];
   return FENC_OK;
+}
+extern "C" fenc_status fenc_square_relin(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const *in, size_t n, fenc_ct **out) {
+  if (!ctx || !K || !in || !out) return FENC_ERR_INVALID_ARG;
+  return cmult_relin(ctx, K, in, in, n, out);
+}
+extern "C" fenc_status fenc_cmult_relin(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const *a, fenc_ct *const *b, size_t n, fenc_ct **out) {
+  if (!ctx || !K || !a || !b || !out) return FENC_ERR_INVALID_ARG;
+  return cmult_relin(ctx, K, a, b, n, out);
+}
+
+// PMultConst (R2.8): every limb times the integer k, given by its residues k mod q_t; the caller states the
+// factor the scale is multiplied by.  add_const: the integer k is added to coefficient 0 of c0 (scale unchanged).
+static fenc_status scalar_op(fenc_ctx *ctx, fenc_ct *const *in, size_t n, const uint64_t *k_res, double factor, bool add_const,
+                             fenc_ct **out) {
+  if (!ctx || !in || !k_res || !out) return FENC_ERR_INVALID_ARG;
+  if (n == 0) return FENC_OK;
+  const int L = in[0]->L;
+  std::vector<u64> kl(L);
+  for (int t = 0; t < L; t++) {
+    if (k_res[t] >= ctx->mod[t]) return fail(ctx, FENC_ERR_INVALID_ARG, "scalar residue %d is not reduced", t);
+    kl[t] = add_const ? k_res[t] : fh::to_mont(k_res[t], ctx->mod[t]);
+  }
+  std::vector<const u64 *> pin(n);
+  std::vector<u64 *> pout(n);
+  std::vector<fenc_ct *> made(n, nullptr);
+  for (size_t i = 0; i < n; i++) {
+    if (in[i]->L != L) return fail(ctx, FENC_ERR_MISMATCH, "scalar op: inputs differ in level");
+    made[i] = new_ct(ctx, L, add_const ? in[i]->scale : in[i]->scale * factor);
+    if (!made[i]) return fail(ctx, FENC_ERR_OOM, "scalar op output");
+    pin[i] = in[i]->d, pout[i] = made[i]->d;
+  }
+  DescStage st(ctx);
+  size_t o0 = st.add(pin), o1 = st.add(pout), o2 = st.add(kl);
+  char *base = st.commit();
+  if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
+  CUDA_OK(ctx, k_scalar(ctx->k, (const u64 *const *)(base + o0), (u64 *const *)(base + o1), (const u64 *)(base + o2), (int)n, L, add_const));
+  for (size_t i = 0; i < n; i++) out[i] = made[i];
+  return FENC_OK;
+}
+extern "C" fenc_status fenc_mul_scalar(fenc_ctx *ctx, fenc_ct *const *in, size_t n, const uint64_t *k_res, double scale_factor,
+                                       fenc_ct **out) {
+  return scalar_op(ctx, in, n, k_res, scale_factor, false, out);
+}
+extern "C" fenc_status fenc_add_const(fenc_ctx *ctx, fenc_ct *const *in, size_t n, const uint64_t *k_res, fenc_ct **out) {
+  return scalar_op(ctx, in, n, k_res, 1.0, true, out);
 }
 
 extern "C" fenc_status fenc_sum_groups(fenc_ctx *ctx, fenc_ct *const *in, size_t group, size_t n_groups, fenc_ct **out) {

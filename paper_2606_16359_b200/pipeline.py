@@ -1,7 +1,32 @@
 """Layer sequencing over the C ABI: a list of fragment-encoded layers (conv / square / pool / fc) evaluated by one
 batched library call per layer (R2.9, R2.12).  Orchestration only: every ciphertext
 operation runs inside libfenc's kernels; this file holds no arithmetic on ciphertext data."""
+import math
+from fractions import Fraction
+
 import numpy as np
+
+POLY3 = (Fraction(1, 2), Fraction(197, 1000), Fraction(-4, 1000))  # BASELINE config 3: 0.5 + 0.197 x - 0.004 x^3
+
+
+def _round_half_up(x):
+    return math.floor(Fraction(x) + Fraction(1, 2))
+
+
+def poly3_activation(ctx, keys, cts, scale, coef=POLY3):
+    """Degree-3 activation a0 + a1 x + a3 x^3 in two levels (R2.12), every step one batched library call.
+    `scale` is the exact rational scale of the inputs (the integer multipliers are rounded exactly on the host, R2.8).
+    Returns (ciphertexts at L-2, their exact scale)."""
+    a0, a1, a3 = (Fraction(c) for c in coef)
+    L, s = cts[0].L, Fraction(scale)
+    q1, q2 = ctx.q[L - 1], ctx.q[L - 2]
+    x2 = ctx.square_relin(keys, cts)
+    t = ctx.rescale(ctx.mul_scalar(cts, _round_half_up(a3 * q1), float(q1)))
+    x3 = ctx.cmult_relin(keys, x2, t)
+    u = ctx.rescale(ctx.rescale(ctx.mul_scalar(cts, _round_half_up(a1 * s * s), float(s * s))))
+    s3 = s ** 3 / (q1 * q2)
+    y = [ctx.add(a, b) for a, b in zip(x3, u)]
+    return ctx.add_const(y, _round_half_up(a0 * s3)), s3
 
 
 class Pipeline:
@@ -33,6 +58,10 @@ class Pipeline:
                 self.need_relin = True
                 self.plan.append(dict(op="square", L=L))
                 L -= 1
+            elif ly["op"] == "poly3":
+                self.need_relin = True
+                self.plan.append(dict(op="poly3", L=L, coef=ly.get("coef", POLY3)))
+                L -= 2
             elif ly["op"] == "pool":
                 self.plan.append(dict(op="pool", L=L))
             else:
@@ -108,18 +137,23 @@ class Pipeline:
                             idx.append(base + (2 * uo + a) * S + (2 * vo + b))
         return idx
 
-    def forward(self, cts, trace=None):
+    def forward(self, cts, trace=None, scale=None):
+        """scale: exact rational scale of the inputs (default: the context's 2^log2_scale); only poly3 needs it."""
         ctx = self.ctx
         S = None
+        sc = Fraction(cts[0].scale) if scale is None else Fraction(scale)
         for p, w in zip(self.plan, self.weights):
             if p["op"] == "conv":
                 cts = ctx.hconv(self.keys, p["conv"], p["lay"], w, cts, do_rescale=True)
-                S = p["lay"].S_out
+                S = p["lay"].S_out  # weights at s_w = q_{L-1} and one rescale: the scale is unchanged (A14)
             elif p["op"] == "fc":
                 cts = ctx.fc(self.keys, p["fc"], w, cts, do_rescale=True)
                 S = 1
             elif p["op"] == "square":
                 cts = ctx.square_relin(self.keys, cts)
+                sc = sc * sc / ctx.q[p["L"] - 1]
+            elif p["op"] == "poly3":
+                cts, sc = poly3_activation(ctx, self.keys, cts, sc, p["coef"])
             elif p["op"] == "pool":
                 cts = ctx.sum_groups([cts[i] for i in self.pool_order(len(cts), S)], 4)
                 S //= 2

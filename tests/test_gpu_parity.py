@@ -461,3 +461,55 @@ def test_config4_mobilenet_layers_full_size_decoded(mods):
     dws = dict(BS=2, C_in=64, H=112, W=112, C_out=64, K=3, stride=2, pad=1, depthwise=True)
     err, lay = decoded_conv_error(mods, "cfg4", dws, 4, 403, w_std=0.05)
     assert lay.S_out == 2 and lay.H_out == 56 and err < 1e-3
+
+
+def test_cmult_scalar_poly3_bit_exact(mods):
+    """a13: general CMult + relin + rescale, PMultConst, constant add and the degree-3 activation of config 3 (R2.12)."""
+    ck, fr, fenc = mods
+    from fractions import Fraction
+    from paper_2606_16359_b200.pipeline import poly3_activation
+    P, ctx = make(mods, "mid12")
+    L = P.nq
+    ok, gk = ck.keygen(P, 61, [], want_relin=True), ctx.keygen(61, [], want_relin=True)
+    rng = np.random.default_rng(13)
+    xs = [rng.uniform(-2, 2, P.n) for _ in range(3)]
+    o_ct, g_ct = [], []
+    for i, x in enumerate(xs):
+        pt = ck.encode(P, x, L)
+        o_ct.append(ck.encrypt(P, ok, pt, 300 + i))
+        g_ct.append(ctx.encrypt(gk, ctx.pt_from_coeffs(pt.coeffs, L, float(pt.scale)), 300 + i))
+    prod = ctx.cmult_relin(gk, g_ct[:2], g_ct[1:])
+    for i in range(2):
+        assert np.array_equal(ctx.ct_export(prod[i]), ck.cmult_relin(P, ok, o_ct[i], o_ct[i + 1]).c)
+    k = ck.round_half_up(Fraction(197, 1000) * o_ct[0].scale ** 2)
+    sc = ctx.mul_scalar(g_ct, k, float(o_ct[0].scale ** 2))
+    ref = ck.mul_const(P, o_ct[2], Fraction(197, 1000), o_ct[2].scale ** 2)
+    assert np.array_equal(ctx.ct_export(sc[2]), ref.c) and abs(sc[2].scale - float(ref.scale)) <= 1e-9 * float(ref.scale)
+    assert np.array_equal(ctx.ct_export(ctx.add_const(g_ct, 12345678901)[1]), ck.add_const(P, o_ct[1], 12345678901).c)
+    act, s3 = poly3_activation(ctx, gk, g_ct, o_ct[0].scale)
+    for i, x in enumerate(xs):
+        ref = ck.poly3(P, ok, o_ct[i])
+        assert s3 == ref.scale and act[i].L == L - 2
+        assert np.array_equal(ctx.ct_export(act[i]), ref.c), i
+        assert np.abs(ctx.decrypt_slots(gk, act[i]).real - (0.5 + 0.197 * x - 0.004 * x ** 3)).max() < 1e-3
+    ctx.close()
+
+
+def test_config3_conv_plus_activation_full_size_decoded(mods):
+    """config 3 at full size: conv 16->16 then the degree-3 activation, decoded against fp64 (property at any size)."""
+    ck, fr, fenc = mods
+    from paper_2606_16359_b200.pipeline import Pipeline
+    ctx = fenc.Context(**wl.PARAMS["cfg3"])
+    kw = wl.CONVS["resnet_16_16"]
+    x, w = wl.conv_inputs(311, kw, kaiming=True)
+    pipe = Pipeline(ctx, [{"op": "conv", "conv": dict(kw), "S": 1, "w": w}, {"op": "poly3"}])
+    keys = pipe.setup(key_seed=311)
+    out = pipe.forward(pipe.encrypt_input(x, 7000))
+    p0 = pipe.plan[0]
+    od = fr.ConvDesc(**kw)
+    Y = np.zeros((1, 16, 32, 32))
+    assert len(out) == 1 and out[0].L == ctx.n_q - 3
+    ctx.decrypt_decode(keys, out[0], p0["conv"], p0["lay"], 1, 0, 0, 0, 0, Y)
+    c = fr.direct_conv(od, x, w)
+    assert np.abs(Y - (0.5 + 0.197 * c - 0.004 * c ** 3)).max() < 1e-3
+    ctx.close()

@@ -96,3 +96,26 @@ def test_encrypted_toy_network_matches_fp64():
     want = plain_network(layers, x)
     assert np.abs(want).max() < 0.45  # a single 40-bit limb at scale 2^40 holds |value| < 0.5 (A23)
     assert np.abs(Y - want).max() < 1e-4
+
+
+def test_cmult_and_poly3_against_fp64():
+    """CMult+relin+rescale decodes to the slot-wise product; the degree-3 activation of BASELINE config 3 decodes to
+    0.5 + 0.197 x - 0.004 x^3 (R2.12) and consumes exactly two levels."""
+    P = ck.Params(9, 4, 40, 2, 60, 2, 40)
+    keys = ck.keygen(P, 21, [], want_relin=True)
+    rng = np.random.default_rng(8)
+    x, y = rng.uniform(-2, 2, P.n), rng.uniform(-1, 1, P.n)
+    cx = ck.encrypt(P, keys, ck.encode(P, x, P.nq), 1)
+    cy = ck.encrypt(P, keys, ck.encode(P, y, P.nq), 2)
+    prod = ck.cmult_relin(P, keys, cx, cy)
+    assert prod.L == P.nq - 1 and np.abs(ck.decrypt_decode(P, keys, prod).real - x * y).max() < 1e-6
+    assert np.array_equal(ck.cmult_relin(P, keys, cx, cx).c, ck.square_relin(P, keys, cx).c)  # x^2 is the case y = x
+    act = ck.poly3(P, keys, cx)
+    assert act.L == P.nq - 2
+    want = 0.5 + 0.197 * x - 0.004 * x ** 3
+    assert np.abs(ck.decrypt_decode(P, keys, act).real - want).max() < 1e-6
+    # PMultConst / add_const closed forms: times the integer 3 at E = 1 triples the slots; adding round(s/4) adds 0.25
+    tri = ck.mul_const(P, cx, 3, 1)
+    assert np.abs(ck.decrypt_decode(P, keys, tri).real - 3 * x).max() < 1e-6
+    quarter = ck.add_const(P, cx, ck.round_half_up(cx.scale / 4))
+    assert np.abs(ck.decrypt_decode(P, keys, quarter).real - (x + 0.25)).max() < 1e-6
