@@ -295,7 +295,8 @@ static fenc_status make_wts(fenc_ctx *ctx, size_t n, const std::function<void(si
   if (n_limbs < 1 || (int)n_limbs > ctx->nq) return FENC_ERR_INVALID_ARG;
   const int L = n_limbs;
   const size_t N = ctx->N;
-  std::unique_ptr<fenc_wts> W(new fenc_wts{ctx, L, scale > 0 ? scale : (double)ctx->mod[L - 1], n});  // A14: s_w = q_{L-1}
+  std::unique_ptr<fenc_wts, void (*)(fenc_wts *)> W(new fenc_wts{ctx, L, scale > 0 ? scale : (double)ctx->mod[L - 1], n},
+                                                     fenc_wts_free);  // A14: s_w = q_{L-1}
   W->slot.resize(n);
   std::vector<std::vector<int64_t>> uniq;
   std::map<std::pair<u64, u64>, int> seen;
@@ -361,6 +362,7 @@ extern "C" void fenc_wts_free(fenc_wts *W) {
 // 3. outer rotations: Rot(P_d, d cs) for d != 0, ONE batch;  4. Y = P_0 + sum of those;  5. one rescale per output (A13)
 static fenc_status run_linear(fenc_ctx *ctx, const fenc_keys *K, const LinGraph &g, const fenc_wts *W, fenc_ct *const *in,
                               size_t n_in, int do_rescale, fenc_ct **out, size_t cap, size_t *n_out) {
+  Scope sc(ctx);
   fenc_status st;
   const size_t nin_bg = g.nin_bg, nout_bg = g.outs.size(), BG = g.BG;
   if (n_in != nin_bg * BG) return fail(ctx, FENC_ERR_MISMATCH, "expected %zu input ciphertexts, got %zu", nin_bg * BG, n_in);
@@ -377,7 +379,7 @@ static fenc_status run_linear(fenc_ctx *ctx, const fenc_keys *K, const LinGraph 
   const size_t N = ctx->N, CT = (size_t)2 * L * N;
   const size_t n_inner = g.inner.size();
   // ---- 1. inner rotations
-  u64 *Rbuf = n_inner ? dalloc_t<u64>(ctx, n_inner * BG * CT) : nullptr;
+  u64 *Rbuf = n_inner ? sc.alloc<u64>(n_inner * BG * CT) : nullptr;
   if (n_inner && !Rbuf) return fail(ctx, FENC_ERR_OOM, "inner-rotation results (%zu ciphertexts)", n_inner * BG);
   {
     std::vector<const u64 *> vin;
@@ -400,12 +402,12 @@ static fenc_status run_linear(fenc_ctx *ctx, const fenc_keys *K, const LinGraph 
   }
   std::vector<fenc_ct *> res(nout_bg * BG, nullptr);
   const double s_acc = s_in * W->scale;
-  u64 *Ybuf = do_rescale ? dalloc_t<u64>(ctx, nout_bg * BG * CT) : nullptr;  // pre-rescale sums
-  u64 *Pbuf = dalloc_t<u64>(ctx, n_P * BG * CT);                               // diagonal partial sums (worst case)
-  u64 *Obuf = n_rot_out ? dalloc_t<u64>(ctx, n_rot_out * BG * CT) : nullptr;   // outer-rotation results
+  u64 *Ybuf = do_rescale ? sc.alloc<u64>(nout_bg * BG * CT) : nullptr;  // pre-rescale sums
+  u64 *Pbuf = sc.alloc<u64>(n_P * BG * CT);                               // diagonal partial sums (worst case)
+  u64 *Obuf = n_rot_out ? sc.alloc<u64>(n_rot_out * BG * CT) : nullptr;   // outer-rotation results
   if ((do_rescale && !Ybuf) || !Pbuf || (n_rot_out && !Obuf)) return fail(ctx, FENC_ERR_OOM, "hconv partial sums");
   for (size_t i = 0; i < res.size(); i++) {
-    res[i] = new_ct(ctx, do_rescale ? L - 1 : L, do_rescale ? s_acc / (double)ctx->mod[L - 1] : s_acc);
+    res[i] = sc.ct(do_rescale ? L - 1 : L, do_rescale ? s_acc / (double)ctx->mod[L - 1] : s_acc);
     if (!res[i]) return fail(ctx, FENC_ERR_OOM, "hconv outputs");
   }
   MacJob job;
@@ -457,7 +459,7 @@ static fenc_status run_linear(fenc_ctx *ctx, const fenc_keys *K, const LinGraph 
     st = rescale_batch(ctx, L, items);
     if (st != FENC_OK) return st;
   }
-  dfree(ctx, Rbuf), dfree(ctx, Ybuf), dfree(ctx, Pbuf), dfree(ctx, Obuf);
+  sc.ok = true;
   for (size_t i = 0; i < res.size(); i++) out[i] = res[i];
   *n_out = res.size();
   return FENC_OK;
@@ -477,6 +479,7 @@ extern "C" fenc_status fenc_hconv(fenc_ctx *ctx, const fenc_keys *K, const fenc_
 extern "C" fenc_status fenc_compress(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const *in, size_t n_in, const fenc_pt *mask_c,
                                      const uint32_t *term_out, const uint32_t *term_src, const int32_t *term_rot, size_t n_terms,
                                      int do_rescale, fenc_ct **out, size_t n_out) {
+  Scope sc(ctx);
   if (!ctx || !K || !in || !term_out || !term_src || !term_rot || !out || n_in == 0 || n_out == 0) return FENC_ERR_INVALID_ARG;
   fenc_pt *mask = const_cast<fenc_pt *>(mask_c);
   const int L = in[0]->L;
@@ -500,7 +503,7 @@ extern "C" fenc_status fenc_compress(fenc_ctx *ctx, const fenc_keys *K, fenc_ct 
     fenc_status st = pt_device(ctx, mask);
     if (st != FENC_OK) return st;
     s_mid = s_in * mask->scale;
-    Mbuf = dalloc_t<u64>(ctx, n_in * CT);
+    Mbuf = sc.alloc<u64>(n_in * CT);
     if (!Mbuf) return fail(ctx, FENC_ERR_OOM, "compress masked sources");
     MacJob job;
     for (size_t i = 0; i < n_in; i++) {
@@ -510,12 +513,12 @@ extern "C" fenc_status fenc_compress(fenc_ctx *ctx, const fenc_keys *K, fenc_ct 
     st = run_mac(ctx, job, L);
     if (st != FENC_OK) return st;
   }
-  u64 *Rbuf = dalloc_t<u64>(ctx, n_terms * CT);
-  u64 *Ybuf = do_rescale ? dalloc_t<u64>(ctx, n_out * CT) : nullptr;
+  u64 *Rbuf = sc.alloc<u64>(n_terms * CT);
+  u64 *Ybuf = do_rescale ? sc.alloc<u64>(n_out * CT) : nullptr;
   if (!Rbuf || (do_rescale && !Ybuf)) return fail(ctx, FENC_ERR_OOM, "compress workspace");
   std::vector<fenc_ct *> res(n_out);
   for (size_t t = 0; t < n_out; t++) {
-    res[t] = new_ct(ctx, do_rescale ? L - 1 : L, do_rescale ? s_mid / (double)ctx->mod[L - 1] : s_mid);
+    res[t] = sc.ct(do_rescale ? L - 1 : L, do_rescale ? s_mid / (double)ctx->mod[L - 1] : s_mid);
     if (!res[t]) return fail(ctx, FENC_ERR_OOM, "compress outputs");
   }
   std::vector<const u64 *> vin(n_terms);
@@ -552,7 +555,7 @@ extern "C" fenc_status fenc_compress(fenc_ctx *ctx, const fenc_keys *K, fenc_ct 
     st = rescale_batch(ctx, L, items);
     if (st != FENC_OK) return st;
   }
-  dfree(ctx, Mbuf), dfree(ctx, Rbuf), dfree(ctx, Ybuf);
+  sc.ok = true;
   for (size_t t = 0; t < n_out; t++) out[t] = res[t];
   return FENC_OK;
 }

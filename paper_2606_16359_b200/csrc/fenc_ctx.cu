@@ -95,7 +95,7 @@ u32 galois_elt(const fenc_ctx *ctx, int step) {
 // ------------------------------------------------------------------------------------------------ context
 extern "C" fenc_status fenc_params_init(const fenc_params_desc *d, fenc_ctx **out) {
   if (!d || !out) return FENC_ERR_INVALID_ARG;
-  std::unique_ptr<fenc_ctx> c(new fenc_ctx());
+  std::unique_ptr<fenc_ctx, void (*)(fenc_ctx *)> c(new fenc_ctx(), fenc_ctx_free);
   fenc_ctx *ctx = c.get();
   if (d->log2N < 4 || d->log2N > 16 || d->n_q < 1 || d->n_p < 1 || d->n_q + d->n_p > FENC_MAX_MOD || d->q_bits > 60 ||
       d->p_bits > 60 || (d->dnum < 1 && !d->dlen_override))

@@ -144,6 +144,34 @@ struct DescStage {
   char *commit();
 };
 fenc_ct *new_ct(fenc_ctx *ctx, int L, double scale);
+extern "C" void fenc_ct_free(fenc_ct *ct);
+// Scope-bound temporaries of one API call: device buffers are released when the call returns (the allocator is
+// stream-ordered: torch's caching allocator on the context's stream, or cudaFree), and ciphertexts created for the
+// outputs are released too unless the call succeeded (ok = true).
+struct Scope {
+  fenc_ctx *ctx;
+  std::vector<void *> bufs;
+  std::vector<fenc_ct *> cts;
+  bool ok = false;
+  explicit Scope(fenc_ctx *c) : ctx(c) {}
+  Scope(const Scope &) = delete;
+  ~Scope() {
+    for (void *b : bufs) dfree(ctx, b);
+    if (!ok)
+      for (fenc_ct *c : cts) fenc_ct_free(c);
+  }
+  template <class T>
+  T *alloc(size_t count) {
+    T *p = dalloc_t<T>(ctx, count);
+    if (p) bufs.push_back(p);
+    return p;
+  }
+  fenc_ct *ct(int L, double scale) {
+    fenc_ct *c = new_ct(ctx, L, scale);
+    if (c) cts.push_back(c);
+    return c;
+  }
+};
 // batched key switch over items (all at level L): out = (ModDown(acc_0) + add0, ModDown(acc_1) + add1)
 fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items);
 // batched rescale: items[i].sub_in = input ct [2][L][N], items[i].out = [2][L-1][N]

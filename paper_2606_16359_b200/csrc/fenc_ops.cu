@@ -12,14 +12,14 @@ static bool scale_close(double a, double b) { return std::fabs(a - b) <= 1e-9 * 
 
 // centred integer coefficients (host) -> [L][N] NTT domain, Montgomery form
 fenc_status coeffs_to_mont(fenc_ctx *ctx, const int64_t *coeffs, int L, u64 *d_out) {
+  Scope sc(ctx);
   const size_t N = ctx->N;
-  i64 *d_c = dalloc_t<i64>(ctx, N);
+  i64 *d_c = sc.alloc<i64>(N);
   if (!d_c) return fail(ctx, FENC_ERR_OOM, "coefficient staging");
   CUDA_OK(ctx, cudaMemcpyAsync(d_c, coeffs, N * 8, cudaMemcpyHostToDevice, ctx->stream));
   CUDA_OK(ctx, k_reduce_signed(ctx->k, d_c, ctx->d_ident_mod, d_out, L));
   CUDA_OK(ctx, k_ntt(ctx->k, d_out, 0, d_out, 0, ctx->d_ident_rows, L, 1));
   CUDA_OK(ctx, k_mont_convert(ctx->k, d_out, d_out, ctx->d_ident_mod, L, true));
-  dfree(ctx, d_c);
   return FENC_OK;
 }
 fenc_status pt_device(fenc_ctx *ctx, fenc_pt *pt) {
@@ -33,11 +33,12 @@ fenc_status pt_device(fenc_ctx *ctx, fenc_pt *pt) {
 // For every digit j over ALL nq+np limbs t: a_j[t] uniform, b_j[t] = -a_j[t] s + e_j + f_{j,t} s' (mod t),
 // f_{j,t} = P mod t if t in D_j else 0.  Stored in NTT domain, Montgomery form: [beta_max][{b,a}][A][N].
 static fenc_status make_switch_key(fenc_ctx *ctx, fenc_keys *K, int64_t key_id, const u64 *d_sp_mont, u32 g, u64 **out) {
+  Scope sc(ctx);
   const int A = ctx->A, N = ctx->N, nq = ctx->nq;
   const size_t AN = (size_t)A * N;
   u64 *evk = dalloc_t<u64>(ctx, (size_t)ctx->beta_max * 2 * AN);
-  u64 *d_a = dalloc_t<u64>(ctx, AN), *d_e = dalloc_t<u64>(ctx, AN);
-  u64 *d_keys = dalloc_t<u64>(ctx, A), *d_f = dalloc_t<u64>(ctx, A);
+  u64 *d_a = sc.alloc<u64>(AN), *d_e = sc.alloc<u64>(AN);
+  u64 *d_keys = sc.alloc<u64>(A), *d_f = sc.alloc<u64>(A);
   if (!evk || !d_a || !d_e || !d_keys || !d_f) return fail(ctx, FENC_ERR_OOM, "evaluation key");
   u64 Pmod[FENC_MAX_MOD];
   for (int t = 0; t < A; t++) {
@@ -62,27 +63,26 @@ static fenc_status make_switch_key(fenc_ctx *ctx, fenc_keys *K, int64_t key_id, 
     CUDA_OK(ctx, k_mont_convert(ctx->k, d_a, ka, ctx->d_ident_mod, A, true));
     CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));  // hk / hf go out of scope
   }
-  dfree(ctx, d_a), dfree(ctx, d_e), dfree(ctx, d_keys), dfree(ctx, d_f);
   *out = evk;
   return FENC_OK;
 }
 
 extern "C" fenc_status fenc_keygen(fenc_ctx *ctx, uint64_t seed, const int32_t *rot_steps, size_t n_rot, int want_relin,
                                    fenc_keys **out) {
+  Scope sc(ctx);
   if (!ctx || !out || (n_rot && !rot_steps)) return FENC_ERR_INVALID_ARG;
-  std::unique_ptr<fenc_keys> K(new fenc_keys{ctx, seed, {}, nullptr, {}});
+  std::unique_ptr<fenc_keys, void (*)(fenc_keys *)> K(new fenc_keys{ctx, seed, {}, nullptr, {}}, fenc_keys_free);
   const int A = ctx->A, N = ctx->N;
   K->s.resize(N);
   fh::sample_ternary(fh::stream_key(seed, PURPOSE_SECRET, 0, 0, 0), N, K->s.data());
   K->d_s_mont = dalloc_t<u64>(ctx, (size_t)A * N);
-  i64 *d_c = dalloc_t<i64>(ctx, N);
+  i64 *d_c = sc.alloc<i64>(N);
   if (!K->d_s_mont || !d_c) return fail(ctx, FENC_ERR_OOM, "secret key");
   CUDA_OK(ctx, cudaMemcpyAsync(d_c, K->s.data(), (size_t)N * 8, cudaMemcpyHostToDevice, ctx->stream));
   CUDA_OK(ctx, k_reduce_signed(ctx->k, d_c, ctx->d_ident_mod, K->d_s_mont, A));
   CUDA_OK(ctx, k_ntt(ctx->k, K->d_s_mont, 0, K->d_s_mont, 0, ctx->d_ident_rows, A, 1));
   CUDA_OK(ctx, k_mont_convert(ctx->k, K->d_s_mont, K->d_s_mont, ctx->d_ident_mod, A, true));
   CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
-  dfree(ctx, d_c);
   for (size_t i = 0; i < n_rot; i++) {
     int r = ((rot_steps[i] % ctx->n) + ctx->n) % ctx->n;
     if (r == 0 || K->evk.count(r)) continue;
@@ -94,14 +94,13 @@ extern "C" fenc_status fenc_keygen(fenc_ctx *ctx, uint64_t seed, const int32_t *
   }
   if (want_relin) {
     // s' = s * s: from Montgomery form, mont_mul(s 2^64, s 2^64) = s^2 2^64 directly
-    u64 *d_s2 = dalloc_t<u64>(ctx, (size_t)A * N), *d_sn = dalloc_t<u64>(ctx, (size_t)A * N);
+    u64 *d_s2 = sc.alloc<u64>((size_t)A * N), *d_sn = sc.alloc<u64>((size_t)A * N);
     if (!d_s2 || !d_sn) return fail(ctx, FENC_ERR_OOM, "relinearisation key");
     CUDA_OK(ctx, k_mont_convert(ctx->k, K->d_s_mont, d_sn, ctx->d_ident_mod, A, false));
     CUDA_OK(ctx, k_mul_rows(ctx->k, d_sn, d_sn, d_s2, ctx->d_ident_mod, A));
     CUDA_OK(ctx, k_mont_convert(ctx->k, d_s2, d_s2, ctx->d_ident_mod, A, true));
     u64 *evk = nullptr;
     fenc_status st = make_switch_key(ctx, K.get(), FENC_RELIN_KEY_ID, d_s2, 1, &evk);
-    dfree(ctx, d_s2), dfree(ctx, d_sn);
     if (st != FENC_OK) return st;
     K->evk[FENC_RELIN_KEY_ID] = evk;
   }
@@ -121,12 +120,13 @@ extern "C" fenc_status fenc_secret_export(fenc_ctx *ctx, const fenc_keys *K, int
   return FENC_OK;
 }
 extern "C" fenc_status fenc_evk_export(fenc_ctx *ctx, const fenc_keys *K, int64_t key_id, uint64_t *b, uint64_t *a) {
+  Scope sc(ctx);
   if (!ctx || !K || !b || !a) return FENC_ERR_INVALID_ARG;
   auto it = K->evk.find(key_id);
   if (it == K->evk.end()) return fail(ctx, FENC_ERR_NO_KEY, "no key %lld", (long long)key_id);
   const int A = ctx->A, N = ctx->N;
   const size_t AN = (size_t)A * N;
-  u64 *tmp = dalloc_t<u64>(ctx, AN);
+  u64 *tmp = sc.alloc<u64>(AN);
   if (!tmp) return fail(ctx, FENC_ERR_OOM, "export staging");
   for (int j = 0; j < ctx->beta_max; j++)
     for (int c = 0; c < 2; c++) {
@@ -135,7 +135,6 @@ extern "C" fenc_status fenc_evk_export(fenc_ctx *ctx, const fenc_keys *K, int64_
       CUDA_OK(ctx, cudaMemcpyAsync((c == 0 ? b : a) + (size_t)j * AN, tmp, AN * 8, cudaMemcpyDeviceToHost, ctx->stream));
     }
   CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
-  dfree(ctx, tmp);
   return FENC_OK;
 }
 
@@ -172,11 +171,12 @@ extern "C" void fenc_pt_free(fenc_pt *pt) {
 
 // ------------------------------------------------------------------------------------------------ encrypt / decrypt (R2.5)
 extern "C" fenc_status fenc_encrypt(fenc_ctx *ctx, const fenc_keys *K, const fenc_pt *pt, uint64_t enc_seed, fenc_ct **out) {
+  Scope sc(ctx);
   if (!ctx || !K || !pt || !out) return FENC_ERR_INVALID_ARG;
   const int L = pt->L, N = ctx->N;
-  fenc_ct *ct = new_ct(ctx, L, pt->scale);
-  i64 *d_m = dalloc_t<i64>(ctx, N);
-  u64 *d_x = dalloc_t<u64>(ctx, (size_t)L * N), *d_keys = dalloc_t<u64>(ctx, L);
+  fenc_ct *ct = sc.ct(L, pt->scale);
+  i64 *d_m = sc.alloc<i64>(N);
+  u64 *d_x = sc.alloc<u64>((size_t)L * N), *d_keys = sc.alloc<u64>(L);
   if (!ct || !d_m || !d_x || !d_keys) return fail(ctx, FENC_ERR_OOM, "encrypt");
   std::vector<u64> hk(L);
   for (int t = 0; t < L; t++) hk[t] = fh::stream_key(enc_seed, PURPOSE_ENC_A, (u64)t, 0, 0);
@@ -189,22 +189,22 @@ extern "C" fenc_status fenc_encrypt(fenc_ctx *ctx, const fenc_keys *K, const fen
   CUDA_OK(ctx, k_ntt(ctx->k, c1, 0, c1, 0, ctx->d_ident_rows, L, 1));
   CUDA_OK(ctx, k_x_minus_as(ctx->k, c1, d_x, K->d_s_mont, c0, ctx->d_ident_mod, L));  // c0 = (e + m) - a s
   CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
-  dfree(ctx, d_m), dfree(ctx, d_x), dfree(ctx, d_keys);
+  sc.ok = true;
   *out = ct;
   return FENC_OK;
 }
 
 extern "C" fenc_status fenc_decrypt_slots(fenc_ctx *ctx, const fenc_keys *K, const fenc_ct *ct, double *re, double *im) {
+  Scope sc(ctx);
   if (!ctx || !K || !ct || !re) return FENC_ERR_INVALID_ARG;
   const int L = ct->L, N = ctx->N;
-  u64 *d_mu = dalloc_t<u64>(ctx, (size_t)L * N);
+  u64 *d_mu = sc.alloc<u64>((size_t)L * N);
   if (!d_mu) return fail(ctx, FENC_ERR_OOM, "decrypt");
   CUDA_OK(ctx, k_dec_combine(ctx->k, ct->d, K->d_s_mont, d_mu, L));
   CUDA_OK(ctx, k_intt(ctx->k, nullptr, d_mu, 0, false, d_mu, 0, ctx->d_ident_rows, L, ctx->d_ninv, 1));
   std::vector<u64> mu((size_t)L * N);
   CUDA_OK(ctx, cudaMemcpyAsync(mu.data(), d_mu, mu.size() * 8, cudaMemcpyDeviceToHost, ctx->stream));
   CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
-  dfree(ctx, d_mu);
   std::vector<long double> m(N);
   fh::crt_centre_scaled(ctx->mod.data(), L, N, mu.data(), (long double)ct->scale, m.data());
   fh::decode_coeffs(ctx->logN, m.data(), re, im);
@@ -212,26 +212,28 @@ extern "C" fenc_status fenc_decrypt_slots(fenc_ctx *ctx, const fenc_keys *K, con
 }
 
 extern "C" fenc_status fenc_ct_export(fenc_ctx *ctx, const fenc_ct *ct, uint64_t *limbs) {
+  Scope sc(ctx);
   if (!ctx || !ct || !limbs) return FENC_ERR_INVALID_ARG;
   LevelPlan *P = get_plan(ctx, ct->L);
   const size_t n = (size_t)2 * ct->L * ctx->N;
-  u64 *tmp = dalloc_t<u64>(ctx, n);
+  u64 *tmp = sc.alloc<u64>(n);
   if (!P || !tmp) return fail(ctx, FENC_ERR_OOM, "export");
   CUDA_OK(ctx, k_intt(ctx->k, nullptr, ct->d, 0, false, tmp, 0, P->d_rows_ct, 2 * ct->L, P->d_scale_ct, 1));
   CUDA_OK(ctx, cudaMemcpyAsync(limbs, tmp, n * 8, cudaMemcpyDeviceToHost, ctx->stream));
   CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
-  dfree(ctx, tmp);
   return FENC_OK;
 }
 extern "C" fenc_status fenc_ct_import(fenc_ctx *ctx, const uint64_t *limbs, uint32_t L, double scale, fenc_ct **out) {
+  Scope sc(ctx);
   if (!ctx || !limbs || !out || L < 1 || (int)L > ctx->nq) return FENC_ERR_INVALID_ARG;
   LevelPlan *P = get_plan(ctx, (int)L);
-  fenc_ct *ct = new_ct(ctx, (int)L, scale > 0 ? scale : ctx->default_scale);
+  fenc_ct *ct = sc.ct((int)L, scale > 0 ? scale : ctx->default_scale);
   if (!P || !ct) return fail(ctx, FENC_ERR_OOM, "import");
   const size_t n = (size_t)2 * L * ctx->N;
   CUDA_OK(ctx, cudaMemcpyAsync(ct->d, limbs, n * 8, cudaMemcpyHostToDevice, ctx->stream));
   CUDA_OK(ctx, k_ntt(ctx->k, ct->d, 0, ct->d, 0, P->d_rows_ct, 2 * (int)L, 1));
   CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+  sc.ok = true;
   *out = ct;
   return FENC_OK;
 }
@@ -298,6 +300,7 @@ double mac_alg_bytes(fenc_ctx *ctx, const std::vector<const u64 *> &tc, const st
 }
 extern "C" fenc_status fenc_rotate(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const *in, const int32_t *steps, size_t n,
                                    fenc_ct **out) {
+  Scope sc(ctx);
   if (!ctx || !K || !in || !steps || !out) return FENC_ERR_INVALID_ARG;
   if (n == 0) return FENC_OK;
   const int L = in[0]->L;
@@ -307,23 +310,19 @@ extern "C" fenc_status fenc_rotate(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *c
   std::vector<fenc_ct *> made(n, nullptr);
   for (size_t i = 0; i < n; i++) {
     if (in[i]->L != L) return fail(ctx, FENC_ERR_MISMATCH, "rotate: inputs differ in level");
-    made[i] = new_ct(ctx, L, in[i]->scale);
-    if (!made[i]) {
-      for (auto *c : made) fenc_ct_free(c);
-      return fail(ctx, FENC_ERR_OOM, "rotate output");
-    }
+    made[i] = sc.ct(L, in[i]->scale);
+    if (!made[i]) return fail(ctx, FENC_ERR_OOM, "rotate output");
     vin[i] = in[i]->d, vout[i] = made[i]->d;
   }
   fenc_status st = rotate_raw(ctx, K, L, vin, vs, vout);
-  if (st != FENC_OK) {
-    for (auto *c : made) fenc_ct_free(c);
-    return st;
-  }
+  if (st != FENC_OK) return st;
+  sc.ok = true;
   for (size_t i = 0; i < n; i++) out[i] = made[i];
   return FENC_OK;
 }
 
 extern "C" fenc_status fenc_rescale(fenc_ctx *ctx, fenc_ct *const *in, size_t n, fenc_ct **out) {
+  Scope sc(ctx);
   if (!ctx || !in || !out) return FENC_ERR_INVALID_ARG;
   if (n == 0) return FENC_OK;
   const int L = in[0]->L;
@@ -332,21 +331,23 @@ extern "C" fenc_status fenc_rescale(fenc_ctx *ctx, fenc_ct *const *in, size_t n,
   std::vector<fenc_ct *> made(n, nullptr);
   for (size_t i = 0; i < n; i++) {
     if (in[i]->L != L) return fail(ctx, FENC_ERR_MISMATCH, "rescale: inputs differ in level");
-    made[i] = new_ct(ctx, L - 1, in[i]->scale / (double)ctx->mod[L - 1]);
+    made[i] = sc.ct(L - 1, in[i]->scale / (double)ctx->mod[L - 1]);
     if (!made[i]) return fail(ctx, FENC_ERR_OOM, "rescale output");
     items[i] = BatchItem{};
     items[i].sub_in = in[i]->d, items[i].out = made[i]->d;
   }
   fenc_status st = rescale_batch(ctx, L, items);
   if (st != FENC_OK) return st;
+  sc.ok = true;
   for (size_t i = 0; i < n; i++) out[i] = made[i];
   return FENC_OK;
 }
 
 extern "C" fenc_status fenc_add(fenc_ctx *ctx, const fenc_ct *a, const fenc_ct *b, fenc_ct **out) {
+  Scope sc(ctx);
   if (!ctx || !a || !b || !out) return FENC_ERR_INVALID_ARG;
   if (a->L != b->L || !scale_close(a->scale, b->scale)) return fail(ctx, FENC_ERR_MISMATCH, "add: level or scale differ");
-  fenc_ct *c = new_ct(ctx, a->L, a->scale);
+  fenc_ct *c = sc.ct(a->L, a->scale);
   if (!c) return fail(ctx, FENC_ERR_OOM, "add");
   std::vector<const u64 *> terms{a->d, b->d};
   std::vector<int> start{0, 2};
@@ -356,11 +357,13 @@ extern "C" fenc_status fenc_add(fenc_ctx *ctx, const fenc_ct *a, const fenc_ct *
   char *base = st.commit();
   if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
   CUDA_OK(ctx, k_add_many(ctx->k, (const u64 *const *)(base + o1), (const int *)(base + o2), (u64 *const *)(base + o3), 1, a->L, 2));
+  sc.ok = true;
   *out = c;
   return FENC_OK;
 }
 
 extern "C" fenc_status fenc_pmult_sum(fenc_ctx *ctx, fenc_ct *const *in, fenc_pt *const *pt, size_t n, fenc_ct **out) {
+  Scope sc(ctx);
   if (!ctx || !in || !pt || !out || n == 0) return FENC_ERR_INVALID_ARG;
   const int L = in[0]->L;
   std::vector<const u64 *> tc(n), tp(n);
@@ -371,7 +374,7 @@ extern "C" fenc_status fenc_pmult_sum(fenc_ctx *ctx, fenc_ct *const *in, fenc_pt
     if (s != FENC_OK) return s;
     tc[i] = in[i]->d, tp[i] = pt[i]->d_mont;
   }
-  fenc_ct *c = new_ct(ctx, L, in[0]->scale * pt[0]->scale);
+  fenc_ct *c = sc.ct(L, in[0]->scale * pt[0]->scale);
   if (!c) return fail(ctx, FENC_ERR_OOM, "pmult");
   MacJob job;
   job.terms.resize(1);
@@ -379,6 +382,7 @@ extern "C" fenc_status fenc_pmult_sum(fenc_ctx *ctx, fenc_ct *const *in, fenc_pt
   job.outs.push_back(c->d);
   fenc_status ms = run_mac(ctx, job, L);
   if (ms != FENC_OK) return ms;
+  sc.ok = true;
   *out = c;
   return FENC_OK;
 }
@@ -386,6 +390,7 @@ extern "C" fenc_status fenc_pmult_sum(fenc_ctx *ctx, fenc_ct *const *in, fenc_pt
 // CMult + relinearise + rescale (a13, R2.12): (d0, d1, d2) = (a0 b0, a0 b1 + a1 b0, a1 b1);
 // (d0, d1) + KS(d2; relin); rescale.  Batched over n pairs; x^2 is the case b = a.
 static fenc_status cmult_relin(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const *ina, fenc_ct *const *inb, size_t n, fenc_ct **out) {
+  Scope sc(ctx);
   if (n == 0) return FENC_OK;
   auto it = K->evk.find(FENC_RELIN_KEY_ID);
   if (it == K->evk.end()) return fail(ctx, FENC_ERR_NO_KEY, "no relinearisation key");
@@ -397,7 +402,7 @@ static fenc_status cmult_relin(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const
     if (ina[i]->L != L || inb[i]->L != L) return fail(ctx, FENC_ERR_MISMATCH, "product: inputs differ in level");
     pa[i] = ina[i]->d, pb[i] = inb[i]->d;
   }
-  u64 *d = dalloc_t<u64>(ctx, n * 3 * LN), *mid = dalloc_t<u64>(ctx, n * 2 * LN);
+  u64 *d = sc.alloc<u64>(n * 3 * LN), *mid = sc.alloc<u64>(n * 2 * LN);
   if (!d || !mid) return fail(ctx, FENC_ERR_OOM, "product");
   {
     DescStage st(ctx);
@@ -413,7 +418,7 @@ static fenc_status cmult_relin(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const
     items[i] = BatchItem{};
     items[i].ks_in = di + 2 * LN, items[i].out = mid + i * 2 * LN, items[i].evk = it->second;
     items[i].add0 = di, items[i].add1 = di + LN, items[i].g = 1;
-    made[i] = new_ct(ctx, L - 1, ina[i]->scale * inb[i]->scale / (double)ctx->mod[L - 1]);
+    made[i] = sc.ct(L - 1, ina[i]->scale * inb[i]->scale / (double)ctx->mod[L - 1]);
     if (!made[i]) return fail(ctx, FENC_ERR_OOM, "product output");
     rs[i] = BatchItem{};
     rs[i].sub_in = mid + i * 2 * LN, rs[i].out = made[i]->d;
@@ -422,7 +427,7 @@ static fenc_status cmult_relin(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const
   if (st != FENC_OK) return st;
   st = rescale_batch(ctx, L, rs);
   if (st != FENC_OK) return st;
-  dfree(ctx, d), dfree(ctx, mid);
+  sc.ok = true;
   for (size_t i = 0; i < n; i++) out[i] = made[i];
   return FENC_OK;
 }
@@ -439,6 +444,7 @@ extern "C" fenc_status fenc_cmult_relin(fenc_ctx *ctx, const fenc_keys *K, fenc_
 // factor the scale is multiplied by.  add_const: the integer k is added to coefficient 0 of c0 (scale unchanged).
 static fenc_status scalar_op(fenc_ctx *ctx, fenc_ct *const *in, size_t n, const uint64_t *k_res, double factor, bool add_const,
                              fenc_ct **out) {
+  Scope sc(ctx);
   if (!ctx || !in || !k_res || !out) return FENC_ERR_INVALID_ARG;
   if (n == 0) return FENC_OK;
   const int L = in[0]->L;
@@ -452,7 +458,7 @@ static fenc_status scalar_op(fenc_ctx *ctx, fenc_ct *const *in, size_t n, const 
   std::vector<fenc_ct *> made(n, nullptr);
   for (size_t i = 0; i < n; i++) {
     if (in[i]->L != L) return fail(ctx, FENC_ERR_MISMATCH, "scalar op: inputs differ in level");
-    made[i] = new_ct(ctx, L, add_const ? in[i]->scale : in[i]->scale * factor);
+    made[i] = sc.ct(L, add_const ? in[i]->scale : in[i]->scale * factor);
     if (!made[i]) return fail(ctx, FENC_ERR_OOM, "scalar op output");
     pin[i] = in[i]->d, pout[i] = made[i]->d;
   }
@@ -461,6 +467,7 @@ static fenc_status scalar_op(fenc_ctx *ctx, fenc_ct *const *in, size_t n, const 
   char *base = st.commit();
   if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
   CUDA_OK(ctx, k_scalar(ctx->k, (const u64 *const *)(base + o0), (u64 *const *)(base + o1), (const u64 *)(base + o2), (int)n, L, add_const));
+  sc.ok = true;
   for (size_t i = 0; i < n; i++) out[i] = made[i];
   return FENC_OK;
 }
@@ -473,6 +480,7 @@ extern "C" fenc_status fenc_add_const(fenc_ctx *ctx, fenc_ct *const *in, size_t 
 }
 
 extern "C" fenc_status fenc_sum_groups(fenc_ctx *ctx, fenc_ct *const *in, size_t group, size_t n_groups, fenc_ct **out) {
+  Scope sc(ctx);
   if (!ctx || !in || !out || group == 0) return FENC_ERR_INVALID_ARG;
   if (n_groups == 0) return FENC_OK;
   const int L = in[0]->L;
@@ -485,7 +493,7 @@ extern "C" fenc_status fenc_sum_groups(fenc_ctx *ctx, fenc_ct *const *in, size_t
     terms[i] = in[i]->d;
   }
   for (size_t g = 0; g < n_groups; g++) {
-    made[g] = new_ct(ctx, L, in[0]->scale);
+    made[g] = sc.ct(L, in[0]->scale);
     if (!made[g]) return fail(ctx, FENC_ERR_OOM, "sum output");
     start[g] = (int)(g * group), outs[g] = made[g]->d;
   }
@@ -496,6 +504,7 @@ extern "C" fenc_status fenc_sum_groups(fenc_ctx *ctx, fenc_ct *const *in, size_t
   if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
   CUDA_OK(ctx, k_add_many(ctx->k, (const u64 *const *)(base + o0), (const int *)(base + o1), (u64 *const *)(base + o2), (int)n_groups, L,
                           (int)terms.size()));
+  sc.ok = true;
   for (size_t g = 0; g < n_groups; g++) out[g] = made[g];
   return FENC_OK;
 }
