@@ -245,6 +245,7 @@ LevelPlan *get_plan(fenc_ctx *ctx, int L) {
   std::vector<ShoupC> scale_in(L), scale_p(2 * np), mul_pinv(A, ShoupC{0, 0}), scale_ct(2 * L);
   std::vector<u64> bc_up, bc_down((size_t)L * np);
   std::vector<int> tmp_index((size_t)P.beta * E, -1);
+  std::vector<ConvGroup> groups_up, groups_down, groups_rs;
   for (int j = 0; j < P.beta; j++) {
     const int lo = j * dlen, hi = std::min(lo + dlen, L);
     for (int i = lo; i < hi; i++) {
@@ -255,6 +256,8 @@ LevelPlan *get_plan(fenc_ctx *ctx, int L) {
       rows_in[i] = RowDesc{i, i, i, 0, 0, {0, 0, 0}};
       scale_in[i] = shoupc(fh::mulmod(ninv, fh::invmod(qhat, qi), qi), qi);
     }
+    groups_up.push_back(ConvGroup{lo, lo, hi - lo, lo, (int)rows_up.size(), E - (hi - lo), {0, 0}});
+    P.n_src_up = std::max(P.n_src_up, hi - lo);
     for (int t = 0; t < E; t++) {
       if (t >= lo && t < hi) continue;
       const u64 T = mod[emod(t)];
@@ -298,6 +301,13 @@ LevelPlan *get_plan(fenc_ctx *ctx, int L) {
       scale_ct[c * L + t] = shoupc(ninv, T);
     }
   }
+  for (int c = 0; c < 2; c++) {
+    groups_down.push_back(ConvGroup{c * np, nq, np, c * np, c * L, L, {0, 0}});
+    groups_rs.push_back(ConvGroup{c, L - 1, 1, c, c * (L - 1), L - 1, {0, 0}});
+  }
+  P.d_groups_up = upload_owned(ctx, P.owned, groups_up);
+  P.d_groups_down = upload_owned(ctx, P.owned, groups_down);
+  P.d_groups_rs = upload_owned(ctx, P.owned, groups_rs);
   P.d_rows_in = upload_owned(ctx, P.owned, rows_in);
   P.d_scale_in = upload_owned(ctx, P.owned, scale_in);
   P.d_rows_up = upload_owned(ctx, P.owned, rows_up);
@@ -376,15 +386,29 @@ fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items) {
     st.add(part);
     const BatchItem *d_items = (const BatchItem *)st.commit();
     if (!d_items) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
-    // a2 + a1: iNTT of sigma_g(d), pre-scaled for ModUp
-    CUDA_OK(ctx, k_intt(k, d_items, nullptr, 0, true, y, (size_t)L * N, P->d_rows_in, L, P->d_scale_in, nb));
-    // a3 + a1 (pass 1): ModUp fused into the first NTT pass
-    CUDA_OK(ctx, k_ntt_cols_bconv(k, y, (size_t)L * N, P->d_bc_up, tmp, (size_t)P->n_up * N, P->d_rows_up, P->n_up, nb, L, ctx->lazy_q));
+    // a2 + a1 + a3: inverse row pass of sigma_g(d); then ONE fused column kernel per digit group: inverse column
+    // stages + ModUp scaling of the digit's limbs in shared memory, base conversion and forward column stages per target
+    const bool fused_up = ctx->logN >= 12 && (size_t)(P->n_src_up + 1) * 8192 <= 200 * 1024;
+    if (fused_up) {
+      CUDA_OK(ctx, k_intt_rows_only(k, d_items, nullptr, 0, true, y, (size_t)L * N, P->d_rows_in, L, nb));
+      CUDA_OK(ctx, k_convert_cols(k, y, (size_t)L * N, P->d_groups_up, P->beta, P->n_src_up, P->d_scale_in, P->d_bc_up, P->d_rows_up,
+                                  P->n_up, tmp, (size_t)P->n_up * N, nb, ctx->lazy_q));
+    } else {
+      CUDA_OK(ctx, k_intt(k, d_items, nullptr, 0, true, y, (size_t)L * N, P->d_rows_in, L, P->d_scale_in, nb));
+      CUDA_OK(ctx, k_ntt_cols_bconv(k, y, (size_t)L * N, P->d_bc_up, tmp, (size_t)P->n_up * N, P->d_rows_up, P->n_up, nb, L, ctx->lazy_q));
+    }
     // a1 (pass 2) + a4: evk inner product
     CUDA_OK(ctx, k_ntt_rows_keymac(k, d_items, L, E, P->beta, P->d_tmp_index, tmp, (size_t)P->n_up * N, acc, (size_t)2 * E * N, nb, P->n_up, n_keys));
-    // a5: ModDown = iNTT of the special limbs, conversion fused into pass 1, divide epilogue fused into pass 2
-    CUDA_OK(ctx, k_intt(k, nullptr, acc, (size_t)2 * E * N, false, yP, (size_t)2 * np * N, P->d_rows_p, 2 * np, P->d_scale_p, nb));
-    CUDA_OK(ctx, k_ntt_cols_bconv(k, yP, (size_t)2 * np * N, P->d_bc_down, tmp2, (size_t)2 * L * N, P->d_rows_down, 2 * L, nb, 2 * np, ctx->lazy_p));
+    // a5: ModDown = inverse row pass of the special limbs, fused column kernel per component, divide epilogue in pass 2
+    const bool fused_down = ctx->logN >= 12 && (size_t)(np + 1) * 8192 <= 200 * 1024;
+    if (fused_down) {
+      CUDA_OK(ctx, k_intt_rows_only(k, nullptr, acc, (size_t)2 * E * N, false, yP, (size_t)2 * np * N, P->d_rows_p, 2 * np, nb));
+      CUDA_OK(ctx, k_convert_cols(k, yP, (size_t)2 * np * N, P->d_groups_down, 2, np, P->d_scale_p, P->d_bc_down, P->d_rows_down, 2 * L,
+                                  tmp2, (size_t)2 * L * N, nb, ctx->lazy_p));
+    } else {
+      CUDA_OK(ctx, k_intt(k, nullptr, acc, (size_t)2 * E * N, false, yP, (size_t)2 * np * N, P->d_rows_p, 2 * np, P->d_scale_p, nb));
+      CUDA_OK(ctx, k_ntt_cols_bconv(k, yP, (size_t)2 * np * N, P->d_bc_down, tmp2, (size_t)2 * L * N, P->d_rows_down, 2 * L, nb, 2 * np, ctx->lazy_p));
+    }
     CUDA_OK(ctx, k_ntt_rows_divide(k, d_items, tmp2, (size_t)2 * L * N, acc, (size_t)2 * E * N, false, P->d_mul_pinv, P->d_rows_div, 2 * L, nb));
   }
   return FENC_OK;
@@ -411,8 +435,14 @@ fenc_status rescale_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items) {
     st.add(part);
     const BatchItem *d_items = (const BatchItem *)st.commit();
     if (!d_items) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
-    CUDA_OK(ctx, k_intt(k, d_items, nullptr, 0, false, yR, 2 * N, P->d_rows_rs_in, 2, P->d_scale_rs, nb));
-    CUDA_OK(ctx, k_ntt_cols_bconv(k, yR, 2 * N, P->d_bc_rs, tmp2, (size_t)2 * L1 * N, P->d_rows_rs_up, 2 * L1, nb, 2, ctx->lazy_q));
+    if (ctx->logN >= 12) {
+      CUDA_OK(ctx, k_intt_rows_only(k, d_items, nullptr, 0, false, yR, 2 * N, P->d_rows_rs_in, 2, nb));
+      CUDA_OK(ctx, k_convert_cols(k, yR, 2 * N, P->d_groups_rs, 2, 1, P->d_scale_rs, P->d_bc_rs, P->d_rows_rs_up, 2 * L1, tmp2,
+                                  (size_t)2 * L1 * N, nb, ctx->lazy_q));
+    } else {
+      CUDA_OK(ctx, k_intt(k, d_items, nullptr, 0, false, yR, 2 * N, P->d_rows_rs_in, 2, P->d_scale_rs, nb));
+      CUDA_OK(ctx, k_ntt_cols_bconv(k, yR, 2 * N, P->d_bc_rs, tmp2, (size_t)2 * L1 * N, P->d_rows_rs_up, 2 * L1, nb, 2, ctx->lazy_q));
+    }
     CUDA_OK(ctx, k_ntt_rows_divide(k, d_items, tmp2, (size_t)2 * L1 * N, nullptr, 0, true, P->d_mul_qlinv, P->d_rows_rs_div, 2 * L1, nb));
   }
   return FENC_OK;

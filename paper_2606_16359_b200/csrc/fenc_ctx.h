@@ -32,6 +32,9 @@ struct LevelPlan {
   u64 *d_bc_rs;              // [L-1] 2^64 mod q_t (i.e. "mod t")
   RowDesc *d_rows_rs_div;    // [2(L-1)]
   ShoupC *d_mul_qlinv;       // [A] q_{L-1}^-1 mod q_t
+  // fused column kernel (fenc_ntt.cu convert_cols_kernel): conversion groups per digit / per component
+  ConvGroup *d_groups_up = nullptr, *d_groups_down = nullptr, *d_groups_rs = nullptr;
+  int n_src_up = 0;          // longest digit in use
   // plain transforms of a whole ciphertext [2][L][N]
   RowDesc *d_rows_ct;        // [2L]
   ShoupC *d_scale_ct;        // [2L] N^-1 mod q_t

@@ -165,6 +165,15 @@ DEVI void tile_round_rt(u64 *sm, const TileGeo &G, int pw, int s_lo, int s_hi, c
   for (int k = 0; k < 8; k++) sm[swz(ebase | (k << pw))] = x[k];
 }
 
+// compile-time schedule over active tile bits [LO, LO+NB) of a 2^LT-element tile; picks the lazy forward butterflies
+// for q < 2^58.  Every thread of the block must call this (it synchronises).
+template <bool FWD, int LT, int LO, int NB>
+DEVI void tile_transform_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, int tid) {
+  const u64 q2 = q + q;
+  if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
+  else tile_rounds_ct<FWD, false, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
+}
+
 // GEO selects the schedule: 0 = runtime (any lo/nb), 1 = row pass of 2048-element tiles with 8 stages,
 // 4..8 = column pass with GEO stages over tiles of 2^(GEO+4) elements (16 columns).
 // Every thread of the block must call this (it synchronises).  Outputs: forward < 33q (use fullred), inverse < 2q.

@@ -78,6 +78,12 @@ struct Prof;
 void prof_begin(Prof *p, void *stream, int id, double alg_bytes, double alg_butterflies = 0);
 void prof_end(Prof *p, void *stream);
 
+// one base-conversion group of the fused column kernel: n_src consecutive source rows (row src_row.. of the inverse
+// row-pass output, moduli src_mod.., scaling constants scale[scale_off..]) converted to n_tgt targets rows[tgt_start..]
+struct ConvGroup {
+  int src_row, src_mod, n_src, scale_off, tgt_start, n_tgt, pad[2];
+};
+
 struct KCtx {  // what kernels need from a context
   void *stream;  // cudaStream_t
   NttGeom geom;
@@ -102,6 +108,15 @@ int k_ntt(const KCtx &k, const u64 *src, size_t src_bstride, u64 *dst, size_t ds
 // value = sum_{s < rows[r].aux} y[b][rows[r].src_row + s][.] * bc[rows[r].aux2 + s] (Montgomery constants)
 int k_ntt_cols_bconv(const KCtx &k, const u64 *y, size_t y_bstride, const u64 *bc, u64 *tmp, size_t tmp_bstride,
                      const RowDesc *rows, int n_rows, int n_batch, int n_src_rows, int max_terms);
+// inverse row pass only (pass A): rows land lazily (< 2q) in dst; the column stages follow in k_convert_cols
+int k_intt_rows_only(const KCtx &k, const BatchItem *items, const u64 *src, size_t src_bstride, bool gather, u64 *dst,
+                     size_t dst_bstride, const RowDesc *rows, int n_rows, int n_batch);
+// fused column kernel (needs N >= 2^12): for every group, the inverse column stages + scaling of its source rows (kept
+// in shared memory), then for each target the base conversion and the forward column stages -> tmp rows (lazy).
+// Returns -2 when the group does not fit shared memory (the caller falls back to k_intt + k_ntt_cols_bconv).
+int k_convert_cols(const KCtx &k, u64 *y, size_t y_bstride, const ConvGroup *groups, int n_groups, int n_src_max,
+                   const ShoupC *scale, const u64 *bc, const RowDesc *rows, int n_tgt_total, u64 *tmp, size_t tmp_bstride,
+                   int n_batch, int max_terms);
 // forward pass 2 (row stages) fused with the evaluation-key inner product (a4) over E = L + np target rows.
 // tmp_index[j*E + t] = row of tmp holding digit j / target t, or -1 when t lies in digit j (then the row is
 // items[b].ks_in[t] itself, read through the Galois gather).  acc[b][c][t][N] canonical.

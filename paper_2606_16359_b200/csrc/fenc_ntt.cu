@@ -127,6 +127,119 @@ int k_intt(const KCtx &k, const BatchItem *items, const u64 *src, size_t src_bst
   return 0;
 }
 
+int k_intt_rows_only(const KCtx &k, const BatchItem *items, const u64 *src, size_t src_bstride, bool gather, u64 *dst,
+                     size_t dst_bstride, const RowDesc *rows, int n_rows, int n_batch) {
+  if (n_rows == 0 || n_batch == 0) return 0;
+  cudaStream_t st = (cudaStream_t)k.stream;
+  const NttGeom &g = k.geom;
+  InttRowP a{items, src, src_bstride, dst, dst_bstride, rows, k.d_mods, k.d_tw_inv, g};
+  dim3 gridA(k.N >> g.lt_row, n_rows, n_batch);
+  PROF(k, K_INTT_ROW, 16.0 * k.N * n_rows * n_batch, HALF_N(k) * g.brow * n_rows * n_batch);
+  if (gather) ROW_GEO(g, (intt_rowpass_kernel<true, GEO><<<gridA, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(a)));
+  else ROW_GEO(g, (intt_rowpass_kernel<false, GEO><<<gridA, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(a)));
+  LAUNCH_CHECK(k);
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------------ fused column kernel (a3 / a5 / a8)
+// One block = one column tile (2^BCOL rows x 2^LC columns = 1024 coefficients) of one conversion group of one batch item.
+// The group's source rows arrive from the inverse row pass; their inverse column stages and the scaling
+// N^-1 (Qhat^-1) run here and the resulting coefficient-domain tiles STAY in shared memory while every target row of
+// the group is produced from them: base conversion (R2.6) + forward column stages -> tmp.  Compared with
+// separate kernels this removes the inverse column pass's round trip and the (targets x sources) re-reads of y.
+struct ConvColP {
+  u64 *y; size_t y_bstride; const ConvGroup *groups; const ShoupC *scale; const u64 *bc; const RowDesc *rows;
+  u64 *tmp; size_t tmp_bstride; const ModConst *mods; const ShoupC *tw_fwd; const ShoupC *tw_inv; int logN, brow, max_terms;
+};
+template <int BCOL>
+__global__ void __launch_bounds__(128, 6) convert_cols_kernel(ConvColP p) {
+  constexpr int LT = 10, LC = LT - BCOL, T = 1 << LT, NTH = T / 8;
+  extern __shared__ u64 smem[];
+  const int tid = threadIdx.x, b = blockIdx.z;
+  const ConvGroup cg = p.groups[blockIdx.y];
+  const int N = 1 << p.logN;
+  TileGeo G{LT, LC, p.brow, p.logN, blockIdx.x};
+  u64 *W = smem + (size_t)cg.n_src * T;  // work tile after the source tiles
+  u64 *ybase = p.y + (size_t)b * p.y_bstride;
+  // ---- sources: fill, inverse column stages, scale -> canonical coefficient tiles in shared memory
+  for (int s = 0; s < cg.n_src; s++) {
+    const u64 *src = ybase + (size_t)(cg.src_row + s) * N;
+    tile_fill(smem + (size_t)s * T, T, tid, NTH, [&](int e) { return src[G.gidx(e)]; });
+  }
+  __syncthreads();
+  for (int s = 0; s < cg.n_src; s++) {
+    u64 *Y = smem + (size_t)s * T;
+    const int mod = cg.src_mod + s;
+    const u64 q = p.mods[mod].q;
+    tile_transform_ct<false, LT, LC, BCOL>(Y, G, p.tw_inv + (size_t)mod * N, q, tid);
+    const ShoupC sc = p.scale[cg.scale_off + s];
+#pragma unroll
+    for (int i = 0; i < 8; i++) {
+      const int e = swz(tid + i * NTH);
+      Y[e] = shoup_mul(Y[e], sc.c, sc.cs, q);
+    }
+  }
+  __syncthreads();
+  // ---- targets
+  for (int t = 0; t < cg.n_tgt; t++) {
+    const RowDesc rd = p.rows[cg.tgt_start + t];
+    const ModConst mc = p.mods[rd.mod];
+    const u64 *bc = p.bc + rd.aux2;
+    u64 lo[8], hi[8], r[8];
+#pragma unroll
+    for (int i = 0; i < 8; i++) lo[i] = hi[i] = r[i] = 0;
+    int lazy = 0;
+    for (int s = 0; s < cg.n_src; s++) {
+      const u64 c = __ldg(bc + s);
+      const u64 *Y = smem + (size_t)s * T;
+#pragma unroll
+      for (int i = 0; i < 8; i++) mac128(lo[i], hi[i], Y[swz(tid + i * NTH)], c);
+      if (++lazy == p.max_terms) {
+#pragma unroll
+        for (int i = 0; i < 8; i++) r[i] = addmod(r[i], mont_redc(lo[i], hi[i], mc.q, mc.qinv_neg), mc.q), lo[i] = hi[i] = 0;
+        lazy = 0;
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < 8; i++) W[swz(tid + i * NTH)] = addmod(r[i], mont_redc(lo[i], hi[i], mc.q, mc.qinv_neg), mc.q);
+    __syncthreads();
+    tile_transform_ct<true, LT, LC, BCOL>(W, G, p.tw_fwd + (size_t)rd.mod * N, mc.q, tid);
+    u64 *dst = p.tmp + (size_t)b * p.tmp_bstride + (size_t)rd.dst_row * N;
+    tile_drain(W, T, tid, NTH, [&](int e, u64 v) { dst[G.gidx(e)] = v; });  // lazy, below 33q
+    __syncthreads();
+  }
+}
+
+int k_convert_cols(const KCtx &k, u64 *y, size_t y_bstride, const ConvGroup *groups, int n_groups, int n_src_max,
+                   const ShoupC *scale, const u64 *bc, const RowDesc *rows, int n_tgt_total, u64 *tmp, size_t tmp_bstride,
+                   int n_batch, int max_terms) {
+  if (n_groups == 0 || n_batch == 0) return 0;
+  const NttGeom &g = k.geom;
+  if (g.logN < 12) return -2;
+  const size_t smem = (size_t)(n_src_max + 1) * 1024 * sizeof(u64);
+  if (smem > 200 * 1024) return -2;
+  ConvColP p{y, y_bstride, groups, scale, bc, rows, tmp, tmp_bstride, k.d_mods, k.d_tw_fwd, k.d_tw_inv, g.logN, g.brow, max_terms};
+  dim3 grid(k.N >> 10, n_groups, n_batch);
+  // algorithmic bytes: every target row written once (+ the sources, counted by the caller's row pass); butterflies of
+  // the forward column stages of every target (the inverse ones of the sources are the smaller part)
+  PROF(k, K_NTT_COL_BCONV, 8.0 * k.N * n_batch * (double)n_tgt_total, HALF_N(k) * g.bcol * (double)n_tgt_total * n_batch);
+#define LAUNCH_CONV(B)                                                                                                          \
+  do {                                                                                                                          \
+    if (smem > 48 * 1024) cudaFuncSetAttribute(convert_cols_kernel<B>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+    convert_cols_kernel<B><<<grid, 128, smem, (cudaStream_t)k.stream>>>(p);                                                     \
+  } while (0)
+  switch (g.bcol) {
+    case 4: LAUNCH_CONV(4); break;
+    case 5: LAUNCH_CONV(5); break;
+    case 6: LAUNCH_CONV(6); break;
+    case 7: LAUNCH_CONV(7); break;
+    default: LAUNCH_CONV(8); break;
+  }
+#undef LAUNCH_CONV
+  LAUNCH_CHECK(k);
+  return 0;
+}
+
 // ------------------------------------------------------------------------------------------------ forward, pass 1
 struct NttColP {
   const u64 *src; size_t src_bstride; const u64 *bc; u64 *dst; size_t dst_bstride;
