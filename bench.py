@@ -254,6 +254,12 @@ def run_ours(args, rank, world):
     else:
         roofline = {"bound": "hbm", "kernel": top, "achieved": round(hbm_ach, 1), "peak": peaks["hbm_gbs"], "unit": "GB/s",
                     "frac": round(hbm_ach / peaks["hbm_gbs"], 4), "traffic": None, "peak_source": peak_src}
+    tpath = os.path.join(ROOT, "profiles", "r01_ncu_traffic.json")  # DRAM bytes per launch from the committed ncu capture
+    if os.path.exists(tpath):
+        tj = json.load(open(tpath))
+        if tj.get("workload") == args.workload and tj.get("batch") == args.batch:
+            roofline["traffic"] = tj["dram_bytes_per_launch"].get(top)
+            roofline["traffic_source"] = tj["source"]
     roofline.update({"avg_launch_us": round(t_ms * 1e3 / t_cnt, 2), "share_of_step": round(t_ms / tot, 4),
                      "alg_bytes_per_launch": t_bytes / t_cnt, "per_kernel": per_kernel, "profiled_step_ms": round(prof_ms, 3),
                      "hbm_peak_GBps": peaks["hbm_gbs"], "hbm_peak_source": peak_src})
