@@ -119,6 +119,7 @@ WORKLOADS = {
     "cfg3_conv_32_64_s2": ("cfg3", lambda bs, seed: conv_layers("resnet_32_64_s2", seed, True),
                            "BASELINE config 3: ResNet-20 3x3 32->64 stride 2, N=2^16, batch 1"),
     "cfg5_rotsweep": (None, None, "BASELINE config 5: rotation / key-switch sweep"),
+    "cfg3_compress": (None, None, "AAC compress micro-benchmark at config 3's parameters"),
 }
 DEFAULT_WORKLOAD = "cfg2_lenet5"
 
@@ -176,6 +177,54 @@ def run_rotsweep(args):
             "config": {"workload": "cfg5_rotsweep", "description": "BASELINE config 5: N=2^16, 64 cts x 32 amounts per point; "
                        "value quoted at L=24, dnum=3", "peak_source": peak_src, "hbm_peak_GBps": peaks["hbm_gbs"]},
             "points": points}
+
+
+def run_compress(args):
+    """AAC compress micro-benchmark (Table X shapes): BG sparse ciphertexts whose valid
+    channel positions are [0, v) of ch are merged into BG*v/ch dense ones (canonical batch-group compaction, R2.11),
+    maskless and masked split-scale, at config 3's parameters."""
+    import torch
+    import paper_2606_16359_b200 as fenc
+    ctx = fenc.Context(**wl.PARAMS["cfg3"])
+    n, L = ctx.n, ctx.n_q
+    rows = []
+    rng = np.random.default_rng(77)
+    for ch, v, n_src in ((8, 2, 4), (32, 8, 64), (32, 2, 64), (128, 8, 64)):
+        cs, per = n // ch, ch // v
+        terms = [(i // per, i, (n - (i % per) * v * cs) % n) for i in range(n_src)]
+        n_out = -(-n_src // per)
+        steps = sorted({r for _, _, r in terms if r})
+        keys = ctx.keygen(9, steps)
+        srcs = []
+        for i in range(n_src):
+            z = np.zeros(n)
+            z[: v * cs] = rng.uniform(-1, 1, v * cs)
+            srcs.append(ctx.encrypt(keys, ctx.encode_slots(z, L), 400 + i))
+        m = np.zeros(n)
+        m[: v * cs] = 1.0
+        mask = ctx.encode_slots(m, L, float(ctx.q[L - 1]))
+        for mode in ("maskless", "masked_split_scale"):
+            kw = dict(mask=mask, do_rescale=True) if mode != "maskless" else {}
+            for _ in range(3):
+                ctx.compress(keys, srcs, terms, n_out, **kw)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(args.steps):
+                out = ctx.compress(keys, srcs, terms, n_out, **kw)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / args.steps
+            rows.append({"ch": ch, "valid": v, "sources": n_src, "outputs": n_out, "mode": mode, "rotations": len([t for t in terms if t[2]]),
+                         "ms": round(ms, 3), "rot_per_s": round(len([t for t in terms if t[2]]) / (ms * 1e-3), 1),
+                         "slot_util_before": v / ch, "slot_util_after": min(1.0, n_src * v / (ch * n_out)), "level_out": out[0].L})
+        del srcs, keys
+    ctx.close()
+    ref = rows[2]
+    return {"metric": METRIC, "value": ref["rot_per_s"], "unit": "key-switched rotations/s", "n_gpus": 1, "steps": args.steps, "warmup": 3,
+            "ms_per_step": ref["ms"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+            "config": {"workload": "cfg3_compress", "description": "AAC compress (fenc_compress) on bottleneck-shaped sources, N=2^16, "
+                       "24x50b+4x60b; value quoted for ch=32, v=8, 64 sources, maskless"}, "points": rows}
 
 
 def run_ours(args, rank, world):
@@ -440,7 +489,12 @@ def main():
         import torch
         torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", 0)))
         torch.distributed.init_process_group("nccl")
-    line = run_rotsweep(args) if args.workload == "cfg5_rotsweep" else run_ours(args, rank, world)
+    if args.workload == "cfg5_rotsweep":
+        line = run_rotsweep(args)
+    elif args.workload == "cfg3_compress":
+        line = run_compress(args)
+    else:
+        line = run_ours(args, rank, world)
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:
