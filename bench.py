@@ -52,7 +52,11 @@ class ClockSampler:
         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
 
     def __init__(self, device):
-        self.rows, self.proc, self.device = [], None, device
+        self.rows, self.proc, self.device, self.first = [], None, device, 0
+
+    def mark(self):
+        """samples from here on belong to the timed region"""
+        self.first = len(self.rows)
 
     def start(self):
         try:
@@ -68,7 +72,10 @@ class ClockSampler:
 
     def stop(self):
         if self.proc:
+            time.sleep(0.12)  # let the last sample of the timed region arrive
             self.proc.terminate()
+        if len(self.rows) > self.first:
+            self.rows = self.rows[self.first:]
         sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
         mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
@@ -250,11 +257,17 @@ def run_ours(args, rank, world):
             torch.distributed.barrier()
         torch.cuda.synchronize()
 
+    # the clock sampler starts BEFORE the warm-up (nvidia-smi's start-up would otherwise perturb the timed steps) and keeps
+    # sampling through the timed region; only samples taken inside the timed region are reported
+    sampler = ClockSampler(dev)
+    sampler.start()
+    t_wait = time.time()
+    while not sampler.rows and time.time() - t_wait < 3.0:
+        time.sleep(0.05)
     for _ in range(args.warmup):
         pipe.forward(cts)
     barrier()
-    sampler = ClockSampler(dev)
-    sampler.start()
+    sampler.mark()
     ctx.launch_count(reset=True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     if args.profile_range:  # for `ncu --profile-from-start off`: only the timed steps are captured
