@@ -2,7 +2,8 @@
 //
 // Arithmetic: 64-bit words on the 32-bit integer pipes (IMAD.WIDE on the fma pipe, IADD3/LOP3 on the alu pipe).
 //  - constant operands (twiddles, scaling constants): Shoup multiplication with a precomputed floor(c 2^64 / q),
-//    Harvey lazy butterflies with values in [0,4q) (forward) / [0,2q) (inverse); needs q < 2^62.
+//    lazy butterflies: forward values grow by at most 2q per stage without any correction for q < 2^58 (one
+//    full reduction at the end), Harvey's [0,4q) form for larger q; inverse values stay in [0,2q); needs q < 2^61.
 //  - variable x variable sums (evk inner product, plaintext MAC, base conversion): 128-bit lazy accumulation of
 //    x * y_mont products followed by ONE Montgomery reduction (y stored as y 2^64 mod q).
 #pragma once

@@ -95,7 +95,7 @@ struct KCtx {  // what kernels need from a context
   Prof *prof;              // NULL unless profiling is enabled
 };
 
-// ---------------------------------------------------------------- launchers (fenc_kernels.cu); return cudaError_t
+// ---------------------------------------------------------------- launchers (fenc_ntt.cu, fenc_elem.cu); return cudaError_t (0 = ok)
 // inverse NTT (both passes).  Source row r of batch b: (items ? items[b].ks_in : src + b*src_bstride) +
 // rows[r].src_row*N, read through the Galois gather of items[b].g when gather.  Result: coefficient domain,
 // canonical, times scale[r], at dst + b*dst_bstride + rows[r].dst_row*N.

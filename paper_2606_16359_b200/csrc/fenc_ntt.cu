@@ -6,7 +6,9 @@
 //   forward = column pass (the bcol high stages, stride 2^brow) then row pass (the brow low stages, contiguous);
 //   inverse = row pass then column pass.
 // Each pass: coalesced tile load -> radix-8 register rounds through swizzled shared memory -> coalesced store.
-// The first touch of a forward transform and the last touch of either direction carry the fused work.
+// The first touch of a forward transform and the last touch of either direction carry the fused work; for ring degrees
+// >= 2^12 the inverse column pass, the base conversion and the forward column pass of a key switch are ONE kernel
+// (convert_cols_kernel) that keeps the converted limbs in shared memory.
 #include "fenc_device.cuh"
 
 // geometry dispatch: row kernels GEO in {0,1}; column kernels GEO in {0,4..8} (fenc_device.cuh tile_transform)
