@@ -326,7 +326,9 @@ def run_ours(args, rank, world):
                      "alg_bytes_per_launch": t_bytes / t_cnt, "per_kernel": per_kernel, "profiled_step_ms": round(prof_ms, 3),
                      "hbm_peak_GBps": peaks["hbm_gbs"], "hbm_peak_source": peak_src})
     # ---- end to end through the C ABI with host buffers: import (H2D + NTT), forward, export (iNTT + D2H)
-    host_in = [ctx.ct_export(c) for c in cts]
+    # host buffers in pinned memory (torch owns them; numpy views are what the C ABI receives)
+    pinned = [torch.from_numpy(ctx.ct_export(c).view(np.int64)).pin_memory() for c in cts]
+    host_in = [t.numpy().view(np.uint64) for t in pinned]
     s_in = cts[0].scale
     h2d = sum(a.nbytes for a in host_in)
     d2h = 0
