@@ -343,6 +343,31 @@ LevelPlan *get_plan(fenc_ctx *ctx, int L) {
         rs_div.push_back(RowDesc{t, c * L1 + t, c * L1 + t, c, c * L + t, {0, 0, 0}});
       }
   }
+  if (L >= 2) {
+    std::vector<RowDesc> rows_p2, rows_down2, rows_div2;
+    std::vector<ShoupC> scale_p2;
+    std::vector<ConvGroup> groups_down2;
+    for (int c = 0; c < 2; c++) {
+      for (int i = 0; i < np; i++) {
+        RowDesc rd = rows_p[c * np + i];
+        rd.dst_row = c * (np + 1) + i;
+        rows_p2.push_back(rd);
+        scale_p2.push_back(scale_p[c * np + i]);
+      }
+      rows_p2.push_back(RowDesc{L1, c * E + L1, c * (np + 1) + np, 1, c, {0, 0, 0}});
+      scale_p2.push_back(rs_scale[c]);
+      groups_down2.push_back(ConvGroup{c * (np + 1), nq, np + 1, c * (np + 1), c * L1, L1, {1, L1}});
+      for (int t = 0; t < L1; t++) {
+        rows_down2.push_back(RowDesc{t, c * (np + 1), c * L1 + t, np, t * np, {0, 0, 0}});
+        rows_div2.push_back(RowDesc{t, c * L1 + t, c * L1 + t, c, c * E + t, {0, 0, 0}});
+      }
+    }
+    P.d_rows_p2 = upload_owned(ctx, P.owned, rows_p2);
+    P.d_scale_p2 = upload_owned(ctx, P.owned, scale_p2);
+    P.d_groups_down2 = upload_owned(ctx, P.owned, groups_down2);
+    P.d_rows_down2 = upload_owned(ctx, P.owned, rows_down2);
+    P.d_rows_div2 = upload_owned(ctx, P.owned, rows_div2);
+  }
   P.d_rows_rs_in = upload_owned(ctx, P.owned, rs_in);
   P.d_scale_rs = upload_owned(ctx, P.owned, rs_scale);
   P.d_rows_rs_up = upload_owned(ctx, P.owned, rs_up);
@@ -360,20 +385,25 @@ LevelPlan *get_plan(fenc_ctx *ctx, int L) {
 // ------------------------------------------------------------------------------------------------ batched key switch
 static const size_t WS_CAP = (size_t)6 << 30;  // workspace budget for one chunk of a batch
 
-fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items) {
+bool ks_can_merge_rescale(const fenc_ctx *ctx, int L) {
+  return L >= 2 && ctx->logN >= 12 && (size_t)(ctx->np + 2) * 8192 <= 200 * 1024;
+}
+
+fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items, bool rescale_after) {
   if (items.empty()) return FENC_OK;
+  if (rescale_after && !ks_can_merge_rescale(ctx, L)) return fail(ctx, FENC_ERR_INVALID_ARG, "merged rescale unavailable here");
   LevelPlan *P = get_plan(ctx, L);
   if (!P) return fail(ctx, FENC_ERR_OOM, "level plan");
   const size_t N = ctx->N;
-  const int E = P->E, np = ctx->np;
-  const size_t per = ((size_t)L + P->n_up + 2 * E + 2 * np + 2 * L) * N;  // u64 per item
+  const int E = P->E, np = ctx->np, npy = rescale_after ? ctx->np + 1 : ctx->np;
+  const size_t per = ((size_t)L + P->n_up + 2 * E + 2 * npy + 2 * L) * N;  // u64 per item
   size_t chunk = WS_CAP / (per * 8);
   if (chunk < 1) chunk = 1;
   if (chunk > items.size()) chunk = items.size();
   u64 *ws = (u64 *)workspace(ctx, chunk * per * 8);
   if (!ws) return fail(ctx, FENC_ERR_OOM, "key-switch workspace (%zu bytes)", chunk * per * 8);
   u64 *y = ws, *tmp = y + chunk * L * N, *acc = tmp + chunk * P->n_up * N, *yP = acc + chunk * 2 * E * N,
-      *tmp2 = yP + chunk * 2 * np * N;
+      *tmp2 = yP + chunk * 2 * npy * N;
   const KCtx &k = ctx->k;
   for (size_t at = 0; at < items.size(); at += chunk) {
     const int nb = (int)std::min(chunk, items.size() - at);
@@ -399,6 +429,18 @@ fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items) {
     }
     // a1 (pass 2) + a4: evk inner product
     CUDA_OK(ctx, k_ntt_rows_keymac(k, d_items, L, E, P->beta, P->d_tmp_index, tmp, (size_t)P->n_up * N, acc, (size_t)2 * E * N, nb, P->n_up, n_keys));
+    if (rescale_after) {
+      // a5 + a8 merged: the limb the rescale drops is inverse-transformed with the special limbs; one column kernel and
+      // one divide epilogue produce the rescaled ciphertext directly
+      const int L1 = L - 1;
+      CUDA_OK(ctx, k_intt_rows_only(k, d_items, acc, (size_t)2 * E * N, false, yP, (size_t)2 * npy * N, P->d_rows_p2, 2 * npy, nb,
+                                    P->d_mul_pinv));
+      CUDA_OK(ctx, k_convert_cols(k, yP, (size_t)2 * npy * N, P->d_groups_down2, 2, npy, P->d_scale_p2, P->d_bc_down, P->d_rows_down2,
+                                  2 * L1, tmp2, (size_t)2 * L1 * N, nb, ctx->lazy_p, P->d_mul_pinv));
+      CUDA_OK(ctx, k_ntt_rows_divide(k, d_items, tmp2, (size_t)2 * L1 * N, acc, (size_t)2 * E * N, false, P->d_mul_qlinv,
+                                     P->d_rows_div2, 2 * L1, nb, P->d_mul_pinv));
+      continue;
+    }
     // a5: ModDown = inverse row pass of the special limbs, fused column kernel per component, divide epilogue in pass 2
     const bool fused_down = ctx->logN >= 12 && (size_t)(np + 1) * 8192 <= 200 * 1024;
     if (fused_down) {

@@ -32,6 +32,13 @@ struct LevelPlan {
   u64 *d_bc_rs;              // [L-1] 2^64 mod q_t (i.e. "mod t")
   RowDesc *d_rows_rs_div;    // [2(L-1)]
   ShoupC *d_mul_qlinv;       // [A] q_{L-1}^-1 mod q_t
+  // ModDown merged with the rescale that follows a relinearisation (bit-identical to the two in turn):
+  // the dropped limb l = L-1 joins the special limbs in the inverse pass and the column kernel, targets are t < L-1
+  RowDesc *d_rows_p2 = nullptr;     // [2 (np+1)] special limbs + the combined limb l (aux = 1, aux2 = component)
+  ShoupC *d_scale_p2 = nullptr;     // [2 (np+1)]
+  ConvGroup *d_groups_down2 = nullptr;  // [2], pad = {1, l}
+  RowDesc *d_rows_down2 = nullptr;  // [2 (L-1)]
+  RowDesc *d_rows_div2 = nullptr;   // [2 (L-1)]
   // fused column kernel (fenc_ntt.cu convert_cols_kernel): conversion groups per digit / per component
   ConvGroup *d_groups_up = nullptr, *d_groups_down = nullptr, *d_groups_rs = nullptr;
   int n_src_up = 0;          // longest digit in use
@@ -176,7 +183,9 @@ struct Scope {
   }
 };
 // batched key switch over items (all at level L): out = (ModDown(acc_0) + add0, ModDown(acc_1) + add1)
-fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items);
+// rescale_after: the rescale is merged into the ModDown (needs both addends, g = 1, N >= 2^12): out is [2][L-1][N]
+fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items, bool rescale_after = false);
+bool ks_can_merge_rescale(const fenc_ctx *ctx, int L);
 // batched rescale: items[i].sub_in = input ct [2][L][N], items[i].out = [2][L-1][N]
 fenc_status rescale_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items);
 // rotation items for (in, step) pairs; step 0 handled by a device copy

@@ -110,13 +110,17 @@ int k_ntt_cols_bconv(const KCtx &k, const u64 *y, size_t y_bstride, const u64 *b
                      const RowDesc *rows, int n_rows, int n_batch, int n_src_rows, int max_terms);
 // inverse row pass only (pass A): rows land lazily (< 2q) in dst; the column stages follow in k_convert_cols
 int k_intt_rows_only(const KCtx &k, const BatchItem *items, const u64 *src, size_t src_bstride, bool gather, u64 *dst,
-                     size_t dst_bstride, const RowDesc *rows, int n_rows, int n_batch);
+                     size_t dst_bstride, const RowDesc *rows, int n_rows, int n_batch, const ShoupC *comb_mul = nullptr);
+// (comb_mul != nullptr: merged ModDown + rescale -- rows with aux = 1 read src * comb_mul[mod] + items[b].add{aux2}[mod],
+//  all rows come from src, never through the gather)
 // fused column kernel (needs N >= 2^12): for every group, the inverse column stages + scaling of its source rows (kept
 // in shared memory), then for each target the base conversion and the forward column stages -> tmp rows (lazy).
 // Returns -2 when the group does not fit shared memory (the caller falls back to k_intt + k_ntt_cols_bconv).
 int k_convert_cols(const KCtx &k, u64 *y, size_t y_bstride, const ConvGroup *groups, int n_groups, int n_src_max,
                    const ShoupC *scale, const u64 *bc, const RowDesc *rows, int n_tgt_total, u64 *tmp, size_t tmp_bstride,
-                   int n_batch, int max_terms);
+                   int n_batch, int max_terms, const ShoupC *merged_pinv = nullptr);
+// (merged_pinv != nullptr: ModDown merged with the rescale; every group carries one extra source row, the inverse-
+//  transformed dropped limb of modulus index groups[g].pad[1], and the targets receive V_t P^-1 + (out_l mod t))
 // forward pass 2 (row stages) fused with the evaluation-key inner product (a4) over E = L + np target rows.
 // tmp_index[j*E + t] = row of tmp holding digit j / target t, or -1 when t lies in digit j (then the row is
 // items[b].ks_in[t] itself, read through the Galois gather).  acc[b][c][t][N] canonical.
@@ -127,7 +131,8 @@ int k_ntt_rows_keymac(const KCtx &k, const BatchItem *items, int L, int E, int b
 // minuend = from_items ? items[b].sub_in : acc + b*acc_bstride
 int k_ntt_rows_divide(const KCtx &k, const BatchItem *items, const u64 *tmp, size_t tmp_bstride, const u64 *acc,
                       size_t acc_bstride, bool minuend_from_items, const ShoupC *mul, const RowDesc *rows, int n_rows,
-                      int n_batch);
+                      int n_batch, const ShoupC *merged_mul2 = nullptr);
+// (merged_mul2 != nullptr: out = ((minuend * merged_mul2[mod] + addend) - X) * mul[mod], the ModDown + rescale merge)
 // MAC (a7) over groups of outputs sharing one ciphertext sequence (register tiling, fenc_elem.cu):
 // out[out_start+i] = sum_{t<n_terms} ct[ct_start+t] (*) pt[pt_start + i*n_terms + t], i < n_out <= FENC_MAC_GROUP
 int k_mac(const KCtx &k, const MacGroup *groups, int n_groups, int max_group, const u64 *const *term_ct, const u64 *const *term_pt,

@@ -67,23 +67,33 @@ static inline int nthreads_for(int lt) { int t = 1 << (lt - 3); return t < 32 ? 
 struct InttRowP {
   const BatchItem *items; const u64 *src; size_t src_bstride; u64 *dst; size_t dst_bstride;
   const RowDesc *rows; const ModConst *mods; const ShoupC *tw; NttGeom g;
+  const ShoupC *comb_mul;  // COMB: rows with aux = 1 read src * comb_mul[mod] + items[b].add{aux2}[mod] (merged rescale)
 };
-template <bool GATHER, int GEO>
+template <bool GATHER, int GEO, bool COMB = false>
 __global__ void __launch_bounds__(256, 5) intt_rowpass_kernel(InttRowP p) {
   extern __shared__ u64 sm[];
   const int tid = threadIdx.x, b = blockIdx.z;
   const RowDesc rd = p.rows[blockIdx.y];
   const int N = 1 << p.g.logN, T = 1 << p.g.lt_row;
   TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, blockIdx.x};
-  const u64 *src = (p.items ? p.items[b].ks_in : p.src + (size_t)b * p.src_bstride) + (size_t)rd.src_row * N;
+  const u64 *src = ((p.items && !COMB) ? p.items[b].ks_in : p.src + (size_t)b * p.src_bstride) + (size_t)rd.src_row * N;
   const u32 gal = GATHER ? p.items[b].g : 1u;
   const int logN = p.g.logN, nth = blockDim.x;
-  tile_fill(sm, T, tid, nth, [&](int e) {
-    const u32 j = G.gidx(e);
-    return __ldg(src + (GATHER ? galois_src(j, gal, logN) : j));
-  });
-  __syncthreads();
   const u64 q = p.mods[rd.mod].q;
+  if (COMB && rd.aux) {
+    const u64 *add = (rd.aux2 == 0 ? p.items[b].add0 : p.items[b].add1) + (size_t)rd.mod * N;
+    const ShoupC mc = p.comb_mul[rd.mod];
+    tile_fill(sm, T, tid, nth, [&](int e) {
+      const u32 j = G.gidx(e);
+      return addmod(shoup_mul(__ldg(src + j), mc.c, mc.cs, q), __ldg(add + j), q);
+    });
+  } else {
+    tile_fill(sm, T, tid, nth, [&](int e) {
+      const u32 j = G.gidx(e);
+      return __ldg(src + (GATHER ? galois_src(j, gal, logN) : j));
+    });
+  }
+  __syncthreads();
   tile_transform<false, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid);
   u64 *dst = p.dst + (size_t)b * p.dst_bstride + (size_t)rd.dst_row * N;
   tile_drain(sm, T, tid, nth, [&](int e, u64 v) { dst[G.gidx(e)] = v; });
@@ -115,7 +125,7 @@ int k_intt(const KCtx &k, const BatchItem *items, const u64 *src, size_t src_bst
   if (n_rows == 0 || n_batch == 0) return 0;
   cudaStream_t st = (cudaStream_t)k.stream;
   const NttGeom &g = k.geom;
-  InttRowP a{items, src, src_bstride, dst, dst_bstride, rows, k.d_mods, k.d_tw_inv, g};
+  InttRowP a{items, src, src_bstride, dst, dst_bstride, rows, k.d_mods, k.d_tw_inv, g, nullptr};
   dim3 gridA(k.N >> g.lt_row, n_rows, n_batch);
   PROF(k, K_INTT_ROW, 16.0 * k.N * n_rows * n_batch, HALF_N(k) * g.brow * n_rows * n_batch);
   if (gather) ROW_GEO(g, (intt_rowpass_kernel<true, GEO><<<gridA, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(a)));
@@ -130,14 +140,15 @@ int k_intt(const KCtx &k, const BatchItem *items, const u64 *src, size_t src_bst
 }
 
 int k_intt_rows_only(const KCtx &k, const BatchItem *items, const u64 *src, size_t src_bstride, bool gather, u64 *dst,
-                     size_t dst_bstride, const RowDesc *rows, int n_rows, int n_batch) {
+                     size_t dst_bstride, const RowDesc *rows, int n_rows, int n_batch, const ShoupC *comb_mul) {
   if (n_rows == 0 || n_batch == 0) return 0;
   cudaStream_t st = (cudaStream_t)k.stream;
   const NttGeom &g = k.geom;
-  InttRowP a{items, src, src_bstride, dst, dst_bstride, rows, k.d_mods, k.d_tw_inv, g};
+  InttRowP a{items, src, src_bstride, dst, dst_bstride, rows, k.d_mods, k.d_tw_inv, g, comb_mul};
   dim3 gridA(k.N >> g.lt_row, n_rows, n_batch);
   PROF(k, K_INTT_ROW, 16.0 * k.N * n_rows * n_batch, HALF_N(k) * g.brow * n_rows * n_batch);
-  if (gather) ROW_GEO(g, (intt_rowpass_kernel<true, GEO><<<gridA, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(a)));
+  if (comb_mul) ROW_GEO(g, (intt_rowpass_kernel<false, GEO, true><<<gridA, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(a)));
+  else if (gather) ROW_GEO(g, (intt_rowpass_kernel<true, GEO><<<gridA, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(a)));
   else ROW_GEO(g, (intt_rowpass_kernel<false, GEO><<<gridA, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(a)));
   LAUNCH_CHECK(k);
   return 0;
@@ -152,8 +163,34 @@ int k_intt_rows_only(const KCtx &k, const BatchItem *items, const u64 *src, size
 struct ConvColP {
   u64 *y; size_t y_bstride; const ConvGroup *groups; const ShoupC *scale; const u64 *bc; const RowDesc *rows;
   u64 *tmp; size_t tmp_bstride; const ModConst *mods; const ShoupC *tw_fwd; const ShoupC *tw_inv; int logN, brow, max_terms;
+  const ShoupC *mulc;  // MERGED: P^-1 mod q_t
 };
-template <int BCOL>
+// sum over the first n source tiles of Y_s[e] * bc[s] for this thread's eight elements, Montgomery-reduced: canonical
+template <int T, int NTH>
+DEVI void conv_dot(const u64 *smem, int n, const u64 *bc, const ModConst &mc, int max_terms, int tid, u64 (&out)[8]) {
+  u64 lo[8], hi[8], r[8];
+#pragma unroll
+  for (int i = 0; i < 8; i++) lo[i] = hi[i] = r[i] = 0;
+  int lazy = 0;
+  for (int s = 0; s < n; s++) {
+    const u64 c = __ldg(bc + s);
+    const u64 *Y = smem + (size_t)s * T;
+#pragma unroll
+    for (int i = 0; i < 8; i++) mac128(lo[i], hi[i], Y[swz(tid + i * NTH)], c);
+    if (++lazy == max_terms) {
+#pragma unroll
+      for (int i = 0; i < 8; i++) r[i] = addmod(r[i], mont_redc(lo[i], hi[i], mc.q, mc.qinv_neg), mc.q), lo[i] = hi[i] = 0;
+      lazy = 0;
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < 8; i++) out[i] = addmod(r[i], mont_redc(lo[i], hi[i], mc.q, mc.qinv_neg), mc.q);
+}
+// MERGED (ModDown followed by the rescale): the group's last source tile is Z = iNTT(acc[l] P^-1 + add[l]) of
+// the limb l = q_{L-1} that the rescale drops (modulus index cg.pad[1]).  With V_t = sum_i y_i (Phat_i mod t):
+//   out_l = Z - V_l P^-1 mod q_l        (the key-switched limb l in the coefficient domain, canonical)
+//   u_t   = V_t P^-1 + (out_l mod t)    (what the divide epilogue subtracts:  c'_t = (acc_t P^-1 + add_t - NTT(u_t)) q_l^-1)
+template <int BCOL, bool MERGED>
 __global__ void __launch_bounds__(128, 6) convert_cols_kernel(ConvColP p) {
   constexpr int LT = 10, LC = LT - BCOL, T = 1 << LT, NTH = T / 8;
   extern __shared__ u64 smem[];
@@ -163,6 +200,7 @@ __global__ void __launch_bounds__(128, 6) convert_cols_kernel(ConvColP p) {
   TileGeo G{LT, LC, p.brow, p.logN, blockIdx.x};
   u64 *W = smem + (size_t)cg.n_src * T;  // work tile after the source tiles
   u64 *ybase = p.y + (size_t)b * p.y_bstride;
+  const int n_conv = MERGED ? cg.n_src - 1 : cg.n_src;  // tiles entering the base conversion
   // ---- sources: fill, inverse column stages, scale -> canonical coefficient tiles in shared memory
   for (int s = 0; s < cg.n_src; s++) {
     const u64 *src = ybase + (size_t)(cg.src_row + s) * N;
@@ -171,7 +209,7 @@ __global__ void __launch_bounds__(128, 6) convert_cols_kernel(ConvColP p) {
   __syncthreads();
   for (int s = 0; s < cg.n_src; s++) {
     u64 *Y = smem + (size_t)s * T;
-    const int mod = cg.src_mod + s;
+    const int mod = (MERGED && s == n_conv) ? cg.pad[1] : cg.src_mod + s;
     const u64 q = p.mods[mod].q;
     tile_transform_ct<false, LT, LC, BCOL>(Y, G, p.tw_inv + (size_t)mod * N, q, tid);
     const ShoupC sc = p.scale[cg.scale_off + s];
@@ -182,28 +220,30 @@ __global__ void __launch_bounds__(128, 6) convert_cols_kernel(ConvColP p) {
     }
   }
   __syncthreads();
+  u64 outl[8];
+  if (MERGED) {
+    const int l = cg.pad[1];
+    const ModConst ml = p.mods[l];
+    const ShoupC pl = p.mulc[l];
+    u64 v[8];
+    conv_dot<T, NTH>(smem, n_conv, p.bc + (size_t)l * n_conv, ml, p.max_terms, tid, v);
+    const u64 *Z = smem + (size_t)n_conv * T;
+#pragma unroll
+    for (int i = 0; i < 8; i++) outl[i] = submod(Z[swz(tid + i * NTH)], shoup_mul(v[i], pl.c, pl.cs, ml.q), ml.q);
+  }
   // ---- targets
   for (int t = 0; t < cg.n_tgt; t++) {
     const RowDesc rd = p.rows[cg.tgt_start + t];
     const ModConst mc = p.mods[rd.mod];
-    const u64 *bc = p.bc + rd.aux2;
-    u64 lo[8], hi[8], r[8];
+    u64 v[8];
+    conv_dot<T, NTH>(smem, n_conv, p.bc + rd.aux2, mc, p.max_terms, tid, v);
+    if (MERGED) {
+      const ShoupC pt = p.mulc[rd.mod];
 #pragma unroll
-    for (int i = 0; i < 8; i++) lo[i] = hi[i] = r[i] = 0;
-    int lazy = 0;
-    for (int s = 0; s < cg.n_src; s++) {
-      const u64 c = __ldg(bc + s);
-      const u64 *Y = smem + (size_t)s * T;
-#pragma unroll
-      for (int i = 0; i < 8; i++) mac128(lo[i], hi[i], Y[swz(tid + i * NTH)], c);
-      if (++lazy == p.max_terms) {
-#pragma unroll
-        for (int i = 0; i < 8; i++) r[i] = addmod(r[i], mont_redc(lo[i], hi[i], mc.q, mc.qinv_neg), mc.q), lo[i] = hi[i] = 0;
-        lazy = 0;
-      }
+      for (int i = 0; i < 8; i++) v[i] = addmod(shoup_mul(v[i], pt.c, pt.cs, mc.q), fullred(outl[i], mc.q, mc.qbar), mc.q);
     }
 #pragma unroll
-    for (int i = 0; i < 8; i++) W[swz(tid + i * NTH)] = addmod(r[i], mont_redc(lo[i], hi[i], mc.q, mc.qinv_neg), mc.q);
+    for (int i = 0; i < 8; i++) W[swz(tid + i * NTH)] = v[i];
     __syncthreads();
     tile_transform_ct<true, LT, LC, BCOL>(W, G, p.tw_fwd + (size_t)rd.mod * N, mc.q, tid);
     u64 *dst = p.tmp + (size_t)b * p.tmp_bstride + (size_t)rd.dst_row * N;
@@ -214,21 +254,27 @@ __global__ void __launch_bounds__(128, 6) convert_cols_kernel(ConvColP p) {
 
 int k_convert_cols(const KCtx &k, u64 *y, size_t y_bstride, const ConvGroup *groups, int n_groups, int n_src_max,
                    const ShoupC *scale, const u64 *bc, const RowDesc *rows, int n_tgt_total, u64 *tmp, size_t tmp_bstride,
-                   int n_batch, int max_terms) {
+                   int n_batch, int max_terms, const ShoupC *merged_pinv) {
   if (n_groups == 0 || n_batch == 0) return 0;
   const NttGeom &g = k.geom;
   if (g.logN < 12) return -2;
   const size_t smem = (size_t)(n_src_max + 1) * 1024 * sizeof(u64);
   if (smem > 200 * 1024) return -2;
-  ConvColP p{y, y_bstride, groups, scale, bc, rows, tmp, tmp_bstride, k.d_mods, k.d_tw_fwd, k.d_tw_inv, g.logN, g.brow, max_terms};
+  ConvColP p{y, y_bstride, groups, scale, bc, rows, tmp, tmp_bstride, k.d_mods, k.d_tw_fwd, k.d_tw_inv, g.logN, g.brow, max_terms,
+             merged_pinv};
   dim3 grid(k.N >> 10, n_groups, n_batch);
   // algorithmic bytes: every target row written once (+ the sources, counted by the caller's row pass); butterflies of
   // the forward column stages of every target (the inverse ones of the sources are the smaller part)
   PROF(k, K_NTT_COL_BCONV, 8.0 * k.N * n_batch * (double)n_tgt_total, HALF_N(k) * g.bcol * (double)n_tgt_total * n_batch);
-#define LAUNCH_CONV(B)                                                                                                          \
-  do {                                                                                                                          \
-    if (smem > 48 * 1024) cudaFuncSetAttribute(convert_cols_kernel<B>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
-    convert_cols_kernel<B><<<grid, 128, smem, (cudaStream_t)k.stream>>>(p);                                                     \
+#define LAUNCH_CONV1(B, M)                                                                                                         \
+  do {                                                                                                                             \
+    if (smem > 48 * 1024) cudaFuncSetAttribute(convert_cols_kernel<B, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+    convert_cols_kernel<B, M><<<grid, 128, smem, (cudaStream_t)k.stream>>>(p);                                                     \
+  } while (0)
+#define LAUNCH_CONV(B)             \
+  do {                             \
+    if (merged_pinv) LAUNCH_CONV1(B, true); \
+    else LAUNCH_CONV1(B, false);   \
   } while (0)
   switch (g.bcol) {
     case 4: LAUNCH_CONV(4); break;
@@ -238,6 +284,7 @@ int k_convert_cols(const KCtx &k, u64 *y, size_t y_bstride, const ConvGroup *gro
     default: LAUNCH_CONV(8); break;
   }
 #undef LAUNCH_CONV
+#undef LAUNCH_CONV1
   LAUNCH_CHECK(k);
   return 0;
 }
@@ -448,8 +495,9 @@ int k_ntt_rows_keymac(const KCtx &k, const BatchItem *items, int L, int E, int b
 struct DivideP {
   const BatchItem *items; const u64 *tmp; size_t tmp_bstride; const u64 *acc; size_t acc_bstride; const ShoupC *mul;
   const RowDesc *rows; const ModConst *mods; const ShoupC *tw; NttGeom g; int from_items;
+  const ShoupC *mul2;  // MERGED: out = ((minuend mul2 + addend) - X) mul   (mul2 = P^-1, mul = q_{L-1}^-1)
 };
-template <int GEO>
+template <int GEO, bool MERGED = false>
 __global__ void __launch_bounds__(256, 5) ntt_rows_divide_kernel(DivideP p) {
   extern __shared__ u64 sm[];
   const int tid = threadIdx.x, b = blockIdx.z;
@@ -482,8 +530,15 @@ __global__ void __launch_bounds__(256, 5) ntt_rows_divide_kernel(DivideP p) {
     const int e = tid + i * nth;
     if (e < T) {
       const u64 x = fullred(sm[swz(e)], q, mq.qbar);
-      u64 v = shoup_mul(submod(mi[i], x, q), mc.c, mc.cs, q);
-      v = addmod(v, ad[i], q);
+      u64 v;
+      if (MERGED) {
+        const ShoupC m2 = p.mul2[rd.mod];
+        v = addmod(shoup_mul(mi[i], m2.c, m2.cs, q), ad[i], q);
+        v = shoup_mul(submod(v, x, q), mc.c, mc.cs, q);
+      } else {
+        v = shoup_mul(submod(mi[i], x, q), mc.c, mc.cs, q);
+        v = addmod(v, ad[i], q);
+      }
       dst[G.gidx(e)] = v;
     }
   }
@@ -491,13 +546,16 @@ __global__ void __launch_bounds__(256, 5) ntt_rows_divide_kernel(DivideP p) {
 
 int k_ntt_rows_divide(const KCtx &k, const BatchItem *items, const u64 *tmp, size_t tmp_bstride, const u64 *acc,
                       size_t acc_bstride, bool minuend_from_items, const ShoupC *mul, const RowDesc *rows, int n_rows,
-                      int n_batch) {
+                      int n_batch, const ShoupC *merged_mul2) {
   if (n_rows == 0 || n_batch == 0) return 0;
   const NttGeom &g = k.geom;
-  DivideP p{items, tmp, tmp_bstride, acc, acc_bstride, mul, rows, k.d_mods, k.d_tw_fwd, g, minuend_from_items ? 1 : 0};
+  DivideP p{items, tmp, tmp_bstride, acc, acc_bstride, mul, rows, k.d_mods, k.d_tw_fwd, g, minuend_from_items ? 1 : 0, merged_mul2};
   dim3 grid(k.N >> g.lt_row, n_rows, n_batch);
   PROF(k, K_DIVIDE, 8.0 * k.N * (3.5 * n_rows) * n_batch, HALF_N(k) * g.brow * n_rows * n_batch);  // temp + minuend + output, addend on half the rows
-  ROW_GEO(g, (ntt_rows_divide_kernel<GEO><<<grid, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p)));
+  if (merged_mul2)
+    ROW_GEO(g, (ntt_rows_divide_kernel<GEO, true><<<grid, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p)));
+  else
+    ROW_GEO(g, (ntt_rows_divide_kernel<GEO><<<grid, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p)));
   LAUNCH_CHECK(k);
   return 0;
 }

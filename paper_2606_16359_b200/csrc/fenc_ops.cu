@@ -402,8 +402,10 @@ static fenc_status cmult_relin(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const
     if (ina[i]->L != L || inb[i]->L != L) return fail(ctx, FENC_ERR_MISMATCH, "product: inputs differ in level");
     pa[i] = ina[i]->d, pb[i] = inb[i]->d;
   }
-  u64 *d = sc.alloc<u64>(n * 3 * LN), *mid = sc.alloc<u64>(n * 2 * LN);
-  if (!d || !mid) return fail(ctx, FENC_ERR_OOM, "product");
+  // N >= 2^12: the rescale is merged into the ModDown of the relinearisation (one pass less over the ciphertext)
+  const bool merged = ks_can_merge_rescale(ctx, L);
+  u64 *d = sc.alloc<u64>(n * 3 * LN), *mid = merged ? nullptr : sc.alloc<u64>(n * 2 * LN);
+  if (!d || (!merged && !mid)) return fail(ctx, FENC_ERR_OOM, "product");
   {
     DescStage st(ctx);
     size_t o0 = st.add(pa), o1 = st.add(pb);
@@ -416,16 +418,16 @@ static fenc_status cmult_relin(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const
   for (size_t i = 0; i < n; i++) {
     u64 *di = d + i * 3 * LN;
     items[i] = BatchItem{};
-    items[i].ks_in = di + 2 * LN, items[i].out = mid + i * 2 * LN, items[i].evk = it->second;
-    items[i].add0 = di, items[i].add1 = di + LN, items[i].g = 1;
     made[i] = sc.ct(L - 1, ina[i]->scale * inb[i]->scale / (double)ctx->mod[L - 1]);
     if (!made[i]) return fail(ctx, FENC_ERR_OOM, "product output");
+    items[i].ks_in = di + 2 * LN, items[i].out = merged ? made[i]->d : mid + i * 2 * LN, items[i].evk = it->second;
+    items[i].add0 = di, items[i].add1 = di + LN, items[i].g = 1;
     rs[i] = BatchItem{};
-    rs[i].sub_in = mid + i * 2 * LN, rs[i].out = made[i]->d;
+    rs[i].sub_in = merged ? nullptr : mid + i * 2 * LN, rs[i].out = made[i]->d;
   }
-  fenc_status st = ks_batch(ctx, L, items);
+  fenc_status st = ks_batch(ctx, L, items, merged);
   if (st != FENC_OK) return st;
-  st = rescale_batch(ctx, L, rs);
+  if (!merged) st = rescale_batch(ctx, L, rs);
   if (st != FENC_OK) return st;
   sc.ok = true;
   for (size_t i = 0; i < n; i++) out[i] = made[i];
