@@ -26,26 +26,107 @@ struct MacP {
   int L, logN, max_lazy;
 };
 #define MAC_TILE 64  // terms whose pointers are staged in shared memory at a time
-// SMALL (every modulus in use < 2^52): operands are split in 26-bit limbs, x = x1 2^26 + x0, and the three partial sums
-// sum x0 w0, sum (x0 w1 + x1 w0), sum x1 w1 are accumulated in plain 64-bit registers by IMAD.WIDE with NO carry
-// handling (each product < 2^52, so 1024 terms fit); they are recombined into a 128-bit value once per flush.  This is
-// 4 IMAD.WIDE + ~1.5 limb-split instructions per multiply-accumulate against ~20 for a carried 64x64->128 MAC.
+// Accumulation modes (chosen from the largest modulus in use):
+//  MODE 0  any modulus: x w accumulated in 128 bits (mad.lo.cc / madc.hi), reduced every max_lazy terms.
+//  MODE 1  moduli < 2^52: operands split in 26-bit limbs, x = x1 2^26 + x0; the partial sums sum x0 w0,
+//          sum (x0 w1 + x1 w0), sum x1 w1 are plain 64-bit integers (IMAD.WIDE, no carries), recombined once per flush.
+//  MODE 2  moduli < 2^40: 20-bit limbs held as DOUBLES; every product (< 2^40) and every partial sum (< 2^53 for up to
+//          2048 terms) is exact in fp64, so the partial sums are accumulated by DFMA.  Measured on B200: DFMA issues at
+//          64 lanes/clk/SM, IMAD.WIDE with a 64-bit addend at about 25, and the two use different pipes from the
+//          integer ALU that does the limb splitting.
 struct Acc3 { u64 a0, a1, a2; };
+// (mad.wide.u32 spelled out: left to itself the compiler sums the two middle products first and adds them with a
+// carry chain, twice the instructions)
+DEVI void madw(u64 &acc, u32 a, u32 b) { asm("mad.wide.u32 %0, %1, %2, %0;" : "+l"(acc) : "r"(a), "r"(b)); }
 DEVI void acc3_mac(Acc3 &A, u32 x0, u32 x1, u32 w0, u32 w1) {
-  A.a0 += (u64)x0 * w0;
-  A.a1 += (u64)x0 * w1;
-  A.a1 += (u64)x1 * w0;
-  A.a2 += (u64)x1 * w1;
+  madw(A.a0, x0, w0);
+  madw(A.a1, x0, w1);
+  madw(A.a1, x1, w0);
+  madw(A.a2, x1, w1);
 }
-DEVI u64 acc3_redc(Acc3 &A, u64 q, u64 qinv_neg) {  // (a0 + a1 2^26 + a2 2^52) 2^-64 mod q, and clears A
-  u64 lo = A.a0, hi = 0, t;
-  t = A.a1 << 26; lo += t; hi += (A.a1 >> 38) + (lo < t ? 1 : 0);
-  t = A.a2 << 52; lo += t; hi += (A.a2 >> 12) + (lo < t ? 1 : 0);
-  A.a0 = A.a1 = A.a2 = 0;
+template <int SH>
+DEVI u64 limbs_redc(u64 a0, u64 a1, u64 a2, u64 q, u64 qinv_neg) {  // (a0 + a1 2^SH + a2 2^2SH) 2^-64 mod q
+  u64 lo = a0, hi = 0, t;
+  t = a1 << SH; lo += t; hi += (a1 >> (64 - SH)) + (lo < t ? 1 : 0);
+  t = a2 << (2 * SH); lo += t; hi += (a2 >> (64 - 2 * SH)) + (lo < t ? 1 : 0);
   return mont_redc(lo, hi, q, qinv_neg);
 }
-template <int G, bool SMALL>
-__global__ void __launch_bounds__(256, 2) mac_kernel(MacP p) {
+struct AccD { double a0, a1, a2; };
+DEVI double u2d(u32 v) { return __hiloint2double(0x43300000, (int)v) - 4503599627370496.0; }  // exact, v < 2^32
+DEVI void accd_mac(AccD &A, double x0, double x1, double w0, double w1) {
+  A.a0 = fma(x0, w0, A.a0);
+  A.a1 = fma(x0, w1, A.a1);
+  A.a1 = fma(x1, w0, A.a1);
+  A.a2 = fma(x1, w1, A.a2);
+}
+template <int G, int MODE>
+struct MacState {
+  u64 lo0[MODE == 0 ? G : 1], hi0[MODE == 0 ? G : 1], lo1[MODE == 0 ? G : 1], hi1[MODE == 0 ? G : 1];
+  Acc3 A0[MODE == 1 ? G : 1], A1[MODE == 1 ? G : 1];
+  AccD D0[MODE == 2 ? G : 1], D1[MODE == 2 ? G : 1];
+  int lazy, max_lazy;
+  DEVI void set(int i, u64 v0, u64 v1) {  // accumulators := the small integers v0, v1
+    if (MODE == 0) lo0[i] = v0, lo1[i] = v1, hi0[i] = hi1[i] = 0;
+    if (MODE == 1) A0[i] = Acc3{v0, 0, 0}, A1[i] = Acc3{v1, 0, 0};
+    if (MODE == 2) D0[i] = AccD{(double)v0, 0, 0}, D1[i] = AccD{(double)v1, 0, 0};
+  }
+  DEVI void init(int ctx_max_lazy) {
+#pragma unroll
+    for (int i = 0; i < G; i++) set(i, 0, 0);
+    // one slot of every bound is left for the folded-back residue (< q)
+    max_lazy = MODE == 0 ? ctx_max_lazy - 1 : (MODE == 1 ? 1023 : 2047);
+    if (max_lazy < 1) max_lazy = 1;
+    lazy = 0;
+  }
+  // the pending sum S as S 2^-64 mod q (canonical)
+  DEVI u64 out0(int i, const ModConst &mc) const {
+    if (MODE == 0) return mont_redc(lo0[i], hi0[i], mc.q, mc.qinv_neg);
+    if (MODE == 1) return limbs_redc<26>(A0[i].a0, A0[i].a1, A0[i].a2, mc.q, mc.qinv_neg);
+    return limbs_redc<20>((u64)D0[i].a0, (u64)D0[i].a1, (u64)D0[i].a2, mc.q, mc.qinv_neg);
+  }
+  DEVI u64 out1(int i, const ModConst &mc) const {
+    if (MODE == 0) return mont_redc(lo1[i], hi1[i], mc.q, mc.qinv_neg);
+    if (MODE == 1) return limbs_redc<26>(A1[i].a0, A1[i].a1, A1[i].a2, mc.q, mc.qinv_neg);
+    return limbs_redc<20>((u64)D1[i].a0, (u64)D1[i].a1, (u64)D1[i].a2, mc.q, mc.qinv_neg);
+  }
+  DEVI void mac(u64 x0, u64 x1, const u64 (&w)[G], const ModConst &mc) {
+    if (MODE == 0) {
+#pragma unroll
+      for (int i = 0; i < G; i++) mac128(lo0[i], hi0[i], x0, w[i]), mac128(lo1[i], hi1[i], x1, w[i]);
+    } else if (MODE == 1) {
+      const u32 m = (1u << 26) - 1;
+      const u32 x00 = (u32)x0 & m, x01 = (u32)(x0 >> 26), x10 = (u32)x1 & m, x11 = (u32)(x1 >> 26);
+#pragma unroll
+      for (int i = 0; i < G; i++) {
+        const u32 w0 = (u32)w[i] & m, w1 = (u32)(w[i] >> 26);
+        acc3_mac(A0[i], x00, x01, w0, w1);
+        acc3_mac(A1[i], x10, x11, w0, w1);
+      }
+    } else {
+      const u32 m = (1u << 20) - 1;
+      const double x00 = u2d((u32)x0 & m), x01 = u2d((u32)(x0 >> 20)), x10 = u2d((u32)x1 & m), x11 = u2d((u32)(x1 >> 20));
+#pragma unroll
+      for (int i = 0; i < G; i++) {
+        const double w0 = u2d((u32)w[i] & m), w1 = u2d((u32)(w[i] >> 20));
+        accd_mac(D0[i], x00, x01, w0, w1);
+        accd_mac(D1[i], x10, x11, w0, w1);
+      }
+    }
+    if (++lazy == max_lazy) {
+      // fold: S 2^-64 mod q times 2^128 2^-64 = S mod q, a residue below q, becomes the new pending sum
+#pragma unroll
+      for (int i = 0; i < G; i++)
+        set(i, mont_mul(out0(i, mc), mc.r2, mc.q, mc.qinv_neg), mont_mul(out1(i, mc), mc.r2, mc.q, mc.qinv_neg));
+      lazy = 0;
+    }
+  }
+};
+
+#ifndef MAC_THREADS
+#define MAC_THREADS 256
+#endif
+template <int G, int MODE>
+__global__ void __launch_bounds__(MAC_THREADS, 512 / MAC_THREADS) mac_kernel(MacP p) {
   __shared__ const u64 *s_ct[MAC_TILE];
   __shared__ const u64 *s_pt[G][MAC_TILE];
   const size_t LN = (size_t)p.L << p.logN;
@@ -53,16 +134,8 @@ __global__ void __launch_bounds__(256, 2) mac_kernel(MacP p) {
   const bool live = idx < LN;
   const MacGroup g = p.groups[blockIdx.x];
   const ModConst mc = p.mods[(live ? idx : 0) >> p.logN];
-  u64 lo0[SMALL ? 1 : G], hi0[SMALL ? 1 : G], lo1[SMALL ? 1 : G], hi1[SMALL ? 1 : G], r0[G], r1[G];
-  Acc3 A0[SMALL ? G : 1], A1[SMALL ? G : 1];
-#pragma unroll
-  for (int i = 0; i < G; i++) r0[i] = r1[i] = 0;
-#pragma unroll
-  for (int i = 0; i < (SMALL ? 1 : G); i++) lo0[i] = hi0[i] = lo1[i] = hi1[i] = 0;
-#pragma unroll
-  for (int i = 0; i < (SMALL ? G : 1); i++) A0[i] = Acc3{0, 0, 0}, A1[i] = Acc3{0, 0, 0};
-  const int max_lazy = SMALL ? (p.max_lazy < 1024 ? p.max_lazy : 1024) : p.max_lazy;
-  int lazy = 0;
+  MacState<G, MODE> st;
+  st.init(p.max_lazy);
   for (int t0 = 0; t0 < g.n_terms; t0 += MAC_TILE) {
     const int nt = g.n_terms - t0 < MAC_TILE ? g.n_terms - t0 : MAC_TILE;
     __syncthreads();
@@ -81,36 +154,7 @@ __global__ void __launch_bounds__(256, 2) mac_kernel(MacP p) {
       u64 w[G];
 #pragma unroll
       for (int i = 0; i < G; i++) w[i] = __ldg(s_pt[i][t] + idx);
-      if (SMALL) {
-        const u32 m26 = (1u << 26) - 1;
-        const u32 x00 = (u32)x0 & m26, x01 = (u32)(x0 >> 26), x10 = (u32)x1 & m26, x11 = (u32)(x1 >> 26);
-#pragma unroll
-        for (int i = 0; i < G; i++) {
-          const u32 w0 = (u32)w[i] & m26, w1 = (u32)(w[i] >> 26);
-          acc3_mac(A0[i], x00, x01, w0, w1);
-          acc3_mac(A1[i], x10, x11, w0, w1);
-        }
-      } else {
-#pragma unroll
-        for (int i = 0; i < G; i++) {
-          mac128(lo0[i], hi0[i], x0, w[i]);
-          mac128(lo1[i], hi1[i], x1, w[i]);
-        }
-      }
-      if (++lazy == max_lazy) {
-#pragma unroll
-        for (int i = 0; i < G; i++) {
-          if (SMALL) {
-            r0[i] = addmod(r0[i], acc3_redc(A0[i], mc.q, mc.qinv_neg), mc.q);
-            r1[i] = addmod(r1[i], acc3_redc(A1[i], mc.q, mc.qinv_neg), mc.q);
-          } else {
-            r0[i] = addmod(r0[i], mont_redc(lo0[i], hi0[i], mc.q, mc.qinv_neg), mc.q);
-            r1[i] = addmod(r1[i], mont_redc(lo1[i], hi1[i], mc.q, mc.qinv_neg), mc.q);
-            lo0[i] = hi0[i] = lo1[i] = hi1[i] = 0;
-          }
-        }
-        lazy = 0;
-      }
+      st.mac(x0, x1, w, mc);
     }
   }
   if (!live) return;
@@ -118,31 +162,31 @@ __global__ void __launch_bounds__(256, 2) mac_kernel(MacP p) {
   for (int i = 0; i < G; i++) {
     if (i < g.n_out) {
       u64 *out = p.outs[g.out_start + i];
-      if (SMALL) {
-        out[idx] = addmod(r0[i], acc3_redc(A0[i], mc.q, mc.qinv_neg), mc.q);
-        out[LN + idx] = addmod(r1[i], acc3_redc(A1[i], mc.q, mc.qinv_neg), mc.q);
-      } else {
-        out[idx] = addmod(r0[i], mont_redc(lo0[i], hi0[i], mc.q, mc.qinv_neg), mc.q);
-        out[LN + idx] = addmod(r1[i], mont_redc(lo1[i], hi1[i], mc.q, mc.qinv_neg), mc.q);
-      }
+      out[idx] = st.out0(i, mc);
+      out[LN + idx] = st.out1(i, mc);
     }
   }
 }
+template <int MODE>
+static void launch_mac(const MacP &p, dim3 grid, cudaStream_t st, int max_group) {
+  if (max_group <= 1) mac_kernel<1, MODE><<<grid, MAC_THREADS, 0, st>>>(p);
+  else if (max_group <= 2) mac_kernel<2, MODE><<<grid, MAC_THREADS, 0, st>>>(p);
+  else mac_kernel<4, MODE><<<grid, MAC_THREADS, 0, st>>>(p);
+}
+
+// q_max = largest modulus among the L limbs in use (selects the accumulation mode)
 int k_mac(const KCtx &k, const MacGroup *groups, int n_groups, int max_group, const u64 *const *term_ct, const u64 *const *term_pt,
-          u64 *const *outs, int L, int max_lazy, bool small_moduli, double alg_bytes) {
+          u64 *const *outs, int L, int max_lazy, u64 q_max, double alg_bytes) {
   if (n_groups == 0) return 0;
   MacP p{groups, term_ct, term_pt, outs, k.d_mods, L, k.geom.logN, max_lazy};
-  dim3 grid(n_groups, (unsigned)(((size_t)L * k.N + 255) / 256));
+  dim3 grid(n_groups, (unsigned)(((size_t)L * k.N + MAC_THREADS - 1) / MAC_THREADS));
   PROF(k, K_MAC, alg_bytes);
-  if (small_moduli) {
-    if (max_group <= 1) mac_kernel<1, true><<<grid, 256, 0, S(k)>>>(p);
-    else if (max_group <= 2) mac_kernel<2, true><<<grid, 256, 0, S(k)>>>(p);
-    else mac_kernel<4, true><<<grid, 256, 0, S(k)>>>(p);
-  } else {
-    if (max_group <= 1) mac_kernel<1, false><<<grid, 256, 0, S(k)>>>(p);
-    else if (max_group <= 2) mac_kernel<2, false><<<grid, 256, 0, S(k)>>>(p);
-    else mac_kernel<4, false><<<grid, 256, 0, S(k)>>>(p);
-  }
+  static const int force_mode = getenv("FENC_MAC_MODE") ? atoi(getenv("FENC_MAC_MODE")) : -1;  // diagnostics: a more general mode
+  int mode = q_max < (1ull << 40) ? 2 : (q_max < (1ull << 52) ? 1 : 0);
+  if (force_mode >= 0 && force_mode < mode) mode = force_mode;
+  if (mode == 2) launch_mac<2>(p, grid, S(k), max_group);
+  else if (mode == 1) launch_mac<1>(p, grid, S(k), max_group);
+  else launch_mac<0>(p, grid, S(k), max_group);
   LAUNCH_CHECK(k);
   return 0;
 }

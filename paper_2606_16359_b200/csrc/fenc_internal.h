@@ -136,7 +136,7 @@ int k_ntt_rows_divide(const KCtx &k, const BatchItem *items, const u64 *tmp, siz
 // MAC (a7) over groups of outputs sharing one ciphertext sequence (register tiling, fenc_elem.cu):
 // out[out_start+i] = sum_{t<n_terms} ct[ct_start+t] (*) pt[pt_start + i*n_terms + t], i < n_out <= FENC_MAC_GROUP
 int k_mac(const KCtx &k, const MacGroup *groups, int n_groups, int max_group, const u64 *const *term_ct, const u64 *const *term_pt,
-          u64 *const *outs, int L, int max_lazy, bool small_moduli, double alg_bytes);
+          u64 *const *outs, int L, int max_lazy, u64 q_max, double alg_bytes);
 // outs[o] = sum of listed [2][L][N] arrays
 int k_add_many(const KCtx &k, const u64 *const *term, const int *start, u64 *const *outs, int n_out, int L, int n_terms);
 // rows kernels: row r uses modulus row_mod[r] (device array)

@@ -288,7 +288,7 @@ fenc_status run_mac(fenc_ctx *ctx, const MacJob &job, int L) {
   char *base = st.commit();
   if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
   CUDA_OK(ctx, k_mac(ctx->k, (const MacGroup *)(base + o0), (int)groups.size(), max_group, (const u64 *const *)(base + o1),
-                     (const u64 *const *)(base + o2), (u64 *const *)(base + o3), L, ctx->max_lazy, ctx->mod[0] < (1ull << 52), mac_alg_bytes(ctx, tc, tp, n, L)));
+                     (const u64 *const *)(base + o2), (u64 *const *)(base + o3), L, ctx->max_lazy, *std::max_element(ctx->mod.begin(), ctx->mod.begin() + L), mac_alg_bytes(ctx, tc, tp, n, L)));
   return FENC_OK;
 }
 // algorithmic bytes of one MAC launch: every distinct ciphertext and plaintext read once, every output written once

@@ -29,6 +29,28 @@ def make(mods, name, **over):
     return P, ctx
 
 
+@pytest.mark.parametrize("q_bits,p_bits", [(30, 31), (50, 60), (58, 60)])
+def test_long_mac_every_accumulation_mode(mods, q_bits, p_bits):
+    """PMult-accumulate of 2100 terms: the MAC kernel's three accumulation modes (20-bit limbs in fp64 below 2^40,
+    26-bit limbs below 2^52, 128-bit otherwise) each fold their pending sum back at least once (a7)."""
+    ck, fr, fenc = mods
+    P, ctx = make(mods, "toy64", q_bits=q_bits, p_bits=p_bits)
+    N, L = P.N, P.nq
+    rng = np.random.default_rng(5)
+    limbs = [wl.random_ct_limbs(100 + i, P.q, L, N) for i in range(5)]
+    ws = [ck.encode(P, rng.normal(0, 0.5, P.n), L, 2.0 ** 20) for _ in range(7)]
+    octs = [ck.Ciphertext(x, L, 2.0 ** 20) for x in limbs]
+    gcts = [ctx.ct_import(x, 2.0 ** 20) for x in limbs]
+    gpts = [ctx.pt_from_coeffs(w.coeffs, L, float(w.scale)) for w in ws]
+    n_terms = 2100
+    acc = np.zeros_like(limbs[0])
+    for t in range(n_terms):
+        ck.pmult_acc(P, acc, octs[t % 5], ws[t % 7])
+    got = ctx.pmult_sum([gcts[t % 5] for t in range(n_terms)], [gpts[t % 7] for t in range(n_terms)])
+    assert np.array_equal(ctx.ct_export(got), acc)
+    ctx.close()
+
+
 @pytest.mark.parametrize("name", ["toy64", "mid10", "mid12"])
 def test_primitives_bit_exact(mods, name):
     ck, fr, fenc = mods
