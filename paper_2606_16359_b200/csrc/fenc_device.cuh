@@ -90,6 +90,32 @@ struct TileGeo {
 // v mod q for any v < 2^64: v - floor(v qbar / 2^64) q lies in [0, 2q) (qbar = floor(2^64 / q)), then one correction
 DEVI u64 fullred(u64 v, u64 q, u64 qbar) { return csub(v - __umul64hi(v, qbar) * q, q); }
 
+// ---------------------------------------------------------------------------------------------- fp64 twiddle multiply
+// For moduli below 2^45 (ModConst.f64 != 0) the butterflies multiply on the FP64 pipe: on B200 every integer multiply
+// shares the fmaheavy pipe (70-75 % busy in the NTT kernels, their top stall) while DFMA issues at 64 lanes/clk/SM on a
+// pipe of its own.  x c mod q for x < 2^51: with xd = x as a double, h + l = xd c exactly (h = rn(xd c),
+// l = fma(xd, c, -h)), k = rint(xd (c/q)) is floor or ceil of the true quotient (the relative error of c/q is 2^-53 and
+// the quotient is below 2^51), so t = (h - k q) + l is the exact integer x c - k q in (-q, q): fma(-k, q, h) is exact
+// because its result, t - l, is an integer below 2^42.  The return value t + q lies in (0, 2q), the range
+// shoup_lazy promises, so the lazy bounds of the integer butterflies carry over unchanged and the canonical results
+// are identical.  Twiddle tables of such moduli hold the pair {(double) w, (double) (w / q)} instead of {w, w'}.
+#define FENC_F64_MAX_BITS 45
+DEVI double u2d52(u64 x) {  // exact for x < 2^52
+  return __dadd_rn(__hiloint2double((int)((u32)(x >> 32) | 0x43300000u), (int)(u32)x), -4503599627370496.0);
+}
+struct F64Mod { double q, q_magic; };  // q and q + 2^52
+DEVI F64Mod f64mod(u64 q) { return F64Mod{(double)q, (double)q + 4503599627370496.0}; }
+DEVI u64 mulmod_f64(u64 x, u64 c_bits, u64 cq_bits, const F64Mod &m) {
+  const double c = __longlong_as_double((long long)c_bits), cq = __longlong_as_double((long long)cq_bits);
+  const double xd = u2d52(x);
+  const double h = __dmul_rn(xd, c);
+  const double l = __fma_rn(xd, c, -h);
+  const double k = __dadd_rn(__fma_rn(xd, cq, 6755399441055744.0), -6755399441055744.0);
+  const double r = __fma_rn(-k, m.q, h);
+  const double t = __dadd_rn(__dadd_rn(r, l), m.q_magic);  // 2^52 + (t + q): the integer sits in the low mantissa bits
+  return (u64)__double_as_longlong(t) & 0xFFFFFFFFFFFFFull;
+}
+
 // ---------------------------------------------------------------------------------------------- tile engine
 // A pass transforms the active tile bits [lo, lo+nb) in radix-8 register rounds (3 stages per round) through
 // swizzled shared memory.  FWD: Cooley-Tukey, high bit first.  INV: Gentleman-Sande, low bit first, values in [0,2q).
@@ -101,8 +127,9 @@ DEVI u64 fullred(u64 v, u64 q, u64 qbar) { return csub(v - __umul64hi(v, qbar) *
 // shared-memory slot is swz(ebase) ^ swz(k << PW): one base computation per thread and round.
 
 // compile-time round: window position and active stages [SLO, SHI) are constants (production geometries)
-template <bool FWD, bool LAZY, int PW, int SLO, int SHI>
+template <bool FWD, bool LAZY, int PW, int SLO, int SHI, bool F64>
 DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid) {
+  const F64Mod fm = f64mod(q);
   const int ebase = ((tid >> PW) << (PW + 3)) | (tid & ((1 << PW) - 1));
   const int gpw = G.gbit(PW);
   const u32 nj = (1u << G.logN) + G.gidx(ebase);
@@ -129,13 +156,13 @@ DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 
       const ulonglong2 w = s == 2 ? t2 : (s == 1 ? t1[k >> 2] : t0[k >> 1]);
       if (FWD) {
         const u64 X = LAZY ? x[k] : csub(x[k], q2);
-        const u64 T = shoup_lazy(x[k2], w.x, w.y, q);
+        const u64 T = F64 ? mulmod_f64(x[k2], w.x, w.y, fm) : shoup_lazy(x[k2], w.x, w.y, q);
         x[k] = X + T;
         x[k2] = X - T + q2;
       } else {
         const u64 U = x[k], V = x[k2];
         x[k] = csub(U + V, q2);
-        x[k2] = shoup_lazy(U - V + q2, w.x, w.y, q);
+        x[k2] = F64 ? mulmod_f64(U - V + q2, w.x, w.y, fm) : shoup_lazy(U - V + q2, w.x, w.y, q);
       }
     }
   }
@@ -143,22 +170,23 @@ DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 
   for (int k = 0; k < 8; k++) sm[sbase ^ swz(k << PW)] = x[k];
 }
 
-template <bool FWD, bool LAZY, int LT, int LO, int NB, int DONE>
+template <bool FWD, bool LAZY, int LT, int LO, int NB, int DONE, bool F64 = false>
 DEVI void tile_rounds_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid) {
   if constexpr (DONE < NB) {
     constexpr int take = NB - DONE < 3 ? NB - DONE : 3;
     constexpr int cur = FWD ? LO + NB - DONE : LO + DONE;         // FWD: exclusive top; INV: inclusive bottom
     constexpr int p = FWD ? cur - take : cur;
     constexpr int pw = p < LT - 3 ? p : LT - 3;
-    if (tid < (1 << (LT - 3))) tile_round_ct<FWD, LAZY, pw, p - pw, p - pw + take>(sm, G, tw, q, q2, tid);
+    if (tid < (1 << (LT - 3))) tile_round_ct<FWD, LAZY, pw, p - pw, p - pw + take, F64>(sm, G, tw, q, q2, tid);
     __syncthreads();
-    tile_rounds_ct<FWD, LAZY, LT, LO, NB, DONE + take>(sm, G, tw, q, q2, tid);
+    tile_rounds_ct<FWD, LAZY, LT, LO, NB, DONE + take, F64>(sm, G, tw, q, q2, tid);
   }
 }
 
 // runtime round (toy ring degrees and any geometry without a compile-time instance)
-template <bool FWD>
+template <bool FWD, bool F64>
 DEVI void tile_round_rt(u64 *sm, const TileGeo &G, int pw, int s_lo, int s_hi, const ShoupC *tw, u64 q, u64 q2, int tid) {
+  const F64Mod fm = f64mod(q);
   const int ebase = ((tid >> pw) << (pw + 3)) | (tid & ((1 << pw) - 1));
   u64 x[8];
 #pragma unroll
@@ -176,13 +204,13 @@ DEVI void tile_round_rt(u64 *sm, const TileGeo &G, int pw, int s_lo, int s_hi, c
       const ShoupC w = tw[(nj >> (gpw + s + 1)) + (k >> (s + 1))];
       if (FWD) {
         u64 X = csub(x[k], q2);
-        u64 T = shoup_lazy(x[k2], w.c, w.cs, q);
+        u64 T = F64 ? mulmod_f64(x[k2], w.c, w.cs, fm) : shoup_lazy(x[k2], w.c, w.cs, q);
         x[k] = X + T;
         x[k2] = X - T + q2;
       } else {
         u64 U = x[k], V = x[k2];
         x[k] = csub(U + V, q2);
-        x[k2] = shoup_lazy(U - V + q2, w.c, w.cs, q);
+        x[k2] = F64 ? mulmod_f64(U - V + q2, w.c, w.cs, fm) : shoup_lazy(U - V + q2, w.c, w.cs, q);
       }
     }
   }
@@ -193,9 +221,10 @@ DEVI void tile_round_rt(u64 *sm, const TileGeo &G, int pw, int s_lo, int s_hi, c
 // compile-time schedule over active tile bits [LO, LO+NB) of a 2^LT-element tile; picks the lazy forward butterflies
 // for q < 2^58.  Every thread of the block must call this (it synchronises).
 template <bool FWD, int LT, int LO, int NB>
-DEVI void tile_transform_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, int tid) {
+DEVI void tile_transform_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, int tid, bool f64) {
   const u64 q2 = q + q;
-  if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
+  if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, true>(sm, G, tw, q, q2, tid);
+  else if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
   else tile_rounds_ct<FWD, false, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
 }
 
@@ -203,7 +232,7 @@ DEVI void tile_transform_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, 
 // 4..8 = column pass with GEO stages over tiles of 2^(GEO+4) elements (16 columns).
 // Every thread of the block must call this (it synchronises).  Outputs: forward < 33q (use fullred), inverse < 2q.
 template <bool FWD, int GEO>
-DEVI void tile_transform(u64 *sm, const TileGeo &G, int lo, int nb, const ShoupC *tw, u64 q, int tid) {
+DEVI void tile_transform(u64 *sm, const TileGeo &G, int lo, int nb, const ShoupC *tw, u64 q, int tid, bool f64) {
   const u64 q2 = q + q;
   if constexpr (GEO == 0) {
     const bool active = tid < (1 << (G.lt - 3));
@@ -213,7 +242,7 @@ DEVI void tile_transform(u64 *sm, const TileGeo &G, int lo, int nb, const ShoupC
         int take = cur - lo < 3 ? cur - lo : 3;
         int p = cur - take;
         int pw = p < G.lt - 3 ? p : G.lt - 3;
-        if (active) tile_round_rt<true>(sm, G, pw, p - pw, cur - pw, tw, q, q2, tid);
+        if (active) { if (f64) tile_round_rt<true, true>(sm, G, pw, p - pw, cur - pw, tw, q, q2, tid); else tile_round_rt<true, false>(sm, G, pw, p - pw, cur - pw, tw, q, q2, tid); }
         __syncthreads();
         cur = p;
       }
@@ -222,14 +251,15 @@ DEVI void tile_transform(u64 *sm, const TileGeo &G, int lo, int nb, const ShoupC
       while (cur < lo + nb) {
         int take = lo + nb - cur < 3 ? lo + nb - cur : 3;
         int pw = cur < G.lt - 3 ? cur : G.lt - 3;
-        if (active) tile_round_rt<false>(sm, G, pw, cur - pw, cur + take - pw, tw, q, q2, tid);
+        if (active) { if (f64) tile_round_rt<false, true>(sm, G, pw, cur - pw, cur + take - pw, tw, q, q2, tid); else tile_round_rt<false, false>(sm, G, pw, cur - pw, cur + take - pw, tw, q, q2, tid); }
         __syncthreads();
         cur += take;
       }
     }
   } else {
     constexpr int LT = GEO == 1 ? FENC_ROW_LT : GEO + 4, LO = GEO == 1 ? 0 : 4, NB = GEO == 1 ? 8 : GEO;
-    if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
+    if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, true>(sm, G, tw, q, q2, tid);
+    else if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
     else tile_rounds_ct<FWD, false, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
   }
 }

@@ -2,6 +2,8 @@
 // generator (host copy, used for the secret), fp64 encode / decode, and the CRT lift used by decryption.
 // Written independently of oracle/ (the two share no code); the rules are those of DESIGN.md section 4.
 #include <cmath>
+#include <cstdlib>
+#include <cstring>
 #include <complex>
 #include <map>
 #include <mutex>
@@ -84,18 +86,30 @@ static u32 bitrev(u32 x, int bits) {
 }
 
 // fwd[k] = psi^bitrev(k), inv[k] = psi^-bitrev(k), each with its Shoup companion
+bool f64_modulus(u64 q) {
+  static const bool off = getenv("FENC_NO_F64") != nullptr;  // diagnostics: integer butterflies everywhere
+  return !off && q < (1ull << 45);
+}
 void build_twiddles(u64 q, u64 psi, int logN, ShoupC *fwd, ShoupC *inv) {
   const u32 N = 1u << logN;
   std::vector<u64> pw(N), ipw(N);
   const u64 ipsi = invmod(psi, q);
   pw[0] = ipw[0] = 1;
   for (u32 i = 1; i < N; i++) pw[i] = mulmod(pw[i - 1], psi, q), ipw[i] = mulmod(ipw[i - 1], ipsi, q);
+  const bool f64 = f64_modulus(q);
+  auto bits = [](double d) { u64 b; memcpy(&b, &d, 8); return b; };
   for (u32 k = 0; k < N; k++) {
     u32 r = bitrev(k, logN);
-    fwd[k].c = pw[r], fwd[k].cs = shoup(pw[r], q);
-    inv[k].c = ipw[r], inv[k].cs = shoup(ipw[r], q);
+    if (f64) {  // {(double) w, (double) (w / q)}: the quotient estimate needs c/q to within a few ulp (fenc_device.cuh)
+      fwd[k].c = bits((double)pw[r]), fwd[k].cs = bits((double)((long double)pw[r] / (long double)q));
+      inv[k].c = bits((double)ipw[r]), inv[k].cs = bits((double)((long double)ipw[r] / (long double)q));
+    } else {
+      fwd[k].c = pw[r], fwd[k].cs = shoup(pw[r], q);
+      inv[k].c = ipw[r], inv[k].cs = shoup(ipw[r], q);
+    }
   }
 }
+
 
 // ------------------------------------------------------------------ counter-based generator (R2.3)
 static const u64 GAMMA = 0x9E3779B97F4A7C15ull;
