@@ -156,7 +156,7 @@ extern "C" fenc_status fenc_params_init(const fenc_params_desc *d, fenc_ctx **ou
     u64 m = ctx->mod[i];
     ctx->psi[i] = fh::find_psi(m, N);
     int bits = 64 - __builtin_clzll(m - 1);
-    mods[i] = ModConst{m, fh::neg_qinv(m), fh::to_mont(fh::to_mont(1, m), m), (bits >= 64 ? ~0ull : (1ull << bits) - 1), (u64)((((u128)1) << 64) / m), fh::f64_modulus(m) ? 1ull : 0ull, {0, 0}};
+    mods[i] = ModConst{m, fh::neg_qinv(m), fh::to_mont(fh::to_mont(1, m), m), (bits >= 64 ? ~0ull : (1ull << bits) - 1), (u64)((((u128)1) << 64) / m), fh::f64_modulus(m) ? fh::double_bits(1.0 / (double)m) : 0ull, {0, 0}};
     fh::build_twiddles(m, ctx->psi[i], ctx->logN, &fwd[(size_t)i * N], &inv[(size_t)i * N]);
     u64 ni = fh::invmod((u64)N % m, m);
     ninv[i] = ShoupC{ni, fh::shoup(ni, m)};

@@ -103,17 +103,28 @@ DEVI u64 fullred(u64 v, u64 q, u64 qbar) { return csub(v - __umul64hi(v, qbar) *
 DEVI double u2d52(u64 x) {  // exact for x < 2^52
   return __dadd_rn(__hiloint2double((int)((u32)(x >> 32) | 0x43300000u), (int)(u32)x), -4503599627370496.0);
 }
-struct F64Mod { double q, q_magic; };  // q and q + 2^52
-DEVI F64Mod f64mod(u64 q) { return F64Mod{(double)q, (double)q + 4503599627370496.0}; }
-DEVI u64 mulmod_f64(u64 x, u64 c_bits, u64 cq_bits, const F64Mod &m) {
-  const double c = __longlong_as_double((long long)c_bits), cq = __longlong_as_double((long long)cq_bits);
-  const double xd = u2d52(x);
+struct F64Mod { double q, qinv; };  // q and 1/q
+DEVI F64Mod f64mod(u64 q, u64 qinv_bits) { return F64Mod{(double)q, __longlong_as_double((long long)qinv_bits)}; }
+#define F64_RINT_MAGIC 6755399441055744.0  // 1.5 2^52: fma(a, b, MAGIC) - MAGIC = rint(a b) for |a b| < 2^51
+// x c - k q in (-q, q) for a double x holding an integer, |x| < 2^51
+DEVI double mulmod_dd(double xd, double c, double cq, const F64Mod &m) {
   const double h = __dmul_rn(xd, c);
   const double l = __fma_rn(xd, c, -h);
-  const double k = __dadd_rn(__fma_rn(xd, cq, 6755399441055744.0), -6755399441055744.0);
-  const double r = __fma_rn(-k, m.q, h);
-  const double t = __dadd_rn(__dadd_rn(r, l), m.q_magic);  // 2^52 + (t + q): the integer sits in the low mantissa bits
-  return (u64)__double_as_longlong(t) & 0xFFFFFFFFFFFFFull;
+  const double k = __dadd_rn(__fma_rn(xd, cq, F64_RINT_MAGIC), -F64_RINT_MAGIC);
+  return __dadd_rn(__fma_rn(-k, m.q, h), l);
+}
+// v - rint(v / q) q: |result| <= q/2 (+1 when v/q is within 2^-53 relative of a half-integer)
+DEVI double reduce_dd(double v, const F64Mod &m) {
+  const double k = __dadd_rn(__fma_rn(v, m.qinv, F64_RINT_MAGIC), -F64_RINT_MAGIC);
+  return __fma_rn(-k, m.q, v);
+}
+// a double holding an integer in [-off, 2^52 - off) -> that integer + off as u64 (off an integer below 2^52)
+DEVI u64 d2u_off(double v, double off_magic /* off + 2^52 */) {
+  return (u64)__double_as_longlong(__dadd_rn(v, off_magic)) & 0xFFFFFFFFFFFFFull;
+}
+DEVI u64 mulmod_f64(u64 x, u64 c_bits, u64 cq_bits, const F64Mod &m) {  // (0, 2q), the range of shoup_lazy
+  const double t = mulmod_dd(u2d52(x), __longlong_as_double((long long)c_bits), __longlong_as_double((long long)cq_bits), m);
+  return d2u_off(t, m.q + 4503599627370496.0);
 }
 
 // ---------------------------------------------------------------------------------------------- tile engine
@@ -128,8 +139,7 @@ DEVI u64 mulmod_f64(u64 x, u64 c_bits, u64 cq_bits, const F64Mod &m) {
 
 // compile-time round: window position and active stages [SLO, SHI) are constants (production geometries)
 template <bool FWD, bool LAZY, int PW, int SLO, int SHI, bool F64>
-DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid) {
-  const F64Mod fm = f64mod(q);
+DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid, u64 f64) {
   const int ebase = ((tid >> PW) << (PW + 3)) | (tid & ((1 << PW) - 1));
   const int gpw = G.gbit(PW);
   const u32 nj = (1u << G.logN) + G.gidx(ebase);
@@ -142,6 +152,40 @@ DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 
 #pragma unroll
   for (int i = 0; i < 4; i++) t0[i] = (0 >= SLO && 0 < SHI) ? __ldg(twv + (nj >> (gpw + 1)) + i) : t2;
   const int sbase = swz(ebase);
+  if constexpr (F64) {
+    // the eight values stay doubles (signed, exact integers) through the round's stages: T in (-q, q), so a forward
+    // stage moves a value by less than q either way and the stored value, shifted by +3q, stays non-negative and grows
+    // by at most 6q per round (36q after the five rounds of a 2^16 transform, inside the 2^51 the multiply accepts);
+    // an inverse round ends with v - rint(v/q) q + q, inside the [0, 2q) the inverse contract promises.
+    const F64Mod fm = f64mod(q, f64);
+    double x[8];
+#pragma unroll
+    for (int k = 0; k < 8; k++) x[k] = u2d52(sm[sbase ^ swz(k << PW)]);
+#pragma unroll
+    for (int ss = 0; ss < 3; ss++) {
+      const int s = FWD ? 2 - ss : ss;
+      if (s < SLO || s >= SHI) continue;
+#pragma unroll
+      for (int k = 0; k < 8; k++) {
+        if (k & (1 << s)) continue;
+        const int k2 = k | (1 << s);
+        const ulonglong2 w = s == 2 ? t2 : (s == 1 ? t1[k >> 2] : t0[k >> 1]);
+        const double c = __longlong_as_double((long long)w.x), cq = __longlong_as_double((long long)w.y);
+        if (FWD) {
+          const double X = x[k], T = mulmod_dd(x[k2], c, cq, fm);
+          x[k] = __dadd_rn(X, T);
+          x[k2] = __dadd_rn(X, -T);
+        } else {
+          const double U = x[k], V = x[k2];
+          x[k] = __dadd_rn(U, V);
+          x[k2] = mulmod_dd(__dadd_rn(U, -V), c, cq, fm);
+        }
+      }
+    }
+    const double off = FWD ? __fma_rn(3.0, fm.q, 4503599627370496.0) : __dadd_rn(fm.q, 4503599627370496.0);
+#pragma unroll
+    for (int k = 0; k < 8; k++) sm[sbase ^ swz(k << PW)] = d2u_off(FWD ? x[k] : reduce_dd(x[k], fm), off);
+  } else {
   u64 x[8];
 #pragma unroll
   for (int k = 0; k < 8; k++) x[k] = sm[sbase ^ swz(k << PW)];
@@ -156,37 +200,38 @@ DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 
       const ulonglong2 w = s == 2 ? t2 : (s == 1 ? t1[k >> 2] : t0[k >> 1]);
       if (FWD) {
         const u64 X = LAZY ? x[k] : csub(x[k], q2);
-        const u64 T = F64 ? mulmod_f64(x[k2], w.x, w.y, fm) : shoup_lazy(x[k2], w.x, w.y, q);
+        const u64 T = shoup_lazy(x[k2], w.x, w.y, q);
         x[k] = X + T;
         x[k2] = X - T + q2;
       } else {
         const u64 U = x[k], V = x[k2];
         x[k] = csub(U + V, q2);
-        x[k2] = F64 ? mulmod_f64(U - V + q2, w.x, w.y, fm) : shoup_lazy(U - V + q2, w.x, w.y, q);
+        x[k2] = shoup_lazy(U - V + q2, w.x, w.y, q);
       }
     }
   }
 #pragma unroll
   for (int k = 0; k < 8; k++) sm[sbase ^ swz(k << PW)] = x[k];
+  }
 }
 
 template <bool FWD, bool LAZY, int LT, int LO, int NB, int DONE, bool F64 = false>
-DEVI void tile_rounds_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid) {
+DEVI void tile_rounds_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid, u64 f64 = 0) {
   if constexpr (DONE < NB) {
     constexpr int take = NB - DONE < 3 ? NB - DONE : 3;
     constexpr int cur = FWD ? LO + NB - DONE : LO + DONE;         // FWD: exclusive top; INV: inclusive bottom
     constexpr int p = FWD ? cur - take : cur;
     constexpr int pw = p < LT - 3 ? p : LT - 3;
-    if (tid < (1 << (LT - 3))) tile_round_ct<FWD, LAZY, pw, p - pw, p - pw + take, F64>(sm, G, tw, q, q2, tid);
+    if (tid < (1 << (LT - 3))) tile_round_ct<FWD, LAZY, pw, p - pw, p - pw + take, F64>(sm, G, tw, q, q2, tid, f64);
     __syncthreads();
-    tile_rounds_ct<FWD, LAZY, LT, LO, NB, DONE + take, F64>(sm, G, tw, q, q2, tid);
+    tile_rounds_ct<FWD, LAZY, LT, LO, NB, DONE + take, F64>(sm, G, tw, q, q2, tid, f64);
   }
 }
 
 // runtime round (toy ring degrees and any geometry without a compile-time instance)
 template <bool FWD, bool F64>
-DEVI void tile_round_rt(u64 *sm, const TileGeo &G, int pw, int s_lo, int s_hi, const ShoupC *tw, u64 q, u64 q2, int tid) {
-  const F64Mod fm = f64mod(q);
+DEVI void tile_round_rt(u64 *sm, const TileGeo &G, int pw, int s_lo, int s_hi, const ShoupC *tw, u64 q, u64 q2, int tid, u64 f64) {
+  const F64Mod fm = f64mod(q, f64);
   const int ebase = ((tid >> pw) << (pw + 3)) | (tid & ((1 << pw) - 1));
   u64 x[8];
 #pragma unroll
@@ -221,9 +266,9 @@ DEVI void tile_round_rt(u64 *sm, const TileGeo &G, int pw, int s_lo, int s_hi, c
 // compile-time schedule over active tile bits [LO, LO+NB) of a 2^LT-element tile; picks the lazy forward butterflies
 // for q < 2^58.  Every thread of the block must call this (it synchronises).
 template <bool FWD, int LT, int LO, int NB>
-DEVI void tile_transform_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, int tid, bool f64) {
+DEVI void tile_transform_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, int tid, u64 f64) {
   const u64 q2 = q + q;
-  if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, true>(sm, G, tw, q, q2, tid);
+  if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, true>(sm, G, tw, q, q2, tid, f64);
   else if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
   else tile_rounds_ct<FWD, false, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
 }
@@ -232,7 +277,7 @@ DEVI void tile_transform_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, 
 // 4..8 = column pass with GEO stages over tiles of 2^(GEO+4) elements (16 columns).
 // Every thread of the block must call this (it synchronises).  Outputs: forward < 33q (use fullred), inverse < 2q.
 template <bool FWD, int GEO>
-DEVI void tile_transform(u64 *sm, const TileGeo &G, int lo, int nb, const ShoupC *tw, u64 q, int tid, bool f64) {
+DEVI void tile_transform(u64 *sm, const TileGeo &G, int lo, int nb, const ShoupC *tw, u64 q, int tid, u64 f64) {
   const u64 q2 = q + q;
   if constexpr (GEO == 0) {
     const bool active = tid < (1 << (G.lt - 3));
@@ -242,7 +287,7 @@ DEVI void tile_transform(u64 *sm, const TileGeo &G, int lo, int nb, const ShoupC
         int take = cur - lo < 3 ? cur - lo : 3;
         int p = cur - take;
         int pw = p < G.lt - 3 ? p : G.lt - 3;
-        if (active) { if (f64) tile_round_rt<true, true>(sm, G, pw, p - pw, cur - pw, tw, q, q2, tid); else tile_round_rt<true, false>(sm, G, pw, p - pw, cur - pw, tw, q, q2, tid); }
+        if (active) { if (f64) tile_round_rt<true, true>(sm, G, pw, p - pw, cur - pw, tw, q, q2, tid, f64); else tile_round_rt<true, false>(sm, G, pw, p - pw, cur - pw, tw, q, q2, tid, 0); }
         __syncthreads();
         cur = p;
       }
@@ -251,14 +296,14 @@ DEVI void tile_transform(u64 *sm, const TileGeo &G, int lo, int nb, const ShoupC
       while (cur < lo + nb) {
         int take = lo + nb - cur < 3 ? lo + nb - cur : 3;
         int pw = cur < G.lt - 3 ? cur : G.lt - 3;
-        if (active) { if (f64) tile_round_rt<false, true>(sm, G, pw, cur - pw, cur + take - pw, tw, q, q2, tid); else tile_round_rt<false, false>(sm, G, pw, cur - pw, cur + take - pw, tw, q, q2, tid); }
+        if (active) { if (f64) tile_round_rt<false, true>(sm, G, pw, cur - pw, cur + take - pw, tw, q, q2, tid, f64); else tile_round_rt<false, false>(sm, G, pw, cur - pw, cur + take - pw, tw, q, q2, tid, 0); }
         __syncthreads();
         cur += take;
       }
     }
   } else {
     constexpr int LT = GEO == 1 ? FENC_ROW_LT : GEO + 4, LO = GEO == 1 ? 0 : 4, NB = GEO == 1 ? 8 : GEO;
-    if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, true>(sm, G, tw, q, q2, tid);
+    if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, true>(sm, G, tw, q, q2, tid, f64);
     else if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
     else tile_rounds_ct<FWD, false, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
   }

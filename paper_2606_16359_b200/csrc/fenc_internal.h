@@ -2,6 +2,7 @@
 // Nothing here is shared with oracle/ (the CPU oracle is an independent program).
 #pragma once
 #include <stddef.h>
+#include <string.h>
 #include <stdint.h>
 
 #include <vector>
@@ -25,7 +26,8 @@ struct ModConst {  // one per modulus, device global memory
   u64 r2;          // 2^128 mod q: mont_mul(x, r2) = x 2^64 mod q
   u64 mask;        // 2^ceil(log2 q) - 1 (uniform rejection sampler)
   u64 qbar;        // floor(2^64 / q): full reduction of a lazy 64-bit value
-  u64 f64;         // != 0: q < 2^45, the twiddle tables of this modulus hold fp64 pairs (fenc_device.cuh mulmod_f64)
+  u64 f64;         // != 0: q < 2^45, the bits of (double)(1/q); the twiddle tables of this modulus hold fp64 pairs
+                   // (fenc_device.cuh mulmod_dd)
   u64 pad[2];
 };
 
@@ -176,7 +178,8 @@ u64 shoup(u64 c, u64 q);    // floor(c 2^64 / q)
 u64 to_mont(u64 c, u64 q);  // c 2^64 mod q
 u64 neg_qinv(u64 q);        // -q^{-1} mod 2^64
 void build_twiddles(u64 q, u64 psi, int logN, ShoupC *fwd, ShoupC *inv);
-bool f64_modulus(u64 q);  // butterflies of this modulus multiply on the FP64 pipe (twiddle tables hold fp64 pairs)
+bool f64_modulus(u64 q);
+inline u64 double_bits(double d) { u64 b; memcpy(&b, &d, 8); return b; }  // butterflies of this modulus multiply on the FP64 pipe (twiddle tables hold fp64 pairs)
 u64 mix64(u64 z);
 u64 stream_key(u64 seed, u64 purpose, u64 a, u64 b, u64 c);
 void sample_ternary(u64 key, int N, int64_t *out);

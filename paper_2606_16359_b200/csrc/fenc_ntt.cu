@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(256, 5) intt_rowpass_kernel(InttRowP p) {
     });
   }
   __syncthreads();
-  tile_transform<false, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid, p.mods[rd.mod].f64 != 0);
+  tile_transform<false, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid, p.mods[rd.mod].f64);
   u64 *dst = p.dst + (size_t)b * p.dst_bstride + (size_t)rd.dst_row * N;
   tile_drain(sm, T, tid, nth, [&](int e, u64 v) { dst[G.gidx(e)] = v; });
 }
@@ -115,7 +115,7 @@ __global__ void __launch_bounds__(512, 3) intt_colpass_kernel(InttColP p) {
   tile_fill(sm, T, tid, nth, [&](int e) { return dst[G.gidx(e)]; });
   __syncthreads();
   const u64 q = p.mods[rd.mod].q;
-  tile_transform<false, GEO>(sm, G, p.g.lc_col, p.g.bcol, p.tw + (size_t)rd.mod * N, q, tid, p.mods[rd.mod].f64 != 0);
+  tile_transform<false, GEO>(sm, G, p.g.lc_col, p.g.bcol, p.tw + (size_t)rd.mod * N, q, tid, p.mods[rd.mod].f64);
   const ShoupC sc = p.scale[blockIdx.y];
   tile_drain(sm, T, tid, nth, [&](int e, u64 v) { dst[G.gidx(e)] = shoup_mul(v, sc.c, sc.cs, q); });
 }
@@ -211,7 +211,7 @@ __global__ void __launch_bounds__(128, 5) convert_cols_kernel(ConvColP p) {
     u64 *Y = smem + (size_t)s * T;
     const int mod = (MERGED && s == n_conv) ? cg.pad[1] : cg.src_mod + s;
     const u64 q = p.mods[mod].q;
-    tile_transform_ct<false, LT, LC, BCOL>(Y, G, p.tw_inv + (size_t)mod * N, q, tid, p.mods[mod].f64 != 0);
+    tile_transform_ct<false, LT, LC, BCOL>(Y, G, p.tw_inv + (size_t)mod * N, q, tid, p.mods[mod].f64);
     const ShoupC sc = p.scale[cg.scale_off + s];
 #pragma unroll
     for (int i = 0; i < 8; i++) {
@@ -245,7 +245,7 @@ __global__ void __launch_bounds__(128, 5) convert_cols_kernel(ConvColP p) {
 #pragma unroll
     for (int i = 0; i < 8; i++) W[swz(tid + i * NTH)] = v[i];
     __syncthreads();
-    tile_transform_ct<true, LT, LC, BCOL>(W, G, p.tw_fwd + (size_t)rd.mod * N, mc.q, tid, mc.f64 != 0);
+    tile_transform_ct<true, LT, LC, BCOL>(W, G, p.tw_fwd + (size_t)rd.mod * N, mc.q, tid, mc.f64);
     u64 *dst = p.tmp + (size_t)b * p.tmp_bstride + (size_t)rd.dst_row * N;
     tile_drain(W, T, tid, NTH, [&](int e, u64 v) { dst[G.gidx(e)] = v; });  // lazy, below 33q
     __syncthreads();
@@ -339,7 +339,7 @@ __global__ void __launch_bounds__(512, 2) ntt_colpass_kernel(NttColP p) {
     tile_fill(sm, T, tid, nth, [&](int e) { return __ldg(src + G.gidx(e)); });
   }
   __syncthreads();
-  tile_transform<true, GEO>(sm, G, p.g.lc_col, p.g.bcol, p.tw + (size_t)rd.mod * N, mc.q, tid, mc.f64 != 0);
+  tile_transform<true, GEO>(sm, G, p.g.lc_col, p.g.bcol, p.tw + (size_t)rd.mod * N, mc.q, tid, mc.f64);
   u64 *dst = p.dst + (size_t)b * p.dst_bstride + (size_t)rd.dst_row * N;
   tile_drain(sm, T, tid, nth, [&](int e, u64 v) { dst[G.gidx(e)] = v; });  // lazy, below 33q
 }
@@ -361,7 +361,7 @@ __global__ void __launch_bounds__(256, 4) ntt_rowpass_kernel(NttRowP p) {
   tile_fill(sm, T, tid, nth, [&](int e) { return src[G.gidx(e)]; });
   __syncthreads();
   const ModConst mc = p.mods[rd.mod];
-  tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, mc.q, tid, mc.f64 != 0);
+  tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, mc.q, tid, mc.f64);
   u64 *dst = p.dst + (size_t)b * p.dst_bstride + (size_t)rd.dst_row * N;
   tile_drain(sm, T, tid, nth, [&](int e, u64 v) { dst[G.gidx(e)] = fullred(v, mc.q, mc.qbar); });
 }
@@ -430,7 +430,7 @@ __global__ void __launch_bounds__(256, 2) ntt_rows_keymac_kernel(KeyMacP p) {
       const u64 *src = p.tmp + (size_t)b * p.tmp_bstride + (size_t)ti * N;
       tile_fill(sm, T, tid, nth, [&](int e) { return src[G.gidx(e)]; });
       __syncthreads();
-      tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)mod * N, mc.q, tid, mc.f64 != 0);
+      tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)mod * N, mc.q, tid, mc.f64);
     }
     // the key words (and, inside the digit, the permuted input words) of 4 elements are loaded together, then used
 #pragma unroll
@@ -522,7 +522,7 @@ __global__ void __launch_bounds__(256, 4) ntt_rows_divide_kernel(DivideP p) {
   __syncthreads();
   const ModConst mq = p.mods[rd.mod];
   const u64 q = mq.q;
-  tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid, mq.f64 != 0);
+  tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid, mq.f64);
   const ShoupC mc = p.mul[rd.mod];
   u64 *dst = it.out + (size_t)rd.dst_row * N;
 #pragma unroll
