@@ -449,7 +449,8 @@ __global__ void __launch_bounds__(256, 2) ntt_rows_keymac_kernel(KeyMacP p) {
 #pragma unroll
       for (int i = 0; i < HB; i++) {
         if (tid + (h + i) * nth < T) {
-          const u64 xx = ti >= 0 ? fullred(x[i], mc.q, mc.qbar) : x[i];
+          // fp64 rows: the transform's output is below 2^52 with q < 2^45, beta x k stays far below q 2^64: no reduction
+          const u64 xx = (ti >= 0 && !mc.f64) ? fullred(x[i], mc.q, mc.qbar) : x[i];
           mac128(a0l[h + i], a0h[h + i], xx, vb[i]);
           mac128(a1l[h + i], a1h[h + i], xx, va[i]);
         }
@@ -524,19 +525,22 @@ __global__ void __launch_bounds__(256, 4) ntt_rows_divide_kernel(DivideP p) {
   const u64 q = mq.q;
   tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid, mq.f64);
   const ShoupC mc = p.mul[rd.mod];
+  const F64Mod fm = f64mod(q, mq.f64);
   u64 *dst = it.out + (size_t)rd.dst_row * N;
 #pragma unroll
   for (int i = 0; i < 8; i++) {
     const int e = tid + i * nth;
     if (e < T) {
-      const u64 x = fullred(sm[swz(e)], q, mq.qbar);
+      // fp64 rows: X mod q as v - rint(v/q) q + q in (0, 2q) on the FP64 pipe; the Shoup multiply takes any 64-bit input
+      const bool fp = mq.f64 != 0;
+      const u64 x = fp ? d2u_off(reduce_dd(u2d52(sm[swz(e)]), fm), fm.q + 4503599627370496.0) : fullred(sm[swz(e)], q, mq.qbar);
       u64 v;
       if (MERGED) {
         const ShoupC m2 = p.mul2[rd.mod];
         v = addmod(shoup_mul(mi[i], m2.c, m2.cs, q), ad[i], q);
-        v = shoup_mul(submod(v, x, q), mc.c, mc.cs, q);
+        v = shoup_mul(fp ? v + 2 * q - x : submod(v, x, q), mc.c, mc.cs, q);
       } else {
-        v = shoup_mul(submod(mi[i], x, q), mc.c, mc.cs, q);
+        v = shoup_mul(fp ? mi[i] + 2 * q - x : submod(mi[i], x, q), mc.c, mc.cs, q);
         v = addmod(v, ad[i], q);
       }
       dst[G.gidx(e)] = v;
