@@ -244,6 +244,7 @@ LevelPlan *get_plan(fenc_ctx *ctx, int L) {
   std::vector<RowDesc> rows_in(L), rows_up, rows_p(2 * np), rows_down(2 * L), rows_div(2 * L), rows_ct(2 * L);
   std::vector<ShoupC> scale_in(L), scale_p(2 * np), mul_pinv(A, ShoupC{0, 0}), scale_ct(2 * L);
   std::vector<u64> bc_up, bc_down((size_t)L * np);
+  std::vector<ShoupC> bc_up_f64, bc_rs_f64;
   std::vector<int> tmp_index((size_t)P.beta * E, -1);
   std::vector<ConvGroup> groups_up, groups_down, groups_rs;
   for (int j = 0; j < P.beta; j++) {
@@ -256,7 +257,9 @@ LevelPlan *get_plan(fenc_ctx *ctx, int L) {
       rows_in[i] = RowDesc{i, i, i, 0, 0, {0, 0, 0}};
       scale_in[i] = shoupc(fh::mulmod(ninv, fh::invmod(qhat, qi), qi), qi);
     }
-    groups_up.push_back(ConvGroup{lo, lo, hi - lo, lo, (int)rows_up.size(), E - (hi - lo), {0, 0}});
+    bool src_f64 = true;
+    for (int i = lo; i < hi; i++) src_f64 = src_f64 && fh::f64_modulus(mod[i]);
+    groups_up.push_back(ConvGroup{lo, lo, hi - lo, lo, (int)rows_up.size(), E - (hi - lo), {src_f64 ? 2 : 0, 0}});
     P.n_src_up = std::max(P.n_src_up, hi - lo);
     for (int t = 0; t < E; t++) {
       if (t >= lo && t < hi) continue;
@@ -267,6 +270,7 @@ LevelPlan *get_plan(fenc_ctx *ctx, int L) {
         for (int i2 = lo; i2 < hi; i2++)
           if (i2 != i) c = fh::mulmod(c, mod[i2] % T, T);
         bc_up.push_back(fh::to_mont(c, T));
+        bc_up_f64.push_back(ShoupC{fh::double_bits((double)c), fh::double_bits((double)((long double)c / (long double)T))});
       }
       tmp_index[(size_t)j * E + t] = rd.dst_row;
       rows_up.push_back(rd);
@@ -303,7 +307,7 @@ LevelPlan *get_plan(fenc_ctx *ctx, int L) {
   }
   for (int c = 0; c < 2; c++) {
     groups_down.push_back(ConvGroup{c * np, nq, np, c * np, c * L, L, {0, 0}});
-    groups_rs.push_back(ConvGroup{c, L - 1, 1, c, c * (L - 1), L - 1, {0, 0}});
+    groups_rs.push_back(ConvGroup{c, L - 1, 1, c, c * (L - 1), L - 1, {(L >= 2 && fh::f64_modulus(mod[L - 1])) ? 2 : 0, 0}});
   }
   P.d_groups_up = upload_owned(ctx, P.owned, groups_up);
   P.d_groups_down = upload_owned(ctx, P.owned, groups_down);
@@ -312,6 +316,7 @@ LevelPlan *get_plan(fenc_ctx *ctx, int L) {
   P.d_scale_in = upload_owned(ctx, P.owned, scale_in);
   P.d_rows_up = upload_owned(ctx, P.owned, rows_up);
   P.d_bc_up = upload_owned(ctx, P.owned, bc_up);
+  P.d_bc_up_f64 = upload_owned(ctx, P.owned, bc_up_f64);
   P.d_tmp_index = upload_owned(ctx, P.owned, tmp_index);
   P.d_rows_p = upload_owned(ctx, P.owned, rows_p);
   P.d_scale_p = upload_owned(ctx, P.owned, scale_p);
@@ -335,6 +340,7 @@ LevelPlan *get_plan(fenc_ctx *ctx, int L) {
     }
     for (int t = 0; t < L1; t++) {
       bc_rs.push_back(fh::to_mont(1, mod[t]));
+      bc_rs_f64.push_back(ShoupC{fh::double_bits(1.0), fh::double_bits(1.0 / (double)mod[t])});
       mul_ql[t] = shoupc(fh::invmod(ql % mod[t], mod[t]), mod[t]);
     }
     for (int c = 0; c < 2; c++)
@@ -372,6 +378,7 @@ LevelPlan *get_plan(fenc_ctx *ctx, int L) {
   P.d_scale_rs = upload_owned(ctx, P.owned, rs_scale);
   P.d_rows_rs_up = upload_owned(ctx, P.owned, rs_up);
   P.d_bc_rs = upload_owned(ctx, P.owned, bc_rs);
+  P.d_bc_rs_f64 = upload_owned(ctx, P.owned, bc_rs_f64);
   P.d_rows_rs_div = upload_owned(ctx, P.owned, rs_div);
   P.d_mul_qlinv = upload_owned(ctx, P.owned, mul_ql);
   cudaStreamSynchronize(ctx->stream);  // host vectors go out of scope
@@ -422,7 +429,7 @@ fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items, bool r
     if (fused_up) {
       CUDA_OK(ctx, k_intt_rows_only(k, d_items, nullptr, 0, true, y, (size_t)L * N, P->d_rows_in, L, nb));
       CUDA_OK(ctx, k_convert_cols(k, y, (size_t)L * N, P->d_groups_up, P->beta, P->n_src_up, P->d_scale_in, P->d_bc_up, P->d_rows_up,
-                                  P->n_up, tmp, (size_t)P->n_up * N, nb, ctx->lazy_q));
+                                  P->n_up, tmp, (size_t)P->n_up * N, nb, ctx->lazy_q, nullptr, P->d_bc_up_f64));
     } else {
       CUDA_OK(ctx, k_intt(k, d_items, nullptr, 0, true, y, (size_t)L * N, P->d_rows_in, L, P->d_scale_in, nb));
       CUDA_OK(ctx, k_ntt_cols_bconv(k, y, (size_t)L * N, P->d_bc_up, tmp, (size_t)P->n_up * N, P->d_rows_up, P->n_up, nb, L, ctx->lazy_q));
@@ -480,7 +487,7 @@ fenc_status rescale_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items) {
     if (ctx->logN >= 12) {
       CUDA_OK(ctx, k_intt_rows_only(k, d_items, nullptr, 0, false, yR, 2 * N, P->d_rows_rs_in, 2, nb));
       CUDA_OK(ctx, k_convert_cols(k, yR, 2 * N, P->d_groups_rs, 2, 1, P->d_scale_rs, P->d_bc_rs, P->d_rows_rs_up, 2 * L1, tmp2,
-                                  (size_t)2 * L1 * N, nb, ctx->lazy_q));
+                                  (size_t)2 * L1 * N, nb, ctx->lazy_q, nullptr, P->d_bc_rs_f64));
     } else {
       CUDA_OK(ctx, k_intt(k, d_items, nullptr, 0, false, yR, 2 * N, P->d_rows_rs_in, 2, P->d_scale_rs, nb));
       CUDA_OK(ctx, k_ntt_cols_bconv(k, yR, 2 * N, P->d_bc_rs, tmp2, (size_t)2 * L1 * N, P->d_rows_rs_up, 2 * L1, nb, 2, ctx->lazy_q));

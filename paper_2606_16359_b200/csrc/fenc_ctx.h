@@ -18,6 +18,7 @@ struct LevelPlan {
   ShoupC *d_scale_in;        // [L] N^-1 * Qhat_{j,t}^-1 mod q_t (the ModUp pre-scaling folded into the iNTT)
   RowDesc *d_rows_up;        // [n_up] ModUp + forward pass 1 job rows
   u64 *d_bc_up;              // Montgomery-form (Q_j / q_i mod t) constants, indexed by RowDesc.aux2 + s
+  ShoupC *d_bc_up_f64 = nullptr, *d_bc_rs_f64 = nullptr;  // the same constants (plain) as fp64 pairs {c, c/t}
   int *d_tmp_index;          // [beta*E] -> row of the ModUp temp or -1
   RowDesc *d_rows_p;         // [2 np] iNTT of the special limbs of both accumulators
   ShoupC *d_scale_p;         // [2 np] N^-1 * Phat_i^-1 mod p_i

@@ -121,7 +121,9 @@ int k_intt_rows_only(const KCtx &k, const BatchItem *items, const u64 *src, size
 // Returns -2 when the group does not fit shared memory (the caller falls back to k_intt + k_ntt_cols_bconv).
 int k_convert_cols(const KCtx &k, u64 *y, size_t y_bstride, const ConvGroup *groups, int n_groups, int n_src_max,
                    const ShoupC *scale, const u64 *bc, const RowDesc *rows, int n_tgt_total, u64 *tmp, size_t tmp_bstride,
-                   int n_batch, int max_terms, const ShoupC *merged_pinv = nullptr);
+                   int n_batch, int max_terms, const ShoupC *merged_pinv = nullptr, const ShoupC *bc_f64 = nullptr);
+// (bc_f64: fp64 pairs {(double) c, (double)(c / t)} of the PLAIN constants, same indexing as bc; used for groups with
+//  pad[0] & 2 -- all source moduli fp64 ones -- and fp64 targets)
 // (merged_pinv != nullptr: ModDown merged with the rescale; every group carries one extra source row, the inverse-
 //  transformed dropped limb of modulus index groups[g].pad[1], and the targets receive V_t P^-1 + (out_l mod t))
 // forward pass 2 (row stages) fused with the evaluation-key inner product (a4) over E = L + np target rows.

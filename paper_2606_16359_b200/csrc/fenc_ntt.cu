@@ -164,6 +164,7 @@ struct ConvColP {
   u64 *y; size_t y_bstride; const ConvGroup *groups; const ShoupC *scale; const u64 *bc; const RowDesc *rows;
   u64 *tmp; size_t tmp_bstride; const ModConst *mods; const ShoupC *tw_fwd; const ShoupC *tw_inv; int logN, brow, max_terms;
   const ShoupC *mulc;  // MERGED: P^-1 mod q_t
+  const ShoupC *bc_f64;  // {(double) c, (double)(c / t)} per entry of bc, used when source and target moduli are fp64 ones
 };
 // sum over the first n source tiles of Y_s[e] * bc[s] for this thread's eight elements, Montgomery-reduced: canonical
 template <int T, int NTH>
@@ -185,6 +186,25 @@ DEVI void conv_dot(const u64 *smem, int n, const u64 *bc, const ModConst &mc, in
   }
 #pragma unroll
   for (int i = 0; i < 8; i++) out[i] = addmod(r[i], mont_redc(lo[i], hi[i], mc.q, mc.qinv_neg), mc.q);
+}
+// The same sum on the FP64 pipe (groups flagged pad[0] & 2: every source modulus below 2^45, and an fp64 target): each
+// term y c - rint(y c / t) t is an exact integer in (-t, t); the sum plus n t is a non-negative representative below
+// 2 n t, which is all the forward fp64 butterflies ask of their input.
+template <int T, int NTH>
+DEVI void conv_dot_f64(const u64 *smem, int n, const ShoupC *bc, const F64Mod &fm, int tid, u64 (&out)[8]) {
+  double acc[8];
+#pragma unroll
+  for (int i = 0; i < 8; i++) acc[i] = 0.0;
+  for (int s = 0; s < n; s++) {
+    const ulonglong2 cc = __ldg(reinterpret_cast<const ulonglong2 *>(bc + s));
+    const double c = __longlong_as_double((long long)cc.x), cq = __longlong_as_double((long long)cc.y);
+    const u64 *Y = smem + (size_t)s * T;
+#pragma unroll
+    for (int i = 0; i < 8; i++) acc[i] = __dadd_rn(acc[i], mulmod_dd(u2d52(Y[swz(tid + i * NTH)]), c, cq, fm));
+  }
+  const double off = __fma_rn((double)n, fm.q, 4503599627370496.0);
+#pragma unroll
+  for (int i = 0; i < 8; i++) out[i] = d2u_off(acc[i], off);
 }
 // MERGED (ModDown followed by the rescale): the group's last source tile is Z = iNTT(acc[l] P^-1 + add[l]) of
 // the limb l = q_{L-1} that the rescale drops (modulus index cg.pad[1]).  With V_t = sum_i y_i (Phat_i mod t):
@@ -236,7 +256,8 @@ __global__ void __launch_bounds__(128, 5) convert_cols_kernel(ConvColP p) {
     const RowDesc rd = p.rows[cg.tgt_start + t];
     const ModConst mc = p.mods[rd.mod];
     u64 v[8];
-    conv_dot<T, NTH>(smem, n_conv, p.bc + rd.aux2, mc, p.max_terms, tid, v);
+    if (!MERGED && p.bc_f64 && (cg.pad[0] & 2) && mc.f64) conv_dot_f64<T, NTH>(smem, n_conv, p.bc_f64 + rd.aux2, f64mod(mc.q, mc.f64), tid, v);
+    else conv_dot<T, NTH>(smem, n_conv, p.bc + rd.aux2, mc, p.max_terms, tid, v);
     if (MERGED) {
       const ShoupC pt = p.mulc[rd.mod];
 #pragma unroll
@@ -254,14 +275,14 @@ __global__ void __launch_bounds__(128, 5) convert_cols_kernel(ConvColP p) {
 
 int k_convert_cols(const KCtx &k, u64 *y, size_t y_bstride, const ConvGroup *groups, int n_groups, int n_src_max,
                    const ShoupC *scale, const u64 *bc, const RowDesc *rows, int n_tgt_total, u64 *tmp, size_t tmp_bstride,
-                   int n_batch, int max_terms, const ShoupC *merged_pinv) {
+                   int n_batch, int max_terms, const ShoupC *merged_pinv, const ShoupC *bc_f64) {
   if (n_groups == 0 || n_batch == 0) return 0;
   const NttGeom &g = k.geom;
   if (g.logN < 12) return -2;
   const size_t smem = (size_t)(n_src_max + 1) * 1024 * sizeof(u64);
   if (smem > 200 * 1024) return -2;
   ConvColP p{y, y_bstride, groups, scale, bc, rows, tmp, tmp_bstride, k.d_mods, k.d_tw_fwd, k.d_tw_inv, g.logN, g.brow, max_terms,
-             merged_pinv};
+             merged_pinv, bc_f64};
   dim3 grid(k.N >> 10, n_groups, n_batch);
   // algorithmic bytes: every target row written once (+ the sources, counted by the caller's row pass); butterflies of
   // the forward column stages of every target (the inverse ones of the sources are the smaller part)
