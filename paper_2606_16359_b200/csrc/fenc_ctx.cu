@@ -17,28 +17,66 @@ fenc_status fail(fenc_ctx *ctx, fenc_status st, const char *fmt, ...) {
   return st;
 }
 
-void *dalloc(fenc_ctx *ctx, size_t bytes) {
-  if (bytes == 0) bytes = 256;
+// Device memory comes from the caller's allocator (a callback into the host framework) or cudaMalloc.  Blocks up to
+// POOL_BLOCK_MAX are kept in per-size free lists when released and handed out again without leaving the library: a
+// layer creates and drops hundreds of ciphertext-sized buffers per call, the same sizes every step, and the callbacks
+// alone made the FC layers host-bound.  Everything the library enqueues runs on the context's stream, so a block reused
+// by a later call is ordered after the work that last touched it.
+static const size_t POOL_BLOCK_MAX = (size_t)64 << 20, POOL_BYTES_MAX = (size_t)4 << 30;
+static void *raw_alloc(fenc_ctx *ctx, size_t bytes) {
   void *p = nullptr;
   if (ctx->dev_alloc) p = ctx->dev_alloc(bytes, ctx->user);
   else if (cudaMalloc(&p, bytes) != cudaSuccess) p = nullptr;
+  if (!p) (void)cudaGetLastError();
+  return p;
+}
+static void raw_free(fenc_ctx *ctx, void *p) {
+  if (ctx->dev_free) ctx->dev_free(p, ctx->user);
+  else cudaFree(p);
+}
+void pool_release(fenc_ctx *ctx) {
+  for (auto &kv : ctx->pool)
+    for (void *p : kv.second) raw_free(ctx, p);
+  ctx->pool.clear();
+  ctx->pool_bytes = 0;
+}
+void *dalloc(fenc_ctx *ctx, size_t bytes) {
+  if (bytes == 0) bytes = 256;
+  void *p = nullptr;
+  if (bytes <= POOL_BLOCK_MAX) {
+    auto it = ctx->pool.find(bytes);
+    if (it != ctx->pool.end() && !it->second.empty()) {
+      p = it->second.back();
+      it->second.pop_back();
+      ctx->pool_bytes -= bytes;
+    }
+  }
+  if (!p) p = raw_alloc(ctx, bytes);
+  if (!p && ctx->pool_bytes) {  // out of memory with blocks parked in the pool: give them back and retry
+    pool_release(ctx);
+    p = raw_alloc(ctx, bytes);
+  }
   if (p) {
     ctx->live[p] = bytes;
     ctx->dev_bytes += bytes;
-  } else {
-    (void)cudaGetLastError();
   }
   return p;
 }
 void dfree(fenc_ctx *ctx, void *p) {
   if (!p) return;
+  size_t bytes = 0;
   auto it = ctx->live.find(p);
   if (it != ctx->live.end()) {
-    ctx->dev_bytes -= it->second;
+    bytes = it->second;
+    ctx->dev_bytes -= bytes;
     ctx->live.erase(it);
   }
-  if (ctx->dev_free) ctx->dev_free(p, ctx->user);
-  else cudaFree(p);
+  if (bytes && bytes <= POOL_BLOCK_MAX && ctx->pool_bytes + bytes <= POOL_BYTES_MAX) {
+    ctx->pool[bytes].push_back(p);
+    ctx->pool_bytes += bytes;
+    return;
+  }
+  raw_free(ctx, p);
 }
 void *workspace(fenc_ctx *ctx, size_t bytes) {
   if (bytes > ctx->ws_bytes) {
@@ -52,7 +90,7 @@ void *workspace(fenc_ctx *ctx, size_t bytes) {
 // Descriptor arrays go through a ring of pinned host slots: a copy from pageable memory would synchronise the stream
 // before every batch (and stall the host-side enqueue of the next kernels behind all queued GPU work).
 static const size_t DESC_SLOT = (size_t)1 << 20;
-static const int DESC_SLOTS = 8;
+static const int DESC_SLOTS = FENC_DESC_SLOTS;
 char *DescStage::commit() {
   size_t need = (host.size() + 255) & ~(size_t)255;
   if (need > ctx->desc_bytes) {
@@ -196,11 +234,12 @@ extern "C" void fenc_ctx_free(fenc_ctx *ctx) {
     for (void *p : kv.second->owned) dfree(ctx, p);
   dfree(ctx, ctx->ws), dfree(ctx, ctx->desc_buf);
   if (ctx->desc_pinned) {
-    for (int i = 0; i < 8; i++) cudaEventDestroy(ctx->desc_ev[i]);
+    for (int i = 0; i < FENC_DESC_SLOTS; i++) cudaEventDestroy(ctx->desc_ev[i]);
     cudaFreeHost(ctx->desc_pinned);
   }
   dfree(ctx, ctx->d_mods), dfree(ctx, ctx->d_tw_fwd), dfree(ctx, ctx->d_tw_inv);
   dfree(ctx, ctx->d_ident_rows), dfree(ctx, ctx->d_ninv), dfree(ctx, ctx->d_ident_mod);
+  pool_release(ctx);
   delete ctx;
 }
 extern "C" const char *fenc_last_error(fenc_ctx *ctx) { return ctx ? ctx->err.c_str() : "null context"; }

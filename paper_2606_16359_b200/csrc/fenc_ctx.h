@@ -10,6 +10,8 @@
 
 #include "fenc_internal.h"
 
+#define FENC_DESC_SLOTS 32  // pinned 1 MiB slots feeding the descriptor buffer: how many batches the host may run ahead
+
 // Per-level (number of ciphertext limbs L) tables of the hybrid key switch and of the rescale (R2.6, R2.8).
 struct LevelPlan {
   int L, E, beta, n_up;      // E = L + np target rows; n_up = rows of the ModUp temp = beta*E - L
@@ -72,13 +74,15 @@ struct fenc_ctx {
   std::string err;
   std::map<int, std::unique_ptr<LevelPlan>> plans;
   std::map<void *, size_t> live;    // device pointer -> bytes (accounting)
+  std::map<size_t, std::vector<void *>> pool;  // released blocks by size, reused by dalloc (fenc_ctx.cu)
+  size_t pool_bytes = 0;
   void *ws = nullptr;               // grow-only key-switch workspace
   size_t ws_bytes = 0;
   void *desc_buf = nullptr;         // device staging for per-call descriptor arrays
   size_t desc_bytes = 0;
   void *desc_pinned = nullptr;      // ring of pinned host slots feeding desc_buf
-  cudaEvent_t desc_ev[8] = {};
-  bool desc_used[8] = {};
+  cudaEvent_t desc_ev[FENC_DESC_SLOTS] = {};
+  bool desc_used[FENC_DESC_SLOTS] = {};
   unsigned desc_next = 0;
   std::map<std::string, std::shared_ptr<LinGraph>> graphs;
 };

@@ -427,8 +427,11 @@ struct KeyMacP {
   const BatchItem *items; const int *tmp_index; const u64 *tmp; size_t tmp_bstride; u64 *acc; size_t acc_bstride;
   const ModConst *mods; const ShoupC *tw; NttGeom g; int L, E, beta, A, nq, n_batch;
 };
+// 3 blocks of 128 threads per SM: 168 registers hold the 32 128-bit accumulators and the fp64 butterflies without
+// spilling (4 blocks at 128 registers spill 160 bytes and run 10 % slower)
+#define KEYMAC_BLOCKS 3
 template <int EPT, int GEO>  // elements per thread
-__global__ void __launch_bounds__(256, 2) ntt_rows_keymac_kernel(KeyMacP p) {
+__global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? KEYMAC_BLOCKS : 2) ntt_rows_keymac_kernel(KeyMacP p) {
   extern __shared__ u64 sm[];
   const int tid = threadIdx.x;
   // batch index fastest: blockIdx.x = tile * n_batch + b
