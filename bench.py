@@ -310,8 +310,8 @@ def run_ours(args, rank, world):
     if t_ops and alu_ach / bfly_peak >= hbm_ach / peaks["hbm_gbs"]:
         roofline = {"bound": "alu", "kernel": top, "achieved": round(alu_ach / 1e9, 2), "peak": round(bfly_peak / 1e9, 2),
                     "unit": "G modular butterflies/s", "frac": round(alu_ach / bfly_peak, 4), "traffic": None,
-                    "peak_source": "measured live: register-only Shoup butterflies of this library on all SMs "
-                                   "(fenc_measure_alu_peak); 32-bit IMAD peak %.2f T lane-ops/s" % (imad_peak / 1e12),
+                    "peak_source": "measured live: register-only butterflies of this library on all SMs, the faster of the integer "
+                                   "Shoup and the fp64 one (fenc_measure_alu_peak); 32-bit IMAD peak %.2f T lane-ops/s" % (imad_peak / 1e12),
                     "butterflies_per_launch": t_ops / t_cnt, "hbm_frac_of_same_kernel": round(hbm_ach / peaks["hbm_gbs"], 4)}
     else:
         roofline = {"bound": "hbm", "kernel": top, "achieved": round(hbm_ach, 1), "peak": peaks["hbm_gbs"], "unit": "GB/s",

@@ -234,8 +234,9 @@ int fenc_profile_kernels(void);
 const char *fenc_profile_name(int id);
 fenc_status fenc_profile_read(fenc_ctx *ctx, double *ms, uint64_t *launches, double *alg_bytes, double *alg_butterflies,
                               int reset);
-/* Measured integer-pipe ceilings on this device: dependency-free 32-bit IMAD lane-ops/s, and
- * register-only forward Shoup butterflies/s of the library's own butterfly (no memory traffic). */
+/* Measured arithmetic ceilings on this device: dependency-free 32-bit IMAD lane-ops/s, and
+ * register-only forward butterflies/s of the library's own butterfly (no memory traffic) -- the integer Shoup butterfly,
+ * or, when q_0 is below 2^45 and the context's butterflies run on the FP64 pipe, the faster of that and the fp64 one. */
 fenc_status fenc_measure_alu_peak(fenc_ctx *ctx, double *imad_lane_ops_per_s, double *butterflies_per_s);
 /* counters since context creation: kernels launched by this library; optional reset */
 uint64_t fenc_launch_count(fenc_ctx *ctx, int reset);

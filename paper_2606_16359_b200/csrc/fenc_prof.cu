@@ -109,6 +109,37 @@ __global__ void __launch_bounds__(256) butterfly_peak_kernel(u64 *out, u64 q, u6
   for (int k = 0; k < 8; k++) s ^= x[k];
   out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
+// the fp64 register round of fenc_device.cuh (moduli below 2^45): convert in, 12 butterflies, convert out
+__global__ void __launch_bounds__(256) butterfly_f64_peak_kernel(u64 *out, u64 q, u64 qinv_bits, u64 c_bits, u64 cq_bits, int iters) {
+  u64 y[8];
+#pragma unroll
+  for (int k = 0; k < 8; k++) y[k] = (threadIdx.x * 8 + k + blockIdx.x) % q;
+  const F64Mod fm = f64mod(q, qinv_bits);
+  const double c = __longlong_as_double((long long)c_bits), cq = __longlong_as_double((long long)cq_bits);
+  const double off = __dadd_rn(fm.q, 4503599627370496.0);
+  for (int it = 0; it < iters; it++) {
+    double x[8];
+#pragma unroll
+    for (int k = 0; k < 8; k++) x[k] = u2d52(y[k]);
+#pragma unroll
+    for (int s = 2; s >= 0; s--) {
+#pragma unroll
+      for (int k = 0; k < 8; k++) {
+        if (k & (1 << s)) continue;
+        const int k2 = k | (1 << s);
+        const double X = x[k], T = mulmod_dd(x[k2], c, cq, fm);
+        x[k] = __dadd_rn(X, T);
+        x[k2] = __dadd_rn(X, -T);
+      }
+    }
+#pragma unroll
+    for (int k = 0; k < 8; k++) y[k] = d2u_off(reduce_dd(x[k], fm), off);  // bounded between rounds, like the inverse round
+  }
+  u64 s = 0;
+#pragma unroll
+  for (int k = 0; k < 8; k++) s ^= y[k];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
 extern "C" fenc_status fenc_measure_alu_peak(fenc_ctx *ctx, double *imad_lane_ops_per_s, double *butterflies_per_s) {
   if (!ctx || !imad_lane_ops_per_s || !butterflies_per_s) return FENC_ERR_INVALID_ARG;
   const int blocks = 148 * 8, iters = 4096;
@@ -134,6 +165,19 @@ extern "C" fenc_status fenc_measure_alu_peak(fenc_ctx *ctx, double *imad_lane_op
     cudaEventElapsedTime(&ms, e0, e1);
   }
   *butterflies_per_s = (double)blocks * 256 * 12.0 * (iters / 8) / (ms * 1e-3);
+  if (fh::f64_modulus(q)) {  // this context's butterflies of q_0 run on the FP64 pipe: report the faster of the two ceilings
+    const u64 qinv = fh::double_bits(1.0 / (double)q), cb = fh::double_bits((double)w), cqb = fh::double_bits((double)((long double)w / (long double)q));
+    for (int rep = 0; rep < 2; rep++) {
+      cudaEventRecord(e0, ctx->stream);
+      butterfly_f64_peak_kernel<<<blocks, 256, 0, ctx->stream>>>(buf, q, qinv, cb, cqb, iters / 8);
+      cudaEventRecord(e1, ctx->stream);
+      CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+      cudaEventElapsedTime(&ms, e0, e1);
+    }
+    const double f = (double)blocks * 256 * 12.0 * (iters / 8) / (ms * 1e-3);
+    if (f > *butterflies_per_s) *butterflies_per_s = f;
+    ctx->launches += 2;
+  }
   cudaEventDestroy(e0), cudaEventDestroy(e1);
   dfree(ctx, buf);
   ctx->launches += 4;
