@@ -430,9 +430,14 @@ struct KeyMacP {
 // 3 blocks of 128 threads per SM: 168 registers hold the 32 128-bit accumulators and the fp64 butterflies without
 // spilling (4 blocks at 128 registers spill 160 bytes and run 10 % slower)
 #define KEYMAC_BLOCKS 3
+DEVI void cp_async8(u64 *dst_smem, const u64 *src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((u32)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
+}
+DEVI void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+DEVI void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 template <int EPT, int GEO>  // elements per thread
 __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? KEYMAC_BLOCKS : 2) ntt_rows_keymac_kernel(KeyMacP p) {
-  extern __shared__ u64 sm[];
+  extern __shared__ u64 sm_all[];  // two tiles: the next digit's words arrive (cp.async) while this one is transformed
   const int tid = threadIdx.x;
   // batch index fastest: blockIdx.x = tile * n_batch + b
   const int nb = p.n_batch, b = blockIdx.x % nb, tile = blockIdx.x / nb, t = blockIdx.y;
@@ -446,16 +451,29 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? KEYMAC_BLOCKS
   for (int i = 0; i < EPT; i++) a0l[i] = a0h[i] = a1l[i] = a1h[i] = 0;
   const int nth = blockDim.x;
   constexpr int HB = EPT < 4 ? EPT : 4;
+  auto request = [&](int j) {  // digit j's tile of the ModUp temp -> buffer j & 1 (nothing to fetch inside the digit)
+    const int ti = p.tmp_index[j * p.E + t];
+    if (ti >= 0) {
+      const u64 *src = p.tmp + (size_t)b * p.tmp_bstride + (size_t)ti * N;
+      u64 *dst = sm_all + (size_t)(j & 1) * T;
+#pragma unroll
+      for (int i = 0; i < EPT; i++) {
+        const int e = tid + i * nth;
+        if (e < T) cp_async8(dst + swz(e), src + G.gidx(e));
+      }
+    }
+    cp_async_commit();
+  };
+  request(0);
   for (int j = 0; j < p.beta; j++) {
     const int ti = p.tmp_index[j * p.E + t];
     const u64 *kb = it.evk + ((size_t)(j * 2 + 0) * p.A + mod) * N;
     const u64 *ka = it.evk + ((size_t)(j * 2 + 1) * p.A + mod) * N;
-    if (ti >= 0) {
-      const u64 *src = p.tmp + (size_t)b * p.tmp_bstride + (size_t)ti * N;
-      tile_fill(sm, T, tid, nth, [&](int e) { return src[G.gidx(e)]; });
-      __syncthreads();
-      tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)mod * N, mc.q, tid, mc.f64);
-    }
+    u64 *sm = sm_all + (size_t)(j & 1) * T;
+    cp_async_wait_all();
+    __syncthreads();  // digit j's tile is complete, and every thread is done with the other buffer (digit j-1)
+    if (j + 1 < p.beta) request(j + 1);
+    if (ti >= 0) tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)mod * N, mc.q, tid, mc.f64);
     // the key words (and, inside the digit, the permuted input words) of 4 elements are loaded together, then used
 #pragma unroll
     for (int h = 0; h < EPT; h += HB) {
@@ -480,7 +498,6 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? KEYMAC_BLOCKS
         }
       }
     }
-    __syncthreads();
   }
   u64 *o0 = p.acc + (size_t)b * p.acc_bstride + (size_t)t * N;
   u64 *o1 = o0 + (size_t)p.E * N;
@@ -507,10 +524,10 @@ int k_ntt_rows_keymac(const KCtx &k, const BatchItem *items, int L, int E, int b
   // algorithmic bytes: ModUp temp + the switched polynomial read once, accumulators written once, each key once
   PROF(k, K_KEYMAC, 8.0 * k.N * (((double)n_up + L + 2.0 * E) * n_batch + 2.0 * beta * E * n_distinct_keys),
        HALF_N(k) * g.brow * n_up * n_batch);
-  if (g.logN >= 12) ntt_rows_keymac_kernel<8, 1><<<grid, nth, sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
-  else if (ept <= 1) ntt_rows_keymac_kernel<1, 0><<<grid, nth, sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
-  else if (ept <= 4) ntt_rows_keymac_kernel<4, 0><<<grid, nth, sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
-  else ntt_rows_keymac_kernel<8, 0><<<grid, nth, sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p);
+  if (g.logN >= 12) ntt_rows_keymac_kernel<8, 1><<<grid, nth, 2 * (sizeof(u64) << g.lt_row), (cudaStream_t)k.stream>>>(p);
+  else if (ept <= 1) ntt_rows_keymac_kernel<1, 0><<<grid, nth, 2 * (sizeof(u64) << g.lt_row), (cudaStream_t)k.stream>>>(p);
+  else if (ept <= 4) ntt_rows_keymac_kernel<4, 0><<<grid, nth, 2 * (sizeof(u64) << g.lt_row), (cudaStream_t)k.stream>>>(p);
+  else ntt_rows_keymac_kernel<8, 0><<<grid, nth, 2 * (sizeof(u64) << g.lt_row), (cudaStream_t)k.stream>>>(p);
   LAUNCH_CHECK(k);
   return 0;
 }
