@@ -535,3 +535,42 @@ def test_config3_conv_plus_activation_full_size_decoded(mods):
     c = fr.direct_conv(od, x, w)
     assert np.abs(Y - (0.5 + 0.197 * c - 0.004 * c ** 3)).max() < 1e-3
     ctx.close()
+
+
+_LENET_DIGEST = r"""
+import sys, hashlib, json
+sys.path.insert(0, %r)
+import numpy as np, torch
+import paper_2606_16359_b200 as fenc, workloads as wl, bench
+from paper_2606_16359_b200.pipeline import Pipeline
+ctx = fenc.Context(**wl.PARAMS["cfg2"])
+layers, x = bench.lenet_layers(128, 2000)
+pipe = Pipeline(ctx, layers)
+pipe.setup(key_seed=2000)
+cts = pipe.encrypt_input(x, 20000)
+out = pipe.forward(cts)
+h = hashlib.sha256()
+for c in out:
+    h.update(np.ascontiguousarray(ctx.ct_export(c)).tobytes())
+print(json.dumps({"digest": h.hexdigest(), "n": len(out), "L": out[0].L}))
+"""
+
+
+@pytest.mark.gpu
+def test_lenet_step_fp64_and_integer_arithmetic_agree():
+    """The whole LeNet-5 step of bench.py (BASELINE config 2, batch 128, N=2^14) run twice in fresh processes: with the
+    40-bit moduli on the FP64 pipe (default: butterflies, base conversions, MAC limbs) and with FENC_NO_F64=1 /
+    FENC_MAC_MODE=0 (integer Shoup butterflies, 128-bit MAC).  Every limb of every output ciphertext must be identical:
+    the fp64 path is an exact reformulation, and the integer path is the one the oracle-checked
+    tests of the 50- and 58-bit parameter sets exercise."""
+    import subprocess, sys, os, json
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    code = _LENET_DIGEST % root
+    res = []
+    for extra in ({}, {"FENC_NO_F64": "1", "FENC_MAC_MODE": "0"}):
+        env = dict(os.environ, **extra)
+        p = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=600)
+        assert p.returncode == 0, p.stderr[-2000:]
+        res.append(json.loads(p.stdout.strip().splitlines()[-1]))
+    assert res[0] == res[1], res
+    assert res[0]["n"] >= 1
