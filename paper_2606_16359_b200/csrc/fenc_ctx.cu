@@ -194,7 +194,7 @@ extern "C" fenc_status fenc_params_init(const fenc_params_desc *d, fenc_ctx **ou
     u64 m = ctx->mod[i];
     ctx->psi[i] = fh::find_psi(m, N);
     int bits = 64 - __builtin_clzll(m - 1);
-    mods[i] = ModConst{m, fh::neg_qinv(m), fh::to_mont(fh::to_mont(1, m), m), (bits >= 64 ? ~0ull : (1ull << bits) - 1), (u64)((((u128)1) << 64) / m), fh::f64_modulus(m) ? fh::double_bits(1.0 / (double)m) : 0ull, {0, 0}};
+    mods[i] = ModConst{m, fh::neg_qinv(m), fh::to_mont(fh::to_mont(1, m), m), (bits >= 64 ? ~0ull : (1ull << bits) - 1), (u64)((((u128)1) << 64) / m), fh::f64_modulus(m, ctx->logN) ? fh::double_bits(1.0 / (double)m) : 0ull, {0, 0}};
     fh::build_twiddles(m, ctx->psi[i], ctx->logN, &fwd[(size_t)i * N], &inv[(size_t)i * N]);
     u64 ni = fh::invmod((u64)N % m, m);
     ninv[i] = ShoupC{ni, fh::shoup(ni, m)};
@@ -297,7 +297,7 @@ LevelPlan *get_plan(fenc_ctx *ctx, int L) {
       scale_in[i] = shoupc(fh::mulmod(ninv, fh::invmod(qhat, qi), qi), qi);
     }
     bool src_f64 = true;
-    for (int i = lo; i < hi; i++) src_f64 = src_f64 && fh::f64_modulus(mod[i]);
+    for (int i = lo; i < hi; i++) src_f64 = src_f64 && fh::f64_narrow(mod[i]);
     groups_up.push_back(ConvGroup{lo, lo, hi - lo, lo, (int)rows_up.size(), E - (hi - lo), {src_f64 ? 2 : 0, 0}});
     P.n_src_up = std::max(P.n_src_up, hi - lo);
     for (int t = 0; t < E; t++) {
@@ -346,7 +346,7 @@ LevelPlan *get_plan(fenc_ctx *ctx, int L) {
   }
   for (int c = 0; c < 2; c++) {
     groups_down.push_back(ConvGroup{c * np, nq, np, c * np, c * L, L, {0, 0}});
-    groups_rs.push_back(ConvGroup{c, L - 1, 1, c, c * (L - 1), L - 1, {(L >= 2 && fh::f64_modulus(mod[L - 1])) ? 2 : 0, 0}});
+    groups_rs.push_back(ConvGroup{c, L - 1, 1, c, c * (L - 1), L - 1, {(L >= 2 && fh::f64_narrow(mod[L - 1])) ? 2 : 0, 0}});
   }
   P.d_groups_up = upload_owned(ctx, P.owned, groups_up);
   P.d_groups_down = upload_owned(ctx, P.owned, groups_down);

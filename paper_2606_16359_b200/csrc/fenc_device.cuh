@@ -138,7 +138,7 @@ DEVI u64 mulmod_f64(u64 x, u64 c_bits, u64 cq_bits, const F64Mod &m) {  // (0, 2
 // shared-memory slot is swz(ebase) ^ swz(k << PW): one base computation per thread and round.
 
 // compile-time round: window position and active stages [SLO, SHI) are constants (production geometries)
-template <bool FWD, bool LAZY, int PW, int SLO, int SHI, bool F64>
+template <bool FWD, bool LAZY, int PW, int SLO, int SHI, int F64>  // F64: 0 integer, 1 fp64 narrow (q < 2^45), 2 fp64 wide
 DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid, u64 f64) {
   const int ebase = ((tid >> PW) << (PW + 3)) | (tid & ((1 << PW) - 1));
   const int gpw = G.gbit(PW);
@@ -152,19 +152,31 @@ DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 
 #pragma unroll
   for (int i = 0; i < 4; i++) t0[i] = (0 >= SLO && 0 < SHI) ? __ldg(twv + (nj >> (gpw + 1)) + i) : t2;
   const int sbase = swz(ebase);
-  if constexpr (F64) {
-    // the eight values stay doubles (signed, exact integers) through the round's stages: T in (-q, q), so a forward
-    // stage moves a value by less than q either way and the stored value, shifted by +3q, stays non-negative and grows
-    // by at most 6q per round (36q after the five rounds of a 2^16 transform, inside the 2^51 the multiply accepts);
-    // an inverse round ends with v - rint(v/q) q + q, inside the [0, 2q) the inverse contract promises.
+  if constexpr (F64 != 0) {
+    // The eight values stay doubles (signed, exact integers) through the round's stages; T is in (-q, q).
+    // Narrow moduli (q < 2^45): a forward stage moves a value by less than q either way; the stored value, shifted by
+    // +3q, stays non-negative and grows by at most 6q per round (36q after the five rounds of a 2^16 transform, inside
+    // the 2^51 the multiply accepts); an inverse round ends with v - rint(v/q) q + q in [0, 2q).
+    // Wide moduli (2^45 <= q < 2^50, compile-time schedules only): every round starts from values in [0, 2q], centred
+    // to [-q, q] while converting, and ends with the same reduction in both directions; an operand that can exceed 2q
+    // (third forward stage, second and third inverse stage) is reduced before it is multiplied, so the quotient
+    // estimate stays below 2^51 and every sum below 2^53.
     const F64Mod fm = f64mod(q, f64);
+    constexpr bool wide = F64 == 2;
+    const double in_off = wide ? -(4503599627370496.0 + fm.q) : -4503599627370496.0;
     double x[8];
 #pragma unroll
-    for (int k = 0; k < 8; k++) x[k] = u2d52(sm[sbase ^ swz(k << PW)]);
+    for (int k = 0; k < 8; k++) {
+      const u64 v = sm[sbase ^ swz(k << PW)];
+      x[k] = __dadd_rn(__hiloint2double((int)((u32)(v >> 32) | 0x43300000u), (int)(u32)v), in_off);
+    }
+    int done = 0;
 #pragma unroll
     for (int ss = 0; ss < 3; ss++) {
       const int s = FWD ? 2 - ss : ss;
       if (s < SLO || s >= SHI) continue;
+      const bool pre = wide && (FWD ? done >= 2 : done >= 1);
+      done++;
 #pragma unroll
       for (int k = 0; k < 8; k++) {
         if (k & (1 << s)) continue;
@@ -172,19 +184,22 @@ DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 
         const ulonglong2 w = s == 2 ? t2 : (s == 1 ? t1[k >> 2] : t0[k >> 1]);
         const double c = __longlong_as_double((long long)w.x), cq = __longlong_as_double((long long)w.y);
         if (FWD) {
-          const double X = x[k], T = mulmod_dd(x[k2], c, cq, fm);
+          const double X = x[k], Y = pre ? reduce_dd(x[k2], fm) : x[k2];
+          const double T = mulmod_dd(Y, c, cq, fm);
           x[k] = __dadd_rn(X, T);
           x[k2] = __dadd_rn(X, -T);
         } else {
           const double U = x[k], V = x[k2];
+          const double D = __dadd_rn(U, -V);
           x[k] = __dadd_rn(U, V);
-          x[k2] = mulmod_dd(__dadd_rn(U, -V), c, cq, fm);
+          x[k2] = mulmod_dd(pre ? reduce_dd(D, fm) : D, c, cq, fm);
         }
       }
     }
-    const double off = FWD ? __fma_rn(3.0, fm.q, 4503599627370496.0) : __dadd_rn(fm.q, 4503599627370496.0);
+    const bool red = !FWD || wide;
+    const double off = red ? __dadd_rn(fm.q, 4503599627370496.0) : __fma_rn(3.0, fm.q, 4503599627370496.0);
 #pragma unroll
-    for (int k = 0; k < 8; k++) sm[sbase ^ swz(k << PW)] = d2u_off(FWD ? x[k] : reduce_dd(x[k], fm), off);
+    for (int k = 0; k < 8; k++) sm[sbase ^ swz(k << PW)] = d2u_off(red ? reduce_dd(x[k], fm) : x[k], off);
   } else {
   u64 x[8];
 #pragma unroll
@@ -215,7 +230,7 @@ DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 
   }
 }
 
-template <bool FWD, bool LAZY, int LT, int LO, int NB, int DONE, bool F64 = false>
+template <bool FWD, bool LAZY, int LT, int LO, int NB, int DONE, int F64 = 0>
 DEVI void tile_rounds_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid, u64 f64 = 0) {
   if constexpr (DONE < NB) {
     constexpr int take = NB - DONE < 3 ? NB - DONE : 3;
@@ -268,7 +283,8 @@ DEVI void tile_round_rt(u64 *sm, const TileGeo &G, int pw, int s_lo, int s_hi, c
 template <bool FWD, int LT, int LO, int NB>
 DEVI void tile_transform_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, int tid, u64 f64) {
   const u64 q2 = q + q;
-  if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, true>(sm, G, tw, q, q2, tid, f64);
+  if (f64 && q < (1ull << FENC_F64_MAX_BITS)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 1>(sm, G, tw, q, q2, tid, f64);
+  else if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 2>(sm, G, tw, q, q2, tid, f64);
   else if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
   else tile_rounds_ct<FWD, false, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
 }
@@ -303,7 +319,8 @@ DEVI void tile_transform(u64 *sm, const TileGeo &G, int lo, int nb, const ShoupC
     }
   } else {
     constexpr int LT = GEO == 1 ? FENC_ROW_LT : GEO + 4, LO = GEO == 1 ? 0 : 4, NB = GEO == 1 ? 8 : GEO;
-    if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, true>(sm, G, tw, q, q2, tid, f64);
+    if (f64 && q < (1ull << FENC_F64_MAX_BITS)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 1>(sm, G, tw, q, q2, tid, f64);
+    else if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 2>(sm, G, tw, q, q2, tid, f64);
     else if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
     else tile_rounds_ct<FWD, false, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
   }

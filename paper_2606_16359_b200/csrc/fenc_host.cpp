@@ -86,9 +86,17 @@ static u32 bitrev(u32 x, int bits) {
 }
 
 // fwd[k] = psi^bitrev(k), inv[k] = psi^-bitrev(k), each with its Shoup companion
-bool f64_modulus(u64 q) {
+// Butterflies of this modulus multiply on the FP64 pipe (fenc_device.cuh): "narrow" moduli below 2^45 everywhere, moduli
+// below 2^50 only with the compile-time tile schedules (ring degree >= 2^12), whose rounds re-centre the values.
+bool f64_narrow(u64 q) {
   static const bool off = getenv("FENC_NO_F64") != nullptr;  // diagnostics: integer butterflies everywhere
   return !off && q < (1ull << 45);
+}
+bool f64_modulus(u64 q, int logN) {
+  static const bool off = getenv("FENC_NO_F64") != nullptr;
+  static const bool no_wide = getenv("FENC_NO_F64_WIDE") != nullptr;
+  if (off) return false;
+  return q < (1ull << 45) || (!no_wide && logN >= 12 && q < (1ull << 50));
 }
 void build_twiddles(u64 q, u64 psi, int logN, ShoupC *fwd, ShoupC *inv) {
   const u32 N = 1u << logN;
@@ -96,7 +104,7 @@ void build_twiddles(u64 q, u64 psi, int logN, ShoupC *fwd, ShoupC *inv) {
   const u64 ipsi = invmod(psi, q);
   pw[0] = ipw[0] = 1;
   for (u32 i = 1; i < N; i++) pw[i] = mulmod(pw[i - 1], psi, q), ipw[i] = mulmod(ipw[i - 1], ipsi, q);
-  const bool f64 = f64_modulus(q);
+  const bool f64 = f64_modulus(q, logN);
   auto bits = [](double d) { u64 b; memcpy(&b, &d, 8); return b; };
   for (u32 k = 0; k < N; k++) {
     u32 r = bitrev(k, logN);

@@ -26,8 +26,8 @@ struct ModConst {  // one per modulus, device global memory
   u64 r2;          // 2^128 mod q: mont_mul(x, r2) = x 2^64 mod q
   u64 mask;        // 2^ceil(log2 q) - 1 (uniform rejection sampler)
   u64 qbar;        // floor(2^64 / q): full reduction of a lazy 64-bit value
-  u64 f64;         // != 0: q < 2^45, the bits of (double)(1/q); the twiddle tables of this modulus hold fp64 pairs
-                   // (fenc_device.cuh mulmod_dd)
+  u64 f64;         // != 0: fp64 butterflies (q < 2^45, or q < 2^50 with N >= 2^12): the bits of (double)(1/q); the twiddle
+                   // tables of this modulus hold fp64 pairs (fenc_device.cuh mulmod_dd)
   u64 pad[2];
 };
 
@@ -180,7 +180,8 @@ u64 shoup(u64 c, u64 q);    // floor(c 2^64 / q)
 u64 to_mont(u64 c, u64 q);  // c 2^64 mod q
 u64 neg_qinv(u64 q);        // -q^{-1} mod 2^64
 void build_twiddles(u64 q, u64 psi, int logN, ShoupC *fwd, ShoupC *inv);
-bool f64_modulus(u64 q);
+bool f64_modulus(u64 q, int logN);
+bool f64_narrow(u64 q);  // below 2^45: also the base conversions run in fp64
 inline u64 double_bits(double d) { u64 b; memcpy(&b, &d, 8); return b; }  // butterflies of this modulus multiply on the FP64 pipe (twiddle tables hold fp64 pairs)
 u64 mix64(u64 z);
 u64 stream_key(u64 seed, u64 purpose, u64 a, u64 b, u64 c);

@@ -256,7 +256,7 @@ __global__ void __launch_bounds__(128, 5) convert_cols_kernel(ConvColP p) {
     const RowDesc rd = p.rows[cg.tgt_start + t];
     const ModConst mc = p.mods[rd.mod];
     u64 v[8];
-    if (!MERGED && p.bc_f64 && (cg.pad[0] & 2) && mc.f64) conv_dot_f64<T, NTH>(smem, n_conv, p.bc_f64 + rd.aux2, f64mod(mc.q, mc.f64), tid, v);
+    if (!MERGED && p.bc_f64 && (cg.pad[0] & 2) && mc.f64 && mc.q < (1ull << FENC_F64_MAX_BITS)) conv_dot_f64<T, NTH>(smem, n_conv, p.bc_f64 + rd.aux2, f64mod(mc.q, mc.f64), tid, v);
     else conv_dot<T, NTH>(smem, n_conv, p.bc + rd.aux2, mc, p.max_terms, tid, v);
     if (MERGED) {
       const ShoupC pt = p.mulc[rd.mod];
