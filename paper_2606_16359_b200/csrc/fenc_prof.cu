@@ -165,7 +165,7 @@ extern "C" fenc_status fenc_measure_alu_peak(fenc_ctx *ctx, double *imad_lane_op
     cudaEventElapsedTime(&ms, e0, e1);
   }
   *butterflies_per_s = (double)blocks * 256 * 12.0 * (iters / 8) / (ms * 1e-3);
-  if (fh::f64_narrow(q)) {  // this context's butterflies of q_0 run on the FP64 pipe: report the faster of the two ceilings
+  if (fh::f64_modulus(q, ctx->logN)) {  // this context's butterflies of q_0 run on the FP64 pipe: report the faster of the two ceilings
     const u64 qinv = fh::double_bits(1.0 / (double)q), cb = fh::double_bits((double)w), cqb = fh::double_bits((double)((long double)w / (long double)q));
     for (int rep = 0; rep < 2; rep++) {
       cudaEventRecord(e0, ctx->stream);
