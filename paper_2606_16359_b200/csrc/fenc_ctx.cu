@@ -432,7 +432,7 @@ LevelPlan *get_plan(fenc_ctx *ctx, int L) {
 static const size_t WS_CAP = (size_t)6 << 30;  // workspace budget for one chunk of a batch
 
 bool ks_can_merge_rescale(const fenc_ctx *ctx, int L) {
-  return L >= 2 && ctx->logN >= 12 && (size_t)(ctx->np + 2) * 8192 <= 200 * 1024;
+  return L >= 2 && convert_cols_fits(ctx->logN, ctx->np + 1, true);
 }
 
 fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items, bool rescale_after) {
@@ -464,7 +464,7 @@ fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items, bool r
     if (!d_items) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
     // a2 + a1 + a3: inverse row pass of sigma_g(d); then ONE fused column kernel per digit group: inverse column
     // stages + ModUp scaling of the digit's limbs in shared memory, base conversion and forward column stages per target
-    const bool fused_up = ctx->logN >= 12 && (size_t)(P->n_src_up + 1) * 8192 <= 200 * 1024;
+    const bool fused_up = convert_cols_fits(ctx->logN, P->n_src_up, false);
     if (fused_up) {
       CUDA_OK(ctx, k_intt_rows_only(k, d_items, nullptr, 0, true, y, (size_t)L * N, P->d_rows_in, L, nb));
       CUDA_OK(ctx, k_convert_cols(k, y, (size_t)L * N, P->d_groups_up, P->beta, P->n_src_up, P->d_scale_in, P->d_bc_up, P->d_rows_up,
@@ -488,7 +488,7 @@ fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items, bool r
       continue;
     }
     // a5: ModDown = inverse row pass of the special limbs, fused column kernel per component, divide epilogue in pass 2
-    const bool fused_down = ctx->logN >= 12 && (size_t)(np + 1) * 8192 <= 200 * 1024;
+    const bool fused_down = convert_cols_fits(ctx->logN, np, false);
     if (fused_down) {
       CUDA_OK(ctx, k_intt_rows_only(k, nullptr, acc, (size_t)2 * E * N, false, yP, (size_t)2 * np * N, P->d_rows_p, 2 * np, nb));
       CUDA_OK(ctx, k_convert_cols(k, yP, (size_t)2 * np * N, P->d_groups_down, 2, np, P->d_scale_p, P->d_bc_down, P->d_rows_down, 2 * L,

@@ -230,16 +230,22 @@ DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 
   }
 }
 
-template <bool FWD, bool LAZY, int LT, int LO, int NB, int DONE, int F64 = 0>
-DEVI void tile_rounds_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid, u64 f64 = 0) {
+// GRP: the tile belongs to a 128-thread group of a larger block; its rounds meet on the named barrier `bar` (1..15)
+template <bool GRP>
+DEVI void tile_sync(int bar) {
+  if constexpr (GRP) asm volatile("bar.sync %0, 128;" ::"r"(bar) : "memory");
+  else __syncthreads();
+}
+template <bool FWD, bool LAZY, int LT, int LO, int NB, int DONE, int F64 = 0, bool GRP = false>
+DEVI void tile_rounds_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid, u64 f64 = 0, int bar = 0) {
   if constexpr (DONE < NB) {
     constexpr int take = NB - DONE < 3 ? NB - DONE : 3;
     constexpr int cur = FWD ? LO + NB - DONE : LO + DONE;         // FWD: exclusive top; INV: inclusive bottom
     constexpr int p = FWD ? cur - take : cur;
     constexpr int pw = p < LT - 3 ? p : LT - 3;
     if (tid < (1 << (LT - 3))) tile_round_ct<FWD, LAZY, pw, p - pw, p - pw + take, F64>(sm, G, tw, q, q2, tid, f64);
-    __syncthreads();
-    tile_rounds_ct<FWD, LAZY, LT, LO, NB, DONE + take, F64>(sm, G, tw, q, q2, tid, f64);
+    tile_sync<GRP>(bar);
+    tile_rounds_ct<FWD, LAZY, LT, LO, NB, DONE + take, F64, GRP>(sm, G, tw, q, q2, tid, f64, bar);
   }
 }
 
@@ -280,13 +286,13 @@ DEVI void tile_round_rt(u64 *sm, const TileGeo &G, int pw, int s_lo, int s_hi, c
 
 // compile-time schedule over active tile bits [LO, LO+NB) of a 2^LT-element tile; picks the lazy forward butterflies
 // for q < 2^58.  Every thread of the block must call this (it synchronises).
-template <bool FWD, int LT, int LO, int NB>
-DEVI void tile_transform_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, int tid, u64 f64) {
+template <bool FWD, int LT, int LO, int NB, bool GRP = false>
+DEVI void tile_transform_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, int tid, u64 f64, int bar = 0) {
   const u64 q2 = q + q;
-  if (f64 && q < (1ull << FENC_F64_MAX_BITS)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 1>(sm, G, tw, q, q2, tid, f64);
-  else if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 2>(sm, G, tw, q, q2, tid, f64);
-  else if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
-  else tile_rounds_ct<FWD, false, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
+  if (f64 && q < (1ull << FENC_F64_MAX_BITS)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 1, GRP>(sm, G, tw, q, q2, tid, f64, bar);
+  else if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 2, GRP>(sm, G, tw, q, q2, tid, f64, bar);
+  else if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 0, GRP>(sm, G, tw, q, q2, tid, 0, bar);
+  else tile_rounds_ct<FWD, false, LT, LO, NB, 0, 0, GRP>(sm, G, tw, q, q2, tid, 0, bar);
 }
 
 // GEO selects the schedule: 0 = runtime (any lo/nb), 1 = row pass of 2048-element tiles with 8 stages,

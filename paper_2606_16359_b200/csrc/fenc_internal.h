@@ -119,6 +119,8 @@ int k_intt_rows_only(const KCtx &k, const BatchItem *items, const u64 *src, size
 // fused column kernel (needs N >= 2^12): for every group, the inverse column stages + scaling of its source rows (kept
 // in shared memory), then for each target the base conversion and the forward column stages -> tmp rows (lazy).
 // Returns -2 when the group does not fit shared memory (the caller falls back to k_intt + k_ntt_cols_bconv).
+// whether the fused column kernel can hold a conversion group of n_src limbs (its tiles + the work tiles) in shared memory
+bool convert_cols_fits(int logN, int n_src, bool merged);
 int k_convert_cols(const KCtx &k, u64 *y, size_t y_bstride, const ConvGroup *groups, int n_groups, int n_src_max,
                    const ShoupC *scale, const u64 *bc, const RowDesc *rows, int n_tgt_total, u64 *tmp, size_t tmp_bstride,
                    int n_batch, int max_terms, const ShoupC *merged_pinv = nullptr, const ShoupC *bc_f64 = nullptr);

@@ -210,28 +210,33 @@ DEVI void conv_dot_f64(const u64 *smem, int n, const ShoupC *bc, const F64Mod &f
 // the limb l = q_{L-1} that the rescale drops (modulus index cg.pad[1]).  With V_t = sum_i y_i (Phat_i mod t):
 //   out_l = Z - V_l P^-1 mod q_l        (the key-switched limb l in the coefficient domain, canonical)
 //   u_t   = V_t P^-1 + (out_l mod t)    (what the divide epilogue subtracts:  c'_t = (acc_t P^-1 + add_t - NTT(u_t)) q_l^-1)
-template <int BCOL, bool MERGED>
-__global__ void __launch_bounds__(128, 5) convert_cols_kernel(ConvColP p) {
+// NG > 1 (digit groups of 6 and more limbs, whose source tiles leave room for one or two blocks per SM only): the block
+// holds NG groups of 128 threads that share the source tiles; group g inverse-transforms the sources s = g mod NG and
+// produces the targets t = g mod NG in a work tile of its own, its rounds meeting on named barrier g + 1.
+template <int BCOL, bool MERGED, int NG>
+__global__ void __launch_bounds__(128 * NG, NG == 1 ? 5 : (NG == 2 ? 2 : 1)) convert_cols_kernel(ConvColP p) {
+  static_assert(!(MERGED && NG > 1), "the merged ModDown+rescale runs one group per block");
   constexpr int LT = 10, LC = LT - BCOL, T = 1 << LT, NTH = T / 8;
+  constexpr bool GRP = NG > 1;
   extern __shared__ u64 smem[];
-  const int tid = threadIdx.x, b = blockIdx.z;
+  const int tid = threadIdx.x & (NTH - 1), grp = threadIdx.x / NTH, bar = grp + 1, b = blockIdx.z;
   const ConvGroup cg = p.groups[blockIdx.y];
   const int N = 1 << p.logN;
   TileGeo G{LT, LC, p.brow, p.logN, blockIdx.x};
-  u64 *W = smem + (size_t)cg.n_src * T;  // work tile after the source tiles
+  u64 *W = smem + (size_t)(cg.n_src + grp) * T;  // work tiles after the source tiles
   u64 *ybase = p.y + (size_t)b * p.y_bstride;
   const int n_conv = MERGED ? cg.n_src - 1 : cg.n_src;  // tiles entering the base conversion
   // ---- sources: fill, inverse column stages, scale -> canonical coefficient tiles in shared memory
-  for (int s = 0; s < cg.n_src; s++) {
+  for (int s = grp; s < cg.n_src; s += NG) {
     const u64 *src = ybase + (size_t)(cg.src_row + s) * N;
     tile_fill(smem + (size_t)s * T, T, tid, NTH, [&](int e) { return src[G.gidx(e)]; });
   }
-  __syncthreads();
-  for (int s = 0; s < cg.n_src; s++) {
+  tile_sync<GRP>(bar);
+  for (int s = grp; s < cg.n_src; s += NG) {
     u64 *Y = smem + (size_t)s * T;
     const int mod = (MERGED && s == n_conv) ? cg.pad[1] : cg.src_mod + s;
     const u64 q = p.mods[mod].q;
-    tile_transform_ct<false, LT, LC, BCOL>(Y, G, p.tw_inv + (size_t)mod * N, q, tid, p.mods[mod].f64);
+    tile_transform_ct<false, LT, LC, BCOL, GRP>(Y, G, p.tw_inv + (size_t)mod * N, q, tid, p.mods[mod].f64, bar);
     const ShoupC sc = p.scale[cg.scale_off + s];
 #pragma unroll
     for (int i = 0; i < 8; i++) {
@@ -252,7 +257,7 @@ __global__ void __launch_bounds__(128, 5) convert_cols_kernel(ConvColP p) {
     for (int i = 0; i < 8; i++) outl[i] = submod(Z[swz(tid + i * NTH)], shoup_mul(v[i], pl.c, pl.cs, ml.q), ml.q);
   }
   // ---- targets
-  for (int t = 0; t < cg.n_tgt; t++) {
+  for (int t = grp; t < cg.n_tgt; t += NG) {
     const RowDesc rd = p.rows[cg.tgt_start + t];
     const ModConst mc = p.mods[rd.mod];
     u64 v[8];
@@ -265,12 +270,18 @@ __global__ void __launch_bounds__(128, 5) convert_cols_kernel(ConvColP p) {
     }
 #pragma unroll
     for (int i = 0; i < 8; i++) W[swz(tid + i * NTH)] = v[i];
-    __syncthreads();
-    tile_transform_ct<true, LT, LC, BCOL>(W, G, p.tw_fwd + (size_t)rd.mod * N, mc.q, tid, mc.f64);
+    tile_sync<GRP>(bar);
+    tile_transform_ct<true, LT, LC, BCOL, GRP>(W, G, p.tw_fwd + (size_t)rd.mod * N, mc.q, tid, mc.f64, bar);
     u64 *dst = p.tmp + (size_t)b * p.tmp_bstride + (size_t)rd.dst_row * N;
     tile_drain(W, T, tid, NTH, [&](int e, u64 v) { dst[G.gidx(e)] = v; });  // lazy, below 33q
-    __syncthreads();
+    tile_sync<GRP>(bar);
   }
+}
+
+// thread groups per block of the fused column kernel for digit groups of n_src limbs
+static inline int convert_groups(int n_src, bool merged) { return (merged || n_src < 6) ? 1 : (n_src < 8 ? 2 : 4); }
+bool convert_cols_fits(int logN, int n_src, bool merged) {
+  return logN >= 12 && (size_t)(n_src + convert_groups(n_src, merged)) * 8192 <= 227 * 1024;
 }
 
 int k_convert_cols(const KCtx &k, u64 *y, size_t y_bstride, const ConvGroup *groups, int n_groups, int n_src_max,
@@ -278,24 +289,26 @@ int k_convert_cols(const KCtx &k, u64 *y, size_t y_bstride, const ConvGroup *gro
                    int n_batch, int max_terms, const ShoupC *merged_pinv, const ShoupC *bc_f64) {
   if (n_groups == 0 || n_batch == 0) return 0;
   const NttGeom &g = k.geom;
-  if (g.logN < 12) return -2;
-  const size_t smem = (size_t)(n_src_max + 1) * 1024 * sizeof(u64);
-  if (smem > 200 * 1024) return -2;
+  if (!convert_cols_fits(g.logN, n_src_max, merged_pinv != nullptr)) return -2;
+  const int ng = convert_groups(n_src_max, merged_pinv != nullptr);
+  const size_t smem = (size_t)(n_src_max + ng) * 1024 * sizeof(u64);
   ConvColP p{y, y_bstride, groups, scale, bc, rows, tmp, tmp_bstride, k.d_mods, k.d_tw_fwd, k.d_tw_inv, g.logN, g.brow, max_terms,
              merged_pinv, bc_f64};
   dim3 grid(k.N >> 10, n_groups, n_batch);
   // algorithmic bytes: every target row written once (+ the sources, counted by the caller's row pass); butterflies of
   // the forward column stages of every target (the inverse ones of the sources are the smaller part)
   PROF(k, K_NTT_COL_BCONV, 8.0 * k.N * n_batch * (double)n_tgt_total, HALF_N(k) * g.bcol * (double)n_tgt_total * n_batch);
-#define LAUNCH_CONV1(B, M)                                                                                                         \
-  do {                                                                                                                             \
-    if (smem > 48 * 1024) cudaFuncSetAttribute(convert_cols_kernel<B, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
-    convert_cols_kernel<B, M><<<grid, 128, smem, (cudaStream_t)k.stream>>>(p);                                                     \
+#define LAUNCH_CONV1(B, M, G)                                                                                                         \
+  do {                                                                                                                                \
+    if (smem > 48 * 1024) cudaFuncSetAttribute(convert_cols_kernel<B, M, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+    convert_cols_kernel<B, M, G><<<grid, 128 * G, smem, (cudaStream_t)k.stream>>>(p);                                                 \
   } while (0)
-#define LAUNCH_CONV(B)             \
-  do {                             \
-    if (merged_pinv) LAUNCH_CONV1(B, true); \
-    else LAUNCH_CONV1(B, false);   \
+#define LAUNCH_CONV(B)                         \
+  do {                                         \
+    if (merged_pinv) LAUNCH_CONV1(B, true, 1); \
+    else if (ng == 4) LAUNCH_CONV1(B, false, 4); \
+    else if (ng == 2) LAUNCH_CONV1(B, false, 2); \
+    else LAUNCH_CONV1(B, false, 1);            \
   } while (0)
   switch (g.bcol) {
     case 4: LAUNCH_CONV(4); break;

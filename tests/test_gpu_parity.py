@@ -277,6 +277,27 @@ def test_rotation_full_size_config3_sampled(mods):
     ctx.close()
 
 
+@pytest.mark.parametrize("n_q,q_bits,n_p,dnum", [(7, 40, 5, 1), (9, 50, 9, 1), (12, 50, 6, 2), (20, 40, 10, 2)])
+def test_rotation_wide_digit_groups(mods, n_q, q_bits, n_p, dnum):
+    """Digit groups of 6 and more limbs (config 5's dnum = 1, 2 points): the fused column kernel runs 2 or 4 thread
+    groups per block over shared source tiles (ragged target counts per group); a second rotation one level down has a
+    short last digit.  N = 2^12: four column tiles per limb."""
+    ck, fr, fenc = mods
+    p = dict(log2N=12, n_q=n_q, q_bits=q_bits, n_p=n_p, p_bits=60, dnum=dnum, log2_scale=q_bits)
+    P = ck.Params(*wl.oracle_params_args(p))
+    ctx = fenc.Context(**p)
+    assert ctx.q == P.q and ctx.p == P.p and ctx.dlen == P.dlen
+    steps = [3, P.n - 7]
+    ok, gk = ck.keygen(P, 9, steps), ctx.keygen(9, steps)
+    for L in (P.nq, P.nq - 1):
+        limbs = wl.random_ct_limbs(100 + L, P.q, L, P.N)
+        gin = ctx.ct_import(limbs)
+        outs = ctx.rotate(gk, [gin, gin, gin], steps + [3])
+        for r, o in zip(steps + [3], outs):
+            assert np.array_equal(ctx.ct_export(o), ck.rotate(P, ok, ck.Ciphertext(limbs, L, 1), r).c), (L, r)
+    ctx.close()
+
+
 # ------------------------------------------------------------------------------------------------ fc, pooling, pipeline
 @pytest.mark.parametrize("kw", [
     dict(BS=2, n_in=32, n_out=5, in_C=2, in_H=4, in_W=4, in_M=4),
