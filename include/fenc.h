@@ -142,6 +142,17 @@ fenc_status fenc_decrypt_decode(fenc_ctx *ctx, const fenc_keys *keys, const fenc
 /* host limbs: uint64 [2][L][N], coefficient domain, canonical residues in [0, q_i) */
 fenc_status fenc_ct_export(fenc_ctx *ctx, const fenc_ct *ct, uint64_t *limbs);
 fenc_status fenc_ct_import(fenc_ctx *ctx, const uint64_t *limbs, uint32_t L, double scale, fenc_ct **out);
+/* fenc_ct_import without the host synchronisation: the host->device copy runs on a copy stream of the context's own
+ * (overlapping work already enqueued on the context's stream), the NTT follows on the context's stream.  `limbs`
+ * (host; page-locked memory for a truly asynchronous copy) stays owned by the caller and must remain valid and
+ * unchanged until the next synchronising call on this context returns (fenc_sync, fenc_ct_export, any decrypt).
+ * Serving loops use it to upload the next request while the current one computes. */
+fenc_status fenc_ct_import_async(fenc_ctx *ctx, const uint64_t *limbs, uint32_t L, double scale, fenc_ct **out);
+/* fenc_ct_export without the host synchronisation: `limbs` (host, page-locked for a truly asynchronous copy; owned by
+ * the caller) holds the result once fenc_export_wait (or any synchronising call) has returned.  fenc_export_wait blocks
+ * until every fenc_ct_export_async issued so far has landed; work enqueued on the context after them is not waited for. */
+fenc_status fenc_ct_export_async(fenc_ctx *ctx, const fenc_ct *ct, uint64_t *limbs);
+fenc_status fenc_export_wait(fenc_ctx *ctx);
 fenc_status fenc_ct_info(fenc_ctx *ctx, const fenc_ct *ct, uint32_t *L, double *scale, void **device_ptr);
 void fenc_ct_free(fenc_ct *ct);
 

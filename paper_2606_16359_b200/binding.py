@@ -64,7 +64,8 @@ SYMBOLS = ["fenc_params_init", "fenc_ctx_free", "fenc_last_error", "fenc_get_pri
            "fenc_compress", "fenc_ntt_rows", "fenc_launch_count", "fenc_device_bytes", "fenc_sum_groups",
            "fenc_profile_enable", "fenc_profile_kernels", "fenc_profile_name", "fenc_profile_read", "fenc_fc_plan",
            "fenc_fc_wts_keys", "fenc_fc_weights", "fenc_fc_weights_from_coeffs", "fenc_fc", "fenc_measure_alu_peak",
-           "fenc_cmult_relin", "fenc_mul_scalar", "fenc_add_const"]
+           "fenc_cmult_relin", "fenc_mul_scalar", "fenc_add_const", "fenc_ct_import_async", "fenc_ct_export_async",
+           "fenc_export_wait"]
 
 _lib = None
 
@@ -97,6 +98,9 @@ def load_library(path=None):
                                 C.c_uint32, C.c_uint32, dp],
         "fenc_ct_export": [vp, vp, u64p],
         "fenc_ct_import": [vp, u64p, C.c_uint32, C.c_double, vpp],
+        "fenc_ct_import_async": [vp, u64p, C.c_uint32, C.c_double, vpp],
+        "fenc_ct_export_async": [vp, vp, u64p],
+        "fenc_export_wait": [vp],
         "fenc_ct_info": [vp, vp, u32p, dp, vpp],
         "fenc_rotate": [vp, vp, vpp, i32p, C.c_size_t, vpp],
         "fenc_rescale": [vp, vpp, C.c_size_t, vpp],
@@ -356,6 +360,24 @@ class Context:
         h = C.c_void_p()
         self._ck(self.lib.fenc_ct_import(self.h, _ptr(a, C.c_uint64), a.shape[1], float(scale), C.byref(h)))
         return Ciphertext(self, h)
+
+    def ct_import_async(self, limbs, scale=0.0):
+        """fenc_ct_import_async: `limbs` (a contiguous uint64 [2][L][N] array, page-locked for a real overlap) must stay
+        alive and unchanged until the next synchronising call (sync, ct_export, decrypt)."""
+        a = limbs
+        assert a.dtype == np.uint64 and a.flags.c_contiguous and a.ndim == 3 and a.shape[0] == 2 and a.shape[2] == self.N
+        h = C.c_void_p()
+        self._ck(self.lib.fenc_ct_import_async(self.h, _ptr(a, C.c_uint64), a.shape[1], float(scale), C.byref(h)))
+        return Ciphertext(self, h)
+
+    def ct_export_async(self, ct, out):
+        """fenc_ct_export_async into `out` (contiguous uint64 [2][L][N], page-locked for a real overlap); valid after
+        export_wait()."""
+        assert out.dtype == np.uint64 and out.flags.c_contiguous and out.shape == (2, ct.L, self.N)
+        self._ck(self.lib.fenc_ct_export_async(self.h, ct.h, _ptr(out, C.c_uint64)))
+
+    def export_wait(self):
+        self._ck(self.lib.fenc_export_wait(self.h))
 
     def _harr(self, handles):
         return (C.c_void_p * len(handles))(*[x.h.value for x in handles])

@@ -53,6 +53,15 @@ struct LevelPlan {
 
 struct LinGraph;  // fenc_conv.cu: operation graph of a linear layer (conv or fc)
 
+// one slot of the staging ring behind fenc_ct_import_async: the copy stream fills it, the context's stream transforms it
+#define FENC_STAGE_SLOTS 64
+#define FENC_STAGE_BYTES ((size_t)256 << 20)
+struct StageSlot {
+  u64 *d = nullptr;
+  size_t bytes = 0;
+  cudaEvent_t copied = nullptr, consumed = nullptr;
+};
+
 struct fenc_ctx {
   int logN = 0, N = 0, n = 0, nq = 0, np = 0, A = 0, dlen = 0, beta_max = 0;
   std::vector<u64> mod, psi;  // q_0..q_{nq-1}, p_0..p_{np-1}
@@ -85,6 +94,10 @@ struct fenc_ctx {
   bool desc_used[FENC_DESC_SLOTS] = {};
   unsigned desc_next = 0;
   std::map<std::string, std::shared_ptr<LinGraph>> graphs;
+  cudaStream_t copy_stream = nullptr;  // host -> staging copies of fenc_ct_import_async (created on first use)
+  std::vector<StageSlot> stage;
+  size_t stage_next = 0;
+  cudaEvent_t export_ev = nullptr;     // behind the last fenc_ct_export_async (fenc_export_wait)
 };
 
 struct fenc_keys {

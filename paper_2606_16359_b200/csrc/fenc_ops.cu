@@ -223,6 +223,27 @@ extern "C" fenc_status fenc_ct_export(fenc_ctx *ctx, const fenc_ct *ct, uint64_t
   CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
   return FENC_OK;
 }
+// Export without the host synchronisation: inverse transform and device->host copy are enqueued on the context's stream
+// and an event is recorded behind them; fenc_export_wait blocks on that event only, so a caller can enqueue the next
+// request's work before it collects this one's result.
+extern "C" fenc_status fenc_ct_export_async(fenc_ctx *ctx, const fenc_ct *ct, uint64_t *limbs) {
+  Scope sc(ctx);
+  if (!ctx || !ct || !limbs) return FENC_ERR_INVALID_ARG;
+  LevelPlan *P = get_plan(ctx, ct->L);
+  const size_t n = (size_t)2 * ct->L * ctx->N;
+  u64 *tmp = sc.alloc<u64>(n);  // returns to the pool behind the copy (same stream)
+  if (!P || !tmp) return fail(ctx, FENC_ERR_OOM, "export");
+  if (!ctx->export_ev) CUDA_OK(ctx, cudaEventCreateWithFlags(&ctx->export_ev, cudaEventDisableTiming));
+  CUDA_OK(ctx, k_intt(ctx->k, nullptr, ct->d, 0, false, tmp, 0, P->d_rows_ct, 2 * ct->L, P->d_scale_ct, 1));
+  CUDA_OK(ctx, cudaMemcpyAsync(limbs, tmp, n * 8, cudaMemcpyDeviceToHost, ctx->stream));
+  CUDA_OK(ctx, cudaEventRecord(ctx->export_ev, ctx->stream));
+  return FENC_OK;
+}
+extern "C" fenc_status fenc_export_wait(fenc_ctx *ctx) {
+  if (!ctx) return FENC_ERR_INVALID_ARG;
+  if (ctx->export_ev) CUDA_OK(ctx, cudaEventSynchronize(ctx->export_ev));
+  return FENC_OK;
+}
 extern "C" fenc_status fenc_ct_import(fenc_ctx *ctx, const uint64_t *limbs, uint32_t L, double scale, fenc_ct **out) {
   Scope sc(ctx);
   if (!ctx || !limbs || !out || L < 1 || (int)L > ctx->nq) return FENC_ERR_INVALID_ARG;
@@ -233,6 +254,46 @@ extern "C" fenc_status fenc_ct_import(fenc_ctx *ctx, const uint64_t *limbs, uint
   CUDA_OK(ctx, cudaMemcpyAsync(ct->d, limbs, n * 8, cudaMemcpyHostToDevice, ctx->stream));
   CUDA_OK(ctx, k_ntt(ctx->k, ct->d, 0, ct->d, 0, P->d_rows_ct, 2 * (int)L, 1));
   CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+  sc.ok = true;
+  *out = ct;
+  return FENC_OK;
+}
+// The same import without a host synchronisation and with the copy off the compute stream: the limbs go to a slot of a
+// staging ring on the context's copy stream (overlapping whatever the compute stream is running), the compute stream
+// waits for that copy only, transforms staging -> ciphertext, and releases the slot.  A slot is never touched by any
+// other kernel, so the copy has to wait for nothing but the transform that last read the slot.
+extern "C" fenc_status fenc_ct_import_async(fenc_ctx *ctx, const uint64_t *limbs, uint32_t L, double scale, fenc_ct **out) {
+  Scope sc(ctx);
+  if (!ctx || !limbs || !out || L < 1 || (int)L > ctx->nq) return FENC_ERR_INVALID_ARG;
+  LevelPlan *P = get_plan(ctx, (int)L);
+  fenc_ct *ct = sc.ct((int)L, scale > 0 ? scale : ctx->default_scale);
+  if (!P || !ct) return fail(ctx, FENC_ERR_OOM, "import");
+  const size_t bytes = (size_t)2 * L * ctx->N * 8;
+  if (!ctx->copy_stream) CUDA_OK(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+  if (ctx->stage.empty()) ctx->stage.resize(FENC_STAGE_SLOTS);
+  size_t n_slots = FENC_STAGE_BYTES / bytes;
+  n_slots = n_slots < 2 ? 2 : (n_slots > FENC_STAGE_SLOTS ? FENC_STAGE_SLOTS : n_slots);
+  StageSlot &sl = ctx->stage[ctx->stage_next++ % n_slots];
+  if (!sl.copied) {
+    CUDA_OK(ctx, cudaEventCreateWithFlags(&sl.copied, cudaEventDisableTiming));
+    CUDA_OK(ctx, cudaEventCreateWithFlags(&sl.consumed, cudaEventDisableTiming));
+  }
+  if (sl.bytes < bytes) {
+    // the old buffer returns to the pool behind the transform that last read it; the new one may come from the pool
+    // with compute-stream work still pending on it, so its first copy waits for everything enqueued so far
+    dfree(ctx, sl.d);
+    sl.bytes = 0;
+    sl.d = (u64 *)dalloc(ctx, bytes);
+    if (!sl.d) return fail(ctx, FENC_ERR_OOM, "import staging (%zu bytes)", bytes);
+    sl.bytes = bytes;
+    CUDA_OK(ctx, cudaEventRecord(sl.consumed, ctx->stream));
+  }
+  CUDA_OK(ctx, cudaStreamWaitEvent(ctx->copy_stream, sl.consumed, 0));
+  CUDA_OK(ctx, cudaMemcpyAsync(sl.d, limbs, bytes, cudaMemcpyHostToDevice, ctx->copy_stream));
+  CUDA_OK(ctx, cudaEventRecord(sl.copied, ctx->copy_stream));
+  CUDA_OK(ctx, cudaStreamWaitEvent(ctx->stream, sl.copied, 0));
+  CUDA_OK(ctx, k_ntt(ctx->k, sl.d, 0, ct->d, 0, P->d_rows_ct, 2 * (int)L, 1));
+  CUDA_OK(ctx, cudaEventRecord(sl.consumed, ctx->stream));
   sc.ok = true;
   *out = ct;
   return FENC_OK;

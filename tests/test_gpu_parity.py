@@ -298,6 +298,43 @@ def test_rotation_wide_digit_groups(mods, n_q, q_bits, n_p, dnum):
     ctx.close()
 
 
+def test_import_async_matches_import(mods):
+    """fenc_ct_import_async (copy stream + staging ring) gives the ciphertexts of fenc_ct_import, also when the ring wraps
+    (more uploads in flight than slots would be needed: 70 > 64), when the level changes between uploads, and with work
+    queued on the compute stream in between."""
+    import torch
+    ck, fr, fenc = mods
+    P, ctx = make(mods, "mid12")
+    gk = ctx.keygen(3, [1])
+    hosts = []
+    for i in range(70):
+        L = P.nq if i % 3 else P.nq - 2
+        a = wl.random_ct_limbs(500 + i, P.q, L, P.N)
+        hosts.append(torch.from_numpy(a.view(np.int64)).pin_memory())
+    views = [t.numpy().view(np.uint64) for t in hosts]
+    cts = []
+    for i, a in enumerate(views):
+        cts.append(ctx.ct_import_async(a))
+        if i % 7 == 0:
+            cts[-1] = ctx.rotate(gk, [cts[-1]], [0])[0]  # compute-stream work between uploads (step 0: a copy)
+    for a, c in zip(views, cts):
+        assert c.L == a.shape[1]
+        assert np.array_equal(ctx.ct_export(c), a)
+    ref = ctx.rotate(gk, [ctx.ct_import(views[1])], [1])[0]
+    got = ctx.rotate(gk, [ctx.ct_import_async(views[1])], [1])[0]
+    assert np.array_equal(ctx.ct_export(got), ctx.ct_export(ref))
+    # asynchronous export: results land in page-locked buffers, complete after export_wait, with later work enqueued behind
+    outs = [torch.zeros(v.shape, dtype=torch.int64).pin_memory().numpy().view(np.uint64) for v in views[:5]]
+    for c, o in zip(cts[:5], outs):
+        ctx.ct_export_async(c, o)
+    later = ctx.rotate(gk, [cts[1]], [1])[0]
+    ctx.export_wait()
+    for a, o in zip(views[:5], outs):
+        assert np.array_equal(a, o)
+    assert np.array_equal(ctx.ct_export(later), ctx.ct_export(ref))
+    ctx.close()
+
+
 # ------------------------------------------------------------------------------------------------ fc, pooling, pipeline
 @pytest.mark.parametrize("kw", [
     dict(BS=2, n_in=32, n_out=5, in_C=2, in_H=4, in_W=4, in_M=4),
