@@ -102,9 +102,9 @@ def lenet_layers(BS, seed, upto="fc"):
         f2 = rng.normal(0, 0.1, (84, 120))
         f3 = rng.normal(0, 0.1, (10, 84))
         layers += [
-            {"op": "fc", "fc": dict(BS=BS, n_in=400, n_out=120, in_C=16, in_H=5, in_W=5, in_M=8), "w": f1},
-            {"op": "fc", "fc": dict(BS=BS, n_in=120, n_out=84, in_M=8), "w": f2},
-            {"op": "fc", "fc": dict(BS=BS, n_in=84, n_out=10, in_M=8), "w": f3},
+            {"op": "fc", "fc": dict(BS=BS, n_in=400, n_out=120, in_C=16, in_H=5, in_W=5, in_M=8, bsgs=0), "w": f1},
+            {"op": "fc", "fc": dict(BS=BS, n_in=120, n_out=84, in_M=8, bsgs=0), "w": f2},
+            {"op": "fc", "fc": dict(BS=BS, n_in=84, n_out=10, in_M=8, bsgs=0), "w": f3},
         ]
     x = rng.uniform(0, 1, (BS, 1, 28, 28))
     return layers, x

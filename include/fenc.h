@@ -204,13 +204,22 @@ fenc_status fenc_hconv(fenc_ctx *ctx, const fenc_keys *keys, const fenc_conv_des
  *   out_{c'} = sum_d Rot( sum_c x_c (*) Wd(c',c,d), d*B ),  Wd(c',c,d)[p] = W[nu(c',(p-d) mod P)][feat(c,p)] or 0.
  * Input features: in_C > 0: the S=1 fragment layout of a [BS][in_C][in_H][in_W] tensor in an in_M x in_M frame
  * (PyTorch flatten order feat = channel*H*W + h*W + w); in_C = 0: the output layout of a previous fc (feat = c*P + p).
- * B = min(next_pow2(BS), (N/2)/in_M^2) samples per ciphertext, as in the conv layouts it chains with. */
+ * B = min(next_pow2(BS), (N/2)/in_M^2) samples per ciphertext, as in the conv layouts it chains with.
+ * Baby-step giant-step ("diagonal-matrix multiplication with BSGS"; R2.12b): with bsgs = g > 1 (a power of
+ * two dividing P) a diagonal is d = i g + j and
+ *   out_{c'} = sum_i Rot( sum_j sum_c Rot(x_c, j B) (*) W'(c',c,d), i g B ),  W'(c',c,d) = Rot(Wd(c',c,d), j B):
+ * (g-1) baby rotations per input ciphertext, shared by every output, and P/g - 1 giant rotations per output ciphertext
+ * instead of P - 1.  bsgs = 0 or 1: plain diagonals; FENC_FC_BSGS_AUTO: the g with the fewest rotations
+ * n_in_ct (g-1) + n_out_ct (P/g - 1), ties to the smaller g.  The weight calls take the same descriptor (the keys stay
+ * (c', c, d); the plaintext of a key is W'). */
+#define FENC_FC_BSGS_AUTO 0xFFFFFFFFu
 typedef struct {
   uint32_t BS, n_in, n_out;
   uint32_t in_C, in_H, in_W, in_M;
+  uint32_t bsgs;
 } fenc_fc_desc;
 typedef struct {
-  uint32_t B, P, BG, n_in_ct, n_out_ct, n_rot, n_pmult, n_distinct_pt, n_rot_keys;
+  uint32_t B, P, BG, n_in_ct, n_out_ct, n_rot /* baby + giant */, n_pmult, n_distinct_pt, n_rot_keys, bsgs /* g used */;
   int32_t rot_steps[512];
 } fenc_fc_info;
 fenc_status fenc_fc_plan(fenc_ctx *ctx, const fenc_fc_desc *fc, fenc_fc_info *out);

@@ -14,12 +14,31 @@ from . import fragment as fr
 
 
 # --------------------------------------------------------------------------- FC by plain diagonals (R2.12)
+def bsgs_auto(P, n_in_ct, n_out_ct):
+    """baby-step count g (a power of two dividing P) with the fewest rotations n_in_ct (g-1) + n_out_ct (P/g - 1) of a
+    dense layer; ties go to the smaller g (R2.12b)."""
+    best, g = None, 1
+    while g <= P:
+        cost = n_in_ct * (g - 1) + n_out_ct * (P // g - 1)
+        if best is None or cost < best[0]:
+            best = (cost, g)
+        g *= 2
+    return best[1]
+
+
 class FcGraph:
     """Position p = cpos*m^2 + k in [0, P), P = n/B.  Input feature <-> (input ct c, p); neuron nu <-> (output ct c', p),
     nu = c'*P + p.  out_{c'} = sum_d Rot(sum_c x_c (*) Wd(c', c, d), d*B), Wd(c', c, d)[p] = W[nu(c', (p-d) mod P), feat(c, p)]
-    or 0 when either index is invalid; terms whose Wd is identically zero are skipped."""
+    or 0 when either index is invalid; terms whose Wd is identically zero are skipped.
 
-    def __init__(self, n, BS, n_in, n_out, in_C=0, in_H=0, in_W=0, in_M=1):
+    Baby-step giant-step ("diagonal-matrix multiplication with BSGS"; R2.12b): with g baby steps a diagonal
+    is d = i g + j, 0 <= j < g, and since Rot(x (*) w, r) = Rot(x, r) (*) Rot(w, r),
+        out_{c'} = sum_i Rot( sum_j sum_c Rot(x_c, j B) (*) W'(c', c, d), i g B ),   W'(c', c, d) = Rot(Wd(c', c, d), j B),
+    i.e. W'(c', c, d)[p] = W[nu(c', (p - i g) mod P), feat(c, (p + j) mod P)].  The baby rotations Rot(x_c, j B) are
+    computed once per input ciphertext and shared by every output and giant step.  bsgs = 1: plain diagonals (no baby
+    rotation, W' = Wd); bsgs = 0: g = bsgs_auto(P, n_in_ct, n_out_ct)."""
+
+    def __init__(self, n, BS, n_in, n_out, in_C=0, in_H=0, in_W=0, in_M=1, bsgs=1):
         self.n, self.BS, self.n_in, self.n_out = n, BS, n_in, n_out
         self.in_C, self.in_H, self.in_W, self.m = in_C, in_H, in_W, in_M
         m2 = in_M * in_M
@@ -34,14 +53,17 @@ class FcGraph:
         else:
             self.n_in_ct = -(-n_in // self.P)
         self.n_out_ct = -(-n_out // self.P)
-        self.terms = {}  # c' -> {d: [(c, wkey (c', c, d))]}
+        self.g = bsgs if bsgs >= 1 else bsgs_auto(self.P, self.n_in_ct, self.n_out_ct)
+        assert self.P % self.g == 0
+        self.terms = {}  # c' -> {giant step i: [(c, baby step j, wkey (c', c, d = i g + j))]}
         for co in range(self.n_out_ct):
-            diags = {}
-            for d in range(self.P):
-                lst = [(ci, (co, ci, d)) for ci in range(self.n_in_ct) if self.nonzero(co, ci, d)]
+            giants = {}
+            for i in range(self.P // self.g):
+                lst = [(ci, j, (co, ci, i * self.g + j)) for j in range(self.g) for ci in range(self.n_in_ct)
+                       if self.nonzero(co, ci, i * self.g + j)]
                 if lst:
-                    diags[d] = lst
-            self.terms[co] = diags
+                    giants[i] = lst
+            self.terms[co] = giants
 
     def feat(self, c, p):
         """PyTorch flatten order channel*H*W + h*W + w through the S=1 layout, or c*P + p after a previous fc."""
@@ -64,32 +86,40 @@ class FcGraph:
 
     def weight_slots(self, wkey, W):
         co, ci, d = wkey
+        j = d % self.g
         vec = np.zeros(self.n)
         for p in range(self.P):
-            f, v = self.feat(ci, p), self.neuron(co, (p - d) % self.P)
+            f, v = self.feat(ci, (p + j) % self.P), self.neuron(co, (p + j - d) % self.P)
             if f >= 0 and v >= 0:
                 vec[p * self.B:(p + 1) * self.B] = W[v, f]
         return vec
 
+    def baby_steps(self):
+        """distinct (input ct, j != 0) pairs some term uses"""
+        return sorted({(ci, j) for giants in self.terms.values() for lst in giants.values() for ci, j, _ in lst if j})
+
     def counts(self):
-        n_rot = sum(len([d for d in diags if d]) for diags in self.terms.values())
-        n_pm = sum(len(lst) for diags in self.terms.values() for lst in diags.values())
-        steps = sorted({d * self.B % self.n for diags in self.terms.values() for d in diags if d})
+        n_giant = sum(len([i for i in giants if i]) for giants in self.terms.values())
+        n_rot = n_giant + len(self.baby_steps())
+        n_pm = sum(len(lst) for giants in self.terms.values() for lst in giants.values())
+        steps = {i * self.g * self.B % self.n for giants in self.terms.values() for i in giants if i}
+        steps |= {j * self.B % self.n for _, j in self.baby_steps()}
         return dict(n_in_ct=self.n_in_ct * self.BG, n_out_ct=self.n_out_ct * self.BG, n_rot=n_rot * self.BG,
-                    n_pmult=n_pm * self.BG, n_distinct_pt=n_pm, rot_steps=steps)
+                    n_pmult=n_pm * self.BG, n_distinct_pt=n_pm, rot_steps=sorted(steps), bsgs=self.g)
 
     def run(self, be, inputs, weights):
         """inputs: list of n_in_ct items of ONE batch group; returns list of n_out_ct items."""
+        baby = {(ci, j): be.rot(inputs[ci], j * self.B % self.n) for ci, j in self.baby_steps()}
         out = []
         for co in range(self.n_out_ct):
             y = None
-            for d in sorted(self.terms[co]):
+            for i in sorted(self.terms[co]):
                 acc = be.zero()
-                for ci, wkey in self.terms[co][d]:
-                    be.pmult_acc(acc, inputs[ci], weights[wkey])
+                for ci, j, wkey in self.terms[co][i]:
+                    be.pmult_acc(acc, baby[(ci, j)] if j else inputs[ci], weights[wkey])
                 pd = be.wrap(acc)
-                if d:
-                    pd = be.rot(pd, d * self.B % self.n)
+                if i:
+                    pd = be.rot(pd, i * self.g * self.B % self.n)
                 y = pd if y is None else be.add(y, pd)
             out.append(y)
         return out
@@ -126,7 +156,7 @@ def fc_counts(n, **kw):
 def fc_slots(graph: FcGraph, X, W):
     """The fc graph on plain slot vectors -> Y[BS][n_out] (pin: must equal X @ W.T)."""
     be = fr.SlotBackend(graph.n)
-    Wp = {wk: graph.weight_slots(wk, W) for diags in graph.terms.values() for lst in diags.values() for _, wk in lst}
+    Wp = {wk: graph.weight_slots(wk, W) for giants in graph.terms.values() for lst in giants.values() for _, _, wk in lst}
     Y = np.zeros((graph.BS, graph.n_out))
     for bg in range(graph.BG):
         ins = [graph.gather_in(X, c, bg) for c in range(graph.n_in_ct)]
@@ -138,7 +168,7 @@ def fc_slots(graph: FcGraph, X, W):
 def encode_fc_weights(ck, params, graph: FcGraph, W, L, scale_w=None):
     sw = Fraction(params.q[L - 1]) if scale_w is None else Fraction(scale_w)
     return {wk: ck.encode(params, graph.weight_slots(wk, W), L, sw)
-            for diags in graph.terms.values() for lst in diags.values() for _, wk in lst}
+            for giants in graph.terms.values() for lst in giants.values() for _, _, wk in lst}
 
 
 def fc(ck, params, keys, graph: FcGraph, inputs, weights, do_rescale=True):

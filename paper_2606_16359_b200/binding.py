@@ -36,12 +36,12 @@ class ConvDesc(C.Structure):
 
 
 class FcDesc(C.Structure):
-    _fields_ = [(k, C.c_uint32) for k in ("BS", "n_in", "n_out", "in_C", "in_H", "in_W", "in_M")]
+    _fields_ = [(k, C.c_uint32) for k in ("BS", "n_in", "n_out", "in_C", "in_H", "in_W", "in_M", "bsgs")]
 
 
 class FcInfo(C.Structure):
     _fields_ = [(k, C.c_uint32) for k in ("B", "P", "BG", "n_in_ct", "n_out_ct", "n_rot", "n_pmult", "n_distinct_pt",
-                                          "n_rot_keys")] + [("rot_steps", C.c_int32 * 512)]
+                                          "n_rot_keys", "bsgs")] + [("rot_steps", C.c_int32 * 512)]
 
 
 class Layout(C.Structure):
@@ -492,8 +492,9 @@ class Context:
         return [Ciphertext(self, C.c_void_p(out[i])) for i in range(n.value)]
 
     # ---- FC by plain diagonals
-    def fc_desc(self, BS, n_in, n_out, in_C=0, in_H=0, in_W=0, in_M=1):
-        return FcDesc(BS, n_in, n_out, in_C, in_H, in_W, in_M)
+    def fc_desc(self, BS, n_in, n_out, in_C=0, in_H=0, in_W=0, in_M=1, bsgs=1):
+        """bsgs: baby-step count g (1 = plain diagonals, 0 = the library's choice, FENC_FC_BSGS_AUTO)"""
+        return FcDesc(BS, n_in, n_out, in_C, in_H, in_W, in_M, 0xFFFFFFFF if bsgs == 0 else bsgs)
 
     def fc_plan(self, fc):
         info = FcInfo()

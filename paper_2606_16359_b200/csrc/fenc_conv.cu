@@ -560,10 +560,12 @@ extern "C" fenc_status fenc_compress(fenc_ctx *ctx, const fenc_keys *K, fenc_ct 
   return FENC_OK;
 }
 
-// ------------------------------------------------------------------------------------------------ FC by plain diagonals (R2.12)
+// ------------------------------------------------------------------------------------------------ FC by diagonals (R2.12, R2.12b)
+// With g baby steps (d = i g + j):  out_{c'} = sum_i Rot( sum_j sum_c Rot(x_c, j B) (*) Rot(Wd(c',c,d), j B), i g B ):
+// the baby rotations are the executor's inner rotations (once per input ciphertext), the giant ones its outer rotations.
 struct FcGraph : LinGraph {
   fenc_fc_desc d;
-  int n, B, P, m, ch, n_in_ct, n_out_ct;
+  int n, B, P, m, ch, n_in_ct, n_out_ct, g = 1;
   std::vector<std::array<u32, 3>> wkeys;  // (c_out_ct, c_in_ct, d)
   // feature index of (input ct c, position p) or -1
   long feat(int c, int p) const {
@@ -586,9 +588,9 @@ struct FcGraph : LinGraph {
   }
   void weight_slots(const std::array<u32, 3> &wk, const double *w, std::vector<double> &vec) const {
     vec.assign(n, 0.0);
-    const int co = wk[0], ci = wk[1], dd = wk[2];
+    const int co = wk[0], ci = wk[1], dd = wk[2], j = dd % g;  // the diagonal, rotated left by its baby step
     for (int p = 0; p < P; p++) {
-      const long f = feat(ci, p), v = neuron(co, ((p - dd) % P + P) % P);
+      const long f = feat(ci, (p + j) % P), v = neuron(co, ((p + j - dd) % P + P) % P);
       if (f < 0 || v < 0) continue;
       const double val = w[(size_t)v * d.n_in + f];
       for (int b = 0; b < B; b++) vec[(size_t)p * B + b] = val;
@@ -598,7 +600,7 @@ struct FcGraph : LinGraph {
 
 static fenc_status fc_graph(fenc_ctx *ctx, const fenc_fc_desc *fd, std::shared_ptr<FcGraph> &out) {
   char keybuf[256];
-  snprintf(keybuf, sizeof keybuf, "fc,%u,%u,%u,%u,%u,%u,%u", fd->BS, fd->n_in, fd->n_out, fd->in_C, fd->in_H, fd->in_W, fd->in_M);
+  snprintf(keybuf, sizeof keybuf, "fc,%u,%u,%u,%u,%u,%u,%u,%u", fd->BS, fd->n_in, fd->n_out, fd->in_C, fd->in_H, fd->in_W, fd->in_M, fd->bsgs);
   auto it = ctx->graphs.find(keybuf);
   if (it != ctx->graphs.end()) {
     out = std::static_pointer_cast<FcGraph>(it->second);
@@ -622,25 +624,44 @@ static fenc_status fc_graph(fenc_ctx *ctx, const fenc_fc_desc *fd, std::shared_p
   }
   g->n_out_ct = (fd->n_out + g->P - 1) / g->P;
   g->nin_bg = g->n_in_ct;
+  // baby-step count: 1 (or 0) = plain diagonals; FENC_FC_BSGS_AUTO = the power of two g | P with the fewest rotations
+  // n_in_ct (g-1) + n_out_ct (P/g - 1) of a dense layer, ties to the smaller g; else a power of two dividing P
+  int gs = fd->bsgs <= 1 ? 1 : (int)fd->bsgs;
+  if (fd->bsgs == FENC_FC_BSGS_AUTO) {
+    long best = -1;
+    for (int c = 1; c <= g->P; c *= 2) {
+      const long cost = (long)g->n_in_ct * (c - 1) + (long)g->n_out_ct * (g->P / c - 1);
+      if (best < 0 || cost < best) best = cost, gs = c;
+    }
+  }
+  if (gs < 1 || gs > g->P || g->P % gs || (gs & (gs - 1))) return fail(ctx, FENC_ERR_LAYOUT, "bsgs=%d must be a power of two dividing P=%d", gs, g->P);
+  g->g = gs;
   std::set<int> steps;
+  std::set<std::pair<int, int>> inner;
   g->outs.resize(g->n_out_ct);
   for (int co = 0; co < g->n_out_ct; co++) {
     OutCt &oc = g->outs[co];
-    for (int dd = 0; dd < g->P; dd++) {
+    for (int i = 0; i < g->P / gs; i++) {
       std::vector<Term> lst;
-      for (int ci = 0; ci < g->n_in_ct; ci++) {
-        if (!g->nonzero(co, ci, dd)) continue;
-        lst.push_back(Term{ci, 0, (int)g->wkeys.size()});
-        g->wkeys.push_back({(u32)co, (u32)ci, (u32)dd});
-      }
+      for (int j = 0; j < gs; j++)
+        for (int ci = 0; ci < g->n_in_ct; ci++) {
+          const int dd = i * gs + j;
+          if (!g->nonzero(co, ci, dd)) continue;
+          const int amt = (int)(((long)j * g->B) % g->n);
+          lst.push_back(Term{ci, amt, (int)g->wkeys.size()});
+          g->wkeys.push_back({(u32)co, (u32)ci, (u32)dd});
+          if (amt) inner.insert({ci, amt}), steps.insert(amt);
+        }
       if (lst.empty()) continue;
-      const int rot = (int)(((long)dd * g->B) % g->n);
-      oc.diags.push_back(dd), oc.rots.push_back(rot);
+      const int rot = (int)(((long)i * gs * g->B) % g->n);
+      oc.diags.push_back(i), oc.rots.push_back(rot);
       g->n_pmult += lst.size();
       oc.terms.push_back(std::move(lst));
-      if (dd) g->n_outer++, steps.insert(rot);
+      if (i) g->n_outer++, steps.insert(rot);
     }
   }
+  g->inner.assign(inner.begin(), inner.end());
+  for (size_t k = 0; k < g->inner.size(); k++) g->inner_index[g->inner[k]] = (int)k;
   g->rot_steps.assign(steps.begin(), steps.end());
   g->n_w = g->wkeys.size();
   ctx->graphs[keybuf] = g;
@@ -653,10 +674,10 @@ extern "C" fenc_status fenc_fc_plan(fenc_ctx *ctx, const fenc_fc_desc *fd, fenc_
   std::shared_ptr<FcGraph> g;
   fenc_status st = fc_graph(ctx, fd, g);
   if (st != FENC_OK) return st;
-  if (g->rot_steps.size() > 512) return fail(ctx, FENC_ERR_LAYOUT, "more than 512 rotation amounts (plain diagonals need B large; BSGS is not built)");
+  if (g->rot_steps.size() > 512) return fail(ctx, FENC_ERR_LAYOUT, "more than 512 rotation amounts (use more baby steps or a larger B)");
   memset(out, 0, sizeof *out);
   out->B = g->B, out->P = g->P, out->BG = (u32)g->BG, out->n_in_ct = g->n_in_ct * (u32)g->BG, out->n_out_ct = g->n_out_ct * (u32)g->BG;
-  out->n_rot = (u32)(g->n_outer * g->BG), out->n_pmult = (u32)(g->n_pmult * g->BG), out->n_distinct_pt = (u32)g->wkeys.size();
+  out->n_rot = (u32)((g->n_outer + g->inner.size()) * g->BG), out->bsgs = (u32)g->g, out->n_pmult = (u32)(g->n_pmult * g->BG), out->n_distinct_pt = (u32)g->wkeys.size();
   out->n_rot_keys = (u32)g->rot_steps.size();
   for (size_t i = 0; i < g->rot_steps.size(); i++) out->rot_steps[i] = g->rot_steps[i];
   return FENC_OK;

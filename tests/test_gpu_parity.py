@@ -340,6 +340,11 @@ def test_import_async_matches_import(mods):
     dict(BS=2, n_in=32, n_out=5, in_C=2, in_H=4, in_W=4, in_M=4),
     dict(BS=40, n_in=3 * 3 * 3, n_out=20, in_C=3, in_H=3, in_W=3, in_M=4),   # B=32, BG=2, P=16, two output cts
     dict(BS=64, n_in=20, n_out=11, in_M=4),                                  # flat input
+    # baby-step giant-step (R2.12b): explicit g and the library's choice (bsgs=0), several input / output ciphertexts
+    dict(BS=2, n_in=32, n_out=5, in_C=2, in_H=4, in_W=4, in_M=4, bsgs=4),
+    dict(BS=40, n_in=3 * 3 * 3, n_out=20, in_C=3, in_H=3, in_W=3, in_M=4, bsgs=0),
+    dict(BS=64, n_in=20, n_out=11, in_M=4, bsgs=2),
+    dict(BS=16, n_in=70, n_out=40, in_M=2, bsgs=0),                          # P = 32: 3 input cts, 2 output cts
 ])
 def test_fc_bit_exact(mods, kw):
     ck, fr, fenc = mods
@@ -350,6 +355,8 @@ def test_fc_bit_exact(mods, kw):
     info = ctx.fc_plan(fcd)
     c = g.counts()
     assert {k: info[k] for k in c} == c
+    if kw.get("bsgs", 1) != 1:
+        assert info["bsgs"] > 1 and info["n_rot"] < nw.FcGraph(P.n, **dict(kw, bsgs=1)).counts()["n_rot"]
     L = P.nq
     rng = np.random.default_rng(9)
     X = rng.uniform(-1, 1, (kw["BS"], kw["n_in"]))
@@ -379,7 +386,8 @@ def test_fc_bit_exact(mods, kw):
     ctx.close()
 
 
-def test_pipeline_toy_network_bit_exact(mods):
+@pytest.mark.parametrize("bsgs", [1, 0])
+def test_pipeline_toy_network_bit_exact(mods, bsgs):
     """conv - square - pool - fc - fc through Pipeline (one batched C-ABI call per layer) vs the oracle's network."""
     ck, fr, fenc = mods
     from oracle import network as nw
@@ -388,7 +396,7 @@ def test_pipeline_toy_network_bit_exact(mods):
     p = dict(log2N=9, n_q=5, q_bits=40, n_p=2, p_bits=60, dnum=3, log2_scale=40)
     P = ck.Params(*wl.oracle_params_args(p))
     ctx = fenc.Context(**p)
-    layers, x = toy_network()
+    layers, x = toy_network(bsgs=bsgs)
     pipe = Pipeline(ctx, layers)
     steps, relin = nw.network_rot_steps(layers, P.n)
     assert sorted(pipe.steps) == steps and pipe.need_relin == relin
@@ -401,7 +409,8 @@ def test_pipeline_toy_network_bit_exact(mods):
             oW = fr.encode_weights(ck, P, g, entry["w"], L)
             return np.stack([oW[tuple(int(v) for v in k)].coeffs for k in ctx.wts_keys(entry["conv"], entry["lay"])])
         fcd = entry["fc"]
-        g = nw.FcGraph(P.n, **{k: int(getattr(fcd, k)) for k in ("BS", "n_in", "n_out", "in_C", "in_H", "in_W", "in_M")})
+        g = nw.FcGraph(P.n, **{k: int(getattr(fcd, k)) for k in ("BS", "n_in", "n_out", "in_C", "in_H", "in_W", "in_M")},
+                       bsgs=0 if fcd.bsgs == 0xFFFFFFFF else int(fcd.bsgs))
         oW = nw.encode_fc_weights(ck, P, g, entry["w"], L)
         return np.stack([oW[tuple(int(v) for v in k)].coeffs for k in ctx.fc_wts_keys(fcd)])
 

@@ -16,6 +16,7 @@ from oracle import network as nw
     dict(n=64, BS=16, n_in=9, n_out=6, in_M=2),                                # B = 16, P = 4: 3 input cts, 2 output cts
 ])
 def test_fc_graph_equals_dense_product(kw):
+    kw = dict(kw)
     n = kw.pop("n")
     g = nw.FcGraph(n, **kw)
     rng = np.random.default_rng(3)
@@ -26,6 +27,41 @@ def test_fc_graph_equals_dense_product(kw):
     # every existing non-zero diagonal costs one rotation per output ciphertext; d*B are the amounts
     assert c["n_rot"] == g.BG * sum(len([d for d in diags if d]) for diags in g.terms.values())
     assert all(s % g.B == 0 and 0 < s < n for s in c["rot_steps"])
+
+
+@pytest.mark.parametrize("bsgs", [2, 4, 0])
+@pytest.mark.parametrize("kw", [
+    dict(n=256, BS=2, n_in=32, n_out=5, in_C=2, in_H=4, in_W=4, in_M=4),
+    dict(n=256, BS=5, n_in=3 * 3 * 3, n_out=70, in_C=3, in_H=3, in_W=3, in_M=4),
+    dict(n=64, BS=40, n_in=10, n_out=7, in_M=2),
+    dict(n=64, BS=16, n_in=9, n_out=6, in_M=2),
+    dict(n=512, BS=8, n_in=150, n_out=120, in_M=2),                            # dense: P = 64, 3 input cts, 2 output cts
+])
+def test_fc_bsgs_equals_dense_product(kw, bsgs):
+    """R2.12b: the baby-step giant-step regrouping computes the same product (pre-rotated diagonals, baby rotations on
+    the inputs, giant rotations on the sums), with the rotation count of the closed form on a dense layer."""
+    kw = dict(kw)
+    n = kw.pop("n")
+    g = nw.FcGraph(n, bsgs=bsgs, **kw)
+    plain = nw.FcGraph(n, **kw)
+    rng = np.random.default_rng(4)
+    X = rng.uniform(-1, 1, (kw["BS"], kw["n_in"]))
+    W = rng.normal(0, 1, (kw["n_out"], kw["n_in"]))
+    assert np.abs(nw.fc_slots(g, X, W) - X @ W.T).max() < 1e-12
+    c, cp = g.counts(), plain.counts()
+    assert c["n_pmult"] == cp["n_pmult"] and c["bsgs"] == g.g and g.P % g.g == 0
+    assert c["n_rot"] <= g.BG * (g.n_in_ct * (g.g - 1) + g.n_out_ct * (g.P // g.g - 1))
+    if kw["n_in"] == 150:  # dense: every (input ct, baby step) and (output ct, giant step) exists
+        assert c["n_rot"] == g.BG * (g.n_in_ct * (g.g - 1) + g.n_out_ct * (g.P // g.g - 1))
+        if bsgs == 0:  # 3 (g-1) + 2 (64/g - 1): g = 4 -> 39, g = 8 -> 35, g = 16 -> 51
+            assert g.g == 8 and c["n_rot"] == 35 and cp["n_rot"] == 2 * 63
+
+
+def test_bsgs_auto_rule():
+    # LeNet-5 (config 2, P = 64): 16 -> 2, 2 -> 2, 2 -> 1 ciphertexts; ties go to the smaller g
+    assert nw.bsgs_auto(64, 16, 2) == 2 and 16 * 1 + 2 * 31 == 78 == 16 * 3 + 2 * 15
+    assert nw.bsgs_auto(64, 2, 2) == 8 and nw.bsgs_auto(64, 2, 1) == 4  # 2*3 + 15 == 2*7 + 7 == 21
+    assert nw.bsgs_auto(1, 3, 3) == 1
 
 
 def test_fc_conv_layout_matches_torch_flatten_order():
@@ -53,13 +89,13 @@ def test_pool_order_is_sum_pool_through_the_layout():
         assert np.abs(a - b).max() < 1e-12
 
 
-def toy_network(BS=2, seed=5):
+def toy_network(BS=2, seed=5, bsgs=1):
     rng = np.random.default_rng(seed)
     layers = [
         {"op": "conv", "conv": dict(BS=BS, C_in=1, H=8, W=8, C_out=2, K=3, stride=1, pad=1), "S": 2, "w": rng.normal(0, 0.3, (2, 1, 3, 3))},
         {"op": "square"}, {"op": "pool"},
-        {"op": "fc", "fc": dict(BS=BS, n_in=32, n_out=5, in_C=2, in_H=4, in_W=4, in_M=4), "w": rng.normal(0, 0.3, (5, 32)) * 0.25},
-        {"op": "fc", "fc": dict(BS=BS, n_in=5, n_out=3, in_M=4), "w": rng.normal(0, 0.3, (3, 5))},
+        {"op": "fc", "fc": dict(BS=BS, n_in=32, n_out=5, in_C=2, in_H=4, in_W=4, in_M=4, bsgs=bsgs), "w": rng.normal(0, 0.3, (5, 32)) * 0.25},
+        {"op": "fc", "fc": dict(BS=BS, n_in=5, n_out=3, in_M=4, bsgs=bsgs), "w": rng.normal(0, 0.3, (3, 5))},
     ]
     x = rng.uniform(0, 1, (BS, 1, 8, 8))
     return layers, x
@@ -80,9 +116,10 @@ def plain_network(layers, x):
     return x
 
 
-def test_encrypted_toy_network_matches_fp64():
+@pytest.mark.parametrize("bsgs", [1, 0])
+def test_encrypted_toy_network_matches_fp64(bsgs):
     P = ck.Params(9, 5, 40, 2, 60, 3, 40)
-    layers, x = toy_network()
+    layers, x = toy_network(bsgs=bsgs)
     steps, relin = nw.network_rot_steps(layers, P.n)
     keys = ck.keygen(P, 11, steps, want_relin=relin)
     lin = fr.Layout(P.n, 8, 2, 2, 1)
