@@ -39,6 +39,7 @@ for _name, _args in {
     "orc_moddown": [ctypes.c_void_p, ctypes.c_int, _u64p, _u64p],
     "orc_keyswitch": [ctypes.c_void_p, ctypes.c_int, _u64p, _u64p, _u64p, _u64p, _u64p],
     "orc_rotate": [ctypes.c_void_p, ctypes.c_int, ctypes.c_uint64, _u64p, _u64p, _u64p, _u64p],
+    "orc_rotate_hoisted": [ctypes.c_void_p, ctypes.c_int, ctypes.c_uint64, _u64p, _u64p, _u64p, _u64p],
     "orc_add": [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, _u64p, _u64p, _u64p],
     "orc_pmult_acc": [ctypes.c_void_p, ctypes.c_int, _u64p, _u64p, _u64p],
     "orc_polymul_rns": [ctypes.c_void_p, ctypes.c_int, _u64p, _u64p, _u64p],
@@ -411,6 +412,18 @@ def rotate(params: Params, keys: Keys, ct: Ciphertext, r: int) -> Ciphertext:
     b, a = keys.evk[r]
     out = np.zeros_like(ct.c)
     _lib.orc_rotate(params._h, ct.L, params.galois(r), _p(ct.c), _p(b), _p(a), _p(out))
+    return Ciphertext(out, ct.L, ct.scale)
+
+
+def rotate_hoisted(params: Params, keys: Keys, ct: Ciphertext, r: int) -> Ciphertext:
+    """Rot(ct, r) with the decomposition hoisted out of the rotation (R2.7b): ModUp of the unrotated c1, automorphism on
+    the extended digits.  Decrypts like rotate(); the limbs differ (a multiple of Q_j per digit before ModDown)."""
+    r %= params.n
+    if r == 0:
+        return Ciphertext(ct.c.copy(), ct.L, ct.scale)
+    b, a = keys.evk[r]
+    out = np.zeros_like(ct.c)
+    _lib.orc_rotate_hoisted(params._h, ct.L, params.galois(r), _p(ct.c), _p(b), _p(a), _p(out))
     return Ciphertext(out, ct.L, ct.scale)
 
 

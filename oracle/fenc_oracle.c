@@ -221,6 +221,39 @@ void orc_rotate(const orc_params *P, int L, u64 g, const u64 *ct, const u64 *key
     free(s0); free(s1);
 }
 
+/* ------------------------------------------------------------------ hoisted rotation (R2.7b)
+ * Several rotations of ONE ciphertext share the decomposition: up_j = ModUp_j(c1) is computed from the UNROTATED c1,
+ * and each rotation applies sigma_g to the extended digits instead of to c1:
+ *   acc_0[t] = sum_j sigma_g(up_j)[t] * b_j[t], acc_1 likewise;  result (sigma_g(c0) + ModDown(acc_0), ModDown(acc_1)).
+ * sigma_g(up_j) is congruent to sigma_g(c1) modulo the digit's primes and differs from ModUp_j(sigma_g(c1)) by a
+ * small multiple of Q_j on the other limbs, so the result decrypts to the same rotation with key-switch noise of the
+ * same size, but its limbs are NOT those of orc_rotate.  Same keys as orc_rotate. */
+void orc_rotate_hoisted(const orc_params *P, int L, u64 g, const u64 *ct, const u64 *key_b, const u64 *key_a, u64 *out) {
+    size_t N = P->N, LN = (size_t)L * N; int E = L + P->np, A = P->nq + P->np;
+    int beta = (L + P->dlen - 1) / P->dlen;
+    u64 *up = malloc((size_t)E * N * sizeof(u64)), *rot = malloc(N * sizeof(u64)), *prod = malloc(N * sizeof(u64));
+    u64 *acc0 = calloc((size_t)E * N, sizeof(u64)), *acc1 = calloc((size_t)E * N, sizeof(u64));
+    for (int j = 0; j < beta; j++) {
+        orc_modup(P, L, j, ct + LN, up);
+        for (int row = 0; row < E; row++) {
+            int mi = ext_mod(P, L, row); u64 t = P->mod[mi], psi = P->psi[mi];
+            const u64 *kb = key_b + ((size_t)j * A + mi) * N, *ka = key_a + ((size_t)j * A + mi) * N;
+            orc_automorph(N, t, g, up + (size_t)row * N, rot);
+            orc_polymul(N, t, psi, rot, kb, prod);
+            for (size_t n = 0; n < N; n++) acc0[(size_t)row * N + n] = orc_addmod(acc0[(size_t)row * N + n], prod[n], t);
+            orc_polymul(N, t, psi, rot, ka, prod);
+            for (size_t n = 0; n < N; n++) acc1[(size_t)row * N + n] = orc_addmod(acc1[(size_t)row * N + n], prod[n], t);
+        }
+    }
+    orc_moddown(P, L, acc0, out);
+    orc_moddown(P, L, acc1, out + LN);
+    for (int t = 0; t < L; t++) {
+        orc_automorph(N, P->mod[t], g, ct + (size_t)t * N, rot);
+        for (size_t n = 0; n < N; n++) out[(size_t)t * N + n] = orc_addmod(out[(size_t)t * N + n], rot[n], P->mod[t]);
+    }
+    free(up); free(rot); free(prod); free(acc0); free(acc1);
+}
+
 /* ------------------------------------------------------------------ Add / PMult / Rescale (R2.8) */
 void orc_add(const orc_params *P, int L, int npoly, const u64 *a, const u64 *b, u64 *out) {
     size_t N = P->N;

@@ -226,7 +226,7 @@ class ConvGraph:
         """inputs: {(u, v, g_in): x}; weights: {wkey: w}.  Returns {(u_o, v_o, g_out): y}."""
         R = {}
         for src, amt in self.inner:
-            R[(src, amt)] = be.rot(inputs[src], amt)  # always from the original input, never chained
+            R[(src, amt)] = be.rot_in(inputs[src], amt)  # always from the original input, never chained
         out = {}
         for okey, diags in self.terms.items():
             y = None
@@ -250,6 +250,8 @@ class SlotBackend:
 
     def rot(self, x, r):
         return np.roll(x, -r)
+
+    rot_in = rot  # inner (input-side) rotations: the same shift
 
     def zero(self):
         return np.zeros(self.n)
@@ -337,12 +339,19 @@ def select_S(desc: ConvDesc, n):
 
 # --------------------------------------------------------------------------- encrypted HConv (R2.9)
 class CtBackend:
-    def __init__(self, ck, params, keys, L, scale_in, scale_w):
+    """hoist: the inner (input-side) rotations, several of which share one input ciphertext, use the hoisted form of
+    R2.7b (ck.rotate_hoisted); the outer rotations, each of a different sum, stay plain rotations."""
+
+    def __init__(self, ck, params, keys, L, scale_in, scale_w, hoist=False):
         self.ck, self.params, self.keys, self.L = ck, params, keys, L
         self.scale_in, self.scale_w = Fraction(scale_in), Fraction(scale_w)
+        self.hoist = hoist
 
     def rot(self, x, r):
         return self.ck.rotate(self.params, self.keys, x, r)
+
+    def rot_in(self, x, r):
+        return (self.ck.rotate_hoisted if self.hoist else self.ck.rotate)(self.params, self.keys, x, r)
 
     def zero(self):
         return np.zeros((2, self.L, self.params.N), dtype=np.uint64)
@@ -370,12 +379,12 @@ def encode_weights(ck, params, graph: ConvGraph, Kw, L, scale_w=None):
     return W
 
 
-def hconv(ck, params, keys, graph: ConvGraph, inputs, weights, do_rescale=True):
+def hconv(ck, params, keys, graph: ConvGraph, inputs, weights, do_rescale=True, hoist=False):
     """inputs {(u, v, g_in): Ciphertext} of ONE batch group -> {(u_o, v_o, g_out): Ciphertext};
     one rescale per output ciphertext after the outer-rotation sum (A13)."""
     any_in = next(iter(inputs.values()))
     any_w = next(iter(weights.values()))
-    be = CtBackend(ck, params, keys, any_in.L, any_in.scale, any_w.scale)
+    be = CtBackend(ck, params, keys, any_in.L, any_in.scale, any_w.scale, hoist)
     outs = graph.run(be, inputs, weights)
     if do_rescale:
         outs = {k: (ck.rescale(params, y) if y is not None else None) for k, y in outs.items()}

@@ -109,7 +109,7 @@ class FcGraph:
 
     def run(self, be, inputs, weights):
         """inputs: list of n_in_ct items of ONE batch group; returns list of n_out_ct items."""
-        baby = {(ci, j): be.rot(inputs[ci], j * self.B % self.n) for ci, j in self.baby_steps()}
+        baby = {(ci, j): be.rot_in(inputs[ci], j * self.B % self.n) for ci, j in self.baby_steps()}
         out = []
         for co in range(self.n_out_ct):
             y = None
@@ -171,10 +171,10 @@ def encode_fc_weights(ck, params, graph: FcGraph, W, L, scale_w=None):
             for giants in graph.terms.values() for lst in giants.values() for _, _, wk in lst}
 
 
-def fc(ck, params, keys, graph: FcGraph, inputs, weights, do_rescale=True):
+def fc(ck, params, keys, graph: FcGraph, inputs, weights, do_rescale=True, hoist=False):
     """inputs: list of Ciphertext of one batch group -> list of Ciphertext; one rescale per output (A13)."""
     w0 = next(iter(weights.values()))
-    be = fr.CtBackend(ck, params, keys, inputs[0].L, inputs[0].scale, w0.scale)
+    be = fr.CtBackend(ck, params, keys, inputs[0].L, inputs[0].scale, w0.scale, hoist)
     outs = graph.run(be, inputs, weights)
     return [ck.rescale(params, y) for y in outs] if do_rescale else outs
 
@@ -205,7 +205,7 @@ def sum_pool(ck, params, cts, S):
 
 
 # --------------------------------------------------------------------------- sequential network
-def run_network(ck, params, keys, layers, cts, L0):
+def run_network(ck, params, keys, layers, cts, L0, hoist=False):
     """layers as in paper_2606_16359_b200.pipeline.Pipeline (dicts with op = conv / square / pool / fc and fp64 weights);
     cts: oracle ciphertexts ordered [bg][g][u][v].  Returns (final ciphertext list, list of per-layer outputs)."""
     L, S, trace = L0, None, []
@@ -218,7 +218,7 @@ def run_network(ck, params, keys, layers, cts, L0):
             for bg in range(graph.lin.BG):
                 ins = {(u, v, g): cts[bg * per + (g * graph.S + u) * graph.S + v]
                        for g in range(graph.lin.G) for u in range(graph.S) for v in range(graph.S)}
-                o = fr.hconv(ck, params, keys, graph, ins, W)
+                o = fr.hconv(ck, params, keys, graph, ins, W, hoist=hoist)
                 So = graph.S_out
                 out += [o[(uo, vo, go)] for go in range(graph.lout.G) for uo in range(So) for vo in range(So)]
             cts, S, L = out, graph.S_out, L - 1
@@ -227,7 +227,7 @@ def run_network(ck, params, keys, layers, cts, L0):
             W = encode_fc_weights(ck, params, graph, ly["w"], L)
             out = []
             for bg in range(graph.BG):
-                out += fc(ck, params, keys, graph, cts[bg * graph.n_in_ct:(bg + 1) * graph.n_in_ct], W)
+                out += fc(ck, params, keys, graph, cts[bg * graph.n_in_ct:(bg + 1) * graph.n_in_ct], W, hoist=hoist)
             cts, S, L = out, 1, L - 1
         elif ly["op"] == "square":
             cts, L = [ck.square_relin(params, keys, c) for c in cts], L - 1

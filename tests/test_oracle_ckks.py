@@ -344,6 +344,28 @@ def test_rotation_is_left_cyclic_shift(toy, toy_keys):
     assert np.abs(ck.decrypt_decode(P, toy_keys, ck.rotate(P, toy_keys, ct3, 2)) - np.roll(z, -2)).max() < 1e-4
 
 
+def test_hoisted_rotation_decrypts_like_rotation(toy, toy_keys):
+    """R2.7b: the hoisted form (ModUp of the unrotated c1, automorphism on the extended digits) is the same LEFT cyclic
+    shift with key-switch noise of the same size: the two decryptions differ by a small integer polynomial (the
+    ModDown of multiples of Q_j times the key), far below the scale, while the limbs themselves differ."""
+    P = toy
+    rng = np.random.default_rng(15)
+    z = rng.uniform(-1, 1, P.n)
+    for L in (P.nq, 3):  # top level, and a short last digit
+        ct = ck.encrypt(P, toy_keys, ck.encode(P, z, L), 90 + L)
+        for r in (1, 2, 5, 17):
+            h, p = ck.rotate_hoisted(P, toy_keys, ct, r), ck.rotate(P, toy_keys, ct, r)
+            d = ck.decrypt_decode(P, toy_keys, h)
+            assert np.abs(d - np.roll(z, -r)).max() < 1e-4
+            assert np.abs(d - np.roll(z, r)).max() > 0.1
+            assert not np.array_equal(h.c, p.c)
+            mh, mp = ck.decrypt_coeffs(P, toy_keys, h), ck.decrypt_coeffs(P, toy_keys, p)
+            diff = max(abs(int(a) - int(b)) for a, b in zip(mh, mp))
+            assert diff < 2 ** 10  # measured about 25; both carry rounding + e-terms of a few bits times sqrt(N); the scale is 2^25 and more
+    same = ck.rotate_hoisted(P, toy_keys, ct, 0)
+    assert np.array_equal(same.c, ct.c)
+
+
 def test_pmult_rescale_and_square(toy, toy_keys):
     P = toy
     rng = np.random.default_rng(6)
