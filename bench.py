@@ -245,6 +245,7 @@ def run_ours(args, rank, world):
     layers, x = builder(args.batch, seed)
     args.batch = int(layers[0]["conv"]["BS"])
     ctx = fenc.Context(device=dev, **wl.PARAMS[pkey])
+    ctx.set_hoisting(not args.no_hoist)  # inner rotations share one decomposition per input ciphertext (R2.7b)
     pipe = Pipeline(ctx, layers)
     pipe.setup(key_seed=seed)
     cts = pipe.encrypt_input(x, enc_seed0=10 * seed)
@@ -379,7 +380,7 @@ def run_ours(args, rank, world):
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(step_ms, 4),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
         "config": {"workload": args.workload, "description": desc, "batch": args.batch, "linear_layers_per_step": n_lin,
-                   "rotations_per_step": n_rot, "relinearisations_per_step": n_relin, "pmults_per_step": n_pm,
+                   "rotations_per_step": n_rot, "relinearisations_per_step": n_relin, "pmults_per_step": n_pm, "inner_rotations": "plain" if args.no_hoist else "hoisted (R2.7b)",
                    "multi_gpu": "replicas only" if world > 1 else "single", "l2": "inputs_exceed_l2: %d MiB resident" % (setup_bytes >> 20)},
         "rotations_per_s": round(world * (n_rot + n_relin) / (step_ms * 1e-3), 1),
         "images_per_s": round(world * args.batch / (step_ms * 1e-3), 2),
@@ -525,6 +526,7 @@ def main():
     ap.add_argument("--batch", type=int, default=128)
     ap.add_argument("--cpu-budget", type=float, default=20.0)
     ap.add_argument("--profile-range", action="store_true", help="cudaProfilerStart/Stop around the timed steps (for ncu)")
+    ap.add_argument("--no-hoist", action="store_true", help="inner rotations as plain rotations (one decomposition each)")
     ap.add_argument("--no-extras", action="store_true", help="skip the per-kernel pass, e2e and cpu_baseline (profiling runs)")
     args = ap.parse_args()
     rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))

@@ -234,6 +234,16 @@ fenc_status fenc_fc_weights_from_coeffs(fenc_ctx *ctx, const fenc_fc_desc *fc, c
 fenc_status fenc_fc(fenc_ctx *ctx, const fenc_keys *keys, const fenc_fc_desc *fc, const fenc_wts *wts, fenc_ct *const *in,
                     size_t n_in, int do_rescale, fenc_ct **out, size_t n_out_capacity, size_t *n_out);
 
+/* ------------------------------------------------------------------ hoisted inner rotations (R2.7b)
+ * The inner rotations of a linear layer (fenc_hconv, fenc_fc) rotate each input ciphertext by several amounts.  With
+ * hoisting on, the decomposition of c1 (inverse NTT, ModUp, forward NTT) runs once per input ciphertext and every rotation
+ * applies its automorphism to the extended digits: Rot = (sigma_g(c0) + ModDown(sum_j sigma_g(up_j) evk_j.b),
+ * ModDown(sum_j sigma_g(up_j) evk_j.a)).  Same keys, same decryption up to key-switch noise of the same size; the limbs
+ * differ from the plain form (sigma_g(ModUp_j(c1)) and ModUp_j(sigma_g(c1)) differ by multiples of Q_j), so a run is
+ * compared with the oracle's hoisted variant.  Outer rotations, fenc_rotate and fenc_compress are unaffected.
+ * Default: off.  Takes effect for the calls that follow. */
+fenc_status fenc_set_hoisting(fenc_ctx *ctx, int on);
+
 /* ------------------------------------------------------------------ AAC compress (R2.11) */
 /* out[t] = sum over the terms with term_out[i] == t of Rot(mask (*) in[term_src[i]], term_rot[i]).
  * mask may be NULL (maskless mode, no level consumed); with a mask and do_rescale != 0 this is the paper's

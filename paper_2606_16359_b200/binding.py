@@ -65,7 +65,7 @@ SYMBOLS = ["fenc_params_init", "fenc_ctx_free", "fenc_last_error", "fenc_get_pri
            "fenc_profile_enable", "fenc_profile_kernels", "fenc_profile_name", "fenc_profile_read", "fenc_fc_plan",
            "fenc_fc_wts_keys", "fenc_fc_weights", "fenc_fc_weights_from_coeffs", "fenc_fc", "fenc_measure_alu_peak",
            "fenc_cmult_relin", "fenc_mul_scalar", "fenc_add_const", "fenc_ct_import_async", "fenc_ct_export_async",
-           "fenc_export_wait"]
+           "fenc_export_wait", "fenc_set_hoisting"]
 
 _lib = None
 
@@ -101,6 +101,7 @@ def load_library(path=None):
         "fenc_ct_import_async": [vp, u64p, C.c_uint32, C.c_double, vpp],
         "fenc_ct_export_async": [vp, vp, u64p],
         "fenc_export_wait": [vp],
+        "fenc_set_hoisting": [vp, C.c_int],
         "fenc_ct_info": [vp, vp, u32p, dp, vpp],
         "fenc_rotate": [vp, vp, vpp, i32p, C.c_size_t, vpp],
         "fenc_rescale": [vp, vpp, C.c_size_t, vpp],
@@ -375,6 +376,10 @@ class Context:
         export_wait()."""
         assert out.dtype == np.uint64 and out.flags.c_contiguous and out.shape == (2, ct.L, self.N)
         self._ck(self.lib.fenc_ct_export_async(self.h, ct.h, _ptr(out, C.c_uint64)))
+
+    def set_hoisting(self, on=True):
+        """inner rotations of hconv / fc in the hoisted form (R2.7b); compare with the oracle's hoist=True runs"""
+        self._ck(self.lib.fenc_set_hoisting(self.h, int(bool(on))))
 
     def export_wait(self):
         self._ck(self.lib.fenc_export_wait(self.h))

@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstring>
 #include <functional>
+#include <map>
 #include <set>
 
 #include "fenc_ctx.h"
@@ -384,14 +385,20 @@ static fenc_status run_linear(fenc_ctx *ctx, const fenc_keys *K, const LinGraph 
   {
     std::vector<const u64 *> vin;
     std::vector<u64 *> vout;
-    std::vector<int> vs;
+    std::vector<int> vs, src_of;
+    std::vector<const u64 *> srcs;  // hoisted form: the distinct inputs that are rotated at all
+    std::map<const u64 *, int> src_index;
     for (size_t bg = 0; bg < BG; bg++)
       for (size_t r = 0; r < n_inner; r++) {
-        vin.push_back(in[bg * nin_bg + g.inner[r].first]->d);
+        const u64 *x = in[bg * nin_bg + g.inner[r].first]->d;
+        vin.push_back(x);
         vs.push_back(g.inner[r].second);
         vout.push_back(Rbuf + (bg * n_inner + r) * CT);
+        auto ins = src_index.insert({x, (int)srcs.size()});
+        if (ins.second) srcs.push_back(x);
+        src_of.push_back(ins.first->second);
       }
-    st = rotate_raw(ctx, K, L, vin, vs, vout);
+    st = ctx->hoist_inner ? rotate_hoisted_raw(ctx, K, L, srcs, src_of, vs, vout) : rotate_raw(ctx, K, L, vin, vs, vout);
     if (st != FENC_OK) return st;
   }
   // ---- 2. MAC over every (bg, output, diagonal)

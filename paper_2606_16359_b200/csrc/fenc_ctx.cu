@@ -270,6 +270,11 @@ extern "C" fenc_status fenc_get_primes(fenc_ctx *ctx, uint64_t *q, uint64_t *p, 
   if (beta_max) *beta_max = ctx->beta_max;
   return FENC_OK;
 }
+extern "C" fenc_status fenc_set_hoisting(fenc_ctx *ctx, int on) {
+  if (!ctx) return FENC_ERR_INVALID_ARG;
+  ctx->hoist_inner = on != 0;
+  return FENC_OK;
+}
 extern "C" fenc_status fenc_sync(fenc_ctx *ctx) {
   if (!ctx) return FENC_ERR_INVALID_ARG;
   CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
@@ -454,7 +459,7 @@ bool ks_can_merge_rescale(const fenc_ctx *ctx, int L) {
   return L >= 2 && convert_cols_fits(ctx->logN, ctx->np + 1, true);
 }
 
-fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items, bool rescale_after) {
+fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items, bool rescale_after, const HoistUp *hoist) {
   if (items.empty()) return FENC_OK;
   if (rescale_after && !ks_can_merge_rescale(ctx, L)) return fail(ctx, FENC_ERR_INVALID_ARG, "merged rescale unavailable here");
   LevelPlan *P = get_plan(ctx, L);
@@ -484,6 +489,11 @@ fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items, bool r
     // a2 + a1 + a3: inverse row pass of sigma_g(d); then ONE fused column kernel per digit group: inverse column
     // stages + ModUp scaling of the digit's limbs in shared memory, base conversion and forward column stages per target
     const bool fused_up = convert_cols_fits(ctx->logN, P->n_src_up, false);
+    if (hoist) {
+      // R2.7b: the decomposition was done once per source (rotate_hoisted_raw); a1 + a4 reduce to a gathered inner product
+      CUDA_OK(ctx, k_hoisted_keymac(k, d_items, L, E, P->beta, P->d_tmp_index, hoist->up, hoist->sstride, acc, (size_t)2 * E * N, nb,
+                                    n_keys, hoist->n_sources, P->n_up));
+    } else {
     if (fused_up) {
       CUDA_OK(ctx, k_intt_rows_only(k, d_items, nullptr, 0, true, y, (size_t)L * N, P->d_rows_in, L, nb));
       CUDA_OK(ctx, k_convert_cols(k, y, (size_t)L * N, P->d_groups_up, P->beta, P->n_src_up, P->d_scale_in, P->d_bc_up, P->d_rows_up,
@@ -494,6 +504,7 @@ fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items, bool r
     }
     // a1 (pass 2) + a4: evk inner product
     CUDA_OK(ctx, k_ntt_rows_keymac(k, d_items, L, E, P->beta, P->d_tmp_index, tmp, (size_t)P->n_up * N, acc, (size_t)2 * E * N, nb, P->n_up, n_keys));
+    }
     if (rescale_after) {
       // a5 + a8 merged: the limb the rescale drops is inverse-transformed with the special limbs; one column kernel and
       // one divide epilogue produce the rescaled ciphertext directly
@@ -553,6 +564,54 @@ fenc_status rescale_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items) {
     CUDA_OK(ctx, k_ntt_rows_divide(k, d_items, tmp2, (size_t)2 * L1 * N, nullptr, 0, true, P->d_mul_qlinv, P->d_rows_rs_div, 2 * L1, nb));
   }
   return FENC_OK;
+}
+
+// Hoisted rotations (R2.7b): per source one inverse transform of c1 (no gather), ModUp with the forward column stages,
+// and the forward row stages -> extended digits in NTT form; then per rotation the gathered inner product and ModDown.
+fenc_status rotate_hoisted_raw(fenc_ctx *ctx, const fenc_keys *keys, int L, const std::vector<const u64 *> &src,
+                               const std::vector<int> &src_of, const std::vector<int> &steps, const std::vector<u64 *> &out) {
+  if (steps.empty()) return FENC_OK;
+  Scope sc(ctx);
+  LevelPlan *P = get_plan(ctx, L);
+  if (!P) return fail(ctx, FENC_ERR_OOM, "level plan");
+  const size_t N = ctx->N, LN = (size_t)L * N;
+  const int ns = (int)src.size();
+  u64 *y = sc.alloc<u64>((size_t)ns * LN), *up = sc.alloc<u64>((size_t)ns * P->n_up * N);
+  if (!y || !up) return fail(ctx, FENC_ERR_OOM, "hoisted decomposition (%d sources)", ns);
+  {
+    DescStage st(ctx);
+    std::vector<BatchItem> sitems(ns);
+    for (int i = 0; i < ns; i++) sitems[i] = BatchItem{}, sitems[i].ks_in = src[i] + LN, sitems[i].g = 1;
+    st.add(sitems);
+    const BatchItem *d_src = (const BatchItem *)st.commit();
+    if (!d_src) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
+    const KCtx &k = ctx->k;
+    if (convert_cols_fits(ctx->logN, P->n_src_up, false)) {
+      CUDA_OK(ctx, k_intt_rows_only(k, d_src, nullptr, 0, true, y, LN, P->d_rows_in, L, ns));
+      CUDA_OK(ctx, k_convert_cols(k, y, LN, P->d_groups_up, P->beta, P->n_src_up, P->d_scale_in, P->d_bc_up, P->d_rows_up, P->n_up, up,
+                                  (size_t)P->n_up * N, ns, ctx->lazy_q, nullptr, P->d_bc_up_f64));
+    } else {
+      CUDA_OK(ctx, k_intt(k, d_src, nullptr, 0, true, y, LN, P->d_rows_in, L, P->d_scale_in, ns));
+      CUDA_OK(ctx, k_ntt_cols_bconv(k, y, LN, P->d_bc_up, up, (size_t)P->n_up * N, P->d_rows_up, P->n_up, ns, L, ctx->lazy_q));
+    }
+    CUDA_OK(ctx, k_ntt_rows_only(k, up, (size_t)P->n_up * N, P->d_rows_up, P->n_up, ns));
+  }
+  std::vector<BatchItem> items;
+  for (size_t i = 0; i < steps.size(); i++) {
+    const int r = ((steps[i] % ctx->n) + ctx->n) % ctx->n;
+    const u64 *in = src[src_of[i]];
+    if (r == 0) {
+      CUDA_OK(ctx, cudaMemcpyAsync(out[i], in, 2 * LN * 8, cudaMemcpyDeviceToDevice, ctx->stream));
+      continue;
+    }
+    auto it = keys->evk.find(r);
+    if (it == keys->evk.end()) return fail(ctx, FENC_ERR_NO_KEY, "no rotation key for step %d", r);
+    BatchItem b{};
+    b.ks_in = in + LN, b.out = out[i], b.evk = it->second, b.add0 = in, b.g = galois_elt(ctx, r), b.pad = (u32)src_of[i];
+    items.push_back(b);
+  }
+  HoistUp h{up, (size_t)P->n_up * N, ns};
+  return ks_batch(ctx, L, items, false, &h);
 }
 
 // Rot(in[i], steps[i]) -> out[i]; all at level L (Eq. 1; R2.7: automorphism first)

@@ -98,6 +98,7 @@ struct fenc_ctx {
   std::vector<StageSlot> stage;
   size_t stage_next = 0;
   cudaEvent_t export_ev = nullptr;     // behind the last fenc_ct_export_async (fenc_export_wait)
+  bool hoist_inner = false;            // fenc_set_hoisting: inner rotations of linear layers in the hoisted form (R2.7b)
 };
 
 struct fenc_keys {
@@ -202,7 +203,16 @@ struct Scope {
 };
 // batched key switch over items (all at level L): out = (ModDown(acc_0) + add0, ModDown(acc_1) + add1)
 // rescale_after: the rescale is merged into the ModDown (needs both addends, g = 1, N >= 2^12): out is [2][L-1][N]
-fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items, bool rescale_after = false);
+// hoisted rotations (R2.7b): the extended digits of the sources' c1 in NTT form, [n_sources][n_up][N]; items[i].pad = source
+struct HoistUp {
+  const u64 *up;
+  size_t sstride;
+  int n_sources;
+};
+fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items, bool rescale_after = false, const HoistUp *hoist = nullptr);
+// Rot(src[src_of[i]], steps[i]) -> out[i] with ONE decomposition (inverse NTT, ModUp, forward NTT) per source
+fenc_status rotate_hoisted_raw(fenc_ctx *ctx, const fenc_keys *keys, int L, const std::vector<const u64 *> &src,
+                               const std::vector<int> &src_of, const std::vector<int> &steps, const std::vector<u64 *> &out);
 bool ks_can_merge_rescale(const fenc_ctx *ctx, int L);
 // batched rescale: items[i].sub_in = input ct [2][L][N], items[i].out = [2][L-1][N]
 fenc_status rescale_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items);

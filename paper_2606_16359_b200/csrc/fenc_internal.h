@@ -59,7 +59,7 @@ struct BatchItem {
   const u64 *add0;   // epilogue addend for component 0 ([L][N], read through the Galois gather) or NULL
   const u64 *add1;   // epilogue addend for component 1 or NULL
   u32 g;             // Galois element (1 = identity)
-  u32 pad;
+  u32 pad;           // hoisted rotations: index of the source ciphertext whose extended digits this item reads
 };
 
 // geometry of the 2-pass NTT for one ring degree
@@ -119,6 +119,12 @@ int k_intt_rows_only(const KCtx &k, const BatchItem *items, const u64 *src, size
 // fused column kernel (needs N >= 2^12): for every group, the inverse column stages + scaling of its source rows (kept
 // in shared memory), then for each target the base conversion and the forward column stages -> tmp rows (lazy).
 // Returns -2 when the group does not fit shared memory (the caller falls back to k_intt + k_ntt_cols_bconv).
+// forward pass 2 alone, in place on rows[r].dst_row of buf (+ b*bstride): canonical results
+int k_ntt_rows_only(const KCtx &k, u64 *buf, size_t bstride, const RowDesc *rows, int n_rows, int n_batch);
+// hoisted rotations (R2.7b): acc[b] = sum_j gather_{g_b}(x_j) (*) evk_b,j over the E target rows, x_j[t] = row
+// tmp_index[j*E+t] of up + items[b].pad*up_sstride, or items[b].ks_in[t] for the digit's own limbs; Montgomery-reduced
+int k_hoisted_keymac(const KCtx &k, const BatchItem *items, int L, int E, int beta, const int *tmp_index, const u64 *up,
+                     size_t up_sstride, u64 *acc, size_t acc_bstride, int n_batch, int n_distinct_keys, int n_sources, int n_up);
 // whether the fused column kernel can hold a conversion group of n_src limbs (its tiles + the work tiles) in shared memory
 bool convert_cols_fits(int logN, int n_src, bool merged);
 int k_convert_cols(const KCtx &k, u64 *y, size_t y_bstride, const ConvGroup *groups, int n_groups, int n_src_max,

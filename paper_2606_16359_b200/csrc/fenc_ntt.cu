@@ -418,6 +418,18 @@ int k_ntt(const KCtx &k, const u64 *src, size_t src_bstride, u64 *dst, size_t ds
   return 0;
 }
 
+// forward pass 2 alone, in place on rows[r].dst_row of buf (rows that a column kernel left in their lazy form): canonical
+int k_ntt_rows_only(const KCtx &k, u64 *buf, size_t bstride, const RowDesc *rows, int n_rows, int n_batch) {
+  if (n_rows == 0 || n_batch == 0) return 0;
+  const NttGeom &g = k.geom;
+  NttRowP r{buf, bstride, buf, bstride, rows, k.d_mods, k.d_tw_fwd, g, 1};
+  dim3 grid2(k.N >> g.lt_row, n_rows, n_batch);
+  PROF(k, K_NTT_ROW, 16.0 * k.N * n_rows * n_batch, HALF_N(k) * g.brow * n_rows * n_batch);
+  ROW_GEO(g, (ntt_rowpass_kernel<GEO><<<grid2, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(r)));
+  LAUNCH_CHECK(k);
+  return 0;
+}
+
 int k_ntt_cols_bconv(const KCtx &k, const u64 *y, size_t y_bstride, const u64 *bc, u64 *tmp, size_t tmp_bstride,
                      const RowDesc *rows, int n_rows, int n_batch, int n_src_rows, int max_terms) {
   if (n_rows == 0 || n_batch == 0) return 0;
@@ -541,6 +553,65 @@ int k_ntt_rows_keymac(const KCtx &k, const BatchItem *items, int L, int E, int b
   else if (ept <= 1) ntt_rows_keymac_kernel<1, 0><<<grid, nth, 2 * (sizeof(u64) << g.lt_row), (cudaStream_t)k.stream>>>(p);
   else if (ept <= 4) ntt_rows_keymac_kernel<4, 0><<<grid, nth, 2 * (sizeof(u64) << g.lt_row), (cudaStream_t)k.stream>>>(p);
   else ntt_rows_keymac_kernel<8, 0><<<grid, nth, 2 * (sizeof(u64) << g.lt_row), (cudaStream_t)k.stream>>>(p);
+  LAUNCH_CHECK(k);
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------------ evk inner product of a hoisted rotation (R2.7b)
+// The extended digits of the source ciphertext's c1 are already in NTT form (up: [source][n_up][N], canonical; the
+// digit's own limbs are the ciphertext's): a rotation is the Galois gather of those rows times its key, accumulated over
+// the digits -- no transform.  Rotations of one source re-read its rows from L2; items sharing a key are neighbours.
+struct HoistMacP {
+  const BatchItem *items; const int *tmp_index; const u64 *up; size_t up_sstride; u64 *acc; size_t acc_bstride;
+  const ModConst *mods; int logN, L, E, beta, A, nq, n_batch;
+};
+template <int EPT>
+__global__ void __launch_bounds__(256) hoisted_keymac_kernel(HoistMacP p) {
+  const int tid = threadIdx.x, nb = p.n_batch, b = blockIdx.x % nb, chunk = blockIdx.x / nb, t = blockIdx.y;
+  const int N = 1 << p.logN;
+  const int mod = t < p.L ? t : p.nq + (t - p.L);
+  const ModConst mc = p.mods[mod];
+  const BatchItem it = p.items[b];
+  u32 pos[EPT], src[EPT];
+  u64 a0l[EPT], a0h[EPT], a1l[EPT], a1h[EPT];
+#pragma unroll
+  for (int i = 0; i < EPT; i++) {
+    pos[i] = ((u32)chunk * EPT + i) * 256u + tid;
+    src[i] = galois_src(pos[i] & (N - 1), it.g, p.logN);
+    a0l[i] = a0h[i] = a1l[i] = a1h[i] = 0;
+  }
+  for (int j = 0; j < p.beta; j++) {
+    const int ti = p.tmp_index[j * p.E + t];
+    const u64 *x = ti >= 0 ? p.up + (size_t)it.pad * p.up_sstride + (size_t)ti * N : it.ks_in + (size_t)t * N;
+    const u64 *kb = it.evk + ((size_t)(j * 2 + 0) * p.A + mod) * N;
+    const u64 *ka = it.evk + ((size_t)(j * 2 + 1) * p.A + mod) * N;
+    u64 xv[EPT], vb[EPT], va[EPT];
+#pragma unroll
+    for (int i = 0; i < EPT; i++)
+      if (pos[i] < (u32)N) xv[i] = __ldg(x + src[i]), vb[i] = __ldg(kb + pos[i]), va[i] = __ldg(ka + pos[i]);
+#pragma unroll
+    for (int i = 0; i < EPT; i++)
+      if (pos[i] < (u32)N) mac128(a0l[i], a0h[i], xv[i], vb[i]), mac128(a1l[i], a1h[i], xv[i], va[i]);
+  }
+  u64 *o0 = p.acc + (size_t)b * p.acc_bstride + (size_t)t * N;
+  u64 *o1 = o0 + (size_t)p.E * N;
+#pragma unroll
+  for (int i = 0; i < EPT; i++)
+    if (pos[i] < (u32)N) {
+      o0[pos[i]] = mont_redc(a0l[i], a0h[i], mc.q, mc.qinv_neg);
+      o1[pos[i]] = mont_redc(a1l[i], a1h[i], mc.q, mc.qinv_neg);
+    }
+}
+int k_hoisted_keymac(const KCtx &k, const BatchItem *items, int L, int E, int beta, const int *tmp_index, const u64 *up,
+                     size_t up_sstride, u64 *acc, size_t acc_bstride, int n_batch, int n_distinct_keys, int n_sources, int n_up) {
+  if (n_batch == 0) return 0;
+  constexpr int EPT = 4;
+  HoistMacP p{items, tmp_index, up, up_sstride, acc, acc_bstride, k.d_mods, k.geom.logN, L, E, beta, k.nq + k.np, k.nq, n_batch};
+  const int chunks = (k.N + 256 * EPT - 1) / (256 * EPT);
+  dim3 grid(chunks * n_batch, E, 1);
+  // algorithmic bytes: accumulators written once, each key and each source's extended digits read once
+  PROF(k, K_KEYMAC, 8.0 * k.N * (2.0 * E * n_batch + 2.0 * beta * E * n_distinct_keys + ((double)n_up + L) * n_sources), 0);
+  hoisted_keymac_kernel<EPT><<<grid, 256, 0, (cudaStream_t)k.stream>>>(p);
   LAUNCH_CHECK(k);
   return 0;
 }

@@ -129,7 +129,7 @@ def test_library_encoder_close_to_oracle(mods):
     ctx.close()
 
 
-def run_hconv(mods, P, ctx, conv_kw, S, seed, do_rescale=True, kaiming=False):
+def run_hconv(mods, P, ctx, conv_kw, S, seed, do_rescale=True, kaiming=False, hoist=False):
     """GPU fenc_hconv vs oracle hconv for every batch group; returns (max decoded error, layout)."""
     ck, fr, fenc = mods
     x, w = wl.conv_inputs(seed, conv_kw, kaiming=kaiming)
@@ -157,12 +157,13 @@ def run_hconv(mods, P, ctx, conv_kw, S, seed, do_rescale=True, kaiming=False):
                     pt = ck.encode(P, lin.gather(x, u, v, g, bg), L)
                     o_in[(bg, u, v, g)] = ck.encrypt(P, ok, pt, 1000 + len(g_in))
                     g_in.append(ctx.encrypt(gk, ctx.pt_from_coeffs(pt.coeffs, L, float(pt.scale)), 1000 + len(g_in)))
+    ctx.set_hoisting(hoist)
     g_out = ctx.hconv(gk, conv, lay, gW, g_in, do_rescale=do_rescale)
     So, lout = graph.S_out, graph.lout
     Y = np.zeros((od.BS, od.C_out, od.H_out, od.W_out))
     for bg in range(lin.BG):
         ins = {(u, v, g): o_in[(bg, u, v, g)] for g in range(lin.G) for u in range(S) for v in range(S)}
-        o_out = fr.hconv(ck, P, ok, graph, ins, oW, do_rescale=do_rescale)
+        o_out = fr.hconv(ck, P, ok, graph, ins, oW, do_rescale=do_rescale, hoist=hoist)
         for go in range(lout.G):
             for uo in range(So):
                 for vo in range(So):
@@ -185,6 +186,21 @@ def run_hconv(mods, P, ctx, conv_kw, S, seed, do_rescale=True, kaiming=False):
 def test_hconv_bit_exact_small(mods, conv_kw, S):
     P, ctx = make(mods, "mid10")
     err, _ = run_hconv(mods, P, ctx, conv_kw, S, seed=3)
+    assert err < 1e-3
+    ctx.close()
+
+
+@pytest.mark.parametrize("name", ["mid10", "mid12"])
+@pytest.mark.parametrize("conv_kw,S", [
+    (dict(BS=2, C_in=4, H=8, W=8, C_out=4, K=3, stride=1, pad=1), 2),      # 3 inner rotations per input ciphertext
+    (dict(BS=1, C_in=3, H=7, W=6, C_out=5, K=3, stride=1, pad=1), 1),      # 8 inner rotations of one ciphertext, outer ones plain
+    (dict(BS=40, C_in=2, H=8, W=8, C_out=3, K=3, stride=1, pad=1), 2),     # two batch groups: sources of both in one batch
+])
+def test_hconv_hoisted_inner_rotations_bit_exact(mods, name, conv_kw, S):
+    """R2.7b: one decomposition per input ciphertext, automorphism on the extended digits; compared limb by limb with
+    the oracle's hoisted variant (ragged digits: 5 limbs, dlen 2), decoded result against the plain convolution."""
+    P, ctx = make(mods, name)
+    err, _ = run_hconv(mods, P, ctx, conv_kw, S, seed=5, hoist=True)
     assert err < 1e-3
     ctx.close()
 
@@ -345,11 +361,16 @@ def test_import_async_matches_import(mods):
     dict(BS=40, n_in=3 * 3 * 3, n_out=20, in_C=3, in_H=3, in_W=3, in_M=4, bsgs=0),
     dict(BS=64, n_in=20, n_out=11, in_M=4, bsgs=2),
     dict(BS=16, n_in=70, n_out=40, in_M=2, bsgs=0),                          # P = 32: 3 input cts, 2 output cts
+    dict(BS=16, n_in=70, n_out=40, in_M=2, bsgs=0, hoist=True),              # baby steps in the hoisted form (R2.7b)
+    dict(BS=40, n_in=3 * 3 * 3, n_out=20, in_C=3, in_H=3, in_W=3, in_M=4, bsgs=4, hoist=True),
 ])
 def test_fc_bit_exact(mods, kw):
     ck, fr, fenc = mods
     from oracle import network as nw
+    kw = dict(kw)
+    hoist = kw.pop("hoist", False)
     P, ctx = make(mods, "mid10")
+    ctx.set_hoisting(hoist)
     g = nw.FcGraph(P.n, **kw)
     fcd = ctx.fc_desc(**kw)
     info = ctx.fc_plan(fcd)
@@ -374,7 +395,7 @@ def test_fc_bit_exact(mods, kw):
     g_out = ctx.fc(gk, fcd, gW, g_in)
     Y = np.zeros((kw["BS"], kw["n_out"]))
     for bg in range(g.BG):
-        ref = nw.fc(ck, P, ok, g, o_in[bg * g.n_in_ct:(bg + 1) * g.n_in_ct], oW)
+        ref = nw.fc(ck, P, ok, g, o_in[bg * g.n_in_ct:(bg + 1) * g.n_in_ct], oW, hoist=hoist)
         for co, r in enumerate(ref):
             got = g_out[bg * g.n_out_ct + co]
             assert np.array_equal(ctx.ct_export(got), r.c), (bg, co)
@@ -386,8 +407,8 @@ def test_fc_bit_exact(mods, kw):
     ctx.close()
 
 
-@pytest.mark.parametrize("bsgs", [1, 0])
-def test_pipeline_toy_network_bit_exact(mods, bsgs):
+@pytest.mark.parametrize("bsgs,hoist", [(1, False), (0, False), (0, True)])
+def test_pipeline_toy_network_bit_exact(mods, bsgs, hoist):
     """conv - square - pool - fc - fc through Pipeline (one batched C-ABI call per layer) vs the oracle's network."""
     ck, fr, fenc = mods
     from oracle import network as nw
@@ -396,6 +417,7 @@ def test_pipeline_toy_network_bit_exact(mods, bsgs):
     p = dict(log2N=9, n_q=5, q_bits=40, n_p=2, p_bits=60, dnum=3, log2_scale=40)
     P = ck.Params(*wl.oracle_params_args(p))
     ctx = fenc.Context(**p)
+    ctx.set_hoisting(hoist)
     layers, x = toy_network(bsgs=bsgs)
     pipe = Pipeline(ctx, layers)
     steps, relin = nw.network_rot_steps(layers, P.n)
@@ -422,7 +444,7 @@ def test_pipeline_toy_network_bit_exact(mods, bsgs):
         pt = ck.encode(P, lin.gather(x, u, v, g, bg), P.nq)
         o_in.append(ck.encrypt(P, ok, pt, 100 + i))
         g_in.append(ctx.encrypt(gk, ctx.pt_from_coeffs(pt.coeffs, P.nq, float(pt.scale)), 100 + i))
-    o_out, o_trace = nw.run_network(ck, P, ok, layers, o_in, P.nq)
+    o_out, o_trace = nw.run_network(ck, P, ok, layers, o_in, P.nq, hoist=hoist)
     g_trace = []
     g_out = pipe.forward(g_in, trace=g_trace)
     for li, (ol, gl) in enumerate(zip(o_trace, g_trace)):
@@ -601,6 +623,37 @@ def test_config3_conv_plus_activation_full_size_decoded(mods):
     ctx.decrypt_decode(keys, out[0], p0["conv"], p0["lay"], 1, 0, 0, 0, 0, Y)
     c = fr.direct_conv(od, x, w)
     assert np.abs(Y - (0.5 + 0.197 * c - 0.004 * c ** 3)).max() < 1e-3
+    ctx.close()
+
+
+def test_lenet5_full_size_bsgs_and_hoisting_decoded(mods):
+    """BASELINE config 2 at the size and in the configuration bench.py times (batch 128, N=2^14, BSGS fully connected
+    layers, inner rotations plain and hoisted): the decoded logits of all 128 samples against the fp64 network."""
+    ck, fr, fenc = mods
+    import bench
+    from oracle import network as nw
+    from paper_2606_16359_b200.pipeline import Pipeline
+    from test_oracle_network import plain_network
+    ctx = fenc.Context(**wl.PARAMS["cfg2"])
+    layers, x = bench.lenet_layers(128, 2000)
+    want = plain_network(layers, x)
+    assert np.abs(want).max() < 0.5  # one 40-bit limb at scale 2^40 is left (A23)
+    pipe = Pipeline(ctx, layers)
+    keys = pipe.setup(key_seed=2000)
+    cts = pipe.encrypt_input(x, 20000)
+    fg = nw.FcGraph(ctx.n, **layers[-1]["fc"])
+    got = {}
+    for hoist in (False, True):
+        ctx.set_hoisting(hoist)
+        out = pipe.forward(cts)
+        assert len(out) == 1 and out[0].L == 1
+        Y = np.zeros((128, 10))
+        fg.scatter_out(Y, ctx.decrypt_slots(keys, out[0]).real, 0, 0)
+        assert np.abs(Y - want).max() < 1e-3, hoist
+        got[hoist] = Y
+    assert np.abs(got[True] - got[False]).max() < 1e-4 and not np.array_equal(got[True], got[False])
+    n_lin, n_rot, n_relin, n_pm = pipe.counts()
+    assert (n_lin, n_rot, n_relin) == (5, 367, 160)  # 48 + 192 conv rotations, 78 + 28 + 21 BSGS rotations (315 plain)
     ctx.close()
 
 
