@@ -565,53 +565,58 @@ struct HoistMacP {
   const BatchItem *items; const int *tmp_index; const u64 *up; size_t up_sstride; u64 *acc; size_t acc_bstride;
   const ModConst *mods; int logN, L, E, beta, A, nq, n_batch;
 };
-template <int EPT>
+// Each thread owns the adjacent positions 2i, 2i+1: their Galois sources are adjacent too (the lowest position bit is
+// the highest bit of the exponent index, which an odd multiplier maps to itself), so x, b and a all arrive as 16-byte
+// loads; the loads of digit j+1 are issued before the products of digit j.
+struct HoistOperands { ulonglong2 x, b, a; };
 __global__ void __launch_bounds__(256) hoisted_keymac_kernel(HoistMacP p) {
   const int tid = threadIdx.x, nb = p.n_batch, b = blockIdx.x % nb, chunk = blockIdx.x / nb, t = blockIdx.y;
   const int N = 1 << p.logN;
   const int mod = t < p.L ? t : p.nq + (t - p.L);
   const ModConst mc = p.mods[mod];
   const BatchItem it = p.items[b];
-  u32 pos[EPT], src[EPT];
-  u64 a0l[EPT], a0h[EPT], a1l[EPT], a1h[EPT];
-#pragma unroll
-  for (int i = 0; i < EPT; i++) {
-    pos[i] = ((u32)chunk * EPT + i) * 256u + tid;
-    src[i] = galois_src(pos[i] & (N - 1), it.g, p.logN);
-    a0l[i] = a0h[i] = a1l[i] = a1h[i] = 0;
-  }
-  for (int j = 0; j < p.beta; j++) {
+  const u32 pos = 2u * ((u32)chunk * 256u + tid);
+  if (pos >= (u32)N) return;
+  const u32 src = galois_src(pos, it.g, p.logN);  // source of pos; pos + 1 reads src ^ 1
+  const bool swap = src & 1u;
+  auto fetch = [&](int j) {
     const int ti = p.tmp_index[j * p.E + t];
     const u64 *x = ti >= 0 ? p.up + (size_t)it.pad * p.up_sstride + (size_t)ti * N : it.ks_in + (size_t)t * N;
     const u64 *kb = it.evk + ((size_t)(j * 2 + 0) * p.A + mod) * N;
     const u64 *ka = it.evk + ((size_t)(j * 2 + 1) * p.A + mod) * N;
-    u64 xv[EPT], vb[EPT], va[EPT];
-#pragma unroll
-    for (int i = 0; i < EPT; i++)
-      if (pos[i] < (u32)N) xv[i] = __ldg(x + src[i]), vb[i] = __ldg(kb + pos[i]), va[i] = __ldg(ka + pos[i]);
-#pragma unroll
-    for (int i = 0; i < EPT; i++)
-      if (pos[i] < (u32)N) mac128(a0l[i], a0h[i], xv[i], vb[i]), mac128(a1l[i], a1h[i], xv[i], va[i]);
+    HoistOperands o;
+    o.x = __ldg(reinterpret_cast<const ulonglong2 *>(x + (src & ~1u)));
+    o.b = __ldg(reinterpret_cast<const ulonglong2 *>(kb + pos));
+    o.a = __ldg(reinterpret_cast<const ulonglong2 *>(ka + pos));
+    return o;
+  };
+  u64 a0l[2] = {0, 0}, a0h[2] = {0, 0}, a1l[2] = {0, 0}, a1h[2] = {0, 0};
+  HoistOperands cur = fetch(0);
+  for (int j = 0; j < p.beta; j++) {
+    HoistOperands nxt = cur;
+    if (j + 1 < p.beta) nxt = fetch(j + 1);
+    const u64 x0 = swap ? cur.x.y : cur.x.x, x1 = swap ? cur.x.x : cur.x.y;
+    mac128(a0l[0], a0h[0], x0, cur.b.x), mac128(a1l[0], a1h[0], x0, cur.a.x);
+    mac128(a0l[1], a0h[1], x1, cur.b.y), mac128(a1l[1], a1h[1], x1, cur.a.y);
+    cur = nxt;
   }
   u64 *o0 = p.acc + (size_t)b * p.acc_bstride + (size_t)t * N;
   u64 *o1 = o0 + (size_t)p.E * N;
-#pragma unroll
-  for (int i = 0; i < EPT; i++)
-    if (pos[i] < (u32)N) {
-      o0[pos[i]] = mont_redc(a0l[i], a0h[i], mc.q, mc.qinv_neg);
-      o1[pos[i]] = mont_redc(a1l[i], a1h[i], mc.q, mc.qinv_neg);
-    }
+  *reinterpret_cast<ulonglong2 *>(o0 + pos) =
+      make_ulonglong2(mont_redc(a0l[0], a0h[0], mc.q, mc.qinv_neg), mont_redc(a0l[1], a0h[1], mc.q, mc.qinv_neg));
+  *reinterpret_cast<ulonglong2 *>(o1 + pos) =
+      make_ulonglong2(mont_redc(a1l[0], a1h[0], mc.q, mc.qinv_neg), mont_redc(a1l[1], a1h[1], mc.q, mc.qinv_neg));
 }
 int k_hoisted_keymac(const KCtx &k, const BatchItem *items, int L, int E, int beta, const int *tmp_index, const u64 *up,
                      size_t up_sstride, u64 *acc, size_t acc_bstride, int n_batch, int n_distinct_keys, int n_sources, int n_up) {
   if (n_batch == 0) return 0;
-  constexpr int EPT = 4;
   HoistMacP p{items, tmp_index, up, up_sstride, acc, acc_bstride, k.d_mods, k.geom.logN, L, E, beta, k.nq + k.np, k.nq, n_batch};
-  const int chunks = (k.N + 256 * EPT - 1) / (256 * EPT);
+  if (k.N < 2) return -2;
+  const int chunks = (k.N / 2 + 255) / 256;
   dim3 grid(chunks * n_batch, E, 1);
   // algorithmic bytes: accumulators written once, each key and each source's extended digits read once
   PROF(k, K_KEYMAC, 8.0 * k.N * (2.0 * E * n_batch + 2.0 * beta * E * n_distinct_keys + ((double)n_up + L) * n_sources), 0);
-  hoisted_keymac_kernel<EPT><<<grid, 256, 0, (cudaStream_t)k.stream>>>(p);
+  hoisted_keymac_kernel<<<grid, 256, 0, (cudaStream_t)k.stream>>>(p);
   LAUNCH_CHECK(k);
   return 0;
 }
