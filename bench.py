@@ -126,6 +126,7 @@ WORKLOADS = {
     "cfg3_conv_32_64_s2": ("cfg3", lambda bs, seed: conv_layers("resnet_32_64_s2", seed, True),
                            "BASELINE config 3: ResNet-20 3x3 32->64 stride 2, N=2^16, batch 1"),
     "cfg5_rotsweep": (None, None, "BASELINE config 5: rotation / key-switch sweep"),
+    "cfg5_rotsweep_hoisted": (None, None, "BASELINE config 5 with hoisted rotations (8 amounts per decomposition)"),
     "cfg3_compress": (None, None, "AAC compress micro-benchmark at config 3's parameters"),
 }
 DEFAULT_WORKLOAD = "cfg2_lenet5"
@@ -138,9 +139,11 @@ def conv_layers(name, seed, kaiming=False):
     return [{"op": "conv", "conv": dict(kw), "S": 0, "w": w}], x
 
 
-def run_rotsweep(args):
+def run_rotsweep(args, hoisted=False):
     """BASELINE config 5: rotation / key-switch sweep at N=2^16 (reading A2: k = dlen = ceil(L/dnum)).  64 ciphertexts with
-    uniform-random limbs, 32 distinct seeded rotation amounts; every amount is one batched fenc_rotate over the 64."""
+    uniform-random limbs, 32 distinct seeded rotation amounts; every amount is one batched fenc_rotate over the 64.
+    hoisted: the same 2048 rotations as 4 calls of fenc_rotate_hoisted (64 ciphertexts x 8 amounts each: one
+    decomposition per ciphertext and call, R2.7b -- the shape of a 3x3 convolution's 8 inner rotations)."""
     import torch
     import paper_2606_16359_b200 as fenc
     peaks, peak_src = measured_peaks()
@@ -154,21 +157,31 @@ def run_rotsweep(args):
             steps = wl.rotation_steps(5000 + L * 10 + dnum, n_steps, ctx.n)
             keys = ctx.keygen(5, steps)
             cts = [ctx.ct_import(wl.random_ct_limbs(100 * L + i, ctx.q, L, N)) for i in range(n_ct)]
-            for r in steps[:2]:
-                ctx.rotate(keys, cts, [r] * n_ct)
+            if hoisted:
+                ctx.rotate_hoisted(keys, cts, steps[:8])
+            else:
+                for r in steps[:2]:
+                    ctx.rotate(keys, cts, [r] * n_ct)
             torch.cuda.synchronize()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             ctx.launch_count(reset=True)
             e0.record()
-            for r in steps:
-                out = ctx.rotate(keys, cts, [r] * n_ct)
-                del out
+            if hoisted:
+                for at in range(0, n_steps, 8):
+                    out = ctx.rotate_hoisted(keys, cts, steps[at:at + 8])
+                    del out
+            else:
+                for r in steps:
+                    out = ctx.rotate(keys, cts, [r] * n_ct)
+                    del out
             e1.record()
             torch.cuda.synchronize()
             ms = e0.elapsed_time(e1)
             rots = n_ct * n_steps
             # algorithmic bytes per rotation: ciphertext in + out, key once per batch of 64
             b_alg = 2 * (2 * L * N * 8) + 2 * beta * (L + k) * N * 8 / n_ct
+            if hoisted:  # input read once per 8 rotations, output once per rotation, key once per 64 ciphertexts
+                b_alg = 2 * L * N * 8 * (1 + 1 / 8) + 2 * beta * (L + k) * N * 8 / n_ct
             gbs = rots * b_alg / (ms * 1e-3) / 1e9
             points.append({"L": L, "dnum": dnum, "dlen": dlen, "k": k, "beta": beta,
                            "ntt_per_rot": beta * (L + k) + 2 * k + 2 * L, "rot_per_s": round(rots / (ms * 1e-3), 1),
@@ -181,8 +194,9 @@ def run_rotsweep(args):
     return {"metric": METRIC, "value": ref["rot_per_s"], "unit": "key-switched rotations/s", "n_gpus": 1, "steps": n_steps,
             "warmup": 2, "ms_per_step": round(1e3 * n_ct / ref["rot_per_s"], 4), "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "u64", "data": "synthetic",
-            "config": {"workload": "cfg5_rotsweep", "description": "BASELINE config 5: N=2^16, 64 cts x 32 amounts per point; "
-                       "value quoted at L=24, dnum=3", "peak_source": peak_src, "hbm_peak_GBps": peaks["hbm_gbs"]},
+            "config": {"workload": "cfg5_rotsweep_hoisted" if hoisted else "cfg5_rotsweep",
+                       "description": "BASELINE config 5: N=2^16, 64 cts x 32 amounts per point; value quoted at L=24, dnum=3"
+                       + ("; hoisted form (R2.7b), 8 amounts per decomposition" if hoisted else ""), "peak_source": peak_src, "hbm_peak_GBps": peaks["hbm_gbs"]},
             "points": points}
 
 
@@ -539,8 +553,8 @@ def main():
         import torch
         torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", 0)))
         torch.distributed.init_process_group("nccl")
-    if args.workload == "cfg5_rotsweep":
-        line = run_rotsweep(args)
+    if args.workload in ("cfg5_rotsweep", "cfg5_rotsweep_hoisted"):
+        line = run_rotsweep(args, hoisted=args.workload.endswith("hoisted"))
     elif args.workload == "cfg3_compress":
         line = run_compress(args)
     else:

@@ -243,6 +243,11 @@ fenc_status fenc_fc(fenc_ctx *ctx, const fenc_keys *keys, const fenc_fc_desc *fc
  * compared with the oracle's hoisted variant.  Outer rotations, fenc_rotate and fenc_compress are unaffected.
  * Default: off.  Takes effect for the calls that follow. */
 fenc_status fenc_set_hoisting(fenc_ctx *ctx, int on);
+/* The same form as a primitive: every input (all at one level) rotated by every amount, one decomposition per input.
+ * out (capacity n_in * n_steps) receives out[i * n_steps + s] = Rot(in[i], steps[s]); an amount of 0 copies.
+ * FENC_ERR_NO_KEY if a rotation key is missing; nothing is written to out on failure. */
+fenc_status fenc_rotate_hoisted(fenc_ctx *ctx, const fenc_keys *keys, fenc_ct *const *in, size_t n_in, const int32_t *steps,
+                                size_t n_steps, fenc_ct **out);
 
 /* ------------------------------------------------------------------ AAC compress (R2.11) */
 /* out[t] = sum over the terms with term_out[i] == t of Rot(mask (*) in[term_src[i]], term_rot[i]).

@@ -65,7 +65,7 @@ SYMBOLS = ["fenc_params_init", "fenc_ctx_free", "fenc_last_error", "fenc_get_pri
            "fenc_profile_enable", "fenc_profile_kernels", "fenc_profile_name", "fenc_profile_read", "fenc_fc_plan",
            "fenc_fc_wts_keys", "fenc_fc_weights", "fenc_fc_weights_from_coeffs", "fenc_fc", "fenc_measure_alu_peak",
            "fenc_cmult_relin", "fenc_mul_scalar", "fenc_add_const", "fenc_ct_import_async", "fenc_ct_export_async",
-           "fenc_export_wait", "fenc_set_hoisting"]
+           "fenc_export_wait", "fenc_set_hoisting", "fenc_rotate_hoisted"]
 
 _lib = None
 
@@ -102,6 +102,7 @@ def load_library(path=None):
         "fenc_ct_export_async": [vp, vp, u64p],
         "fenc_export_wait": [vp],
         "fenc_set_hoisting": [vp, C.c_int],
+        "fenc_rotate_hoisted": [vp, vp, vpp, C.c_size_t, i32p, C.c_size_t, vpp],
         "fenc_ct_info": [vp, vp, u32p, dp, vpp],
         "fenc_rotate": [vp, vp, vpp, i32p, C.c_size_t, vpp],
         "fenc_rescale": [vp, vpp, C.c_size_t, vpp],
@@ -383,6 +384,14 @@ class Context:
 
     def export_wait(self):
         self._ck(self.lib.fenc_export_wait(self.h))
+
+    def rotate_hoisted(self, keys, cts, steps):
+        """every ciphertext by every amount, one decomposition per ciphertext (R2.7b) -> list [ct][step]"""
+        st = np.asarray(list(steps), dtype=np.int32)
+        n, m = len(cts), len(st)
+        out = (C.c_void_p * (n * m))()
+        self._ck(self.lib.fenc_rotate_hoisted(self.h, keys.h, self._harr(cts), n, _ptr(st, C.c_int32), m, out))
+        return [[Ciphertext(self, C.c_void_p(out[i * m + s])) for s in range(m)] for i in range(n)]
 
     def _harr(self, handles):
         return (C.c_void_p * len(handles))(*[x.h.value for x in handles])

@@ -382,6 +382,33 @@ extern "C" fenc_status fenc_rotate(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *c
   return FENC_OK;
 }
 
+// every input rotated by every amount with ONE decomposition per input (R2.7b); out[i * n_steps + s] = Rot(in[i], steps[s])
+extern "C" fenc_status fenc_rotate_hoisted(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const *in, size_t n_in, const int32_t *steps,
+                                           size_t n_steps, fenc_ct **out) {
+  Scope sc(ctx);
+  if (!ctx || !K || !in || !steps || !out) return FENC_ERR_INVALID_ARG;
+  if (n_in == 0 || n_steps == 0) return FENC_OK;
+  const int L = in[0]->L;
+  std::vector<const u64 *> src(n_in);
+  std::vector<int> src_of, vs;
+  std::vector<u64 *> vout;
+  std::vector<fenc_ct *> made;
+  for (size_t i = 0; i < n_in; i++) {
+    if (in[i]->L != L) return fail(ctx, FENC_ERR_MISMATCH, "rotate: inputs differ in level");
+    src[i] = in[i]->d;
+    for (size_t s = 0; s < n_steps; s++) {
+      fenc_ct *c = sc.ct(L, in[i]->scale);
+      if (!c) return fail(ctx, FENC_ERR_OOM, "rotate output");
+      made.push_back(c), vout.push_back(c->d), src_of.push_back((int)i), vs.push_back(steps[s]);
+    }
+  }
+  fenc_status st = rotate_hoisted_raw(ctx, K, L, src, src_of, vs, vout);
+  if (st != FENC_OK) return st;
+  sc.ok = true;
+  for (size_t i = 0; i < made.size(); i++) out[i] = made[i];
+  return FENC_OK;
+}
+
 extern "C" fenc_status fenc_rescale(fenc_ctx *ctx, fenc_ct *const *in, size_t n, fenc_ct **out) {
   Scope sc(ctx);
   if (!ctx || !in || !out) return FENC_ERR_INVALID_ARG;

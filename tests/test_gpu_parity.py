@@ -314,6 +314,43 @@ def test_rotation_wide_digit_groups(mods, n_q, q_bits, n_p, dnum):
     ctx.close()
 
 
+@pytest.mark.parametrize("name", ["toy64", "mid10", "mid12"])
+def test_rotate_hoisted_bit_exact(mods, name):
+    """fenc_rotate_hoisted (R2.7b) against the oracle's hoisted rotation: several ciphertexts by several amounts
+    (including 0 and n-1) at the top level and one level down (short last digit)."""
+    ck, fr, fenc = mods
+    P, ctx = make(mods, name)
+    steps = [1, 5, 0, P.n - 1, P.n // 2]
+    ok, gk = ck.keygen(P, 17, steps), ctx.keygen(17, steps)
+    for L in (P.nq, P.nq - 1):
+        limbs = [wl.random_ct_limbs(40 + 3 * L + i, P.q, L, P.N) for i in range(3)]
+        outs = ctx.rotate_hoisted(gk, [ctx.ct_import(a) for a in limbs], steps)
+        for a, row in zip(limbs, outs):
+            for r, o in zip(steps, row):
+                assert np.array_equal(ctx.ct_export(o), ck.rotate_hoisted(P, ok, ck.Ciphertext(a, L, 1), r).c), (L, r)
+    z = np.random.default_rng(2).uniform(-1, 1, P.n)
+    pt = ck.encode(P, z, P.nq)
+    g = ctx.encrypt(gk, ctx.pt_from_coeffs(pt.coeffs, P.nq, float(pt.scale)), 3)
+    assert np.abs(ctx.decrypt_slots(gk, ctx.rotate_hoisted(gk, [g], [5])[0][0]).real - np.roll(z, -5)).max() < 1e-3
+    ctx.close()
+
+
+def test_rotate_hoisted_full_size_config3_sampled(mods):
+    """N=2^16, 24+4 limbs (config 3), the launch configuration of the hoisted sweep: two ciphertexts by two amounts, the
+    oracle checks one of the four fully."""
+    ck, fr, fenc = mods
+    P, ctx = make(mods, "cfg3")
+    steps = [1, 12345]
+    gk = ctx.keygen(5, steps)
+    ok = ck.keygen(P, 5, steps[1:])
+    L = P.nq
+    limbs = [wl.random_ct_limbs(21 + i, P.q, L, P.N) for i in range(2)]
+    outs = ctx.rotate_hoisted(gk, [ctx.ct_import(a) for a in limbs], steps)
+    ref = ck.rotate_hoisted(P, ok, ck.Ciphertext(limbs[1], L, 1), 12345)
+    assert np.array_equal(ctx.ct_export(outs[1][1]), ref.c)
+    ctx.close()
+
+
 def test_import_async_matches_import(mods):
     """fenc_ct_import_async (copy stream + staging ring) gives the ciphertexts of fenc_ct_import, also when the ring wraps
     (more uploads in flight than slots would be needed: 70 > 64), when the level changes between uploads, and with work
