@@ -482,6 +482,30 @@ def square_relin(params: Params, keys: Keys, ct: Ciphertext) -> Ciphertext:
     return rescale(params, Ciphertext(out, L, ct.scale * ct.scale))
 
 
+def square_sum_relin(params: Params, keys: Keys, cts) -> Ciphertext:
+    """Sum of squares with ONE relinearisation (R2.12c; x^2 followed by sum-pooling): the tensor products
+    are added component-wise first, (D0, D1, D2) = sum_i (c0_i c0_i, 2 c0_i c1_i, c1_i c1_i), then
+    (D0, D1) + KS(D2; relin) and one rescale.  Decrypts to sum_i x_i^2; for a single ciphertext it is square_relin."""
+    L, N = cts[0].L, params.N
+    D = np.zeros((3, L, N), dtype=np.uint64)
+    t0 = np.zeros((L, N), dtype=np.uint64)
+    for ct in cts:
+        assert ct.L == L and ct.scale == cts[0].scale
+        for k, (a, b) in enumerate(((0, 0), (0, 1), (1, 1))):
+            _lib.orc_polymul_rns(params._h, L, _p(ct.c[a]), _p(ct.c[b]), _p(t0))
+            for t in range(L):
+                q = np.uint64(params.mod[t])
+                term = (t0[t] + t0[t]) % q if k == 1 else t0[t]
+                D[k, t] = (D[k, t] + term) % q
+    k0, k1 = keyswitch(params, L, D[2], keys.evk[RELIN_KEY_ID])
+    out = np.zeros_like(cts[0].c)
+    for t in range(L):
+        q = np.uint64(params.mod[t])
+        out[0, t] = (D[0, t] + k0[t]) % q
+        out[1, t] = (D[1, t] + k1[t]) % q
+    return rescale(params, Ciphertext(out, L, cts[0].scale * cts[0].scale))
+
+
 # --------------------------------------------------------------------------- CMult, PMultConst, degree-3 activation (R2.8, R2.12)
 def cmult_relin(params: Params, keys: Keys, x: Ciphertext, y: Ciphertext) -> Ciphertext:
     """(d0, d1, d2) = (x0 y0, x0 y1 + x1 y0, x1 y1); (d0, d1) + KS(d2; relin); then rescale (PAPER.md:63 CMult; R2.12)."""

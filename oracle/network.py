@@ -205,11 +205,25 @@ def sum_pool(ck, params, cts, S):
 
 
 # --------------------------------------------------------------------------- sequential network
-def run_network(ck, params, keys, layers, cts, L0, hoist=False):
+def square_pool(ck, params, keys, cts, S):
+    """x^2 followed by the 2x2 sum-pool as one step with lazy relinearisation (R2.12c): one ck.square_sum_relin per
+    pooled output over its four fragments (order as in sum_pool)."""
+    order = pool_order(len(cts), S)
+    return [ck.square_sum_relin(params, keys, [cts[j] for j in order[i:i + 4]]) for i in range(0, len(order), 4)]
+
+
+def run_network(ck, params, keys, layers, cts, L0, hoist=False, lazy_relin=False):
     """layers as in paper_2606_16359_b200.pipeline.Pipeline (dicts with op = conv / square / pool / fc and fp64 weights);
     cts: oracle ciphertexts ordered [bg][g][u][v].  Returns (final ciphertext list, list of per-layer outputs)."""
     L, S, trace = L0, None, []
-    for ly in layers:
+    for li, ly in enumerate(layers):
+        if lazy_relin and ly["op"] == "pool" and li > 0 and layers[li - 1]["op"] == "square":
+            trace.append(cts)  # done together with the square before it
+            continue
+        if lazy_relin and ly["op"] == "square" and li + 1 < len(layers) and layers[li + 1]["op"] == "pool":
+            cts, S, L = square_pool(ck, params, keys, cts, S), S // 2, L - 1
+            trace.append(cts)
+            continue
         if ly["op"] == "conv":
             graph = fr.ConvGraph(fr.ConvDesc(S=ly["S"], **ly["conv"]), params.n)
             W = fr.encode_weights(ck, params, graph, ly["w"], L)

@@ -344,6 +344,29 @@ def test_rotation_is_left_cyclic_shift(toy, toy_keys):
     assert np.abs(ck.decrypt_decode(P, toy_keys, ck.rotate(P, toy_keys, ct3, 2)) - np.roll(z, -2)).max() < 1e-4
 
 
+def test_square_sum_relin_is_sum_of_squares(toy, toy_keys):
+    """R2.12c: the tensor products of several ciphertexts added before ONE relinearisation decrypt to the sum of the
+    squared slot vectors; with one ciphertext the limbs are square_relin's; with four they are not the sum of four
+    square_relin results (one key-switch noise instead of four), but decrypt to the same values."""
+    P = toy
+    rng = np.random.default_rng(31)
+    zs = [rng.uniform(-1, 1, P.n) for _ in range(4)]
+    cts = [ck.encrypt(P, toy_keys, ck.encode(P, z, P.nq), 200 + i) for i, z in enumerate(zs)]
+    one = ck.square_sum_relin(P, toy_keys, cts[:1])
+    assert np.array_equal(one.c, ck.square_relin(P, toy_keys, cts[0]).c) and one.L == P.nq - 1
+    four = ck.square_sum_relin(P, toy_keys, cts)
+    assert four.L == P.nq - 1 and four.scale == one.scale
+    want = sum(z * z for z in zs)
+    assert np.abs(ck.decrypt_decode(P, toy_keys, four).real - want).max() < 1e-3
+    eager = ck.square_relin(P, toy_keys, cts[0])
+    for c in cts[1:]:
+        eager = ck.add(P, eager, ck.square_relin(P, toy_keys, c))
+    assert not np.array_equal(eager.c, four.c)
+    assert np.abs(ck.decrypt_decode(P, toy_keys, eager).real - ck.decrypt_decode(P, toy_keys, four).real).max() < 1e-3
+    two = ck.square_sum_relin(P, toy_keys, cts[:2])
+    assert np.abs(ck.decrypt_decode(P, toy_keys, two).real - (zs[0] ** 2 + zs[1] ** 2)).max() < 1e-3
+
+
 def test_hoisted_rotation_decrypts_like_rotation(toy, toy_keys):
     """R2.7b: the hoisted form (ModUp of the unrotated c1, automorphism on the extended digits) is the same LEFT cyclic
     shift with key-switch noise of the same size: the two decryptions differ by a small integer polynomial (the

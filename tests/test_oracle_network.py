@@ -116,8 +116,8 @@ def plain_network(layers, x):
     return x
 
 
-@pytest.mark.parametrize("bsgs,hoist", [(1, False), (0, False), (0, True)])
-def test_encrypted_toy_network_matches_fp64(bsgs, hoist):
+@pytest.mark.parametrize("bsgs,hoist,lazy", [(1, False, False), (0, False, False), (0, True, False), (0, True, True)])
+def test_encrypted_toy_network_matches_fp64(bsgs, hoist, lazy):
     P = ck.Params(9, 5, 40, 2, 60, 3, 40)
     layers, x = toy_network(bsgs=bsgs)
     steps, relin = nw.network_rot_steps(layers, P.n)
@@ -125,7 +125,8 @@ def test_encrypted_toy_network_matches_fp64(bsgs, hoist):
     lin = fr.Layout(P.n, 8, 2, 2, 1)
     cts = [ck.encrypt(P, keys, ck.encode(P, lin.gather(x, u, v, g, bg), P.nq), 100 + i)
            for i, (u, v, g, bg) in enumerate(lin.ct_keys())]
-    out, _ = nw.run_network(ck, P, keys, layers, cts, P.nq, hoist=hoist)
+    out, trace = nw.run_network(ck, P, keys, layers, cts, P.nq, hoist=hoist, lazy_relin=lazy)
+    assert len(trace) == len(layers)
     assert len(out) == 1 and out[0].L == 1
     g = nw.FcGraph(P.n, **layers[-1]["fc"])
     Y = np.zeros((2, 3))
