@@ -169,6 +169,14 @@ fenc_status fenc_pmult_sum(fenc_ctx *ctx, fenc_ct *const *in, fenc_pt *const *pt
 /* out[i] = in[i]^2 relinearised and rescaled (a13; R2.12), all n in ONE batched key switch; inputs share the level */
 fenc_status fenc_square_relin(fenc_ctx *ctx, const fenc_keys *keys, fenc_ct *const *in, size_t n, fenc_ct **out);
 /* out[i] = a[i] * b[i] relinearised and rescaled (CMult; R2.12); square_relin is the case b = a */
+/* Sum of squares with ONE relinearisation (R2.12c; x^2 followed by the 2x2 sum-pool of PAPER.md:284): output o is
+ *   rescale( (D0, D1) + KS(D2; relin) ),  (D0, D1, D2) = sum_{i < group} (c0 c0, 2 c0 c1, c1 c1) of in[o*group + i]:
+ * the tensor products are added before the key switch, so a pooled output costs one relinearisation instead of `group`.
+ * in: n_out*group ciphertexts at one level and scale (host array of handles); out: n_out new ciphertexts at L-1 and
+ * scale^2 / q_{L-1}.  group = 1 is fenc_square_relin.  Decrypts to the sum of the squared slot vectors; the limbs
+ * differ from the sum of `group` fenc_square_relin results (compare with the oracle's square_sum_relin). */
+fenc_status fenc_square_sum_relin(fenc_ctx *ctx, const fenc_keys *keys, fenc_ct *const *in, size_t n_out, size_t group,
+                                  fenc_ct **out);
 fenc_status fenc_cmult_relin(fenc_ctx *ctx, const fenc_keys *keys, fenc_ct *const *a, fenc_ct *const *b, size_t n, fenc_ct **out);
 /* PMultConst (R2.8): out[i] = in[i] * k for the integer k given by its residues, host k_res[L] with k_res[t] = k mod q_t
  * (the caller rounds c*E exactly, R2.8); the scale is multiplied by scale_factor (= E).  No level is consumed. */

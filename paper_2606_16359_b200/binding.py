@@ -65,7 +65,7 @@ SYMBOLS = ["fenc_params_init", "fenc_ctx_free", "fenc_last_error", "fenc_get_pri
            "fenc_profile_enable", "fenc_profile_kernels", "fenc_profile_name", "fenc_profile_read", "fenc_fc_plan",
            "fenc_fc_wts_keys", "fenc_fc_weights", "fenc_fc_weights_from_coeffs", "fenc_fc", "fenc_measure_alu_peak",
            "fenc_cmult_relin", "fenc_mul_scalar", "fenc_add_const", "fenc_ct_import_async", "fenc_ct_export_async",
-           "fenc_export_wait", "fenc_set_hoisting", "fenc_rotate_hoisted"]
+           "fenc_export_wait", "fenc_set_hoisting", "fenc_rotate_hoisted", "fenc_square_sum_relin"]
 
 _lib = None
 
@@ -102,6 +102,7 @@ def load_library(path=None):
         "fenc_ct_export_async": [vp, vp, u64p],
         "fenc_export_wait": [vp],
         "fenc_set_hoisting": [vp, C.c_int],
+        "fenc_square_sum_relin": [vp, vp, vpp, C.c_size_t, C.c_size_t, vpp],
         "fenc_rotate_hoisted": [vp, vp, vpp, C.c_size_t, i32p, C.c_size_t, vpp],
         "fenc_ct_info": [vp, vp, u32p, dp, vpp],
         "fenc_rotate": [vp, vp, vpp, i32p, C.c_size_t, vpp],
@@ -428,6 +429,15 @@ class Context:
         self._ck(self.lib.fenc_square_relin(self.h, keys.h, self._harr(lst), len(lst), out))
         res = [Ciphertext(self, C.c_void_p(out[i])) for i in range(len(lst))]
         return res[0] if single else res
+
+    def square_sum_relin(self, keys, cts, group):
+        """consecutive groups of `group` ciphertexts -> sum of their squares with one relinearisation each (R2.12c)"""
+        lst = list(cts)
+        assert group >= 1 and len(lst) % group == 0
+        n = len(lst) // group
+        out = (C.c_void_p * n)()
+        self._ck(self.lib.fenc_square_sum_relin(self.h, keys.h, self._harr(lst), n, group, out))
+        return [Ciphertext(self, C.c_void_p(out[i])) for i in range(n)]
 
     def cmult_relin(self, keys, a, b):
         out = (C.c_void_p * len(a))()

@@ -299,6 +299,33 @@ __global__ void __launch_bounds__(256) tensor_product_kernel(const u64 *const *i
   o[LN + i] = addmod(mont_mul(a0, b1m, mc.q, mc.qinv_neg), mont_mul(a1, b0m, mc.q, mc.qinv_neg), mc.q);
   o[2 * LN + i] = mont_mul(a1, b1m, mc.q, mc.qinv_neg);
 }
+// sums of squares (R2.12c): d[o] = sum over the group's ciphertexts in[o*group + i] of (c0 c0, 2 c0 c1, c1 c1); d: [n][3][L][N]
+__global__ void __launch_bounds__(256) square_sum_kernel(const u64 *const *in, int group, u64 *d, const ModConst *mods, int L, int logN) {
+  const size_t LN = (size_t)L << logN;
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= LN) return;
+  const ModConst mc = mods[i >> logN];
+  u64 s0 = 0, s1 = 0, s2 = 0;
+  for (int gidx = 0; gidx < group; gidx++) {
+    const u64 *a = in[(size_t)blockIdx.y * group + gidx];
+    const u64 a0 = a[i], a1 = a[LN + i];
+    const u64 a0m = mont_mul(a0, mc.r2, mc.q, mc.qinv_neg), a1m = mont_mul(a1, mc.r2, mc.q, mc.qinv_neg);
+    const u64 x = mont_mul(a0, a1m, mc.q, mc.qinv_neg);
+    s0 = addmod(s0, mont_mul(a0, a0m, mc.q, mc.qinv_neg), mc.q);
+    s1 = addmod(s1, addmod(x, x, mc.q), mc.q);
+    s2 = addmod(s2, mont_mul(a1, a1m, mc.q, mc.qinv_neg), mc.q);
+  }
+  u64 *o = d + (size_t)blockIdx.y * 3 * LN;
+  o[i] = s0, o[LN + i] = s1, o[2 * LN + i] = s2;
+}
+int k_square_sum(const KCtx &k, const u64 *const *in, int group, u64 *d, int n, int L) {
+  if (n == 0) return 0;
+  dim3 grid((unsigned)(((size_t)L * k.N + 255) / 256), n);
+  PROF(k, K_ROWOP, (16.0 * group + 24.0) * L * k.N * n);
+  square_sum_kernel<<<grid, 256, 0, S(k)>>>(in, group, d, k.d_mods, L, k.geom.logN);
+  LAUNCH_CHECK(k);
+  return 0;
+}
 int k_tensor_product(const KCtx &k, const u64 *const *ina, const u64 *const *inb, u64 *d, int n, int L) {
   if (n == 0) return 0;
   dim3 grid((unsigned)(((size_t)L * k.N + 255) / 256), n);

@@ -171,6 +171,8 @@ int k_add_f_sprime(const KCtx &k, const u64 *x, const u64 *sp_mont, u32 g, const
 int k_mul_rows(const KCtx &k, const u64 *a, const u64 *b, u64 *out, const int *row_mod, int n_rows);
 // tensor product of n ciphertext pairs: d[b] = (a0 b0, a0 b1 + a1 b0, a1 b1), d: [n][3][L][N]
 int k_tensor_product(const KCtx &k, const u64 *const *ina, const u64 *const *inb, u64 *d, int n, int L);
+// d[o] = sum_{i < group} (c0 c0, 2 c0 c1, c1 c1) of in[o*group + i]  (R2.12c)
+int k_square_sum(const KCtx &k, const u64 *const *in, int group, u64 *d, int n, int L);
 // out[b] = in[b] * k (kl: per-limb Montgomery form) or, add_const, c0 += k (kl: per-limb residues)
 int k_scalar(const KCtx &k, const u64 *const *in, u64 *const *out, const u64 *kl, int n, int L, bool add_const);
 // out[r] = a[r] + b[r] (+ b[r] again when twice)

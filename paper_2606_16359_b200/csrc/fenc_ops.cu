@@ -477,17 +477,23 @@ extern "C" fenc_status fenc_pmult_sum(fenc_ctx *ctx, fenc_ct *const *in, fenc_pt
 
 // CMult + relinearise + rescale (a13, R2.12): (d0, d1, d2) = (a0 b0, a0 b1 + a1 b0, a1 b1);
 // (d0, d1) + KS(d2; relin); rescale.  Batched over n pairs; x^2 is the case b = a.
-static fenc_status cmult_relin(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const *ina, fenc_ct *const *inb, size_t n, fenc_ct **out) {
+// group > 0 (R2.12c): inb is unused, ina holds n*group ciphertexts and output o is the sum of the squares of
+// ina[o*group .. o*group+group-1] with ONE relinearisation.
+static fenc_status cmult_relin(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const *ina, fenc_ct *const *inb, size_t n, fenc_ct **out,
+                               size_t group = 0) {
   Scope sc(ctx);
   if (n == 0) return FENC_OK;
+  const size_t n_in = group ? n * group : n;
+  if (group) inb = ina;
   auto it = K->evk.find(FENC_RELIN_KEY_ID);
   if (it == K->evk.end()) return fail(ctx, FENC_ERR_NO_KEY, "no relinearisation key");
   const int L = ina[0]->L;
   if (L < 2) return fail(ctx, FENC_ERR_LEVEL, "a product needs a level to rescale into");
   const size_t LN = (size_t)L * ctx->N;
-  std::vector<const u64 *> pa(n), pb(n);
-  for (size_t i = 0; i < n; i++) {
+  std::vector<const u64 *> pa(n_in), pb(n_in);
+  for (size_t i = 0; i < n_in; i++) {
     if (ina[i]->L != L || inb[i]->L != L) return fail(ctx, FENC_ERR_MISMATCH, "product: inputs differ in level");
+    if (group && !scale_close(ina[i]->scale, ina[0]->scale)) return fail(ctx, FENC_ERR_MISMATCH, "sum of squares: inputs differ in scale");
     pa[i] = ina[i]->d, pb[i] = inb[i]->d;
   }
   // N >= 2^12: the rescale is merged into the ModDown of the relinearisation (one pass less over the ciphertext)
@@ -499,14 +505,16 @@ static fenc_status cmult_relin(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const
     size_t o0 = st.add(pa), o1 = st.add(pb);
     char *base = st.commit();
     if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
-    CUDA_OK(ctx, k_tensor_product(ctx->k, (const u64 *const *)(base + o0), (const u64 *const *)(base + o1), d, (int)n, L));
+    if (group) CUDA_OK(ctx, k_square_sum(ctx->k, (const u64 *const *)(base + o0), (int)group, d, (int)n, L));
+    else CUDA_OK(ctx, k_tensor_product(ctx->k, (const u64 *const *)(base + o0), (const u64 *const *)(base + o1), d, (int)n, L));
   }
   std::vector<BatchItem> items(n), rs(n);
   std::vector<fenc_ct *> made(n, nullptr);
   for (size_t i = 0; i < n; i++) {
     u64 *di = d + i * 3 * LN;
     items[i] = BatchItem{};
-    made[i] = sc.ct(L - 1, ina[i]->scale * inb[i]->scale / (double)ctx->mod[L - 1]);
+    const size_t i0 = group ? i * group : i;
+    made[i] = sc.ct(L - 1, ina[i0]->scale * inb[i0]->scale / (double)ctx->mod[L - 1]);
     if (!made[i]) return fail(ctx, FENC_ERR_OOM, "product output");
     items[i].ks_in = di + 2 * LN, items[i].out = merged ? made[i]->d : mid + i * 2 * LN, items[i].evk = it->second;
     items[i].add0 = di, items[i].add1 = di + LN, items[i].g = 1;
@@ -524,6 +532,11 @@ static fenc_status cmult_relin(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const
 extern "C" fenc_status fenc_square_relin(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const *in, size_t n, fenc_ct **out) {
   if (!ctx || !K || !in || !out) return FENC_ERR_INVALID_ARG;
   return cmult_relin(ctx, K, in, in, n, out);
+}
+extern "C" fenc_status fenc_square_sum_relin(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const *in, size_t n_out, size_t group,
+                                             fenc_ct **out) {
+  if (!ctx || !K || !in || !out || group < 1) return FENC_ERR_INVALID_ARG;
+  return cmult_relin(ctx, K, in, in, n_out, out, group);
 }
 extern "C" fenc_status fenc_cmult_relin(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const *a, fenc_ct *const *b, size_t n, fenc_ct **out) {
   if (!ctx || !K || !a || !b || !out) return FENC_ERR_INVALID_ARG;

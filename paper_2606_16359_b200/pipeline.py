@@ -69,11 +69,11 @@ class Pipeline:
         self.L_out = L
         self.keys, self.weights = None, []
 
-    def counts(self):
+    def counts(self, lazy_relin=False):
         """(linear layers, key-switched rotations, relinearisations, PMults) of one forward pass."""
         lin = rot = relin = pm = 0
         n_ct = None
-        for p in self.plan:
+        for li, p in enumerate(self.plan):
             if p["op"] == "conv":
                 lin += 1
                 rot += p["lay"].n_inner_rot + p["lay"].n_outer_rot
@@ -85,7 +85,8 @@ class Pipeline:
                 pm += p["info"]["n_pmult"]
                 n_ct = p["info"]["n_out_ct"]
             elif p["op"] == "square":
-                relin += n_ct
+                pooled = lazy_relin and li + 1 < len(self.plan) and self.plan[li + 1]["op"] == "pool"
+                relin += n_ct // 4 if pooled else n_ct
             elif p["op"] == "pool":
                 n_ct //= 4
         return lin, rot, relin, pm
@@ -137,13 +138,23 @@ class Pipeline:
                             idx.append(base + (2 * uo + a) * S + (2 * vo + b))
         return idx
 
-    def forward(self, cts, trace=None, scale=None):
-        """scale: exact rational scale of the inputs (default: the context's 2^log2_scale); only poly3 needs it."""
+    def forward(self, cts, trace=None, scale=None, lazy_relin=False):
+        """scale: exact rational scale of the inputs (default: the context's 2^log2_scale); only poly3 needs it.
+        lazy_relin: a square directly followed by a pool runs as ONE step, fenc_square_sum_relin over the four fragments of
+        every pooled output (one relinearisation instead of four, R2.12c); the trace then holds the pooled
+        ciphertexts at both positions."""
         ctx = self.ctx
         S = None
         sc = Fraction(cts[0].scale) if scale is None else Fraction(scale)
-        for p, w in zip(self.plan, self.weights):
-            if p["op"] == "conv":
+        for li, (p, w) in enumerate(zip(self.plan, self.weights)):
+            fused_prev = lazy_relin and p["op"] == "pool" and li > 0 and self.plan[li - 1]["op"] == "square"
+            if fused_prev:
+                pass  # done together with the square before it
+            elif lazy_relin and p["op"] == "square" and li + 1 < len(self.plan) and self.plan[li + 1]["op"] == "pool":
+                cts = ctx.square_sum_relin(self.keys, [cts[i] for i in self.pool_order(len(cts), S)], 4)
+                sc = sc * sc / ctx.q[p["L"] - 1]
+                S //= 2
+            elif p["op"] == "conv":
                 cts = ctx.hconv(self.keys, p["conv"], p["lay"], w, cts, do_rescale=True)
                 S = p["lay"].S_out  # weights at s_w = q_{L-1} and one rescale: the scale is unchanged (A14)
             elif p["op"] == "fc":

@@ -444,8 +444,34 @@ def test_fc_bit_exact(mods, kw):
     ctx.close()
 
 
-@pytest.mark.parametrize("bsgs,hoist", [(1, False), (0, False), (0, True)])
-def test_pipeline_toy_network_bit_exact(mods, bsgs, hoist):
+def test_square_sum_relin_bit_exact(mods):
+    """fenc_square_sum_relin (R2.12c) against the oracle's square_sum_relin: groups of 4, 2 and 1 ciphertexts at two ring
+    sizes (merged and unmerged ModDown + rescale), and the decoded sum of squares."""
+    ck, fr, fenc = mods
+    for name in ("mid10", "mid12"):
+        P, ctx = make(mods, name)
+        ok, gk = ck.keygen(P, 23, [], want_relin=True), ctx.keygen(23, [], want_relin=True)
+        rng = np.random.default_rng(12)
+        zs = [rng.uniform(-1, 1, P.n) for _ in range(8)]
+        o_in, g_in = [], []
+        for i, z in enumerate(zs):
+            pt = ck.encode(P, z, P.nq)
+            o_in.append(ck.encrypt(P, ok, pt, 300 + i))
+            g_in.append(ctx.encrypt(gk, ctx.pt_from_coeffs(pt.coeffs, P.nq, float(pt.scale)), 300 + i))
+        for group in (4, 2, 1):
+            got = ctx.square_sum_relin(gk, g_in, group)
+            assert len(got) == 8 // group
+            for o, g in enumerate(got):
+                ref = ck.square_sum_relin(P, ok, o_in[o * group:(o + 1) * group])
+                assert g.L == ref.L and np.array_equal(ctx.ct_export(g), ref.c), (name, group, o)
+                assert abs(g.scale - float(ref.scale)) <= 1e-9 * float(ref.scale)
+            want = sum(z * z for z in zs[:group])
+            assert np.abs(ctx.decrypt_slots(gk, got[0]).real - want).max() < 1e-4
+        ctx.close()
+
+
+@pytest.mark.parametrize("bsgs,hoist,lazy", [(1, False, False), (0, False, False), (0, True, False), (0, True, True)])
+def test_pipeline_toy_network_bit_exact(mods, bsgs, hoist, lazy):
     """conv - square - pool - fc - fc through Pipeline (one batched C-ABI call per layer) vs the oracle's network."""
     ck, fr, fenc = mods
     from oracle import network as nw
@@ -481,9 +507,9 @@ def test_pipeline_toy_network_bit_exact(mods, bsgs, hoist):
         pt = ck.encode(P, lin.gather(x, u, v, g, bg), P.nq)
         o_in.append(ck.encrypt(P, ok, pt, 100 + i))
         g_in.append(ctx.encrypt(gk, ctx.pt_from_coeffs(pt.coeffs, P.nq, float(pt.scale)), 100 + i))
-    o_out, o_trace = nw.run_network(ck, P, ok, layers, o_in, P.nq, hoist=hoist)
+    o_out, o_trace = nw.run_network(ck, P, ok, layers, o_in, P.nq, hoist=hoist, lazy_relin=lazy)
     g_trace = []
-    g_out = pipe.forward(g_in, trace=g_trace)
+    g_out = pipe.forward(g_in, trace=g_trace, lazy_relin=lazy)
     for li, (ol, gl) in enumerate(zip(o_trace, g_trace)):
         assert len(ol) == len(gl), li
         for a, b in zip(ol, gl):
@@ -680,17 +706,19 @@ def test_lenet5_full_size_bsgs_and_hoisting_decoded(mods):
     cts = pipe.encrypt_input(x, 20000)
     fg = nw.FcGraph(ctx.n, **layers[-1]["fc"])
     got = {}
-    for hoist in (False, True):
+    for hoist, lazy in ((False, False), (True, False), (True, True)):
         ctx.set_hoisting(hoist)
-        out = pipe.forward(cts)
+        out = pipe.forward(cts, lazy_relin=lazy)
         assert len(out) == 1 and out[0].L == 1
         Y = np.zeros((128, 10))
         fg.scatter_out(Y, ctx.decrypt_slots(keys, out[0]).real, 0, 0)
-        assert np.abs(Y - want).max() < 1e-3, hoist
-        got[hoist] = Y
-    assert np.abs(got[True] - got[False]).max() < 1e-4 and not np.array_equal(got[True], got[False])
+        assert np.abs(Y - want).max() < 1e-3, (hoist, lazy)
+        got[(hoist, lazy)] = Y
+    assert np.abs(got[(True, False)] - got[(False, False)]).max() < 1e-4 and not np.array_equal(got[(True, False)], got[(False, False)])
+    assert np.abs(got[(True, True)] - got[(True, False)]).max() < 1e-4 and not np.array_equal(got[(True, True)], got[(True, False)])
     n_lin, n_rot, n_relin, n_pm = pipe.counts()
     assert (n_lin, n_rot, n_relin) == (5, 367, 160)  # 48 + 192 conv rotations, 78 + 28 + 21 BSGS rotations (315 plain)
+    assert pipe.counts(lazy_relin=True)[2] == 40      # 24 + 16 pooled outputs, one relinearisation each
     ctx.close()
 
 
