@@ -480,7 +480,8 @@ def cpu_baseline(args, pipe, budget_s=20.0):
     n_lin = pipe.counts()[0]
     return {"value": round(n_lin / est, 6), "unit": "encrypted conv layers/s", "cores": 1, "kind": "oracle",
             "sample": "one rotation, PMult-accumulate, rescale and square+relin per level used (%s), timed once each on the "
-                      "oracle and scaled by the step's exact operation counts; estimated oracle step %.1f s" % (
+                      "oracle and scaled by the step's exact operation counts (rotations as plain ones -- the oracle's hoisted rotation costs "
+                      "the same --, squares counted before the pool); estimated oracle step %.1f s" % (
                           ", ".join("L=%d" % L for L in sorted(ops, reverse=True)), est),
             "seconds_per_op": detail}
 
