@@ -569,7 +569,7 @@ struct HoistMacP {
 // the highest bit of the exponent index, which an odd multiplier maps to itself), so x, b and a all arrive as 16-byte
 // loads; the loads of digit j+1 are issued before the products of digit j.
 struct HoistOperands { ulonglong2 x, b, a; };
-__global__ void __launch_bounds__(256) hoisted_keymac_kernel(HoistMacP p) {
+__global__ void __launch_bounds__(256, 4) hoisted_keymac_kernel(HoistMacP p) {
   const int tid = threadIdx.x, nb = p.n_batch, b = blockIdx.x % nb, chunk = blockIdx.x / nb, t = blockIdx.y;
   const int N = 1 << p.logN;
   const int mod = t < p.L ? t : p.nq + (t - p.L);
