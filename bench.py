@@ -85,6 +85,9 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------ workloads
+FC_BSGS = 0  # baby-step count of the fully connected layers: 0 = library's choice (R2.12b), 1 = plain diagonals (--plain-fc)
+
+
 def lenet_layers(BS, seed, upto="fc"):
     """BASELINE config 2: LeNet-5-shaped network on MNIST-shaped input (D2).  S=4 for conv1
     (the paper's best LeNet block size); pooling halves S; the 1/4 pool factors live in the next weights."""
@@ -102,9 +105,9 @@ def lenet_layers(BS, seed, upto="fc"):
         f2 = rng.normal(0, 0.1, (84, 120))
         f3 = rng.normal(0, 0.1, (10, 84))
         layers += [
-            {"op": "fc", "fc": dict(BS=BS, n_in=400, n_out=120, in_C=16, in_H=5, in_W=5, in_M=8, bsgs=0), "w": f1},
-            {"op": "fc", "fc": dict(BS=BS, n_in=120, n_out=84, in_M=8, bsgs=0), "w": f2},
-            {"op": "fc", "fc": dict(BS=BS, n_in=84, n_out=10, in_M=8, bsgs=0), "w": f3},
+            {"op": "fc", "fc": dict(BS=BS, n_in=400, n_out=120, in_C=16, in_H=5, in_W=5, in_M=8, bsgs=FC_BSGS), "w": f1},
+            {"op": "fc", "fc": dict(BS=BS, n_in=120, n_out=84, in_M=8, bsgs=FC_BSGS), "w": f2},
+            {"op": "fc", "fc": dict(BS=BS, n_in=84, n_out=10, in_M=8, bsgs=FC_BSGS), "w": f3},
         ]
     x = rng.uniform(0, 1, (BS, 1, 28, 28))
     return layers, x
@@ -543,10 +546,14 @@ def main():
     ap.add_argument("--batch", type=int, default=128)
     ap.add_argument("--cpu-budget", type=float, default=20.0)
     ap.add_argument("--profile-range", action="store_true", help="cudaProfilerStart/Stop around the timed steps (for ncu)")
+    ap.add_argument("--plain-fc", action="store_true", help="fully connected layers by plain diagonals (no baby-step giant-step)")
     ap.add_argument("--eager-relin", action="store_true", help="x^2 and the pool after it as two steps (four relinearisations per pooled output)")
     ap.add_argument("--no-hoist", action="store_true", help="inner rotations as plain rotations (one decomposition each)")
     ap.add_argument("--no-extras", action="store_true", help="skip the per-kernel pass, e2e and cpu_baseline (profiling runs)")
     args = ap.parse_args()
+    if args.plain_fc:
+        global FC_BSGS
+        FC_BSGS = 1
     rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
     if args.impl == "reference":
         if rank == 0:
