@@ -576,12 +576,13 @@ def test_lenet_conv1_full_size_sampled(mods):
 
 
 # ------------------------------------------------------------------------------------------------ full-size properties (configs 3, 4)
-def decoded_conv_error(mods, pkey, conv_kw, S, seed, kaiming=False, w_std=0.1):
+def decoded_conv_error(mods, pkey, conv_kw, S, seed, kaiming=False, w_std=0.1, hoist=False):
     """Encrypted conv at a BASELINE parameter set through the library's own encoder; returns max |decoded - fp64 conv|.
     (The oracle needs minutes per output ciphertext at N=2^16, so full-size configs 3/4 are checked by this property,
     which holds at any size; their limbs are covered bit-exactly by the same graphs at reduced N above.)"""
     ck, fr, fenc = mods
     ctx = fenc.Context(**wl.PARAMS[pkey])
+    ctx.set_hoisting(hoist)
     x, w = wl.conv_inputs(seed, conv_kw, kaiming=kaiming, w_std=w_std)
     conv = ctx.conv_desc(S=S, **conv_kw)
     lay = ctx.layout_plan(conv)
@@ -620,6 +621,15 @@ def test_config3_resnet_layers_full_size_decoded(mods):
     assert err < 1e-3
     err, lay = decoded_conv_error(mods, "cfg3", wl.CONVS["resnet_32_64_s2"], 2, 303, kaiming=True)
     assert (lay.n_in_ct, lay.n_out_ct, lay.n_inner_rot, lay.n_outer_rot, lay.n_pmult) == (4, 1, 5, 94, 855)
+    assert err < 1e-3
+
+
+def test_config3_resnet_layer_full_size_hoisted_decoded(mods):
+    """The configuration bench.py's cfg3 workloads time: inner rotations in the hoisted form (R2.7b) at N=2^16, wide
+    fp64 butterflies, dlen 4 -- 8 rotations of one input ciphertext share one decomposition."""
+    err, lay = decoded_conv_error(mods, "cfg3", wl.CONVS["resnet_16_16"], 0, 301, kaiming=True, hoist=True)
+    assert (lay.n_inner_rot, lay.n_outer_rot) == (8, 30) and err < 1e-3
+    err, lay = decoded_conv_error(mods, "cfg3", wl.CONVS["resnet_16_32_s2"], 2, 302, kaiming=True, hoist=True)
     assert err < 1e-3
 
 
