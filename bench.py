@@ -150,9 +150,9 @@ def run_rotsweep(args, hoisted=False):
     import torch
     import paper_2606_16359_b200 as fenc
     peaks, peak_src = measured_peaks()
-    n_ct, n_steps, points = 64, 32, []
-    for L in (4, 8, 16, 24, 36):
-        for dnum in (1, 2, 3, 4):
+    n_ct, n_steps, points = args.sweep_cts, args.sweep_steps, []
+    for L in (args.sweep_L or (4, 8, 16, 24, 36)):
+        for dnum in (args.sweep_dnum or (1, 2, 3, 4)):
             pr = wl.sweep_params(L, dnum)
             ctx = fenc.Context(**pr)
             N, k, dlen = ctx.N, ctx.n_p, ctx.dlen
@@ -193,7 +193,7 @@ def run_rotsweep(args, hoisted=False):
             del cts, keys
             ctx.close()
             torch.cuda.empty_cache()
-    ref = [p for p in points if p["L"] == 24 and p["dnum"] == 3][0]
+    ref = ([p for p in points if p["L"] == 24 and p["dnum"] == 3] or points)[0]
     return {"metric": METRIC, "value": ref["rot_per_s"], "unit": "key-switched rotations/s", "n_gpus": 1, "steps": n_steps,
             "warmup": 2, "ms_per_step": round(1e3 * n_ct / ref["rot_per_s"], 4), "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "u64", "data": "synthetic",
@@ -549,6 +549,10 @@ def main():
     ap.add_argument("--plain-fc", action="store_true", help="fully connected layers by plain diagonals (no baby-step giant-step)")
     ap.add_argument("--eager-relin", action="store_true", help="x^2 and the pool after it as two steps (four relinearisations per pooled output)")
     ap.add_argument("--no-hoist", action="store_true", help="inner rotations as plain rotations (one decomposition each)")
+    ap.add_argument("--sweep-L", type=int, nargs="*", help="config 5: only these limb counts")
+    ap.add_argument("--sweep-dnum", type=int, nargs="*", help="config 5: only these dnum values")
+    ap.add_argument("--sweep-cts", type=int, default=64, help="config 5: ciphertexts per batched rotation (BASELINE: 64)")
+    ap.add_argument("--sweep-steps", type=int, default=32, help="config 5: distinct rotation amounts (BASELINE: 32)")
     ap.add_argument("--no-extras", action="store_true", help="skip the per-kernel pass, e2e and cpu_baseline (profiling runs)")
     args = ap.parse_args()
     if args.plain_fc:

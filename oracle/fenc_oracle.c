@@ -21,7 +21,7 @@
 typedef uint64_t u64;
 typedef unsigned __int128 u128;
 
-#define ORC_MAXLIMB 64
+#define ORC_MAXLIMB 96 /* config 5's largest point: 36 ciphertext + 36 special limbs */
 
 /* ------------------------------------------------------------------ modular scalars */
 u64 orc_mulmod(u64 a, u64 b, u64 q) { return (u64)(((u128)a * b) % q); }

@@ -454,6 +454,7 @@ LevelPlan *get_plan(fenc_ctx *ctx, int L) {
 
 // ------------------------------------------------------------------------------------------------ batched key switch
 static const size_t WS_CAP = (size_t)6 << 30;  // workspace budget for one chunk of a batch
+static const size_t GRID_Z_MAX = 65535;          // CUDA's limit on gridDim.z (small rings reach it before WS_CAP)
 
 bool ks_can_merge_rescale(const fenc_ctx *ctx, int L) {
   return L >= 2 && convert_cols_fits(ctx->logN, ctx->np + 1, true);
@@ -469,6 +470,7 @@ fenc_status ks_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items, bool r
   const size_t per = ((size_t)L + P->n_up + 2 * E + 2 * npy + 2 * L) * N;  // u64 per item
   size_t chunk = WS_CAP / (per * 8);
   if (chunk < 1) chunk = 1;
+  if (chunk > GRID_Z_MAX) chunk = GRID_Z_MAX;  // the batch index is blockIdx.z in the transform kernels
   if (chunk > items.size()) chunk = items.size();
   u64 *ws = (u64 *)workspace(ctx, chunk * per * 8);
   if (!ws) return fail(ctx, FENC_ERR_OOM, "key-switch workspace (%zu bytes)", chunk * per * 8);
@@ -540,7 +542,7 @@ fenc_status rescale_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items) {
   const size_t N = ctx->N;
   const int L1 = L - 1;
   const size_t per = ((size_t)2 + 2 * L1) * N;
-  size_t chunk = std::min(items.size(), std::max<size_t>(1, WS_CAP / (per * 8)));
+  size_t chunk = std::min(std::min(items.size(), GRID_Z_MAX), std::max<size_t>(1, WS_CAP / (per * 8)));
   u64 *ws = (u64 *)workspace(ctx, chunk * per * 8);
   if (!ws) return fail(ctx, FENC_ERR_OOM, "rescale workspace");
   u64 *yR = ws, *tmp2 = yR + chunk * 2 * N;
@@ -571,47 +573,66 @@ fenc_status rescale_batch(fenc_ctx *ctx, int L, std::vector<BatchItem> &items) {
 fenc_status rotate_hoisted_raw(fenc_ctx *ctx, const fenc_keys *keys, int L, const std::vector<const u64 *> &src,
                                const std::vector<int> &src_of, const std::vector<int> &steps, const std::vector<u64 *> &out) {
   if (steps.empty()) return FENC_OK;
-  Scope sc(ctx);
   LevelPlan *P = get_plan(ctx, L);
   if (!P) return fail(ctx, FENC_ERR_OOM, "level plan");
   const size_t N = ctx->N, LN = (size_t)L * N;
-  const int ns = (int)src.size();
-  u64 *y = sc.alloc<u64>((size_t)ns * LN), *up = sc.alloc<u64>((size_t)ns * P->n_up * N);
-  if (!y || !up) return fail(ctx, FENC_ERR_OOM, "hoisted decomposition (%d sources)", ns);
-  {
-    DescStage st(ctx);
-    std::vector<BatchItem> sitems(ns);
-    for (int i = 0; i < ns; i++) sitems[i] = BatchItem{}, sitems[i].ks_in = src[i] + LN, sitems[i].g = 1;
-    st.add(sitems);
-    const BatchItem *d_src = (const BatchItem *)st.commit();
-    if (!d_src) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
-    const KCtx &k = ctx->k;
-    if (convert_cols_fits(ctx->logN, P->n_src_up, false)) {
-      CUDA_OK(ctx, k_intt_rows_only(k, d_src, nullptr, 0, true, y, LN, P->d_rows_in, L, ns));
-      CUDA_OK(ctx, k_convert_cols(k, y, LN, P->d_groups_up, P->beta, P->n_src_up, P->d_scale_in, P->d_bc_up, P->d_rows_up, P->n_up, up,
-                                  (size_t)P->n_up * N, ns, ctx->lazy_q, nullptr, P->d_bc_up_f64));
-    } else {
-      CUDA_OK(ctx, k_intt(k, d_src, nullptr, 0, true, y, LN, P->d_rows_in, L, P->d_scale_in, ns));
-      CUDA_OK(ctx, k_ntt_cols_bconv(k, y, LN, P->d_bc_up, up, (size_t)P->n_up * N, P->d_rows_up, P->n_up, ns, L, ctx->lazy_q));
-    }
-    CUDA_OK(ctx, k_ntt_rows_only(k, up, (size_t)P->n_up * N, P->d_rows_up, P->n_up, ns));
-  }
-  std::vector<BatchItem> items;
+  // every key is looked up before anything is enqueued: nothing is written on FENC_ERR_NO_KEY
+  std::vector<const u64 *> evk(steps.size(), nullptr);
+  std::vector<int> red(steps.size());
   for (size_t i = 0; i < steps.size(); i++) {
-    const int r = ((steps[i] % ctx->n) + ctx->n) % ctx->n;
-    const u64 *in = src[src_of[i]];
-    if (r == 0) {
-      CUDA_OK(ctx, cudaMemcpyAsync(out[i], in, 2 * LN * 8, cudaMemcpyDeviceToDevice, ctx->stream));
-      continue;
-    }
-    auto it = keys->evk.find(r);
-    if (it == keys->evk.end()) return fail(ctx, FENC_ERR_NO_KEY, "no rotation key for step %d", r);
-    BatchItem b{};
-    b.ks_in = in + LN, b.out = out[i], b.evk = it->second, b.add0 = in, b.g = galois_elt(ctx, r), b.pad = (u32)src_of[i];
-    items.push_back(b);
+    red[i] = ((steps[i] % ctx->n) + ctx->n) % ctx->n;
+    if (red[i] == 0) continue;
+    auto it = keys->evk.find(red[i]);
+    if (it == keys->evk.end()) return fail(ctx, FENC_ERR_NO_KEY, "no rotation key for step %d", red[i]);
+    evk[i] = it->second;
   }
-  HoistUp h{up, (size_t)P->n_up * N, ns};
-  return ks_batch(ctx, L, items, false, &h);
+  // sources are processed in chunks whose decompositions (y + extended digits) stay under the workspace budget, so a
+  // large layer or batch costs more launches instead of FENC_ERR_OOM (the plain path chunks the same way in ks_batch)
+  const size_t per_src = (LN + (size_t)P->n_up * N) * 8;
+  const size_t ns_all = src.size();
+  const size_t chunk = std::min<size_t>(std::min(ns_all, GRID_Z_MAX), std::max<size_t>(1, WS_CAP / per_src));
+  std::vector<std::vector<size_t>> rots_of(ns_all);
+  for (size_t i = 0; i < steps.size(); i++) rots_of[src_of[i]].push_back(i);
+  for (size_t s0 = 0; s0 < ns_all; s0 += chunk) {
+    Scope sc(ctx);
+    const int ns = (int)std::min(chunk, ns_all - s0);
+    u64 *y = sc.alloc<u64>((size_t)ns * LN), *up = sc.alloc<u64>((size_t)ns * P->n_up * N);
+    if (!y || !up) return fail(ctx, FENC_ERR_OOM, "hoisted decomposition (%d sources)", ns);
+    {
+      DescStage st(ctx);
+      std::vector<BatchItem> sitems(ns);
+      for (int i = 0; i < ns; i++) sitems[i] = BatchItem{}, sitems[i].ks_in = src[s0 + i] + LN, sitems[i].g = 1;
+      st.add(sitems);
+      const BatchItem *d_src = (const BatchItem *)st.commit();
+      if (!d_src) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
+      const KCtx &k = ctx->k;
+      if (convert_cols_fits(ctx->logN, P->n_src_up, false)) {
+        CUDA_OK(ctx, k_intt_rows_only(k, d_src, nullptr, 0, true, y, LN, P->d_rows_in, L, ns));
+        CUDA_OK(ctx, k_convert_cols(k, y, LN, P->d_groups_up, P->beta, P->n_src_up, P->d_scale_in, P->d_bc_up, P->d_rows_up, P->n_up, up,
+                                    (size_t)P->n_up * N, ns, ctx->lazy_q, nullptr, P->d_bc_up_f64));
+      } else {
+        CUDA_OK(ctx, k_intt(k, d_src, nullptr, 0, true, y, LN, P->d_rows_in, L, P->d_scale_in, ns));
+        CUDA_OK(ctx, k_ntt_cols_bconv(k, y, LN, P->d_bc_up, up, (size_t)P->n_up * N, P->d_rows_up, P->n_up, ns, L, ctx->lazy_q));
+      }
+      CUDA_OK(ctx, k_ntt_rows_only(k, up, (size_t)P->n_up * N, P->d_rows_up, P->n_up, ns));
+    }
+    std::vector<BatchItem> items;
+    for (int si = 0; si < ns; si++)
+      for (size_t i : rots_of[s0 + si]) {
+        const u64 *in = src[s0 + si];
+        if (red[i] == 0) {
+          CUDA_OK(ctx, cudaMemcpyAsync(out[i], in, 2 * LN * 8, cudaMemcpyDeviceToDevice, ctx->stream));
+          continue;
+        }
+        BatchItem b{};
+        b.ks_in = in + LN, b.out = out[i], b.evk = evk[i], b.add0 = in, b.g = galois_elt(ctx, red[i]), b.pad = (u32)si;
+        items.push_back(b);
+      }
+    HoistUp h{up, (size_t)P->n_up * N, ns};
+    fenc_status st = ks_batch(ctx, L, items, false, &h);
+    if (st != FENC_OK) return st;
+  }
+  return FENC_OK;
 }
 
 // Rot(in[i], steps[i]) -> out[i]; all at level L (Eq. 1; R2.7: automorphism first)

@@ -36,7 +36,12 @@ static fenc_status make_switch_key(fenc_ctx *ctx, fenc_keys *K, int64_t key_id, 
   Scope sc(ctx);
   const int A = ctx->A, N = ctx->N, nq = ctx->nq;
   const size_t AN = (size_t)A * N;
-  u64 *evk = dalloc_t<u64>(ctx, (size_t)ctx->beta_max * 2 * AN);
+  // held by a guard until the key is complete: every early return below releases it
+  struct EvkGuard {
+    fenc_ctx *ctx; u64 *p;
+    ~EvkGuard() { if (p) dfree(ctx, p); }
+  } guard{ctx, dalloc_t<u64>(ctx, (size_t)ctx->beta_max * 2 * AN)};
+  u64 *evk = guard.p;
   u64 *d_a = sc.alloc<u64>(AN), *d_e = sc.alloc<u64>(AN);
   u64 *d_keys = sc.alloc<u64>(A), *d_f = sc.alloc<u64>(A);
   if (!evk || !d_a || !d_e || !d_keys || !d_f) return fail(ctx, FENC_ERR_OOM, "evaluation key");
@@ -64,6 +69,7 @@ static fenc_status make_switch_key(fenc_ctx *ctx, fenc_keys *K, int64_t key_id, 
     CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));  // hk / hf go out of scope
   }
   *out = evk;
+  guard.p = nullptr;
   return FENC_OK;
 }
 
