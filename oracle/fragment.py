@@ -208,6 +208,60 @@ class ConvGraph:
                     vec[base:base + L.B] = val
         return vec
 
+    # ---- factored weights (R2.9c; the large-batch case of PAPER.md:218-222, where one ciphertext holds one channel)
+    def weight_factor(self, wkey, Kw):
+        """(v, mkey) with weight_slots(wkey, Kw) == v * mask_slots(mkey), or None when the plaintext has more than one
+        valid channel position (then it is not a scalar times a 0/1 mask).  v = K[o, c, i, j]; mkey = (cpos, rows, cols)."""
+        _, _, _, _, _, i, j = wkey
+        cp, rows, cols = self._weight_factors(wkey)
+        if len(cp) != 1:
+            return None
+        cpos, o, c = cp[0]
+        return Kw[o, 0 if self.desc.depthwise else c, i, j], (cpos, tuple(rows), tuple(cols))
+
+    def mask_slots(self, mkey):
+        """0/1 slot vector of mask key (cpos, rows, cols): 1 at slot(cpos, bi*m + bj, b) for bi in rows, bj in cols, all b."""
+        cpos, rows, cols = mkey
+        L = self.lin
+        vec = np.zeros(self.n, dtype=np.float64)
+        for bi in rows:
+            for bj in cols:
+                base = L.slot(cpos, bi * L.m + bj, 0)
+                vec[base:base + L.B] = 1.0
+        return vec
+
+    def factorable(self):
+        """every weight plaintext of the layer is a scalar times a mask (true whenever ch = 1)"""
+        return all(len(self._weight_factors(wk)[0]) == 1 for diags in self.terms.values() for lst in diags.values() for _, _, wk in lst)
+
+    def run_factored(self, be, inputs, values, masks):
+        """The same graph with every weight plaintext replaced by its factors (R2.9c): per output and diagonal
+            P_d = sum over masks mu of  M_mu (*) ( sum over the terms t with mask mu of  v_t . R_t ),
+        v_t . R_t a scalar multiple of a (rotated) input, M_mu a mask plaintext.  values: {wkey: v}; masks: {mkey: M};
+        self.mask_of[wkey] = mkey (set by the caller through factor_weights)."""
+        R = {}
+        for src, amt in self.inner:
+            R[(src, amt)] = be.rot_in(inputs[src], amt)
+        out = {}
+        for okey, diags in self.terms.items():
+            y = None
+            for dd in sorted(diags):
+                by_mask = {}
+                for src, amt, wkey in diags[dd]:
+                    by_mask.setdefault(self.mask_of[wkey], []).append((src, amt, wkey))
+                acc = be.zero()
+                for mkey, lst in by_mask.items():
+                    S = be.zero_in()
+                    for src, amt, wkey in lst:
+                        S = be.scale_acc(S, R[(src, amt)] if amt else inputs[src], values[wkey])
+                    be.pmult_acc(acc, S, masks[mkey])
+                pd = be.wrap(acc)
+                if dd:
+                    pd = be.rot(pd, dd * self.lin.cs % self.n)
+                y = pd if y is None else be.add(y, pd)
+            out[okey] = y
+        return out
+
     # ---- exact counts of this graph (per batch group; multiply by BG for the layer)
     def counts(self):
         n_outer = 0
@@ -264,6 +318,12 @@ class SlotBackend:
 
     def add(self, x, y):
         return x + y
+
+    def zero_in(self):
+        return np.zeros(self.n)
+
+    def scale_acc(self, S, x, v):
+        return S + v * x
 
 
 def hconv_slots(desc: ConvDesc, n: int, X, Kw):
@@ -366,6 +426,15 @@ class CtBackend:
     def add(self, x, y):
         return self.ck.add(self.params, x, y)
 
+    # factored weights (R2.9c): S = sum_t round_half_up(v_t E1) . R_t at scale s_in E1, then acc += S (*) M with M at E2
+    def zero_in(self):
+        return None
+
+    def scale_acc(self, S, x, v):
+        assert x.scale == self.scale_in
+        t = self.ck.mul_const(self.params, x, v, self.E1)
+        return t if S is None else self.ck.add(self.params, S, t)
+
 
 def encode_weights(ck, params, graph: ConvGraph, Kw, L, scale_w=None):
     """Every non-zero weight plaintext of the graph, encoded at s_w (default q_{L-1}, A14) on L limbs."""
@@ -377,6 +446,66 @@ def encode_weights(ck, params, graph: ConvGraph, Kw, L, scale_w=None):
                 if wk not in W:
                     W[wk] = ck.encode(params, graph.weight_slots(wk, Kw), L, sw)
     return W
+
+
+def factor_scales(scale_w):
+    """(E1, E2) with E1 E2 = s_w and E1 = 2^ceil(log2(s_w) / 2): the split Delta_1 Delta_2 = Delta of PAPER.md:276, applied
+    to a weight value (E1) and the 0/1 validity mask it multiplies (E2), so the two products still cost one level."""
+    sw = Fraction(scale_w)
+    bits = 0
+    while Fraction(2) ** bits < sw:
+        bits += 1
+    E1 = Fraction(2) ** (-(-bits // 2))
+    return E1, sw / E1
+
+
+def factor_weights(ck, params, graph: ConvGraph, Kw, L, scale_w=None):
+    """R2.9c: every weight plaintext of a layer whose ciphertexts hold one channel each (ch = 1, the large-batch case of
+    PAPER.md:218-222) is a real value times a 0/1 mask; the value is kept as a real (rounded to the integer
+    round_half_up(v E1) when it multiplies a ciphertext, R2.8), the distinct masks are encoded at E2.
+    Returns (values {wkey: v}, masks {mkey: Plaintext}, E1); sets graph.mask_of."""
+    assert graph.factorable(), "a weight plaintext with several channel positions is not a scalar times a mask"
+    sw = Fraction(params.q[L - 1]) if scale_w is None else Fraction(scale_w)
+    E1, E2 = factor_scales(sw)
+    values, masks, graph.mask_of = {}, {}, {}
+    for diags in graph.terms.values():
+        for lst in diags.values():
+            for _, _, wk in lst:
+                if wk in values:
+                    continue
+                v, mk = graph.weight_factor(wk, Kw)
+                values[wk], graph.mask_of[wk] = float(v), mk
+                if mk not in masks:
+                    masks[mk] = ck.encode(params, graph.mask_slots(mk), L, E2)
+    return values, masks, E1
+
+
+def hconv_factored(ck, params, keys, graph: ConvGraph, inputs, values, masks, E1, do_rescale=True, hoist=False):
+    """hconv with factored weights (R2.9c): inputs {(u, v, g_in): Ciphertext} of one batch group."""
+    any_in = next(iter(inputs.values()))
+    any_m = next(iter(masks.values()))
+    be = CtBackend(ck, params, keys, any_in.L, any_in.scale, any_m.scale, hoist)
+    # the ciphertexts entering scale_acc are at the input scale; the sums S entering pmult_acc at s_in E1
+    be.E1, be.scale_S = Fraction(E1), any_in.scale * Fraction(E1)
+    outs = graph.run_factored(_FactoredView(be), inputs, values, masks)
+    if do_rescale:
+        outs = {k: (ck.rescale(params, y) if y is not None else None) for k, y in outs.items()}
+    return outs
+
+
+class _FactoredView:
+    """CtBackend seen from run_factored: PMult-accumulate takes the sums S (scale s_in E1) and the masks (scale E2)."""
+
+    def __init__(self, be):
+        self.be = be
+        self.rot, self.rot_in, self.zero, self.add, self.zero_in, self.scale_acc = be.rot, be.rot_in, be.zero, be.add, be.zero_in, be.scale_acc
+
+    def pmult_acc(self, acc, S, M):
+        assert S.scale == self.be.scale_S and M.scale == self.be.scale_w
+        self.be.ck.pmult_acc(self.be.params, acc, S, M)
+
+    def wrap(self, acc):
+        return self.be.ck.Ciphertext(acc, self.be.L, self.be.scale_S * self.be.scale_w)
 
 
 def hconv(ck, params, keys, graph: ConvGraph, inputs, weights, do_rescale=True, hoist=False):

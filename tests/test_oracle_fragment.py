@@ -8,6 +8,7 @@ import pytest
 
 from oracle import ckks as ck
 from oracle import fragment as fr
+import workloads as wl
 
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
 
@@ -220,3 +221,86 @@ def test_compress_fig5_shape(toy32):
     out = fr.compress(ck, P, keys, plan, srcs, mask_pt=mpt, do_rescale=True)[0]
     assert out.L == P.nq - 1 and out.scale == P.scale
     assert np.abs(ck.decrypt_decode(P, keys, out).real - exp).max() < 1e-3
+
+
+# --------------------------------------------------------------------------- factored weights (R2.9c)
+FACTORED_SHAPES = [
+    dict(BS=8, C_in=3, H=4, W=4, C_out=5, K=3, stride=1, pad=1),                    # n=128: m=4, B=8, ch=1
+    dict(BS=16, C_in=2, H=7, W=6, C_out=3, K=3, stride=2, pad=1),                   # frame 8 > data, stride 2 (S=2)
+    dict(BS=8, C_in=4, H=4, W=4, C_out=4, K=3, stride=1, pad=1, depthwise=True),
+    dict(BS=8, C_in=5, H=4, W=4, C_out=7, K=1, stride=1, pad=0),                    # point-wise
+    dict(BS=20, C_in=2, H=4, W=4, C_out=2, K=5, stride=1, pad=2),                   # BS not 2^k: 3 batch groups, last ragged
+]
+
+
+@pytest.mark.parametrize("kw", FACTORED_SHAPES)
+def test_factored_weights_identity_and_plain_slots(kw):
+    """R2.9c: (i) every weight plaintext of a ch = 1 layer equals value x mask exactly; (ii) the factored graph on plain slot
+    vectors (rotation = cyclic shift) reproduces direct convolution."""
+    n = 128
+    S = 2 if kw["stride"] == 2 else 1
+    d = fr.ConvDesc(S=S, **kw)
+    g = fr.ConvGraph(d, n)
+    assert g.lin.ch == 1 and g.factorable()
+    x, w = wl.conv_inputs(7, kw)
+    values, mask_of, masks = {}, {}, {}
+    for diags in g.terms.values():
+        for lst in diags.values():
+            for _, _, wk in lst:
+                v, mk = g.weight_factor(wk, w)
+                assert np.array_equal(v * g.mask_slots(mk), g.weight_slots(wk, w))
+                values[wk], mask_of[wk] = v, mk
+                masks[mk] = g.mask_slots(mk)
+    g.mask_of = mask_of
+    be = fr.SlotBackend(n)
+    Y = np.zeros((d.BS, d.C_out, d.H_out, d.W_out))
+    for bg in range(g.lin.BG):
+        ins = {(u, v, gi): g.lin.gather(x, u, v, gi, bg) for u in range(S) for v in range(S) for gi in range(g.lin.G)}
+        for (uo, vo, go), y in g.run_factored(be, ins, values, masks).items():
+            g.lout.scatter(Y, y, uo, vo, go, bg)
+    assert np.abs(Y - fr.direct_conv(d, x, w)).max() < 1e-12
+
+
+def test_factor_scales_split():
+    """E1 E2 = s_w exactly, E1 a power of two of half the bits (Delta_1 Delta_2 = Delta)."""
+    from fractions import Fraction
+    for sw in (1099511480321, 1125899906826241, 2 ** 40, 2 ** 25):
+        E1, E2 = fr.factor_scales(sw)
+        assert E1 * E2 == sw and E1 == Fraction(2) ** ((int(sw - 1).bit_length() + 1) // 2)
+
+
+def test_not_factorable_with_several_channel_positions():
+    g = fr.ConvGraph(fr.ConvDesc(S=1, BS=1, C_in=4, H=4, W=4, C_out=4, K=3, stride=1, pad=1), 128)
+    assert g.lin.ch > 1 and not g.factorable()
+
+
+@pytest.mark.parametrize("kw,hoist", [(FACTORED_SHAPES[0], False), (FACTORED_SHAPES[1], True), (FACTORED_SHAPES[3], False)])
+def test_factored_weights_encrypted_decodes_to_convolution(kw, hoist):
+    """R2.9c on ciphertexts: decrypt(hconv_factored) = direct convolution within 1e-3; same level and scale as the plain
+    form; the limbs differ from it (two roundings instead of one) while the decoded values agree to 1e-4."""
+    P = ck.Params(8, 4, 40, 2, 60, 2, 40)
+    L = P.nq
+    S = 2 if kw["stride"] == 2 else 1
+    d = fr.ConvDesc(S=S, **kw)
+    g = fr.ConvGraph(d, P.n)
+    x, w = wl.conv_inputs(8, kw)
+    keys = ck.keygen(P, 3, g.counts()["rot_steps"])
+    values, masks, E1 = fr.factor_weights(ck, P, g, w, L)
+    E2 = next(iter(masks.values())).scale
+    assert E1 * E2 == P.q[L - 1] and E1 == 2 ** 20
+    W = fr.encode_weights(ck, P, g, w, L)
+    Yf = np.zeros((d.BS, d.C_out, d.H_out, d.W_out))
+    Yp = np.zeros_like(Yf)
+    differ = False
+    for bg in range(g.lin.BG):
+        ins = {(u, v, gi): ck.encrypt(P, keys, ck.encode(P, g.lin.gather(x, u, v, gi, bg), L), 100 + 16 * bg + 4 * gi + 2 * u + v)
+               for u in range(S) for v in range(S) for gi in range(g.lin.G)}
+        of = fr.hconv_factored(ck, P, keys, g, ins, values, masks, E1, hoist=hoist)
+        op = fr.hconv(ck, P, keys, g, ins, W, hoist=hoist)
+        for k in of:
+            assert of[k].L == op[k].L == L - 1 and of[k].scale == op[k].scale == P.scale
+            differ = differ or not np.array_equal(of[k].c, op[k].c)
+            g.lout.scatter(Yf, ck.decrypt_decode(P, keys, of[k]).real, *k, bg)
+            g.lout.scatter(Yp, ck.decrypt_decode(P, keys, op[k]).real, *k, bg)
+    want = fr.direct_conv(d, x, w)
+    assert np.abs(Yf - want).max() < 1e-3 and np.abs(Yf - Yp).max() < 1e-4 and differ
