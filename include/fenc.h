@@ -199,6 +199,31 @@ fenc_status fenc_conv_weights_from_coeffs(fenc_ctx *ctx, const fenc_conv_desc *c
                                           const int64_t *coeffs, size_t n, uint32_t n_limbs, double scale,
                                           fenc_wts **out);
 void fenc_wts_free(fenc_wts *w);
+/* ---- factored weights for the large-batch case (R2.9c; "Special Case: Large Batch", and the
+ * scale split Delta_1 Delta_2 = Delta of PAPER.md:276).  When a ciphertext holds ONE channel (layout ch = 1, or any layer
+ * whose weight plaintexts have a single valid channel position) every weight plaintext is a real value v times a 0/1
+ * validity mask mu (zero padding, frame padding, stride).  The factored form stores per weight only the integer
+ * k = round_half_up(v E1) (one residue per limb) and per DISTINCT mask one plaintext M = encode(mu, E2), E1 E2 = s_w
+ * (default s_w = q_{L-1}, E1 = 2^ceil(log2(s_w)/2)), and fenc_hconv evaluates per output and diagonal
+ *   P_d = sum_mu M_mu (*) ( sum_{terms t with mask mu} k_t . R_t ):
+ * scalar multiply-accumulates of (rotated) input ciphertexts, then one plaintext product per mask.  Same level use and
+ * output scale as the plain form; the limbs differ from it (compare with the oracle's hconv_factored).  A layer of C_out x
+ * C_in x K^2 weights then needs C_out C_in K^2 L words instead of that many plaintexts of L N words.
+ * fenc_wts_factors: mask id of every weight in fenc_wts_keys order (ids in order of first appearance) and the number of
+ * distinct masks; FENC_ERR_LAYOUT when some weight plaintext has several valid channel positions.
+ * fenc_wts_mask_slots: the 0/1 slot vector of one mask, host slots[N/2]. */
+fenc_status fenc_wts_factors(fenc_ctx *ctx, const fenc_conv_desc *conv, const fenc_layout *layout, uint32_t *mask_of,
+                             size_t capacity, size_t *n, size_t *n_masks);
+fenc_status fenc_wts_mask_slots(fenc_ctx *ctx, const fenc_conv_desc *conv, const fenc_layout *layout, uint32_t mask_id,
+                                double *slots);
+/* host w[C_out][C_in or 1][K][K]; scale <= 0: s_w = q_{L-1} (A14) */
+fenc_status fenc_conv_weights_factored(fenc_ctx *ctx, const fenc_conv_desc *conv, const fenc_layout *layout, const double *w,
+                                       uint32_t n_limbs, double scale, fenc_wts **out);
+/* the same from integers (A7: parity starts at integer coefficients): host k[n] = the multipliers round_half_up(v E1) in
+ * fenc_wts_keys order, host mask_coeffs[n_masks][N] = centred coefficients of the masks encoded at E2, in mask-id order */
+fenc_status fenc_conv_weights_factored_from_ints(fenc_ctx *ctx, const fenc_conv_desc *conv, const fenc_layout *layout,
+                                                 const int64_t *k, size_t n, const int64_t *mask_coeffs, size_t n_masks,
+                                                 uint32_t n_limbs, double E1, double E2, fenc_wts **out);
 /* One fragment-encoded conv layer over ALL batch groups.  in: n_in = S^2 G_in BG ciphertexts ordered
  * [bg][g][u][v]; out: n_out = S_out^2 G_out BG ciphertexts ordered [bg][g_out][u_o][v_o].  Inner rotations
  * (batched), MAC, outer rotations (batched), one rescale per output ciphertext when do_rescale != 0 (A13). */

@@ -65,7 +65,8 @@ SYMBOLS = ["fenc_params_init", "fenc_ctx_free", "fenc_last_error", "fenc_get_pri
            "fenc_profile_enable", "fenc_profile_kernels", "fenc_profile_name", "fenc_profile_read", "fenc_fc_plan",
            "fenc_fc_wts_keys", "fenc_fc_weights", "fenc_fc_weights_from_coeffs", "fenc_fc", "fenc_measure_alu_peak",
            "fenc_cmult_relin", "fenc_mul_scalar", "fenc_add_const", "fenc_ct_import_async", "fenc_ct_export_async",
-           "fenc_export_wait", "fenc_set_hoisting", "fenc_rotate_hoisted", "fenc_square_sum_relin"]
+           "fenc_export_wait", "fenc_set_hoisting", "fenc_rotate_hoisted", "fenc_square_sum_relin",
+           "fenc_wts_factors", "fenc_wts_mask_slots", "fenc_conv_weights_factored", "fenc_conv_weights_factored_from_ints"]
 
 _lib = None
 
@@ -123,6 +124,11 @@ def load_library(path=None):
                                           C.c_double, vpp],
         "fenc_hconv": [vp, vp, C.POINTER(ConvDesc), C.POINTER(Layout), vp, vpp, C.c_size_t, C.c_int, vpp, C.c_size_t,
                        C.POINTER(C.c_size_t)],
+        "fenc_wts_factors": [vp, C.POINTER(ConvDesc), C.POINTER(Layout), u32p, C.c_size_t, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)],
+        "fenc_wts_mask_slots": [vp, C.POINTER(ConvDesc), C.POINTER(Layout), C.c_uint32, dp],
+        "fenc_conv_weights_factored": [vp, C.POINTER(ConvDesc), C.POINTER(Layout), dp, C.c_uint32, C.c_double, vpp],
+        "fenc_conv_weights_factored_from_ints": [vp, C.POINTER(ConvDesc), C.POINTER(Layout), i64p, C.c_size_t, i64p, C.c_size_t,
+                                                 C.c_uint32, C.c_double, C.c_double, vpp],
         "fenc_fc_plan": [vp, C.POINTER(FcDesc), C.POINTER(FcInfo)],
         "fenc_fc_wts_keys": [vp, C.POINTER(FcDesc), u32p, C.c_size_t, C.POINTER(C.c_size_t)],
         "fenc_fc_weights": [vp, C.POINTER(FcDesc), dp, C.c_uint32, C.c_double, vpp],
@@ -505,6 +511,35 @@ class Context:
         h = C.c_void_p()
         self._ck(self.lib.fenc_conv_weights_from_coeffs(self.h, C.byref(conv), C.byref(lay), _ptr(c, C.c_int64), c.shape[0],
                                                         n_limbs, float(scale), C.byref(h)))
+        return Weights(self, h)
+
+    # ---- factored weights (R2.9c)
+    def wts_factors(self, conv, lay):
+        """(mask id of every weight in wts_keys order, number of distinct masks)"""
+        n, nm = C.c_size_t(), C.c_size_t()
+        self._ck(self.lib.fenc_wts_factors(self.h, C.byref(conv), C.byref(lay), None, 0, C.byref(n), C.byref(nm)))
+        m = np.zeros(n.value, dtype=np.uint32)
+        self._ck(self.lib.fenc_wts_factors(self.h, C.byref(conv), C.byref(lay), _ptr(m, C.c_uint32), n.value, C.byref(n), C.byref(nm)))
+        return m, nm.value
+
+    def wts_mask_slots(self, conv, lay, mask_id):
+        v = np.zeros(self.n, dtype=np.float64)
+        self._ck(self.lib.fenc_wts_mask_slots(self.h, C.byref(conv), C.byref(lay), int(mask_id), _ptr(v, C.c_double)))
+        return v
+
+    def conv_weights_factored(self, conv, lay, w, n_limbs, scale=0.0):
+        w = np.ascontiguousarray(w, dtype=np.float64)
+        h = C.c_void_p()
+        self._ck(self.lib.fenc_conv_weights_factored(self.h, C.byref(conv), C.byref(lay), _ptr(w, C.c_double), n_limbs, float(scale), C.byref(h)))
+        return Weights(self, h)
+
+    def conv_weights_factored_from_ints(self, conv, lay, k, mask_coeffs, n_limbs, E1, E2):
+        k = np.ascontiguousarray(k, dtype=np.int64)
+        mc = np.ascontiguousarray(mask_coeffs, dtype=np.int64)
+        assert mc.ndim == 2 and mc.shape[1] == self.N
+        h = C.c_void_p()
+        self._ck(self.lib.fenc_conv_weights_factored_from_ints(self.h, C.byref(conv), C.byref(lay), _ptr(k, C.c_int64), k.shape[0],
+                                                               _ptr(mc, C.c_int64), mc.shape[0], n_limbs, float(E1), float(E2), C.byref(h)))
         return Weights(self, h)
 
     def hconv(self, keys, conv, lay, wts, cts, do_rescale=True):

@@ -6,6 +6,7 @@
 #include <functional>
 #include <map>
 #include <set>
+#include <tuple>
 
 #include "fenc_ctx.h"
 
@@ -38,6 +39,42 @@ struct ConvGraph : LinGraph {              // outs index: (g_out * S_out + u_o) 
   fenc_conv_desc d;
   int n, M, S, S_out, m, B, ch, cs, G_in, G_out, H_out, W_out;
   std::vector<std::array<u32, 7>> wkeys;      // (u_o, v_o, g_out, g_in, d, i, j) per weight plaintext
+  // factored form (R2.9c), built on first use: a weight plaintext with ONE valid channel position is value x mask
+  struct Mask { int cpos; std::vector<int> rows, cols; };
+  bool factors_built = false, factorable = false;
+  std::vector<int> mask_of;                   // weight index -> mask id (first-appearance order)
+  std::vector<Mask> masks;
+  void build_factors() {
+    if (factors_built) return;
+    factors_built = true, factorable = true;
+    std::map<std::tuple<int, std::vector<int>, std::vector<int>>, int> seen;
+    mask_of.assign(wkeys.size(), -1);
+    for (size_t w = 0; w < wkeys.size(); w++) {
+      const auto &wk = wkeys[w];
+      auto cp = valid_cpos(wk[2], wk[3], wk[4]);
+      if (cp.size() != 1) { factorable = false; mask_of.clear(); masks.clear(); return; }
+      auto key = std::make_tuple(cp[0][0], valid_blocks(wk[0], wk[5], d.H, H_out), valid_blocks(wk[1], wk[6], d.W, W_out));
+      auto it = seen.find(key);
+      if (it == seen.end()) {
+        it = seen.emplace(key, (int)masks.size()).first;
+        masks.push_back(Mask{std::get<0>(key), std::get<1>(key), std::get<2>(key)});
+      }
+      mask_of[w] = it->second;
+    }
+  }
+  double weight_value(const std::array<u32, 7> &wk, const double *w) const {  // the single valid channel position's K[o][c][i][j]
+    auto cp = valid_cpos(wk[2], wk[3], wk[4]);
+    const int K = d.K, Cw = d.depthwise ? 1 : (int)d.C_in;
+    return w[(((size_t)cp[0][1] * Cw + (d.depthwise ? 0 : cp[0][2])) * K + wk[5]) * K + wk[6]];
+  }
+  void mask_slots(const Mask &mk, std::vector<double> &vec) const {
+    vec.assign(n, 0.0);
+    for (int bi : mk.rows)
+      for (int bj : mk.cols) {
+        size_t base = (size_t)mk.cpos * cs + (size_t)(bi * m + bj) * B;
+        for (int b = 0; b < B; b++) vec[base + b] = 1.0;
+      }
+  }
   // R2.9 step 2: the validity conditions factorise into channel positions, block rows and block columns
   std::vector<std::array<int, 3>> valid_cpos(int go, int gi, int dd) const {
     std::vector<std::array<int, 3>> v;
@@ -354,7 +391,115 @@ extern "C" void fenc_wts_free(fenc_wts *W) {
   if (!W) return;
   cudaStreamSynchronize(W->ctx->stream);
   dfree(W->ctx, W->d_all);
+  dfree(W->ctx, W->d_k);
   delete W;
+}
+
+// ------------------------------------------------------------------------------------------------ factored weights (R2.9c)
+extern "C" fenc_status fenc_wts_factors(fenc_ctx *ctx, const fenc_conv_desc *cd, const fenc_layout *lay, uint32_t *mask_of, size_t capacity,
+                                        size_t *n, size_t *n_masks) {
+  if (!ctx || !cd || !n || !n_masks) return FENC_ERR_INVALID_ARG;
+  std::shared_ptr<ConvGraph> g;
+  fenc_status st = graph_for(ctx, cd, lay, g);
+  if (st != FENC_OK) return st;
+  g->build_factors();
+  if (!g->factorable) return fail(ctx, FENC_ERR_LAYOUT, "a weight plaintext has several valid channel positions (ch = %d): not value x mask", g->ch);
+  *n = g->wkeys.size(), *n_masks = g->masks.size();
+  if (mask_of) {
+    if (capacity < g->wkeys.size()) return fail(ctx, FENC_ERR_INVALID_ARG, "capacity %zu < %zu weights", capacity, g->wkeys.size());
+    for (size_t i = 0; i < g->wkeys.size(); i++) mask_of[i] = (uint32_t)g->mask_of[i];
+  }
+  return FENC_OK;
+}
+extern "C" fenc_status fenc_wts_mask_slots(fenc_ctx *ctx, const fenc_conv_desc *cd, const fenc_layout *lay, uint32_t mask_id, double *slots) {
+  if (!ctx || !cd || !slots) return FENC_ERR_INVALID_ARG;
+  std::shared_ptr<ConvGraph> g;
+  fenc_status st = graph_for(ctx, cd, lay, g);
+  if (st != FENC_OK) return st;
+  g->build_factors();
+  if (!g->factorable || mask_id >= g->masks.size()) return fail(ctx, FENC_ERR_LAYOUT, "no such mask");
+  std::vector<double> v;
+  g->mask_slots(g->masks[mask_id], v);
+  memcpy(slots, v.data(), v.size() * sizeof(double));
+  return FENC_OK;
+}
+// k[n]: integer multipliers; mask coefficient vectors either given (parity path) or encoded here at E2
+static fenc_status make_factored(fenc_ctx *ctx, ConvGraph &g, const int64_t *k, const int64_t *mask_coeffs, uint32_t n_limbs, double E1,
+                                 double E2, fenc_wts **out) {
+  if (n_limbs < 1 || (int)n_limbs > ctx->nq) return FENC_ERR_INVALID_ARG;
+  const int L = n_limbs;
+  const size_t N = ctx->N, n = g.wkeys.size(), nm = g.masks.size();
+  std::unique_ptr<fenc_wts, void (*)(fenc_wts *)> W(new fenc_wts{ctx, L, E1 * E2, n}, fenc_wts_free);
+  W->factored = true, W->n_unique = nm, W->slot = g.mask_of;
+  W->k_fp64 = true;
+  for (int t = 0; t < L; t++) W->k_fp64 = W->k_fp64 && fh::f64_modulus(ctx->mod[t], ctx->logN);
+  W->d_all = dalloc_t<u64>(ctx, nm * L * N);
+  W->d_k = dalloc_t<ShoupC>(ctx, n * L);
+  if (!W->d_all || !W->d_k) return fail(ctx, FENC_ERR_OOM, "factored weights (%zu masks, %zu scalars)", nm, n);
+  std::vector<double> vec;
+  std::vector<int64_t> c(N);
+  for (size_t i = 0; i < nm; i++) {
+    const int64_t *src = mask_coeffs ? mask_coeffs + i * N : c.data();
+    if (!mask_coeffs) {
+      g.mask_slots(g.masks[i], vec);
+      fh::encode_slots(ctx->logN, vec.data(), nullptr, E2, c.data());
+    }
+    fenc_status st = coeffs_to_mont(ctx, src, L, W->d_all + i * L * N);
+    if (st != FENC_OK) return st;
+    if (cudaStreamSynchronize(ctx->stream) != cudaSuccess) return FENC_ERR_CUDA;  // c is reused
+  }
+  std::vector<ShoupC> kp(n * L);
+  for (size_t i = 0; i < n; i++)
+    for (int t = 0; t < L; t++) {
+      const u64 q = ctx->mod[t];
+      const u64 mag = (u64)(k[i] < 0 ? -k[i] : k[i]) % q;
+      const u64 r = (k[i] < 0 && mag) ? q - mag : mag;
+      kp[i * L + t] = W->k_fp64 ? ShoupC{fh::double_bits((double)r), fh::double_bits((double)((long double)r / (long double)q))}
+                                : ShoupC{fh::to_mont(r, q), 0};
+    }
+  if (cudaMemcpyAsync(W->d_k, kp.data(), kp.size() * sizeof(ShoupC), cudaMemcpyHostToDevice, ctx->stream) != cudaSuccess ||
+      cudaStreamSynchronize(ctx->stream) != cudaSuccess)
+    return FENC_ERR_CUDA;
+  *out = W.release();
+  return FENC_OK;
+}
+// (E1, E2) with E1 E2 = s_w, E1 = 2^ceil(log2(s_w)/2)
+static void factor_scales(double sw, double *E1, double *E2) {
+  int bits = 0;
+  while (std::ldexp(1.0, bits) < sw) bits++;
+  *E1 = std::ldexp(1.0, (bits + 1) / 2);
+  *E2 = sw / *E1;  // exact: a division by a power of two
+}
+extern "C" fenc_status fenc_conv_weights_factored(fenc_ctx *ctx, const fenc_conv_desc *cd, const fenc_layout *lay, const double *w,
+                                                  uint32_t n_limbs, double scale, fenc_wts **out) {
+  if (!ctx || !cd || !w || !out || n_limbs < 1 || (int)n_limbs > ctx->nq) return FENC_ERR_INVALID_ARG;
+  std::shared_ptr<ConvGraph> g;
+  fenc_status st = graph_for(ctx, cd, lay, g);
+  if (st != FENC_OK) return st;
+  g->build_factors();
+  if (!g->factorable) return fail(ctx, FENC_ERR_LAYOUT, "a weight plaintext has several valid channel positions (ch = %d): not value x mask", g->ch);
+  double E1, E2;
+  factor_scales(scale > 0 ? scale : (double)ctx->mod[n_limbs - 1], &E1, &E2);
+  std::vector<int64_t> k(g->wkeys.size());
+  for (size_t i = 0; i < k.size(); i++) {
+    // round_half_up(v E1): v E1 is exact (E1 a power of two), its floor and fractional part are exact doubles
+    const double a = g->weight_value(g->wkeys[i], w) * E1, f = std::floor(a);
+    k[i] = (int64_t)f + ((a - f) >= 0.5 ? 1 : 0);
+  }
+  return make_factored(ctx, *g, k.data(), nullptr, n_limbs, E1, E2, out);
+}
+extern "C" fenc_status fenc_conv_weights_factored_from_ints(fenc_ctx *ctx, const fenc_conv_desc *cd, const fenc_layout *lay,
+                                                            const int64_t *k, size_t n, const int64_t *mask_coeffs, size_t n_masks,
+                                                            uint32_t n_limbs, double E1, double E2, fenc_wts **out) {
+  if (!ctx || !cd || !k || !mask_coeffs || !out || !(E1 > 0) || !(E2 > 0)) return FENC_ERR_INVALID_ARG;
+  std::shared_ptr<ConvGraph> g;
+  fenc_status st = graph_for(ctx, cd, lay, g);
+  if (st != FENC_OK) return st;
+  g->build_factors();
+  if (!g->factorable) return fail(ctx, FENC_ERR_LAYOUT, "a weight plaintext has several valid channel positions (ch = %d): not value x mask", g->ch);
+  if (n != g->wkeys.size() || n_masks != g->masks.size())
+    return fail(ctx, FENC_ERR_MISMATCH, "expected %zu multipliers and %zu masks, got %zu and %zu", g->wkeys.size(), g->masks.size(), n, n_masks);
+  return make_factored(ctx, *g, k, mask_coeffs, n_limbs, E1, E2, out);
 }
 
 // ------------------------------------------------------------------------------------------------ HConv (R2.9)
@@ -404,20 +549,21 @@ static fenc_status run_linear(fenc_ctx *ctx, const fenc_keys *K, const LinGraph 
   // ---- 2. MAC over every (bg, output, diagonal)
   size_t n_P = 0, n_rot_out = 0;
   for (auto &oc : g.outs) {
-    n_P += oc.diags.size();
+    if (!(oc.diags.size() == 1 && oc.diags[0] == 0)) n_P += oc.diags.size();  // a lone diagonal 0 is summed in place
     for (int d : oc.diags) n_rot_out += d != 0;
   }
   std::vector<fenc_ct *> res(nout_bg * BG, nullptr);
   const double s_acc = s_in * W->scale;
   u64 *Ybuf = do_rescale ? sc.alloc<u64>(nout_bg * BG * CT) : nullptr;  // pre-rescale sums
-  u64 *Pbuf = sc.alloc<u64>(n_P * BG * CT);                               // diagonal partial sums (worst case)
+  u64 *Pbuf = n_P ? sc.alloc<u64>(n_P * BG * CT) : nullptr;               // diagonal partial sums
   u64 *Obuf = n_rot_out ? sc.alloc<u64>(n_rot_out * BG * CT) : nullptr;   // outer-rotation results
-  if ((do_rescale && !Ybuf) || !Pbuf || (n_rot_out && !Obuf)) return fail(ctx, FENC_ERR_OOM, "hconv partial sums");
+  if ((do_rescale && !Ybuf) || (n_P && !Pbuf) || (n_rot_out && !Obuf)) return fail(ctx, FENC_ERR_OOM, "hconv partial sums");
   for (size_t i = 0; i < res.size(); i++) {
     res[i] = sc.ct(do_rescale ? L - 1 : L, do_rescale ? s_acc / (double)ctx->mod[L - 1] : s_acc);
     if (!res[i]) return fail(ctx, FENC_ERR_OOM, "hconv outputs");
   }
   MacJob job;
+  SmacJob sjob;  // factored weights (R2.9c): scalar multiply-accumulates, one plaintext product per mask
   std::vector<const u64 *> rot_in, sum_terms;
   std::vector<u64 *> rot_out, sum_out;
   std::vector<int> rot_step, sum_start{0};
@@ -429,11 +575,17 @@ static fenc_status run_linear(fenc_ctx *ctx, const fenc_keys *K, const LinGraph 
       const bool single = oc.diags.size() == 1 && oc.diags[0] == 0;
       for (size_t k = 0; k < oc.diags.size(); k++) {
         u64 *P = single ? Y : Pbuf + (pi++) * CT;
-        job.terms.emplace_back();
-        for (const Term &t : oc.terms[k])
-          job.terms.back().push_back({t.amt ? Rbuf + (bg * n_inner + g.inner_index.at({t.src, t.amt})) * CT : in[bg * nin_bg + t.src]->d,
-                                      W->d_all + (size_t)W->slot[t.w] * L * N});
-        job.outs.push_back(P);
+        auto ct_of = [&](const Term &t) { return t.amt ? Rbuf + (bg * n_inner + g.inner_index.at({t.src, t.amt})) * CT : in[bg * nin_bg + t.src]->d; };
+        if (W->factored) {
+          sjob.terms.emplace_back();
+          for (const Term &t : oc.terms[k]) sjob.terms.back().push_back({ct_of(t), t.w, W->d_all + (size_t)W->slot[t.w] * L * N});
+          std::stable_sort(sjob.terms.back().begin(), sjob.terms.back().end(), [](const SmacTerm &a, const SmacTerm &b) { return a.mask < b.mask; });
+          sjob.outs.push_back(P);
+        } else {
+          job.terms.emplace_back();
+          for (const Term &t : oc.terms[k]) job.terms.back().push_back({ct_of(t), W->d_all + (size_t)W->slot[t.w] * L * N});
+          job.outs.push_back(P);
+        }
         if (single) continue;
         if (oc.diags[k] == 0) sum_terms.push_back(P);
         else {
@@ -444,7 +596,7 @@ static fenc_status run_linear(fenc_ctx *ctx, const fenc_keys *K, const LinGraph 
       }
       if (!single) sum_start.push_back((int)sum_terms.size()), sum_out.push_back(Y);
     }
-  st = run_mac(ctx, job, L);
+  st = W->factored ? run_smac(ctx, sjob, W, L) : run_mac(ctx, job, L);
   if (st != FENC_OK) return st;
   // ---- 3. outer rotations, 4. sums
   st = rotate_raw(ctx, K, L, rot_in, rot_step, rot_out);

@@ -132,6 +132,10 @@ struct fenc_wts {
   size_t n_unique = 0;
   std::vector<int> slot;  // weight index (fenc_wts_keys order) -> storage slot; identical plaintexts share one
   u64 *d_all = nullptr;  // [n_unique][L][N] NTT domain, Montgomery form
+  // factored form (R2.9c): d_all holds the n_unique distinct MASK plaintexts, slot[i] the mask of weight i, and
+  // d_k the per-weight integer multipliers, [n][L] 16-byte entries (fenc_internal.h k_smac)
+  bool factored = false, k_fp64 = false;
+  ShoupC *d_k = nullptr;
 };
 
 // ---------------------------------------------------------------- helpers (fenc_ctx.cu)
@@ -227,5 +231,16 @@ struct MacJob {
   std::vector<u64 *> outs;
 };
 fenc_status run_mac(fenc_ctx *ctx, const MacJob &job, int L);
+// the same for factored weights: per output a list of (ciphertext, weight index, mask plaintext), mask-major
+struct SmacTerm {
+  const u64 *ct;
+  int w;
+  const u64 *mask;
+};
+struct SmacJob {
+  std::vector<std::vector<SmacTerm>> terms;  // per output, sorted so that equal masks are consecutive
+  std::vector<u64 *> outs;
+};
+fenc_status run_smac(fenc_ctx *ctx, const SmacJob &job, const fenc_wts *W, int L);
 double mac_alg_bytes(fenc_ctx *ctx, const std::vector<const u64 *> &tc, const std::vector<const u64 *> &tp, size_t n_out, int L);
 fenc_status coeffs_to_mont(fenc_ctx *ctx, const int64_t *coeffs_host, int L, u64 *d_out);

@@ -191,6 +191,136 @@ int k_mac(const KCtx &k, const MacGroup *groups, int n_groups, int max_group, co
   return 0;
 }
 
+// ------------------------------------------------------------------------------------------------ scalar MAC (factored weights, R2.9c)
+// out_i = sum over mask segments s of  M_s (*) ( sum_{t in s} k_{i,t} . ct_t ),  k an integer scalar per (weight, limb).
+// A group = up to G outputs reading one ciphertext sequence with one segmentation (the output channels of one fragment):
+// each ciphertext word is loaded once and multiplied into G x 2 accumulators -- a register-tiled modular GEMM whose
+// "weights" are L words per scalar instead of L N words per plaintext.  The scalars of the block's limb are staged in
+// shared memory (a block never straddles limbs), the products run on the FP64 pipe when every modulus in use is below
+// 2^50: t = x k - rint(x k / q) q is an exact integer in (-q, q) (fenc_device.cuh mulmod_dd, |x| < 2^51), a sum of
+// floor(2^53 / q) - 1 of them plus a reduced remainder (at most q/2 + 1 in magnitude) is exact in a double, then
+// v - rint(v / q) q brings it back.  Integer mode (larger moduli): 128-bit lazy sums of x k_mont as in the plaintext MAC.
+struct SmacP {
+  const SmacGroup *groups; const u64 *const *term_ct; const int *kidx; const ShoupC *kpair; const int *seg_end;
+  const u64 *const *seg_mask; u64 *const *outs; const ModConst *mods; int L, logN, max_lazy;
+};
+#define SMAC_TILE 64
+template <int G, bool F64>
+__global__ void __launch_bounds__(256, G >= 8 ? 2 : 3) smac_kernel(SmacP p) {
+  __shared__ const u64 *s_ct[SMAC_TILE];
+  __shared__ ulonglong2 s_k[G][SMAC_TILE];
+  const size_t LN = (size_t)p.L << p.logN;
+  const size_t idx = (size_t)blockIdx.y * blockDim.x + threadIdx.x;  // blockDim divides N: idx < L N, one limb per block
+  const int limb = (int)(((size_t)blockIdx.y * blockDim.x) >> p.logN);
+  const SmacGroup g = p.groups[blockIdx.x];
+  const ModConst mc = p.mods[limb];
+  const F64Mod fm = f64mod(mc.q, mc.f64);
+  double acc[G][2];
+  u64 lo[F64 ? 1 : G][2], hi[F64 ? 1 : G][2], tot[G][2];
+#pragma unroll
+  for (int i = 0; i < G; i++) {
+    acc[i][0] = acc[i][1] = 0.0, tot[i][0] = tot[i][1] = 0;
+    if (!F64) lo[i][0] = lo[i][1] = hi[i][0] = hi[i][1] = 0;
+  }
+  int seg = 0, cur_end = p.seg_end[g.seg_start], lazy = 0;
+  for (int t0 = 0; t0 < g.n_terms; t0 += SMAC_TILE) {
+    const int nt = g.n_terms - t0 < SMAC_TILE ? g.n_terms - t0 : SMAC_TILE;
+    __syncthreads();
+    for (int j = threadIdx.x; j < nt * (G + 1); j += blockDim.x) {
+      const int i = j / nt, t = j - i * nt;
+      if (i == 0) s_ct[t] = p.term_ct[g.ct_start + t0 + t];
+      else {
+        const int o = i - 1 < g.n_out ? i - 1 : 0;  // unused lanes of a short group repeat output 0 (never stored)
+        const int w = p.kidx[g.k_start + o * g.n_terms + t0 + t];
+        s_k[i - 1][t] = __ldg(reinterpret_cast<const ulonglong2 *>(p.kpair) + (size_t)w * p.L + limb);
+      }
+    }
+    __syncthreads();
+#pragma unroll 2
+    for (int t = 0; t < nt; t++) {
+      const u64 *c = s_ct[t];
+      const u64 x0 = __ldg(c + idx), x1 = __ldg(c + LN + idx);
+      if (F64) {
+        const double xd0 = u2d52(x0), xd1 = u2d52(x1);
+#pragma unroll
+        for (int i = 0; i < G; i++) {
+          const ulonglong2 kk = s_k[i][t];
+          const double kd = __longlong_as_double((long long)kk.x), kq = __longlong_as_double((long long)kk.y);
+          acc[i][0] = __dadd_rn(acc[i][0], mulmod_dd(xd0, kd, kq, fm));
+          acc[i][1] = __dadd_rn(acc[i][1], mulmod_dd(xd1, kd, kq, fm));
+        }
+        if (++lazy == p.max_lazy) {
+#pragma unroll
+          for (int i = 0; i < G; i++) acc[i][0] = reduce_dd(acc[i][0], fm), acc[i][1] = reduce_dd(acc[i][1], fm);
+          lazy = 1;  // the reduced remainder counts as one term
+        }
+      } else {
+#pragma unroll
+        for (int i = 0; i < G; i++) {
+          const u64 km = s_k[i][t].x;
+          mac128(lo[i][0], hi[i][0], x0, km), mac128(lo[i][1], hi[i][1], x1, km);
+        }
+        if (++lazy == p.max_lazy) {
+          // fold: (S 2^-64 mod q) 2^128 2^-64 = S mod q, a residue below q, becomes the pending sum
+#pragma unroll
+          for (int i = 0; i < G; i++)
+#pragma unroll
+            for (int cpn = 0; cpn < 2; cpn++)
+              lo[i][cpn] = mont_mul(mont_redc(lo[i][cpn], hi[i][cpn], mc.q, mc.qinv_neg), mc.r2, mc.q, mc.qinv_neg), hi[i][cpn] = 0;
+          lazy = 1;
+        }
+      }
+      if (t0 + t + 1 == cur_end) {  // end of a mask segment (uniform over the block): tot += M (*) S
+        const u64 m = __ldg(p.seg_mask[g.seg_start + seg] + idx);
+#pragma unroll
+        for (int i = 0; i < G; i++)
+#pragma unroll
+          for (int cpn = 0; cpn < 2; cpn++) {
+            u64 S;
+            if (F64) {
+              S = csub(d2u_off(reduce_dd(acc[i][cpn], fm), fm.q + 4503599627370496.0), mc.q);
+              acc[i][cpn] = 0.0;
+            } else {
+              S = mont_redc(lo[i][cpn], hi[i][cpn], mc.q, mc.qinv_neg);
+              lo[i][cpn] = hi[i][cpn] = 0;
+            }
+            tot[i][cpn] = addmod(tot[i][cpn], mont_mul(S, m, mc.q, mc.qinv_neg), mc.q);
+          }
+        lazy = 0;
+        seg++;
+        cur_end = seg < g.n_seg ? p.seg_end[g.seg_start + seg] : -1;
+      }
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < G; i++)
+    if (i < g.n_out) {
+      u64 *out = p.outs[g.out_start + i];
+      out[idx] = tot[i][0];
+      out[LN + idx] = tot[i][1];
+    }
+}
+template <bool F64>
+static void launch_smac(const SmacP &p, dim3 grid, int nth, cudaStream_t st, int max_group) {
+  if (max_group <= 1) smac_kernel<1, F64><<<grid, nth, 0, st>>>(p);
+  else if (max_group <= 2) smac_kernel<2, F64><<<grid, nth, 0, st>>>(p);
+  else if (max_group <= 4) smac_kernel<4, F64><<<grid, nth, 0, st>>>(p);
+  else smac_kernel<FENC_SMAC_GROUP, F64><<<grid, nth, 0, st>>>(p);
+}
+int k_smac(const KCtx &k, const SmacGroup *groups, int n_groups, int max_group, const u64 *const *term_ct, const int *kidx,
+           const ShoupC *kpair, const int *seg_end, const u64 *const *seg_mask, u64 *const *outs, int L, bool fp64_mode,
+           int max_lazy, double alg_bytes) {
+  if (n_groups == 0) return 0;
+  SmacP p{groups, term_ct, kidx, kpair, seg_end, seg_mask, outs, k.d_mods, L, k.geom.logN, max_lazy < 2 ? 2 : max_lazy};
+  const int nth = k.N < 256 ? k.N : 256;
+  dim3 grid(n_groups, (unsigned)(((size_t)L * k.N) / nth));
+  PROF(k, K_SMAC, alg_bytes);
+  if (fp64_mode) launch_smac<true>(p, grid, nth, S(k), max_group);
+  else launch_smac<false>(p, grid, nth, S(k), max_group);
+  LAUNCH_CHECK(k);
+  return 0;
+}
+
 // ------------------------------------------------------------------------------------------------ sum of ciphertexts
 struct AddManyP { const u64 *const *term; const int *start; u64 *const *outs; const ModConst *mods; int L, logN; };
 __global__ void __launch_bounds__(256) add_many_kernel(AddManyP p) {

@@ -75,7 +75,7 @@ struct NttGeom {
 // per-kernel-class timing with CUDA events on the launching stream (measurement only; off by default)
 enum KernelId {
   K_INTT_ROW, K_INTT_COL, K_NTT_COL, K_NTT_COL_BCONV, K_NTT_ROW, K_KEYMAC, K_DIVIDE, K_MAC, K_ADD_MANY, K_ROWOP, K_SAMPLE,
-  K_COUNT
+  K_SMAC, K_COUNT
 };
 struct Prof;
 void prof_begin(Prof *p, void *stream, int id, double alg_bytes, double alg_butterflies = 0);
@@ -150,6 +150,16 @@ int k_ntt_rows_divide(const KCtx &k, const BatchItem *items, const u64 *tmp, siz
 // out[out_start+i] = sum_{t<n_terms} ct[ct_start+t] (*) pt[pt_start + i*n_terms + t], i < n_out <= FENC_MAC_GROUP
 int k_mac(const KCtx &k, const MacGroup *groups, int n_groups, int max_group, const u64 *const *term_ct, const u64 *const *term_pt,
           u64 *const *outs, int L, int max_lazy, u64 q_max, double alg_bytes);
+// scalar MAC of factored weights (R2.9c): a group = up to FENC_SMAC_GROUP outputs sharing one ciphertext sequence and one
+// mask segmentation; out[out_start+i] = sum_s M_s (*) ( sum_{t in segment s} k[kidx[k_start + i*n_terms + t]] . ct[ct_start+t] )
+#define FENC_SMAC_GROUP 8
+struct SmacGroup {
+  int n_out, n_terms, ct_start, k_start, out_start, seg_start, n_seg, pad;
+};
+// kpair: [n_w][L] 16-byte entries: fp64 mode {(double) k, (double)(k / q)}, integer mode {k 2^64 mod q, 0}
+int k_smac(const KCtx &k, const SmacGroup *groups, int n_groups, int max_group, const u64 *const *term_ct, const int *kidx,
+           const ShoupC *kpair, const int *seg_end, const u64 *const *seg_mask, u64 *const *outs, int L, bool fp64_mode,
+           int max_lazy, double alg_bytes);
 // outs[o] = sum of listed [2][L][N] arrays
 int k_add_many(const KCtx &k, const u64 *const *term, const int *start, u64 *const *outs, int n_out, int L, int n_terms);
 // rows kernels: row r uses modulus row_mod[r] (device array)

@@ -358,6 +358,60 @@ fenc_status run_mac(fenc_ctx *ctx, const MacJob &job, int L) {
                      (const u64 *const *)(base + o2), (u64 *const *)(base + o3), L, ctx->max_lazy, *std::max_element(ctx->mod.begin(), ctx->mod.begin() + L), mac_alg_bytes(ctx, tc, tp, n, L)));
   return FENC_OK;
 }
+// Factored weights (R2.9c): outputs with the same ciphertext sequence AND the same mask segmentation (the output channels
+// of one fragment) form groups of up to FENC_SMAC_GROUP; one launch for all of them.
+fenc_status run_smac(fenc_ctx *ctx, const SmacJob &job, const fenc_wts *W, int L) {
+  const size_t n = job.outs.size();
+  if (n == 0) return FENC_OK;
+  typedef std::pair<std::vector<const u64 *>, std::vector<const u64 *>> Seq;  // (ciphertexts, masks) per term
+  std::map<Seq, std::vector<int>> by_seq;
+  std::vector<Seq> order;
+  for (size_t o = 0; o < n; o++) {
+    Seq seq;
+    for (auto &t : job.terms[o]) seq.first.push_back(t.ct), seq.second.push_back(t.mask);
+    auto it = by_seq.find(seq);
+    if (it == by_seq.end()) order.push_back(seq), by_seq[seq] = {(int)o};
+    else it->second.push_back((int)o);
+  }
+  std::vector<SmacGroup> groups;
+  std::vector<const u64 *> tc, seg_mask, all_masks;
+  std::vector<int> kidx, seg_end;
+  std::vector<u64 *> outs;
+  int max_group = 1;
+  for (auto &seq : order) {
+    const std::vector<int> &members = by_seq[seq];
+    const int nt = (int)seq.first.size();
+    std::vector<int> ends;
+    std::vector<const u64 *> masks;
+    for (int t = 0; t < nt; t++)
+      if (t + 1 == nt || seq.second[t + 1] != seq.second[t]) ends.push_back(t + 1), masks.push_back(seq.second[t]);
+    for (size_t at = 0; at < members.size(); at += FENC_SMAC_GROUP) {
+      const int ng = (int)std::min<size_t>(FENC_SMAC_GROUP, members.size() - at);
+      groups.push_back(SmacGroup{ng, nt, (int)tc.size(), (int)kidx.size(), (int)outs.size(), (int)seg_end.size(), (int)ends.size(), 0});
+      tc.insert(tc.end(), seq.first.begin(), seq.first.end());
+      seg_end.insert(seg_end.end(), ends.begin(), ends.end());
+      seg_mask.insert(seg_mask.end(), masks.begin(), masks.end());
+      for (int i = 0; i < ng; i++) {
+        for (auto &t : job.terms[members[at + i]]) kidx.push_back(t.w);
+        outs.push_back(job.outs[members[at + i]]);
+      }
+      max_group = std::max(max_group, ng);
+    }
+    all_masks.insert(all_masks.end(), masks.begin(), masks.end());
+  }
+  DescStage st(ctx);
+  size_t o0 = st.add(groups), o1 = st.add(tc), o2 = st.add(kidx), o3 = st.add(seg_end), o4 = st.add(seg_mask), o5 = st.add(outs);
+  char *base = st.commit();
+  if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
+  // algorithmic bytes: every distinct ciphertext and mask read once, every output written once, the scalars once
+  const double bytes = mac_alg_bytes(ctx, tc, all_masks, n, L) + 16.0 * L * (double)W->n;
+  const u64 qmax = *std::max_element(ctx->mod.begin(), ctx->mod.begin() + L);
+  const int lazy = W->k_fp64 ? (int)std::min<u64>(((u64)1 << 53) / qmax, 1u << 20) - 1 : ctx->max_lazy - 1;
+  CUDA_OK(ctx, k_smac(ctx->k, (const SmacGroup *)(base + o0), (int)groups.size(), max_group, (const u64 *const *)(base + o1),
+                      (const int *)(base + o2), W->d_k, (const int *)(base + o3), (const u64 *const *)(base + o4),
+                      (u64 *const *)(base + o5), L, W->k_fp64, lazy, bytes));
+  return FENC_OK;
+}
 // algorithmic bytes of one MAC launch: every distinct ciphertext and plaintext read once, every output written once
 double mac_alg_bytes(fenc_ctx *ctx, const std::vector<const u64 *> &tc, const std::vector<const u64 *> &tp, size_t n_out, int L) {
   std::vector<const u64 *> a(tc), b(tp);

@@ -27,7 +27,7 @@ void prof_begin(Prof *p, void *stream, int id, double alg_bytes, double alg_butt
 void prof_end(Prof *p, void *stream) { cudaEventRecord(p->recs.back().b, (cudaStream_t)stream); }
 
 static const char *kNames[K_COUNT] = {"intt_rowpass", "intt_colpass", "ntt_colpass", "ntt_colpass_bconv", "ntt_rowpass",
-                                      "ntt_rows_keymac", "ntt_rows_divide", "mac", "add_many", "rowop", "sample"};
+                                      "ntt_rows_keymac", "ntt_rows_divide", "mac", "add_many", "rowop", "sample", "smac"};
 
 extern "C" fenc_status fenc_profile_enable(fenc_ctx *ctx, int on) {
   if (!ctx) return FENC_ERR_INVALID_ARG;

@@ -1,6 +1,8 @@
 """GPU parity (-m gpu): libfenc's CUDA path, called through the C ABI, against the CPU oracle element by element on
 the same seeded inputs.  Bar: bit-exact on every RNS limb (integer work); decoded outputs within 1e-3 of plaintext
 fp64 convolution (BASELINE.json north_star).  Parity starts at integer plaintext coefficients (A7)."""
+from fractions import Fraction
+
 import numpy as np
 import pytest
 
@@ -202,6 +204,100 @@ def test_hconv_hoisted_inner_rotations_bit_exact(mods, name, conv_kw, S):
     P, ctx = make(mods, name)
     err, _ = run_hconv(mods, P, ctx, conv_kw, S, seed=5, hoist=True)
     assert err < 1e-3
+    ctx.close()
+
+
+def run_hconv_factored(mods, P, ctx, conv_kw, S, seed, hoist=False):
+    """GPU fenc_hconv with factored weights (R2.9c) vs the oracle's hconv_factored for every batch group; parity starts at
+    the integer multipliers and the masks' integer coefficients (A7).  Returns the max decoded error."""
+    ck, fr, fenc = mods
+    x, w = wl.conv_inputs(seed, conv_kw)
+    od = fr.ConvDesc(S=S, **conv_kw)
+    graph = fr.ConvGraph(od, P.n)
+    conv = ctx.conv_desc(S=S, **conv_kw)
+    lay = ctx.layout_plan(conv)
+    assert lay.ch == 1
+    c = graph.counts()
+    L = P.nq
+    ok, gk = ck.keygen(P, 200 + seed, c["rot_steps"]), ctx.keygen(200 + seed, c["rot_steps"])
+    values, masks, E1 = fr.factor_weights(ck, P, graph, w, L)
+    E2 = next(iter(masks.values())).scale
+    keys = [tuple(int(v) for v in k) for k in ctx.wts_keys(conv, lay)]
+    mask_of, n_masks = ctx.wts_factors(conv, lay)
+    assert n_masks == len(masks) and len(mask_of) == len(keys)
+    by_id = {}
+    for wk, mid in zip(keys, mask_of):
+        assert by_id.setdefault(int(mid), graph.mask_of[wk]) == graph.mask_of[wk]  # the same partition of the weights
+    assert len(set(by_id.values())) == n_masks
+    for mid, mk in by_id.items():
+        assert np.array_equal(ctx.wts_mask_slots(conv, lay, mid), graph.mask_slots(mk))
+    k = np.array([ck.round_half_up(Fraction(values[wk]) * E1) for wk in keys], dtype=np.int64)
+    mc = np.stack([masks[by_id[i]].coeffs for i in range(n_masks)])
+    gW = ctx.conv_weights_factored_from_ints(conv, lay, k, mc, L, float(E1), float(E2))
+    lin = graph.lin
+    g_in, o_in = [], {}
+    for bg in range(lin.BG):
+        for g in range(lin.G):
+            for u in range(S):
+                for v in range(S):
+                    pt = ck.encode(P, lin.gather(x, u, v, g, bg), L)
+                    o_in[(bg, u, v, g)] = ck.encrypt(P, ok, pt, 1000 + len(g_in))
+                    g_in.append(ctx.encrypt(gk, ctx.pt_from_coeffs(pt.coeffs, L, float(pt.scale)), 1000 + len(g_in)))
+    ctx.set_hoisting(hoist)
+    g_out = ctx.hconv(gk, conv, lay, gW, g_in)
+    So, lout = graph.S_out, graph.lout
+    Y = np.zeros((od.BS, od.C_out, od.H_out, od.W_out))
+    for bg in range(lin.BG):
+        ins = {(u, v, g): o_in[(bg, u, v, g)] for g in range(lin.G) for u in range(S) for v in range(S)}
+        o_out = fr.hconv_factored(ck, P, ok, graph, ins, values, masks, E1, hoist=hoist)
+        for go in range(lout.G):
+            for uo in range(So):
+                for vo in range(So):
+                    gct = g_out[((bg * lout.G + go) * So + uo) * So + vo]
+                    ref = o_out[(uo, vo, go)]
+                    assert np.array_equal(ctx.ct_export(gct), ref.c), (bg, go, uo, vo)
+                    assert abs(gct.scale - float(ref.scale)) <= 1e-9 * float(ref.scale)
+                    ctx.decrypt_decode(gk, gct, conv, lay, 1, uo, vo, go, bg, Y)
+    err = np.abs(Y - fr.direct_conv(od, x, w)).max()
+    # the library's own factoring (fp64 weights in, multipliers rounded and masks encoded on the library side)
+    outs2 = ctx.hconv(gk, conv, lay, ctx.conv_weights_factored(conv, lay, w, L), g_in)
+    Y2 = np.zeros_like(Y)
+    i = 0
+    for bg in range(lin.BG):
+        for go in range(lout.G):
+            for uo in range(So):
+                for vo in range(So):
+                    ctx.decrypt_decode(gk, outs2[i], conv, lay, 1, uo, vo, go, bg, Y2)
+                    i += 1
+    assert np.abs(Y2 - Y).max() < 1e-5
+    return err
+
+
+@pytest.mark.parametrize("name,over,conv_kw,S,hoist", [
+    ("mid10", {}, dict(BS=32, C_in=3, H=4, W=4, C_out=5, K=3, stride=1, pad=1), 1, False),           # 27 terms, border masks
+    ("mid10", {}, dict(BS=64, C_in=2, H=7, W=6, C_out=3, K=3, stride=2, pad=1), 2, True),            # stride, frame > data, BG=2, hoisted
+    ("mid10", {}, dict(BS=32, C_in=4, H=4, W=4, C_out=4, K=3, stride=1, pad=1, depthwise=True), 1, False),
+    ("mid10", {}, dict(BS=40, C_in=9, H=4, W=4, C_out=11, K=1, stride=1, pad=0), 1, False),          # point-wise: groups of 8 + 3 outputs, ragged batch
+    ("mid12", dict(q_bits=50, log2_scale=50), dict(BS=32, C_in=3, H=8, W=8, C_out=9, K=3, stride=1, pad=1), 1, True),  # 50-bit: fp64 sums reduced every 7 terms
+    ("toy64", dict(q_bits=58, p_bits=60, log2_scale=30), dict(BS=8, C_in=5, H=2, W=2, C_out=3, K=1, stride=1, pad=0), 1, False),  # 58-bit: integer mode
+])
+def test_hconv_factored_weights_bit_exact(mods, name, over, conv_kw, S, hoist):
+    """R2.9c (large-batch layouts, ch = 1): weight plaintexts replaced by integer multipliers and shared mask plaintexts;
+    limbs against the oracle's factored variant, decoded result against direct convolution."""
+    P, ctx = make(mods, name, **over)
+    err = run_hconv_factored(mods, P, ctx, conv_kw, S, seed=6, hoist=hoist)
+    assert err < (1e-3 if name != "toy64" else 5e-2)
+    ctx.close()
+
+
+def test_factored_weights_need_one_channel_per_ciphertext(mods):
+    ck, fr, fenc = mods
+    P, ctx = make(mods, "mid10")
+    conv = ctx.conv_desc(S=1, BS=1, C_in=4, H=4, W=4, C_out=4, K=3, stride=1, pad=1)
+    lay = ctx.layout_plan(conv)
+    assert lay.ch > 1
+    with pytest.raises(fenc.FencError, match="LAYOUT"):
+        ctx.conv_weights_factored(conv, lay, np.zeros((4, 4, 3, 3)), P.nq)
     ctx.close()
 
 
