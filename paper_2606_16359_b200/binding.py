@@ -66,7 +66,8 @@ SYMBOLS = ["fenc_params_init", "fenc_ctx_free", "fenc_last_error", "fenc_get_pri
            "fenc_fc_wts_keys", "fenc_fc_weights", "fenc_fc_weights_from_coeffs", "fenc_fc", "fenc_measure_alu_peak",
            "fenc_cmult_relin", "fenc_mul_scalar", "fenc_add_const", "fenc_ct_import_async", "fenc_ct_export_async",
            "fenc_export_wait", "fenc_set_hoisting", "fenc_rotate_hoisted", "fenc_square_sum_relin",
-           "fenc_wts_factors", "fenc_wts_mask_slots", "fenc_conv_weights_factored", "fenc_conv_weights_factored_from_ints"]
+           "fenc_wts_factors", "fenc_wts_mask_slots", "fenc_conv_weights_factored", "fenc_conv_weights_factored_from_ints",
+           "fenc_measure_smac_peak"]
 
 _lib = None
 
@@ -117,6 +118,7 @@ def load_library(path=None):
         "fenc_add_const": [vp, vpp, C.c_size_t, u64p, vpp],
         "fenc_profile_enable": [vp, C.c_int],
         "fenc_measure_alu_peak": [vp, dp, dp],
+        "fenc_measure_smac_peak": [vp, dp],
         "fenc_profile_read": [vp, dp, u64p, dp, dp, C.c_int],
         "fenc_wts_keys": [vp, C.POINTER(ConvDesc), C.POINTER(Layout), u32p, C.c_size_t, C.POINTER(C.c_size_t)],
         "fenc_conv_weights": [vp, C.POINTER(ConvDesc), C.POINTER(Layout), dp, C.c_uint32, C.c_double, vpp],
@@ -478,6 +480,11 @@ class Context:
         a, b = C.c_double(), C.c_double()
         self._ck(self.lib.fenc_measure_alu_peak(self.h, C.byref(a), C.byref(b)))
         return a.value, b.value
+
+    def measure_smac_peak(self):
+        v = C.c_double()
+        self._ck(self.lib.fenc_measure_smac_peak(self.h, C.byref(v)))
+        return v.value
 
     def profile_enable(self, on=True):
         self._ck(self.lib.fenc_profile_enable(self.h, int(on)))

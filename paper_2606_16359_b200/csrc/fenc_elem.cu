@@ -4,6 +4,7 @@
 #include "fenc_device.cuh"
 
 #define PROF(k, id, bytes) if ((k).prof) prof_begin((k).prof, (k).stream, id, (double)(bytes))
+#define PROF2(k, id, bytes, ops) if ((k).prof) prof_begin((k).prof, (k).stream, id, (double)(bytes), (double)(ops))
 #define LAUNCH_CHECK(k)                            \
   do {                                             \
     (*(k).launches)++;                             \
@@ -309,12 +310,12 @@ static void launch_smac(const SmacP &p, dim3 grid, int nth, cudaStream_t st, int
 }
 int k_smac(const KCtx &k, const SmacGroup *groups, int n_groups, int max_group, const u64 *const *term_ct, const int *kidx,
            const ShoupC *kpair, const int *seg_end, const u64 *const *seg_mask, u64 *const *outs, int L, bool fp64_mode,
-           int max_lazy, double alg_bytes) {
+           int max_lazy, double alg_bytes, double alg_mulaccs) {
   if (n_groups == 0) return 0;
   SmacP p{groups, term_ct, kidx, kpair, seg_end, seg_mask, outs, k.d_mods, L, k.geom.logN, max_lazy < 2 ? 2 : max_lazy};
   const int nth = k.N < 256 ? k.N : 256;
   dim3 grid(n_groups, (unsigned)(((size_t)L * k.N) / nth));
-  PROF(k, K_SMAC, alg_bytes);
+  PROF2(k, K_SMAC, alg_bytes, alg_mulaccs);  // second counter of this class: modular multiply-accumulates
   if (fp64_mode) launch_smac<true>(p, grid, nth, S(k), max_group);
   else launch_smac<false>(p, grid, nth, S(k), max_group);
   LAUNCH_CHECK(k);

@@ -159,7 +159,7 @@ struct SmacGroup {
 // kpair: [n_w][L] 16-byte entries: fp64 mode {(double) k, (double)(k / q)}, integer mode {k 2^64 mod q, 0}
 int k_smac(const KCtx &k, const SmacGroup *groups, int n_groups, int max_group, const u64 *const *term_ct, const int *kidx,
            const ShoupC *kpair, const int *seg_end, const u64 *const *seg_mask, u64 *const *outs, int L, bool fp64_mode,
-           int max_lazy, double alg_bytes);
+           int max_lazy, double alg_bytes, double alg_mulaccs);
 // outs[o] = sum of listed [2][L][N] arrays
 int k_add_many(const KCtx &k, const u64 *const *term, const int *start, u64 *const *outs, int n_out, int L, int n_terms);
 // rows kernels: row r uses modulus row_mod[r] (device array)

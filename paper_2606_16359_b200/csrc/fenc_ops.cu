@@ -405,11 +405,13 @@ fenc_status run_smac(fenc_ctx *ctx, const SmacJob &job, const fenc_wts *W, int L
   if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
   // algorithmic bytes: every distinct ciphertext and mask read once, every output written once, the scalars once
   const double bytes = mac_alg_bytes(ctx, tc, all_masks, n, L) + 16.0 * L * (double)W->n;
+  double mulaccs = 0;
+  for (auto &tl : job.terms) mulaccs += 2.0 * (double)tl.size() * L * ctx->N;
   const u64 qmax = *std::max_element(ctx->mod.begin(), ctx->mod.begin() + L);
   const int lazy = W->k_fp64 ? (int)std::min<u64>(((u64)1 << 53) / qmax, 1u << 20) - 1 : ctx->max_lazy - 1;
   CUDA_OK(ctx, k_smac(ctx->k, (const SmacGroup *)(base + o0), (int)groups.size(), max_group, (const u64 *const *)(base + o1),
                       (const int *)(base + o2), W->d_k, (const int *)(base + o3), (const u64 *const *)(base + o4),
-                      (u64 *const *)(base + o5), L, W->k_fp64, lazy, bytes));
+                      (u64 *const *)(base + o5), L, W->k_fp64, lazy, bytes, mulaccs));
   return FENC_OK;
 }
 // algorithmic bytes of one MAC launch: every distinct ciphertext and plaintext read once, every output written once

@@ -140,6 +140,61 @@ __global__ void __launch_bounds__(256) butterfly_f64_peak_kernel(u64 *out, u64 q
   for (int k = 0; k < 8; k++) s ^= y[k];
   out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
+// the scalar MAC's inner operation (fenc_elem.cu smac_kernel, fp64 mode) on registers only: 16 accumulators, one exact
+// x k mod q product and one add each per step, reduced every 7 steps as for a 50-bit modulus
+__global__ void __launch_bounds__(256) smac_peak_kernel(u64 *out, u64 q, u64 qinv_bits, u64 c_bits, u64 cq_bits, int iters) {
+  const F64Mod fm = f64mod(q, qinv_bits);
+  double acc[16], cs[8], cqs[8];
+  double x0 = u2d52((threadIdx.x * 7919u + blockIdx.x) % q), x1 = u2d52((threadIdx.x * 104729u + blockIdx.x) % q);
+#pragma unroll
+  for (int k = 0; k < 8; k++) {  // eight scalars (one per output of a group), each with its quotient constant
+    cs[k] = __longlong_as_double((long long)c_bits) - (double)k;
+    cqs[k] = cs[k] * fm.qinv;
+  }
+#pragma unroll
+  for (int k = 0; k < 16; k++) acc[k] = 0.0;
+  for (int it = 0; it < iters; it++) {
+#pragma unroll
+    for (int u = 0; u < 7; u++) {
+#pragma unroll
+      for (int k = 0; k < 8; k++) {
+        acc[2 * k] = __dadd_rn(acc[2 * k], mulmod_dd(x0, cs[k], cqs[k], fm));
+        acc[2 * k + 1] = __dadd_rn(acc[2 * k + 1], mulmod_dd(x1, cs[k], cqs[k], fm));
+      }
+      x0 += 1.0, x1 += 3.0;  // a new ciphertext word per term (stays far below 2^51 over the run)
+    }
+#pragma unroll
+    for (int k = 0; k < 16; k++) acc[k] = reduce_dd(acc[k], fm);
+  }
+  double s = 0;
+#pragma unroll
+  for (int k = 0; k < 16; k++) s += acc[k];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = (u64)__double_as_longlong(s);
+}
+extern "C" fenc_status fenc_measure_smac_peak(fenc_ctx *ctx, double *mulaccs_per_s) {
+  if (!ctx || !mulaccs_per_s) return FENC_ERR_INVALID_ARG;
+  const int blocks = 148 * 8, iters = 1024;
+  u64 *buf = dalloc_t<u64>(ctx, (size_t)blocks * 256);
+  if (!buf) return fail(ctx, FENC_ERR_OOM, "peak buffer");
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0), cudaEventCreate(&e1);
+  float ms = 0;
+  const u64 q = ctx->mod[0], w = ctx->psi[0];
+  const u64 qinv = fh::double_bits(1.0 / (double)q), cb = fh::double_bits((double)w), cqb = fh::double_bits((double)((long double)w / (long double)q));
+  for (int rep = 0; rep < 2; rep++) {
+    cudaEventRecord(e0, ctx->stream);
+    smac_peak_kernel<<<blocks, 256, 0, ctx->stream>>>(buf, q, qinv, cb, cqb, iters);
+    (void)cqb;
+    cudaEventRecord(e1, ctx->stream);
+    CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+    cudaEventElapsedTime(&ms, e0, e1);
+  }
+  *mulaccs_per_s = (double)blocks * 256 * 16.0 * 7.0 * iters / (ms * 1e-3);
+  cudaEventDestroy(e0), cudaEventDestroy(e1);
+  dfree(ctx, buf);
+  ctx->launches += 2;
+  return FENC_OK;
+}
 extern "C" fenc_status fenc_measure_alu_peak(fenc_ctx *ctx, double *imad_lane_ops_per_s, double *butterflies_per_s) {
   if (!ctx || !imad_lane_ops_per_s || !butterflies_per_s) return FENC_ERR_INVALID_ARG;
   const int blocks = 148 * 8, iters = 4096;

@@ -31,7 +31,8 @@ def poly3_activation(ctx, keys, cts, scale, coef=POLY3):
 
 class Pipeline:
     """layers: list of dicts
-         {"op": "conv", "conv": {BS, C_in, H, W, C_out, K, stride, pad, [depthwise], [M]}, "S": S, "w": ndarray}
+         {"op": "conv", "conv": {BS, C_in, H, W, C_out, K, stride, pad, [depthwise], [M]}, "S": S, "w": ndarray,
+          ["factored": True]}                  factored: weights as integer multipliers + mask plaintexts (R2.9c, ch = 1)
          {"op": "square"}                      x -> x^2, relinearised and rescaled (one level)
          {"op": "pool"}                        2x2 sum-pool by fragment selection (S halves; factor 1/4 goes into the next w)
          {"op": "fc", "fc": {...}, "w": ndarray[n_out][n_in]}     plain-diagonal fully connected layer
@@ -46,7 +47,7 @@ class Pipeline:
                 conv = ctx.conv_desc(S=ly["S"], **ly["conv"])
                 lay = ctx.layout_plan(conv)
                 self.steps.update(lay.steps())
-                self.plan.append(dict(op="conv", conv=conv, lay=lay, L=L, w=ly.get("w")))
+                self.plan.append(dict(op="conv", conv=conv, lay=lay, L=L, w=ly.get("w"), factored=bool(ly.get("factored"))))
                 L -= 1
             elif ly["op"] == "fc":
                 fc = ctx.fc_desc(**ly["fc"])
@@ -99,7 +100,9 @@ class Pipeline:
         self.weights = []
         for p in self.plan:
             if p["op"] == "conv":
-                if encode_weight is not None:
+                if p["factored"]:  # value x mask weights of a one-channel-per-ciphertext layout (R2.9c)
+                    self.weights.append(ctx.conv_weights_factored(p["conv"], p["lay"], p["w"], p["L"]))
+                elif encode_weight is not None:
                     self.weights.append(ctx.conv_weights_from_coeffs(p["conv"], p["lay"], encode_weight(p), p["L"]))
                 else:
                     self.weights.append(ctx.conv_weights(p["conv"], p["lay"], p["w"], p["L"]))
