@@ -280,6 +280,10 @@ class Context:
     def launch_count(self, reset=False):
         return int(self.lib.fenc_launch_count(self.h, int(reset)))
 
+    def ct_bytes(self, ct):
+        """device bytes of a ciphertext: uint64 [2][L][N]"""
+        return 2 * ct.L * self.N * 8
+
     def device_bytes(self):
         return int(self.lib.fenc_device_bytes(self.h))
 

@@ -40,16 +40,26 @@ def test_max_over_ranks_and_aggregate_gloo_world2():
         assert abs(agg - 2 * 5 / 15e-3) < 1e-9   # whole-job units over that time
 
 
-def test_level_ops_counts_match_plan_shape():
+def test_oracle_op_counts_follow_the_variant_the_gpu_arm_runs():
+    """bench.py's CPU arm counts the SAME operation graph as the GPU arm: hoisted inner rotations, one relinearisation per
+    pooled output, baby-step giant-step fc layers (BASELINE config 2: 48 + 192 conv rotations, 78 + 28 + 21 fc rotations,
+    24 + 16 lazy relinearisations), and factored weights for config 4 (scalar multiply-accumulates + one product per mask)."""
     sys.path.insert(0, ROOT)
     import bench
-
-    class Lay:
-        n_inner_rot, n_outer_rot, n_pmult, n_out_ct = 48, 0, 2400, 96
-    plan = [dict(op="conv", L=8, lay=Lay), dict(op="square", L=7), dict(op="pool", L=6),
-            dict(op="fc", L=6, info=dict(n_rot=126, n_pmult=2048, n_out_ct=2))]
-    ops = bench.level_ops(plan)
-    assert ops[8] == [48, 2400, 96, 0] and ops[7] == [0, 0, 0, 96] and ops[6] == [126, 2048, 2, 0]
+    layers, _ = bench.lenet_layers(128, 2000)
+    ops = bench.oracle_op_counts(layers, 8192, 8, hoist=True, lazy=True)
+    kinds = lambda k: sum(v for (kk, _), v in ops.items() if kk == k)
+    assert kinds("rot_h") == 48 + 192 + 36 and kinds("rot") == 367 - 276
+    assert ops[("square_sum4", 7)] == 24 and ops[("square_sum4", 5)] == 16 and kinds("square") == 0
+    assert ops[("pmult", 8)] == 2400 and ops[("pmult", 6)] == 9600 and ops[("rescale", 8)] == 96
+    eager = bench.oracle_op_counts(layers, 8192, 8, hoist=False, lazy=False)
+    assert sum(v for (k, _), v in eager.items() if k == "square") == 160 and sum(v for (k, _), v in eager.items() if k == "rot") == 367
+    assert not any(k == "rot_h" for k, _ in eager)
+    m, _ = bench.mobilenet_layers(32, 2000)
+    ops4 = bench.oracle_op_counts(m, 32768, 30, hoist=True, lazy=True)
+    assert ops4[("rot_h", 30)] == 51 and ops4[("rot_h", 29)] == 640 and ops4[("rot_h", 27)] == 576
+    assert ops4[("smul", 28)] == 32768 and ops4[("smul", 26)] == 32768 and ops4[("pmult", 28)] == 1024 and ops4[("pmult", 26)] == 512
+    assert not any(k == "rot" for k, _ in ops4)  # ch = 1: no outer rotations at all (PAPER.md:218-222)
 
 
 @pytest.mark.timeout(600)
@@ -63,4 +73,4 @@ def test_reference_arm_prints_one_line_under_torchrun_world2():
     assert len(lines) == 1
     d = json.loads(lines[0])
     assert d["impl"] == "reference" and d["cpu_baseline"]["kind"] == "oracle" and d["value"] > 0
-    assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["n_gpus"] == 2
+    assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["n_gpus"] == 0 and d["cpu_baseline"]["same_graph"] is True

@@ -7,6 +7,8 @@ and the rotation of an all-zero ciphertext are exactly zero on both sides and th
 evaluation of the sampled terms alone -- the full layer still runs on the GPU (same grids, same batches).
 Inputs are ciphertexts with uniform-random limbs (BASELINE config 5's recipe): bit-exactness does not need a message;
 the decoded <= 1e-3 checks of the same layers are in test_gpu_parity.py."""
+from fractions import Fraction
+
 import numpy as np
 import pytest
 
@@ -248,4 +250,115 @@ def test_rotation_config5_L36_dnum1_full_size(mods):
     outs = ctx.rotate(gk, [ctx.ct_import(a) for a in limbs], steps * 3)
     ref = ck.rotate(P, ok, ck.Ciphertext(limbs[1], 36, 1), 12345)
     assert np.array_equal(ctx.ct_export(outs[1]), ref.c)
+    ctx.close()
+
+
+# ------------------------------------------------------------------------------------------------ config 4 (factored weights, R2.9c)
+def oracle_factored_sample(ck, P, ok, L, graph, inputs, okey, values, masks, E1, hoist):
+    """One output ciphertext of a factored layer (R2.9c) from the oracle: hoisted inner rotations in worker processes,
+    S_mu = sum_t round_half_up(v_t E1) . R_t per mask, acc = sum_mu S_mu (*) M_mu, rescale.  (ch = 1: diagonal 0 only.)"""
+    (d, lst), = graph.terms[okey].items()
+    assert d == 0
+    need = sorted({(src, amt) for src, amt, _ in lst if amt})
+    rot = pmap(dict(ck=ck, P=P, keys=ok, inputs=inputs), job_rotate, [(src, amt, hoist) for src, amt in need])
+    R = {k: ck.Ciphertext(c, L, inputs[k[0]].scale) for k, c in zip(need, rot)}
+    by_mask = {}
+    for src, amt, wk in lst:
+        by_mask.setdefault(graph.mask_of[wk], []).append((src, amt, wk))
+    acc = np.zeros((2, L, P.N), dtype=np.uint64)
+    s_in = next(iter(inputs.values())).scale
+    for mk, tl in by_mask.items():
+        S = None
+        for src, amt, wk in tl:
+            t = ck.mul_const(P, R[(src, amt)] if amt else inputs[src], values[wk], E1)
+            S = t if S is None else ck.add(P, S, t)
+        ck.pmult_acc(P, acc, S, masks[mk])
+    return ck.rescale(P, ck.Ciphertext(acc, L, s_in * E1 * masks[mk].scale))
+
+
+def factored_sampled_layer(mods, P, ctx, conv_kw, S, L, okey, seed, hoist=True):
+    """Run one factored layer at full size on the GPU with every multiplier outside output `okey` set to zero, and compare
+    that output with the oracle; another output must be exactly the zero ciphertext."""
+    ck, fr, fenc = mods
+    graph = fr.ConvGraph(fr.ConvDesc(S=S, **conv_kw), P.n)
+    conv = ctx.conv_desc(S=S, **conv_kw)
+    lay = ctx.layout_plan(conv)
+    assert lay.ch == 1 and lay.n_outer_rot == 0
+    cw = 1 if conv_kw.get("depthwise") else conv_kw["C_in"]
+    w = np.random.default_rng(seed).normal(0, 0.05, (conv_kw["C_out"], cw, conv_kw["K"], conv_kw["K"]))
+    values, masks, E1 = fr.factor_weights(ck, P, graph, w, L)
+    E2 = next(iter(masks.values())).scale
+    keys = [tuple(int(v) for v in k) for k in ctx.wts_keys(conv, lay)]
+    mask_of, n_masks = ctx.wts_factors(conv, lay)
+    by_id = {}
+    for wk, mid in zip(keys, mask_of):
+        assert by_id.setdefault(int(mid), graph.mask_of[wk]) == graph.mask_of[wk]
+    assert n_masks == len(masks) == len(by_id)
+    sampled = {wk for _, _, wk in graph.terms[okey][0]}
+    k = np.array([ck.round_half_up(Fraction(values[wk]) * E1) if wk in sampled else 0 for wk in keys], dtype=np.int64)
+    assert np.count_nonzero(k) == len(sampled)
+    mc = np.stack([masks[by_id[i]].coeffs for i in range(n_masks)])
+    gW = ctx.conv_weights_factored_from_ints(conv, lay, k, mc, L, float(E1), float(E2))
+    need = sorted({amt for _, amt, _ in graph.terms[okey][0] if amt})
+    gk, ok = ctx.keygen(90 + seed, lay.steps()), ck.keygen(P, 90 + seed, need)
+    o_in, g_in = {}, []
+    for (u, v, g, bg) in graph.lin.ct_keys():
+        limbs = wl.random_ct_limbs(8000 + len(g_in), P.q, L, P.N)
+        o_in[(u, v, g)] = ck.Ciphertext(limbs, L, P.scale)
+        g_in.append(ctx.ct_import(limbs, float(P.scale)))
+    ctx.set_hoisting(hoist)
+    g_out = ctx.hconv(gk, conv, lay, gW, g_in)
+    uo, vo, go = okey
+    So = graph.S_out
+    got = g_out[(go * So + uo) * So + vo]
+    ref = oracle_factored_sample(ck, P, ok, L, graph, o_in, okey, values, masks, E1, hoist)
+    assert got.L == L - 1 and np.array_equal(ctx.ct_export(got), ref.c)
+    other = g_out[0] if (go, uo, vo) != (0, 0, 0) else g_out[1]
+    assert not ctx.ct_export(other).any()
+
+
+def test_cfg4_conv1_factored_full_size_sampled(mods):
+    """BASELINE config 4's first layer as bench.py runs it: conv 3 -> 32, 3x3, stride 2, 224 x 224 in a 256 frame, S = 8,
+    BS = 32 (B = 32, ch = 1), N=2^16, L=30, dlen 5: 192 -> 512 ciphertexts, 51 hoisted inner rotations, 13824 scalar
+    multiply-accumulates on the FP64 pipe, masks for the frame and the zero padding.  One border output against the oracle."""
+    P, ctx = make(mods, wl.PARAMS["cfg4"])
+    kw = dict(BS=32, C_in=3, H=224, W=224, C_out=32, K=3, stride=2, pad=1)
+    factored_sampled_layer(mods, P, ctx, kw, 8, 30, (0, 0, 5), seed=1)
+    ctx.close()
+
+
+def test_cfg4_pointwise_factored_full_size_sampled(mods):
+    """BASELINE config 4's last layer: pointwise 64 -> 128 at 56 x 56 (frame 64, S = 2), BS = 32, L=26: 256 -> 512
+    ciphertexts, no rotation at all, 32768 scalar multiply-accumulates in groups of 8 outputs, one mask product each."""
+    P, ctx = make(mods, wl.PARAMS["cfg4"])
+    kw = dict(BS=32, C_in=64, H=56, W=56, C_out=128, K=1, stride=1, pad=0)
+    factored_sampled_layer(mods, P, ctx, kw, 2, 26, (1, 0, 77), seed=2)
+    ctx.close()
+
+
+def test_cfg4_mobilenet_chain_full_size_decoded(mods):
+    """The whole config-4 step of bench.py for one batch group of 32 images (five chained layers, levels 30 -> 25, factored
+    weights, hoisted rotations): sampled output ciphertexts decrypt to the fp64 evaluation of the same five convolutions
+    within 1e-3 (north_star's decoded bar)."""
+    ck, fr, fenc = mods
+    import bench
+    from paper_2606_16359_b200.pipeline import Pipeline
+    ctx = fenc.Context(**wl.PARAMS["cfg4"])
+    ctx.set_hoisting(True)
+    layers, x = bench.mobilenet_layers(32, 2004)
+    pipe = Pipeline(ctx, layers)
+    keys = pipe.setup(key_seed=2004)
+    out = pipe.forward(pipe.encrypt_input(x, 30000))
+    assert len(out) == 512 and out[0].L == 25
+    want = x
+    for ly in layers:
+        want = fr.direct_conv(fr.ConvDesc(**ly["conv"]), want, ly["w"])
+    assert want.shape == (32, 128, 56, 56)
+    p = pipe.plan[-1]
+    Y = np.full(want.shape, np.nan)
+    for go, uo, vo in ((0, 0, 0), (127, 1, 1), (64, 0, 1), (31, 1, 0)):
+        ctx.decrypt_decode(keys, out[(go * 2 + uo) * 2 + vo], p["conv"], p["lay"], 1, uo, vo, go, 0, Y)
+    seen = ~np.isnan(Y)
+    assert seen.sum() == 4 * 32 * 28 * 28
+    assert np.abs(Y[seen] - want[seen]).max() < 1e-3
     ctx.close()
