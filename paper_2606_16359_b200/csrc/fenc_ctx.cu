@@ -321,7 +321,7 @@ LevelPlan *get_plan(fenc_ctx *ctx, int L) {
       scale_in[i] = shoupc(fh::mulmod(ninv, fh::invmod(qhat, qi), qi), qi);
     }
     bool src_f64 = true;
-    for (int i = lo; i < hi; i++) src_f64 = src_f64 && fh::f64_narrow(mod[i]);
+    for (int i = lo; i < hi; i++) src_f64 = src_f64 && fh::f64_modulus(mod[i], ctx->logN);  // below 2^50: conv_dot_f64
     groups_up.push_back(ConvGroup{lo, lo, hi - lo, lo, (int)rows_up.size(), E - (hi - lo), {src_f64 ? 2 : 0, 0}});
     P.n_src_up = std::max(P.n_src_up, hi - lo);
     for (int t = 0; t < E; t++) {
@@ -370,7 +370,7 @@ LevelPlan *get_plan(fenc_ctx *ctx, int L) {
   }
   for (int c = 0; c < 2; c++) {
     groups_down.push_back(ConvGroup{c * np, nq, np, c * np, c * L, L, {0, 0}});
-    groups_rs.push_back(ConvGroup{c, L - 1, 1, c, c * (L - 1), L - 1, {(L >= 2 && fh::f64_narrow(mod[L - 1])) ? 2 : 0, 0}});
+    groups_rs.push_back(ConvGroup{c, L - 1, 1, c, c * (L - 1), L - 1, {(L >= 2 && fh::f64_modulus(mod[L - 1], ctx->logN)) ? 2 : 0, 0}});
   }
   P.d_groups_up = upload_owned(ctx, P.owned, groups_up);
   P.d_groups_down = upload_owned(ctx, P.owned, groups_down);

@@ -166,9 +166,10 @@ struct ConvColP {
   const ShoupC *mulc;  // MERGED: P^-1 mod q_t
   const ShoupC *bc_f64;  // {(double) c, (double)(c / t)} per entry of bc, used when source and target moduli are fp64 ones
 };
-// sum over the first n source tiles of Y_s[e] * bc[s] for this thread's eight elements, Montgomery-reduced: canonical
+// sum over the first n source tiles of Y_s[e] * bc[s] for this thread's eight elements, Montgomery-reduced: canonical.
+// YDBL: the tiles hold the values as doubles (see conv_dot_f64); they are exact integers below 2^50.
 template <int T, int NTH>
-DEVI void conv_dot(const u64 *smem, int n, const u64 *bc, const ModConst &mc, int max_terms, int tid, u64 (&out)[8]) {
+DEVI void conv_dot(const u64 *smem, int n, const u64 *bc, const ModConst &mc, int max_terms, int tid, u64 (&out)[8], bool ydbl) {
   u64 lo[8], hi[8], r[8];
 #pragma unroll
   for (int i = 0; i < 8; i++) lo[i] = hi[i] = r[i] = 0;
@@ -177,7 +178,10 @@ DEVI void conv_dot(const u64 *smem, int n, const u64 *bc, const ModConst &mc, in
     const u64 c = __ldg(bc + s);
     const u64 *Y = smem + (size_t)s * T;
 #pragma unroll
-    for (int i = 0; i < 8; i++) mac128(lo[i], hi[i], Y[swz(tid + i * NTH)], c);
+    for (int i = 0; i < 8; i++) {
+      const u64 w = Y[swz(tid + i * NTH)];
+      mac128(lo[i], hi[i], ydbl ? d2u_off(__longlong_as_double((long long)w), 4503599627370496.0) : w, c);
+    }
     if (++lazy == max_terms) {
 #pragma unroll
       for (int i = 0; i < 8; i++) r[i] = addmod(r[i], mont_redc(lo[i], hi[i], mc.q, mc.qinv_neg), mc.q), lo[i] = hi[i] = 0;
@@ -187,24 +191,33 @@ DEVI void conv_dot(const u64 *smem, int n, const u64 *bc, const ModConst &mc, in
 #pragma unroll
   for (int i = 0; i < 8; i++) out[i] = addmod(r[i], mont_redc(lo[i], hi[i], mc.q, mc.qinv_neg), mc.q);
 }
-// The same sum on the FP64 pipe (groups flagged pad[0] & 2: every source modulus below 2^45, and an fp64 target): each
-// term y c - rint(y c / t) t is an exact integer in (-t, t); the sum plus n t is a non-negative representative below
-// 2 n t, which is all the forward fp64 butterflies ask of their input.
+// The same sum on the FP64 pipe (groups flagged pad[0] & 2: every source modulus an fp64 one, i.e. below 2^50; and an fp64
+// target): the source tiles hold the canonical values as DOUBLES, each term y c - rint(y c / t) t is an exact integer in
+// (-t, t) (mulmod_dd: |y| < 2^51, c < t < 2^50), a sum of `lazy_max` = floor(2^53 / t) - 1 terms plus a reduced remainder
+// (at most t/2 + 1) is exact, and v - rint(v / t) t + t in (0, 2t) is what the forward fp64 butterflies ask of their input.
+// Measured (profiles/r02_convert_cols.md): the 128-bit integer form of this sum was 38 % IMAD + 18 % IADD3 of the kernel's
+// instructions with the fp64 pipe 16 % busy.
 template <int T, int NTH>
-DEVI void conv_dot_f64(const u64 *smem, int n, const ShoupC *bc, const F64Mod &fm, int tid, u64 (&out)[8]) {
+DEVI void conv_dot_f64(const u64 *smem, int n, const ShoupC *bc, const F64Mod &fm, int lazy_max, int tid, u64 (&out)[8]) {
   double acc[8];
 #pragma unroll
   for (int i = 0; i < 8; i++) acc[i] = 0.0;
+  int lazy = 0;
   for (int s = 0; s < n; s++) {
     const ulonglong2 cc = __ldg(reinterpret_cast<const ulonglong2 *>(bc + s));
     const double c = __longlong_as_double((long long)cc.x), cq = __longlong_as_double((long long)cc.y);
     const u64 *Y = smem + (size_t)s * T;
 #pragma unroll
-    for (int i = 0; i < 8; i++) acc[i] = __dadd_rn(acc[i], mulmod_dd(u2d52(Y[swz(tid + i * NTH)]), c, cq, fm));
-  }
-  const double off = __fma_rn((double)n, fm.q, 4503599627370496.0);
+    for (int i = 0; i < 8; i++) acc[i] = __dadd_rn(acc[i], mulmod_dd(__longlong_as_double((long long)Y[swz(tid + i * NTH)]), c, cq, fm));
+    if (++lazy == lazy_max) {
 #pragma unroll
-  for (int i = 0; i < 8; i++) out[i] = d2u_off(acc[i], off);
+      for (int i = 0; i < 8; i++) acc[i] = reduce_dd(acc[i], fm);
+      lazy = 1;
+    }
+  }
+  const double off = __dadd_rn(fm.q, 4503599627370496.0);
+#pragma unroll
+  for (int i = 0; i < 8; i++) out[i] = d2u_off(reduce_dd(acc[i], fm), off);
 }
 // MERGED (ModDown followed by the rescale): the group's last source tile is Z = iNTT(acc[l] P^-1 + add[l]) of
 // the limb l = q_{L-1} that the rescale drops (modulus index cg.pad[1]).  With V_t = sum_i y_i (Phat_i mod t):
@@ -226,6 +239,7 @@ __global__ void __launch_bounds__(128 * NG, NG == 1 ? 5 : (NG == 2 ? 2 : 1)) con
   u64 *W = smem + (size_t)(cg.n_src + grp) * T;  // work tiles after the source tiles
   u64 *ybase = p.y + (size_t)b * p.y_bstride;
   const int n_conv = MERGED ? cg.n_src - 1 : cg.n_src;  // tiles entering the base conversion
+  const bool ydbl = !MERGED && p.bc_f64 && (cg.pad[0] & 2);  // the converted tiles are kept as doubles (conv_dot_f64)
   // ---- sources: fill, inverse column stages, scale -> canonical coefficient tiles in shared memory
   for (int s = grp; s < cg.n_src; s += NG) {
     const u64 *src = ybase + (size_t)(cg.src_row + s) * N;
@@ -241,7 +255,8 @@ __global__ void __launch_bounds__(128 * NG, NG == 1 ? 5 : (NG == 2 ? 2 : 1)) con
 #pragma unroll
     for (int i = 0; i < 8; i++) {
       const int e = swz(tid + i * NTH);
-      Y[e] = shoup_mul(Y[e], sc.c, sc.cs, q);
+      const u64 y = shoup_mul(Y[e], sc.c, sc.cs, q);
+      Y[e] = ydbl ? (u64)__double_as_longlong(u2d52(y)) : y;
     }
   }
   __syncthreads();
@@ -251,7 +266,7 @@ __global__ void __launch_bounds__(128 * NG, NG == 1 ? 5 : (NG == 2 ? 2 : 1)) con
     const ModConst ml = p.mods[l];
     const ShoupC pl = p.mulc[l];
     u64 v[8];
-    conv_dot<T, NTH>(smem, n_conv, p.bc + (size_t)l * n_conv, ml, p.max_terms, tid, v);
+    conv_dot<T, NTH>(smem, n_conv, p.bc + (size_t)l * n_conv, ml, p.max_terms, tid, v, false);
     const u64 *Z = smem + (size_t)n_conv * T;
 #pragma unroll
     for (int i = 0; i < 8; i++) outl[i] = submod(Z[swz(tid + i * NTH)], shoup_mul(v[i], pl.c, pl.cs, ml.q), ml.q);
@@ -261,8 +276,8 @@ __global__ void __launch_bounds__(128 * NG, NG == 1 ? 5 : (NG == 2 ? 2 : 1)) con
     const RowDesc rd = p.rows[cg.tgt_start + t];
     const ModConst mc = p.mods[rd.mod];
     u64 v[8];
-    if (!MERGED && p.bc_f64 && (cg.pad[0] & 2) && mc.f64 && mc.q < (1ull << FENC_F64_MAX_BITS)) conv_dot_f64<T, NTH>(smem, n_conv, p.bc_f64 + rd.aux2, f64mod(mc.q, mc.f64), tid, v);
-    else conv_dot<T, NTH>(smem, n_conv, p.bc + rd.aux2, mc, p.max_terms, tid, v);
+    if (ydbl && mc.f64) conv_dot_f64<T, NTH>(smem, n_conv, p.bc_f64 + rd.aux2, f64mod(mc.q, mc.f64), mc.q < (1ull << FENC_F64_MAX_BITS) ? 255 : 7, tid, v);
+    else conv_dot<T, NTH>(smem, n_conv, p.bc + rd.aux2, mc, p.max_terms, tid, v, ydbl);
     if (MERGED) {
       const ShoupC pt = p.mulc[rd.mod];
 #pragma unroll
