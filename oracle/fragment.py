@@ -23,19 +23,33 @@ def next_pow2(x: int) -> int:
 class Layout:
     """Layout(n, M, S, BS, C): ciphertext (u, v, g, bg) holds at slot(cpos, k, b) the value
     X_pad[bg*B + b, g*ch + cpos, bi*S + u, bj*S + v], k = bi*m + bj  (PAPER.md:170-176 read
-    0-based with floors, A3; "filled first with other samples then other channels", PAPER.md:190)."""
+    0-based with floors, A3; "filled first with other samples then other channels", PAPER.md:190).
 
-    def __init__(self, n, M, S, BS, C):
+    Segmented form (v > 0; the layout AAC's canonical compaction produces, R2.11 / R2.11b): the chp
+    physical channel positions of a ciphertext are seg = chp / v segments of v positions; segment sg holds the v channels
+    g*v .. g*v + v - 1 of the samples of batch group bg*seg + sg, i.e. slot((sg*v + pl), k, b) holds
+    X_pad[(bg*seg + sg)*B + b, g*v + pl, ...].  ch is the number of channel positions of one segment (v); v = 0 or
+    v = chp is the plain layout (one segment).  Bcap > 0 caps the samples per ciphertext below "batch first"'s n/m^2
+    (B = min(BS^, n/m^2, Bcap)): then a large batch has several batch groups AND several channel positions per ciphertext,
+    which is where a channel-reducing layer leaves ciphertexts sparse and batch-group compaction (R2.11) applies."""
+
+    def __init__(self, n, M, S, BS, C, v=0, Bcap=0):
         assert M % S == 0
         self.n, self.M, self.S, self.BS, self.C = n, M, S, BS, C
         self.m = M // S
         m2 = self.m * self.m
         assert m2 <= n and n % m2 == 0, "m^2 must divide the slot count"
         self.B = min(next_pow2(BS), n // m2)
-        self.ch = n // (self.B * m2)
+        if Bcap:  # samples per ciphertext capped by the caller (a serving system's request size): channels fill the rest
+            self.B = min(self.B, Bcap)
+        self.chp = n // (self.B * m2)
+        self.v = v if v else self.chp
+        assert self.chp % self.v == 0, "the segment size must divide the channel positions"
+        self.seg = self.chp // self.v
+        self.ch = self.v
         self.cs = self.B * m2
         self.G = -(-C // self.ch)
-        self.BG = -(-BS // self.B)
+        self.BG = -(-(-(-BS // self.B)) // self.seg)
 
     def slot(self, cpos, k, b):
         return cpos * self.cs + k * self.B + b
@@ -43,53 +57,47 @@ class Layout:
     def ct_keys(self):
         return [(u, v, g, bg) for bg in range(self.BG) for g in range(self.G) for u in range(self.S) for v in range(self.S)]
 
+    def _entries(self, g, bg, BS, C, H, W, u, v):
+        """(slot, sample, channel, h, w) of every tensor entry ciphertext (u, v, g, bg) holds"""
+        for sg in range(self.seg):
+            for pl in range(self.ch):
+                c = g * self.ch + pl
+                if c >= C:
+                    continue
+                for b in range(self.B):
+                    bb = (bg * self.seg + sg) * self.B + b
+                    if bb >= BS:
+                        continue
+                    for bi in range(self.m):
+                        h = bi * self.S + u
+                        if h >= H:
+                            continue
+                        for bj in range(self.m):
+                            w = bj * self.S + v
+                            if w < W:
+                                yield self.slot(sg * self.ch + pl, bi * self.m + bj, b), bb, c, h, w
+
     def gather(self, X, u, v, g, bg):
         """Slot vector of ciphertext (u, v, g, bg) for X[BS, C, H, W] (zero outside the tensor)."""
         BS, C, H, W = X.shape
         vec = np.zeros(self.n, dtype=np.float64)
-        for cpos in range(self.ch):
-            c = g * self.ch + cpos
-            if c >= C:
-                continue
-            for b in range(self.B):
-                bb = bg * self.B + b
-                if bb >= BS:
-                    continue
-                for bi in range(self.m):
-                    h = bi * self.S + u
-                    if h >= H:
-                        continue
-                    for bj in range(self.m):
-                        w = bj * self.S + v
-                        if w < W:
-                            vec[self.slot(cpos, bi * self.m + bj, b)] = X[bb, c, h, w]
+        for sl, bb, c, h, w in self._entries(g, bg, BS, C, H, W, u, v):
+            vec[sl] = X[bb, c, h, w]
         return vec
 
     def scatter(self, Y, vec, u, v, g, bg):
         """Inverse of gather: write this ciphertext's entries into Y[BS, C, H, W]."""
         BS, C, H, W = Y.shape
-        for cpos in range(self.ch):
-            c = g * self.ch + cpos
-            if c >= C:
-                continue
-            for b in range(self.B):
-                bb = bg * self.B + b
-                if bb >= BS:
-                    continue
-                for bi in range(self.m):
-                    h = bi * self.S + u
-                    if h >= H:
-                        continue
-                    for bj in range(self.m):
-                        w = bj * self.S + v
-                        if w < W:
-                            Y[bb, c, h, w] = vec[self.slot(cpos, bi * self.m + bj, b)]
+        for sl, bb, c, h, w in self._entries(g, bg, BS, C, H, W, u, v):
+            Y[bb, c, h, w] = vec[sl]
 
 
 class ConvDesc:
-    def __init__(self, BS, C_in, H, W, C_out, K, stride=1, pad=0, depthwise=False, S=0, M=0):
+    def __init__(self, BS, C_in, H, W, C_out, K, stride=1, pad=0, depthwise=False, S=0, M=0, seg_v=0, Bcap=0):
         self.BS, self.C_in, self.H, self.W, self.C_out, self.K = BS, C_in, H, W, C_out, K
         self.stride, self.pad, self.depthwise, self.S, self.M = stride, pad, depthwise, S, M
+        self.seg_v = seg_v  # > 0: input and output ciphertexts in the segmented layout with v = seg_v (R2.11b)
+        self.Bcap = Bcap    # > 0: at most Bcap samples per ciphertext (Layout)
         self.H_out = (H + 2 * pad - K) // stride + 1
         self.W_out = (W + 2 * pad - K) // stride + 1
 
@@ -115,7 +123,13 @@ class ConvGraph:
     """Static operation graph of one fragment-encoded conv layer for one batch group.
 
     terms[(u_o, v_o, g_out)][d] = list of (src_key (u', v', g_in), amt, wkey (u_o, v_o, g_out, g_in, d, i, j));
-    inner = sorted set of (src_key, amt != 0); outer[(u_o, v_o, g_out)] = existing diagonals d."""
+    inner = sorted set of (src_key, amt != 0); outer[(u_o, v_o, g_out)] = existing diagonals d.
+
+    Segmented layouts (desc.seg_v = v > 0 with several segments, R2.11b: the consumer of AAC's output):
+    channel diagonal d must wrap inside each v-position segment, not around the whole ciphertext, so it splits in two
+    partial sums: part 0 holds the input positions pl >= d of every segment and is rotated by d*cs, part 1 the positions
+    pl < d and is rotated by (d - v)*cs (both masks folded into the weight plaintexts); the diagonal key is
+    dkey = d + part*chp (chp = physical channel positions), and diag_rot(dkey) is its outer rotation amount."""
 
     def __init__(self, desc: ConvDesc, n: int):
         d = desc
@@ -123,10 +137,11 @@ class ConvGraph:
         self.M = d.M if d.M else next_pow2(max(d.H, d.W))
         self.S = d.S
         assert self.S >= 1 and self.S % d.stride == 0, "stride must divide S"
-        self.lin = Layout(n, self.M, self.S, d.BS, d.C_in)
+        self.lin = Layout(n, self.M, self.S, d.BS, d.C_in, d.seg_v, d.Bcap)
         self.S_out = self.S // d.stride
-        self.lout = Layout(n, self.M // d.stride, self.S_out, d.BS, d.C_out)
+        self.lout = Layout(n, self.M // d.stride, self.S_out, d.BS, d.C_out, d.seg_v, d.Bcap)
         assert (self.lout.m, self.lout.B, self.lout.ch) == (self.lin.m, self.lin.B, self.lin.ch)
+        self.dkeys = list(range(self.lin.ch)) + ([self.lin.chp + dd for dd in range(1, self.lin.ch)] if self.lin.seg > 1 else [])
         self._wcache = {}
         self.terms, inner = {}, set()
         L = self.lin
@@ -134,7 +149,7 @@ class ConvGraph:
             for vo in range(self.S_out):
                 for go in range(self.lout.G):
                     diags = {}
-                    for dd in range(L.ch):
+                    for dd in self.dkeys:
                         lst = []
                         for gi in range(L.G):
                             for i in range(d.K):
@@ -162,14 +177,24 @@ class ConvGraph:
         key = ("c", go, gi, dd)
         if key not in self._wcache:
             d, L = self.desc, self.lin
+            part, dl = divmod(dd, L.chp) if L.seg > 1 else (0, dd)
             out = []
-            for cpos in range(L.ch):
-                c = gi * L.ch + cpos
-                o = go * L.ch + ((cpos - dd) % L.ch)
-                if c < d.C_in and o < d.C_out and (not d.depthwise or o == c):
-                    out.append((cpos, o, c))
+            for sg in range(L.seg):
+                for pl in range(L.ch):
+                    if L.seg > 1 and (pl >= dl) != (part == 0):
+                        continue  # part 0: the positions that stay inside their segment under a shift by dl; part 1: those that wrap
+                    c = gi * L.ch + pl
+                    o = go * L.ch + ((pl - dl) % L.ch)
+                    if c < d.C_in and o < d.C_out and (not d.depthwise or o == c):
+                        out.append((sg * L.ch + pl, o, c))
             self._wcache[key] = out
         return self._wcache[key]
+
+    def diag_rot(self, dd):
+        """outer rotation amount of diagonal key dd: d*cs, or (d - v)*cs for the wrapping part of a segmented layout"""
+        L = self.lin
+        part, dl = divmod(dd, L.chp) if L.seg > 1 else (0, dd)
+        return ((dl - L.ch) * L.cs) % self.n if part else (dl * L.cs) % self.n
 
     def _valid_blocks(self, frag_o, tap, size_in, size_out):
         """Block indices bi with h_o = bi*S_o + frag_o < size_out and 0 <= stride*h_o + tap - pad < size_in."""
@@ -256,8 +281,8 @@ class ConvGraph:
                         S = be.scale_acc(S, R[(src, amt)] if amt else inputs[src], values[wkey])
                     be.pmult_acc(acc, S, masks[mkey])
                 pd = be.wrap(acc)
-                if dd:
-                    pd = be.rot(pd, dd * self.lin.cs % self.n)
+                if self.diag_rot(dd):
+                    pd = be.rot(pd, self.diag_rot(dd))
                 y = pd if y is None else be.add(y, pd)
             out[okey] = y
         return out
@@ -267,10 +292,10 @@ class ConvGraph:
         n_outer = 0
         n_pmult = 0
         for diags in self.terms.values():
-            n_outer += len([x for x in diags if x != 0])  # every existing diagonal d != 0 is rotated once
+            n_outer += len([x for x in diags if self.diag_rot(x)])  # every existing diagonal d != 0 is rotated once
             n_pmult += sum(len(v) for v in diags.values())
         bg = self.lin.BG
-        steps = sorted({amt for _, amt in self.inner} | {dd * self.lin.cs % self.n for diags in self.terms.values() for dd in diags if dd})
+        steps = sorted({amt for _, amt in self.inner} | {self.diag_rot(dd) for diags in self.terms.values() for dd in diags if self.diag_rot(dd)})
         return dict(n_in_ct=self.S * self.S * self.lin.G * bg, n_out_ct=self.S_out ** 2 * self.lout.G * bg,
                     n_inner_rot=len(self.inner) * bg, n_outer_rot=n_outer * bg, n_pmult=n_pmult * bg,
                     n_distinct_pt=n_pmult, rot_steps=steps)
@@ -289,8 +314,8 @@ class ConvGraph:
                 for src, amt, wkey in diags[dd]:
                     be.pmult_acc(acc, R[(src, amt)] if amt else inputs[src], weights[wkey])
                 pd = be.wrap(acc)
-                if dd:
-                    pd = be.rot(pd, dd * self.lin.cs % self.n)
+                if self.diag_rot(dd):
+                    pd = be.rot(pd, self.diag_rot(dd))
                 y = pd if y is None else be.add(y, pd)
             out[okey] = y
         return out
@@ -383,7 +408,7 @@ def candidates(desc: ConvDesc, n):
 
 
 def with_S(desc: ConvDesc, S):
-    return ConvDesc(desc.BS, desc.C_in, desc.H, desc.W, desc.C_out, desc.K, desc.stride, desc.pad, desc.depthwise, S, desc.M)
+    return ConvDesc(desc.BS, desc.C_in, desc.H, desc.W, desc.C_out, desc.K, desc.stride, desc.pad, desc.depthwise, S, desc.M, desc.seg_v, desc.Bcap)
 
 
 def select_S(desc: ConvDesc, n):

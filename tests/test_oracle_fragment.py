@@ -304,3 +304,70 @@ def test_factored_weights_encrypted_decodes_to_convolution(kw, hoist):
             g.lout.scatter(Yp, ck.decrypt_decode(P, keys, op[k]).real, *k, bg)
     want = fr.direct_conv(d, x, w)
     assert np.abs(Yf - want).max() < 1e-3 and np.abs(Yf - Yp).max() < 1e-4 and differ
+
+
+# --------------------------------------------------------------------------- segmented layouts: the consumer of AAC's output (R2.11b)
+SEG_CASES = [
+    # (n, v, conv kwargs with Bcap): Fig. 5's shape 8 -> 2 -> 8: chp = 8, two valid channels, four sources per output
+    (128, 2, dict(BS=4, C_in=2, H=4, W=4, C_out=8, K=3, stride=1, pad=1, Bcap=1)),
+    (128, 2, dict(BS=7, C_in=2, H=4, W=4, C_out=5, K=1, stride=1, pad=0, Bcap=1)),      # ragged: 7 batch groups in 2 compressed ones, 5 channels
+    (256, 4, dict(BS=16, C_in=3, H=4, W=4, C_out=8, K=3, stride=1, pad=1, Bcap=2)),     # B=2, chp=8, v=4 (3 of 4 positions used), 8 groups
+    (256, 2, dict(BS=8, C_in=4, H=8, W=8, C_out=4, K=3, stride=2, pad=1, Bcap=4)),      # S=2: m=4, B=4, chp=4, two segments, two input groups
+]
+
+
+@pytest.mark.parametrize("n,v,kw", SEG_CASES)
+def test_segmented_consumer_on_plain_slots(n, v, kw):
+    """R2.11b: a convolution whose input (and output) ciphertexts are in the segmented layout AAC produces -- diagonal d
+    as two partial sums rotated by d*cs and (d - v)*cs -- equals direct convolution, and the canonical compaction of
+    plain-layout ciphertexts (R2.11) yields exactly that segmented layout."""
+    S = 2 if kw["stride"] == 2 else 1
+    d = fr.ConvDesc(S=S, seg_v=v, **kw)
+    shape = {k: val for k, val in kw.items() if k != "Bcap"}
+    x, w = wl.conv_inputs(11, shape)
+    assert np.abs(fr.hconv_slots(d, n, x, w) - fr.direct_conv(d, x, w)).max() < 1e-12
+    g = fr.ConvGraph(d, n)
+    assert g.lin.seg > 1 and g.lin.ch == v
+    # compress: plain-layout ciphertexts whose valid positions are [0, v) -> the segmented ciphertext (a rotation by r is
+    # a left shift, np.roll by -r)
+    plain = fr.Layout(n, g.M, S, kw["BS"], kw["C_in"], 0, kw["Bcap"])
+    if plain.G == 1 and kw["C_in"] <= v:  # the reducing layer left at most v channels in one group: the canonical plan applies
+        plan = fr.compress_plan(n, plain.chp, plain.cs, v, plain.BG)
+        for (u, vv, gi, t) in g.lin.ct_keys():
+            got = sum(np.roll(plain.gather(x, u, vv, 0, i), -r) for i, r in plan[t])
+            assert np.array_equal(got, g.lin.gather(x, u, vv, gi, t))
+    # rotation count: d = 0 plus two parts for each d in 1..v-1
+    assert all(len([k for k in diags if g.diag_rot(k)]) <= 2 * (v - 1) for diags in g.terms.values())
+
+
+def test_segmented_bottleneck_encrypted_fig5():
+    """Fig. 5 end to end on ciphertexts: reduce 8 -> 2 channels (1x1), compress four 25 %-full
+    ciphertexts into one, expand 2 -> 8 (3x3) on the segmented layout; decoded result = the two convolutions in fp64, and
+    the expansion reads 1 input ciphertext per compressed group instead of 4."""
+    P = ck.Params(8, 5, 40, 2, 60, 3, 40)
+    n, L = P.n, P.nq
+    red = dict(BS=4, C_in=8, H=4, W=4, C_out=2, K=1, stride=1, pad=0, Bcap=1)
+    exp = dict(BS=4, C_in=2, H=4, W=4, C_out=8, K=3, stride=1, pad=1, Bcap=1)
+    rng = np.random.default_rng(3)
+    x = rng.uniform(-1, 1, (4, 8, 4, 4))
+    w1, w2 = rng.normal(0, 0.3, (2, 8, 1, 1)), rng.normal(0, 0.3, (8, 2, 3, 3))
+    g1 = fr.ConvGraph(fr.ConvDesc(S=1, **red), n)
+    g2 = fr.ConvGraph(fr.ConvDesc(S=1, seg_v=2, **exp), n)
+    assert (g1.lin.chp, g1.lin.BG, g2.lin.seg, g2.lin.BG, g2.lout.G) == (8, 4, 4, 1, 4)
+    plan = fr.compress_plan(n, 8, g1.lin.cs, 2, 4)
+    steps = set(g1.counts()["rot_steps"]) | set(g2.counts()["rot_steps"]) | {r for tl in plan for _, r in tl if r}
+    keys = ck.keygen(P, 4, sorted(steps))
+    W1, W2 = fr.encode_weights(ck, P, g1, w1, L), fr.encode_weights(ck, P, g2, w2, L - 1)
+    mids = []
+    for bg in range(4):
+        ins = {(0, 0, gi): ck.encrypt(P, keys, ck.encode(P, g1.lin.gather(x, 0, 0, gi, bg), L), 40 + bg) for gi in range(g1.lin.G)}
+        mids.append(fr.hconv(ck, P, keys, g1, ins, W1)[(0, 0, 0)])
+    packed = fr.compress(ck, P, keys, plan, mids)
+    assert len(packed) == 1 and packed[0].L == L - 1
+    outs = fr.hconv(ck, P, keys, g2, {(0, 0, 0): packed[0]}, W2)
+    Y = np.zeros((4, 8, 4, 4))
+    for (uo, vo, go), y in outs.items():
+        g2.lout.scatter(Y, ck.decrypt_decode(P, keys, y).real, uo, vo, go, 0)
+    want = fr.direct_conv(fr.ConvDesc(**exp), fr.direct_conv(fr.ConvDesc(**red), x, w1), w2)
+    assert sum(len(tl) for tl in plan) == 4 and len(outs) == 4  # 4 sparse ciphertexts -> 1 dense one -> 4 dense outputs
+    assert np.abs(Y - want).max() < 1e-3
