@@ -76,12 +76,22 @@ typedef struct {
   int32_t depthwise;
   uint32_t S; /* fragment (block) size; 0 = Conv-aware selection (R2.10) */
   uint32_t M; /* square padded frame; 0 = next power of two >= max(H, W) (A4)             */
+  /* Segmented layout (R2.11b; the consumer of AAC's output): seg_v = v > 0 means the input
+   * AND output ciphertexts hold ch_phys / v segments of v channel positions, segment sg carrying the v channels of batch
+   * group bg*seg + sg -- the layout the canonical batch-group compaction (fenc_compress) produces.  Channel diagonal d
+   * then wraps inside a segment: two partial sums, rotated by d*cs and (d - v)*cs, masks folded into the weights.
+   * 0 (or ch_phys) = the plain layout. */
+  uint32_t seg_v;
+  /* cap on the samples per ciphertext, B = min(next_pow2(BS), (N/2)/m^2, B_cap); 0 = none ("batch first").
+   * With a cap a large batch has several batch groups and several channel positions per ciphertext. */
+  uint32_t B_cap;
 } fenc_conv_desc;
 
 /* Filled by fenc_layout_plan.  All counts are exact for the operation graph of DESIGN.md R2.9. */
 typedef struct {
   uint32_t S, S_out, M, M_out, m, B, ch, cs, G_in, G_out, BG, H_out, W_out;
   uint32_t n_in_ct, n_out_ct, n_inner_rot, n_outer_rot, n_pmult, n_distinct_pt, n_rot_keys;
+  uint32_t ch_phys, seg;             /* channel positions of a whole ciphertext; segments (ch_phys = seg * ch)              */
   double S_star_real;                /* (K^2 C_in BS / (alpha C_out))^(1/4): Eq. 8 with BS restored (A5) */
   double paper_rot_count;            /* #Rot as Table IX prints it (A6, A18)           */
   int32_t rot_steps[512];            /* the n_rot_keys distinct rotation amounts the layer needs          */

@@ -29,19 +29,19 @@ class Layout:
     physical channel positions of a ciphertext are seg = chp / v segments of v positions; segment sg holds the v channels
     g*v .. g*v + v - 1 of the samples of batch group bg*seg + sg, i.e. slot((sg*v + pl), k, b) holds
     X_pad[(bg*seg + sg)*B + b, g*v + pl, ...].  ch is the number of channel positions of one segment (v); v = 0 or
-    v = chp is the plain layout (one segment).  Bcap > 0 caps the samples per ciphertext below "batch first"'s n/m^2
-    (B = min(BS^, n/m^2, Bcap)): then a large batch has several batch groups AND several channel positions per ciphertext,
+    v = chp is the plain layout (one segment).  B_cap > 0 caps the samples per ciphertext below "batch first"'s n/m^2
+    (B = min(BS^, n/m^2, B_cap)): then a large batch has several batch groups AND several channel positions per ciphertext,
     which is where a channel-reducing layer leaves ciphertexts sparse and batch-group compaction (R2.11) applies."""
 
-    def __init__(self, n, M, S, BS, C, v=0, Bcap=0):
+    def __init__(self, n, M, S, BS, C, v=0, B_cap=0):
         assert M % S == 0
         self.n, self.M, self.S, self.BS, self.C = n, M, S, BS, C
         self.m = M // S
         m2 = self.m * self.m
         assert m2 <= n and n % m2 == 0, "m^2 must divide the slot count"
         self.B = min(next_pow2(BS), n // m2)
-        if Bcap:  # samples per ciphertext capped by the caller (a serving system's request size): channels fill the rest
-            self.B = min(self.B, Bcap)
+        if B_cap:  # samples per ciphertext capped by the caller (a serving system's request size): channels fill the rest
+            self.B = min(self.B, B_cap)
         self.chp = n // (self.B * m2)
         self.v = v if v else self.chp
         assert self.chp % self.v == 0, "the segment size must divide the channel positions"
@@ -93,11 +93,11 @@ class Layout:
 
 
 class ConvDesc:
-    def __init__(self, BS, C_in, H, W, C_out, K, stride=1, pad=0, depthwise=False, S=0, M=0, seg_v=0, Bcap=0):
+    def __init__(self, BS, C_in, H, W, C_out, K, stride=1, pad=0, depthwise=False, S=0, M=0, seg_v=0, B_cap=0):
         self.BS, self.C_in, self.H, self.W, self.C_out, self.K = BS, C_in, H, W, C_out, K
         self.stride, self.pad, self.depthwise, self.S, self.M = stride, pad, depthwise, S, M
         self.seg_v = seg_v  # > 0: input and output ciphertexts in the segmented layout with v = seg_v (R2.11b)
-        self.Bcap = Bcap    # > 0: at most Bcap samples per ciphertext (Layout)
+        self.B_cap = B_cap    # > 0: at most B_cap samples per ciphertext (Layout)
         self.H_out = (H + 2 * pad - K) // stride + 1
         self.W_out = (W + 2 * pad - K) // stride + 1
 
@@ -137,9 +137,9 @@ class ConvGraph:
         self.M = d.M if d.M else next_pow2(max(d.H, d.W))
         self.S = d.S
         assert self.S >= 1 and self.S % d.stride == 0, "stride must divide S"
-        self.lin = Layout(n, self.M, self.S, d.BS, d.C_in, d.seg_v, d.Bcap)
+        self.lin = Layout(n, self.M, self.S, d.BS, d.C_in, d.seg_v, d.B_cap)
         self.S_out = self.S // d.stride
-        self.lout = Layout(n, self.M // d.stride, self.S_out, d.BS, d.C_out, d.seg_v, d.Bcap)
+        self.lout = Layout(n, self.M // d.stride, self.S_out, d.BS, d.C_out, d.seg_v, d.B_cap)
         assert (self.lout.m, self.lout.B, self.lout.ch) == (self.lin.m, self.lin.B, self.lin.ch)
         self.dkeys = list(range(self.lin.ch)) + ([self.lin.chp + dd for dd in range(1, self.lin.ch)] if self.lin.seg > 1 else [])
         self._wcache = {}
@@ -408,7 +408,7 @@ def candidates(desc: ConvDesc, n):
 
 
 def with_S(desc: ConvDesc, S):
-    return ConvDesc(desc.BS, desc.C_in, desc.H, desc.W, desc.C_out, desc.K, desc.stride, desc.pad, desc.depthwise, S, desc.M, desc.seg_v, desc.Bcap)
+    return ConvDesc(desc.BS, desc.C_in, desc.H, desc.W, desc.C_out, desc.K, desc.stride, desc.pad, desc.depthwise, S, desc.M, desc.seg_v, desc.B_cap)
 
 
 def select_S(desc: ConvDesc, n):

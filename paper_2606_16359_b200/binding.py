@@ -32,7 +32,7 @@ class ParamsDesc(C.Structure):
 class ConvDesc(C.Structure):
     _fields_ = [("BS", C.c_uint32), ("C_in", C.c_uint32), ("H", C.c_uint32), ("W", C.c_uint32), ("C_out", C.c_uint32),
                 ("K", C.c_uint32), ("stride", C.c_uint32), ("pad", C.c_uint32), ("depthwise", C.c_int32),
-                ("S", C.c_uint32), ("M", C.c_uint32)]
+                ("S", C.c_uint32), ("M", C.c_uint32), ("seg_v", C.c_uint32), ("B_cap", C.c_uint32)]
 
 
 class FcDesc(C.Structure):
@@ -47,7 +47,7 @@ class FcInfo(C.Structure):
 class Layout(C.Structure):
     _fields_ = [(k, C.c_uint32) for k in ("S", "S_out", "M", "M_out", "m", "B", "ch", "cs", "G_in", "G_out", "BG",
                                           "H_out", "W_out", "n_in_ct", "n_out_ct", "n_inner_rot", "n_outer_rot",
-                                          "n_pmult", "n_distinct_pt", "n_rot_keys")] + \
+                                          "n_pmult", "n_distinct_pt", "n_rot_keys", "ch_phys", "seg")] + \
                [("S_star_real", C.c_double), ("paper_rot_count", C.c_double), ("rot_steps", C.c_int32 * 512)]
 
     def steps(self):
@@ -288,8 +288,8 @@ class Context:
         return int(self.lib.fenc_device_bytes(self.h))
 
     # ---- planner
-    def conv_desc(self, BS, C_in, H, W, C_out, K, stride=1, pad=0, depthwise=False, S=0, M=0):
-        return ConvDesc(BS, C_in, H, W, C_out, K, stride, pad, int(depthwise), S, M)
+    def conv_desc(self, BS, C_in, H, W, C_out, K, stride=1, pad=0, depthwise=False, S=0, M=0, seg_v=0, B_cap=0):
+        return ConvDesc(BS, C_in, H, W, C_out, K, stride, pad, int(depthwise), S, M, seg_v, B_cap)
 
     def layout_plan(self, conv):
         lay = Layout()

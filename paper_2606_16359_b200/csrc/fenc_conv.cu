@@ -38,7 +38,22 @@ struct LinGraph {
 struct ConvGraph : LinGraph {              // outs index: (g_out * S_out + u_o) * S_out + v_o
   fenc_conv_desc d;
   int n, M, S, S_out, m, B, ch, cs, G_in, G_out, H_out, W_out;
-  std::vector<std::array<u32, 7>> wkeys;      // (u_o, v_o, g_out, g_in, d, i, j) per weight plaintext
+  int chp = 0, seg = 1;  // physical channel positions of a ciphertext = seg segments of ch positions (R2.11b; seg = 1: plain)
+  std::vector<std::array<u32, 7>> wkeys;      // (u_o, v_o, g_out, g_in, dkey, i, j) per weight plaintext
+  // diagonal keys: d in [0, ch); in a segmented layout also chp + d (d >= 1), the part of diagonal d that wraps inside
+  // its segment (input positions pl < d, outer rotation (d - ch) cs instead of d cs)
+  std::vector<int> dkeys() const {
+    std::vector<int> k;
+    for (int dd = 0; dd < ch; dd++) k.push_back(dd);
+    if (seg > 1)
+      for (int dd = 1; dd < ch; dd++) k.push_back(chp + dd);
+    return k;
+  }
+  int diag_rot(int dkey) const {
+    const int part = seg > 1 ? dkey / chp : 0, dl = seg > 1 ? dkey % chp : dkey;
+    const long r = part ? (long)(dl - ch) * cs : (long)dl * cs;
+    return (int)(((r % n) + n) % n);
+  }
   // factored form (R2.9c), built on first use: a weight plaintext with ONE valid channel position is value x mask
   struct Mask { int cpos; std::vector<int> rows, cols; };
   bool factors_built = false, factorable = false;
@@ -76,12 +91,15 @@ struct ConvGraph : LinGraph {              // outs index: (g_out * S_out + u_o) 
       }
   }
   // R2.9 step 2: the validity conditions factorise into channel positions, block rows and block columns
-  std::vector<std::array<int, 3>> valid_cpos(int go, int gi, int dd) const {
+  std::vector<std::array<int, 3>> valid_cpos(int go, int gi, int dkey) const {  // (physical position, o, c)
     std::vector<std::array<int, 3>> v;
-    for (int cpos = 0; cpos < ch; cpos++) {
-      int c = gi * ch + cpos, o = go * ch + (((cpos - dd) % ch + ch) % ch);
-      if (c < (int)d.C_in && o < (int)d.C_out && (!d.depthwise || o == c)) v.push_back({cpos, o, c});
-    }
+    const int part = seg > 1 ? dkey / chp : 0, dl = seg > 1 ? dkey % chp : dkey;
+    for (int sg = 0; sg < seg; sg++)
+      for (int pl = 0; pl < ch; pl++) {
+        if (seg > 1 && (pl >= dl) != (part == 0)) continue;  // part 0 stays inside its segment under a shift by dl, part 1 wraps
+        int c = gi * ch + pl, o = go * ch + (((pl - dl) % ch + ch) % ch);
+        if (c < (int)d.C_in && o < (int)d.C_out && (!d.depthwise || o == c)) v.push_back({sg * ch + pl, o, c});
+      }
     return v;
   }
   std::vector<int> valid_blocks(int frag_o, int tap, int size_in, int size_out) const {
@@ -112,8 +130,8 @@ struct ConvGraph : LinGraph {              // outs index: (g_out * S_out + u_o) 
 
 static fenc_status build_graph(fenc_ctx *ctx, const fenc_conv_desc *cd, int S, std::shared_ptr<ConvGraph> &out) {
   char keybuf[256];
-  snprintf(keybuf, sizeof keybuf, "%u,%u,%u,%u,%u,%u,%u,%u,%d,%d,%u", cd->BS, cd->C_in, cd->H, cd->W, cd->C_out, cd->K,
-           cd->stride, cd->pad, cd->depthwise, S, cd->M);
+  snprintf(keybuf, sizeof keybuf, "%u,%u,%u,%u,%u,%u,%u,%u,%d,%d,%u,%u,%u", cd->BS, cd->C_in, cd->H, cd->W, cd->C_out, cd->K,
+           cd->stride, cd->pad, cd->depthwise, S, cd->M, cd->seg_v, cd->B_cap);
   auto it = ctx->graphs.find(keybuf);
   if (it != ctx->graphs.end()) {
     out = std::static_pointer_cast<ConvGraph>(it->second);
@@ -133,15 +151,21 @@ static fenc_status build_graph(fenc_ctx *ctx, const fenc_conv_desc *cd, int S, s
   const long m2 = (long)g->m * g->m;
   if (m2 > g->n || g->n % m2) return fail(ctx, FENC_ERR_LAYOUT, "m^2=%ld does not fit %d slots", m2, g->n);
   g->B = (int)std::min<long>(next_pow2(cd->BS), g->n / m2);
-  g->ch = (int)(g->n / (g->B * m2));
+  if (cd->B_cap) g->B = (int)std::min<long>(g->B, cd->B_cap);
+  if (g->B & (g->B - 1)) return fail(ctx, FENC_ERR_LAYOUT, "B_cap=%u must be a power of two", cd->B_cap);
+  g->chp = (int)(g->n / (g->B * m2));
+  g->ch = cd->seg_v ? (int)cd->seg_v : g->chp;
+  if (g->ch < 1 || g->chp % g->ch) return fail(ctx, FENC_ERR_LAYOUT, "segment size %d must divide the %d channel positions", g->ch, g->chp);
+  g->seg = g->chp / g->ch;
   g->cs = (int)(g->B * m2);
   g->G_in = (cd->C_in + g->ch - 1) / g->ch;
   g->G_out = (cd->C_out + g->ch - 1) / g->ch;
-  g->BG = (cd->BS + g->B - 1) / g->B;
+  g->BG = ((cd->BS + g->B - 1) / g->B + g->seg - 1) / g->seg;
   g->S_out = S / cd->stride;
   g->H_out = (cd->H + 2 * cd->pad - cd->K) / cd->stride + 1;
   g->W_out = (cd->W + 2 * cd->pad - cd->K) / cd->stride + 1;
-  const int K = cd->K, So = g->S_out, ch = g->ch;
+  const int K = cd->K, So = g->S_out;
+  const std::vector<int> dkeys = g->dkeys();
   std::set<std::pair<int, int>> inner;
   std::set<int> steps;
   g->outs.resize((size_t)g->G_out * So * So);
@@ -149,7 +173,7 @@ static fenc_status build_graph(fenc_ctx *ctx, const fenc_conv_desc *cd, int S, s
     for (int vo = 0; vo < So; vo++)
       for (int go = 0; go < g->G_out; go++) {
         OutCt &oc = g->outs[((size_t)go * So + uo) * So + vo];
-        for (int dd = 0; dd < ch; dd++) {
+        for (int dd : dkeys) {
           std::vector<Term> lst;
           for (int gi = 0; gi < g->G_in; gi++) {
             if (g->valid_cpos(go, gi, dd).empty()) continue;
@@ -171,10 +195,10 @@ static fenc_status build_graph(fenc_ctx *ctx, const fenc_conv_desc *cd, int S, s
           }
           if (!lst.empty()) {
             oc.diags.push_back(dd);
-            oc.rots.push_back((int)(((long)dd * g->cs) % g->n));
+            oc.rots.push_back(g->diag_rot(dd));
             oc.terms.push_back(std::move(lst));
             g->n_pmult += oc.terms.back().size();
-            if (dd) g->n_outer++, steps.insert((int)(((long)dd * g->cs) % g->n));
+            if (g->diag_rot(dd)) g->n_outer++, steps.insert(g->diag_rot(dd));
           }
         }
       }
@@ -228,6 +252,7 @@ extern "C" fenc_status fenc_layout_plan(fenc_ctx *ctx, const fenc_conv_desc *cd,
   memset(out, 0, sizeof *out);
   out->S = g->S, out->S_out = g->S_out, out->M = g->M, out->M_out = g->M / cd->stride, out->m = g->m, out->B = g->B;
   out->ch = g->ch, out->cs = g->cs, out->G_in = g->G_in, out->G_out = g->G_out, out->BG = g->BG;
+  out->ch_phys = g->chp, out->seg = g->seg;
   out->H_out = g->H_out, out->W_out = g->W_out;
   out->n_in_ct = g->S * g->S * g->G_in * g->BG;
   out->n_out_ct = g->S_out * g->S_out * g->G_out * g->BG;
@@ -257,22 +282,24 @@ extern "C" fenc_status fenc_encode_fragment(fenc_ctx *ctx, const fenc_conv_desc 
   if (u >= lay->S || v >= lay->S || group >= lay->G_in || bgi >= lay->BG) return fail(ctx, FENC_ERR_LAYOUT, "fragment index out of range");
   std::vector<double> vec(ctx->n, 0.0);
   const int m = lay->m, B = lay->B, S = lay->S;
-  for (u32 cpos = 0; cpos < lay->ch; cpos++) {
-    u32 c = group * lay->ch + cpos;
-    if (c >= cd->C_in) continue;
-    for (int b = 0; b < B; b++) {
-      u32 bb = bgi * B + b;
-      if (bb >= cd->BS) continue;
-      for (int bi = 0; bi < m; bi++) {
-        u32 h = bi * S + u;
-        if (h >= cd->H) continue;
-        for (int bj = 0; bj < m; bj++) {
-          u32 w = bj * S + v;
-          if (w < cd->W) vec[(size_t)cpos * lay->cs + (size_t)(bi * m + bj) * B + b] = x[(((size_t)bb * cd->C_in + c) * cd->H + h) * cd->W + w];
+  const u32 seg = lay->seg ? lay->seg : 1;
+  for (u32 sg = 0; sg < seg; sg++)
+    for (u32 pl = 0; pl < lay->ch; pl++) {
+      u32 c = group * lay->ch + pl;
+      if (c >= cd->C_in) continue;
+      for (int b = 0; b < B; b++) {
+        u32 bb = (bgi * seg + sg) * B + b;
+        if (bb >= cd->BS) continue;
+        for (int bi = 0; bi < m; bi++) {
+          u32 h = bi * S + u;
+          if (h >= cd->H) continue;
+          for (int bj = 0; bj < m; bj++) {
+            u32 w = bj * S + v;
+            if (w < cd->W) vec[(size_t)(sg * lay->ch + pl) * lay->cs + (size_t)(bi * m + bj) * B + b] = x[(((size_t)bb * cd->C_in + c) * cd->H + h) * cd->W + w];
+          }
         }
       }
     }
-  }
   return fenc_encode_slots(ctx, vec.data(), nullptr, n_limbs, scale, out);
 }
 
@@ -287,22 +314,24 @@ extern "C" fenc_status fenc_decrypt_decode(fenc_ctx *ctx, const fenc_keys *K, co
   fenc_status st = fenc_decrypt_slots(ctx, K, ct, vec.data(), nullptr);
   if (st != FENC_OK) return st;
   const int m = lay->m, B = lay->B;
-  for (u32 cpos = 0; cpos < lay->ch; cpos++) {
-    u32 c = group * lay->ch + cpos;
-    if (c >= C) continue;
-    for (int b = 0; b < B; b++) {
-      u32 bb = bgi * B + b;
-      if (bb >= cd->BS) continue;
-      for (int bi = 0; bi < m; bi++) {
-        u32 h = bi * S + u;
-        if (h >= H) continue;
-        for (int bj = 0; bj < m; bj++) {
-          u32 w = bj * S + v;
-          if (w < W) y[(((size_t)bb * C + c) * H + h) * W + w] = vec[(size_t)cpos * lay->cs + (size_t)(bi * m + bj) * B + b];
+  const u32 seg = lay->seg ? lay->seg : 1;
+  for (u32 sg = 0; sg < seg; sg++)
+    for (u32 pl = 0; pl < lay->ch; pl++) {
+      u32 c = group * lay->ch + pl;
+      if (c >= C) continue;
+      for (int b = 0; b < B; b++) {
+        u32 bb = (bgi * seg + sg) * B + b;
+        if (bb >= cd->BS) continue;
+        for (int bi = 0; bi < m; bi++) {
+          u32 h = bi * S + u;
+          if (h >= H) continue;
+          for (int bj = 0; bj < m; bj++) {
+            u32 w = bj * S + v;
+            if (w < W) y[(((size_t)bb * C + c) * H + h) * W + w] = vec[(size_t)(sg * lay->ch + pl) * lay->cs + (size_t)(bi * m + bj) * B + b];
+          }
         }
       }
     }
-  }
   return FENC_OK;
 }
 
@@ -549,8 +578,8 @@ static fenc_status run_linear(fenc_ctx *ctx, const fenc_keys *K, const LinGraph 
   // ---- 2. MAC over every (bg, output, diagonal)
   size_t n_P = 0, n_rot_out = 0;
   for (auto &oc : g.outs) {
-    if (!(oc.diags.size() == 1 && oc.diags[0] == 0)) n_P += oc.diags.size();  // a lone diagonal 0 is summed in place
-    for (int d : oc.diags) n_rot_out += d != 0;
+    if (!(oc.diags.size() == 1 && oc.rots[0] == 0)) n_P += oc.diags.size();  // a lone unrotated diagonal is summed in place
+    for (int r : oc.rots) n_rot_out += r != 0;
   }
   std::vector<fenc_ct *> res(nout_bg * BG, nullptr);
   const double s_acc = s_in * W->scale;
@@ -572,7 +601,7 @@ static fenc_status run_linear(fenc_ctx *ctx, const fenc_keys *K, const LinGraph 
     for (size_t o = 0; o < nout_bg; o++) {
       const OutCt &oc = g.outs[o];
       u64 *Y = do_rescale ? Ybuf + (bg * nout_bg + o) * CT : res[bg * nout_bg + o]->d;
-      const bool single = oc.diags.size() == 1 && oc.diags[0] == 0;
+      const bool single = oc.diags.size() == 1 && oc.rots[0] == 0;
       for (size_t k = 0; k < oc.diags.size(); k++) {
         u64 *P = single ? Y : Pbuf + (pi++) * CT;
         auto ct_of = [&](const Term &t) { return t.amt ? Rbuf + (bg * n_inner + g.inner_index.at({t.src, t.amt})) * CT : in[bg * nin_bg + t.src]->d; };
@@ -587,7 +616,7 @@ static fenc_status run_linear(fenc_ctx *ctx, const fenc_keys *K, const LinGraph 
           job.outs.push_back(P);
         }
         if (single) continue;
-        if (oc.diags[k] == 0) sum_terms.push_back(P);
+        if (oc.rots[k] == 0) sum_terms.push_back(P);
         else {
           u64 *R = Obuf + (oi++) * CT;
           rot_in.push_back(P), rot_out.push_back(R), rot_step.push_back(oc.rots[k]);

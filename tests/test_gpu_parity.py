@@ -301,6 +301,68 @@ def test_factored_weights_need_one_channel_per_ciphertext(mods):
     ctx.close()
 
 
+@pytest.mark.parametrize("conv_kw,S,hoist", [
+    (dict(BS=4, C_in=2, H=4, W=4, C_out=8, K=3, stride=1, pad=1, seg_v=2, B_cap=4), 1, False),    # n=512: m=4, B=4, chp=8, 4 segments
+    (dict(BS=7, C_in=2, H=4, W=4, C_out=5, K=1, stride=1, pad=0, seg_v=2, B_cap=1), 1, False),    # chp=32, 16 segments, ragged
+    (dict(BS=16, C_in=3, H=8, W=8, C_out=8, K=3, stride=2, pad=1, seg_v=4, B_cap=2), 2, True),    # S=2, B=2, chp=16, v=4, two output groups, hoisted
+])
+def test_hconv_segmented_layout_bit_exact(mods, conv_kw, S, hoist):
+    """R2.11b: fenc_hconv over the segmented layout AAC's compaction produces (diagonal d as two partial sums rotated by
+    d*cs and (d - v)*cs), every limb against the oracle's graph, decoded against direct convolution."""
+    P, ctx = make(mods, "mid10")
+    err, lay = run_hconv(mods, P, ctx, conv_kw, S, seed=8, hoist=hoist)
+    assert lay.seg > 1 and lay.ch == conv_kw["seg_v"] and lay.ch_phys == lay.seg * lay.ch
+    assert err < 1e-3
+    ctx.close()
+
+
+def test_bottleneck_compress_then_segmented_conv_bit_exact(mods):
+    """Fig. 5 through the C ABI: reduce 8 -> 2 channels (1x1) on plain-layout ciphertexts, fenc_compress
+    the 25 %-full outputs of four batch groups into one dense ciphertext, expand 2 -> 8 (3x3) with fenc_hconv on the
+    segmented layout.  Every ciphertext of the chain equals the oracle's; the decoded result equals the two convolutions."""
+    ck, fr, fenc = mods
+    p = dict(wl.PARAMS["mid10"], log2N=8)
+    P = ck.Params(*wl.oracle_params_args(p))
+    ctx = fenc.Context(**p)
+    n, L = P.n, P.nq
+    red = dict(BS=4, C_in=8, H=4, W=4, C_out=2, K=1, stride=1, pad=0, B_cap=1)
+    exp = dict(BS=4, C_in=2, H=4, W=4, C_out=8, K=3, stride=1, pad=1, B_cap=1, seg_v=2)
+    rng = np.random.default_rng(3)
+    x = rng.uniform(-1, 1, (4, 8, 4, 4))
+    w1, w2 = rng.normal(0, 0.3, (2, 8, 1, 1)), rng.normal(0, 0.3, (8, 2, 3, 3))
+    g1, g2 = fr.ConvGraph(fr.ConvDesc(S=1, **red), n), fr.ConvGraph(fr.ConvDesc(S=1, **exp), n)
+    c1, c2 = ctx.conv_desc(S=1, **red), ctx.conv_desc(S=1, **exp)
+    l1, l2 = ctx.layout_plan(c1), ctx.layout_plan(c2)
+    assert (l1.ch, l1.BG, l2.seg, l2.BG, l2.G_out, l2.n_in_ct, l2.n_out_ct) == (8, 4, 4, 1, 4, 1, 4)
+    plan = fr.compress_plan(n, 8, g1.lin.cs, 2, 4)
+    steps = sorted(set(l1.steps()) | set(l2.steps()) | {r for tl in plan for _, r in tl if r})
+    assert set(l2.steps()) == set(g2.counts()["rot_steps"])
+    ok, gk = ck.keygen(P, 4, steps), ctx.keygen(4, steps)
+    W1, W2 = fr.encode_weights(ck, P, g1, w1, L), fr.encode_weights(ck, P, g2, w2, L - 1)
+    gW1 = ctx.conv_weights_from_coeffs(c1, l1, np.stack([W1[tuple(int(v) for v in k)].coeffs for k in ctx.wts_keys(c1, l1)]), L, float(P.q[L - 1]))
+    gW2 = ctx.conv_weights_from_coeffs(c2, l2, np.stack([W2[tuple(int(v) for v in k)].coeffs for k in ctx.wts_keys(c2, l2)]), L - 1, float(P.q[L - 2]))
+    o_mid, g_in = [], []
+    for bg in range(4):
+        pt = ck.encode(P, g1.lin.gather(x, 0, 0, 0, bg), L)
+        o_mid.append(fr.hconv(ck, P, ok, g1, {(0, 0, 0): ck.encrypt(P, ok, pt, 40 + bg)}, W1)[(0, 0, 0)])
+        g_in.append(ctx.encrypt(gk, ctx.pt_from_coeffs(pt.coeffs, L, float(pt.scale)), 40 + bg))
+    g_mid = ctx.hconv(gk, c1, l1, gW1, g_in)
+    for a, b in zip(g_mid, o_mid):
+        assert np.array_equal(ctx.ct_export(a), b.c)
+    o_packed = fr.compress(ck, P, ok, plan, o_mid)
+    g_packed = ctx.compress(gk, g_mid, [(t, i, r) for t, tl in enumerate(plan) for i, r in tl], len(plan))
+    assert len(g_packed) == 1 and np.array_equal(ctx.ct_export(g_packed[0]), o_packed[0].c)
+    o_out = fr.hconv(ck, P, ok, g2, {(0, 0, 0): o_packed[0]}, W2)
+    g_out = ctx.hconv(gk, c2, l2, gW2, g_packed)
+    Y = np.zeros((4, 8, 4, 4))
+    for go in range(4):
+        assert np.array_equal(ctx.ct_export(g_out[go]), o_out[(0, 0, go)].c), go
+        ctx.decrypt_decode(gk, g_out[go], c2, l2, 1, 0, 0, go, 0, Y)
+    want = fr.direct_conv(fr.ConvDesc(**exp), fr.direct_conv(fr.ConvDesc(**red), x, w1), w2)
+    assert np.abs(Y - want).max() < 1e-3
+    ctx.close()
+
+
 def test_hconv_fig4_toy(mods):
     """PAPER.md:160 (Fig. 4): input 1x16x4x4, conv(16,16,3,1), 16-slot ciphertexts, S in {1,2,4}."""
     ck, fr, fenc = mods

@@ -308,11 +308,11 @@ def test_factored_weights_encrypted_decodes_to_convolution(kw, hoist):
 
 # --------------------------------------------------------------------------- segmented layouts: the consumer of AAC's output (R2.11b)
 SEG_CASES = [
-    # (n, v, conv kwargs with Bcap): Fig. 5's shape 8 -> 2 -> 8: chp = 8, two valid channels, four sources per output
-    (128, 2, dict(BS=4, C_in=2, H=4, W=4, C_out=8, K=3, stride=1, pad=1, Bcap=1)),
-    (128, 2, dict(BS=7, C_in=2, H=4, W=4, C_out=5, K=1, stride=1, pad=0, Bcap=1)),      # ragged: 7 batch groups in 2 compressed ones, 5 channels
-    (256, 4, dict(BS=16, C_in=3, H=4, W=4, C_out=8, K=3, stride=1, pad=1, Bcap=2)),     # B=2, chp=8, v=4 (3 of 4 positions used), 8 groups
-    (256, 2, dict(BS=8, C_in=4, H=8, W=8, C_out=4, K=3, stride=2, pad=1, Bcap=4)),      # S=2: m=4, B=4, chp=4, two segments, two input groups
+    # (n, v, conv kwargs with B_cap): Fig. 5's shape 8 -> 2 -> 8: chp = 8, two valid channels, four sources per output
+    (128, 2, dict(BS=4, C_in=2, H=4, W=4, C_out=8, K=3, stride=1, pad=1, B_cap=1)),
+    (128, 2, dict(BS=7, C_in=2, H=4, W=4, C_out=5, K=1, stride=1, pad=0, B_cap=1)),      # ragged: 7 batch groups in 2 compressed ones, 5 channels
+    (256, 4, dict(BS=16, C_in=3, H=4, W=4, C_out=8, K=3, stride=1, pad=1, B_cap=2)),     # B=2, chp=8, v=4 (3 of 4 positions used), 8 groups
+    (256, 2, dict(BS=8, C_in=4, H=8, W=8, C_out=4, K=3, stride=2, pad=1, B_cap=4)),      # S=2: m=4, B=4, chp=4, two segments, two input groups
 ]
 
 
@@ -323,14 +323,14 @@ def test_segmented_consumer_on_plain_slots(n, v, kw):
     plain-layout ciphertexts (R2.11) yields exactly that segmented layout."""
     S = 2 if kw["stride"] == 2 else 1
     d = fr.ConvDesc(S=S, seg_v=v, **kw)
-    shape = {k: val for k, val in kw.items() if k != "Bcap"}
+    shape = {k: val for k, val in kw.items() if k != "B_cap"}
     x, w = wl.conv_inputs(11, shape)
     assert np.abs(fr.hconv_slots(d, n, x, w) - fr.direct_conv(d, x, w)).max() < 1e-12
     g = fr.ConvGraph(d, n)
     assert g.lin.seg > 1 and g.lin.ch == v
     # compress: plain-layout ciphertexts whose valid positions are [0, v) -> the segmented ciphertext (a rotation by r is
     # a left shift, np.roll by -r)
-    plain = fr.Layout(n, g.M, S, kw["BS"], kw["C_in"], 0, kw["Bcap"])
+    plain = fr.Layout(n, g.M, S, kw["BS"], kw["C_in"], 0, kw["B_cap"])
     if plain.G == 1 and kw["C_in"] <= v:  # the reducing layer left at most v channels in one group: the canonical plan applies
         plan = fr.compress_plan(n, plain.chp, plain.cs, v, plain.BG)
         for (u, vv, gi, t) in g.lin.ct_keys():
@@ -346,8 +346,8 @@ def test_segmented_bottleneck_encrypted_fig5():
     the expansion reads 1 input ciphertext per compressed group instead of 4."""
     P = ck.Params(8, 5, 40, 2, 60, 3, 40)
     n, L = P.n, P.nq
-    red = dict(BS=4, C_in=8, H=4, W=4, C_out=2, K=1, stride=1, pad=0, Bcap=1)
-    exp = dict(BS=4, C_in=2, H=4, W=4, C_out=8, K=3, stride=1, pad=1, Bcap=1)
+    red = dict(BS=4, C_in=8, H=4, W=4, C_out=2, K=1, stride=1, pad=0, B_cap=1)
+    exp = dict(BS=4, C_in=2, H=4, W=4, C_out=8, K=3, stride=1, pad=1, B_cap=1)
     rng = np.random.default_rng(3)
     x = rng.uniform(-1, 1, (4, 8, 4, 4))
     w1, w2 = rng.normal(0, 0.3, (2, 8, 1, 1)), rng.normal(0, 0.3, (8, 2, 3, 3))
