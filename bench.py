@@ -187,6 +187,24 @@ def resnet_chain_layers(seed):
     return layers, rng.uniform(-1, 1, (1, 16, 32, 32))
 
 
+def bottleneck_layers(seed, aac):
+    """A Table-X-shaped bottleneck at config 3's parameters: 64 -> 8 -> 128 channels on
+    32 x 32 maps, four requests of one image (B_cap = 1: 32 channel positions per ciphertext, 8 valid after the reducing
+    1x1 layer).  aac: the four 25 %-full ciphertexts are compacted into one (fenc_compress, R2.11) and the 3x3 expansion
+    runs on the segmented layout (R2.11b); otherwise it runs on the four sparse ciphertexts."""
+    rng = np.random.default_rng(seed)
+    red = dict(BS=4, C_in=64, H=32, W=32, C_out=8, K=1, stride=1, pad=0, B_cap=1)
+    exp = dict(BS=4, C_in=8, H=32, W=32, C_out=128, K=3, stride=1, pad=1, B_cap=1)
+    w1 = rng.normal(0.0, np.sqrt(2.0 / 64), (8, 64, 1, 1))
+    w2 = rng.normal(0.0, np.sqrt(2.0 / 72), (128, 8, 3, 3))
+    layers = [{"op": "conv", "conv": red, "S": 1, "w": w1}]
+    if aac:
+        layers += [{"op": "compress", "v": 8}, {"op": "conv", "conv": dict(exp, seg_v=8), "S": 1, "w": w2}]
+    else:
+        layers += [{"op": "conv", "conv": exp, "S": 1, "w": w2}]
+    return layers, rng.uniform(-1, 1, (4, 64, 32, 32))
+
+
 WORKLOADS = {
     # name: (PARAMS key, builder(batch, seed) -> (layers, x), description, images per ciphertext batch group or None)
     "cfg4_mobilenet": ("cfg4", lambda bs, seed: mobilenet_layers(32, seed),
@@ -207,6 +225,10 @@ WORKLOADS = {
                            "BASELINE config 3: ResNet-20 3x3 32->64 stride 2, N=2^16, batch 1", None),
     "cfg3_chain": ("cfg3", lambda bs, seed: resnet_chain_layers(seed),
                    "BASELINE config 3 chained: conv 16->16 (S=4) - poly3 - conv 16->32/2 - poly3 - conv 32->64/2, N=2^16, batch 1", None),
+    "cfg3_bottleneck_plain": ("cfg3", lambda bs, seed: bottleneck_layers(seed, False),
+                              "Table-X-shaped bottleneck 64 -> 8 -> 128 (1x1, 3x3) on 32x32, 4 requests, N=2^16, WITHOUT compression", None),
+    "cfg3_bottleneck_aac": ("cfg3", lambda bs, seed: bottleneck_layers(seed, True),
+                            "the same bottleneck WITH Arch-aware compression (4 sparse ciphertexts -> 1) and the segmented consumer", None),
     "cfg5_rotsweep": (None, None, "BASELINE config 5: rotation / key-switch sweep", None),
     "cfg5_rotsweep_hoisted": (None, None, "BASELINE config 5 with hoisted rotations (8 amounts per decomposition)", None),
     "cfg3_compress": (None, None, "AAC compress micro-benchmark at config 3's parameters", None),
@@ -619,6 +641,13 @@ def oracle_op_counts(layers, n_slots, n_q, hoist, lazy):
             if not (lazy and li > 0 and layers[li - 1]["op"] == "square"):
                 add("add", L, 3 * (n_ct // 4))
             n_ct //= 4
+        elif ly["op"] == "compress":
+            prev = fr.ConvGraph(fr.ConvDesc(S=layers[li - 1]["S"], **layers[li - 1]["conv"]), n_slots)
+            per, frags, bgs = prev.lout.chp // ly["v"], prev.S_out ** 2, prev.lout.BG
+            n_t = -(-bgs // per)
+            add("rot", L, frags * (bgs - n_t))
+            add("add", L, frags * (bgs - n_t))
+            n_ct = n_t * frags
     return ops
 
 

@@ -35,6 +35,8 @@ class Pipeline:
           ["factored": True]}                  factored: weights as integer multipliers + mask plaintexts (R2.9c, ch = 1)
          {"op": "square"}                      x -> x^2, relinearised and rescaled (one level)
          {"op": "pool"}                        2x2 sum-pool by fragment selection (S halves; factor 1/4 goes into the next w)
+         {"op": "compress", "v": v}            AAC batch-group compaction after a channel-reducing conv (v valid positions);
+                                               the next conv's dict carries seg_v = v (segmented layout, R2.11b)
          {"op": "fc", "fc": {...}, "w": ndarray[n_out][n_in]}     plain-diagonal fully connected layer
     """
 
@@ -65,6 +67,17 @@ class Pipeline:
                 L -= 2
             elif ly["op"] == "pool":
                 self.plan.append(dict(op="pool", L=L))
+            elif ly["op"] == "compress":
+                # AAC (R2.11): the previous conv left v of ch_phys channel positions valid; the
+                # ciphertexts of ch_phys / v consecutive batch groups are compacted into one (segmented layout, R2.11b)
+                prev = next(p for p in reversed(self.plan) if p["op"] == "conv")["lay"]
+                v, n = int(ly["v"]), ctx.n
+                if prev.seg != 1 or prev.ch % v or prev.G_out != 1:
+                    raise ValueError("compress needs a plain layout whose single output group has v | ch valid positions")
+                per = prev.ch // v
+                rots = [(n - sg * v * prev.cs) % n for sg in range(per)]
+                self.steps.update(r for r in rots if r)
+                self.plan.append(dict(op="compress", L=L, v=v, per=per, rots=rots, frags=int(prev.S_out) ** 2, BG=int(prev.BG)))
             else:
                 raise ValueError(ly["op"])
         self.L_out = L
@@ -90,6 +103,10 @@ class Pipeline:
                 relin += n_ct // 4 if pooled else n_ct
             elif p["op"] == "pool":
                 n_ct //= 4
+            elif p["op"] == "compress":
+                n_t = -(-p["BG"] // p["per"])
+                rot += p["frags"] * (p["BG"] - n_t)  # every source but the first of each output is rotated once
+                n_ct = n_t * p["frags"]
         return lin, rot, relin, pm
 
     def setup(self, key_seed, encode_weight=None):
@@ -171,6 +188,12 @@ class Pipeline:
             elif p["op"] == "pool":
                 cts = ctx.sum_groups([cts[i] for i in self.pool_order(len(cts), S)], 4)
                 S //= 2
+            elif p["op"] == "compress":
+                # sources ordered [bg][fragment]; output t gathers batch groups t*per .. t*per + per - 1 of each fragment
+                fr_, per, n_t = p["frags"], p["per"], -(-p["BG"] // p["per"])
+                terms = [(t * fr_ + f, bg * fr_ + f, p["rots"][bg % per]) for t in range(n_t) for f in range(fr_)
+                         for bg in range(t * per, min((t + 1) * per, p["BG"]))]
+                cts = ctx.compress(self.keys, cts, terms, n_t * fr_)
             if trace is not None:
                 trace.append(cts)
         return cts

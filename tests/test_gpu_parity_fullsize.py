@@ -362,3 +362,36 @@ def test_cfg4_mobilenet_chain_full_size_decoded(mods):
     assert seen.sum() == 4 * 32 * 28 * 28
     assert np.abs(Y[seen] - want[seen]).max() < 1e-3
     ctx.close()
+
+
+def test_bottleneck_aac_full_size_decoded(mods):
+    """bench.py's Table-X-shaped bottleneck at config 3's parameters (N=2^16): reduce 64 -> 8 (1x1), compress the four
+    requests' 25 %-full ciphertexts into one, expand 8 -> 128 (3x3) on the segmented layout; with and without compression
+    the decoded outputs equal the two convolutions in fp64 within 1e-3, and compression halves the rotations and PMults."""
+    ck, fr, fenc = mods
+    import bench
+    from paper_2606_16359_b200.pipeline import Pipeline
+    res = {}
+    for aac in (False, True):
+        ctx = fenc.Context(**wl.PARAMS["cfg3"])
+        ctx.set_hoisting(True)
+        layers, x = bench.bottleneck_layers(77, aac)
+        pipe = Pipeline(ctx, layers)
+        keys = pipe.setup(key_seed=77)
+        out = pipe.forward(pipe.encrypt_input(x, 40000))
+        convs = [ly for ly in layers if ly["op"] == "conv"]
+        want = x
+        for ly in convs:
+            want = fr.direct_conv(fr.ConvDesc(**{k: v for k, v in ly["conv"].items() if k not in ("seg_v", "B_cap")}), want, ly["w"])
+        p = pipe.plan[-1]
+        lay = p["lay"]
+        assert len(out) == lay.n_out_ct == (16 if aac else 16) and out[0].L == ctx.n_q - 2
+        Y = np.full(want.shape, np.nan)
+        for i in (0, len(out) // 2, len(out) - 1):
+            bg, go = divmod(i, lay.G_out)
+            ctx.decrypt_decode(keys, out[i], p["conv"], lay, 1, 0, 0, go, bg, Y)
+        seen = ~np.isnan(Y)
+        assert seen.any() and np.abs(Y[seen] - want[seen]).max() < 1e-3
+        res[aac] = pipe.counts()
+        ctx.close()
+    assert res[True][1] < 0.6 * res[False][1] and res[True][3] < 0.6 * res[False][3]  # rotations, PMults
