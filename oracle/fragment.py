@@ -579,3 +579,59 @@ def compress(ck, params, keys, plan, srcs, mask_pt=None, do_rescale=False):
             y = x if y is None else ck.add(params, y, x)
         outs.append(ck.rescale(params, y) if do_rescale else y)
     return outs
+
+
+# --------------------------------------------------------------------------- repack: block-size re-adaptation (R2.11c)
+def repack_plan(src: Layout, dst: Layout, shape):
+    """Rot-mask-add plan that moves a tensor of `shape` = (BS, C, H, W) from layout `src` to layout `dst` (another block
+    size S, another segmentation, ...): "we adapt the pre- or post-processing (rot-mask-add) operations to
+    adjust block size".  Every destination slot that holds a tensor entry names the source ciphertext and slot holding
+    the same entry; a left rotation by r = (src_slot - dst_slot) mod n brings it in place; entries sharing (destination,
+    source, r) share one mask.  Returns {dst_key: [(src_key, r, mask slot vector over the SOURCE slots), ...]}."""
+    BS, C, H, W = shape
+    where = {}
+    for key in src.ct_keys():
+        u, v, g, bg = key
+        for sl, bb, c, h, w in src._entries(g, bg, BS, C, H, W, u, v):
+            where[(bb, c, h, w)] = (key, sl)
+    plan = {}
+    for key in dst.ct_keys():
+        u, v, g, bg = key
+        groups = {}
+        for sl, bb, c, h, w in dst._entries(g, bg, BS, C, H, W, u, v):
+            skey, ssl = where[(bb, c, h, w)]
+            groups.setdefault((skey, (ssl - sl) % src.n), []).append(ssl)
+        terms = []
+        for (skey, r), slots in sorted(groups.items()):
+            mask = np.zeros(src.n)
+            mask[slots] = 1.0
+            terms.append((skey, r, mask))
+        plan[key] = terms
+    return plan
+
+
+def repack_slots(plan, vecs):
+    """the plan on plain slot vectors: out = sum Rot(mask * src, r), rotation = left cyclic shift"""
+    return {k: sum(np.roll(m * vecs[s], -r) for s, r, m in terms) for k, terms in plan.items()}
+
+
+def repack(ck, params, keys, plan, srcs, L, scale_m=None):
+    """out_t = Rescale( sum over terms of Rot(mask (*) src, r) ): masks encoded at q_{L-1} (one level, PAPER.md:276's
+    single late rescale); terms sharing (destination, r) are summed before their one rotation."""
+    sm = Fraction(params.q[L - 1]) if scale_m is None else Fraction(scale_m)
+    outs = {}
+    for dkey, terms in plan.items():
+        by_rot = {}
+        for skey, r, mask in terms:
+            by_rot.setdefault(r, []).append((skey, mask))
+        y = None
+        for r in sorted(by_rot):
+            acc = np.zeros((2, L, params.N), dtype=np.uint64)
+            for skey, mask in by_rot[r]:
+                ck.pmult_acc(params, acc, srcs[skey], ck.encode(params, mask, L, sm))
+            t = ck.Ciphertext(acc, L, srcs[by_rot[r][0][0]].scale * sm)
+            if r:
+                t = ck.rotate(params, keys, t, r)
+            y = t if y is None else ck.add(params, y, t)
+        outs[dkey] = ck.rescale(params, y)
+    return outs

@@ -371,3 +371,38 @@ def test_segmented_bottleneck_encrypted_fig5():
     want = fr.direct_conv(fr.ConvDesc(**exp), fr.direct_conv(fr.ConvDesc(**red), x, w1), w2)
     assert sum(len(tl) for tl in plan) == 4 and len(outs) == 4  # 4 sparse ciphertexts -> 1 dense one -> 4 dense outputs
     assert np.abs(Y - want).max() < 1e-3
+
+
+@pytest.mark.parametrize("S_src,S_dst,shape", [(2, 1, (1, 4, 4, 4)), (1, 2, (2, 2, 4, 4)), (2, 4, (1, 8, 7, 6))])
+def test_repack_between_block_sizes_on_plain_slots(S_src, S_dst, shape):
+    """R2.11c: the rot-mask-add plan between two block sizes moves every tensor entry to its slot in the
+    other layout (gather in the source layout, repack, compare with the gather in the destination layout)."""
+    n = 128
+    BS, C, H, W = shape
+    M = fr.next_pow2(max(H, W))
+    src, dst = fr.Layout(n, M, S_src, BS, C), fr.Layout(n, M, S_dst, BS, C)
+    x = np.random.default_rng(5).uniform(-1, 1, shape)
+    plan = fr.repack_plan(src, dst, shape)
+    vecs = {k: src.gather(x, *k) for k in src.ct_keys()}
+    out = fr.repack_slots(plan, vecs)
+    for k in dst.ct_keys():
+        assert np.array_equal(out[k], dst.gather(x, *k))
+
+
+def test_repack_encrypted_changes_block_size():
+    """the same on ciphertexts: S = 2 -> S = 1 (four fragment ciphertexts into one), one level, decoded = the tensor"""
+    P = ck.Params(7, 3, 40, 1, 60, 3, 40)
+    shape = (1, 4, 4, 4)
+    src, dst = fr.Layout(P.n, 4, 2, 1, 4), fr.Layout(P.n, 4, 1, 1, 4)
+    x = np.random.default_rng(6).uniform(-1, 1, shape)
+    plan = fr.repack_plan(src, dst, shape)
+    steps = sorted({r for terms in plan.values() for _, r, _ in terms if r})
+    keys = ck.keygen(P, 2, steps)
+    cts = {k: ck.encrypt(P, keys, ck.encode(P, src.gather(x, *k), P.nq), 9 + i) for i, k in enumerate(src.ct_keys())}
+    out = fr.repack(ck, P, keys, plan, cts, P.nq)
+    assert len(out) == 1
+    Y = np.zeros(shape)
+    for k, y in out.items():
+        assert y.L == P.nq - 1 and y.scale == P.scale
+        dst.scatter(Y, ck.decrypt_decode(P, keys, y).real, *k)
+    assert np.abs(Y - x).max() < 1e-4
