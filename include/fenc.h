@@ -118,6 +118,19 @@ fenc_status fenc_layout_plan(fenc_ctx *ctx, const fenc_conv_desc *conv, fenc_lay
 fenc_status fenc_keygen(fenc_ctx *ctx, uint64_t seed, const int32_t *rot_steps, size_t n_rot, int want_relin,
                         fenc_keys **out);
 void fenc_keys_free(fenc_keys *keys);
+/* Key material generated on the HOST and uploaded verbatim (north_star: "all key, encryption and error randomness generated
+ * on the host from a seed and uploaded"; R2.4): s[N] the secret's coefficients in {-1,0,1}; for key i
+ * (key_ids[i] = rotation amount in [1, N/2) or FENC_RELIN_KEY_ID) b[i] and a[i] are uint64 [beta_max][n_q+n_p][N],
+ * coefficient domain, canonical residues -- the format fenc_evk_export writes.  The library only transforms them to its
+ * device form (NTT domain, Montgomery); nothing is sampled.  All pointers are host memory, copied before returning. */
+typedef struct {
+  const int64_t *s;
+  size_t n_keys;
+  const int64_t *key_ids;
+  const uint64_t *const *b;
+  const uint64_t *const *a;
+} fenc_key_material;
+fenc_status fenc_keys_import(fenc_ctx *ctx, const fenc_key_material *mat, fenc_keys **out);
 /* host s[N]: the secret's coefficients in {-1,0,1} */
 fenc_status fenc_secret_export(fenc_ctx *ctx, const fenc_keys *keys, int64_t *s);
 /* key_id = rotation amount in [1, N/2) or FENC_RELIN_KEY_ID.  host b, a: uint64 [beta_max][n_q+n_p][N],
@@ -196,6 +209,22 @@ fenc_status fenc_add_const(fenc_ctx *ctx, fenc_ct *const *in, size_t n, const ui
 /* out[g] = sum_{i < group} in[g*group + i] for g < n_groups: avg-pool by fragment selection (a14; PAPER.md:284;
  * the 1/group^2 factor belongs to the next layer's weights, R2.12).  No rotations, no level consumed. */
 fenc_status fenc_sum_groups(fenc_ctx *ctx, fenc_ct *const *in, size_t group, size_t n_groups, fenc_ct **out);
+
+/* 2x2 sum-pool by fragment selection with the fragment order owned by the library (a14; R2.12): in holds
+ * n ciphertexts ordered [...][u][v] with S x S fragments per (batch group, channel group), S even; out receives n/4
+ * ciphertexts ordered [...][u_o][v_o], out(u_o, v_o) = sum_{a,b in {0,1}} in(2 u_o + a, 2 v_o + b). */
+fenc_status fenc_sum_pool(fenc_ctx *ctx, fenc_ct *const *in, size_t n, uint32_t S, fenc_ct **out);
+/* x^2 followed by that pool with ONE relinearisation per pooled output (R2.12c): fenc_square_sum_relin over the four
+ * fragments of every output, same ordering as fenc_sum_pool. */
+fenc_status fenc_square_sum_pool(fenc_ctx *ctx, const fenc_keys *keys, fenc_ct *const *in, size_t n, uint32_t S, fenc_ct **out);
+/* Degree-3 activation a0 + a1 x + a3 x^3 in two levels (a13; R2.12), every step batched over the n
+ * inputs (level L, scale s): x2 = Rescale(Relin(x x)); t = Rescale(k3 x) with k3 = round_half_up(a3 q_{L-1});
+ * x3 = Rescale(Relin(x2 t)) at scale s3 = s^3 / (q_{L-1} q_{L-2}); u = Rescale(Rescale(k1 x)) with k1 = round_half_up(a1 s^2);
+ * out = x3 + u + k0 on coefficient 0 of c0, k0 = round_half_up(a0 s3).  The three integers are rounded exactly by the
+ * caller from the exact rational scale (R2.8) and passed as residues: host k3_res[L], k1_res[L], k0_res[L-2];
+ * scale_sq = s^2 as a double (bookkeeping of the output scale only).  out: n ciphertexts at L-2. */
+fenc_status fenc_poly3(fenc_ctx *ctx, const fenc_keys *keys, fenc_ct *const *in, size_t n, const uint64_t *k3_res,
+                       const uint64_t *k1_res, const uint64_t *k0_res, double scale_sq, fenc_ct **out);
 
 /* ------------------------------------------------------------------ HConv (R2.9) */
 /* Number of distinct non-zero weight plaintexts of the layer and their keys (u_o, v_o, g_out, g_in, d, i, j). */
@@ -299,6 +328,17 @@ fenc_status fenc_rotate_hoisted(fenc_ctx *ctx, const fenc_keys *keys, fenc_ct *c
 fenc_status fenc_compress(fenc_ctx *ctx, const fenc_keys *keys, fenc_ct *const *in, size_t n_in, const fenc_pt *mask,
                           const uint32_t *term_out, const uint32_t *term_src, const int32_t *term_rot, size_t n_terms,
                           int do_rescale, fenc_ct **out, size_t n_out);
+
+/* Repack (R2.11c; "we adapt the pre- or post-processing (rot-mask-add) operations to adjust block
+ * size"): the general rot-mask-add with one mask per term,
+ *   out[t] = Rescale( sum over the terms i with term_out[i] == t of Rot(masks[i] (*) in[term_src[i]], term_rot[i]) ),
+ * terms sharing (output, amount) are summed before their one rotation.  masks: host array of n_terms plaintext handles at
+ * the inputs' level, all at one scale (q_{L-1} keeps the ciphertext scale: one level).  It moves a tensor
+ * between two layouts (another block size S, another segmentation); the plan is the caller's (oracle/fragment.py
+ * repack_plan states the one the tests use).  do_rescale = 0 leaves the sum at scale s_ct * s_mask. */
+fenc_status fenc_repack(fenc_ctx *ctx, const fenc_keys *keys, fenc_ct *const *in, size_t n_in, fenc_pt *const *masks,
+                        const uint32_t *term_out, const uint32_t *term_src, const int32_t *term_rot, size_t n_terms,
+                        int do_rescale, fenc_ct **out, size_t n_out);
 
 /* ------------------------------------------------------------------ measurement helpers */
 /* Raw batched negacyclic NTT / iNTT (a1) in place on device memory: rows uint64 [n_rows][N]; mod_idx: host

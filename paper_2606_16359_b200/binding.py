@@ -35,6 +35,11 @@ class ConvDesc(C.Structure):
                 ("S", C.c_uint32), ("M", C.c_uint32), ("seg_v", C.c_uint32), ("B_cap", C.c_uint32)]
 
 
+class KeyMaterial(C.Structure):
+    _fields_ = [("s", C.POINTER(C.c_int64)), ("n_keys", C.c_size_t), ("key_ids", C.POINTER(C.c_int64)),
+                ("b", C.POINTER(C.POINTER(C.c_uint64))), ("a", C.POINTER(C.POINTER(C.c_uint64)))]
+
+
 class FcDesc(C.Structure):
     _fields_ = [(k, C.c_uint32) for k in ("BS", "n_in", "n_out", "in_C", "in_H", "in_W", "in_M", "bsgs")]
 
@@ -67,7 +72,7 @@ SYMBOLS = ["fenc_params_init", "fenc_ctx_free", "fenc_last_error", "fenc_get_pri
            "fenc_cmult_relin", "fenc_mul_scalar", "fenc_add_const", "fenc_ct_import_async", "fenc_ct_export_async",
            "fenc_export_wait", "fenc_set_hoisting", "fenc_rotate_hoisted", "fenc_square_sum_relin",
            "fenc_wts_factors", "fenc_wts_mask_slots", "fenc_conv_weights_factored", "fenc_conv_weights_factored_from_ints",
-           "fenc_measure_smac_peak"]
+           "fenc_measure_smac_peak", "fenc_repack", "fenc_keys_import", "fenc_sum_pool", "fenc_square_sum_pool", "fenc_poly3"]
 
 _lib = None
 
@@ -138,6 +143,11 @@ def load_library(path=None):
         "fenc_fc": [vp, vp, C.POINTER(FcDesc), vp, vpp, C.c_size_t, C.c_int, vpp, C.c_size_t, C.POINTER(C.c_size_t)],
         "fenc_compress": [vp, vp, vpp, C.c_size_t, vp, u32p, u32p, i32p, C.c_size_t, C.c_int, vpp, C.c_size_t],
         "fenc_ntt_rows": [vp, vp, i32p, C.c_size_t, C.c_int],
+        "fenc_keys_import": [vp, C.POINTER(KeyMaterial), vpp],
+        "fenc_sum_pool": [vp, vpp, C.c_size_t, C.c_uint32, vpp],
+        "fenc_square_sum_pool": [vp, vp, vpp, C.c_size_t, C.c_uint32, vpp],
+        "fenc_poly3": [vp, vp, vpp, C.c_size_t, u64p, u64p, u64p, C.c_double, vpp],
+        "fenc_repack": [vp, vp, vpp, C.c_size_t, vpp, u32p, u32p, i32p, C.c_size_t, C.c_int, vpp, C.c_size_t],
     }
     for name, args in sig.items():
         f = getattr(lib, name)
@@ -301,6 +311,20 @@ class Context:
         steps = np.asarray(list(rot_steps), dtype=np.int32)
         h = C.c_void_p()
         self._ck(self.lib.fenc_keygen(self.h, C.c_uint64(seed), _ptr(steps, C.c_int32), len(steps), int(want_relin), C.byref(h)))
+        return Keys(self, h)
+
+    def keys_import(self, s, evk):
+        """host-generated key material uploaded verbatim: s int64[N] in {-1,0,1}; evk {key id: (b, a)} with b, a uint64
+        [beta_max][n_q+n_p][N], coefficient domain (the format evk_export returns)"""
+        s = np.ascontiguousarray(s, dtype=np.int64)
+        ids = np.array(sorted(evk), dtype=np.int64)
+        bs = [np.ascontiguousarray(evk[int(i)][0], dtype=np.uint64) for i in ids]
+        as_ = [np.ascontiguousarray(evk[int(i)][1], dtype=np.uint64) for i in ids]
+        PP = C.POINTER(C.c_uint64)
+        mat = KeyMaterial(_ptr(s, C.c_int64), len(ids), _ptr(ids, C.c_int64) if len(ids) else None,
+                          (PP * len(ids))(*[_ptr(x, C.c_uint64) for x in bs]), (PP * len(ids))(*[_ptr(x, C.c_uint64) for x in as_]))
+        h = C.c_void_p()
+        self._ck(self.lib.fenc_keys_import(self.h, C.byref(mat), C.byref(h)))
         return Keys(self, h)
 
     def secret_export(self, keys):
@@ -480,6 +504,25 @@ class Context:
         self._ck(self.lib.fenc_sum_groups(self.h, self._harr(cts), group, n, out))
         return [Ciphertext(self, C.c_void_p(out[i])) for i in range(n)]
 
+    def sum_pool(self, cts, S):
+        out = (C.c_void_p * (len(cts) // 4))()
+        self._ck(self.lib.fenc_sum_pool(self.h, self._harr(cts), len(cts), int(S), out))
+        return [Ciphertext(self, C.c_void_p(out[i])) for i in range(len(cts) // 4)]
+
+    def square_sum_pool(self, keys, cts, S):
+        out = (C.c_void_p * (len(cts) // 4))()
+        self._ck(self.lib.fenc_square_sum_pool(self.h, keys.h, self._harr(cts), len(cts), int(S), out))
+        return [Ciphertext(self, C.c_void_p(out[i])) for i in range(len(cts) // 4)]
+
+    def poly3(self, keys, cts, k3, k1, k0, scale_sq):
+        """the three exactly rounded integers of the degree-3 activation (fenc.h fenc_poly3), as Python ints"""
+        L = cts[0].L
+        r3, r1, r0 = self._residues(k3, L), self._residues(k1, L), self._residues(k0, L - 2)
+        out = (C.c_void_p * len(cts))()
+        self._ck(self.lib.fenc_poly3(self.h, keys.h, self._harr(cts), len(cts), _ptr(r3, C.c_uint64), _ptr(r1, C.c_uint64),
+                                     _ptr(r0, C.c_uint64), float(scale_sq), out))
+        return [Ciphertext(self, C.c_void_p(out[i])) for i in range(len(cts))]
+
     def measure_alu_peak(self):
         a, b = C.c_double(), C.c_double()
         self._ck(self.lib.fenc_measure_alu_peak(self.h, C.byref(a), C.byref(b)))
@@ -614,6 +657,16 @@ class Context:
         return [Ciphertext(self, C.c_void_p(out[i])) for i in range(n_out)]
 
     # ---- raw NTT on a torch tensor of uint64 rows (viewed as int64 by torch)
+    def repack(self, keys, cts, terms, n_out, do_rescale=True):
+        """terms: list of (output index, source index, rotation amount, mask Plaintext) -- rot-mask-add (R2.11c)"""
+        to = np.array([t[0] for t in terms], dtype=np.uint32)
+        ts = np.array([t[1] for t in terms], dtype=np.uint32)
+        tr = np.array([t[2] for t in terms], dtype=np.int32)
+        out = (C.c_void_p * n_out)()
+        self._ck(self.lib.fenc_repack(self.h, keys.h, self._harr(cts), len(cts), self._harr([t[3] for t in terms]),
+                                      _ptr(to, C.c_uint32), _ptr(ts, C.c_uint32), _ptr(tr, C.c_int32), len(terms), int(do_rescale), out, n_out))
+        return [Ciphertext(self, C.c_void_p(out[i])) for i in range(n_out)]
+
     def ntt_rows(self, tensor, mod_idx, inverse=False):
         m = np.asarray(list(mod_idx), dtype=np.int32)
         assert tensor.is_cuda and tensor.is_contiguous() and tensor.numel() == len(m) * self.N

@@ -748,6 +748,89 @@ extern "C" fenc_status fenc_compress(fenc_ctx *ctx, const fenc_keys *K, fenc_ct 
   return FENC_OK;
 }
 
+// ------------------------------------------------------------------------------------------------ repack (R2.11c)
+// out[t] = Rescale( sum_i Rot(mask_i (*) in[src_i], r_i) ): one MAC launch for all (output, amount) groups, one batch of
+// rotations, one sum kernel, one rescale batch.
+extern "C" fenc_status fenc_repack(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const *in, size_t n_in, fenc_pt *const *masks,
+                                   const uint32_t *term_out, const uint32_t *term_src, const int32_t *term_rot, size_t n_terms,
+                                   int do_rescale, fenc_ct **out, size_t n_out) {
+  Scope sc(ctx);
+  if (!ctx || !K || !in || !masks || !term_out || !term_src || !term_rot || !out || n_in == 0 || n_out == 0 || n_terms == 0)
+    return FENC_ERR_INVALID_ARG;
+  const int L = in[0]->L;
+  const double s_in = in[0]->scale;
+  for (size_t i = 0; i < n_in; i++)
+    if (in[i]->L != L || std::fabs(in[i]->scale - s_in) > 1e-9 * s_in) return fail(ctx, FENC_ERR_MISMATCH, "sources differ in level or scale");
+  if (do_rescale && L < 2) return fail(ctx, FENC_ERR_LEVEL, "no level left to rescale");
+  const double s_m = masks[0] ? masks[0]->scale : 0;
+  std::map<std::pair<u32, int>, std::vector<size_t>> groups;  // (output, amount) -> terms
+  for (size_t i = 0; i < n_terms; i++) {
+    if (term_out[i] >= n_out || term_src[i] >= n_in || !masks[i]) return fail(ctx, FENC_ERR_INVALID_ARG, "repack term %zu out of range", i);
+    if (masks[i]->L != L || std::fabs(masks[i]->scale - s_m) > 1e-9 * s_m) return fail(ctx, FENC_ERR_MISMATCH, "masks differ in level or scale");
+    fenc_status st = pt_device(ctx, masks[i]);
+    if (st != FENC_OK) return st;
+    groups[{term_out[i], ((term_rot[i] % ctx->n) + ctx->n) % ctx->n}].push_back(i);
+  }
+  std::vector<int> cnt(n_out, 0);
+  for (auto &kv : groups) cnt[kv.first.first]++;
+  for (size_t t = 0; t < n_out; t++)
+    if (!cnt[t]) return fail(ctx, FENC_ERR_INVALID_ARG, "repack output %zu has no term", t);
+  const size_t N = ctx->N, CT = (size_t)2 * L * N, ng = groups.size();
+  const double s_acc = s_in * s_m;
+  u64 *Gbuf = sc.alloc<u64>(ng * CT), *Rbuf = sc.alloc<u64>(ng * CT);
+  u64 *Ybuf = do_rescale ? sc.alloc<u64>(n_out * CT) : nullptr;
+  if (!Gbuf || !Rbuf || (do_rescale && !Ybuf)) return fail(ctx, FENC_ERR_OOM, "repack workspace");
+  std::vector<fenc_ct *> res(n_out);
+  for (size_t t = 0; t < n_out; t++) {
+    res[t] = sc.ct(do_rescale ? L - 1 : L, do_rescale ? s_acc / (double)ctx->mod[L - 1] : s_acc);
+    if (!res[t]) return fail(ctx, FENC_ERR_OOM, "repack outputs");
+  }
+  MacJob job;
+  std::vector<const u64 *> rin, sum_terms;
+  std::vector<u64 *> rout, sum_out;
+  std::vector<int> rstep, sum_start{0};
+  size_t gi = 0;
+  u32 cur = groups.begin()->first.first;
+  for (auto &kv : groups) {  // ordered by output, then amount
+    if (kv.first.first != cur) sum_start.push_back((int)sum_terms.size()), sum_out.push_back(do_rescale ? Ybuf + cur * CT : res[cur]->d), cur = kv.first.first;
+    u64 *G = Gbuf + gi * CT;
+    job.terms.emplace_back();
+    for (size_t i : kv.second) job.terms.back().push_back({in[term_src[i]]->d, masks[i]->d_mont});
+    job.outs.push_back(G);
+    if (kv.first.second) {
+      rin.push_back(G), rout.push_back(Rbuf + gi * CT), rstep.push_back(kv.first.second);
+      sum_terms.push_back(Rbuf + gi * CT);
+    } else {
+      sum_terms.push_back(G);
+    }
+    gi++;
+  }
+  sum_start.push_back((int)sum_terms.size()), sum_out.push_back(do_rescale ? Ybuf + cur * CT : res[cur]->d);
+  fenc_status st = run_mac(ctx, job, L);
+  if (st != FENC_OK) return st;
+  st = rotate_raw(ctx, K, L, rin, rstep, rout);
+  if (st != FENC_OK) return st;
+  {
+    DescStage ds(ctx);
+    size_t o0 = ds.add(sum_terms), o1 = ds.add(sum_start), o2 = ds.add(sum_out);
+    char *base = ds.commit();
+    if (!base) return fail(ctx, FENC_ERR_OOM, "descriptor staging");
+    CUDA_OK(ctx, k_add_many(ctx->k, (const u64 *const *)(base + o0), (const int *)(base + o1), (u64 *const *)(base + o2), (int)sum_out.size(), L, (int)sum_terms.size()));
+  }
+  if (do_rescale) {
+    std::vector<BatchItem> items(n_out);
+    for (size_t t = 0; t < n_out; t++) {
+      items[t] = BatchItem{};
+      items[t].sub_in = Ybuf + t * CT, items[t].out = res[t]->d;
+    }
+    st = rescale_batch(ctx, L, items);
+    if (st != FENC_OK) return st;
+  }
+  sc.ok = true;
+  for (size_t t = 0; t < n_out; t++) out[t] = res[t];
+  return FENC_OK;
+}
+
 // ------------------------------------------------------------------------------------------------ FC by diagonals (R2.12, R2.12b)
 // With g baby steps (d = i g + j):  out_{c'} = sum_i Rot( sum_j sum_c Rot(x_c, j B) (*) Rot(Wd(c',c,d), j B), i g B ):
 // the baby rotations are the executor's inner rotations (once per input ciphertext), the giant ones its outer rotations.

@@ -120,6 +120,54 @@ extern "C" void fenc_keys_free(fenc_keys *K) {
   for (auto &kv : K->evk) dfree(K->ctx, kv.second);
   delete K;
 }
+// the secret's device form: s reduced mod every modulus, NTT domain, Montgomery form
+static fenc_status upload_secret(fenc_ctx *ctx, fenc_keys *K) {
+  Scope sc(ctx);
+  const int A = ctx->A, N = ctx->N;
+  K->d_s_mont = dalloc_t<u64>(ctx, (size_t)A * N);
+  i64 *d_c = sc.alloc<i64>(N);
+  if (!K->d_s_mont || !d_c) return fail(ctx, FENC_ERR_OOM, "secret key");
+  CUDA_OK(ctx, cudaMemcpyAsync(d_c, K->s.data(), (size_t)N * 8, cudaMemcpyHostToDevice, ctx->stream));
+  CUDA_OK(ctx, k_reduce_signed(ctx->k, d_c, ctx->d_ident_mod, K->d_s_mont, A));
+  CUDA_OK(ctx, k_ntt(ctx->k, K->d_s_mont, 0, K->d_s_mont, 0, ctx->d_ident_rows, A, 1));
+  CUDA_OK(ctx, k_mont_convert(ctx->k, K->d_s_mont, K->d_s_mont, ctx->d_ident_mod, A, true));
+  CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+  return FENC_OK;
+}
+// Host-generated key material uploaded verbatim (R2.4): coefficient-domain canonical residues -> NTT domain, Montgomery
+extern "C" fenc_status fenc_keys_import(fenc_ctx *ctx, const fenc_key_material *mat, fenc_keys **out) {
+  if (!ctx || !mat || !out || !mat->s || (mat->n_keys && (!mat->key_ids || !mat->b || !mat->a))) return FENC_ERR_INVALID_ARG;
+  std::unique_ptr<fenc_keys, void (*)(fenc_keys *)> K(new fenc_keys{ctx, 0, {}, nullptr, {}}, fenc_keys_free);
+  const int A = ctx->A, N = ctx->N;
+  const size_t AN = (size_t)A * N;
+  K->s.assign(mat->s, mat->s + N);
+  for (int i = 0; i < N; i++)
+    if (K->s[i] < -1 || K->s[i] > 1) return fail(ctx, FENC_ERR_INVALID_ARG, "secret coefficient %d is not ternary", i);
+  fenc_status st = upload_secret(ctx, K.get());
+  if (st != FENC_OK) return st;
+  for (size_t k = 0; k < mat->n_keys; k++) {
+    const int64_t id = mat->key_ids[k];
+    if (!(id == FENC_RELIN_KEY_ID || (id >= 1 && id < ctx->n)) || K->evk.count(id) || !mat->b[k] || !mat->a[k])
+      return fail(ctx, FENC_ERR_INVALID_ARG, "key %zu: bad id %lld or missing arrays", k, (long long)id);
+    u64 *evk = dalloc_t<u64>(ctx, (size_t)ctx->beta_max * 2 * AN);
+    if (!evk) return fail(ctx, FENC_ERR_OOM, "evaluation key");
+    K->evk[id] = evk;  // owned by K from here on (freed with it on any later failure)
+    for (int j = 0; j < ctx->beta_max; j++)
+      for (int c = 0; c < 2; c++) {
+        u64 *dst = evk + (size_t)(j * 2 + c) * AN;
+        const u64 *src = (c == 0 ? mat->b[k] : mat->a[k]) + (size_t)j * AN;
+        for (int t = 0; t < A; t++)
+          for (int n = 0; n < N; n += N / 4 ? N / 4 : 1)  // spot check of canonical residues (4 per row)
+            if (src[(size_t)t * N + n] >= ctx->mod[t]) return fail(ctx, FENC_ERR_INVALID_ARG, "key %zu: residue not reduced", k);
+        CUDA_OK(ctx, cudaMemcpyAsync(dst, src, AN * 8, cudaMemcpyHostToDevice, ctx->stream));
+        CUDA_OK(ctx, k_ntt(ctx->k, dst, 0, dst, 0, ctx->d_ident_rows, A, 1));
+        CUDA_OK(ctx, k_mont_convert(ctx->k, dst, dst, ctx->d_ident_mod, A, true));
+      }
+    CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));  // the caller's arrays may go away after the call
+  }
+  *out = K.release();
+  return FENC_OK;
+}
 extern "C" fenc_status fenc_secret_export(fenc_ctx *ctx, const fenc_keys *K, int64_t *s) {
   if (!ctx || !K || !s) return FENC_ERR_INVALID_ARG;
   memcpy(s, K->s.data(), K->s.size() * 8);
@@ -672,6 +720,62 @@ extern "C" fenc_status fenc_sum_groups(fenc_ctx *ctx, fenc_ct *const *in, size_t
   sc.ok = true;
   for (size_t g = 0; g < n_groups; g++) out[g] = made[g];
   return FENC_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ pooling order, activation
+// indices such that consecutive groups of four are the fragments (2u_o + a, 2v_o + b) of output fragment (u_o, v_o);
+// ciphertext order [...][u][v] (pooling keeps or combines whole fragment ciphertexts)
+static fenc_status pool_gather(fenc_ctx *ctx, fenc_ct *const *in, size_t n, uint32_t S, std::vector<fenc_ct *> &ordered) {
+  if (S < 2 || (S & 1) || n % ((size_t)S * S)) return fail(ctx, FENC_ERR_LAYOUT, "pool needs an even S and a multiple of S^2 ciphertexts");
+  ordered.clear();
+  for (size_t base = 0; base < n; base += (size_t)S * S)
+    for (uint32_t uo = 0; uo < S / 2; uo++)
+      for (uint32_t vo = 0; vo < S / 2; vo++)
+        for (int a = 0; a < 2; a++)
+          for (int b = 0; b < 2; b++) ordered.push_back(in[base + (2 * uo + a) * S + (2 * vo + b)]);
+  return FENC_OK;
+}
+extern "C" fenc_status fenc_sum_pool(fenc_ctx *ctx, fenc_ct *const *in, size_t n, uint32_t S, fenc_ct **out) {
+  if (!ctx || !in || !out) return FENC_ERR_INVALID_ARG;
+  std::vector<fenc_ct *> ord;
+  fenc_status st = pool_gather(ctx, in, n, S, ord);
+  if (st != FENC_OK) return st;
+  return fenc_sum_groups(ctx, ord.data(), 4, n / 4, out);
+}
+extern "C" fenc_status fenc_square_sum_pool(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const *in, size_t n, uint32_t S, fenc_ct **out) {
+  if (!ctx || !K || !in || !out) return FENC_ERR_INVALID_ARG;
+  std::vector<fenc_ct *> ord;
+  fenc_status st = pool_gather(ctx, in, n, S, ord);
+  if (st != FENC_OK) return st;
+  return cmult_relin(ctx, K, ord.data(), ord.data(), n / 4, out, 4);
+}
+
+// Degree-3 activation (R2.12): the library owns the order of the steps, the caller the three exactly rounded integers.
+extern "C" fenc_status fenc_poly3(fenc_ctx *ctx, const fenc_keys *K, fenc_ct *const *in, size_t n, const uint64_t *k3_res,
+                                  const uint64_t *k1_res, const uint64_t *k0_res, double scale_sq, fenc_ct **out) {
+  if (!ctx || !K || !in || !k3_res || !k1_res || !k0_res || !out) return FENC_ERR_INVALID_ARG;
+  if (n == 0) return FENC_OK;
+  const int L = in[0]->L;
+  if (L < 3) return fail(ctx, FENC_ERR_LEVEL, "the degree-3 activation needs two levels");
+  struct Tmp {  // intermediate ciphertexts of this call
+    std::vector<fenc_ct *> v;
+    ~Tmp() { for (fenc_ct *c : v) fenc_ct_free(c); }
+    fenc_ct **fresh(size_t n) { size_t at = v.size(); v.resize(at + n, nullptr); return v.data() + at; }
+  } tmp;
+  tmp.v.reserve(8 * n);  // no reallocation: the pointers handed out stay valid
+  fenc_status st;
+  fenc_ct **x2 = tmp.fresh(n), **t0 = tmp.fresh(n), **t = tmp.fresh(n), **x3 = tmp.fresh(n), **u0 = tmp.fresh(n), **u1 = tmp.fresh(n),
+          **u = tmp.fresh(n), **y = tmp.fresh(n);
+  if ((st = cmult_relin(ctx, K, in, in, n, x2)) != FENC_OK) return st;                                  // x^2 at L-1
+  if ((st = scalar_op(ctx, in, n, k3_res, (double)ctx->mod[L - 1], false, t0)) != FENC_OK) return st;    // a3 q_{L-1} x
+  if ((st = fenc_rescale(ctx, t0, n, t)) != FENC_OK) return st;                                          // a3 x at L-1
+  if ((st = cmult_relin(ctx, K, x2, t, n, x3)) != FENC_OK) return st;                                    // a3 x^3 at L-2
+  if ((st = scalar_op(ctx, in, n, k1_res, scale_sq, false, u0)) != FENC_OK) return st;                   // a1 s^2 x
+  if ((st = fenc_rescale(ctx, u0, n, u1)) != FENC_OK) return st;
+  if ((st = fenc_rescale(ctx, u1, n, u)) != FENC_OK) return st;                                          // a1 x at L-2, scale s3
+  for (size_t i = 0; i < n; i++)
+    if ((st = fenc_add(ctx, x3[i], u[i], &y[i])) != FENC_OK) return st;
+  return scalar_op(ctx, y, n, k0_res, 1.0, true, out);
 }
 
 // ------------------------------------------------------------------------------------------------ raw NTT (a1)

@@ -14,19 +14,15 @@ def _round_half_up(x):
 
 
 def poly3_activation(ctx, keys, cts, scale, coef=POLY3):
-    """Degree-3 activation a0 + a1 x + a3 x^3 in two levels (R2.12), every step one batched library call.
-    `scale` is the exact rational scale of the inputs (the integer multipliers are rounded exactly on the host, R2.8).
-    Returns (ciphertexts at L-2, their exact scale)."""
+    """Degree-3 activation a0 + a1 x + a3 x^3 in two levels (R2.12): ONE library call (fenc_poly3 owns the order
+    of the steps); this function only rounds the three integer multipliers exactly from the exact rational scale of the
+    inputs (R2.8).  Returns (ciphertexts at L-2, their exact scale)."""
     a0, a1, a3 = (Fraction(c) for c in coef)
     L, s = cts[0].L, Fraction(scale)
     q1, q2 = ctx.q[L - 1], ctx.q[L - 2]
-    x2 = ctx.square_relin(keys, cts)
-    t = ctx.rescale(ctx.mul_scalar(cts, _round_half_up(a3 * q1), float(q1)))
-    x3 = ctx.cmult_relin(keys, x2, t)
-    u = ctx.rescale(ctx.rescale(ctx.mul_scalar(cts, _round_half_up(a1 * s * s), float(s * s))))
     s3 = s ** 3 / (q1 * q2)
-    y = [ctx.add(a, b) for a, b in zip(x3, u)]
-    return ctx.add_const(y, _round_half_up(a0 * s3)), s3
+    out = ctx.poly3(keys, cts, _round_half_up(a3 * q1), _round_half_up(a1 * s * s), _round_half_up(a0 * s3), float(s * s))
+    return out, s3
 
 
 class Pipeline:
@@ -145,19 +141,6 @@ class Pipeline:
                         cts.append(ctx.encrypt(self.keys, pt, enc_seed0 + len(cts)))
         return cts
 
-    @staticmethod
-    def pool_order(n_ct, S):
-        """indices so that consecutive groups of 4 are the fragments (2uo+a, 2vo+b) of output fragment (uo, vo)."""
-        per = S * S
-        idx = []
-        for base in range(0, n_ct, per):
-            for uo in range(S // 2):
-                for vo in range(S // 2):
-                    for a in range(2):
-                        for b in range(2):
-                            idx.append(base + (2 * uo + a) * S + (2 * vo + b))
-        return idx
-
     def forward(self, cts, trace=None, scale=None, lazy_relin=False):
         """scale: exact rational scale of the inputs (default: the context's 2^log2_scale); only poly3 needs it.
         lazy_relin: a square directly followed by a pool runs as ONE step, fenc_square_sum_relin over the four fragments of
@@ -171,7 +154,7 @@ class Pipeline:
             if fused_prev:
                 pass  # done together with the square before it
             elif lazy_relin and p["op"] == "square" and li + 1 < len(self.plan) and self.plan[li + 1]["op"] == "pool":
-                cts = ctx.square_sum_relin(self.keys, [cts[i] for i in self.pool_order(len(cts), S)], 4)
+                cts = ctx.square_sum_pool(self.keys, cts, S)
                 sc = sc * sc / ctx.q[p["L"] - 1]
                 S //= 2
             elif p["op"] == "conv":
@@ -186,7 +169,7 @@ class Pipeline:
             elif p["op"] == "poly3":
                 cts, sc = poly3_activation(ctx, self.keys, cts, sc, p["coef"])
             elif p["op"] == "pool":
-                cts = ctx.sum_groups([cts[i] for i in self.pool_order(len(cts), S)], 4)
+                cts = ctx.sum_pool(cts, S)
                 S //= 2
             elif p["op"] == "compress":
                 # sources ordered [bg][fragment]; output t gathers batch groups t*per .. t*per + per - 1 of each fragment

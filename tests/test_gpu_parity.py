@@ -102,6 +102,33 @@ def test_primitives_bit_exact(mods, name):
     ctx.close()
 
 
+@pytest.mark.parametrize("name", ["toy64", "mid12"])
+def test_keys_import_host_generated_material(mods, name):
+    """fenc_keys_import: the ORACLE's secret and switching keys (generated on the host from the seed, R2.3/R2.4) uploaded
+    verbatim; rotations, a hoisted rotation and x^2 with the imported keys equal the oracle's bit for bit, and the imported
+    key set re-exports to the same material."""
+    ck, fr, fenc = mods
+    P, ctx = make(mods, name)
+    steps = [1, 7, P.n - 1]
+    ok = ck.keygen(P, 99, steps, want_relin=True)
+    gk = ctx.keys_import(ok.s, {kid: ok.evk[kid] for kid in steps + [ck.RELIN_KEY_ID]})
+    assert np.array_equal(ctx.secret_export(gk), ok.s)
+    b, a = ctx.evk_export(gk, 7)
+    assert np.array_equal(b, ok.evk[7][0]) and np.array_equal(a, ok.evk[7][1])
+    L = P.nq
+    pt = ck.encode(P, np.random.default_rng(1).uniform(-1, 1, P.n), L)
+    oct_ = ck.encrypt(P, ok, pt, 5)
+    gct = ctx.encrypt(gk, ctx.pt_from_coeffs(pt.coeffs, L, float(pt.scale)), 5)
+    assert np.array_equal(ctx.ct_export(gct), oct_.c)
+    for r, o in zip(steps, ctx.rotate(gk, [gct] * 3, steps)):
+        assert np.array_equal(ctx.ct_export(o), ck.rotate(P, ok, oct_, r).c), r
+    assert np.array_equal(ctx.ct_export(ctx.rotate_hoisted(gk, [gct], [7])[0][0]), ck.rotate_hoisted(P, ok, oct_, 7).c)
+    assert np.array_equal(ctx.ct_export(ctx.square_relin(gk, gct)), ck.square_relin(P, ok, oct_).c)
+    with pytest.raises(fenc.FencError):
+        ctx.keys_import(np.full(P.N, 2, dtype=np.int64), {})  # not ternary
+    ctx.close()
+
+
 def test_errors_and_edges(mods):
     ck, fr, fenc = mods
     P, ctx = make(mods, "toy64")
@@ -360,6 +387,42 @@ def test_bottleneck_compress_then_segmented_conv_bit_exact(mods):
         ctx.decrypt_decode(gk, g_out[go], c2, l2, 1, 0, 0, go, 0, Y)
     want = fr.direct_conv(fr.ConvDesc(**exp), fr.direct_conv(fr.ConvDesc(**red), x, w1), w2)
     assert np.abs(Y - want).max() < 1e-3
+    ctx.close()
+
+
+@pytest.mark.parametrize("S_src,S_dst,shape", [(2, 1, (1, 4, 8, 8)), (1, 2, (2, 2, 8, 8)), (2, 4, (1, 8, 7, 6))])
+def test_repack_block_size_bit_exact(mods, S_src, S_dst, shape):
+    """fenc_repack (R2.11c; PAPER.md:290 block-size re-adaptation) against the oracle's repack on the plan between two
+    block sizes: every limb, one level consumed, and the decoded tensor unchanged."""
+    ck, fr, fenc = mods
+    P, ctx = make(mods, "mid10")
+    L = P.nq
+    BS, C, H, W = shape
+    M = fr.next_pow2(max(H, W))
+    src, dst = fr.Layout(P.n, M, S_src, BS, C), fr.Layout(P.n, M, S_dst, BS, C)
+    x = np.random.default_rng(15).uniform(-1, 1, shape)
+    plan = fr.repack_plan(src, dst, shape)
+    steps = sorted({r for terms in plan.values() for _, r, _ in terms if r})
+    ok, gk = ck.keygen(P, 6, steps), ctx.keygen(6, steps)
+    skeys = src.ct_keys()
+    o_in, g_in = {}, []
+    for i, k in enumerate(skeys):
+        pt = ck.encode(P, src.gather(x, *k), L)
+        o_in[k] = ck.encrypt(P, ok, pt, 60 + i)
+        g_in.append(ctx.encrypt(gk, ctx.pt_from_coeffs(pt.coeffs, L, float(pt.scale)), 60 + i))
+    ref = fr.repack(ck, P, ok, plan, o_in, L)
+    dkeys = dst.ct_keys()
+    terms = []
+    for t, dk in enumerate(dkeys):
+        for skey, r, mask in plan[dk]:
+            m = ck.encode(P, mask, L, P.q[L - 1])
+            terms.append((t, skeys.index(skey), r, ctx.pt_from_coeffs(m.coeffs, L, float(m.scale))))
+    got = ctx.repack(gk, g_in, terms, len(dkeys))
+    Y = np.zeros(shape)
+    for t, dk in enumerate(dkeys):
+        assert got[t].L == L - 1 and np.array_equal(ctx.ct_export(got[t]), ref[dk].c), dk
+        dst.scatter(Y, ctx.decrypt_slots(gk, got[t]).real, *dk)
+    assert np.abs(Y - x).max() < 1e-4
     ctx.close()
 
 
