@@ -462,6 +462,25 @@ def per_kernel_profile(nb, steps):
     return prof, wall_ms
 
 
+def per_layer_profile(nb):
+    """--per-layer: one step with the library's per-class CUDA-event hooks read out after every layer (the read-out
+    synchronises the stream, so the layers do not overlap: a breakdown, not a throughput)."""
+    ctx = nb.ctx
+    rows = []
+    ctx.profile_enable(True)
+    for gi, g in enumerate(nb.groups):
+        def done(li, p, gi=gi):
+            prof = ctx.profile_read()
+            conv = p.get("conv")
+            name = p["op"] + ("" if conv is None else " %d->%d k%d s%d%s L=%d" % (conv.C_in, conv.C_out, conv.K, conv.stride, " dw" if conv.depthwise else "", p["L"]))
+            rows.append({"group": gi, "layer": li, "op": name, "ms": round(sum(v[0] for v in prof.values()), 3),
+                         "per_kernel_ms": {k: round(v[0], 3) for k, v in sorted(prof.items(), key=lambda kv: -kv[1][0])}})
+        out = nb.pipe.forward(g, lazy_relin=nb.lazy, on_layer=done)
+        del out
+    ctx.profile_enable(False)
+    return rows
+
+
 NTT_CLASSES = ("intt_rowpass", "intt_colpass", "ntt_colpass", "ntt_colpass_bconv", "ntt_rowpass", "ntt_rows_keymac", "ntt_rows_divide")
 
 
@@ -795,6 +814,9 @@ def run_ours(args, rank, world):
     t, out = time_resident(nb, args.steps, args.warmup, world, sampler, args.profile_range)
     del out
     summ = net_summary(nb, t, world)
+    if args.per_layer:
+        sampler.stop()
+        return {"workload": name, "batch": nb.batch, "ms_per_step": summ["ms_per_step"], "clocks": summ["clocks"], "per_layer": per_layer_profile(nb)}
     if args.no_extras:
         sampler.stop()
         return {"metric": METRIC, "value": summ["conv_layers_per_s"], "unit": "encrypted conv layers/s", "ms_per_step": summ["ms_per_step"],
@@ -926,6 +948,7 @@ def main():
     ap.add_argument("--sweep-cts", type=int, default=64, help="config 5: ciphertexts per batched rotation (BASELINE: 64)")
     ap.add_argument("--sweep-steps", type=int, default=32, help="config 5: distinct rotation amounts (BASELINE: 32)")
     ap.add_argument("--no-extras", action="store_true", help="timed steps only: skip the per-kernel pass, e2e, cpu_baseline, companions (profiling runs)")
+    ap.add_argument("--per-layer", action="store_true", help="print a per-layer, per-kernel-class breakdown of one step instead of the bench line")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-companions", action="store_true", help="default workload only: skip the config 5 / 2 / 3 companions")
     args = ap.parse_args()

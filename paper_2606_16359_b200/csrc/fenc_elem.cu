@@ -237,10 +237,23 @@ __global__ void __launch_bounds__(256, G >= 8 ? 2 : 3) smac_kernel(SmacP p) {
       }
     }
     __syncthreads();
+    // the next term's ciphertext words are requested before this term's products (register double buffer): with two blocks
+    // of 8 warps per SM the loads would otherwise sit in front of 112 dependent FP64 operations
+    u64 nx0 = 0, nx1 = 0;
+    if (G >= 4) nx0 = __ldg(s_ct[0] + idx), nx1 = __ldg(s_ct[0] + LN + idx);
 #pragma unroll 2
     for (int t = 0; t < nt; t++) {
-      const u64 *c = s_ct[t];
-      const u64 x0 = __ldg(c + idx), x1 = __ldg(c + LN + idx);
+      u64 x0, x1;
+      if (G >= 4) {
+        x0 = nx0, x1 = nx1;
+        if (t + 1 < nt) {
+          const u64 *c = s_ct[t + 1];
+          nx0 = __ldg(c + idx), nx1 = __ldg(c + LN + idx);
+        }
+      } else {
+        const u64 *c = s_ct[t];
+        x0 = __ldg(c + idx), x1 = __ldg(c + LN + idx);
+      }
       if (F64) {
         const double xd0 = u2d52(x0), xd1 = u2d52(x1);
 #pragma unroll
@@ -301,6 +314,79 @@ __global__ void __launch_bounds__(256, G >= 8 ? 2 : 3) smac_kernel(SmacP p) {
       out[LN + idx] = tot[i][1];
     }
 }
+// Single-output groups in fp64 mode (depthwise layers: every output has its own ciphertext sequence, nothing to share):
+// a streaming kernel, two adjacent coefficients per thread with 16-byte loads, the loads of up to four terms of a mask
+// segment in flight before their products.  HBM-bound: 16 (L N) bytes read per term and output.
+__global__ void __launch_bounds__(256, 4) smac1_kernel(SmacP p) {
+  __shared__ const u64 *s_ct[SMAC_TILE];
+  __shared__ ulonglong2 s_k[SMAC_TILE];
+  const size_t LN = (size_t)p.L << p.logN;
+  const size_t idx = ((size_t)blockIdx.y * blockDim.x + threadIdx.x) * 2;
+  const int limb = (int)(((size_t)blockIdx.y * blockDim.x * 2) >> p.logN);
+  const SmacGroup g = p.groups[blockIdx.x];
+  const ModConst mc = p.mods[limb];
+  const F64Mod fm = f64mod(mc.q, mc.f64);
+  double acc[4] = {0.0, 0.0, 0.0, 0.0};  // (c0, c1) x (even, odd coefficient)
+  u64 tot[4] = {0, 0, 0, 0};
+  int seg = 0, cur_end = p.seg_end[g.seg_start], lazy = 0;
+  auto term = [&](const ulonglong2 &a, const ulonglong2 &b, int t) {
+    const ulonglong2 kk = s_k[t];
+    const double kd = __longlong_as_double((long long)kk.x), kq = __longlong_as_double((long long)kk.y);
+    acc[0] = __dadd_rn(acc[0], mulmod_dd(u2d52(a.x), kd, kq, fm));
+    acc[1] = __dadd_rn(acc[1], mulmod_dd(u2d52(a.y), kd, kq, fm));
+    acc[2] = __dadd_rn(acc[2], mulmod_dd(u2d52(b.x), kd, kq, fm));
+    acc[3] = __dadd_rn(acc[3], mulmod_dd(u2d52(b.y), kd, kq, fm));
+    if (++lazy == p.max_lazy) {
+#pragma unroll
+      for (int i = 0; i < 4; i++) acc[i] = reduce_dd(acc[i], fm);
+      lazy = 1;
+    }
+  };
+  for (int t0 = 0; t0 < g.n_terms; t0 += SMAC_TILE) {
+    const int nt = g.n_terms - t0 < SMAC_TILE ? g.n_terms - t0 : SMAC_TILE;
+    __syncthreads();
+    for (int t = threadIdx.x; t < nt; t += blockDim.x) {
+      s_ct[t] = p.term_ct[g.ct_start + t0 + t];
+      s_k[t] = __ldg(reinterpret_cast<const ulonglong2 *>(p.kpair) + (size_t)p.kidx[g.k_start + t0 + t] * p.L + limb);
+    }
+    __syncthreads();
+    int t = 0;
+    while (t < nt) {
+      const int e = cur_end - t0 < nt ? cur_end - t0 : nt;  // end of this segment inside the tile
+      for (; t + 4 <= e; t += 4) {
+        ulonglong2 a[4], b[4];
+#pragma unroll
+        for (int u = 0; u < 4; u++) {
+          const u64 *c = s_ct[t + u];
+          a[u] = __ldg(reinterpret_cast<const ulonglong2 *>(c + idx));
+          b[u] = __ldg(reinterpret_cast<const ulonglong2 *>(c + LN + idx));
+        }
+#pragma unroll
+        for (int u = 0; u < 4; u++) term(a[u], b[u], t + u);
+      }
+      for (; t < e; t++) {
+        const u64 *c = s_ct[t];
+        term(__ldg(reinterpret_cast<const ulonglong2 *>(c + idx)), __ldg(reinterpret_cast<const ulonglong2 *>(c + LN + idx)), t);
+      }
+      if (t0 + t == cur_end) {  // tot += M (*) S
+        const ulonglong2 m = __ldg(reinterpret_cast<const ulonglong2 *>(p.seg_mask[g.seg_start + seg] + idx));
+        const double off = fm.q + 4503599627370496.0;
+#pragma unroll
+        for (int i = 0; i < 4; i++) {
+          const u64 S = csub(d2u_off(reduce_dd(acc[i], fm), off), mc.q);
+          tot[i] = addmod(tot[i], mont_mul(S, (i & 1) ? m.y : m.x, mc.q, mc.qinv_neg), mc.q);
+          acc[i] = 0.0;
+        }
+        lazy = 0;
+        seg++;
+        cur_end = seg < g.n_seg ? p.seg_end[g.seg_start + seg] : 1 << 30;
+      }
+    }
+  }
+  u64 *out = p.outs[g.out_start];
+  *reinterpret_cast<ulonglong2 *>(out + idx) = make_ulonglong2(tot[0], tot[1]);
+  *reinterpret_cast<ulonglong2 *>(out + LN + idx) = make_ulonglong2(tot[2], tot[3]);
+}
 template <bool F64>
 static void launch_smac(const SmacP &p, dim3 grid, int nth, cudaStream_t st, int max_group) {
   if (max_group <= 1) smac_kernel<1, F64><<<grid, nth, 0, st>>>(p);
@@ -316,7 +402,8 @@ int k_smac(const KCtx &k, const SmacGroup *groups, int n_groups, int max_group, 
   const int nth = k.N < 256 ? k.N : 256;
   dim3 grid(n_groups, (unsigned)(((size_t)L * k.N) / nth));
   PROF2(k, K_SMAC, alg_bytes, alg_mulaccs);  // second counter of this class: modular multiply-accumulates
-  if (fp64_mode) launch_smac<true>(p, grid, nth, S(k), max_group);
+  if (fp64_mode && max_group <= 1 && k.N >= 512) smac1_kernel<<<dim3(n_groups, (unsigned)(((size_t)L * k.N) / 512)), 256, 0, S(k)>>>(p);
+  else if (fp64_mode) launch_smac<true>(p, grid, nth, S(k), max_group);
   else launch_smac<false>(p, grid, nth, S(k), max_group);
   LAUNCH_CHECK(k);
   return 0;

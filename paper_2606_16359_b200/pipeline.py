@@ -141,11 +141,11 @@ class Pipeline:
                         cts.append(ctx.encrypt(self.keys, pt, enc_seed0 + len(cts)))
         return cts
 
-    def forward(self, cts, trace=None, scale=None, lazy_relin=False):
+    def forward(self, cts, trace=None, scale=None, lazy_relin=False, on_layer=None):
         """scale: exact rational scale of the inputs (default: the context's 2^log2_scale); only poly3 needs it.
         lazy_relin: a square directly followed by a pool runs as ONE step, fenc_square_sum_relin over the four fragments of
         every pooled output (one relinearisation instead of four, R2.12c); the trace then holds the pooled
-        ciphertexts at both positions."""
+        ciphertexts at both positions.  on_layer(index, plan entry): called after each layer's calls are enqueued."""
         ctx = self.ctx
         S = None
         sc = Fraction(cts[0].scale) if scale is None else Fraction(scale)
@@ -179,4 +179,6 @@ class Pipeline:
                 cts = ctx.compress(self.keys, cts, terms, n_t * fr_)
             if trace is not None:
                 trace.append(cts)
+            if on_layer is not None and not fused_prev:
+                on_layer(li, p)
         return cts
