@@ -398,22 +398,49 @@ struct NttRowP {
   const u64 *src; size_t src_bstride; u64 *dst; size_t dst_bstride; const RowDesc *rows; const ModConst *mods;
   const ShoupC *tw; NttGeom g; int src_is_dst_row;
 };
+// ROW_TPB consecutive tiles of one row per block (compile-time geometries): the next tile's words are requested into
+// registers before the current tile is transformed, so a block keeps loads in flight during its arithmetic (one tile
+// per block left about 13 KB per SM in flight on average, a third of what HBM's latency needs).
+#ifndef FENC_ROW_TPB
+#define FENC_ROW_TPB 4
+#endif
 template <int GEO>
-__global__ void __launch_bounds__(256, 4) ntt_rowpass_kernel(NttRowP p) {
+__global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? 6 : 4) ntt_rowpass_kernel(NttRowP p) {
   extern __shared__ u64 sm[];
   const int tid = threadIdx.x, b = blockIdx.z;
   const RowDesc rd = p.rows[blockIdx.y];
   const int N = 1 << p.g.logN, T = 1 << p.g.lt_row;
-  TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, blockIdx.x};
+  constexpr int TPB = GEO == 1 ? FENC_ROW_TPB : 1;
   const u64 *src = p.src + (size_t)b * p.src_bstride + (size_t)(p.src_is_dst_row ? rd.dst_row : rd.src_row) * N;
-  const int nth = blockDim.x;
-  tile_fill(sm, T, tid, nth, [&](int e) { return src[G.gidx(e)]; });
-  __syncthreads();
-  const ModConst mc = p.mods[rd.mod];
-  tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, mc.q, tid, mc.f64);
   u64 *dst = p.dst + (size_t)b * p.dst_bstride + (size_t)rd.dst_row * N;
-  tile_drain(sm, T, tid, nth, [&](int e, u64 v) { dst[G.gidx(e)] = fullred(v, mc.q, mc.qbar); });
+  const int nth = blockDim.x;
+  const ModConst mc = p.mods[rd.mod];
+  u64 v[8];
+  auto request = [&](u32 tile) {
+    TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, tile};
+#pragma unroll
+    for (int i = 0; i < 8; i++) {
+      const int e = tid + i * nth;
+      if (e < T) v[i] = src[G.gidx(e)];
+    }
+  };
+  request(blockIdx.x * TPB);
+#pragma unroll 1
+  for (int k = 0; k < TPB; k++) {
+    TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, blockIdx.x * TPB + k};
+#pragma unroll
+    for (int i = 0; i < 8; i++) {
+      const int e = tid + i * nth;
+      if (e < T) sm[swz(e)] = v[i];
+    }
+    __syncthreads();
+    if (k + 1 < TPB) request(blockIdx.x * TPB + k + 1);
+    tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, mc.q, tid, mc.f64);
+    tile_drain(sm, T, tid, nth, [&](int e, u64 x) { dst[G.gidx(e)] = fullred(x, mc.q, mc.qbar); });
+    if (k + 1 < TPB) __syncthreads();  // every thread has read its results before the next tile overwrites them
+  }
 }
+static inline unsigned row_grid_x(const NttGeom &g, int N) { return (unsigned)((N >> g.lt_row) / (g.logN >= 12 ? FENC_ROW_TPB : 1)); }
 
 int k_ntt(const KCtx &k, const u64 *src, size_t src_bstride, u64 *dst, size_t dst_bstride, const RowDesc *rows, int n_rows,
           int n_batch) {
@@ -426,7 +453,7 @@ int k_ntt(const KCtx &k, const u64 *src, size_t src_bstride, u64 *dst, size_t ds
   COL_GEO(g, (ntt_colpass_kernel<false, GEO><<<grid1, nthreads_for(g.lt_col), sizeof(u64) << g.lt_col, st>>>(a)));
   LAUNCH_CHECK(k);
   NttRowP r{dst, dst_bstride, dst, dst_bstride, rows, k.d_mods, k.d_tw_fwd, g, 1};
-  dim3 grid2(k.N >> g.lt_row, n_rows, n_batch);
+  dim3 grid2(row_grid_x(g, k.N), n_rows, n_batch);
   PROF(k, K_NTT_ROW, 16.0 * k.N * n_rows * n_batch, HALF_N(k) * g.brow * n_rows * n_batch);
   ROW_GEO(g, (ntt_rowpass_kernel<GEO><<<grid2, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(r)));
   LAUNCH_CHECK(k);
@@ -438,7 +465,7 @@ int k_ntt_rows_only(const KCtx &k, u64 *buf, size_t bstride, const RowDesc *rows
   if (n_rows == 0 || n_batch == 0) return 0;
   const NttGeom &g = k.geom;
   NttRowP r{buf, bstride, buf, bstride, rows, k.d_mods, k.d_tw_fwd, g, 1};
-  dim3 grid2(k.N >> g.lt_row, n_rows, n_batch);
+  dim3 grid2(row_grid_x(g, k.N), n_rows, n_batch);
   PROF(k, K_NTT_ROW, 16.0 * k.N * n_rows * n_batch, HALF_N(k) * g.brow * n_rows * n_batch);
   ROW_GEO(g, (ntt_rowpass_kernel<GEO><<<grid2, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(r)));
   LAUNCH_CHECK(k);
@@ -644,52 +671,72 @@ struct DivideP {
   const ShoupC *mul2;  // MERGED: out = ((minuend mul2 + addend) - X) mul   (mul2 = P^-1, mul = q_{L-1}^-1)
 };
 template <int GEO, bool MERGED = false>
-__global__ void __launch_bounds__(256, 4) ntt_rows_divide_kernel(DivideP p) {
+__global__ void __launch_bounds__(GEO == 1 ? 128 : 256, 4) ntt_rows_divide_kernel(DivideP p) {
   extern __shared__ u64 sm[];
   const int tid = threadIdx.x, b = blockIdx.z;
   const RowDesc rd = p.rows[blockIdx.y];
   const int N = 1 << p.g.logN, T = 1 << p.g.lt_row;
-  TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, blockIdx.x};
+  constexpr int TPB = GEO == 1 ? FENC_ROW_TPB : 1;  // tiles per block, the next one prefetched (see ntt_rowpass_kernel)
   const u64 *src = p.tmp + (size_t)b * p.tmp_bstride + (size_t)rd.src_row * N;
   const int nth = blockDim.x, logN = p.g.logN;
   const BatchItem it = p.items[b];
   const u64 *minuend = (p.from_items ? it.sub_in : p.acc + (size_t)b * p.acc_bstride) + (size_t)rd.aux2 * N;
   const u64 *addend = rd.aux == 0 ? it.add0 : it.add1;
   if (addend) addend += (size_t)rd.mod * N;
-  // epilogue operands are fetched BEFORE the transform so that their latency hides behind it
-  u64 mi[8], ad[8];
-#pragma unroll
-  for (int i = 0; i < 8; i++) {
-    const u32 j = G.gidx((tid + i * nth) & (T - 1));
-    mi[i] = __ldg(minuend + j);
-    ad[i] = addend ? __ldg(addend + galois_src(j, it.g, logN)) : 0;
-  }
-  tile_fill(sm, T, tid, nth, [&](int e) { return src[G.gidx(e)]; });
-  __syncthreads();
   const ModConst mq = p.mods[rd.mod];
   const u64 q = mq.q;
-  tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid, mq.f64);
   const ShoupC mc = p.mul[rd.mod];
   const F64Mod fm = f64mod(q, mq.f64);
   u64 *dst = it.out + (size_t)rd.dst_row * N;
+  u64 v[8];
+  auto request = [&](u32 tile) {
+    TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, tile};
 #pragma unroll
-  for (int i = 0; i < 8; i++) {
-    const int e = tid + i * nth;
-    if (e < T) {
-      // fp64 rows: X mod q as v - rint(v/q) q + q in (0, 2q) on the FP64 pipe; the Shoup multiply takes any 64-bit input
-      const bool fp = mq.f64 != 0;
-      const u64 x = fp ? d2u_off(reduce_dd(u2d52(sm[swz(e)]), fm), fm.q + 4503599627370496.0) : fullred(sm[swz(e)], q, mq.qbar);
-      u64 v;
-      if (MERGED) {
-        const ShoupC m2 = p.mul2[rd.mod];
-        v = addmod(shoup_mul(mi[i], m2.c, m2.cs, q), ad[i], q);
-        v = shoup_mul(fp ? v + 2 * q - x : submod(v, x, q), mc.c, mc.cs, q);
-      } else {
-        v = shoup_mul(fp ? mi[i] + 2 * q - x : submod(mi[i], x, q), mc.c, mc.cs, q);
-        v = addmod(v, ad[i], q);
-      }
-      dst[G.gidx(e)] = v;
+    for (int i = 0; i < 8; i++) {
+      const int e = tid + i * nth;
+      if (e < T) v[i] = src[G.gidx(e)];
     }
+  };
+  request(blockIdx.x * TPB);
+#pragma unroll 1
+  for (int k = 0; k < TPB; k++) {
+    TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, blockIdx.x * TPB + k};
+#pragma unroll
+    for (int i = 0; i < 8; i++) {
+      const int e = tid + i * nth;
+      if (e < T) sm[swz(e)] = v[i];
+    }
+    __syncthreads();
+    // epilogue operands of this tile and the words of the next tile are fetched BEFORE the transform: their latency hides behind it
+    u64 mi[8], ad[8];
+#pragma unroll
+    for (int i = 0; i < 8; i++) {
+      const u32 j = G.gidx((tid + i * nth) & (T - 1));
+      mi[i] = __ldg(minuend + j);
+      ad[i] = addend ? __ldg(addend + galois_src(j, it.g, logN)) : 0;
+    }
+    if (k + 1 < TPB) request(blockIdx.x * TPB + k + 1);
+    tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid, mq.f64);
+#pragma unroll
+    for (int i = 0; i < 8; i++) {
+      const int e = tid + i * nth;
+      if (e < T) {
+        // fp64 rows: X mod q as v - rint(v/q) q + q in (0, 2q) on the FP64 pipe; the Shoup multiply takes any 64-bit input
+        const bool fp = mq.f64 != 0;
+        const u64 x = fp ? d2u_off(reduce_dd(u2d52(sm[swz(e)]), fm), fm.q + 4503599627370496.0) : fullred(sm[swz(e)], q, mq.qbar);
+        u64 r;
+        if (MERGED) {
+          const ShoupC m2 = p.mul2[rd.mod];
+          r = addmod(shoup_mul(mi[i], m2.c, m2.cs, q), ad[i], q);
+          r = shoup_mul(fp ? r + 2 * q - x : submod(r, x, q), mc.c, mc.cs, q);
+        } else {
+          r = shoup_mul(fp ? mi[i] + 2 * q - x : submod(mi[i], x, q), mc.c, mc.cs, q);
+          r = addmod(r, ad[i], q);
+        }
+        dst[G.gidx(e)] = r;
+      }
+    }
+    if (k + 1 < TPB) __syncthreads();
   }
 }
 
@@ -699,7 +746,7 @@ int k_ntt_rows_divide(const KCtx &k, const BatchItem *items, const u64 *tmp, siz
   if (n_rows == 0 || n_batch == 0) return 0;
   const NttGeom &g = k.geom;
   DivideP p{items, tmp, tmp_bstride, acc, acc_bstride, mul, rows, k.d_mods, k.d_tw_fwd, g, minuend_from_items ? 1 : 0, merged_mul2};
-  dim3 grid(k.N >> g.lt_row, n_rows, n_batch);
+  dim3 grid(row_grid_x(g, k.N), n_rows, n_batch);
   PROF(k, K_DIVIDE, 8.0 * k.N * (3.5 * n_rows) * n_batch, HALF_N(k) * g.brow * n_rows * n_batch);  // temp + minuend + output, addend on half the rows
   if (merged_mul2)
     ROW_GEO(g, (ntt_rows_divide_kernel<GEO, true><<<grid, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p)));
