@@ -41,30 +41,6 @@ DEVI u64 mont_mul(u64 a, u64 b, u64 q, u64 qinv_neg) {
 DEVI u64 addmod(u64 a, u64 b, u64 q) { return csub(a + b, q); }
 DEVI u64 submod(u64 a, u64 b, u64 q) { return a >= b ? a - b : a + q - b; }
 
-// ---------------------------------------------------------------------------------------------- bulk async copies
-// TMA bulk copies (global -> shared, 1-D, no tensor map) completing on an mbarrier; sizes and addresses 16-byte aligned.
-DEVI u32 smem_u32(const void *p) { return (u32)__cvta_generic_to_shared(p); }
-DEVI void mbar_init(u64 *bar, u32 count) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory"); }
-DEVI void mbar_init_fence() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-DEVI void mbar_arrive(u64 *bar) { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory"); }
-DEVI void mbar_arrive_expect_tx(u64 *bar, u32 bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-DEVI void mbar_wait(u64 *bar, u32 parity) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "WAIT_LOOP:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-      "@p bra WAIT_DONE;\n\t"
-      "bra WAIT_LOOP;\n\t"
-      "WAIT_DONE:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-DEVI void bulk_g2s(void *dst_smem, const void *src_gmem, u32 bytes, u64 *bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
-               "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
-               : "memory");
-}
-
 // NTT-domain index map of the Galois automorphism sigma_g (R2.7): position p of the transform holds the
 // evaluation at psi^(2 brev(p) + 1); sigma_g(a) evaluated there is a evaluated at psi^((2 brev(p) + 1) g).
 DEVI u32 galois_src(u32 p, u32 g, int logN) {

@@ -1,6 +1,7 @@
-// fenc_elem.cu -- element-wise kernels of the hot path: plaintext MAC (a7), ciphertext sums, encrypt / decrypt
-// combines, the counter-based samplers (R2.3) and Montgomery-form conversions.  sm_100a.
-// All are HBM-bound streaming kernels: 16-byte vector accesses, limb-major, one pass.
+// fenc_elem.cu -- element-wise kernels of the hot path: plaintext MAC (a7), the scalar MAC of factored weights (R2.9c),
+// ciphertext sums, encrypt / decrypt combines, the counter-based samplers (R2.3) and Montgomery-form
+// conversions.  sm_100a.  Limb-major, one pass; the sums, the streaming scalar MAC and the hoisted inner product use
+// 16-byte accesses, the grouped MACs 8-byte ones (one coefficient per thread, up to 8 outputs per loaded word).
 #include "fenc_device.cuh"
 
 #define PROF(k, id, bytes) if ((k).prof) prof_begin((k).prof, (k).stream, id, (double)(bytes))

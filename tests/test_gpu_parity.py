@@ -767,7 +767,6 @@ def test_lenet_conv1_full_size_sampled(mods):
     keys7 = ctx.wts_keys(conv, lay)
     wanted = {wk for ok_ in sample for lst in graph.terms[ok_].values() for _, _, wk in lst}
     oW = {wk: ck.encode(P, graph.weight_slots(wk, w), L, P.q[L - 1]) for wk in wanted}
-    gW = ctx.conv_weights(conv, lay, w, L)  # library encoder for all 2400; the sampled ones are checked against the oracle's
     o_in, g_in = {}, []
     for (u, v, g, bg) in graph.lin.ct_keys():
         pt = ck.encode(P, graph.lin.gather(x, u, v, g, bg), L)
@@ -775,8 +774,6 @@ def test_lenet_conv1_full_size_sampled(mods):
         g_in.append(ctx.encrypt(gk, ctx.pt_from_coeffs(pt.coeffs, L, float(pt.scale)), 3000 + len(g_in)))
     # weights through the oracle's integers for the sampled outputs only: rebuild the full coefficient table
     coeffs = np.zeros((len(keys7), P.N), dtype=np.int64)
-    lib = ctx.conv_weights(conv, lay, w, L)
-    del lib
     for i, k in enumerate(keys7):
         wk = tuple(int(v) for v in k)
         if wk in oW:
