@@ -340,6 +340,27 @@ fenc_status fenc_repack(fenc_ctx *ctx, const fenc_keys *keys, fenc_ct *const *in
                         const uint32_t *term_out, const uint32_t *term_src, const int32_t *term_rot, size_t n_terms,
                         int do_rescale, fenc_ct **out, size_t n_out);
 
+/* ------------------------------------------------------------------ allocation-free rescale
+ * For callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): fenc_rescale (a8; R2.8) with its intermediates in a file-scope device array of FENC_STATIC_SCRATCH_BYTES
+ * that every GPU loading the library holds until exit, instead of the context's workspace and descriptor ring.
+ * fenc_rescale_static_prepare(ctx, L) is the SET-UP step (it may allocate): builds the tables of level L and resolves the
+ * array's device address for the context's device; call it once per (context, level) before the first static call.
+ * fenc_rescale_static(ctx, in, out): out := in with its last limb dropped (floor rounding on the canonical representative,
+ * A10), bit-identical to fenc_rescale.  `in` is a ciphertext at L >= 2 limbs, `out` an EXISTING ciphertext of the same
+ * context at L-1 limbs, owned by the caller (its contents are overwritten, its scale set to in.scale / q_{L-1}); the call
+ * makes no cudaMalloc / cudaFree, no allocator callback, and creates no stream or event; work is enqueued on the
+ * context's stream.  It needs 256 + (2 + 2(L-1)) * N * 8 bytes of the array: N = 2^16 up to L = 31 (every BASELINE layer
+ * configuration: at most 30 limbs), N <= 2^15 at any level this library supports; larger requests fail with FENC_ERR_INVALID_ARG and a message naming both sizes;
+ * a level whose tables do not exist yet, a device whose array address has not been resolved (no prepare call yet in this
+ * process), or a context with the profiling hooks enabled, fails with FENC_ERR_INVALID_ARG too.
+ * Every call on a device shares the array and finds the previous call's contents in it (every word a call reads it has
+ * written first, so nothing needs clearing); calls enqueued on one stream are ordered, calls that OVERLAP on the GPU
+ * (two contexts or streams on the same device) race -- serialise them. */
+#define FENC_STATIC_SCRATCH_BYTES (32u << 20)
+fenc_status fenc_rescale_static_prepare(fenc_ctx *ctx, uint32_t L);
+fenc_status fenc_rescale_static(fenc_ctx *ctx, const fenc_ct *in, fenc_ct *out);
+
 /* ------------------------------------------------------------------ measurement helpers */
 /* Raw batched negacyclic NTT / iNTT (a1) in place on device memory: rows uint64 [n_rows][N]; mod_idx: host
  * array, row r uses modulus mod_idx[r] (0..n_q-1 ciphertext primes, n_q.. special primes). */

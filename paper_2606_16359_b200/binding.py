@@ -72,7 +72,8 @@ SYMBOLS = ["fenc_params_init", "fenc_ctx_free", "fenc_last_error", "fenc_get_pri
            "fenc_cmult_relin", "fenc_mul_scalar", "fenc_add_const", "fenc_ct_import_async", "fenc_ct_export_async",
            "fenc_export_wait", "fenc_set_hoisting", "fenc_rotate_hoisted", "fenc_square_sum_relin",
            "fenc_wts_factors", "fenc_wts_mask_slots", "fenc_conv_weights_factored", "fenc_conv_weights_factored_from_ints",
-           "fenc_measure_smac_peak", "fenc_repack", "fenc_keys_import", "fenc_sum_pool", "fenc_square_sum_pool", "fenc_poly3"]
+           "fenc_measure_smac_peak", "fenc_repack", "fenc_keys_import", "fenc_sum_pool", "fenc_square_sum_pool", "fenc_poly3",
+           "fenc_rescale_static_prepare", "fenc_rescale_static"]
 
 _lib = None
 
@@ -143,6 +144,8 @@ def load_library(path=None):
         "fenc_fc": [vp, vp, C.POINTER(FcDesc), vp, vpp, C.c_size_t, C.c_int, vpp, C.c_size_t, C.POINTER(C.c_size_t)],
         "fenc_compress": [vp, vp, vpp, C.c_size_t, vp, u32p, u32p, i32p, C.c_size_t, C.c_int, vpp, C.c_size_t],
         "fenc_ntt_rows": [vp, vp, i32p, C.c_size_t, C.c_int],
+        "fenc_rescale_static_prepare": [vp, C.c_uint32],
+        "fenc_rescale_static": [vp, vp, vp],
         "fenc_keys_import": [vp, C.POINTER(KeyMaterial), vpp],
         "fenc_sum_pool": [vp, vpp, C.c_size_t, C.c_uint32, vpp],
         "fenc_square_sum_pool": [vp, vp, vpp, C.c_size_t, C.c_uint32, vpp],
@@ -447,6 +450,15 @@ class Context:
         out = (C.c_void_p * n)()
         self._ck(self.lib.fenc_rescale(self.h, self._harr(cts), n, out))
         return [Ciphertext(self, C.c_void_p(out[i])) for i in range(n)]
+
+    def rescale_static_prepare(self, L):
+        """set-up of rescale_static for level L (may allocate)"""
+        self._ck(self.lib.fenc_rescale_static_prepare(self.h, int(L)))
+
+    def rescale_static(self, ct, out):
+        """out := rescale(ct) with no device allocation: `out` is an existing ciphertext at L-1 limbs (fenc.h)"""
+        self._ck(self.lib.fenc_rescale_static(self.h, ct.h, out.h))
+        return out
 
     def add(self, a, b):
         h = C.c_void_p()

@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfenc.so")
-SOURCES = ["fenc_ntt.cu", "fenc_elem.cu", "fenc_ctx.cu", "fenc_ops.cu", "fenc_conv.cu", "fenc_prof.cu", "fenc_host.cpp"]
+SOURCES = ["fenc_ntt.cu", "fenc_elem.cu", "fenc_ctx.cu", "fenc_ops.cu", "fenc_conv.cu", "fenc_prof.cu", "fenc_static.cu", "fenc_host.cpp"]
 HEADERS = ["fenc_internal.h", "fenc_device.cuh", "fenc_ctx.h", os.path.join("..", "..", "include", "fenc.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]
