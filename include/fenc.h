@@ -377,8 +377,9 @@ fenc_status fenc_profile_read(fenc_ctx *ctx, double *ms, uint64_t *launches, dou
  * register-only forward butterflies/s of the library's own butterfly (no memory traffic) -- the integer Shoup butterfly,
  * or, when q_0 is below 2^45 and the context's butterflies run on the FP64 pipe, the faster of that and the fp64 one. */
 fenc_status fenc_measure_alu_peak(fenc_ctx *ctx, double *imad_lane_ops_per_s, double *butterflies_per_s);
-/* The arithmetic ceiling of the scalar MAC of factored weights (R2.9c): exact x k mod q products with one add each on
- * the FP64 pipe, registers only, all SMs (q = q_0, which must be below 2^50) -- modular multiply-accumulates per second.
+/* The arithmetic ceiling of the scalar MAC of factored weights (R2.9c): its inner operation in the mode ordinary weights
+ * run in (the ciphertext word split in 2 x 25 bits times the small signed multiplier: 2 DFMA per multiply-accumulate plus
+ * the shared conversions), registers only, all SMs (q = q_0, below 2^50) -- modular multiply-accumulates per second.
  * For kernel class "smac" the second counter of fenc_profile_read holds multiply-accumulates, not butterflies. */
 fenc_status fenc_measure_smac_peak(fenc_ctx *ctx, double *mulaccs_per_s);
 /* counters since context creation: kernels launched by this library; optional reset */

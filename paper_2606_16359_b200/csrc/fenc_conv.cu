@@ -462,6 +462,27 @@ static fenc_status make_factored(fenc_ctx *ctx, ConvGraph &g, const int64_t *k, 
   W->factored = true, W->n_unique = nm, W->slot = g.mask_of;
   W->k_fp64 = true;
   for (int t = 0; t < L; t++) W->k_fp64 = W->k_fp64 && fh::f64_modulus(ctx->mod[t], ctx->logN);
+  // Mode of the scalar MAC (fenc_elem.cu): with every modulus below 2^50 and small multipliers the ciphertext word is
+  // split in 2 x 25 (or 3 x 17) bits and the SIGNED k multiplies the pieces; `lazy` products plus a reduced remainder
+  // (< 2^49) must sum exactly in a double: 2^49 + lazy 2^B kmax <= 2^53.  FENC_SMAC_MODE=1|2|3 forces a mode that is valid
+  // (diagnostics and tests: all modes give identical limbs).
+  {
+    u64 kmax = 1, qmax = 0;
+    for (size_t i = 0; i < n; i++) kmax = std::max<u64>(kmax, (u64)(k[i] < 0 ? -k[i] : k[i]));
+    for (int t = 0; t < L; t++) qmax = std::max(qmax, ctx->mod[t]);
+    const long double room = 9007199254740992.0L - 562949953421312.0L;  // 2^53 - 2^49
+    const u64 lazy2 = (u64)(room / (33554432.0L * (long double)kmax)), lazy3 = (u64)(room / (131072.0L * (long double)kmax));
+    const u64 lazy1 = (((u64)1 << 53) / qmax) - 1;
+    const char *force = getenv("FENC_SMAC_MODE");
+    const int want = force ? atoi(force) : 0;
+    int mode = !W->k_fp64 ? 0 : (lazy2 >= 8 ? 2 : (lazy3 >= 8 ? 3 : 1));
+    if (W->k_fp64 && want == 1) mode = 1;
+    if (W->k_fp64 && want == 2 && lazy2 >= 1) mode = 2;
+    if (W->k_fp64 && want == 3 && lazy3 >= 1) mode = 3;
+    W->k_mode = mode;
+    const u64 lz = mode == 2 ? lazy2 : (mode == 3 ? lazy3 : (mode == 1 ? lazy1 : (u64)std::max(1, ctx->max_lazy - 1)));
+    W->k_lazy = (int)std::min<u64>(lz, 1u << 20);
+  }
   W->d_all = dalloc_t<u64>(ctx, nm * L * N);
   W->d_k = dalloc_t<ShoupC>(ctx, n * L);
   if (!W->d_all || !W->d_k) return fail(ctx, FENC_ERR_OOM, "factored weights (%zu masks, %zu scalars)", nm, n);
@@ -483,8 +504,9 @@ static fenc_status make_factored(fenc_ctx *ctx, ConvGraph &g, const int64_t *k, 
       const u64 q = ctx->mod[t];
       const u64 mag = (u64)(k[i] < 0 ? -k[i] : k[i]) % q;
       const u64 r = (k[i] < 0 && mag) ? q - mag : mag;
-      kp[i * L + t] = W->k_fp64 ? ShoupC{fh::double_bits((double)r), fh::double_bits((double)((long double)r / (long double)q))}
-                                : ShoupC{fh::to_mont(r, q), 0};
+      kp[i * L + t] = W->k_mode >= 2 ? ShoupC{fh::double_bits((double)k[i]), 0}
+                      : W->k_mode == 1 ? ShoupC{fh::double_bits((double)r), fh::double_bits((double)((long double)r / (long double)q))}
+                                       : ShoupC{fh::to_mont(r, q), 0};
     }
   if (cudaMemcpyAsync(W->d_k, kp.data(), kp.size() * sizeof(ShoupC), cudaMemcpyHostToDevice, ctx->stream) != cudaSuccess ||
       cudaStreamSynchronize(ctx->stream) != cudaSuccess)

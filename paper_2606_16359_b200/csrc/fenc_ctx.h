@@ -135,6 +135,8 @@ struct fenc_wts {
   // factored form (R2.9c): d_all holds the n_unique distinct MASK plaintexts, slot[i] the mask of weight i, and
   // d_k the per-weight integer multipliers, [n][L] 16-byte entries (fenc_internal.h k_smac)
   bool factored = false, k_fp64 = false;
+  int k_mode = 0;        // fenc_internal.h k_smac: 0 integer, 1 fp64 residues, 2 / 3 signed multipliers (split modes)
+  int k_lazy = 1;        // terms per exact partial sum in that mode
   ShoupC *d_k = nullptr;
 };
 

@@ -202,27 +202,53 @@ int k_mac(const KCtx &k, const MacGroup *groups, int n_groups, int max_group, co
 // 2^50: t = x k - rint(x k / q) q is an exact integer in (-q, q) (fenc_device.cuh mulmod_dd, |x| < 2^51), a sum of
 // floor(2^53 / q) - 1 of them plus a reduced remainder (at most q/2 + 1 in magnitude) is exact in a double, then
 // v - rint(v / q) q brings it back.  Integer mode (larger moduli): 128-bit lazy sums of x k_mont as in the plaintext MAC.
+// Split modes (MODE 2, 3; moduli below 2^50 and small multipliers): the multiplier of a factored weight is the integer
+// k = round_half_up(v E1), a SMALL signed number (|k| < 2^26 for |v| < 2 at E1 = 2^25), not a 50-bit quantity -- only its
+// residue is.  With the ciphertext word split in P pieces of B bits, x = sum_p x_p 2^(pB), every product x_p k is below
+// 2^B kmax and `max_lazy` of them sum EXACTLY in a double by plain DFMA: P DFMA per multiply-accumulate (2 for B = 25,
+// 3 for B = 17) instead of the 7 operations of an exact 50 x 50-bit product, the pieces' conversions shared by the G
+// outputs.  A mask segment ends with S = S_0 + S_1 2^B (+ S_2 2^2B) mod q (one or two exact products per accumulator).
+// The residues are those of MODE 1 (k and k mod q differ by a multiple of q), so the outputs are bit-identical.
 struct SmacP {
   const SmacGroup *groups; const u64 *const *term_ct; const int *kidx; const ShoupC *kpair; const int *seg_end;
   const u64 *const *seg_mask; u64 *const *outs; const ModConst *mods; int L, logN, max_lazy;
+  int signed_k;  // kpair entries hold {(double) k, 0} with k the SIGNED multiplier (split modes) instead of {k mod q, (k mod q) / q}
 };
 #define SMAC_TILE 64
-template <int G, bool F64>
-__global__ void __launch_bounds__(256, G >= 8 ? 2 : 3) smac_kernel(SmacP p) {
+#ifndef SMAC_RING
+#define SMAC_RING 4  // terms whose ciphertext words are in flight per thread (grouped kernel)
+#endif
+DEVI void smac_cp_async8(u64 *dst_smem, const u64 *src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((u32)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
+}
+template <int G, int MODE>  // MODE 0: 128-bit integer sums; 1: exact fp64 products of residues; 2 / 3: split modes with 2 x 25 / 3 x 17 bits
+__global__ void __launch_bounds__(256, (G >= 8 || MODE == 3) ? 2 : 3) smac_kernel(SmacP p) {
+  constexpr bool F64 = MODE == 1;
+  constexpr bool SPLIT = MODE >= 2;
+  constexpr int NP = MODE == 3 ? 3 : 2, PB = MODE == 3 ? 17 : 25;  // pieces and bits per piece (split modes)
   __shared__ const u64 *s_ct[SMAC_TILE];
   __shared__ ulonglong2 s_k[G][SMAC_TILE];
+  __shared__ u64 s_ring[G >= 4 ? SMAC_RING : 1][2][G >= 4 ? 256 : 1];
   const size_t LN = (size_t)p.L << p.logN;
   const size_t idx = (size_t)blockIdx.y * blockDim.x + threadIdx.x;  // blockDim divides N: idx < L N, one limb per block
   const int limb = (int)(((size_t)blockIdx.y * blockDim.x) >> p.logN);
   const SmacGroup g = p.groups[blockIdx.x];
   const ModConst mc = p.mods[limb];
   const F64Mod fm = f64mod(mc.q, mc.f64);
-  double acc[G][2];
-  u64 lo[F64 ? 1 : G][2], hi[F64 ? 1 : G][2], tot[G][2];
+  double acc[F64 ? G : 1][2];
+  double sp[SPLIT ? G : 1][2][NP];
+  u64 lo[MODE == 0 ? G : 1][2], hi[MODE == 0 ? G : 1][2], tot[G][2];
 #pragma unroll
   for (int i = 0; i < G; i++) {
-    acc[i][0] = acc[i][1] = 0.0, tot[i][0] = tot[i][1] = 0;
-    if (!F64) lo[i][0] = lo[i][1] = hi[i][0] = hi[i][1] = 0;
+    tot[i][0] = tot[i][1] = 0;
+    if (F64) acc[i][0] = acc[i][1] = 0.0;
+    if (MODE == 0) lo[i][0] = lo[i][1] = hi[i][0] = hi[i][1] = 0;
+    if (SPLIT) {
+#pragma unroll
+      for (int c = 0; c < 2; c++)
+#pragma unroll
+        for (int q2 = 0; q2 < NP; q2++) sp[i][c][q2] = 0.0;
+    }
   }
   int seg = 0, cur_end = p.seg_end[g.seg_start], lazy = 0;
   for (int t0 = 0; t0 < g.n_terms; t0 += SMAC_TILE) {
@@ -240,22 +266,62 @@ __global__ void __launch_bounds__(256, G >= 8 ? 2 : 3) smac_kernel(SmacP p) {
     __syncthreads();
     // the next term's ciphertext words are requested before this term's products (register double buffer): with two blocks
     // of 8 warps per SM the loads would otherwise sit in front of 112 dependent FP64 operations
-    u64 nx0 = 0, nx1 = 0;
-    if (G >= 4) nx0 = __ldg(s_ct[0] + idx), nx1 = __ldg(s_ct[0] + LN + idx);
+    // Groups of 4 and more outputs: the ciphertext words of the next SMAC_RING - 1 terms are in flight while this term's
+    // products run.  A term's arithmetic (about 300 clocks per scheduler with four warps) is shorter than an L2 / HBM
+    // round trip, so with one term ahead the loop ran at the memory latency (measured: 2 TB/s of operand traffic, a
+    // quarter of what the FP64 pipe would allow).  The ring lives in shared memory (cp.async, 8 bytes per copy): each
+    // thread owns its slots, so no barrier is needed and no register is spent on the depth.
+    auto ring_issue = [&](int t) {
+      if (t < nt) {
+        const u64 *c = s_ct[t];
+        smac_cp_async8(&s_ring[t % SMAC_RING][0][threadIdx.x], c + idx);
+        smac_cp_async8(&s_ring[t % SMAC_RING][1][threadIdx.x], c + LN + idx);
+      }
+      asm volatile("cp.async.commit_group;" ::: "memory");  // a group per term, empty past the end: the wait below counts groups
+    };
+    if (G >= 4) {
+#pragma unroll
+      for (int t = 0; t < SMAC_RING - 1; t++) ring_issue(t);
+    }
 #pragma unroll 2
     for (int t = 0; t < nt; t++) {
       u64 x0, x1;
       if (G >= 4) {
-        x0 = nx0, x1 = nx1;
-        if (t + 1 < nt) {
-          const u64 *c = s_ct[t + 1];
-          nx0 = __ldg(c + idx), nx1 = __ldg(c + LN + idx);
-        }
+        ring_issue(t + SMAC_RING - 1);  // overwrites the slot of term t - 1, already consumed by this thread
+        asm volatile("cp.async.wait_group %0;" ::"n"(SMAC_RING - 1) : "memory");
+        x0 = s_ring[t % SMAC_RING][0][threadIdx.x], x1 = s_ring[t % SMAC_RING][1][threadIdx.x];
       } else {
         const u64 *c = s_ct[t];
         x0 = __ldg(c + idx), x1 = __ldg(c + LN + idx);
       }
-      if (F64) {
+      if (SPLIT) {
+        constexpr u32 pm = (1u << PB) - 1u;
+        double xp[2][NP];
+#pragma unroll
+        for (int c = 0; c < 2; c++) {
+          const u64 x = c ? x1 : x0;  // below 2^50: the top piece fits 32 bits in both splits
+          xp[c][0] = u2d((u32)x & pm);
+          if (NP == 2) xp[c][1] = u2d((u32)(x >> PB));
+          else xp[c][1] = u2d((u32)(x >> PB) & pm), xp[c][NP - 1] = u2d((u32)(x >> (2 * PB)));
+        }
+#pragma unroll
+        for (int i = 0; i < G; i++) {
+          const double kd = __longlong_as_double((long long)s_k[i][t].x);
+#pragma unroll
+          for (int c = 0; c < 2; c++)
+#pragma unroll
+            for (int q2 = 0; q2 < NP; q2++) sp[i][c][q2] = __fma_rn(xp[c][q2], kd, sp[i][c][q2]);
+        }
+        if (++lazy == p.max_lazy) {  // every partial sum back to at most q/2 in magnitude (congruent mod q): exactness budget restored
+#pragma unroll
+          for (int i = 0; i < G; i++)
+#pragma unroll
+            for (int c = 0; c < 2; c++)
+#pragma unroll
+              for (int q2 = 0; q2 < NP; q2++) sp[i][c][q2] = reduce_dd(sp[i][c][q2], fm);
+          lazy = 0;
+        }
+      } else if (F64) {
         const double xd0 = u2d52(x0), xd1 = u2d52(x1);
 #pragma unroll
         for (int i = 0; i < G; i++) {
@@ -292,7 +358,18 @@ __global__ void __launch_bounds__(256, G >= 8 ? 2 : 3) smac_kernel(SmacP p) {
 #pragma unroll
           for (int cpn = 0; cpn < 2; cpn++) {
             u64 S;
-            if (F64) {
+            if (SPLIT) {
+              // S_0 + S_1 2^B (+ S_2 2^2B) mod q: the powers of two as representatives in [-q/2, q/2], exact products
+              const double c1 = reduce_dd((double)(1ull << PB), fm);
+              double r = __dadd_rn(reduce_dd(sp[i][cpn][0], fm), mulmod_dd(reduce_dd(sp[i][cpn][1], fm), c1, __dmul_rn(c1, fm.qinv), fm));
+              if (NP == 3) {
+                const double c2 = reduce_dd((double)(1ull << (2 * PB)), fm);
+                r = __dadd_rn(r, mulmod_dd(reduce_dd(sp[i][cpn][NP - 1], fm), c2, __dmul_rn(c2, fm.qinv), fm));
+              }
+              S = csub(d2u_off(reduce_dd(r, fm), fm.q + 4503599627370496.0), mc.q);
+#pragma unroll
+              for (int q2 = 0; q2 < NP; q2++) sp[i][cpn][q2] = 0.0;
+            } else if (F64) {
               S = csub(d2u_off(reduce_dd(acc[i][cpn], fm), fm.q + 4503599627370496.0), mc.q);
               acc[i][cpn] = 0.0;
             } else {
@@ -332,6 +409,7 @@ __global__ void __launch_bounds__(256, 4) smac1_kernel(SmacP p) {
   int seg = 0, cur_end = p.seg_end[g.seg_start], lazy = 0;
   auto term = [&](const ulonglong2 &a, const ulonglong2 &b, int t) {
     const ulonglong2 kk = s_k[t];
+    // (split-mode tables hold the SIGNED k, |k| < 2^35: x k is still exact as h + l and the quotient estimate from k / q holds)
     const double kd = __longlong_as_double((long long)kk.x), kq = __longlong_as_double((long long)kk.y);
     acc[0] = __dadd_rn(acc[0], mulmod_dd(u2d52(a.x), kd, kq, fm));
     acc[1] = __dadd_rn(acc[1], mulmod_dd(u2d52(a.y), kd, kq, fm));
@@ -348,7 +426,9 @@ __global__ void __launch_bounds__(256, 4) smac1_kernel(SmacP p) {
     __syncthreads();
     for (int t = threadIdx.x; t < nt; t += blockDim.x) {
       s_ct[t] = p.term_ct[g.ct_start + t0 + t];
-      s_k[t] = __ldg(reinterpret_cast<const ulonglong2 *>(p.kpair) + (size_t)p.kidx[g.k_start + t0 + t] * p.L + limb);
+      ulonglong2 kk = __ldg(reinterpret_cast<const ulonglong2 *>(p.kpair) + (size_t)p.kidx[g.k_start + t0 + t] * p.L + limb);
+      if (p.signed_k) kk.y = (u64)__double_as_longlong(__dmul_rn(__longlong_as_double((long long)kk.x), fm.qinv));  // k / q for the signed k
+      s_k[t] = kk;
     }
     __syncthreads();
     int t = 0;
@@ -388,24 +468,28 @@ __global__ void __launch_bounds__(256, 4) smac1_kernel(SmacP p) {
   *reinterpret_cast<ulonglong2 *>(out + idx) = make_ulonglong2(tot[0], tot[1]);
   *reinterpret_cast<ulonglong2 *>(out + LN + idx) = make_ulonglong2(tot[2], tot[3]);
 }
-template <bool F64>
+template <int MODE>
 static void launch_smac(const SmacP &p, dim3 grid, int nth, cudaStream_t st, int max_group) {
-  if (max_group <= 1) smac_kernel<1, F64><<<grid, nth, 0, st>>>(p);
-  else if (max_group <= 2) smac_kernel<2, F64><<<grid, nth, 0, st>>>(p);
-  else if (max_group <= 4) smac_kernel<4, F64><<<grid, nth, 0, st>>>(p);
-  else smac_kernel<FENC_SMAC_GROUP, F64><<<grid, nth, 0, st>>>(p);
+  if (max_group <= 1) smac_kernel<1, MODE><<<grid, nth, 0, st>>>(p);
+  else if (max_group <= 2) smac_kernel<2, MODE><<<grid, nth, 0, st>>>(p);
+  else if (max_group <= 4 || MODE == 3) smac_kernel<4, MODE><<<grid, nth, 0, st>>>(p);  // MODE 3: the caller groups by 4 (3 sums per accumulator)
+  else smac_kernel<FENC_SMAC_GROUP, MODE><<<grid, nth, 0, st>>>(p);
 }
+// k_mode: 0 integer, 1 fp64 residues, 2 / 3 signed multipliers with the ciphertext word split in 2 x 25 / 3 x 17 bits
 int k_smac(const KCtx &k, const SmacGroup *groups, int n_groups, int max_group, const u64 *const *term_ct, const int *kidx,
-           const ShoupC *kpair, const int *seg_end, const u64 *const *seg_mask, u64 *const *outs, int L, bool fp64_mode,
+           const ShoupC *kpair, const int *seg_end, const u64 *const *seg_mask, u64 *const *outs, int L, int k_mode,
            int max_lazy, double alg_bytes, double alg_mulaccs) {
   if (n_groups == 0) return 0;
-  SmacP p{groups, term_ct, kidx, kpair, seg_end, seg_mask, outs, k.d_mods, L, k.geom.logN, max_lazy < 2 ? 2 : max_lazy};
+  if (k_mode == 3 && max_group > 4) return -3;
+  SmacP p{groups, term_ct, kidx, kpair, seg_end, seg_mask, outs, k.d_mods, L, k.geom.logN, max_lazy < 2 ? 2 : max_lazy, k_mode >= 2 ? 1 : 0};
   const int nth = k.N < 256 ? k.N : 256;
   dim3 grid(n_groups, (unsigned)(((size_t)L * k.N) / nth));
   PROF2(k, K_SMAC, alg_bytes, alg_mulaccs);  // second counter of this class: modular multiply-accumulates
-  if (fp64_mode && max_group <= 1 && k.N >= 512) smac1_kernel<<<dim3(n_groups, (unsigned)(((size_t)L * k.N) / 512)), 256, 0, S(k)>>>(p);
-  else if (fp64_mode) launch_smac<true>(p, grid, nth, S(k), max_group);
-  else launch_smac<false>(p, grid, nth, S(k), max_group);
+  if (k_mode >= 1 && max_group <= 1 && k.N >= 512) smac1_kernel<<<dim3(n_groups, (unsigned)(((size_t)L * k.N) / 512)), 256, 0, S(k)>>>(p);
+  else if (k_mode == 3) launch_smac<3>(p, grid, nth, S(k), max_group);
+  else if (k_mode == 2) launch_smac<2>(p, grid, nth, S(k), max_group);
+  else if (k_mode == 1) launch_smac<1>(p, grid, nth, S(k), max_group);
+  else launch_smac<0>(p, grid, nth, S(k), max_group);
   LAUNCH_CHECK(k);
   return 0;
 }

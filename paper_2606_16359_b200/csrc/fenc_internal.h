@@ -156,9 +156,10 @@ int k_mac(const KCtx &k, const MacGroup *groups, int n_groups, int max_group, co
 struct SmacGroup {
   int n_out, n_terms, ct_start, k_start, out_start, seg_start, n_seg, pad;
 };
-// kpair: [n_w][L] 16-byte entries: fp64 mode {(double) k, (double)(k / q)}, integer mode {k 2^64 mod q, 0}
+// kpair: [n_w][L] 16-byte entries: k_mode 0 {k 2^64 mod q, 0}; 1 {(double)(k mod q), (double)((k mod q) / q)};
+// 2, 3 {(double) k signed, 0} (fenc_elem.cu: the ciphertext word split in 2 x 25 / 3 x 17 bits; mode 3 groups <= 4 outputs)
 int k_smac(const KCtx &k, const SmacGroup *groups, int n_groups, int max_group, const u64 *const *term_ct, const int *kidx,
-           const ShoupC *kpair, const int *seg_end, const u64 *const *seg_mask, u64 *const *outs, int L, bool fp64_mode,
+           const ShoupC *kpair, const int *seg_end, const u64 *const *seg_mask, u64 *const *outs, int L, int k_mode,
            int max_lazy, double alg_bytes, double alg_mulaccs);
 // outs[o] = sum of listed [2][L][N] arrays
 int k_add_many(const KCtx &k, const u64 *const *term, const int *start, u64 *const *outs, int n_out, int L, int n_terms);

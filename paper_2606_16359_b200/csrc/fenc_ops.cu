@@ -433,8 +433,9 @@ fenc_status run_smac(fenc_ctx *ctx, const SmacJob &job, const fenc_wts *W, int L
     std::vector<const u64 *> masks;
     for (int t = 0; t < nt; t++)
       if (t + 1 == nt || seq.second[t + 1] != seq.second[t]) ends.push_back(t + 1), masks.push_back(seq.second[t]);
-    for (size_t at = 0; at < members.size(); at += FENC_SMAC_GROUP) {
-      const int ng = (int)std::min<size_t>(FENC_SMAC_GROUP, members.size() - at);
+    const size_t gcap = W->k_mode == 3 ? 4 : FENC_SMAC_GROUP;  // three partial sums per accumulator: groups of 4 outputs
+    for (size_t at = 0; at < members.size(); at += gcap) {
+      const int ng = (int)std::min<size_t>(gcap, members.size() - at);
       groups.push_back(SmacGroup{ng, nt, (int)tc.size(), (int)kidx.size(), (int)outs.size(), (int)seg_end.size(), (int)ends.size(), 0});
       tc.insert(tc.end(), seq.first.begin(), seq.first.end());
       seg_end.insert(seg_end.end(), ends.begin(), ends.end());
@@ -455,11 +456,9 @@ fenc_status run_smac(fenc_ctx *ctx, const SmacJob &job, const fenc_wts *W, int L
   const double bytes = mac_alg_bytes(ctx, tc, all_masks, n, L) + 16.0 * L * (double)W->n;
   double mulaccs = 0;
   for (auto &tl : job.terms) mulaccs += 2.0 * (double)tl.size() * L * ctx->N;
-  const u64 qmax = *std::max_element(ctx->mod.begin(), ctx->mod.begin() + L);
-  const int lazy = W->k_fp64 ? (int)std::min<u64>(((u64)1 << 53) / qmax, 1u << 20) - 1 : ctx->max_lazy - 1;
   CUDA_OK(ctx, k_smac(ctx->k, (const SmacGroup *)(base + o0), (int)groups.size(), max_group, (const u64 *const *)(base + o1),
                       (const int *)(base + o2), W->d_k, (const int *)(base + o3), (const u64 *const *)(base + o4),
-                      (u64 *const *)(base + o5), L, W->k_fp64, lazy, bytes, mulaccs));
+                      (u64 *const *)(base + o5), L, W->k_mode, W->k_lazy, bytes, mulaccs));
   return FENC_OK;
 }
 // algorithmic bytes of one MAC launch: every distinct ciphertext and plaintext read once, every output written once

@@ -140,40 +140,46 @@ __global__ void __launch_bounds__(256) butterfly_f64_peak_kernel(u64 *out, u64 q
   for (int k = 0; k < 8; k++) s ^= y[k];
   out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
-// the scalar MAC's inner operation (fenc_elem.cu smac_kernel, fp64 mode) on registers only: 16 accumulators, one exact
-// x k mod q product and one add each per step, reduced every 7 steps as for a 50-bit modulus
-__global__ void __launch_bounds__(256) smac_peak_kernel(u64 *out, u64 q, u64 qinv_bits, u64 c_bits, u64 cq_bits, int iters) {
+// the scalar MAC's inner operation (fenc_elem.cu smac_kernel, the 2 x 25-bit split mode ordinary weights run in) on
+// registers only: per term two ciphertext words are split in two pieces each (4 conversions) and multiplied into 8 x 2 x 2
+// partial sums by DFMA -- 16 multiply-accumulates for 32 DFMA --, the sums reduced every 32 terms
+__global__ void __launch_bounds__(256, 2) smac_peak_kernel(u64 *out, u64 q, u64 qinv_bits, u64 c_bits, u64 cq_bits, int iters) {
   const F64Mod fm = f64mod(q, qinv_bits);
-  double acc[16], cs[8], cqs[8];
-  double x0 = u2d52((threadIdx.x * 7919u + blockIdx.x) % q), x1 = u2d52((threadIdx.x * 104729u + blockIdx.x) % q);
+  double sp[8][2][2], kd[8];
+  u64 x0 = (threadIdx.x * 7919u + blockIdx.x) % q, x1 = (threadIdx.x * 104729u + blockIdx.x) % q;
 #pragma unroll
-  for (int k = 0; k < 8; k++) {  // eight scalars (one per output of a group), each with its quotient constant
-    cs[k] = __longlong_as_double((long long)c_bits) - (double)k;
-    cqs[k] = cs[k] * fm.qinv;
+  for (int i = 0; i < 8; i++) {
+    kd[i] = 1048573.0 - 37.0 * i;  // eight small multipliers, as round(v 2^25) of ordinary weights
+    sp[i][0][0] = sp[i][0][1] = sp[i][1][0] = sp[i][1][1] = 0.0;
   }
-#pragma unroll
-  for (int k = 0; k < 16; k++) acc[k] = 0.0;
   for (int it = 0; it < iters; it++) {
+#pragma unroll 4
+    for (int u = 0; u < 32; u++) {
+      const double a0 = __hiloint2double(0x43300000, (int)((u32)x0 & 0x1FFFFFFu)) - 4503599627370496.0;
+      const double a1 = __hiloint2double(0x43300000, (int)(u32)(x0 >> 25)) - 4503599627370496.0;
+      const double b0 = __hiloint2double(0x43300000, (int)((u32)x1 & 0x1FFFFFFu)) - 4503599627370496.0;
+      const double b1 = __hiloint2double(0x43300000, (int)(u32)(x1 >> 25)) - 4503599627370496.0;
 #pragma unroll
-    for (int u = 0; u < 7; u++) {
-#pragma unroll
-      for (int k = 0; k < 8; k++) {
-        acc[2 * k] = __dadd_rn(acc[2 * k], mulmod_dd(x0, cs[k], cqs[k], fm));
-        acc[2 * k + 1] = __dadd_rn(acc[2 * k + 1], mulmod_dd(x1, cs[k], cqs[k], fm));
+      for (int i = 0; i < 8; i++) {
+        sp[i][0][0] = __fma_rn(a0, kd[i], sp[i][0][0]), sp[i][0][1] = __fma_rn(a1, kd[i], sp[i][0][1]);
+        sp[i][1][0] = __fma_rn(b0, kd[i], sp[i][1][0]), sp[i][1][1] = __fma_rn(b1, kd[i], sp[i][1][1]);
       }
-      x0 += 1.0, x1 += 3.0;  // a new ciphertext word per term (stays far below 2^51 over the run)
+      x0 += 0x9E3779B1ull, x1 += 0x85EBCA77ull;  // a new ciphertext word per term
+      x0 &= 0x3FFFFFFFFFFFFull, x1 &= 0x3FFFFFFFFFFFFull;  // below 2^50
     }
 #pragma unroll
-    for (int k = 0; k < 16; k++) acc[k] = reduce_dd(acc[k], fm);
+    for (int i = 0; i < 8; i++)
+      sp[i][0][0] = reduce_dd(sp[i][0][0], fm), sp[i][0][1] = reduce_dd(sp[i][0][1], fm), sp[i][1][0] = reduce_dd(sp[i][1][0], fm),
+      sp[i][1][1] = reduce_dd(sp[i][1][1], fm);
   }
   double s = 0;
 #pragma unroll
-  for (int k = 0; k < 16; k++) s += acc[k];
-  out[blockIdx.x * blockDim.x + threadIdx.x] = (u64)__double_as_longlong(s);
+  for (int i = 0; i < 8; i++) s += sp[i][0][0] + sp[i][0][1] + sp[i][1][0] + sp[i][1][1];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = (u64)__double_as_longlong(s) ^ c_bits ^ cq_bits;
 }
 extern "C" fenc_status fenc_measure_smac_peak(fenc_ctx *ctx, double *mulaccs_per_s) {
   if (!ctx || !mulaccs_per_s) return FENC_ERR_INVALID_ARG;
-  const int blocks = 148 * 8, iters = 1024;
+  const int blocks = 148 * 8, iters = 256;
   u64 *buf = dalloc_t<u64>(ctx, (size_t)blocks * 256);
   if (!buf) return fail(ctx, FENC_ERR_OOM, "peak buffer");
   cudaEvent_t e0, e1;
@@ -189,7 +195,7 @@ extern "C" fenc_status fenc_measure_smac_peak(fenc_ctx *ctx, double *mulaccs_per
     CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
     cudaEventElapsedTime(&ms, e0, e1);
   }
-  *mulaccs_per_s = (double)blocks * 256 * 16.0 * 7.0 * iters / (ms * 1e-3);
+  *mulaccs_per_s = (double)blocks * 256 * 16.0 * 32.0 * iters / (ms * 1e-3);
   cudaEventDestroy(e0), cudaEventDestroy(e1);
   dfree(ctx, buf);
   ctx->launches += 2;

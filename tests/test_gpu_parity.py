@@ -234,11 +234,12 @@ def test_hconv_hoisted_inner_rotations_bit_exact(mods, name, conv_kw, S):
     ctx.close()
 
 
-def run_hconv_factored(mods, P, ctx, conv_kw, S, seed, hoist=False):
+def run_hconv_factored(mods, P, ctx, conv_kw, S, seed, hoist=False, w_scale=1.0):
     """GPU fenc_hconv with factored weights (R2.9c) vs the oracle's hconv_factored for every batch group; parity starts at
     the integer multipliers and the masks' integer coefficients (A7).  Returns the max decoded error."""
     ck, fr, fenc = mods
     x, w = wl.conv_inputs(seed, conv_kw)
+    w = w * w_scale
     od = fr.ConvDesc(S=S, **conv_kw)
     graph = fr.ConvGraph(od, P.n)
     conv = ctx.conv_desc(S=S, **conv_kw)
@@ -296,7 +297,7 @@ def run_hconv_factored(mods, P, ctx, conv_kw, S, seed, hoist=False):
                 for vo in range(So):
                     ctx.decrypt_decode(gk, outs2[i], conv, lay, 1, uo, vo, go, bg, Y2)
                     i += 1
-    assert np.abs(Y2 - Y).max() < 1e-5
+    assert np.abs(Y2 - Y).max() < 1e-5 * max(1.0, w_scale)
     return err
 
 
@@ -314,6 +315,30 @@ def test_hconv_factored_weights_bit_exact(mods, name, over, conv_kw, S, hoist):
     P, ctx = make(mods, name, **over)
     err = run_hconv_factored(mods, P, ctx, conv_kw, S, seed=6, hoist=hoist)
     assert err < (1e-3 if name != "toy64" else 5e-2)
+    ctx.close()
+
+
+@pytest.mark.parametrize("mode", ["1", "2", "3"])
+@pytest.mark.parametrize("name,over", [("mid12", dict(q_bits=50, log2_scale=50)), ("mid10", {})])
+def test_smac_modes_give_identical_limbs(mods, monkeypatch, name, over, mode):
+    """The scalar MAC's arithmetic modes (fenc_elem.cu: exact fp64 products of residues; the ciphertext word split in
+    2 x 25 or 3 x 17 bits times the SIGNED multiplier) forced one by one on the same layer: each equals the oracle's
+    factored variant limb by limb.  9 output channels: groups of 8 + 1 outputs (4 + 4 + 1 in the 3-piece mode), hoisted."""
+    monkeypatch.setenv("FENC_SMAC_MODE", mode)
+    P, ctx = make(mods, name, **over)
+    err = run_hconv_factored(mods, P, ctx, dict(BS=32, C_in=3, H=8, W=8, C_out=9, K=3, stride=1, pad=1), 1, seed=7, hoist=True)
+    assert err < 1e-3
+    ctx.close()
+
+
+@pytest.mark.parametrize("w_scale,bound", [(12.0, 1e-3), (4000.0, None)])
+def test_smac_mode_selection_for_large_multipliers(mods, w_scale, bound):
+    """Weights 12 x larger (|k| up to 2^30: the 2-piece products no longer sum exactly, the library picks 3 pieces) and
+    4000 x larger (|k| beyond 2^36: back to exact products of residues): limbs against the oracle in both; the decoded
+    bar only where the outputs stay of ordinary size."""
+    P, ctx = make(mods, "mid12", q_bits=50, log2_scale=50)
+    err = run_hconv_factored(mods, P, ctx, dict(BS=32, C_in=3, H=8, W=8, C_out=5, K=3, stride=1, pad=1), 1, seed=9, w_scale=w_scale)
+    assert bound is None or err < bound
     ctx.close()
 
 
