@@ -310,9 +310,11 @@ int k_convert_cols(const KCtx &k, u64 *y, size_t y_bstride, const ConvGroup *gro
   ConvColP p{y, y_bstride, groups, scale, bc, rows, tmp, tmp_bstride, k.d_mods, k.d_tw_fwd, k.d_tw_inv, g.logN, g.brow, max_terms,
              merged_pinv, bc_f64};
   dim3 grid(k.N >> 10, n_groups, n_batch);
-  // algorithmic bytes: every target row written once (+ the sources, counted by the caller's row pass); butterflies of
-  // the forward column stages of every target (the inverse ones of the sources are the smaller part)
-  PROF(k, K_NTT_COL_BCONV, 8.0 * k.N * n_batch * (double)n_tgt_total, HALF_N(k) * g.bcol * (double)n_tgt_total * n_batch);
+  // algorithmic bytes: every target row written once (+ the sources, counted by the caller's row pass); butterflies: the
+  // forward column stages of every target AND the inverse column stages of every source row (y holds y_bstride / N of them
+  // per item at every call site); the base-conversion products (targets x sources per coefficient) are not counted
+  PROF(k, K_NTT_COL_BCONV, 8.0 * k.N * n_batch * (double)n_tgt_total,
+       HALF_N(k) * g.bcol * ((double)n_tgt_total + (double)(y_bstride / (size_t)k.N)) * n_batch);
 #define LAUNCH_CONV1(B, M, G)                                                                                                         \
   do {                                                                                                                                \
     if (smem > 48 * 1024) cudaFuncSetAttribute(convert_cols_kernel<B, M, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
