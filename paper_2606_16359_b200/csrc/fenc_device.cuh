@@ -114,7 +114,12 @@ DEVI u64 mulmod_f64(u64 x, u64 c_bits, u64 cq_bits, const F64Mod &m) {  // (0, 2
 // shared-memory slot is swz(ebase) ^ swz(k << PW): one base computation per thread and round.
 
 // compile-time round: window position and active stages [SLO, SHI) are constants (production geometries)
-template <bool FWD, bool LAZY, int PW, int SLO, int SHI, int F64>  // F64: 0 integer, 1 fp64 narrow (q < 2^45), 2 fp64 wide
+// FIRST / LAST (fp64 rounds): whether this is the first / last round of the transform.  Between the rounds of one
+// transform the tile holds the values as DOUBLES (signed, exact integers; reduced to at most q/2 in magnitude wherever a
+// round ends with a reduction); only the first round converts from the unsigned words of the fill and only the last one
+// back to the unsigned lazy words every consumer expects.  ncu on the fused column kernel (profiles/r02_cfg4_step_ncu.md):
+// FP64 pipe 59 % busy, and a quarter of its FP64 instructions were these per-round conversions.
+template <bool FWD, bool LAZY, int PW, int SLO, int SHI, int F64, bool FIRST = true, bool LAST = true>  // F64: 0 integer, 1 fp64 narrow (q < 2^45), 2 fp64 wide
 DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid, u64 f64) {
   const int ebase = ((tid >> PW) << (PW + 3)) | (tid & ((1 << PW) - 1));
   const int gpw = G.gbit(PW);
@@ -130,9 +135,9 @@ DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 
   const int sbase = swz(ebase);
   if constexpr (F64 != 0) {
     // The eight values stay doubles (signed, exact integers) through the round's stages; T is in (-q, q).
-    // Narrow moduli (q < 2^45): a forward stage moves a value by less than q either way; the stored value, shifted by
-    // +3q, stays non-negative and grows by at most 6q per round (36q after the five rounds of a 2^16 transform, inside
-    // the 2^51 the multiply accepts); an inverse round ends with v - rint(v/q) q + q in [0, 2q).
+    // Narrow moduli (q < 2^45): a forward stage moves a value by less than q either way, so after the (at most 16) stages
+    // of a pass a value that entered below 2^50 is below 2^50 + 16 q < 2^51 in magnitude, inside what the multiply
+    // accepts, and no forward round reduces; an inverse round ends with v - rint(v/q) q (+ q in the last round: [0, 2q)).
     // Wide moduli (2^45 <= q < 2^50, compile-time schedules only): every round starts from values in [0, 2q], centred
     // to [-q, q] while converting, and ends with the same reduction in both directions; an operand that can exceed 2q
     // (third forward stage, second and third inverse stage) is reduced before it is multiplied, so the quotient
@@ -144,7 +149,7 @@ DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 
 #pragma unroll
     for (int k = 0; k < 8; k++) {
       const u64 v = sm[sbase ^ swz(k << PW)];
-      x[k] = __dadd_rn(__hiloint2double((int)((u32)(v >> 32) | 0x43300000u), (int)(u32)v), in_off);
+      x[k] = FIRST ? __dadd_rn(__hiloint2double((int)((u32)(v >> 32) | 0x43300000u), (int)(u32)v), in_off) : __longlong_as_double((long long)v);
     }
     int done = 0;
 #pragma unroll
@@ -173,9 +178,16 @@ DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 
       }
     }
     const bool red = !FWD || wide;
-    const double off = red ? __dadd_rn(fm.q, 4503599627370496.0) : __fma_rn(3.0, fm.q, 4503599627370496.0);
+    if (LAST) {
+      // narrow forward values are signed and have moved by less than q per stage since the fill (at most 16 stages): + 16 q
+      // makes them non-negative and keeps them below 2^52; reduced values (+ q) land in (0, 2q)
+      const double off = red ? __dadd_rn(fm.q, 4503599627370496.0) : __fma_rn(16.0, fm.q, 4503599627370496.0);
 #pragma unroll
-    for (int k = 0; k < 8; k++) sm[sbase ^ swz(k << PW)] = d2u_off(red ? reduce_dd(x[k], fm) : x[k], off);
+      for (int k = 0; k < 8; k++) sm[sbase ^ swz(k << PW)] = d2u_off(red ? reduce_dd(x[k], fm) : x[k], off);
+    } else {
+#pragma unroll
+      for (int k = 0; k < 8; k++) sm[sbase ^ swz(k << PW)] = (u64)__double_as_longlong(red ? reduce_dd(x[k], fm) : x[k]);
+    }
   } else {
   u64 x[8];
 #pragma unroll
@@ -219,7 +231,7 @@ DEVI void tile_rounds_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64
     constexpr int cur = FWD ? LO + NB - DONE : LO + DONE;         // FWD: exclusive top; INV: inclusive bottom
     constexpr int p = FWD ? cur - take : cur;
     constexpr int pw = p < LT - 3 ? p : LT - 3;
-    if (tid < (1 << (LT - 3))) tile_round_ct<FWD, LAZY, pw, p - pw, p - pw + take, F64>(sm, G, tw, q, q2, tid, f64);
+    if (tid < (1 << (LT - 3))) tile_round_ct<FWD, LAZY, pw, p - pw, p - pw + take, F64, DONE == 0, (DONE + take >= NB)>(sm, G, tw, q, q2, tid, f64);
     tile_sync<GRP>(bar);
     tile_rounds_ct<FWD, LAZY, LT, LO, NB, DONE + take, F64, GRP>(sm, G, tw, q, q2, tid, f64, bar);
   }
