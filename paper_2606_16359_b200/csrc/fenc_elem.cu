@@ -127,10 +127,17 @@ struct MacState {
 #ifndef MAC_THREADS
 #define MAC_THREADS 256
 #endif
+#ifndef MAC_RING
+#define MAC_RING 3  // terms whose operands are in flight per thread (36 KiB of shared memory at 4 outputs per group)
+#endif
+DEVI void mac_cp_async8(u64 *dst_smem, const u64 *src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((u32)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
+}
 template <int G, int MODE>
 __global__ void __launch_bounds__(MAC_THREADS, 512 / MAC_THREADS) mac_kernel(MacP p) {
   __shared__ const u64 *s_ct[MAC_TILE];
   __shared__ const u64 *s_pt[G][MAC_TILE];
+  __shared__ u64 s_ring[MODE == 2 ? 1 : MAC_RING][MODE == 2 ? 1 : 2 + G][MODE == 2 ? 1 : MAC_THREADS];
   const size_t LN = (size_t)p.L << p.logN;
   const size_t idx = (size_t)blockIdx.y * blockDim.x + threadIdx.x;
   const bool live = idx < LN;
@@ -149,13 +156,43 @@ __global__ void __launch_bounds__(MAC_THREADS, 512 / MAC_THREADS) mac_kernel(Mac
     }
     __syncthreads();
     if (!live) continue;
+    // Integer modes (0, 1): the operands of the next MAC_RING - 1 terms are in flight while this term's products run, in a
+    // per-thread cp.async ring in shared memory (every thread owns its slots: no barrier, no registers spent on the depth):
+    // config 3's 26-bit-limb MAC -11 %.  The fp64 mode (2) keeps plain loads: measured with the ring it is 8 % SLOWER
+    // (config 2's conv2: 1.38 -> 1.49 ms) -- it is bound by its 10 FP64 operations per output-term, not by the latency,
+    // and the ring's shared-memory traffic competes with them (round 1 saw the same with every staged variant).
+    if (MODE == 2) {
+#pragma unroll 2
+      for (int t = 0; t < nt; t++) {
+        const u64 *c = s_ct[t];
+        const u64 x0 = __ldg(c + idx), x1 = __ldg(c + LN + idx);
+        u64 w[G];
+#pragma unroll
+        for (int i = 0; i < G; i++) w[i] = __ldg(s_pt[i][t] + idx);
+        st.mac(x0, x1, w, mc);
+      }
+      continue;
+    }
+    auto ring_issue = [&](int t) {
+      if (t < nt) {
+        const u64 *c = s_ct[t];
+        mac_cp_async8(&s_ring[t % MAC_RING][0][threadIdx.x], c + idx);
+        mac_cp_async8(&s_ring[t % MAC_RING][1][threadIdx.x], c + LN + idx);
+#pragma unroll
+        for (int i = 0; i < G; i++) mac_cp_async8(&s_ring[t % MAC_RING][2 + i][threadIdx.x], s_pt[i][t] + idx);
+      }
+      asm volatile("cp.async.commit_group;" ::: "memory");  // one group per term, empty past the end
+    };
+#pragma unroll
+    for (int t = 0; t < MAC_RING - 1; t++) ring_issue(t);
 #pragma unroll 2
     for (int t = 0; t < nt; t++) {
-      const u64 *c = s_ct[t];
-      const u64 x0 = __ldg(c + idx), x1 = __ldg(c + LN + idx);
+      ring_issue(t + MAC_RING - 1);  // overwrites the slot of term t - 1, already consumed by this thread
+      asm volatile("cp.async.wait_group %0;" ::"n"(MAC_RING - 1) : "memory");
+      const u64 x0 = s_ring[t % MAC_RING][0][threadIdx.x], x1 = s_ring[t % MAC_RING][1][threadIdx.x];
       u64 w[G];
 #pragma unroll
-      for (int i = 0; i < G; i++) w[i] = __ldg(s_pt[i][t] + idx);
+      for (int i = 0; i < G; i++) w[i] = s_ring[t % MAC_RING][2 + i][threadIdx.x];
       st.mac(x0, x1, w, mc);
     }
   }
