@@ -93,11 +93,12 @@ class Layout:
 
 
 class ConvDesc:
-    def __init__(self, BS, C_in, H, W, C_out, K, stride=1, pad=0, depthwise=False, S=0, M=0, seg_v=0, B_cap=0):
+    def __init__(self, BS, C_in, H, W, C_out, K, stride=1, pad=0, depthwise=False, S=0, M=0, seg_v=0, B_cap=0, bsgs=1):
         self.BS, self.C_in, self.H, self.W, self.C_out, self.K = BS, C_in, H, W, C_out, K
         self.stride, self.pad, self.depthwise, self.S, self.M = stride, pad, depthwise, S, M
         self.seg_v = seg_v  # > 0: input and output ciphertexts in the segmented layout with v = seg_v (R2.11b)
         self.B_cap = B_cap    # > 0: at most B_cap samples per ciphertext (Layout)
+        self.bsgs = bsgs      # baby steps over the channel diagonals (R2.9d): 1 = none, g > 1 explicit, 0 = fewest rotations
         self.H_out = (H + 2 * pad - K) // stride + 1
         self.W_out = (W + 2 * pad - K) // stride + 1
 
@@ -129,7 +130,15 @@ class ConvGraph:
     channel diagonal d must wrap inside each v-position segment, not around the whole ciphertext, so it splits in two
     partial sums: part 0 holds the input positions pl >= d of every segment and is rotated by d*cs, part 1 the positions
     pl < d and is rotated by (d - v)*cs (both masks folded into the weight plaintexts); the diagonal key is
-    dkey = d + part*chp (chp = physical channel positions), and diag_rot(dkey) is its outer rotation amount."""
+    dkey = d + part*chp (chp = physical channel positions), and diag_rot(dkey) is its outer rotation amount.
+
+    Baby-step giant-step over the channel diagonals (desc.bsgs = g > 1; R2.9d; PAPER.md:82 names the outer rotations as
+    the cost to cut, PAPER.md:284 uses BSGS for the diagonals of the FC layers): with d = i g + j, 0 <= j < g,
+        Y = sum_i Rot( sum_j sum_t Rot(in_t, amt_t + j cs) (*) W'(t, d), i g cs ),   W'(t, d) = Rot(W(t, d), j cs),
+    because Rot(x (*) w, r) = Rot(x, r) (*) Rot(w, r) and Rot(Rot(in, amt), j cs) = Rot(in, amt + j cs): the baby step is
+    folded into the INNER rotation (still one rotation of the original input, shared by every output and hoistable), the
+    giant steps are the outer rotations -- ch/g - 1 per output instead of ch - 1.  After the regrouping the keys of
+    terms[okey] are the giant steps i, the term amounts are the composite ones, and weight_slots shifts by j cs."""
 
     def __init__(self, desc: ConvDesc, n: int):
         d = desc
@@ -169,6 +178,34 @@ class ConvGraph:
                             diags[dd] = lst
                     self.terms[(uo, vo, go)] = diags
         self.inner = sorted(inner)
+        self.g = 1
+        if d.bsgs != 1 and L.seg == 1 and L.ch > 1:
+            cands = [d.bsgs] if d.bsgs > 1 else [1 << k for k in range(0, L.ch.bit_length()) if L.ch % (1 << k) == 0]
+            best = None
+            for g in cands:
+                assert L.ch % g == 0 and g & (g - 1) == 0, "bsgs must be a power of two dividing the channel positions"
+                terms, inner_g = self._regroup(g)
+                n_rot = len(inner_g) + sum(len([i for i in giants if i]) for giants in terms.values())
+                if best is None or n_rot < best[0]:  # fewest rotations, ties to the smaller g
+                    best = (n_rot, g, terms, inner_g)
+            _, self.g, self.terms, inner_g = best
+            self.inner = sorted(inner_g)
+
+    def _regroup(self, g):
+        """the plain graph's diagonals d = i g + j regrouped by giant step i (R2.9d); g = 1 returns the plain graph"""
+        L, n = self.lin, self.n
+        terms, inner = {}, set()
+        for okey, diags in self.terms.items():
+            giants = {}
+            for dd in sorted(diags):
+                i, j = divmod(dd, g)
+                for src, amt, wkey in diags[dd]:
+                    a = (amt + j * L.cs) % n
+                    giants.setdefault(i, []).append((src, a, wkey))
+                    if a:
+                        inner.add((src, a))
+            terms[okey] = giants
+        return terms, inner
 
     # Which entries of weight plaintext wkey can be non-zero (independent of the values).  The validity
     # conditions of R2.9 step 2 factorise: channel positions (c < C_in, o < C_out, depthwise o == c),
@@ -193,6 +230,8 @@ class ConvGraph:
     def diag_rot(self, dd):
         """outer rotation amount of diagonal key dd: d*cs, or (d - v)*cs for the wrapping part of a segmented layout"""
         L = self.lin
+        if self.g > 1:
+            return (dd * self.g * L.cs) % self.n  # dd is a giant step i (R2.9d)
         part, dl = divmod(dd, L.chp) if L.seg > 1 else (0, dd)
         return ((dl - L.ch) * L.cs) % self.n if part else (dl * L.cs) % self.n
 
@@ -231,6 +270,8 @@ class ConvGraph:
                 for bj in cols:
                     base = L.slot(cpos, bi * L.m + bj, 0)
                     vec[base:base + L.B] = val
+        if self.g > 1:  # W' = Rot(W, j cs) with j the baby step of this plaintext's diagonal (R2.9d)
+            vec = np.roll(vec, -((wkey[4] % self.g) * L.cs))
         return vec
 
     # ---- factored weights (R2.9c; the large-batch case of PAPER.md:218-222, where one ciphertext holds one channel)
@@ -408,7 +449,7 @@ def candidates(desc: ConvDesc, n):
 
 
 def with_S(desc: ConvDesc, S):
-    return ConvDesc(desc.BS, desc.C_in, desc.H, desc.W, desc.C_out, desc.K, desc.stride, desc.pad, desc.depthwise, S, desc.M, desc.seg_v, desc.B_cap)
+    return ConvDesc(desc.BS, desc.C_in, desc.H, desc.W, desc.C_out, desc.K, desc.stride, desc.pad, desc.depthwise, S, desc.M, desc.seg_v, desc.B_cap, desc.bsgs)
 
 
 def select_S(desc: ConvDesc, n):

@@ -406,3 +406,73 @@ def test_repack_encrypted_changes_block_size():
         assert y.L == P.nq - 1 and y.scale == P.scale
         dst.scatter(Y, ck.decrypt_decode(P, keys, y).real, *k)
     assert np.abs(Y - x).max() < 1e-4
+
+
+# --------------------------------------------------------------------------- BSGS over the channel diagonals (R2.9d)
+BSGS_SHAPES = [
+    (128, dict(BS=1, C_in=8, H=4, W=4, C_out=8, K=3, stride=1, pad=1), 1),       # ch = 8, dense channels
+    (128, dict(BS=1, C_in=5, H=4, W=4, C_out=7, K=3, stride=1, pad=1), 1),       # ragged channels
+    (128, dict(BS=2, C_in=4, H=8, W=8, C_out=8, K=3, stride=2, pad=1), 2),       # S = 2, stride 2, two output groups
+    (512, dict(BS=1, C_in=16, H=4, W=4, C_out=16, K=3, stride=1, pad=1), 1),     # ch = 32: the auto rule picks g > 1
+    (512, dict(BS=3, C_in=6, H=4, W=4, C_out=9, K=1, stride=1, pad=0, B_cap=2), 1),  # 1x1, two batch groups, ch = 16
+]
+
+
+@pytest.mark.parametrize("n,kw,S", BSGS_SHAPES)
+@pytest.mark.parametrize("g", [2, 4, 0])
+def test_conv_bsgs_on_plain_slots_and_counts(n, kw, S, g):
+    """R2.9d: the regrouped graph on plain slot vectors (rotation = cyclic shift) equals direct convolution; its rotation
+    counts follow the closed form (every (input, amount) of the plain graph, the unrotated input included, appears with
+    each of the g baby steps; one outer rotation per non-zero giant step that has a term); PMult count and weight keys are
+    those of the plain graph; auto (0) never needs more rotations than plain or any explicit g."""
+    shape = {k: v for k, v in kw.items() if k != "B_cap"}
+    x, w = wl.conv_inputs(21, shape)
+    plain = fr.ConvGraph(fr.ConvDesc(S=S, **kw), n)
+    d = fr.ConvDesc(S=S, bsgs=g, **kw)
+    G = fr.ConvGraph(d, n)
+    assert np.abs(fr.hconv_slots(d, n, x, w) - fr.direct_conv(d, x, w)).max() < 1e-12
+    cp, cg = plain.counts(), G.counts()
+    assert cg["n_pmult"] == cp["n_pmult"] and cg["n_out_ct"] == cp["n_out_ct"]
+    keys = lambda gr: sorted(wk for diags in gr.terms.values() for lst in diags.values() for _, _, wk in lst)
+    assert keys(G) == keys(plain)
+    gg = G.g
+    assert gg == g or g == 0
+    # closed form from the plain graph
+    pairs = {(src, amt, dd % gg) for diags in plain.terms.values() for dd, lst in diags.items() for src, amt, _ in lst}
+    inner = {(src, (amt + j * plain.lin.cs) % n) for src, amt, j in pairs} - {(src, 0) for src, _, _ in pairs}
+    outer = sum(len({dd // gg for dd in diags} - {0}) for diags in plain.terms.values())
+    assert cg["n_inner_rot"] == len(inner) * plain.lin.BG and cg["n_outer_rot"] == outer * plain.lin.BG
+    if g == 0:
+        tot = lambda c: c["n_inner_rot"] + c["n_outer_rot"]
+        for other in (1, 2, 4):
+            if plain.lin.ch % other == 0:
+                assert tot(cg) <= tot(fr.ConvGraph(fr.ConvDesc(S=S, bsgs=other, **kw), n).counts())
+    if n == 512 and kw["C_in"] == 16:
+        assert (cp["n_inner_rot"], cp["n_outer_rot"]) == (8, 30)       # BASELINE config 3's 16 -> 16 layer has this profile
+        if g == 0:
+            assert G.g == 2 and (cg["n_inner_rot"], cg["n_outer_rot"]) == (17, 15)
+
+
+def test_conv_bsgs_encrypted_decodes_and_differs_from_plain():
+    """R2.9d on ciphertexts (hoisted inner rotations): decrypt = direct convolution within 1e-3, same level and scale as the
+    plain graph; the limbs differ (other rotations, other key-switch noise) while the decoded values agree to 1e-4."""
+    P = ck.Params(8, 4, 40, 2, 60, 2, 40)
+    kw = dict(BS=1, C_in=8, H=4, W=4, C_out=8, K=3, stride=1, pad=1)
+    x, w = wl.conv_inputs(22, kw)
+    L = P.nq
+    res = {}
+    for g in (1, 2):
+        d = fr.ConvDesc(S=1, bsgs=g, **kw)
+        G = fr.ConvGraph(d, P.n)
+        keys = ck.keygen(P, 5, G.counts()["rot_steps"])
+        W = fr.encode_weights(ck, P, G, w, L)
+        ins = {(0, 0, gi): ck.encrypt(P, keys, ck.encode(P, G.lin.gather(x, 0, 0, gi, 0), L), 70 + gi) for gi in range(G.lin.G)}
+        out = fr.hconv(ck, P, keys, G, ins, W, hoist=True)
+        Y = np.zeros((1, 8, 4, 4))
+        for k, y in out.items():
+            assert y.L == L - 1 and y.scale == P.scale
+            G.lout.scatter(Y, ck.decrypt_decode(P, keys, y).real, *k, 0)
+        res[g] = (Y, out)
+    want = fr.direct_conv(fr.ConvDesc(**kw), x, w)
+    assert np.abs(res[2][0] - want).max() < 1e-3 and np.abs(res[2][0] - res[1][0]).max() < 1e-4
+    assert any(not np.array_equal(res[1][1][k].c, res[2][1][k].c) for k in res[1][1])
