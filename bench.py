@@ -116,6 +116,7 @@ def timed_clocks(sampler, fn):
 
 # ------------------------------------------------------------------------------------------------ workloads
 FC_BSGS = 0  # baby-step count of the fully connected layers: 0 = library's choice (R2.12b), 1 = plain diagonals (--plain-fc)
+CONV_BSGS = 0  # baby steps over the conv layers' channel diagonals: 0 = fewest rotations (R2.9d), 1 = plain (--plain-conv)
 
 
 def lenet_layers(BS, seed, upto="fc"):
@@ -170,7 +171,7 @@ def conv_layers(name, seed, kaiming=False):
     """one encrypted conv layer of a BASELINE config at the top level (reading A20), planner-selected S."""
     kw = wl.CONVS[name]
     x, w = wl.conv_inputs(seed, kw, kaiming=kaiming)
-    return [{"op": "conv", "conv": dict(kw), "S": 0, "w": w}], x
+    return [{"op": "conv", "conv": dict(kw, bsgs=CONV_BSGS), "S": 0, "w": w}], x
 
 
 def resnet_chain_layers(seed):
@@ -181,7 +182,7 @@ def resnet_chain_layers(seed):
     layers = []
     for i, (kw, S) in enumerate(shapes):
         std = np.sqrt(2.0 / (kw["C_in"] * kw["K"] ** 2))
-        layers.append({"op": "conv", "conv": dict(kw), "S": S, "w": rng.normal(0.0, std, (kw["C_out"], kw["C_in"], kw["K"], kw["K"]))})
+        layers.append({"op": "conv", "conv": dict(kw, bsgs=CONV_BSGS), "S": S, "w": rng.normal(0.0, std, (kw["C_out"], kw["C_in"], kw["K"], kw["K"]))})
         if i < 2:
             layers.append({"op": "poly3"})
     return layers, rng.uniform(-1, 1, (1, 16, 32, 32))
@@ -197,11 +198,11 @@ def bottleneck_layers(seed, aac):
     exp = dict(BS=4, C_in=8, H=32, W=32, C_out=128, K=3, stride=1, pad=1, B_cap=1)
     w1 = rng.normal(0.0, np.sqrt(2.0 / 64), (8, 64, 1, 1))
     w2 = rng.normal(0.0, np.sqrt(2.0 / 72), (128, 8, 3, 3))
-    layers = [{"op": "conv", "conv": red, "S": 1, "w": w1}]
+    layers = [{"op": "conv", "conv": dict(red, bsgs=CONV_BSGS), "S": 1, "w": w1}]
     if aac:
-        layers += [{"op": "compress", "v": 8}, {"op": "conv", "conv": dict(exp, seg_v=8), "S": 1, "w": w2}]
+        layers += [{"op": "compress", "v": 8}, {"op": "conv", "conv": dict(exp, seg_v=8, bsgs=CONV_BSGS), "S": 1, "w": w2}]
     else:
-        layers += [{"op": "conv", "conv": exp, "S": 1, "w": w2}]
+        layers += [{"op": "conv", "conv": dict(exp, bsgs=CONV_BSGS), "S": 1, "w": w2}]
     return layers, rng.uniform(-1, 1, (4, 64, 32, 32))
 
 
@@ -941,6 +942,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3, help="steps of each end-to-end leg (at most --steps)")
     ap.add_argument("--profile-range", action="store_true", help="cudaProfilerStart/Stop around the timed steps (for ncu)")
     ap.add_argument("--plain-fc", action="store_true", help="fully connected layers by plain diagonals (no baby-step giant-step)")
+    ap.add_argument("--plain-conv", action="store_true", help="conv layers' channel diagonals without baby-step giant-step (config 3 workloads)")
     ap.add_argument("--eager-relin", action="store_true", help="x^2 and the pool after it as two steps (four relinearisations per pooled output)")
     ap.add_argument("--no-hoist", action="store_true", help="inner rotations as plain rotations (one decomposition each)")
     ap.add_argument("--sweep-L", type=int, nargs="*", help="config 5: only these limb counts")
@@ -952,9 +954,11 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-companions", action="store_true", help="default workload only: skip the config 5 / 2 / 3 companions")
     args = ap.parse_args()
+    global FC_BSGS, CONV_BSGS
     if args.plain_fc:
-        global FC_BSGS
         FC_BSGS = 1
+    if args.plain_conv:
+        CONV_BSGS = 1
     rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
     if args.impl == "reference":
         if rank == 0:

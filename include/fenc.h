@@ -85,7 +85,16 @@ typedef struct {
   /* cap on the samples per ciphertext, B = min(next_pow2(BS), (N/2)/m^2, B_cap); 0 = none ("batch first").
    * With a cap a large batch has several batch groups and several channel positions per ciphertext. */
   uint32_t B_cap;
+  /* Baby-step giant-step over the channel diagonals (R2.9d): with bsgs = g > 1 (a power of two
+   * dividing ch) a diagonal is d = i g + j and
+   *   Y = sum_i Rot( sum_j sum_t Rot(in_t, amt_t + j cs) (*) W'(t, d), i g cs ),  W'(t, d) = Rot(W(t, d), j cs):
+   * the baby step is folded into the inner rotation (one rotation of the original input, hoistable), ch/g - 1 outer
+   * rotations per output instead of ch - 1.  0 or 1: plain diagonals; FENC_CONV_BSGS_AUTO: the g with the fewest rotations
+   * (inner + outer), ties to the smaller g.  On a segmented layout (seg_v = v, g | v) the two parts of diagonal d keep
+   * its baby step and rotate by i g cs and (i g - v) cs.  The weight keys stay (.., d, ..); the plaintext of a key is W'. */
+  uint32_t bsgs;
 } fenc_conv_desc;
+#define FENC_CONV_BSGS_AUTO 0xFFFFFFFFu
 
 /* Filled by fenc_layout_plan.  All counts are exact for the operation graph of DESIGN.md R2.9. */
 typedef struct {

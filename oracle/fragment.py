@@ -138,7 +138,9 @@ class ConvGraph:
     because Rot(x (*) w, r) = Rot(x, r) (*) Rot(w, r) and Rot(Rot(in, amt), j cs) = Rot(in, amt + j cs): the baby step is
     folded into the INNER rotation (still one rotation of the original input, shared by every output and hoistable), the
     giant steps are the outer rotations -- ch/g - 1 per output instead of ch - 1.  After the regrouping the keys of
-    terms[okey] are the giant steps i, the term amounts are the composite ones, and weight_slots shifts by j cs."""
+    terms[okey] are the giant steps i, the term amounts are the composite ones, and weight_slots shifts by j cs.
+    On a segmented layout the two parts of diagonal d = i g + j keep their baby step j and become giant keys i and
+    i + chp with outer rotations i g cs and (i g - v) cs."""
 
     def __init__(self, desc: ConvDesc, n: int):
         d = desc
@@ -179,7 +181,7 @@ class ConvGraph:
                     self.terms[(uo, vo, go)] = diags
         self.inner = sorted(inner)
         self.g = 1
-        if d.bsgs != 1 and L.seg == 1 and L.ch > 1:
+        if d.bsgs != 1 and L.ch > 1:
             cands = [d.bsgs] if d.bsgs > 1 else [1 << k for k in range(0, L.ch.bit_length()) if L.ch % (1 << k) == 0]
             best = None
             for g in cands:
@@ -198,7 +200,11 @@ class ConvGraph:
         for okey, diags in self.terms.items():
             giants = {}
             for dd in sorted(diags):
-                i, j = divmod(dd, g)
+                # segmented layouts (R2.11b): dd = d + part*chp; both parts of diagonal d share its baby step, the giant
+                # key keeps the part (its outer rotation is (i g - part v) cs, see diag_rot)
+                part, dl = divmod(dd, L.chp) if L.seg > 1 else (0, dd)
+                i, j = divmod(dl, g)
+                i += part * L.chp
                 for src, amt, wkey in diags[dd]:
                     a = (amt + j * L.cs) % n
                     giants.setdefault(i, []).append((src, a, wkey))
@@ -230,8 +236,9 @@ class ConvGraph:
     def diag_rot(self, dd):
         """outer rotation amount of diagonal key dd: d*cs, or (d - v)*cs for the wrapping part of a segmented layout"""
         L = self.lin
-        if self.g > 1:
-            return (dd * self.g * L.cs) % self.n  # dd is a giant step i (R2.9d)
+        if self.g > 1:  # dd is a giant step i (R2.9d), + chp for the wrapping part of a segmented layout
+            part, i = divmod(dd, L.chp) if L.seg > 1 else (0, dd)
+            return ((i * self.g - part * L.ch) * L.cs) % self.n
         part, dl = divmod(dd, L.chp) if L.seg > 1 else (0, dd)
         return ((dl - L.ch) * L.cs) % self.n if part else (dl * L.cs) % self.n
 

@@ -32,7 +32,7 @@ class ParamsDesc(C.Structure):
 class ConvDesc(C.Structure):
     _fields_ = [("BS", C.c_uint32), ("C_in", C.c_uint32), ("H", C.c_uint32), ("W", C.c_uint32), ("C_out", C.c_uint32),
                 ("K", C.c_uint32), ("stride", C.c_uint32), ("pad", C.c_uint32), ("depthwise", C.c_int32),
-                ("S", C.c_uint32), ("M", C.c_uint32), ("seg_v", C.c_uint32), ("B_cap", C.c_uint32)]
+                ("S", C.c_uint32), ("M", C.c_uint32), ("seg_v", C.c_uint32), ("B_cap", C.c_uint32), ("bsgs", C.c_uint32)]
 
 
 class KeyMaterial(C.Structure):
@@ -301,8 +301,9 @@ class Context:
         return int(self.lib.fenc_device_bytes(self.h))
 
     # ---- planner
-    def conv_desc(self, BS, C_in, H, W, C_out, K, stride=1, pad=0, depthwise=False, S=0, M=0, seg_v=0, B_cap=0):
-        return ConvDesc(BS, C_in, H, W, C_out, K, stride, pad, int(depthwise), S, M, seg_v, B_cap)
+    def conv_desc(self, BS, C_in, H, W, C_out, K, stride=1, pad=0, depthwise=False, S=0, M=0, seg_v=0, B_cap=0, bsgs=1):
+        """bsgs: baby steps over the channel diagonals (1 = plain, 0 = the library's choice, FENC_CONV_BSGS_AUTO)"""
+        return ConvDesc(BS, C_in, H, W, C_out, K, stride, pad, int(depthwise), S, M, seg_v, B_cap, 0xFFFFFFFF if bsgs == 0 else bsgs)
 
     def layout_plan(self, conv):
         lay = Layout()

@@ -39,6 +39,7 @@ struct ConvGraph : LinGraph {              // outs index: (g_out * S_out + u_o) 
   fenc_conv_desc d;
   int n, M, S, S_out, m, B, ch, cs, G_in, G_out, H_out, W_out;
   int chp = 0, seg = 1;  // physical channel positions of a ciphertext = seg segments of ch positions (R2.11b; seg = 1: plain)
+  int g = 1;             // baby steps over the channel diagonals (R2.9d); OutCt.diags then hold the giant steps
   std::vector<std::array<u32, 7>> wkeys;      // (u_o, v_o, g_out, g_in, dkey, i, j) per weight plaintext
   // diagonal keys: d in [0, ch); in a segmented layout also chp + d (d >= 1), the part of diagonal d that wraps inside
   // its segment (input positions pl < d, outer rotation (d - ch) cs instead of d cs)
@@ -125,13 +126,17 @@ struct ConvGraph : LinGraph {              // outs index: (g_out * S_out + u_o) 
           for (int b = 0; b < B; b++) vec[base + b] = val;
         }
     }
+    if (g > 1) {  // W' = Rot(W, j cs), j = d mod g: the baby step of this plaintext's diagonal (R2.9d)
+      const size_t sh = (size_t)(dd % g) * cs % n;
+      if (sh) std::rotate(vec.begin(), vec.begin() + sh, vec.end());
+    }
   }
 };
 
 static fenc_status build_graph(fenc_ctx *ctx, const fenc_conv_desc *cd, int S, std::shared_ptr<ConvGraph> &out) {
   char keybuf[256];
-  snprintf(keybuf, sizeof keybuf, "%u,%u,%u,%u,%u,%u,%u,%u,%d,%d,%u,%u,%u", cd->BS, cd->C_in, cd->H, cd->W, cd->C_out, cd->K,
-           cd->stride, cd->pad, cd->depthwise, S, cd->M, cd->seg_v, cd->B_cap);
+  snprintf(keybuf, sizeof keybuf, "%u,%u,%u,%u,%u,%u,%u,%u,%d,%d,%u,%u,%u,%u", cd->BS, cd->C_in, cd->H, cd->W, cd->C_out, cd->K,
+           cd->stride, cd->pad, cd->depthwise, S, cd->M, cd->seg_v, cd->B_cap, cd->bsgs);
   auto it = ctx->graphs.find(keybuf);
   if (it != ctx->graphs.end()) {
     out = std::static_pointer_cast<ConvGraph>(it->second);
@@ -202,6 +207,62 @@ static fenc_status build_graph(fenc_ctx *ctx, const fenc_conv_desc *cd, int S, s
           }
         }
       }
+  // ---- baby-step giant-step over the channel diagonals (R2.9d): regroup the plain graph's diagonals d = i gs + j by giant
+  // step i; the baby step joins the inner amount, the outer rotation becomes i gs cs
+  if (cd->bsgs > 1 && g->ch > 1) {
+    auto regroup = [&](int gs, std::vector<OutCt> &outs, std::set<std::pair<int, int>> &inn, std::set<int> &stp, size_t &n_outer) {
+      outs.assign(g->outs.size(), OutCt{});
+      n_outer = 0;
+      for (size_t o = 0; o < g->outs.size(); o++) {
+        const OutCt &src = g->outs[o];
+        std::map<int, std::vector<Term>> giants;
+        for (size_t k = 0; k < src.diags.size(); k++) {
+          // segmented layouts (R2.11b): dd = d + part*chp; both parts of diagonal d share its baby step, the giant key
+          // keeps the part and its outer rotation is (i gs - part ch) cs
+          const int dd = src.diags[k], part = g->seg > 1 ? dd / g->chp : 0, dl = g->seg > 1 ? dd % g->chp : dd;
+          const int gi = dl / gs + part * g->chp, j = dl % gs;
+          for (Term t : src.terms[k]) {
+            t.amt = (int)(((long)t.amt + (long)j * g->cs) % g->n);
+            giants[gi].push_back(t);
+            if (t.amt) inn.insert({t.src, t.amt}), stp.insert(t.amt);
+          }
+        }
+        for (auto &kv : giants) {
+          const int kpart = g->seg > 1 ? kv.first / g->chp : 0, ki = g->seg > 1 ? kv.first % g->chp : kv.first;
+          const long r0 = ((long)ki * gs - (long)kpart * g->ch) * g->cs;
+          const int rot = (int)(((r0 % g->n) + g->n) % g->n);
+          outs[o].diags.push_back(kv.first), outs[o].rots.push_back(rot), outs[o].terms.push_back(std::move(kv.second));
+          if (rot) n_outer++, stp.insert(rot);
+        }
+      }
+    };
+    std::vector<int> cands;
+    if (cd->bsgs == FENC_CONV_BSGS_AUTO) {
+      for (int c = 1; c <= g->ch; c *= 2)
+        if (g->ch % c == 0) cands.push_back(c);
+    } else {
+      const int c = (int)cd->bsgs;
+      if (c > g->ch || g->ch % c || (c & (c - 1))) return fail(ctx, FENC_ERR_LAYOUT, "bsgs=%d must be a power of two dividing ch=%d", c, g->ch);
+      cands.push_back(c);
+    }
+    size_t best = ~(size_t)0;
+    int best_g = 1;
+    for (int c : cands) {  // fewest rotations (inner + outer), ties to the smaller g
+      std::vector<OutCt> o2;
+      std::set<std::pair<int, int>> i2;
+      std::set<int> s2;
+      size_t no = 0;
+      regroup(c, o2, i2, s2, no);
+      if (i2.size() + no < best) best = i2.size() + no, best_g = c;
+    }
+    if (best_g > 1) {
+      std::vector<OutCt> o2;
+      size_t no = 0;
+      inner.clear(), steps.clear();
+      regroup(best_g, o2, inner, steps, no);
+      g->outs = std::move(o2), g->n_outer = no, g->g = best_g;
+    }
+  }
   g->inner.assign(inner.begin(), inner.end());
   for (size_t i = 0; i < g->inner.size(); i++) g->inner_index[g->inner[i]] = (int)i;
   g->rot_steps.assign(steps.begin(), steps.end());

@@ -162,7 +162,7 @@ def run_hconv(mods, P, ctx, conv_kw, S, seed, do_rescale=True, kaiming=False, ho
     """GPU fenc_hconv vs oracle hconv for every batch group; returns (max decoded error, layout)."""
     ck, fr, fenc = mods
     x, w = wl.conv_inputs(seed, conv_kw, kaiming=kaiming)
-    od = fr.ConvDesc(S=S, **conv_kw)
+    od = fr.ConvDesc(S=S, **conv_kw)  # (seg_v / B_cap / bsgs ride along in conv_kw: both descriptors take them)
     graph = fr.ConvGraph(od, P.n)
     conv = ctx.conv_desc(S=S, **conv_kw)
     lay = ctx.layout_plan(conv)
@@ -448,6 +448,27 @@ def test_repack_block_size_bit_exact(mods, S_src, S_dst, shape):
         assert got[t].L == L - 1 and np.array_equal(ctx.ct_export(got[t]), ref[dk].c), dk
         dst.scatter(Y, ctx.decrypt_slots(gk, got[t]).real, *dk)
     assert np.abs(Y - x).max() < 1e-4
+    ctx.close()
+
+
+@pytest.mark.parametrize("conv_kw,S,hoist", [
+    (dict(BS=1, C_in=8, H=8, W=8, C_out=8, K=3, stride=1, pad=1, bsgs=2), 1, False),    # n=512: ch=8, 17 inner + 3 outer
+    (dict(BS=1, C_in=5, H=8, W=8, C_out=7, K=3, stride=1, pad=1, bsgs=4), 1, True),     # ragged channels, hoisted composite amounts
+    (dict(BS=2, C_in=4, H=8, W=8, C_out=8, K=3, stride=2, pad=1, bsgs=2), 2, True),     # S=2, stride 2, two output groups
+    (dict(BS=1, C_in=16, H=4, W=4, C_out=16, K=3, stride=1, pad=1, bsgs=0), 1, True),   # ch=32: the auto rule picks g=2
+    (dict(BS=4, C_in=8, H=4, W=4, C_out=16, K=3, stride=1, pad=1, B_cap=1, seg_v=8, bsgs=2), 1, True),  # segmented layout (R2.11b) + BSGS
+])
+def test_hconv_bsgs_channel_diagonals_bit_exact(mods, conv_kw, S, hoist):
+    """R2.9d: baby-step giant-step over the convolution's channel diagonals (baby step folded into the inner rotation,
+    weight plaintexts shifted, giant steps as outer rotations): every limb against the oracle's variant, same counts and
+    rotation amounts on both sides (asserted in run_hconv), decoded against direct convolution."""
+    P, ctx = make(mods, "mid10")
+    plain = ctx.layout_plan(ctx.conv_desc(S=S, **dict(conv_kw, bsgs=1)))
+    err, lay = run_hconv(mods, P, ctx, conv_kw, S, seed=10, hoist=hoist)
+    assert err < 1e-3
+    assert lay.n_outer_rot < plain.n_outer_rot and lay.n_pmult == plain.n_pmult and lay.n_distinct_pt == plain.n_distinct_pt
+    if conv_kw["bsgs"] == 0:
+        assert lay.n_inner_rot + lay.n_outer_rot < plain.n_inner_rot + plain.n_outer_rot
     ctx.close()
 
 

@@ -476,3 +476,27 @@ def test_conv_bsgs_encrypted_decodes_and_differs_from_plain():
     want = fr.direct_conv(fr.ConvDesc(**kw), x, w)
     assert np.abs(res[2][0] - want).max() < 1e-3 and np.abs(res[2][0] - res[1][0]).max() < 1e-4
     assert any(not np.array_equal(res[1][1][k].c, res[2][1][k].c) for k in res[1][1])
+
+
+@pytest.mark.parametrize("n,v,kw", [(128, 2, dict(BS=4, C_in=2, H=4, W=4, C_out=8, K=3, stride=1, pad=1, B_cap=1)),
+                                    (256, 4, dict(BS=16, C_in=3, H=4, W=4, C_out=8, K=3, stride=1, pad=1, B_cap=2)),
+                                    (1024, 8, dict(BS=4, C_in=8, H=4, W=4, C_out=16, K=3, stride=1, pad=1, B_cap=1))])
+@pytest.mark.parametrize("g", [2, 4, 0])
+def test_conv_bsgs_on_segmented_layouts(n, v, kw, g):
+    """R2.9d on the segmented layout of R2.11b: both parts of diagonal d = i g + j keep the baby step j; their giant
+    rotations are i g cs and (i g - v) cs.  The graph on plain slot vectors equals direct convolution; explicit g halves
+    (quarters) the outer rotations; auto never needs more rotations than plain."""
+    if g > 1 and v % g:
+        pytest.skip("g must divide the segment size")
+    shape = {k: x for k, x in kw.items() if k != "B_cap"}
+    x, w = wl.conv_inputs(23, shape)
+    d = fr.ConvDesc(S=1, seg_v=v, bsgs=g, **kw)
+    G = fr.ConvGraph(d, n)
+    assert np.abs(fr.hconv_slots(d, n, x, w) - fr.direct_conv(d, x, w)).max() < 1e-12
+    cp, cg = fr.ConvGraph(fr.ConvDesc(S=1, seg_v=v, **kw), n).counts(), G.counts()
+    if g > 1:
+        assert G.g == g and cg["n_outer_rot"] * g <= cp["n_outer_rot"] + cg["n_out_ct"] * g
+    else:
+        assert cg["n_inner_rot"] + cg["n_outer_rot"] <= cp["n_inner_rot"] + cp["n_outer_rot"]
+    if n == 1024 and g == 0:
+        assert G.g == 2 and (cp["n_outer_rot"], cg["n_outer_rot"]) == (28, 14)
