@@ -36,9 +36,17 @@ class FcGraph:
         out_{c'} = sum_i Rot( sum_j sum_c Rot(x_c, j B) (*) W'(c', c, d), i g B ),   W'(c', c, d) = Rot(Wd(c', c, d), j B),
     i.e. W'(c', c, d)[p] = W[nu(c', (p - i g) mod P), feat(c, (p + j) mod P)].  The baby rotations Rot(x_c, j B) are
     computed once per input ciphertext and shared by every output and giant step.  bsgs = 1: plain diagonals (no baby
-    rotation, W' = Wd); bsgs = 0: g = bsgs_auto(P, n_in_ct, n_out_ct)."""
+    rotation, W' = Wd); bsgs = 0: g = bsgs_auto(P, n_in_ct, n_out_ct).
 
-    def __init__(self, n, BS, n_in, n_out, in_C=0, in_H=0, in_W=0, in_M=1, bsgs=1):
+    Fragment-encoded embeddings (R2.13, the Transformer extension): BS is the number of tokens, a token's
+    embedding of dimension E is split in E/S sub-blocks of S coordinates, and coordinate e = p S + u of every token lives
+    in ciphertext u (the fragment, 0 <= u < S) at position p -- "fragments from different tokens are interleaved across
+    ciphertexts".  frag_in = S: feat(c, p) = p S + c with S input ciphertexts; frag_out = S': neuron(c', p) = p S' + c'
+    with S' output ciphertexts.  X W^T is then this same graph; with E = S P its embedding aggregation costs P - 1 = E/S - 1
+    rotations per output ciphertext instead of the E - 1 of full-embedding packing."""
+
+    def __init__(self, n, BS, n_in, n_out, in_C=0, in_H=0, in_W=0, in_M=1, bsgs=1, frag_in=0, frag_out=0):
+        self.frag_in, self.frag_out = frag_in, frag_out
         self.n, self.BS, self.n_in, self.n_out = n, BS, n_in, n_out
         self.in_C, self.in_H, self.in_W, self.m = in_C, in_H, in_W, in_M
         m2 = in_M * in_M
@@ -47,12 +55,19 @@ class FcGraph:
         self.P = n // self.B
         self.ch = n // (self.B * m2)
         self.BG = -(-BS // self.B)
-        if in_C:
+        if frag_in:
+            assert not in_C and -(-n_in // frag_in) <= self.P, "E/S sub-blocks must fit the positions of a ciphertext"
+            self.n_in_ct = frag_in
+        elif in_C:
             assert in_C * in_H * in_W == n_in
             self.n_in_ct = -(-in_C // self.ch)
         else:
             self.n_in_ct = -(-n_in // self.P)
-        self.n_out_ct = -(-n_out // self.P)
+        if frag_out:
+            assert -(-n_out // frag_out) <= self.P
+            self.n_out_ct = frag_out
+        else:
+            self.n_out_ct = -(-n_out // self.P)
         self.g = bsgs if bsgs >= 1 else bsgs_auto(self.P, self.n_in_ct, self.n_out_ct)
         assert self.P % self.g == 0
         self.terms = {}  # c' -> {giant step i: [(c, baby step j, wkey (c', c, d = i g + j))]}
@@ -67,6 +82,9 @@ class FcGraph:
 
     def feat(self, c, p):
         """PyTorch flatten order channel*H*W + h*W + w through the S=1 layout, or c*P + p after a previous fc."""
+        if self.frag_in:
+            f = p * self.frag_in + c
+            return f if f < self.n_in else -1
         if self.in_C:
             m2 = self.m * self.m
             cpos, k = divmod(p, m2)
@@ -78,7 +96,7 @@ class FcGraph:
         return f if f < self.n_in else -1
 
     def neuron(self, c, p):
-        v = c * self.P + p
+        v = p * self.frag_out + c if self.frag_out else c * self.P + p
         return v if v < self.n_out else -1
 
     def nonzero(self, co, ci, d):

@@ -157,3 +157,59 @@ def test_cmult_and_poly3_against_fp64():
     assert np.abs(ck.decrypt_decode(P, keys, tri).real - 3 * x).max() < 1e-6
     quarter = ck.add_const(P, cx, ck.round_half_up(cx.scale / 4))
     assert np.abs(ck.decrypt_decode(P, keys, quarter).real - (x + 0.25)).max() < 1e-6
+
+
+# --------------------------------------------------------------------------- fragment-encoded embeddings (R2.13)
+@pytest.mark.parametrize("n,BS,E,Eo,M,S,So,g", [
+    (64, 4, 24, 24, 4, 3, 3, 1),      # E/S = 8 sub-blocks in P = 16 positions (not aligned), plain diagonals
+    (64, 8, 16, 32, 2, 2, 4, 0),      # E = S P exactly; another fragment count on the output side; auto BSGS
+    (128, 16, 20, 12, 2, 4, 2, 2),    # ragged: 20 = 4 * 5 coordinates in P = 8 positions
+    (256, 8, 96, 96, 4, 3, 3, 0),     # a fragment count that is not a power of two (96 = 3 * 32)
+    (256, 20, 64, 64, 4, 4, 4, 4),    # 20 tokens: two batch groups (B = 16), the second ragged
+])
+def test_fragment_encoded_matmul_on_plain_slots(n, BS, E, Eo, M, S, So, g):
+    """R2.13: token embeddings split in E/S sub-blocks across S ciphertexts (coordinate e = p S + u in ciphertext u at
+    position p); X W^T by the diagonal graph on plain slot vectors equals the dense product; gather / scatter are inverse."""
+    rng = np.random.default_rng(31)
+    G = nw.FcGraph(n, BS, E, Eo, in_M=M, bsgs=g, frag_in=S, frag_out=So)
+    assert (G.n_in_ct, G.n_out_ct) == (S, So)
+    X, W = rng.uniform(-1, 1, (BS, E)), rng.normal(0, 0.3, (Eo, E))
+    assert np.abs(nw.fc_slots(G, X, W) - X @ W.T).max() < 1e-12
+    # the layout itself: coordinate e of token b sits in ciphertext e mod S at position e // S
+    v = G.gather_in(X, 1 % S, 0)
+    for b in (0, min(BS, G.B) - 1):
+        for p in range(-(-E // S)):
+            e = p * S + 1 % S
+            assert v[p * G.B + b] == (X[b, e] if e < E else 0.0)
+
+
+def test_fragment_encoding_rotation_count_matches_the_papers_claim():
+    """"the number of rotations required for embedding aggregation is reduced from E-1 in full-embedding
+    packing to E/S - 1 under fragmented encoding".  With E = S P and plain diagonals the graph needs exactly P - 1 = E/S - 1
+    rotations per output ciphertext; full-embedding packing (S = 1, P = E positions) needs E - 1."""
+    n, E = 512, 64
+    for S, M in ((1, 8), (4, 4), (16, 2)):   # P = M^2 = E / S positions, B = n / P tokens per ciphertext
+        P = M * M
+        assert S * P == E
+        G = nw.FcGraph(n, n // P, E, E, in_M=M, frag_in=S, frag_out=S)
+        assert G.P == P and G.counts()["n_rot"] == S * (P - 1) == S * (E // S - 1)
+    # and BSGS on top of the fragments (R2.12b) lowers it further
+    G = nw.FcGraph(n, n // 16, E, E, in_M=4, frag_in=4, frag_out=4, bsgs=0)
+    assert G.counts()["n_rot"] < 4 * 15
+
+
+def test_fragment_encoded_matmul_encrypted():
+    """the same on ciphertexts (hoisted baby steps): decrypt = X W^T within 1e-3, one level"""
+    P = ck.Params(8, 4, 40, 2, 60, 2, 40)
+    rng = np.random.default_rng(32)
+    G = nw.FcGraph(P.n, 8, 48, 48, in_M=4, bsgs=0, frag_in=3, frag_out=3)
+    X, W = rng.uniform(-1, 1, (8, 48)), rng.normal(0, 0.2, (48, 48))
+    keys = ck.keygen(P, 8, G.counts()["rot_steps"])
+    Wp = nw.encode_fc_weights(ck, P, G, W, P.nq)
+    ins = [ck.encrypt(P, keys, ck.encode(P, G.gather_in(X, c, 0), P.nq), 90 + c) for c in range(3)]
+    outs = nw.fc(ck, P, keys, G, ins, Wp, hoist=True)
+    Y = np.zeros((8, 48))
+    for c, y in enumerate(outs):
+        assert y.L == P.nq - 1
+        G.scatter_out(Y, ck.decrypt_decode(P, keys, y).real, c, 0)
+    assert np.abs(Y - X @ W.T).max() < 1e-3
