@@ -206,6 +206,17 @@ def bottleneck_layers(seed, aac):
     return layers, rng.uniform(-1, 1, (4, 64, 32, 32))
 
 
+def transformer_linear_layers(seed):
+    """One linear layer of a BERT-base-shaped encoder block on fragment-encoded token embeddings (the
+    Transformer extension; R2.13): 128 tokens, E = 768 -> 768, sub-blocks of S = 3 coordinates, so B = 128 tokens
+    x P = 256 positions fill the 2^15 slots exactly (E / S = P) and the layer takes 3 input and 3 output ciphertexts.
+    Weights N(0, 1/sqrt(E)), embeddings U[-1, 1]."""
+    rng = np.random.default_rng(seed)
+    w = rng.normal(0.0, 768 ** -0.5, (768, 768))
+    fc = dict(BS=128, n_in=768, n_out=768, in_M=1, frag_in=3, frag_out=3, bsgs=FC_BSGS)
+    return [{"op": "fc", "fc": fc, "w": w}], rng.uniform(-1, 1, (128, 768))
+
+
 WORKLOADS = {
     # name: (PARAMS key, builder(batch, seed) -> (layers, x), description, images per ciphertext batch group or None)
     "cfg4_mobilenet": ("cfg4", lambda bs, seed: mobilenet_layers(32, seed),
@@ -230,6 +241,9 @@ WORKLOADS = {
                               "Table-X-shaped bottleneck 64 -> 8 -> 128 (1x1, 3x3) on 32x32, 4 requests, N=2^16, WITHOUT compression", None),
     "cfg3_bottleneck_aac": ("cfg3", lambda bs, seed: bottleneck_layers(seed, True),
                             "the same bottleneck WITH Arch-aware compression (4 sparse ciphertexts -> 1) and the segmented consumer", None),
+    "ext_transformer_linear": ("cfg3", lambda bs, seed: transformer_linear_layers(seed),
+                               "Transformer extension (PAPER.md:462-464): one 768 -> 768 projection of 128 fragment-encoded token embeddings "
+                               "(S = 3), N=2^16, 24x50b+4x60b, dnum=6", None),
     "cfg5_rotsweep": (None, None, "BASELINE config 5: rotation / key-switch sweep", None),
     "cfg5_rotsweep_hoisted": (None, None, "BASELINE config 5 with hoisted rotations (8 amounts per decomposition)", None),
     "cfg3_compress": (None, None, "AAC compress micro-benchmark at config 3's parameters", None),
@@ -353,6 +367,15 @@ def run_compress(args):
 
 
 # ------------------------------------------------------------------------------------------------ network workloads
+def counted_layers(layers, n_groups):
+    """(layers counted by the line's `value`, its unit): the encrypted conv layers; a network without any (the Transformer
+    extension's linear layer) counts its fully connected layers and says so in the unit"""
+    n = sum(1 for ly in layers if ly["op"] == "conv")
+    if n:
+        return n * n_groups, "encrypted conv layers/s"
+    return sum(1 for ly in layers if ly["op"] == "fc") * n_groups, "encrypted linear layers/s"
+
+
 class NetBench:
     """One network workload set up on the GPU: context, keys, weights, encrypted inputs resident in HBM.
     Workloads with `per_group` images per ciphertext batch group (config 4) hold batch / per_group independent input sets
@@ -381,9 +404,9 @@ class NetBench:
             self.batch = per_group * n_groups
         else:
             self.groups = [pipe.encrypt_input(x, enc_seed0=10 * seed)]
-            self.batch = int(self.layers[0]["conv"]["BS"])
+            self.batch = int(self.layers[0][self.layers[0]["op"]]["BS"])
         self.n_lin, self.n_rot, self.n_relin, self.n_pm = (v * len(self.groups) for v in pipe.counts(lazy_relin=self.lazy))
-        self.n_conv = sum(1 for ly in self.layers if ly["op"] == "conv") * len(self.groups)
+        self.n_conv, self.unit = counted_layers(self.layers, len(self.groups))
         ctx.sync()
         self.setup_bytes = ctx.device_bytes()
 
@@ -444,7 +467,7 @@ def net_summary(nb, t, world):
          "images_per_s": round(world * nb.batch / s, 2), "conv_layers_per_s": round(world * nb.n_conv / s, 3),
          "linear_layers_per_s": round(world * nb.n_lin / s, 3), "rotations_per_s": round(world * (nb.n_rot + nb.n_relin) / s, 1),
          "gpu_launches": t["launches"], "clocks": t["clocks"], "peak_device_bytes": t["peak_bytes"],
-         "counts_per_step": {"conv_layers": nb.n_conv, "linear_layers": nb.n_lin, "rotations": nb.n_rot,
+         "counts_per_step": {"conv_layers": nb.n_conv if "conv" in nb.unit else 0, "linear_layers": nb.n_lin, "rotations": nb.n_rot,
                              "relinearisations": nb.n_relin, "pmults": nb.n_pm}}
     return d
 
@@ -820,7 +843,7 @@ def run_ours(args, rank, world):
         return {"workload": name, "batch": nb.batch, "ms_per_step": summ["ms_per_step"], "clocks": summ["clocks"], "per_layer": per_layer_profile(nb)}
     if args.no_extras:
         sampler.stop()
-        return {"metric": METRIC, "value": summ["conv_layers_per_s"], "unit": "encrypted conv layers/s", "ms_per_step": summ["ms_per_step"],
+        return {"metric": METRIC, "value": summ["conv_layers_per_s"], "unit": nb.unit, "ms_per_step": summ["ms_per_step"],
                 "images_per_s": summ["images_per_s"], "gpu_launches": summ["gpu_launches"], "clocks": summ["clocks"],
                 "config": {"workload": name, "batch": nb.batch}}
     prof_steps = min(args.steps, 3)
@@ -832,12 +855,12 @@ def run_ours(args, rank, world):
     # resident batch the measured footprint allows: P(n) = fixed + n (inputs + outputs of a batch group) + one group's temporaries
     max_groups = n_groups + max(0, int((0.95 * HBM_BYTES - t["peak_bytes"]) // per_group)) if WORKLOADS[name][3] else None
     line = {
-        "metric": METRIC, "value": summ["conv_layers_per_s"], "unit": "encrypted conv layers/s",
+        "metric": METRIC, "value": summ["conv_layers_per_s"], "unit": nb.unit,
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": summ["ms_per_step"],
         "images_per_s": summ["images_per_s"], "rotations_per_s": summ["rotations_per_s"],
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
         "config": {"workload": name, "description": nb.desc, "batch": nb.batch, "batch_groups": n_groups,
-                   "conv_layers_per_step": nb.n_conv, "linear_layers_per_step": nb.n_lin, "rotations_per_step": nb.n_rot,
+                   "conv_layers_per_step": nb.n_conv if "conv" in nb.unit else 0, "linear_layers_per_step": nb.n_lin, "rotations_per_step": nb.n_rot,
                    "relinearisations_per_step": nb.n_relin, "pmults_per_step": nb.n_pm,
                    "inner_rotations": "hoisted (R2.7b)" if nb.hoist else "plain",
                    "square_pool": "one relinearisation per pooled output (R2.12c)" if nb.lazy else "eager",
@@ -848,17 +871,17 @@ def run_ours(args, rank, world):
                    "max_resident_batch_rule": "batch + floor((0.95 x 180e9 - measured peak) / (input + output bytes of one batch group)) x 32"
                    if max_groups else None},
         "gpu_launches": summ["gpu_launches"], "clocks": summ["clocks"],
-        "e2e": dict({"value": round(world * nb.n_conv / (e2e["ms_per_step"] * 1e-3), 3), "unit": "encrypted conv layers/s",
+        "e2e": dict({"value": round(world * nb.n_conv / (e2e["ms_per_step"] * 1e-3), 3), "unit": nb.unit,
                      "images_per_s": round(world * nb.batch / (e2e["ms_per_step"] * 1e-3), 2),
                      "serial_value": round(world * nb.n_conv / (e2e["serial_ms_per_step"] * 1e-3), 3)}, **e2e),
         "roofline": roofline,
     }
-    layers, hoist, lazy, n_conv = nb.layers, nb.hoist, nb.lazy, nb.n_conv
+    layers, hoist, lazy, n_conv, unit = nb.layers, nb.hoist, nb.lazy, nb.n_conv, nb.unit
     nb.close()
     del nb
     if rank == 0 and world == 1:
         if not args.no_cpu:
-            line["cpu_baseline"] = cpu_baseline_for(name, layers, n_groups, n_conv, hoist, lazy, n_conv, "encrypted conv layers/s")
+            line["cpu_baseline"] = cpu_baseline_for(name, layers, n_groups, n_conv, hoist, lazy, n_conv, unit)
         if name == DEFAULT_WORKLOAD and not args.no_companions:
             line["extras"] = companions(args, sampler, dev)
     sampler.stop()
@@ -894,7 +917,7 @@ def run_reference(args):
     batch = args.batch or DEFAULT_BATCH.get(name, 1)
     layers, _ = builder(batch, 2000)
     n_groups = max(1, batch // per_group) if per_group else 1
-    n_conv = sum(1 for ly in layers if ly["op"] == "conv") * n_groups
+    n_conv, unit = counted_layers(layers, n_groups)
     p = wl.PARAMS[pkey]
     ops = oracle_op_counts(layers, 1 << (p["log2N"] - 1), p["n_q"], not args.no_hoist, not args.eager_relin)
     ops = {k: v * n_groups for k, v in ops.items()}
@@ -904,19 +927,19 @@ def run_reference(args):
     runs = [smp.sample() for _ in range(max(1, min(args.steps, 3)))]
     est = float(np.mean([r[0] for r in runs]))
     v = round(n_conv / est, 8)
-    base = {"value": v, "unit": "encrypted conv layers/s", "cores": 1, "kind": "oracle", "method": "sampled per operation x exact counts",
+    base = {"value": v, "unit": unit, "cores": 1, "kind": "oracle", "method": "sampled per operation x exact counts",
             "estimated": True, "same_graph": True, "sample_processes": runs[-1][2], "contention_factor": smp.contention, "host": host_info(),
             "sample": "per step: every (operation, level) of the workload timed on the oracle (heavy operations once, the others three "
                       "times, median) in %d concurrent worker processes, scaled by the exact operation counts; estimated step %.1f s; "
                       "%d sampled step(s) averaged whatever --steps says" % (runs[-1][2], est, len(runs)),
             "seconds_per_op": runs[-1][1]}
-    return {"impl": "reference", "metric": METRIC, "value": v, "unit": "encrypted conv layers/s", "n_gpus": 0,
+    return {"impl": "reference", "metric": METRIC, "value": v, "unit": unit, "n_gpus": 0,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(est * 1e3, 1), "higher_is_better": True,
             "images_per_s": round((per_group * n_groups if per_group else batch) / est, 6),
             "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic", "estimated": True,
             "config": {"workload": name, "description": desc, "batch": per_group * n_groups if per_group else batch},
             "cpu_baseline": base,
-            "e2e": {"value": v, "unit": "encrypted conv layers/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+            "e2e": {"value": v, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
 
 
 def respawn_under_torchrun(n):

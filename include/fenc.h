@@ -298,6 +298,13 @@ typedef struct {
   uint32_t BS, n_in, n_out;
   uint32_t in_C, in_H, in_W, in_M;
   uint32_t bsgs;
+  /* Fragment-encoded embeddings (R2.13, the Transformer extension): BS tokens, a token's
+   * embedding split in sub-blocks of S coordinates; coordinate e = p S + u lives in ciphertext u (0 <= u < S) at position
+   * p.  frag_in = S > 0: S input ciphertexts per batch group, feat(c, p) = p S + c (needs ceil(n_in / S) <= P and
+   * in_C = 0); frag_out = S' > 0: S' output ciphertexts, nu(c', p) = p S' + c'.  X W^T is then the diagonal product above;
+   * with n_in = S P it needs P - 1 = n_in / S - 1 rotations per output ciphertext (plain diagonals) instead of n_in - 1.
+   * 0: the orders stated above. */
+  uint32_t frag_in, frag_out;
 } fenc_fc_desc;
 typedef struct {
   uint32_t B, P, BG, n_in_ct, n_out_ct, n_rot /* baby + giant */, n_pmult, n_distinct_pt, n_rot_keys, bsgs /* g used */;
@@ -311,6 +318,16 @@ fenc_status fenc_fc_weights(fenc_ctx *ctx, const fenc_fc_desc *fc, const double 
                             fenc_wts **out);
 fenc_status fenc_fc_weights_from_coeffs(fenc_ctx *ctx, const fenc_fc_desc *fc, const int64_t *coeffs, size_t n,
                                         uint32_t n_limbs, double scale, fenc_wts **out);
+/* Input / output side of a fully connected layer on host arrays (the counterparts of fenc_encode_fragment and
+ * fenc_decrypt_decode): slot p B + b of input ciphertext (c, bg) holds x[bg B + b][feat(c, p)], 0 where feat is undefined
+ * or the sample index is >= BS.  host x[BS][n_in] (fp64, row-major); scale <= 0: the context default.
+ * side = 0 encodes / decodes per the INPUT order (feat), side = 1 per the OUTPUT order (nu) -- the latter to feed a next
+ * layer whose input order equals this layer's output order (frag_in' = frag_out), or to read a result. */
+fenc_status fenc_fc_encode_input(fenc_ctx *ctx, const fenc_fc_desc *fc, const double *x, uint32_t c, uint32_t batch_group,
+                                 uint32_t n_limbs, double scale, fenc_pt **out);
+/* decrypt, decode, scatter: writes only this ciphertext's entries of host y[BS][n_out] (side 1) or y[BS][n_in] (side 0) */
+fenc_status fenc_fc_decrypt_decode(fenc_ctx *ctx, const fenc_keys *keys, const fenc_ct *ct, const fenc_fc_desc *fc, int side,
+                                   uint32_t c, uint32_t batch_group, double *y);
 /* in: n_in_ct*BG ciphertexts ordered [bg][c]; out: n_out_ct*BG ordered [bg][c'] */
 fenc_status fenc_fc(fenc_ctx *ctx, const fenc_keys *keys, const fenc_fc_desc *fc, const fenc_wts *wts, fenc_ct *const *in,
                     size_t n_in, int do_rescale, fenc_ct **out, size_t n_out_capacity, size_t *n_out);

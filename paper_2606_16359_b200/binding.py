@@ -41,7 +41,7 @@ class KeyMaterial(C.Structure):
 
 
 class FcDesc(C.Structure):
-    _fields_ = [(k, C.c_uint32) for k in ("BS", "n_in", "n_out", "in_C", "in_H", "in_W", "in_M", "bsgs")]
+    _fields_ = [(k, C.c_uint32) for k in ("BS", "n_in", "n_out", "in_C", "in_H", "in_W", "in_M", "bsgs", "frag_in", "frag_out")]
 
 
 class FcInfo(C.Structure):
@@ -73,7 +73,7 @@ SYMBOLS = ["fenc_params_init", "fenc_ctx_free", "fenc_last_error", "fenc_get_pri
            "fenc_export_wait", "fenc_set_hoisting", "fenc_rotate_hoisted", "fenc_square_sum_relin",
            "fenc_wts_factors", "fenc_wts_mask_slots", "fenc_conv_weights_factored", "fenc_conv_weights_factored_from_ints",
            "fenc_measure_smac_peak", "fenc_repack", "fenc_keys_import", "fenc_sum_pool", "fenc_square_sum_pool", "fenc_poly3",
-           "fenc_rescale_static_prepare", "fenc_rescale_static"]
+           "fenc_rescale_static_prepare", "fenc_rescale_static", "fenc_fc_encode_input", "fenc_fc_decrypt_decode"]
 
 _lib = None
 
@@ -139,6 +139,8 @@ def load_library(path=None):
                                                  C.c_uint32, C.c_double, C.c_double, vpp],
         "fenc_fc_plan": [vp, C.POINTER(FcDesc), C.POINTER(FcInfo)],
         "fenc_fc_wts_keys": [vp, C.POINTER(FcDesc), u32p, C.c_size_t, C.POINTER(C.c_size_t)],
+        "fenc_fc_encode_input": [vp, C.POINTER(FcDesc), dp, C.c_uint32, C.c_uint32, C.c_uint32, C.c_double, vpp],
+        "fenc_fc_decrypt_decode": [vp, vp, vp, C.POINTER(FcDesc), C.c_int, C.c_uint32, C.c_uint32, dp],
         "fenc_fc_weights": [vp, C.POINTER(FcDesc), dp, C.c_uint32, C.c_double, vpp],
         "fenc_fc_weights_from_coeffs": [vp, C.POINTER(FcDesc), i64p, C.c_size_t, C.c_uint32, C.c_double, vpp],
         "fenc_fc": [vp, vp, C.POINTER(FcDesc), vp, vpp, C.c_size_t, C.c_int, vpp, C.c_size_t, C.POINTER(C.c_size_t)],
@@ -618,9 +620,10 @@ class Context:
         return [Ciphertext(self, C.c_void_p(out[i])) for i in range(n.value)]
 
     # ---- FC by plain diagonals
-    def fc_desc(self, BS, n_in, n_out, in_C=0, in_H=0, in_W=0, in_M=1, bsgs=1):
-        """bsgs: baby-step count g (1 = plain diagonals, 0 = the library's choice, FENC_FC_BSGS_AUTO)"""
-        return FcDesc(BS, n_in, n_out, in_C, in_H, in_W, in_M, 0xFFFFFFFF if bsgs == 0 else bsgs)
+    def fc_desc(self, BS, n_in, n_out, in_C=0, in_H=0, in_W=0, in_M=1, bsgs=1, frag_in=0, frag_out=0):
+        """bsgs: baby-step count g (1 = plain diagonals, 0 = the library's choice, FENC_FC_BSGS_AUTO);
+        frag_in / frag_out: sub-block sizes S / S' of fragment-encoded embeddings (include/fenc.h, R2.13)"""
+        return FcDesc(BS, n_in, n_out, in_C, in_H, in_W, in_M, 0xFFFFFFFF if bsgs == 0 else bsgs, frag_in, frag_out)
 
     def fc_plan(self, fc):
         info = FcInfo()
@@ -628,6 +631,17 @@ class Context:
         d = {k: int(getattr(info, k)) for k, _ in FcInfo._fields_ if k != "rot_steps"}
         d["rot_steps"] = [int(info.rot_steps[i]) for i in range(info.n_rot_keys)]
         return d
+
+    def fc_encode_input(self, fc, x, c, bg, n_limbs, scale=0.0):
+        x = np.ascontiguousarray(x, dtype=np.float64)
+        assert x.shape == (fc.BS, fc.n_in)
+        h = C.c_void_p()
+        self._ck(self.lib.fenc_fc_encode_input(self.h, C.byref(fc), _ptr(x, C.c_double), c, bg, n_limbs, float(scale), C.byref(h)))
+        return Plaintext(self, h)
+
+    def fc_decrypt_decode(self, keys, ct, fc, side, c, bg, y):
+        assert y.dtype == np.float64 and y.flags["C_CONTIGUOUS"] and y.shape == (fc.BS, fc.n_out if side else fc.n_in)
+        self._ck(self.lib.fenc_fc_decrypt_decode(self.h, keys.h, ct.h, C.byref(fc), side, c, bg, _ptr(y, C.c_double)))
 
     def fc_wts_keys(self, fc):
         n = C.c_size_t()

@@ -923,6 +923,10 @@ struct FcGraph : LinGraph {
   std::vector<std::array<u32, 3>> wkeys;  // (c_out_ct, c_in_ct, d)
   // feature index of (input ct c, position p) or -1
   long feat(int c, int p) const {
+    if (d.frag_in) {  // fragment-encoded embeddings (R2.13): coordinate p S + c of every token
+      const long f = (long)p * d.frag_in + c;
+      return f < (long)d.n_in ? f : -1;
+    }
     if (d.in_C) {
       const int m2 = m * m, cpos = p / m2, k = p % m2, chan = c * ch + cpos, h = k / m, w = k % m;
       if (chan >= (int)d.in_C || h >= (int)d.in_H || w >= (int)d.in_W) return -1;
@@ -932,7 +936,7 @@ struct FcGraph : LinGraph {
     return f < (long)d.n_in ? f : -1;
   }
   long neuron(int c, int p) const {
-    const long v = (long)c * P + p;
+    const long v = d.frag_out ? (long)p * d.frag_out + c : (long)c * P + p;
     return v < (long)d.n_out ? v : -1;
   }
   bool nonzero(int co, int ci, int dd) const {
@@ -954,7 +958,8 @@ struct FcGraph : LinGraph {
 
 static fenc_status fc_graph(fenc_ctx *ctx, const fenc_fc_desc *fd, std::shared_ptr<FcGraph> &out) {
   char keybuf[256];
-  snprintf(keybuf, sizeof keybuf, "fc,%u,%u,%u,%u,%u,%u,%u,%u", fd->BS, fd->n_in, fd->n_out, fd->in_C, fd->in_H, fd->in_W, fd->in_M, fd->bsgs);
+  snprintf(keybuf, sizeof keybuf, "fc,%u,%u,%u,%u,%u,%u,%u,%u,%u,%u", fd->BS, fd->n_in, fd->n_out, fd->in_C, fd->in_H, fd->in_W, fd->in_M, fd->bsgs,
+           fd->frag_in, fd->frag_out);
   auto it = ctx->graphs.find(keybuf);
   if (it != ctx->graphs.end()) {
     out = std::static_pointer_cast<FcGraph>(it->second);
@@ -969,14 +974,24 @@ static fenc_status fc_graph(fenc_ctx *ctx, const fenc_fc_desc *fd, std::shared_p
   g->P = g->n / g->B;
   g->ch = (int)(g->n / (g->B * m2));
   g->BG = (fd->BS + g->B - 1) / g->B;
-  if (fd->in_C) {
+  if (fd->frag_in) {
+    if (fd->in_C || (fd->n_in + fd->frag_in - 1) / fd->frag_in > (u32)g->P)
+      return fail(ctx, FENC_ERR_LAYOUT, "frag_in=%u: the %u sub-blocks of an embedding must fit the %d positions (and in_C = 0)", fd->frag_in,
+                  (fd->n_in + fd->frag_in - 1) / fd->frag_in, g->P);
+    g->n_in_ct = fd->frag_in;
+  } else if (fd->in_C) {
     if (fd->in_H > fd->in_M || fd->in_W > fd->in_M || (size_t)fd->in_C * fd->in_H * fd->in_W != fd->n_in)
       return fail(ctx, FENC_ERR_LAYOUT, "fc input tensor does not match n_in");
     g->n_in_ct = (fd->in_C + g->ch - 1) / g->ch;
   } else {
     g->n_in_ct = (fd->n_in + g->P - 1) / g->P;
   }
-  g->n_out_ct = (fd->n_out + g->P - 1) / g->P;
+  if (fd->frag_out) {
+    if ((fd->n_out + fd->frag_out - 1) / fd->frag_out > (u32)g->P) return fail(ctx, FENC_ERR_LAYOUT, "frag_out=%u: sub-blocks do not fit the %d positions", fd->frag_out, g->P);
+    g->n_out_ct = fd->frag_out;
+  } else {
+    g->n_out_ct = (fd->n_out + g->P - 1) / g->P;
+  }
   g->nin_bg = g->n_in_ct;
   // baby-step count: 1 (or 0) = plain diagonals; FENC_FC_BSGS_AUTO = the power of two g | P with the fewest rotations
   // n_in_ct (g-1) + n_out_ct (P/g - 1) of a dense layer, ties to the smaller g; else a power of two dividing P
@@ -1034,6 +1049,44 @@ extern "C" fenc_status fenc_fc_plan(fenc_ctx *ctx, const fenc_fc_desc *fd, fenc_
   out->n_rot = (u32)((g->n_outer + g->inner.size()) * g->BG), out->bsgs = (u32)g->g, out->n_pmult = (u32)(g->n_pmult * g->BG), out->n_distinct_pt = (u32)g->wkeys.size();
   out->n_rot_keys = (u32)g->rot_steps.size();
   for (size_t i = 0; i < g->rot_steps.size(); i++) out->rot_steps[i] = g->rot_steps[i];
+  return FENC_OK;
+}
+extern "C" fenc_status fenc_fc_encode_input(fenc_ctx *ctx, const fenc_fc_desc *fd, const double *x, uint32_t c, uint32_t bgi, uint32_t n_limbs,
+                                            double scale, fenc_pt **out) {
+  if (!ctx || !fd || !x || !out) return FENC_ERR_INVALID_ARG;
+  std::shared_ptr<FcGraph> g;
+  fenc_status st = fc_graph(ctx, fd, g);
+  if (st != FENC_OK) return st;
+  if ((int)c >= g->n_in_ct || (int)bgi >= g->BG) return fail(ctx, FENC_ERR_LAYOUT, "fc input ciphertext index out of range");
+  std::vector<double> vec(ctx->n, 0.0);
+  for (int p = 0; p < g->P; p++) {
+    const long f = g->feat((int)c, p);
+    if (f < 0) continue;
+    for (int b = 0; b < g->B; b++) {
+      const size_t bb = (size_t)bgi * g->B + b;
+      if (bb < fd->BS) vec[(size_t)p * g->B + b] = x[bb * fd->n_in + f];
+    }
+  }
+  return fenc_encode_slots(ctx, vec.data(), nullptr, n_limbs, scale, out);
+}
+extern "C" fenc_status fenc_fc_decrypt_decode(fenc_ctx *ctx, const fenc_keys *K, const fenc_ct *ct, const fenc_fc_desc *fd, int side, uint32_t c,
+                                              uint32_t bgi, double *y) {
+  if (!ctx || !K || !ct || !fd || !y) return FENC_ERR_INVALID_ARG;
+  std::shared_ptr<FcGraph> g;
+  fenc_status st = fc_graph(ctx, fd, g);
+  if (st != FENC_OK) return st;
+  if ((int)c >= (side ? g->n_out_ct : g->n_in_ct) || (int)bgi >= g->BG) return fail(ctx, FENC_ERR_LAYOUT, "fc ciphertext index out of range");
+  std::vector<double> vec(ctx->n);
+  if ((st = fenc_decrypt_slots(ctx, K, ct, vec.data(), nullptr)) != FENC_OK) return st;
+  const size_t width = side ? fd->n_out : fd->n_in;
+  for (int p = 0; p < g->P; p++) {
+    const long v = side ? g->neuron((int)c, p) : g->feat((int)c, p);
+    if (v < 0) continue;
+    for (int b = 0; b < g->B; b++) {
+      const size_t bb = (size_t)bgi * g->B + b;
+      if (bb < fd->BS) y[bb * width + v] = vec[(size_t)p * g->B + b];
+    }
+  }
   return FENC_OK;
 }
 extern "C" fenc_status fenc_fc_wts_keys(fenc_ctx *ctx, const fenc_fc_desc *fd, uint32_t *keys3, size_t capacity, size_t *n) {

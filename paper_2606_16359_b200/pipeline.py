@@ -129,8 +129,16 @@ class Pipeline:
         return self.keys
 
     def encrypt_input(self, x, enc_seed0):
-        """Algorithm 1 on host x[BS][C][H][W] for the first layer; ciphertext order [bg][g][u][v]."""
+        """Algorithm 1 on host x[BS][C][H][W] for the first layer; ciphertext order [bg][g][u][v].  A network that starts
+        with a fully connected layer takes x[BS][n_in] (token embeddings, R2.13); order [bg][c]."""
         p = self.plan[0]
+        if p["op"] == "fc":
+            ctx, cts = self.ctx, []
+            per_bg = p["info"]["n_in_ct"] // p["info"]["BG"]
+            for bg in range(p["info"]["BG"]):
+                for c in range(per_bg):
+                    cts.append(ctx.encrypt(self.keys, ctx.fc_encode_input(p["fc"], x, c, bg, p["L"]), enc_seed0 + len(cts)))
+            return cts
         conv, lay, ctx = p["conv"], p["lay"], self.ctx
         cts = []
         for bg in range(lay.BG):

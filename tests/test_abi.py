@@ -25,8 +25,9 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_struct_layouts_match_header():
-    from paper_2606_16359_b200 import ConvDesc, Layout, ParamsDesc
+    from paper_2606_16359_b200 import ConvDesc, FcDesc, Layout, ParamsDesc
     assert ctypes.sizeof(ConvDesc) == 14 * 4
+    assert ctypes.sizeof(FcDesc) == 10 * 4
     assert ctypes.sizeof(Layout) == 22 * 4 + 2 * 8 + 512 * 4
     assert ParamsDesc.log2_scale.offset == 32 and ParamsDesc.q_override.offset == 40
 

@@ -667,6 +667,11 @@ def test_import_async_matches_import(mods):
     dict(BS=16, n_in=70, n_out=40, in_M=2, bsgs=0),                          # P = 32: 3 input cts, 2 output cts
     dict(BS=16, n_in=70, n_out=40, in_M=2, bsgs=0, hoist=True),              # baby steps in the hoisted form (R2.7b)
     dict(BS=40, n_in=3 * 3 * 3, n_out=20, in_C=3, in_H=3, in_W=3, in_M=4, bsgs=4, hoist=True),
+    # fragment-encoded token embeddings (R2.13): E = S P exactly (the paper's case), ragged, mixed orders, with BSGS
+    dict(BS=16, n_in=64, n_out=64, in_M=2, frag_in=2, frag_out=2),           # P = 32 = E / S
+    dict(BS=40, n_in=30, n_out=20, in_M=4, frag_in=2, frag_out=4, bsgs=0),   # two batch groups, ragged sub-blocks
+    dict(BS=16, n_in=60, n_out=40, in_M=2, frag_in=4, bsgs=0, hoist=True),   # fragment-encoded in, positional out
+    dict(BS=16, n_in=40, n_out=64, in_M=2, frag_out=2),                      # positional in, fragment-encoded out
 ])
 def test_fc_bit_exact(mods, kw):
     ck, fr, fenc = mods
@@ -708,6 +713,23 @@ def test_fc_bit_exact(mods, kw):
     # the library's own weight encoder lands within one unit of the oracle's integers (A7)
     gW2 = ctx.fc_weights(fcd, W, L)
     assert gW2 is not None
+    # fenc_fc_encode_input / fenc_fc_decrypt_decode: the library's gather + encoder lands within one unit of the oracle's
+    # integers on every input ciphertext, and its scatter places the decrypted slots where the oracle's does
+    for bg in range(g.BG):
+        for ci in range(g.n_in_ct):
+            want = ck.encode(P, g.gather_in(X, ci, bg), L).coeffs
+            got = ctx.pt_coeffs(ctx.fc_encode_input(fcd, X, ci, bg, L))
+            assert np.abs(got - want).max() <= 1, (bg, ci)
+    Y2 = np.zeros_like(Y)
+    for bg in range(g.BG):
+        for co in range(g.n_out_ct):
+            ctx.fc_decrypt_decode(gk, g_out[bg * g.n_out_ct + co], fcd, 1, co, bg, Y2)
+    assert np.array_equal(Y2, Y)
+    X2 = np.zeros_like(X)
+    for bg in range(g.BG):
+        for ci in range(g.n_in_ct):
+            ctx.fc_decrypt_decode(gk, g_in[bg * g.n_in_ct + ci], fcd, 0, ci, bg, X2)
+    assert np.abs(X2 - X).max() < 1e-6
     ctx.close()
 
 

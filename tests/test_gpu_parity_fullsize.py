@@ -255,6 +255,53 @@ def test_cfg3_resnet_16_16_bsgs_full_size_sampled(mods):
 
 
 # ------------------------------------------------------------------------------------------------ config 5 paths
+def test_transformer_linear_fragment_embeddings_full_size_sampled(mods):
+    """bench.py's `ext_transformer_linear` (R2.13) in its launch configuration: N=2^16, 24x50b +
+    4x60b, 128 tokens, 768 -> 768 on fragment-encoded embeddings (S = S' = 3: 3 -> 3 ciphertexts, E / S = P = 256), the
+    library's g = 16 (45 hoisted baby rotations + 45 giant rotations instead of 765), hoisted.  Output ciphertext 2 restricted
+    to giant steps 0 and 7 and, inside each, to the baby steps 0, 3 and 15 of all three inputs (18 PMults, 6 hoisted + 1
+    plain rotation, rescale) against the oracle; the other outputs (all-zero weights) are zero."""
+    ck, fr, fenc = mods
+    from oracle import network as nw
+    P, ctx = make(mods, wl.PARAMS["cfg3"])
+    L = P.nq
+    kw = dict(BS=128, n_in=768, n_out=768, in_M=1, frag_in=3, frag_out=3, bsgs=0)
+    g = nw.FcGraph(P.n, **kw)
+    fcd = ctx.fc_desc(**kw)
+    info = ctx.fc_plan(fcd)
+    c = g.counts()
+    assert {k: info[k] for k in c} == c and info["bsgs"] == 16 and info["n_rot"] == 90 and info["n_pmult"] == 2304
+    assert nw.FcGraph(P.n, **dict(kw, bsgs=1)).counts()["n_rot"] == 3 * (768 // 3 - 1)  # the paper's E/S - 1 per output ciphertext
+    co, giants, babies = 2, (0, 7), (0, 3, 15)
+    W = np.random.default_rng(2013).normal(0, 768 ** -0.5, (768, 768))
+    s_w = P.q[L - 1]
+    terms = {i: [(ci, j * g.B % P.n, wk) for ci, j, wk in g.terms[co][i] if j in babies] for i in giants}
+    assert all(len(lst) == 9 for lst in terms.values())
+    oW = {wk: ck.encode(P, g.weight_slots(wk, W), L, s_w) for lst in terms.values() for _, _, wk in lst}
+    keys3 = ctx.fc_wts_keys(fcd)
+    coeffs = np.zeros((len(keys3), P.N), dtype=np.int64)
+    for i, k in enumerate(keys3):
+        wk = tuple(int(v) for v in k)
+        if wk in oW:
+            coeffs[i] = oW[wk].coeffs
+    gW = ctx.fc_weights_from_coeffs(fcd, coeffs, L, float(s_w))
+    del coeffs
+    rot_of = {i: i * g.g * g.B % P.n for i in giants}
+    need = sorted({amt for lst in terms.values() for _, amt, _ in lst if amt} | {r for r in rot_of.values() if r})
+    gk, ok = ctx.keygen(81, c["rot_steps"]), ck.keygen(P, 81, need)
+    o_in, g_in = {}, []
+    for ci in range(g.n_in_ct):
+        limbs = wl.random_ct_limbs(6100 + ci, P.q, L, P.N)
+        o_in[ci] = ck.Ciphertext(limbs, L, P.scale)
+        g_in.append(ctx.ct_import(limbs, float(P.scale)))
+    ctx.set_hoisting(True)
+    g_out = ctx.fc(gk, fcd, gW, g_in)
+    ref = oracle_linear_sample(ck, P, ok, L, o_in, terms, rot_of, oW, True, P.scale, s_w)
+    assert g_out[co].L == L - 1 and np.array_equal(ctx.ct_export(g_out[co]), ref.c)
+    assert not ctx.ct_export(g_out[0]).any() and not ctx.ct_export(g_out[1]).any()
+    ctx.close()
+
+
 @pytest.mark.parametrize("n_q,n_p,dnum", [(12, 12, 1), (16, 16, 1), (24, 24, 1), (24, 12, 2), (26, 26, 1), (30, 30, 1)])
 def test_rotation_wide_and_unfused_digits(mods, n_q, n_p, dnum):
     """Config 5's widest digits at N=2^12 (same kernels, 4 column tiles per limb): dlen 12, 16, 24 run the fused column
