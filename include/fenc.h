@@ -180,9 +180,13 @@ fenc_status fenc_ct_import(fenc_ctx *ctx, const uint64_t *limbs, uint32_t L, dou
  * unchanged until the next synchronising call on this context returns (fenc_sync, fenc_ct_export, any decrypt).
  * Serving loops use it to upload the next request while the current one computes. */
 fenc_status fenc_ct_import_async(fenc_ctx *ctx, const uint64_t *limbs, uint32_t L, double scale, fenc_ct **out);
-/* fenc_ct_export without the host synchronisation: `limbs` (host, page-locked for a truly asynchronous copy; owned by
- * the caller) holds the result once fenc_export_wait (or any synchronising call) has returned.  fenc_export_wait blocks
- * until every fenc_ct_export_async issued so far has landed; work enqueued on the context after them is not waited for. */
+/* fenc_ct_export without the host synchronisation: the inverse transform is enqueued on the context's stream, the
+ * device->host copy on a second stream of the context's own, so kernels enqueued behind the export do not wait for the
+ * bus.  `limbs` (host, page-locked for a truly asynchronous copy; owned by the caller) holds the result once
+ * fenc_export_wait or fenc_sync has returned.  fenc_export_wait blocks until every fenc_ct_export_async issued so far has
+ * landed; work enqueued on the context after them is not waited for.  The ciphertext may be freed or overwritten right
+ * after the call (the transform reads it in stream order).  While in flight an export holds a device buffer of the
+ * ciphertext's size. */
 fenc_status fenc_ct_export_async(fenc_ctx *ctx, const fenc_ct *ct, uint64_t *limbs);
 fenc_status fenc_export_wait(fenc_ctx *ctx);
 fenc_status fenc_ct_info(fenc_ctx *ctx, const fenc_ct *ct, uint32_t *L, double *scale, void **device_ptr);

@@ -250,7 +250,10 @@ extern "C" void fenc_ctx_free(fenc_ctx *ctx) {
     if (sl.consumed) cudaEventDestroy(sl.consumed);
   }
   if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
-  if (ctx->export_ev) cudaEventDestroy(ctx->export_ev);
+  export_drain(ctx, true);
+  for (cudaEvent_t e : ctx->export_events) cudaEventDestroy(e);
+  if (ctx->export_ready) cudaEventDestroy(ctx->export_ready);
+  if (ctx->d2h_stream) cudaStreamDestroy(ctx->d2h_stream);
   dfree(ctx, ctx->ws), dfree(ctx, ctx->desc_buf);
   if (ctx->desc_pinned) {
     for (int i = 0; i < FENC_DESC_SLOTS; i++) cudaEventDestroy(ctx->desc_ev[i]);
@@ -278,7 +281,7 @@ extern "C" fenc_status fenc_set_hoisting(fenc_ctx *ctx, int on) {
 extern "C" fenc_status fenc_sync(fenc_ctx *ctx) {
   if (!ctx) return FENC_ERR_INVALID_ARG;
   CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
-  return FENC_OK;
+  return export_drain(ctx, true);  // results of fenc_ct_export_async have landed once a synchronising call returns
 }
 extern "C" uint64_t fenc_launch_count(fenc_ctx *ctx, int reset) {
   if (!ctx) return 0;

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <array>
+#include <deque>
 #include <map>
 #include <memory>
 #include <string>
@@ -53,9 +54,13 @@ struct LevelPlan {
 
 struct LinGraph;  // fenc_conv.cu: operation graph of a linear layer (conv or fc)
 
-// one slot of the staging ring behind fenc_ct_import_async: the copy stream fills it, the context's stream transforms it
-#define FENC_STAGE_SLOTS 64
-#define FENC_STAGE_BYTES ((size_t)256 << 20)
+// one slot of the staging queue behind fenc_ct_import_async: the copy stream fills it, the context's stream transforms it.
+// The queue is first-in first-out and GROWS while its oldest slot is still waiting for its transform, up to
+// FENC_STAGE_BYTES_MAX (environment FENC_STAGE_MAX_MB): a serving loop uploads request i+2 while request i+1 computes, and
+// the transforms of those uploads are enqueued BEHIND request i+1's kernels, so a queue shorter than one request's inputs
+// stalls the bus until request i+1 has finished (measured on config 4: 8 slots of 31 MB for 6 GB of inputs left the
+// compute stream idle for about 100 ms per request).
+#define FENC_STAGE_BYTES_MAX ((size_t)8 << 30)
 struct StageSlot {
   u64 *d = nullptr;
   size_t bytes = 0;
@@ -95,11 +100,20 @@ struct fenc_ctx {
   unsigned desc_next = 0;
   std::map<std::string, std::shared_ptr<LinGraph>> graphs;
   cudaStream_t copy_stream = nullptr;  // host -> staging copies of fenc_ct_import_async (created on first use)
-  std::vector<StageSlot> stage;
-  size_t stage_next = 0;
-  cudaEvent_t export_ev = nullptr;     // behind the last fenc_ct_export_async (fenc_export_wait)
+  std::deque<StageSlot> stage;         // oldest use first
+  size_t stage_bytes = 0, stage_max = 0;
+  // fenc_ct_export_async: the inverse transform runs on the context's stream into a buffer of its own, the device -> host
+  // copy on d2h_stream; the buffer returns to the pool once its copy has landed (export_drain)
+  cudaStream_t d2h_stream = nullptr;
+  cudaEvent_t export_ready = nullptr;  // re-recorded behind every export's transform; the copy stream waits for it
+  struct PendingExport { void *buf; cudaEvent_t landed; };
+  std::deque<PendingExport> exports;   // in issue order
+  std::vector<cudaEvent_t> export_events;  // recycled `landed` events
   bool hoist_inner = false;            // fenc_set_hoisting: inner rotations of linear layers in the hoisted form (R2.7b)
 };
+
+// returns the staging buffers of exports whose copies have landed to the pool; block: wait for all of them
+fenc_status export_drain(fenc_ctx *ctx, bool block);
 
 struct fenc_keys {
   fenc_ctx *ctx;

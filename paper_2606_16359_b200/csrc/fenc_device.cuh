@@ -119,7 +119,16 @@ DEVI u64 mulmod_f64(u64 x, u64 c_bits, u64 cq_bits, const F64Mod &m) {  // (0, 2
 // round ends with a reduction); only the first round converts from the unsigned words of the fill and only the last one
 // back to the unsigned lazy words every consumer expects.  ncu on the fused column kernel (profiles/r02_cfg4_step_ncu.md):
 // FP64 pipe 59 % busy, and a quarter of its FP64 instructions were these per-round conversions.
-template <bool FWD, bool LAZY, int PW, int SLO, int SHI, int F64, bool FIRST = true, bool LAST = true>  // F64: 0 integer, 1 fp64 narrow (q < 2^45), 2 fp64 wide
+// TWS: `tw` points at a copy of the pass's twiddles in SHARED memory (a "slab", see tw_slab_fill) that the block filled
+// once and reuses for every tile it transforms with these twiddles; the caller passes the geometry the copy is indexed
+// by.  Without it every round fetches its seven twiddle pairs from L2 -- for a row pass 16 KB of twiddles per 8 KB tile,
+// and the first multiply of every round waits for them (ncu, divide pass: 9 % of all stall samples on that one DFMA).
+template <int TWS>
+DEVI ulonglong2 tw_load(const ulonglong2 *p) {
+  if constexpr (TWS != 0) return *p;
+  else return __ldg(p);
+}
+template <bool FWD, bool LAZY, int PW, int SLO, int SHI, int F64, bool FIRST = true, bool LAST = true, int TWS = 0>  // F64: 0 integer, 1 fp64 narrow (q < 2^45), 2 fp64 wide
 DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid, u64 f64) {
   const int ebase = ((tid >> PW) << (PW + 3)) | (tid & ((1 << PW) - 1));
   const int gpw = G.gbit(PW);
@@ -127,11 +136,22 @@ DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 
   const ulonglong2 *twv = reinterpret_cast<const ulonglong2 *>(tw);
   ulonglong2 t2 = make_ulonglong2(0, 0), t1[2], t0[4];
   // twiddles first: their L2 latency overlaps the shared-memory loads
-  if (2 >= SLO && 2 < SHI) t2 = __ldg(twv + (nj >> (gpw + 3)));
+  if (2 >= SLO && 2 < SHI) t2 = tw_load<TWS>(twv + (nj >> (gpw + 3)));
+  if constexpr (TWS == 2 && PW == 0) {
+    // row slab, round over the lowest bits: thread tid owns elements 8 tid .. 8 tid + 7, whose two (four) twiddles of
+    // bit 1 (bit 0) are adjacent entries -- a stride of 32 (64) bytes between threads, a 2-way (4-way) bank conflict.
+    // tw_slab_fill stores these two levels transposed, [i][tid], so each of the loads is unit-stride.
+    const int nth = 1 << (G.logN - 3);
 #pragma unroll
-  for (int i = 0; i < 2; i++) t1[i] = (1 >= SLO && 1 < SHI) ? __ldg(twv + (nj >> (gpw + 2)) + i) : t2;
+    for (int i = 0; i < 2; i++) t1[i] = (1 >= SLO && 1 < SHI) ? twv[(2 + i) * nth + tid] : t2;
 #pragma unroll
-  for (int i = 0; i < 4; i++) t0[i] = (0 >= SLO && 0 < SHI) ? __ldg(twv + (nj >> (gpw + 1)) + i) : t2;
+    for (int i = 0; i < 4; i++) t0[i] = (0 >= SLO && 0 < SHI) ? twv[(4 + i) * nth + tid] : t2;
+  } else {
+#pragma unroll
+    for (int i = 0; i < 2; i++) t1[i] = (1 >= SLO && 1 < SHI) ? tw_load<TWS>(twv + (nj >> (gpw + 2)) + i) : t2;
+#pragma unroll
+    for (int i = 0; i < 4; i++) t0[i] = (0 >= SLO && 0 < SHI) ? tw_load<TWS>(twv + (nj >> (gpw + 1)) + i) : t2;
+  }
   const int sbase = swz(ebase);
   if constexpr (F64 != 0) {
     // The eight values stay doubles (signed, exact integers) through the round's stages; T is in (-q, q).
@@ -224,16 +244,16 @@ DEVI void tile_sync(int bar) {
   if constexpr (GRP) asm volatile("bar.sync %0, 128;" ::"r"(bar) : "memory");
   else __syncthreads();
 }
-template <bool FWD, bool LAZY, int LT, int LO, int NB, int DONE, int F64 = 0, bool GRP = false>
+template <bool FWD, bool LAZY, int LT, int LO, int NB, int DONE, int F64 = 0, bool GRP = false, int TWS = 0>
 DEVI void tile_rounds_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid, u64 f64 = 0, int bar = 0) {
   if constexpr (DONE < NB) {
     constexpr int take = NB - DONE < 3 ? NB - DONE : 3;
     constexpr int cur = FWD ? LO + NB - DONE : LO + DONE;         // FWD: exclusive top; INV: inclusive bottom
     constexpr int p = FWD ? cur - take : cur;
     constexpr int pw = p < LT - 3 ? p : LT - 3;
-    if (tid < (1 << (LT - 3))) tile_round_ct<FWD, LAZY, pw, p - pw, p - pw + take, F64, DONE == 0, (DONE + take >= NB)>(sm, G, tw, q, q2, tid, f64);
+    if (tid < (1 << (LT - 3))) tile_round_ct<FWD, LAZY, pw, p - pw, p - pw + take, F64, DONE == 0, (DONE + take >= NB), TWS>(sm, G, tw, q, q2, tid, f64);
     tile_sync<GRP>(bar);
-    tile_rounds_ct<FWD, LAZY, LT, LO, NB, DONE + take, F64, GRP>(sm, G, tw, q, q2, tid, f64, bar);
+    tile_rounds_ct<FWD, LAZY, LT, LO, NB, DONE + take, F64, GRP, TWS>(sm, G, tw, q, q2, tid, f64, bar);
   }
 }
 
@@ -274,21 +294,49 @@ DEVI void tile_round_rt(u64 *sm, const TileGeo &G, int pw, int s_lo, int s_hi, c
 
 // compile-time schedule over active tile bits [LO, LO+NB) of a 2^LT-element tile; picks the lazy forward butterflies
 // for q < 2^58.  Every thread of the block must call this (it synchronises).
-template <bool FWD, int LT, int LO, int NB, bool GRP = false>
+template <bool FWD, int LT, int LO, int NB, bool GRP = false, int TWS = 0>
 DEVI void tile_transform_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, int tid, u64 f64, int bar = 0) {
   const u64 q2 = q + q;
-  if (f64 && q < (1ull << FENC_F64_MAX_BITS)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 1, GRP>(sm, G, tw, q, q2, tid, f64, bar);
-  else if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 2, GRP>(sm, G, tw, q, q2, tid, f64, bar);
-  else if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 0, GRP>(sm, G, tw, q, q2, tid, 0, bar);
-  else tile_rounds_ct<FWD, false, LT, LO, NB, 0, 0, GRP>(sm, G, tw, q, q2, tid, 0, bar);
+  if (f64 && q < (1ull << FENC_F64_MAX_BITS)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 1, GRP, TWS>(sm, G, tw, q, q2, tid, f64, bar);
+  else if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 2, GRP, TWS>(sm, G, tw, q, q2, tid, f64, bar);
+  else if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 0, GRP, TWS>(sm, G, tw, q, q2, tid, 0, bar);
+  else tile_rounds_ct<FWD, false, LT, LO, NB, 0, 0, GRP, TWS>(sm, G, tw, q, q2, tid, 0, bar);
 }
+
+// The twiddles of a ROW pass over the 2^LT contiguous coefficients of tile `tile`, copied to shared memory in heap order:
+// slab[(2^LT + e) >> (g + 1)] is the twiddle of global bit g (0 <= g < LT) for the tile-local element e, i.e. entry
+// idx in [2^lvl, 2^(lvl+1)) is tw[((N + tile 2^LT) >> (LT - lvl)) + idx - 2^lvl].  A round indexes the slab exactly as it
+// indexes the table when it is given the geometry row_slab_geo(): ring degree 2^LT, tile 0 -- except the two lowest
+// levels (bits 1 and 0), which are stored transposed for the round over the lowest bits (TWS = 2 in tile_round_ct): entry
+// 2^(LT-2) + 2 t + i sits at (2 + i) 2^(LT-3) + t and entry 2^(LT-1) + 4 t + i at (4 + i) 2^(LT-3) + t.
+// 2^LT entries of 16 bytes (entry 0 unused), copied with cp.async: the caller commits, waits and synchronises before the
+// first transform.
+DEVI void cp_async16(void *dst_smem, const void *src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
+}
+template <int LT>
+DEVI void tw_slab_fill(ShoupC *slab, const ShoupC *tw, int logN, u32 tile, int tid, int nth) {
+  constexpr int NT8 = 1 << (LT - 3);
+  const u32 base = (1u << logN) + (tile << LT);
+  for (int idx = tid; idx < (1 << LT); idx += nth) {
+    if (idx == 0) continue;
+    const int lvl = 31 - __clz(idx), loc = idx - (1 << lvl);
+    const int pos = lvl == LT - 1 ? (4 + (loc & 3)) * NT8 + (loc >> 2) : (lvl == LT - 2 ? (2 + (loc & 1)) * NT8 + (loc >> 1) : idx);
+    cp_async16(slab + pos, tw + (base >> (LT - lvl)) + loc);
+  }
+  asm volatile("cp.async.commit_group;" ::: "memory");
+}
+DEVI void tw_slab_wait() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+template <int LT>
+DEVI TileGeo row_slab_geo() { return TileGeo{LT, LT, 0, LT, 0}; }
 
 // GEO selects the schedule: 0 = runtime (any lo/nb), 1 = row pass of 2048-element tiles with 8 stages,
 // 4..8 = column pass with GEO stages over tiles of 2^(GEO+4) elements (16 columns).
 // Every thread of the block must call this (it synchronises).  Outputs: forward < 33q (use fullred), inverse < 2q.
-template <bool FWD, int GEO>
+template <bool FWD, int GEO, int TWS = 0>
 DEVI void tile_transform(u64 *sm, const TileGeo &G, int lo, int nb, const ShoupC *tw, u64 q, int tid, u64 f64) {
   const u64 q2 = q + q;
+  static_assert(!(TWS && GEO == 0), "twiddle slabs exist for the compile-time schedules only");
   if constexpr (GEO == 0) {
     const bool active = tid < (1 << (G.lt - 3));
     if (FWD) {
@@ -313,9 +361,9 @@ DEVI void tile_transform(u64 *sm, const TileGeo &G, int lo, int nb, const ShoupC
     }
   } else {
     constexpr int LT = GEO == 1 ? FENC_ROW_LT : GEO + 4, LO = GEO == 1 ? 0 : 4, NB = GEO == 1 ? 8 : GEO;
-    if (f64 && q < (1ull << FENC_F64_MAX_BITS)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 1>(sm, G, tw, q, q2, tid, f64);
-    else if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 2>(sm, G, tw, q, q2, tid, f64);
-    else if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
-    else tile_rounds_ct<FWD, false, LT, LO, NB, 0>(sm, G, tw, q, q2, tid);
+    if (f64 && q < (1ull << FENC_F64_MAX_BITS)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 1, false, TWS>(sm, G, tw, q, q2, tid, f64);
+    else if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 2, false, TWS>(sm, G, tw, q, q2, tid, f64);
+    else if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 0, false, TWS>(sm, G, tw, q, q2, tid);
+    else tile_rounds_ct<FWD, false, LT, LO, NB, 0, 0, false, TWS>(sm, G, tw, q, q2, tid);
   }
 }

@@ -399,47 +399,81 @@ __global__ void __launch_bounds__(512, 2) ntt_colpass_kernel(NttColP p) {
 struct NttRowP {
   const u64 *src; size_t src_bstride; u64 *dst; size_t dst_bstride; const RowDesc *rows; const ModConst *mods;
   const ShoupC *tw; NttGeom g; int src_is_dst_row;
+  int n_batch, bpb;  // SLAB: batch items per block
 };
 // ROW_TPB consecutive tiles of one row per block (compile-time geometries): the next tile's words are requested into
 // registers before the current tile is transformed, so a block keeps loads in flight during its arithmetic (one tile
 // per block left about 13 KB per SM in flight on average, a third of what HBM's latency needs).
+// SLAB (batches of FENC_SLAB_MIN_BATCH items and more): the block stays on ONE tile position of its row and walks over
+// p.bpb batch items, so the row pass's twiddles for that position (16 KB, twice the tile) are copied to shared memory
+// once per block instead of being fetched from L2 by every round of every tile; the next item's tile is prefetched into
+// registers all the same.
 #ifndef FENC_ROW_TPB
 #define FENC_ROW_TPB 4
 #endif
-template <int GEO>
+#ifndef FENC_SLAB_MIN_BATCH
+#define FENC_SLAB_MIN_BATCH 4
+#endif
+#ifndef FENC_SLAB_BPB
+#define FENC_SLAB_BPB 4
+#endif
+static inline bool use_slab(const NttGeom &g, int n_batch) { return g.logN >= 12 && n_batch >= FENC_SLAB_MIN_BATCH; }
+static inline size_t slab_bytes(const NttGeom &g) { return (sizeof(u64) << g.lt_row) + (sizeof(ShoupC) << g.lt_row); }
+template <int GEO, bool SLAB = false>
 __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? 6 : 4) ntt_rowpass_kernel(NttRowP p) {
+  static_assert(!SLAB || GEO == 1, "slabs: compile-time row geometry");
   extern __shared__ u64 sm[];
-  const int tid = threadIdx.x, b = blockIdx.z;
+  const int tid = threadIdx.x;
   const RowDesc rd = p.rows[blockIdx.y];
   const int N = 1 << p.g.logN, T = 1 << p.g.lt_row;
   constexpr int TPB = GEO == 1 ? FENC_ROW_TPB : 1;
-  const u64 *src = p.src + (size_t)b * p.src_bstride + (size_t)(p.src_is_dst_row ? rd.dst_row : rd.src_row) * N;
-  u64 *dst = p.dst + (size_t)b * p.dst_bstride + (size_t)rd.dst_row * N;
+  const int b0 = SLAB ? blockIdx.z * p.bpb : blockIdx.z;
+  const int n_it = SLAB ? min(p.bpb, p.n_batch - b0) : TPB;
+  const size_t src_off = (size_t)(p.src_is_dst_row ? rd.dst_row : rd.src_row) * N, dst_off = (size_t)rd.dst_row * N;
   const int nth = blockDim.x;
   const ModConst mc = p.mods[rd.mod];
+  ShoupC *slab = reinterpret_cast<ShoupC *>(sm + T);
   u64 v[8];
-  auto request = [&](u32 tile) {
-    TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, tile};
+  auto request = [&](int k) {
+    TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, SLAB ? blockIdx.x : blockIdx.x * TPB + k};
+    const u64 *src = p.src + (size_t)(SLAB ? b0 + k : b0) * p.src_bstride + src_off;
 #pragma unroll
     for (int i = 0; i < 8; i++) {
       const int e = tid + i * nth;
       if (e < T) v[i] = src[G.gidx(e)];
     }
   };
-  request(blockIdx.x * TPB);
+  request(0);
+  if constexpr (SLAB) tw_slab_fill<FENC_ROW_LT>(slab, p.tw + (size_t)rd.mod * N, p.g.logN, blockIdx.x, tid, nth);
 #pragma unroll 1
-  for (int k = 0; k < TPB; k++) {
-    TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, blockIdx.x * TPB + k};
+  for (int k = 0; k < n_it; k++) {
+    TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, SLAB ? blockIdx.x : blockIdx.x * TPB + k};
+    u64 *dst = p.dst + (size_t)(SLAB ? b0 + k : b0) * p.dst_bstride + dst_off;
 #pragma unroll
     for (int i = 0; i < 8; i++) {
       const int e = tid + i * nth;
       if (e < T) sm[swz(e)] = v[i];
     }
+    if (SLAB && k == 0) tw_slab_wait();
     __syncthreads();
-    if (k + 1 < TPB) request(blockIdx.x * TPB + k + 1);
-    tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, mc.q, tid, mc.f64);
+    if (k + 1 < n_it) request(k + 1);
+    if constexpr (SLAB) tile_transform<true, GEO, 2>(sm, row_slab_geo<FENC_ROW_LT>(), 0, p.g.brow, slab, mc.q, tid, mc.f64);
+    else tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, mc.q, tid, mc.f64);
     tile_drain(sm, T, tid, nth, [&](int e, u64 x) { dst[G.gidx(e)] = fullred(x, mc.q, mc.qbar); });
-    if (k + 1 < TPB) __syncthreads();  // every thread has read its results before the next tile overwrites them
+    if (k + 1 < n_it) __syncthreads();  // every thread has read its results before the next tile overwrites them
+  }
+}
+// launch of the forward row pass over (rows x batch), slab form for batches
+static void launch_ntt_rowpass(const KCtx &k, NttRowP r, int n_rows, int n_batch) {
+  const NttGeom &g = k.geom;
+  cudaStream_t st = (cudaStream_t)k.stream;
+  r.n_batch = n_batch, r.bpb = FENC_SLAB_BPB;
+  if (use_slab(g, n_batch)) {
+    dim3 sgrid(k.N >> g.lt_row, n_rows, (n_batch + FENC_SLAB_BPB - 1) / FENC_SLAB_BPB);
+    ntt_rowpass_kernel<1, true><<<sgrid, nthreads_for(g.lt_row), slab_bytes(g), st>>>(r);
+  } else {
+    dim3 grid2((unsigned)((k.N >> g.lt_row) / (g.logN >= 12 ? FENC_ROW_TPB : 1)), n_rows, n_batch);
+    ROW_GEO(g, (ntt_rowpass_kernel<GEO><<<grid2, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(r)));
   }
 }
 static inline unsigned row_grid_x(const NttGeom &g, int N) { return (unsigned)((N >> g.lt_row) / (g.logN >= 12 ? FENC_ROW_TPB : 1)); }
@@ -455,9 +489,8 @@ int k_ntt(const KCtx &k, const u64 *src, size_t src_bstride, u64 *dst, size_t ds
   COL_GEO(g, (ntt_colpass_kernel<false, GEO><<<grid1, nthreads_for(g.lt_col), sizeof(u64) << g.lt_col, st>>>(a)));
   LAUNCH_CHECK(k);
   NttRowP r{dst, dst_bstride, dst, dst_bstride, rows, k.d_mods, k.d_tw_fwd, g, 1};
-  dim3 grid2(row_grid_x(g, k.N), n_rows, n_batch);
   PROF(k, K_NTT_ROW, 16.0 * k.N * n_rows * n_batch, HALF_N(k) * g.brow * n_rows * n_batch);
-  ROW_GEO(g, (ntt_rowpass_kernel<GEO><<<grid2, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, st>>>(r)));
+  launch_ntt_rowpass(k, r, n_rows, n_batch);
   LAUNCH_CHECK(k);
   return 0;
 }
@@ -467,9 +500,8 @@ int k_ntt_rows_only(const KCtx &k, u64 *buf, size_t bstride, const RowDesc *rows
   if (n_rows == 0 || n_batch == 0) return 0;
   const NttGeom &g = k.geom;
   NttRowP r{buf, bstride, buf, bstride, rows, k.d_mods, k.d_tw_fwd, g, 1};
-  dim3 grid2(row_grid_x(g, k.N), n_rows, n_batch);
   PROF(k, K_NTT_ROW, 16.0 * k.N * n_rows * n_batch, HALF_N(k) * g.brow * n_rows * n_batch);
-  ROW_GEO(g, (ntt_rowpass_kernel<GEO><<<grid2, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(r)));
+  launch_ntt_rowpass(k, r, n_rows, n_batch);
   LAUNCH_CHECK(k);
   return 0;
 }
@@ -671,43 +703,56 @@ struct DivideP {
   const BatchItem *items; const u64 *tmp; size_t tmp_bstride; const u64 *acc; size_t acc_bstride; const ShoupC *mul;
   const RowDesc *rows; const ModConst *mods; const ShoupC *tw; NttGeom g; int from_items;
   const ShoupC *mul2;  // MERGED: out = ((minuend mul2 + addend) - X) mul   (mul2 = P^-1, mul = q_{L-1}^-1)
+  int n_batch, bpb;    // SLAB: batch items per block
 };
-template <int GEO, bool MERGED = false>
+// SLAB (batches of FENC_SLAB_MIN_BATCH items and more): the block stays on ONE tile position of its row and walks over
+// p.bpb batch items, so the row pass's twiddles for that position (16 KB, twice the tile) are copied to shared memory
+// once per block instead of being fetched from L2 by every round of every tile; the next item's tile is prefetched into
+// registers as before.  Otherwise: FENC_ROW_TPB consecutive tiles of one item's row per block.
+template <int GEO, bool MERGED = false, bool SLAB = false>
 __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, 4) ntt_rows_divide_kernel(DivideP p) {
+  static_assert(!SLAB || GEO == 1, "slabs: compile-time row geometry");
   extern __shared__ u64 sm[];
-  const int tid = threadIdx.x, b = blockIdx.z;
+  const int tid = threadIdx.x;
   const RowDesc rd = p.rows[blockIdx.y];
   const int N = 1 << p.g.logN, T = 1 << p.g.lt_row;
   constexpr int TPB = GEO == 1 ? FENC_ROW_TPB : 1;  // tiles per block, the next one prefetched (see ntt_rowpass_kernel)
-  const u64 *src = p.tmp + (size_t)b * p.tmp_bstride + (size_t)rd.src_row * N;
   const int nth = blockDim.x, logN = p.g.logN;
-  const BatchItem it = p.items[b];
-  const u64 *minuend = (p.from_items ? it.sub_in : p.acc + (size_t)b * p.acc_bstride) + (size_t)rd.aux2 * N;
-  const u64 *addend = rd.aux == 0 ? it.add0 : it.add1;
-  if (addend) addend += (size_t)rd.mod * N;
   const ModConst mq = p.mods[rd.mod];
   const u64 q = mq.q;
   const ShoupC mc = p.mul[rd.mod];
   const F64Mod fm = f64mod(q, mq.f64);
-  u64 *dst = it.out + (size_t)rd.dst_row * N;
+  const int b0 = SLAB ? blockIdx.z * p.bpb : blockIdx.z;
+  const int n_it = SLAB ? min(p.bpb, p.n_batch - b0) : TPB;
+  ShoupC *slab = reinterpret_cast<ShoupC *>(sm + T);
   u64 v[8];
-  auto request = [&](u32 tile) {
-    TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, tile};
+  auto request = [&](int k) {  // iteration k's tile of the temp
+    TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, SLAB ? blockIdx.x : blockIdx.x * TPB + k};
+    const u64 *src = p.tmp + (size_t)(SLAB ? b0 + k : b0) * p.tmp_bstride + (size_t)rd.src_row * N;
 #pragma unroll
     for (int i = 0; i < 8; i++) {
       const int e = tid + i * nth;
       if (e < T) v[i] = src[G.gidx(e)];
     }
   };
-  request(blockIdx.x * TPB);
+  request(0);
+  if constexpr (SLAB) tw_slab_fill<FENC_ROW_LT>(slab, p.tw + (size_t)rd.mod * N, logN, blockIdx.x, tid, nth);
+  BatchItem it = p.items[b0];
 #pragma unroll 1
-  for (int k = 0; k < TPB; k++) {
-    TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, blockIdx.x * TPB + k};
+  for (int k = 0; k < n_it; k++) {
+    const int b = SLAB ? b0 + k : b0;
+    TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, SLAB ? blockIdx.x : blockIdx.x * TPB + k};
+    const u64 *minuend = (p.from_items ? it.sub_in : p.acc + (size_t)b * p.acc_bstride) + (size_t)rd.aux2 * N;
+    const u64 *addend = rd.aux == 0 ? it.add0 : it.add1;
+    if (addend) addend += (size_t)rd.mod * N;
+    u64 *dst = it.out + (size_t)rd.dst_row * N;
+    const u32 gal = it.g;
 #pragma unroll
     for (int i = 0; i < 8; i++) {
       const int e = tid + i * nth;
       if (e < T) sm[swz(e)] = v[i];
     }
+    if (SLAB && k == 0) tw_slab_wait();
     __syncthreads();
     // epilogue operands of this tile and the words of the next tile are fetched BEFORE the transform: their latency hides behind it
     u64 mi[8], ad[8];
@@ -715,10 +760,14 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, 4) ntt_rows_divide_kerne
     for (int i = 0; i < 8; i++) {
       const u32 j = G.gidx((tid + i * nth) & (T - 1));
       mi[i] = __ldg(minuend + j);
-      ad[i] = addend ? __ldg(addend + galois_src(j, it.g, logN)) : 0;
+      ad[i] = addend ? __ldg(addend + galois_src(j, gal, logN)) : 0;
     }
-    if (k + 1 < TPB) request(blockIdx.x * TPB + k + 1);
-    tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid, mq.f64);
+    if (k + 1 < n_it) {
+      request(k + 1);
+      if (SLAB) it = p.items[b + 1];
+    }
+    if constexpr (SLAB) tile_transform<true, GEO, 2>(sm, row_slab_geo<FENC_ROW_LT>(), 0, p.g.brow, slab, q, tid, mq.f64);
+    else tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid, mq.f64);
 #pragma unroll
     for (int i = 0; i < 8; i++) {
       const int e = tid + i * nth;
@@ -738,7 +787,7 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, 4) ntt_rows_divide_kerne
         dst[G.gidx(e)] = r;
       }
     }
-    if (k + 1 < TPB) __syncthreads();
+    if (k + 1 < n_it) __syncthreads();
   }
 }
 
@@ -747,10 +796,15 @@ int k_ntt_rows_divide(const KCtx &k, const BatchItem *items, const u64 *tmp, siz
                       int n_batch, const ShoupC *merged_mul2) {
   if (n_rows == 0 || n_batch == 0) return 0;
   const NttGeom &g = k.geom;
-  DivideP p{items, tmp, tmp_bstride, acc, acc_bstride, mul, rows, k.d_mods, k.d_tw_fwd, g, minuend_from_items ? 1 : 0, merged_mul2};
+  DivideP p{items, tmp, tmp_bstride, acc, acc_bstride, mul, rows, k.d_mods, k.d_tw_fwd, g, minuend_from_items ? 1 : 0, merged_mul2,
+            n_batch, FENC_SLAB_BPB};
   dim3 grid(row_grid_x(g, k.N), n_rows, n_batch);
   PROF(k, K_DIVIDE, 8.0 * k.N * (3.5 * n_rows) * n_batch, HALF_N(k) * g.brow * n_rows * n_batch);  // temp + minuend + output, addend on half the rows
-  if (merged_mul2)
+  if (use_slab(g, n_batch)) {
+    dim3 sgrid(k.N >> g.lt_row, n_rows, (n_batch + FENC_SLAB_BPB - 1) / FENC_SLAB_BPB);
+    if (merged_mul2) ntt_rows_divide_kernel<1, true, true><<<sgrid, nthreads_for(g.lt_row), slab_bytes(g), (cudaStream_t)k.stream>>>(p);
+    else ntt_rows_divide_kernel<1, false, true><<<sgrid, nthreads_for(g.lt_row), slab_bytes(g), (cudaStream_t)k.stream>>>(p);
+  } else if (merged_mul2)
     ROW_GEO(g, (ntt_rows_divide_kernel<GEO, true><<<grid, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p)));
   else
     ROW_GEO(g, (ntt_rows_divide_kernel<GEO><<<grid, nthreads_for(g.lt_row), sizeof(u64) << g.lt_row, (cudaStream_t)k.stream>>>(p)));

@@ -1,4 +1,5 @@
 // fenc_ops.cu -- keys, plaintexts, encryption / decryption and the ciphertext primitives of the C ABI.
+#include <cstdlib>
 #include <algorithm>
 #include <cmath>
 #include <cstring>
@@ -277,26 +278,58 @@ extern "C" fenc_status fenc_ct_export(fenc_ctx *ctx, const fenc_ct *ct, uint64_t
   CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
   return FENC_OK;
 }
-// Export without the host synchronisation: inverse transform and device->host copy are enqueued on the context's stream
-// and an event is recorded behind them; fenc_export_wait blocks on that event only, so a caller can enqueue the next
-// request's work before it collects this one's result.
+// Export without the host synchronisation.  The inverse transform runs on the context's stream (so it reads the
+// ciphertext in stream order, whatever the caller does with the handle afterwards) into a buffer of its own; the
+// device -> host copy runs on a second stream, d2h_stream, behind an event: on the context's stream a copy of a request's
+// results (config 4: 13.4 GB per batch group, a third of a second on the bus) would hold back every kernel of the next
+// request enqueued behind it -- measured before this split: a period of 1007 ms per request for 630 ms of kernels.  The
+// buffer returns to the pool when its copy has landed (export_drain, polled by the next export and by every
+// synchronising call), so a request's exports hold one copy of its results on the device while they are in flight.
+fenc_status export_drain(fenc_ctx *ctx, bool block) {
+  while (!ctx->exports.empty()) {
+    fenc_ctx::PendingExport &e = ctx->exports.front();
+    if (block) CUDA_OK(ctx, cudaEventSynchronize(e.landed));
+    else {
+      cudaError_t q = cudaEventQuery(e.landed);
+      if (q == cudaErrorNotReady) break;
+      CUDA_OK(ctx, q);
+    }
+    dfree(ctx, e.buf);
+    ctx->export_events.push_back(e.landed);
+    ctx->exports.pop_front();
+  }
+  return FENC_OK;
+}
 extern "C" fenc_status fenc_ct_export_async(fenc_ctx *ctx, const fenc_ct *ct, uint64_t *limbs) {
-  Scope sc(ctx);
   if (!ctx || !ct || !limbs) return FENC_ERR_INVALID_ARG;
+  fenc_status st = export_drain(ctx, false);
+  if (st != FENC_OK) return st;
   LevelPlan *P = get_plan(ctx, ct->L);
   const size_t n = (size_t)2 * ct->L * ctx->N;
-  u64 *tmp = sc.alloc<u64>(n);  // returns to the pool behind the copy (same stream)
-  if (!P || !tmp) return fail(ctx, FENC_ERR_OOM, "export");
-  if (!ctx->export_ev) CUDA_OK(ctx, cudaEventCreateWithFlags(&ctx->export_ev, cudaEventDisableTiming));
-  CUDA_OK(ctx, k_intt(ctx->k, nullptr, ct->d, 0, false, tmp, 0, P->d_rows_ct, 2 * ct->L, P->d_scale_ct, 1));
-  CUDA_OK(ctx, cudaMemcpyAsync(limbs, tmp, n * 8, cudaMemcpyDeviceToHost, ctx->stream));
-  CUDA_OK(ctx, cudaEventRecord(ctx->export_ev, ctx->stream));
+  if (!ctx->d2h_stream) CUDA_OK(ctx, cudaStreamCreateWithFlags(&ctx->d2h_stream, cudaStreamNonBlocking));
+  if (!ctx->export_ready) CUDA_OK(ctx, cudaEventCreateWithFlags(&ctx->export_ready, cudaEventDisableTiming));
+  cudaEvent_t landed = nullptr;
+  if (!ctx->export_events.empty()) landed = ctx->export_events.back(), ctx->export_events.pop_back();
+  else CUDA_OK(ctx, cudaEventCreateWithFlags(&landed, cudaEventDisableTiming));
+  u64 *tmp = (u64 *)dalloc(ctx, n * 8);
+  if (!P || !tmp) {
+    ctx->export_events.push_back(landed);
+    dfree(ctx, tmp);
+    return fail(ctx, FENC_ERR_OOM, "export");
+  }
+  ctx->exports.push_back({tmp, landed});  // from here on the buffer is released by export_drain, also after an error
+  cudaError_t e = (cudaError_t)k_intt(ctx->k, nullptr, ct->d, 0, false, tmp, 0, P->d_rows_ct, 2 * ct->L, P->d_scale_ct, 1);
+  if (e == cudaSuccess) e = cudaEventRecord(ctx->export_ready, ctx->stream);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->d2h_stream, ctx->export_ready, 0);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(limbs, tmp, n * 8, cudaMemcpyDeviceToHost, ctx->d2h_stream);
+  cudaError_t e2 = cudaEventRecord(landed, ctx->d2h_stream);  // recorded in every case: export_drain waits on it
+  CUDA_OK(ctx, e);
+  CUDA_OK(ctx, e2);
   return FENC_OK;
 }
 extern "C" fenc_status fenc_export_wait(fenc_ctx *ctx) {
   if (!ctx) return FENC_ERR_INVALID_ARG;
-  if (ctx->export_ev) CUDA_OK(ctx, cudaEventSynchronize(ctx->export_ev));
-  return FENC_OK;
+  return export_drain(ctx, true);
 }
 extern "C" fenc_status fenc_ct_import(fenc_ctx *ctx, const uint64_t *limbs, uint32_t L, double scale, fenc_ct **out) {
   Scope sc(ctx);
@@ -313,7 +346,7 @@ extern "C" fenc_status fenc_ct_import(fenc_ctx *ctx, const uint64_t *limbs, uint
   return FENC_OK;
 }
 // The same import without a host synchronisation and with the copy off the compute stream: the limbs go to a slot of a
-// staging ring on the context's copy stream (overlapping whatever the compute stream is running), the compute stream
+// staging queue on the context's copy stream (overlapping whatever the compute stream is running), the compute stream
 // waits for that copy only, transforms staging -> ciphertext, and releases the slot.  A slot is never touched by any
 // other kernel, so the copy has to wait for nothing but the transform that last read the slot.
 extern "C" fenc_status fenc_ct_import_async(fenc_ctx *ctx, const uint64_t *limbs, uint32_t L, double scale, fenc_ct **out) {
@@ -324,11 +357,19 @@ extern "C" fenc_status fenc_ct_import_async(fenc_ctx *ctx, const uint64_t *limbs
   if (!P || !ct) return fail(ctx, FENC_ERR_OOM, "import");
   const size_t bytes = (size_t)2 * L * ctx->N * 8;
   if (!ctx->copy_stream) CUDA_OK(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
-  if (ctx->stage.empty()) ctx->stage.resize(FENC_STAGE_SLOTS);
-  size_t n_slots = FENC_STAGE_BYTES / bytes;
-  n_slots = n_slots < 2 ? 2 : (n_slots > FENC_STAGE_SLOTS ? FENC_STAGE_SLOTS : n_slots);
-  StageSlot &sl = ctx->stage[ctx->stage_next++ % n_slots];
-  if (!sl.copied) {
+  if (!ctx->stage_max) {
+    const char *mb = getenv("FENC_STAGE_MAX_MB");
+    ctx->stage_max = mb && atoll(mb) > 0 ? (size_t)atoll(mb) << 20 : FENC_STAGE_BYTES_MAX;
+  }
+  // the oldest slot if its transform has run (or the queue may not grow any further: then the copy waits for it), else a new one
+  StageSlot sl;
+  bool reuse = ctx->stage.size() >= 2 && (cudaEventQuery(ctx->stage.front().consumed) == cudaSuccess || ctx->stage_bytes + bytes > ctx->stage_max);
+  (void)cudaGetLastError();  // cudaErrorNotReady is not an error
+  if (reuse) {
+    sl = ctx->stage.front();
+    ctx->stage.pop_front();
+    ctx->stage_bytes -= sl.bytes;
+  } else {
     CUDA_OK(ctx, cudaEventCreateWithFlags(&sl.copied, cudaEventDisableTiming));
     CUDA_OK(ctx, cudaEventCreateWithFlags(&sl.consumed, cudaEventDisableTiming));
   }
@@ -338,10 +379,15 @@ extern "C" fenc_status fenc_ct_import_async(fenc_ctx *ctx, const uint64_t *limbs
     dfree(ctx, sl.d);
     sl.bytes = 0;
     sl.d = (u64 *)dalloc(ctx, bytes);
-    if (!sl.d) return fail(ctx, FENC_ERR_OOM, "import staging (%zu bytes)", bytes);
-    sl.bytes = bytes;
-    CUDA_OK(ctx, cudaEventRecord(sl.consumed, ctx->stream));
+    if (sl.d) sl.bytes = bytes;
+    if (sl.d) CUDA_OK(ctx, cudaEventRecord(sl.consumed, ctx->stream));
   }
+  if (!sl.d) {
+    cudaEventDestroy(sl.copied), cudaEventDestroy(sl.consumed);
+    return fail(ctx, FENC_ERR_OOM, "import staging (%zu bytes)", bytes);
+  }
+  ctx->stage.push_back(sl);
+  ctx->stage_bytes += sl.bytes;
   CUDA_OK(ctx, cudaStreamWaitEvent(ctx->copy_stream, sl.consumed, 0));
   CUDA_OK(ctx, cudaMemcpyAsync(sl.d, limbs, bytes, cudaMemcpyHostToDevice, ctx->copy_stream));
   CUDA_OK(ctx, cudaEventRecord(sl.copied, ctx->copy_stream));
