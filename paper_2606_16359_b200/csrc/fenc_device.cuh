@@ -311,6 +311,11 @@ DEVI void tile_transform_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, 
 // 2^(LT-2) + 2 t + i sits at (2 + i) 2^(LT-3) + t and entry 2^(LT-1) + 4 t + i at (4 + i) 2^(LT-3) + t.
 // 2^LT entries of 16 bytes (entry 0 unused), copied with cp.async: the caller commits, waits and synchronises before the
 // first transform.
+DEVI void cp_async8(u64 *dst_smem, const u64 *src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((u32)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
+}
+DEVI void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+DEVI void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 DEVI void cp_async16(void *dst_smem, const void *src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
 }

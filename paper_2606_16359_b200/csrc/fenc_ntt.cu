@@ -165,17 +165,31 @@ struct ConvColP {
   u64 *tmp; size_t tmp_bstride; const ModConst *mods; const ShoupC *tw_fwd; const ShoupC *tw_inv; int logN, brow, max_terms;
   const ShoupC *mulc;  // MERGED: P^-1 mod q_t
   const ShoupC *bc_f64;  // {(double) c, (double)(c / t)} per entry of bc, used when source and target moduli are fp64 ones
+  int smem_tiles;        // tiles ahead of the twiddle buffers and the target descriptors in shared memory
 };
+// What a target row's iteration needs, staged in shared memory when the block starts: from global memory the chain
+// rows[] -> mods[] -> (constants, twiddles) put two dependent L2 latencies in front of every target (ncu on the config-4
+// step: 9 % of the kernel's stall samples on the two instructions that first use them).
+struct TgtDesc { int mod, dst_row, aux2, pad; u64 q, qinv_neg, qbar, f64; };
+#define CONV_DESC_CAP 56            // targets per group staged; later ones are read from global memory
+#define CONV_BC_CAP 32              // base-conversion constants of one target staged (groups of more sources read them from global memory)
+#define CONV_TW_WORDS (512 + 4 * CONV_BC_CAP)  // u64 words of one group's buffer: tw[0 .. 256) of the target's modulus, then two buffers of constants
+DEVI TgtDesc tgt_desc_load(const ConvColP &p, int row) {
+  const RowDesc rd = p.rows[row];
+  const ModConst mc = p.mods[rd.mod];
+  return TgtDesc{rd.mod, rd.dst_row, rd.aux2, 0, mc.q, mc.qinv_neg, mc.qbar, mc.f64};
+}
 // sum over the first n source tiles of Y_s[e] * bc[s] for this thread's eight elements, Montgomery-reduced: canonical.
 // YDBL: the tiles hold the values as doubles (see conv_dot_f64); they are exact integers below 2^50.
-template <int T, int NTH>
+// CS: the constants were staged in shared memory (stride 2 words: they share the slots of the fp64 pairs)
+template <int T, int NTH, bool CS = false>
 DEVI void conv_dot(const u64 *smem, int n, const u64 *bc, const ModConst &mc, int max_terms, int tid, u64 (&out)[8], bool ydbl) {
   u64 lo[8], hi[8], r[8];
 #pragma unroll
   for (int i = 0; i < 8; i++) lo[i] = hi[i] = r[i] = 0;
   int lazy = 0;
   for (int s = 0; s < n; s++) {
-    const u64 c = __ldg(bc + s);
+    const u64 c = CS ? bc[2 * s] : __ldg(bc + s);
     const u64 *Y = smem + (size_t)s * T;
 #pragma unroll
     for (int i = 0; i < 8; i++) {
@@ -197,14 +211,14 @@ DEVI void conv_dot(const u64 *smem, int n, const u64 *bc, const ModConst &mc, in
 // (at most t/2 + 1) is exact, and v - rint(v / t) t + t in (0, 2t) is what the forward fp64 butterflies ask of their input.
 // Measured (profiles/r02_convert_cols.md): the 128-bit integer form of this sum was 38 % IMAD + 18 % IADD3 of the kernel's
 // instructions with the fp64 pipe 16 % busy.
-template <int T, int NTH>
+template <int T, int NTH, bool CS = false>
 DEVI void conv_dot_f64(const u64 *smem, int n, const ShoupC *bc, const F64Mod &fm, int lazy_max, int tid, u64 (&out)[8]) {
   double acc[8];
 #pragma unroll
   for (int i = 0; i < 8; i++) acc[i] = 0.0;
   int lazy = 0;
   for (int s = 0; s < n; s++) {
-    const ulonglong2 cc = __ldg(reinterpret_cast<const ulonglong2 *>(bc + s));
+    const ulonglong2 cc = CS ? *reinterpret_cast<const ulonglong2 *>(bc + s) : __ldg(reinterpret_cast<const ulonglong2 *>(bc + s));
     const double c = __longlong_as_double((long long)cc.x), cq = __longlong_as_double((long long)cc.y);
     const u64 *Y = smem + (size_t)s * T;
 #pragma unroll
@@ -237,9 +251,22 @@ __global__ void __launch_bounds__(128 * NG, NG == 1 ? 5 : (NG == 2 ? 2 : 1)) con
   const int N = 1 << p.logN;
   TileGeo G{LT, LC, p.brow, p.logN, blockIdx.x};
   u64 *W = smem + (size_t)(cg.n_src + grp) * T;  // work tiles after the source tiles
+  ShoupC *twb = reinterpret_cast<ShoupC *>(smem + (size_t)p.smem_tiles * T + (size_t)grp * CONV_TW_WORDS);  // this group's forward twiddles
+  TgtDesc *sdesc = reinterpret_cast<TgtDesc *>(smem + (size_t)p.smem_tiles * T + (size_t)NG * CONV_TW_WORDS);
+  for (int t = threadIdx.x; t < cg.n_tgt && t < CONV_DESC_CAP; t += NTH * NG) sdesc[t] = tgt_desc_load(p, cg.tgt_start + t);
   u64 *ybase = p.y + (size_t)b * p.y_bstride;
   const int n_conv = MERGED ? cg.n_src - 1 : cg.n_src;  // tiles entering the base conversion
   const bool ydbl = !MERGED && p.bc_f64 && (cg.pad[0] & 2);  // the converted tiles are kept as doubles (conv_dot_f64)
+  const bool cstage = n_conv <= CONV_BC_CAP;
+  // target t's constants -> a buffer of this group (cp.async; the caller commits): fp64 pairs, or the integers at stride 2
+  auto stage_consts = [&](ShoupC *dst, int t, bool staged_desc) {
+    if (!cstage || tid >= n_conv) return;
+    const TgtDesc d = staged_desc && t < CONV_DESC_CAP ? sdesc[t] : tgt_desc_load(p, cg.tgt_start + t);
+    if (ydbl && d.f64) cp_async16(dst + tid, p.bc_f64 + d.aux2 + tid);
+    else cp_async8(reinterpret_cast<u64 *>(dst + tid), p.bc + d.aux2 + tid);
+  };
+  if (grp < cg.n_tgt) stage_consts(twb + 256, grp, false);  // the descriptors in shared memory are not published yet
+  cp_async_commit();
   // ---- sources: fill, inverse column stages, scale -> canonical coefficient tiles in shared memory
   for (int s = grp; s < cg.n_src; s += NG) {
     const u64 *src = ybase + (size_t)(cg.src_row + s) * N;
@@ -259,6 +286,7 @@ __global__ void __launch_bounds__(128 * NG, NG == 1 ? 5 : (NG == 2 ? 2 : 1)) con
       Y[e] = ydbl ? (u64)__double_as_longlong(u2d52(y)) : y;
     }
   }
+  cp_async_wait_all();
   __syncthreads();
   u64 outl[8];
   if (MERGED) {
@@ -272,11 +300,27 @@ __global__ void __launch_bounds__(128 * NG, NG == 1 ? 5 : (NG == 2 ? 2 : 1)) con
     for (int i = 0; i < 8; i++) outl[i] = submod(Z[swz(tid + i * NTH)], shoup_mul(v[i], pl.c, pl.cs, ml.q), ml.q);
   }
   // ---- targets
-  for (int t = grp; t < cg.n_tgt; t += NG) {
-    const RowDesc rd = p.rows[cg.tgt_start + t];
-    const ModConst mc = p.mods[rd.mod];
+  int it = 0;
+  for (int t = grp; t < cg.n_tgt; t += NG, it++) {
+    const TgtDesc rd = t < CONV_DESC_CAP ? sdesc[t] : tgt_desc_load(p, cg.tgt_start + t);
+    const ModConst mc{rd.q, rd.qinv_neg, 0, 0, rd.qbar, rd.f64, {0, 0}};
+    // the 255 twiddles of this target's forward column stages and the NEXT target's base-conversion constants arrive in
+    // shared memory while the base conversion runs (read per source term from global memory, the first use of a constant
+    // was 9 % of the ModUp launches' stall samples: an L2 latency per term with nothing to overlap it)
+    const bool f64dot = ydbl && mc.f64;
+    ShoupC *cb = twb + 256 + (it & 1) * CONV_BC_CAP;
+    {
+      const ShoupC *twg = p.tw_fwd + (size_t)rd.mod * N;
+      for (int i = tid; i < 256; i += NTH) cp_async16(twb + i, twg + i);
+      if (t + NG < cg.n_tgt) stage_consts(twb + 256 + ((it + 1) & 1) * CONV_BC_CAP, t + NG, true);
+      cp_async_commit();
+    }
     u64 v[8];
-    if (ydbl && mc.f64) conv_dot_f64<T, NTH>(smem, n_conv, p.bc_f64 + rd.aux2, f64mod(mc.q, mc.f64), mc.q < (1ull << FENC_F64_MAX_BITS) ? 255 : 7, tid, v);
+    if (f64dot) {
+      const int lazy_max = mc.q < (1ull << FENC_F64_MAX_BITS) ? 255 : 7;
+      if (cstage) conv_dot_f64<T, NTH, true>(smem, n_conv, cb, f64mod(mc.q, mc.f64), lazy_max, tid, v);
+      else conv_dot_f64<T, NTH>(smem, n_conv, p.bc_f64 + rd.aux2, f64mod(mc.q, mc.f64), lazy_max, tid, v);
+    } else if (cstage) conv_dot<T, NTH, true>(smem, n_conv, reinterpret_cast<const u64 *>(cb), mc, p.max_terms, tid, v, ydbl);
     else conv_dot<T, NTH>(smem, n_conv, p.bc + rd.aux2, mc, p.max_terms, tid, v, ydbl);
     if (MERGED) {
       const ShoupC pt = p.mulc[rd.mod];
@@ -285,8 +329,9 @@ __global__ void __launch_bounds__(128 * NG, NG == 1 ? 5 : (NG == 2 ? 2 : 1)) con
     }
 #pragma unroll
     for (int i = 0; i < 8; i++) W[swz(tid + i * NTH)] = v[i];
+    cp_async_wait_all();
     tile_sync<GRP>(bar);
-    tile_transform_ct<true, LT, LC, BCOL, GRP>(W, G, p.tw_fwd + (size_t)rd.mod * N, mc.q, tid, mc.f64, bar);
+    tile_transform_ct<true, LT, LC, BCOL, GRP, 1>(W, G, twb, mc.q, tid, mc.f64, bar);
     u64 *dst = p.tmp + (size_t)b * p.tmp_bstride + (size_t)rd.dst_row * N;
     tile_drain(W, T, tid, NTH, [&](int e, u64 v) { dst[G.gidx(e)] = v; });  // lazy, below 33q
     tile_sync<GRP>(bar);
@@ -295,8 +340,11 @@ __global__ void __launch_bounds__(128 * NG, NG == 1 ? 5 : (NG == 2 ? 2 : 1)) con
 
 // thread groups per block of the fused column kernel for digit groups of n_src limbs
 static inline int convert_groups(int n_src, bool merged) { return (merged || n_src < 6) ? 1 : (n_src < 8 ? 2 : 4); }
+static inline size_t convert_smem(int n_src, int ng) {  // source + work tiles, twiddle buffers, target descriptors
+  return (size_t)(n_src + ng) * 8192 + (size_t)ng * CONV_TW_WORDS * 8 + (size_t)CONV_DESC_CAP * sizeof(TgtDesc);
+}
 bool convert_cols_fits(int logN, int n_src, bool merged) {
-  return logN >= 12 && (size_t)(n_src + convert_groups(n_src, merged)) * 8192 <= 227 * 1024;
+  return logN >= 12 && convert_smem(n_src, convert_groups(n_src, merged)) <= 227 * 1024;
 }
 
 int k_convert_cols(const KCtx &k, u64 *y, size_t y_bstride, const ConvGroup *groups, int n_groups, int n_src_max,
@@ -306,9 +354,9 @@ int k_convert_cols(const KCtx &k, u64 *y, size_t y_bstride, const ConvGroup *gro
   const NttGeom &g = k.geom;
   if (!convert_cols_fits(g.logN, n_src_max, merged_pinv != nullptr)) return -2;
   const int ng = convert_groups(n_src_max, merged_pinv != nullptr);
-  const size_t smem = (size_t)(n_src_max + ng) * 1024 * sizeof(u64);
+  const size_t smem = convert_smem(n_src_max, ng);
   ConvColP p{y, y_bstride, groups, scale, bc, rows, tmp, tmp_bstride, k.d_mods, k.d_tw_fwd, k.d_tw_inv, g.logN, g.brow, max_terms,
-             merged_pinv, bc_f64};
+             merged_pinv, bc_f64, n_src_max + ng};
   dim3 grid(k.N >> 10, n_groups, n_batch);
   // algorithmic bytes: every target row written once (+ the sources, counted by the caller's row pass); butterflies: the
   // forward column stages of every target AND the inverse column stages of every source row (y holds y_bstride / N of them
@@ -531,11 +579,6 @@ struct KeyMacP {
 // 3 blocks of 128 threads per SM: 168 registers hold the 32 128-bit accumulators and the fp64 butterflies without
 // spilling (4 blocks at 128 registers spill 160 bytes and run 10 % slower)
 #define KEYMAC_BLOCKS 3
-DEVI void cp_async8(u64 *dst_smem, const u64 *src) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((u32)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
-}
-DEVI void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-DEVI void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 template <int EPT, int GEO>  // elements per thread
 __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? KEYMAC_BLOCKS : 2) ntt_rows_keymac_kernel(KeyMacP p) {
   extern __shared__ u64 sm_all[];  // two tiles: the next digit's words arrive (cp.async) while this one is transformed
