@@ -263,21 +263,32 @@ __global__ void __launch_bounds__(256, (G >= 8 || MODE == 3) ? 2 : 3) smac_kerne
   constexpr bool F64 = MODE == 1;
   constexpr bool SPLIT = MODE >= 2;
   constexpr int NP = MODE == 3 ? 3 : 2, PB = MODE == 3 ? 17 : 25;  // pieces and bits per piece (split modes)
+  // TS (groups of 4 and more outputs): the running totals over the mask segments live in shared memory (dynamic, one slot
+  // per thread, output and component), touched at segment ends only.  In registers they took 4 G of the 128 a thread may
+  // have beside the 4 G (6 G) accumulators, and the compiler rebuilt every loop invariant (thread index, limb offset,
+  // ring addresses) in every term: 106 instructions per term around 32 DFMA (ncu, profiles/r02_smac_loop_before.md).
+  constexpr bool TS = G >= 4;
+  extern __shared__ u64 s_tot[];  // TS: [G][2][blockDim.x]
   __shared__ const u64 *s_ct[SMAC_TILE];
-  __shared__ ulonglong2 s_k[G][SMAC_TILE];
+  __shared__ ulonglong2 s_k[SPLIT ? 1 : G][SPLIT ? 1 : SMAC_TILE];
+  __shared__ __align__(16) double s_kd[SPLIT ? SMAC_TILE : 1][SPLIT ? G : 1];  // split modes: the G multipliers of a term side by side
   __shared__ u64 s_ring[G >= 4 ? SMAC_RING : 1][2][G >= 4 ? 256 : 1];
-  const size_t LN = (size_t)p.L << p.logN;
-  const size_t idx = (size_t)blockIdx.y * blockDim.x + threadIdx.x;  // blockDim divides N: idx < L N, one limb per block
-  const int limb = (int)(((size_t)blockIdx.y * blockDim.x) >> p.logN);
+  const u32 LN = (u32)p.L << p.logN;                           // L N < 2^32 (at most 2^7 limbs of 2^17 coefficients)
+  const u32 idx = blockIdx.y * blockDim.x + threadIdx.x;       // blockDim divides N: idx < L N, one limb per block
+  const int limb = (int)((blockIdx.y * blockDim.x) >> p.logN);
   const SmacGroup g = p.groups[blockIdx.x];
   const ModConst mc = p.mods[limb];
-  const F64Mod fm = f64mod(mc.q, mc.f64);
+  F64Mod fm = f64mod(mc.q, mc.f64);
+  if (G >= 4) {  // (double) q is an integer-to-double conversion the compiler otherwise repeats per term
+    asm volatile("mov.f64 %0, %0;" : "+d"(fm.q));
+    asm volatile("mov.f64 %0, %0;" : "+d"(fm.qinv));
+  }
   double acc[F64 ? G : 1][2];
   double sp[SPLIT ? G : 1][2][NP];
-  u64 lo[MODE == 0 ? G : 1][2], hi[MODE == 0 ? G : 1][2], tot[G][2];
+  u64 lo[MODE == 0 ? G : 1][2], hi[MODE == 0 ? G : 1][2], tot[TS ? 1 : G][2];
 #pragma unroll
   for (int i = 0; i < G; i++) {
-    tot[i][0] = tot[i][1] = 0;
+    if (!TS) tot[i][0] = tot[i][1] = 0;
     if (F64) acc[i][0] = acc[i][1] = 0.0;
     if (MODE == 0) lo[i][0] = lo[i][1] = hi[i][0] = hi[i][1] = 0;
     if (SPLIT) {
@@ -286,6 +297,16 @@ __global__ void __launch_bounds__(256, (G >= 8 || MODE == 3) ? 2 : 3) smac_kerne
 #pragma unroll
         for (int q2 = 0; q2 < NP; q2++) sp[i][c][q2] = 0.0;
     }
+  }
+  u32 a_ring = (u32)__cvta_generic_to_shared(&s_ring[0][0][G >= 4 ? threadIdx.x : 0]);
+  u32 a_ct = (u32)__cvta_generic_to_shared(&s_ct[0]);
+  u32 idx_r = idx, ln_r = LN + idx, a_kd = (u32)__cvta_generic_to_shared(&s_kd[0][0]);
+  if (G >= 4) {
+    asm volatile("mov.u32 %0, %0;" : "+r"(a_kd));  // opaque copies: values the compiler must keep in registers instead of rebuilding them from special registers per term
+    asm volatile("mov.u32 %0, %0;" : "+r"(a_ring));
+    asm volatile("mov.u32 %0, %0;" : "+r"(a_ct));
+    asm volatile("mov.u32 %0, %0;" : "+r"(idx_r));
+    asm volatile("mov.u32 %0, %0;" : "+r"(ln_r));
   }
   int seg = 0, cur_end = p.seg_end[g.seg_start], lazy = 0;
   for (int t0 = 0; t0 < g.n_terms; t0 += SMAC_TILE) {
@@ -297,7 +318,9 @@ __global__ void __launch_bounds__(256, (G >= 8 || MODE == 3) ? 2 : 3) smac_kerne
       else {
         const int o = i - 1 < g.n_out ? i - 1 : 0;  // unused lanes of a short group repeat output 0 (never stored)
         const int w = p.kidx[g.k_start + o * g.n_terms + t0 + t];
-        s_k[i - 1][t] = __ldg(reinterpret_cast<const ulonglong2 *>(p.kpair) + (size_t)w * p.L + limb);
+        const ulonglong2 kk = __ldg(reinterpret_cast<const ulonglong2 *>(p.kpair) + (size_t)w * p.L + limb);
+        if (SPLIT) s_kd[t][i - 1] = __longlong_as_double((long long)kk.x);
+        else s_k[i - 1][t] = kk;
       }
     }
     __syncthreads();
@@ -308,11 +331,15 @@ __global__ void __launch_bounds__(256, (G >= 8 || MODE == 3) ? 2 : 3) smac_kerne
     // round trip, so with one term ahead the loop ran at the memory latency (measured: 2 TB/s of operand traffic, a
     // quarter of what the FP64 pipe would allow).  The ring lives in shared memory (cp.async, 8 bytes per copy): each
     // thread owns its slots, so no barrier is needed and no register is spent on the depth.
+    // (shared-memory addresses as 32-bit window offsets computed once: left to the compiler, the generic-to-shared
+    // conversions of the ring slots were redone in every term)
     auto ring_issue = [&](int t) {
       if (t < nt) {
-        const u64 *c = s_ct[t];
-        smac_cp_async8(&s_ring[t % SMAC_RING][0][threadIdx.x], c + idx);
-        smac_cp_async8(&s_ring[t % SMAC_RING][1][threadIdx.x], c + LN + idx);
+        u64 c;
+        asm volatile("ld.shared.u64 %0, [%1];" : "=l"(c) : "r"(a_ct + (u32)t * 8u));
+        const u32 slot = a_ring + ((u32)t % SMAC_RING) * (u32)(2 * 256 * sizeof(u64));
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(slot), "l"(c + (u64)idx_r * 8u) : "memory");
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(slot + (u32)(256 * sizeof(u64))), "l"(c + (u64)ln_r * 8u) : "memory");
       }
       asm volatile("cp.async.commit_group;" ::: "memory");  // a group per term, empty past the end: the wait below counts groups
     };
@@ -326,7 +353,9 @@ __global__ void __launch_bounds__(256, (G >= 8 || MODE == 3) ? 2 : 3) smac_kerne
       if (G >= 4) {
         ring_issue(t + SMAC_RING - 1);  // overwrites the slot of term t - 1, already consumed by this thread
         asm volatile("cp.async.wait_group %0;" ::"n"(SMAC_RING - 1) : "memory");
-        x0 = s_ring[t % SMAC_RING][0][threadIdx.x], x1 = s_ring[t % SMAC_RING][1][threadIdx.x];
+        const u32 slot = a_ring + ((u32)t % SMAC_RING) * (u32)(2 * 256 * sizeof(u64));
+        asm volatile("ld.shared.u64 %0, [%1];" : "=l"(x0) : "r"(slot) : "memory");
+        asm volatile("ld.shared.u64 %0, [%1];" : "=l"(x1) : "r"(slot + (u32)(256 * sizeof(u64))) : "memory");
       } else {
         const u64 *c = s_ct[t];
         x0 = __ldg(c + idx), x1 = __ldg(c + LN + idx);
@@ -341,9 +370,18 @@ __global__ void __launch_bounds__(256, (G >= 8 || MODE == 3) ? 2 : 3) smac_kerne
           if (NP == 2) xp[c][1] = u2d((u32)(x >> PB));
           else xp[c][1] = u2d((u32)(x >> PB) & pm), xp[c][NP - 1] = u2d((u32)(x >> (2 * PB)));
         }
+        double kds[G];
+        if (G >= 4) {
+#pragma unroll
+          for (int i = 0; i < G; i += 2)
+            asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(kds[i]), "=d"(kds[i + 1]) : "r"(a_kd + (u32)(t * G + i) * 8u) : "memory");
+        } else {
+#pragma unroll
+          for (int i = 0; i < G; i++) kds[i] = s_kd[t][i];
+        }
 #pragma unroll
         for (int i = 0; i < G; i++) {
-          const double kd = __longlong_as_double((long long)s_k[i][t].x);
+          const double kd = kds[i];
 #pragma unroll
           for (int c = 0; c < 2; c++)
 #pragma unroll
@@ -413,7 +451,16 @@ __global__ void __launch_bounds__(256, (G >= 8 || MODE == 3) ? 2 : 3) smac_kerne
               S = mont_redc(lo[i][cpn], hi[i][cpn], mc.q, mc.qinv_neg);
               lo[i][cpn] = hi[i][cpn] = 0;
             }
-            tot[i][cpn] = addmod(tot[i][cpn], mont_mul(S, m, mc.q, mc.qinv_neg), mc.q);
+            const u64 prod = mont_mul(S, m, mc.q, mc.qinv_neg);
+            if (TS) {
+              // first segment: nothing to add; last segment: straight to the output (a one-segment group never touches s_tot)
+              u64 *slot = s_tot + (size_t)(i * 2 + cpn) * blockDim.x + threadIdx.x;
+              const u64 v = seg == 0 ? prod : addmod(*slot, prod, mc.q);
+              if (seg + 1 < g.n_seg) *slot = v;
+              else if (i < g.n_out) p.outs[g.out_start + i][(cpn ? LN : 0u) + idx] = v;
+            } else {
+              tot[i][cpn] = addmod(tot[i][cpn], prod, mc.q);
+            }
           }
         lazy = 0;
         seg++;
@@ -421,13 +468,15 @@ __global__ void __launch_bounds__(256, (G >= 8 || MODE == 3) ? 2 : 3) smac_kerne
       }
     }
   }
+  if (!TS || seg == 0) {  // TS: a group without any segment (no terms) is all zero
 #pragma unroll
-  for (int i = 0; i < G; i++)
-    if (i < g.n_out) {
-      u64 *out = p.outs[g.out_start + i];
-      out[idx] = tot[i][0];
-      out[LN + idx] = tot[i][1];
-    }
+    for (int i = 0; i < G; i++)
+      if (i < g.n_out) {
+        u64 *out = p.outs[g.out_start + i];
+        out[idx] = TS ? 0 : tot[i][0];
+        out[LN + idx] = TS ? 0 : tot[i][1];
+      }
+  }
 }
 // Single-output groups in fp64 mode (depthwise layers: every output has its own ciphertext sequence, nothing to share):
 // a streaming kernel, two adjacent coefficients per thread with 16-byte loads, the loads of up to four terms of a mask
@@ -505,12 +554,22 @@ __global__ void __launch_bounds__(256, 4) smac1_kernel(SmacP p) {
   *reinterpret_cast<ulonglong2 *>(out + idx) = make_ulonglong2(tot[0], tot[1]);
   *reinterpret_cast<ulonglong2 *>(out + LN + idx) = make_ulonglong2(tot[2], tot[3]);
 }
+template <int G, int MODE>
+static void launch_smac_g(const SmacP &p, dim3 grid, int nth, cudaStream_t st) {
+  const size_t dyn = G >= 4 ? (size_t)G * 2 * nth * sizeof(u64) : 0;  // the totals over the mask segments (TS)
+  static bool attr_set = false;  // static + dynamic shared memory pass 48 KB for G = 8
+  if (dyn && !attr_set) {
+    cudaFuncSetAttribute(smac_kernel<G, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)G * 2 * 256 * sizeof(u64)));
+    attr_set = true;
+  }
+  smac_kernel<G, MODE><<<grid, nth, dyn, st>>>(p);
+}
 template <int MODE>
 static void launch_smac(const SmacP &p, dim3 grid, int nth, cudaStream_t st, int max_group) {
-  if (max_group <= 1) smac_kernel<1, MODE><<<grid, nth, 0, st>>>(p);
-  else if (max_group <= 2) smac_kernel<2, MODE><<<grid, nth, 0, st>>>(p);
-  else if (max_group <= 4 || MODE == 3) smac_kernel<4, MODE><<<grid, nth, 0, st>>>(p);  // MODE 3: the caller groups by 4 (3 sums per accumulator)
-  else smac_kernel<FENC_SMAC_GROUP, MODE><<<grid, nth, 0, st>>>(p);
+  if (max_group <= 1) launch_smac_g<1, MODE>(p, grid, nth, st);
+  else if (max_group <= 2) launch_smac_g<2, MODE>(p, grid, nth, st);
+  else if (max_group <= 4 || MODE == 3) launch_smac_g<4, MODE>(p, grid, nth, st);  // MODE 3: the caller groups by 4 (3 sums per accumulator)
+  else launch_smac_g<FENC_SMAC_GROUP, MODE>(p, grid, nth, st);
 }
 // k_mode: 0 integer, 1 fp64 residues, 2 / 3 signed multipliers with the ciphertext word split in 2 x 25 / 3 x 17 bits
 int k_smac(const KCtx &k, const SmacGroup *groups, int n_groups, int max_group, const u64 *const *term_ct, const int *kidx,
