@@ -266,7 +266,7 @@ __global__ void __launch_bounds__(256, (G >= 8 || MODE == 3) ? 2 : 3) smac_kerne
   // TS (groups of 4 and more outputs): the running totals over the mask segments live in shared memory (dynamic, one slot
   // per thread, output and component), touched at segment ends only.  In registers they took 4 G of the 128 a thread may
   // have beside the 4 G (6 G) accumulators, and the compiler rebuilt every loop invariant (thread index, limb offset,
-  // ring addresses) in every term: 106 instructions per term around 32 DFMA (ncu, profiles/r02_smac_loop_before.md).
+  // ring addresses) in every term: 106 instructions per term around 32 DFMA (ncu, profiles/r02_late_captures.md).
   constexpr bool TS = G >= 4;
   extern __shared__ u64 s_tot[];  // TS: [G][2][blockDim.x]
   __shared__ const u64 *s_ct[SMAC_TILE];
