@@ -158,11 +158,15 @@ __global__ void __launch_bounds__(MAC_THREADS, 512 / MAC_THREADS) mac_kernel(Mac
     if (!live) continue;
     // Integer modes (0, 1): the operands of the next MAC_RING - 1 terms are in flight while this term's products run, in a
     // per-thread cp.async ring in shared memory (every thread owns its slots: no barrier, no registers spent on the depth):
-    // config 3's 26-bit-limb MAC -11 %.  The fp64 mode (2) keeps plain loads: measured with the ring it is 8 % SLOWER
-    // (config 2's conv2: 1.38 -> 1.49 ms) -- it is bound by its 10 FP64 operations per output-term, not by the latency,
-    // and the ring's shared-memory traffic competes with them (round 1 saw the same with every staged variant).
+    // config 3's 26-bit-limb MAC -11 %.  The fp64 mode (2) keeps plain loads in batches of three terms.  ncu (config 2's
+    // conv2, profiles/r02_late_captures.md): half of all stall samples sit on the first use of a loaded word, the FP64 pipe
+    // is 41 % busy.  Measured against batches of two (2.40 ms of MAC per LeNet-5 step): batches of three 2.08 ms, of four
+    // 2.41 ms; the ring +8 % (its shared-memory wavefronts compete with the loads); three register sets with the loads of
+    // terms t+1, t+2 requested before term t's products 3.44 ms; groups of two outputs at three blocks per SM 2.59 ms; one
+    // ciphertext component per thread (half the accumulators, up to twice the warps) 2.97-5.03 ms; 4-64 consecutive
+    // coefficient chunks per group in the block order 2.11-2.47 ms.  More warps or more requests in flight make it slower.
     if (MODE == 2) {
-#pragma unroll 2
+#pragma unroll 3
       for (int t = 0; t < nt; t++) {
         const u64 *c = s_ct[t];
         const u64 x0 = __ldg(c + idx), x1 = __ldg(c + LN + idx);
