@@ -655,6 +655,50 @@ def test_import_async_matches_import(mods):
     ctx.close()
 
 
+def test_export_async_survives_free_and_reuse_of_the_ciphertext(mods):
+    """fenc_ct_export_async reads the ciphertext in stream order and copies on a stream of its own (include/fenc.h): the
+    handle may be freed right after the call and its memory reused by later work; the staging queue of the imports grows
+    with a cap (FENC_STAGE_MAX_MB, here 1 MiB = two slots: every upload then waits for its slot's previous transform);
+    fenc_sync, not only fenc_export_wait, makes the results visible; the device bytes held return to their level once the
+    exports have landed."""
+    import os
+    import torch
+    ck, fr, fenc = mods
+    os.environ["FENC_STAGE_MAX_MB"] = "1"
+    try:
+        P, ctx = make(mods, "mid12")
+        gk = ctx.keygen(4, [1, 2])
+        views = []
+        for i in range(24):
+            a = wl.random_ct_limbs(700 + i, P.q, P.nq, P.N)
+            views.append(torch.from_numpy(a.view(np.int64)).pin_memory().numpy().view(np.uint64))
+        want = [ctx.ct_export(ctx.rotate(gk, [ctx.ct_import(a)], [1])[0]) for a in views]
+        ctx.sync()
+        base, held = ctx.device_bytes(), None
+        for rnd in range(2):  # second round: the export buffers and events of the first are reused
+            outs = [torch.zeros(v.shape, dtype=torch.int64).pin_memory().numpy().view(np.uint64) for v in views]
+            for a, o in zip(views, outs):
+                c = ctx.rotate(gk, [ctx.ct_import_async(a)], [1])[0]
+                ctx.ct_export_async(c, o)
+                del c  # freed while the export is in flight: the next iteration's buffers come from the same pool
+            junk = ctx.rotate(gk, [ctx.ct_import(views[0])] * 8, [2] * 8)  # more work behind the exports, reusing freed blocks
+            if rnd == 0:
+                ctx.export_wait()
+            else:
+                ctx.sync()
+            for w_, o in zip(want, outs):
+                assert np.array_equal(w_, o)
+            del junk
+            ctx.sync()
+            if held is None:
+                held = ctx.device_bytes()  # what stays: the staging slots of the imports, capped
+                assert 0 < held - base <= (1 << 20) + 2 * P.nq * P.N * 8
+            assert ctx.device_bytes() == held  # every export buffer has returned
+        ctx.close()
+    finally:
+        del os.environ["FENC_STAGE_MAX_MB"]
+
+
 # ------------------------------------------------------------------------------------------------ fc, pooling, pipeline
 @pytest.mark.parametrize("kw", [
     dict(BS=2, n_in=32, n_out=5, in_C=2, in_H=4, in_W=4, in_M=4),
