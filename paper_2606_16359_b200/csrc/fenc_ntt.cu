@@ -462,9 +462,14 @@ struct NttRowP {
 #ifndef FENC_SLAB_MIN_BATCH
 #define FENC_SLAB_MIN_BATCH 4
 #endif
-#ifndef FENC_SLAB_BPB
-#define FENC_SLAB_BPB 4
-#endif
+// batch items per block: the longer the walk, the fewer copies of the twiddles (config-4 step, 32 images: 2 items 618.5 ms,
+// 4 items 605.9, 8 items 600.6, 16 items 599.1), as long as the grid still has blocks for every SM
+// (8 waves of 148 x 6 blocks; config 2's grids at N = 2^14 are small and keep 4: with 16 its step went 6.49 -> 6.60 ms)
+static inline int slab_bpb(long blocks_per_item, int n_batch) {
+  for (int b = 16; b > 4; b >>= 1)
+    if (blocks_per_item * ((n_batch + b - 1) / b) >= 8L * 148 * 6) return b;
+  return 4;
+}
 static inline bool use_slab(const NttGeom &g, int n_batch) { return g.logN >= 12 && n_batch >= FENC_SLAB_MIN_BATCH; }
 static inline size_t slab_bytes(const NttGeom &g) { return (sizeof(u64) << g.lt_row) + (sizeof(ShoupC) << g.lt_row); }
 template <int GEO, bool SLAB = false>
@@ -515,9 +520,9 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? 6 : 4) ntt_ro
 static void launch_ntt_rowpass(const KCtx &k, NttRowP r, int n_rows, int n_batch) {
   const NttGeom &g = k.geom;
   cudaStream_t st = (cudaStream_t)k.stream;
-  r.n_batch = n_batch, r.bpb = FENC_SLAB_BPB;
+  r.n_batch = n_batch, r.bpb = slab_bpb((long)(k.N >> g.lt_row) * n_rows, n_batch);
   if (use_slab(g, n_batch)) {
-    dim3 sgrid(k.N >> g.lt_row, n_rows, (n_batch + FENC_SLAB_BPB - 1) / FENC_SLAB_BPB);
+    dim3 sgrid(k.N >> g.lt_row, n_rows, (n_batch + r.bpb - 1) / r.bpb);
     ntt_rowpass_kernel<1, true><<<sgrid, nthreads_for(g.lt_row), slab_bytes(g), st>>>(r);
   } else {
     dim3 grid2((unsigned)((k.N >> g.lt_row) / (g.logN >= 12 ? FENC_ROW_TPB : 1)), n_rows, n_batch);
@@ -840,11 +845,11 @@ int k_ntt_rows_divide(const KCtx &k, const BatchItem *items, const u64 *tmp, siz
   if (n_rows == 0 || n_batch == 0) return 0;
   const NttGeom &g = k.geom;
   DivideP p{items, tmp, tmp_bstride, acc, acc_bstride, mul, rows, k.d_mods, k.d_tw_fwd, g, minuend_from_items ? 1 : 0, merged_mul2,
-            n_batch, FENC_SLAB_BPB};
+            n_batch, slab_bpb((long)(k.N >> g.lt_row) * n_rows, n_batch)};
   dim3 grid(row_grid_x(g, k.N), n_rows, n_batch);
   PROF(k, K_DIVIDE, 8.0 * k.N * (3.5 * n_rows) * n_batch, HALF_N(k) * g.brow * n_rows * n_batch);  // temp + minuend + output, addend on half the rows
   if (use_slab(g, n_batch)) {
-    dim3 sgrid(k.N >> g.lt_row, n_rows, (n_batch + FENC_SLAB_BPB - 1) / FENC_SLAB_BPB);
+    dim3 sgrid(k.N >> g.lt_row, n_rows, (n_batch + p.bpb - 1) / p.bpb);
     if (merged_mul2) ntt_rows_divide_kernel<1, true, true><<<sgrid, nthreads_for(g.lt_row), slab_bytes(g), (cudaStream_t)k.stream>>>(p);
     else ntt_rows_divide_kernel<1, false, true><<<sgrid, nthreads_for(g.lt_row), slab_bytes(g), (cudaStream_t)k.stream>>>(p);
   } else if (merged_mul2)
