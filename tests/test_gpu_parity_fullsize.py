@@ -322,6 +322,30 @@ def test_rotation_wide_and_unfused_digits(mods, n_q, n_p, dnum):
     ctx.close()
 
 
+def test_more_targets_than_staged_descriptors(mods):
+    """60 ciphertext limbs, digits of 6 (N=2^12): a ModUp group has 60 targets and a rescale 59, more than the 56 target
+    descriptors the fused column kernel stages in shared memory (CONV_DESC_CAP) -- the targets past the cap take their
+    descriptors and constants from global memory.  A batch of five rotations (slab row passes: batches of four and more)
+    and a batched rescale against the oracle, limb by limb."""
+    ck, fr, fenc = mods
+    P, ctx = make(mods, dict(log2N=12, n_q=60, q_bits=50, n_p=6, p_bits=60, dnum=10, log2_scale=50))
+    assert P.nq + len(P.p) - P.dlen > 56
+    steps = [3, P.n - 7]
+    ok, gk = ck.keygen(P, 11, steps), ctx.keygen(11, steps)
+    L = P.nq
+    limbs = [wl.random_ct_limbs(260 + i, P.q, L, P.N) for i in range(2)]
+    gin = [ctx.ct_import(a) for a in limbs]
+    outs = ctx.rotate(gk, [gin[0], gin[1], gin[0], gin[1], gin[0]], [3, 3, P.n - 7, P.n - 7, 3])
+    jobs = [(0, 3, False), (1, 3, False), (0, P.n - 7, False), (1, P.n - 7, False)]
+    refs = pmap(dict(ck=ck, P=P, keys=ok, inputs={i: ck.Ciphertext(a, L, 1) for i, a in enumerate(limbs)}), job_rotate, jobs)
+    for o, ref in zip(outs, refs + refs[:1]):
+        assert np.array_equal(ctx.ct_export(o), ref)
+    res = ctx.rescale(outs[:4])
+    for o, ref in zip(res, refs):
+        assert o.L == L - 1 and np.array_equal(ctx.ct_export(o), ck.rescale(P, ck.Ciphertext(ref, L, 2.0 ** 50)).c)
+    ctx.close()
+
+
 def test_rotation_config5_L36_dnum1_full_size(mods):
     """Config 5's largest point, N=2^16, L=36, dnum=1 (k = dlen = 36, 72 moduli): one rotation out of a batch of three
     checked fully against the oracle (unfused key switch: 36 source limbs do not fit the fused column kernel)."""
