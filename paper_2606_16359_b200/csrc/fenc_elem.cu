@@ -254,6 +254,7 @@ struct SmacP {
   const SmacGroup *groups; const u64 *const *term_ct; const int *kidx; const ShoupC *kpair; const int *seg_end;
   const u64 *const *seg_mask; u64 *const *outs; const ModConst *mods; int L, logN, max_lazy;
   int signed_k;  // kpair entries hold {(double) k, 0} with k the SIGNED multiplier (split modes) instead of {k mod q, (k mod q) / q}
+  int cpb;       // consecutive coefficient chunks (of blockDim.x words, all in one limb) a block of smac_kernel walks over
 };
 #define SMAC_TILE 64
 #ifndef SMAC_RING
@@ -278,8 +279,11 @@ __global__ void __launch_bounds__(256, (G >= 8 || MODE == 3) ? 2 : 3) smac_kerne
   __shared__ __align__(16) double s_kd[SPLIT ? SMAC_TILE : 1][SPLIT ? G : 1];  // split modes: the G multipliers of a term side by side
   __shared__ u64 s_ring[G >= 4 ? SMAC_RING : 1][2][G >= 4 ? 256 : 1];
   const u32 LN = (u32)p.L << p.logN;                           // L N < 2^32 (at most 2^7 limbs of 2^17 coefficients)
-  const u32 idx = blockIdx.y * blockDim.x + threadIdx.x;       // blockDim divides N: idx < L N, one limb per block
-  const int limb = (int)((blockIdx.y * blockDim.x) >> p.logN);
+  // a block walks over p.cpb consecutive chunks of one limb: the pointers and multipliers of a group of at most SMAC_TILE
+  // terms are staged once for all of them (a block of the pointwise layers lives for 32-64 terms only; ncu: 7 % of its
+  // stall samples on the staging's dependent loads and barrier)
+  u32 idx = blockIdx.y * p.cpb * blockDim.x + threadIdx.x;     // blockDim divides N: idx < L N, one limb per block
+  const int limb = (int)((blockIdx.y * p.cpb * blockDim.x) >> p.logN);
   const SmacGroup g = p.groups[blockIdx.x];
   const ModConst mc = p.mods[limb];
   F64Mod fm = f64mod(mc.q, mc.f64);
@@ -290,6 +294,7 @@ __global__ void __launch_bounds__(256, (G >= 8 || MODE == 3) ? 2 : 3) smac_kerne
   double acc[F64 ? G : 1][2];
   double sp[SPLIT ? G : 1][2][NP];
   u64 lo[MODE == 0 ? G : 1][2], hi[MODE == 0 ? G : 1][2], tot[TS ? 1 : G][2];
+  for (int cc = 0; cc < p.cpb; cc++, idx += blockDim.x) {
 #pragma unroll
   for (int i = 0; i < G; i++) {
     if (!TS) tot[i][0] = tot[i][1] = 0;
@@ -315,6 +320,7 @@ __global__ void __launch_bounds__(256, (G >= 8 || MODE == 3) ? 2 : 3) smac_kerne
   int seg = 0, cur_end = p.seg_end[g.seg_start], lazy = 0;
   for (int t0 = 0; t0 < g.n_terms; t0 += SMAC_TILE) {
     const int nt = g.n_terms - t0 < SMAC_TILE ? g.n_terms - t0 : SMAC_TILE;
+    if (cc == 0 || g.n_terms > SMAC_TILE) {  // a single tile of terms stays staged for the block's later chunks
     __syncthreads();
     for (int j = threadIdx.x; j < nt * (G + 1); j += blockDim.x) {
       const int i = j / nt, t = j - i * nt;
@@ -328,6 +334,7 @@ __global__ void __launch_bounds__(256, (G >= 8 || MODE == 3) ? 2 : 3) smac_kerne
       }
     }
     __syncthreads();
+    }
     // the next term's ciphertext words are requested before this term's products (register double buffer): with two blocks
     // of 8 warps per SM the loads would otherwise sit in front of 112 dependent FP64 operations
     // Groups of 4 and more outputs: the ciphertext words of the next SMAC_RING - 1 terms are in flight while this term's
@@ -481,6 +488,7 @@ __global__ void __launch_bounds__(256, (G >= 8 || MODE == 3) ? 2 : 3) smac_kerne
         out[LN + idx] = TS ? 0 : tot[i][1];
       }
   }
+  }  // chunks of the block
 }
 // Single-output groups in fp64 mode (depthwise layers: every output has its own ciphertext sequence, nothing to share):
 // a streaming kernel, two adjacent coefficients per thread with 16-byte loads, the loads of up to four terms of a mask
@@ -581,9 +589,15 @@ int k_smac(const KCtx &k, const SmacGroup *groups, int n_groups, int max_group, 
            int max_lazy, double alg_bytes, double alg_mulaccs) {
   if (n_groups == 0) return 0;
   if (k_mode == 3 && max_group > 4) return -3;
-  SmacP p{groups, term_ct, kidx, kpair, seg_end, seg_mask, outs, k.d_mods, L, k.geom.logN, max_lazy < 2 ? 2 : max_lazy, k_mode >= 2 ? 1 : 0};
+  SmacP p{groups, term_ct, kidx, kpair, seg_end, seg_mask, outs, k.d_mods, L, k.geom.logN, max_lazy < 2 ? 2 : max_lazy, k_mode >= 2 ? 1 : 0, 1};
   const int nth = k.N < 256 ? k.N : 256;
-  dim3 grid(n_groups, (unsigned)(((size_t)L * k.N) / nth));
+  // chunks per block of the grouped kernel: SMAC_CPB when a limb has that many and the grid keeps eight waves of blocks
+  const size_t chunks = ((size_t)L * k.N) / nth;
+#ifndef SMAC_CPB
+#define SMAC_CPB 8
+#endif
+  if ((k.N / nth) % SMAC_CPB == 0 && (size_t)n_groups * (chunks / SMAC_CPB) >= (size_t)8 * 148 * 2) p.cpb = SMAC_CPB;
+  dim3 grid(n_groups, (unsigned)(chunks / p.cpb));
   PROF2(k, K_SMAC, alg_bytes, alg_mulaccs);  // second counter of this class: modular multiply-accumulates
   if (k_mode >= 1 && max_group <= 1 && k.N >= 512) smac1_kernel<<<dim3(n_groups, (unsigned)(((size_t)L * k.N) / 512)), 256, 0, S(k)>>>(p);
   else if (k_mode == 3) launch_smac<3>(p, grid, nth, S(k), max_group);
