@@ -471,7 +471,9 @@ static inline int slab_bpb(long blocks_per_item, int n_batch) {
   return 4;
 }
 static inline bool use_slab(const NttGeom &g, int n_batch) { return g.logN >= 12 && n_batch >= FENC_SLAB_MIN_BATCH; }
-static inline size_t slab_bytes(const NttGeom &g) { return (sizeof(u64) << g.lt_row) + (sizeof(ShoupC) << g.lt_row); }
+static inline size_t slab_bytes(const NttGeom &g) {  // tile, twiddle slab, the item descriptors of the divide pass
+  return (sizeof(u64) << g.lt_row) + (sizeof(ShoupC) << g.lt_row) + 16 * sizeof(BatchItem);
+}
 template <int GEO, bool SLAB = false>
 __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? 6 : 4) ntt_rowpass_kernel(NttRowP p) {
   static_assert(!SLAB || GEO == 1, "slabs: compile-time row geometry");
@@ -784,17 +786,19 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, 4) ntt_rows_divide_kerne
     }
   };
   request(0);
-  if constexpr (SLAB) tw_slab_fill<FENC_ROW_LT>(slab, p.tw + (size_t)rd.mod * N, logN, blockIdx.x, tid, nth);
-  BatchItem it = p.items[b0];
+  // SLAB: the descriptors of the block's items are copied to shared memory behind the slab (read from global memory one
+  // iteration ahead, their first use -- a pointer moved to a uniform register -- still held 5 % of the stall samples)
+  BatchItem *s_items = reinterpret_cast<BatchItem *>(sm + 3 * (size_t)T);
+  if constexpr (SLAB) {
+    tw_slab_fill<FENC_ROW_LT>(slab, p.tw + (size_t)rd.mod * N, logN, blockIdx.x, tid, nth);
+    static_assert(sizeof(BatchItem) % 8 == 0, "copied as 64-bit words");
+    for (int i = tid; i < n_it * (int)(sizeof(BatchItem) / 8); i += nth)
+      reinterpret_cast<u64 *>(s_items)[i] = reinterpret_cast<const u64 *>(p.items + b0)[i];
+  }
 #pragma unroll 1
   for (int k = 0; k < n_it; k++) {
     const int b = SLAB ? b0 + k : b0;
     TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, SLAB ? blockIdx.x : blockIdx.x * TPB + k};
-    const u64 *minuend = (p.from_items ? it.sub_in : p.acc + (size_t)b * p.acc_bstride) + (size_t)rd.aux2 * N;
-    const u64 *addend = rd.aux == 0 ? it.add0 : it.add1;
-    if (addend) addend += (size_t)rd.mod * N;
-    u64 *dst = it.out + (size_t)rd.dst_row * N;
-    const u32 gal = it.g;
 #pragma unroll
     for (int i = 0; i < 8; i++) {
       const int e = tid + i * nth;
@@ -802,6 +806,12 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, 4) ntt_rows_divide_kerne
     }
     if (SLAB && k == 0) tw_slab_wait();
     __syncthreads();
+    const BatchItem it = SLAB ? s_items[k] : p.items[b0];
+    const u64 *minuend = (p.from_items ? it.sub_in : p.acc + (size_t)b * p.acc_bstride) + (size_t)rd.aux2 * N;
+    const u64 *addend = rd.aux == 0 ? it.add0 : it.add1;
+    if (addend) addend += (size_t)rd.mod * N;
+    u64 *dst = it.out + (size_t)rd.dst_row * N;
+    const u32 gal = it.g;
     // epilogue operands of this tile and the words of the next tile are fetched BEFORE the transform: their latency hides behind it
     u64 mi[8], ad[8];
 #pragma unroll
@@ -810,10 +820,7 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, 4) ntt_rows_divide_kerne
       mi[i] = __ldg(minuend + j);
       ad[i] = addend ? __ldg(addend + galois_src(j, gal, logN)) : 0;
     }
-    if (k + 1 < n_it) {
-      request(k + 1);
-      if (SLAB) it = p.items[b + 1];
-    }
+    if (k + 1 < n_it) request(k + 1);
     if constexpr (SLAB) tile_transform<true, GEO, 2>(sm, row_slab_geo<FENC_ROW_LT>(), 0, p.g.brow, slab, q, tid, mq.f64);
     else tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid, mq.f64);
 #pragma unroll
