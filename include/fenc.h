@@ -178,7 +178,10 @@ fenc_status fenc_ct_import(fenc_ctx *ctx, const uint64_t *limbs, uint32_t L, dou
  * (overlapping work already enqueued on the context's stream), the NTT follows on the context's stream.  `limbs`
  * (host; page-locked memory for a truly asynchronous copy) stays owned by the caller and must remain valid and
  * unchanged until the next synchronising call on this context returns (fenc_sync, fenc_ct_export, any decrypt).
- * Serving loops use it to upload the next request while the current one computes. */
+ * Serving loops use it to upload the next request while the current one computes.  The copies land
+ * in a queue of staging buffers that the library grows on demand (while the oldest buffer still waits for its transform)
+ * up to 8 GiB of device memory, or FENC_STAGE_MAX_MB MiB if that environment variable is set when the context's first
+ * asynchronous import runs; at the cap an upload waits for the transform that frees the oldest buffer. */
 fenc_status fenc_ct_import_async(fenc_ctx *ctx, const uint64_t *limbs, uint32_t L, double scale, fenc_ct **out);
 /* fenc_ct_export without the host synchronisation: the inverse transform is enqueued on the context's stream, the
  * device->host copy on a second stream of the context's own, so kernels enqueued behind the export do not wait for the
