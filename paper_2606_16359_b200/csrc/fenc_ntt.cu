@@ -339,7 +339,10 @@ __global__ void __launch_bounds__(128 * NG, NG == 1 ? 5 : (NG == 2 ? 2 : 1)) con
 }
 
 // thread groups per block of the fused column kernel for digit groups of n_src limbs
-static inline int convert_groups(int n_src, bool merged) { return (merged || n_src < 6) ? 1 : (n_src < 8 ? 2 : 4); }
+// digits of 6-9 limbs: two groups per block, two blocks per SM; from 10 limbs four groups, one block per SM (config 5,
+// measured: digits of 8 with two groups 4464 rotations/s, with four 4397; digits of 12 with two groups 3789, with four 4275)
+#define CONV_NG4_FROM 10
+static inline int convert_groups(int n_src, bool merged) { return (merged || n_src < 6) ? 1 : (n_src < CONV_NG4_FROM ? 2 : 4); }
 static inline size_t convert_smem(int n_src, int ng) {  // source + work tiles, twiddle buffers, target descriptors
   return (size_t)(n_src + ng) * 8192 + (size_t)ng * CONV_TW_WORDS * 8 + (size_t)CONV_DESC_CAP * sizeof(TgtDesc);
 }

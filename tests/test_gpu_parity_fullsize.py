@@ -302,10 +302,10 @@ def test_transformer_linear_fragment_embeddings_full_size_sampled(mods):
     ctx.close()
 
 
-@pytest.mark.parametrize("n_q,n_p,dnum", [(12, 12, 1), (16, 16, 1), (24, 24, 1), (24, 12, 2), (26, 26, 1), (30, 30, 1)])
+@pytest.mark.parametrize("n_q,n_p,dnum", [(6, 6, 1), (8, 8, 1), (18, 9, 2), (12, 12, 1), (16, 16, 1), (24, 24, 1), (24, 12, 2), (26, 26, 1), (30, 30, 1)])
 def test_rotation_wide_and_unfused_digits(mods, n_q, n_p, dnum):
-    """Config 5's widest digits at N=2^12 (same kernels, 4 column tiles per limb): dlen 12, 16, 24 run the fused column
-    kernel with 4 thread groups sharing up to 24 source tiles; dlen 26 and 30 exceed its shared memory and take the
+    """Config 5's widest digits at N=2^12 (same kernels, 4 column tiles per limb): dlen 6, 8, 9 run the fused column kernel
+    with 2 thread groups per block, dlen 12, 16, 24 with 4 thread groups sharing up to 24 source tiles; dlen 26 and 30 exceed its shared memory and take the
     unfused inverse / base-conversion pair (the path of the L=36, dnum=1 point).  Top level and one level down (short
     digit), 50-bit ciphertext primes, 60-bit special primes (A2)."""
     ck, fr, fenc = mods
