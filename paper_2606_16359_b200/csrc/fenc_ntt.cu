@@ -627,7 +627,24 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? KEYMAC_BLOCKS
     cp_async_wait_all();
     __syncthreads();  // digit j's tile is complete, and every thread is done with the other buffer (digit j-1)
     if (j + 1 < p.beta) request(j + 1);
+    // KEYS (compile-time row geometry): this digit's key words for the thread's own elements are requested into shared
+    // memory before the transform and read after it (every thread owns its slots: no barrier).  Loaded after the transform
+    // in two batches of four elements, their latency was exposed twice per digit: the kernel has 12 warps per SM at 168
+    // registers to hide it with.
+    constexpr bool KEYS = GEO == 1;
+    u64 *skb = sm_all + 2 * (size_t)T, *ska = skb + T;
+    if constexpr (KEYS) {
+#pragma unroll
+      for (int i = 0; i < EPT; i++) {
+        const int e = (tid + i * nth) & (T - 1);
+        const u32 jj = G.gidx(e);
+        cp_async8(skb + e, kb + jj);
+        cp_async8(ska + e, ka + jj);
+      }
+      cp_async_commit();
+    }
     if (ti >= 0) tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)mod * N, mc.q, tid, mc.f64);
+    if constexpr (KEYS) cp_async_wait_all();  // (the next digit's tile has had the transform's time as well)
     // the key words (and, inside the digit, the permuted input words) of 4 elements are loaded together, then used
 #pragma unroll
     for (int h = 0; h < EPT; h += HB) {
@@ -637,8 +654,8 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? KEYMAC_BLOCKS
       for (int i = 0; i < HB; i++) {
         const int e = (tid + (h + i) * nth) & (T - 1);
         jj[i] = G.gidx(e);
-        vb[i] = __ldg(kb + jj[i]);
-        va[i] = __ldg(ka + jj[i]);
+        vb[i] = KEYS ? skb[e] : __ldg(kb + jj[i]);
+        va[i] = KEYS ? ska[e] : __ldg(ka + jj[i]);
         if (ti >= 0) x[i] = sm[swz(e)];
         else x[i] = __ldg(it.ks_in + (size_t)t * N + galois_src(jj[i], it.g, p.g.logN));
       }
@@ -678,7 +695,7 @@ int k_ntt_rows_keymac(const KCtx &k, const BatchItem *items, int L, int E, int b
   // algorithmic bytes: ModUp temp + the switched polynomial read once, accumulators written once, each key once
   PROF(k, K_KEYMAC, 8.0 * k.N * (((double)n_up + L + 2.0 * E) * n_batch + 2.0 * beta * E * n_distinct_keys),
        HALF_N(k) * g.brow * n_up * n_batch);
-  if (g.logN >= 12) ntt_rows_keymac_kernel<8, 1><<<grid, nth, 2 * (sizeof(u64) << g.lt_row), (cudaStream_t)k.stream>>>(p);
+  if (g.logN >= 12) ntt_rows_keymac_kernel<8, 1><<<grid, nth, 4 * (sizeof(u64) << g.lt_row), (cudaStream_t)k.stream>>>(p);  // two tiles + the key words
   else if (ept <= 1) ntt_rows_keymac_kernel<1, 0><<<grid, nth, 2 * (sizeof(u64) << g.lt_row), (cudaStream_t)k.stream>>>(p);
   else if (ept <= 4) ntt_rows_keymac_kernel<4, 0><<<grid, nth, 2 * (sizeof(u64) << g.lt_row), (cudaStream_t)k.stream>>>(p);
   else ntt_rows_keymac_kernel<8, 0><<<grid, nth, 2 * (sizeof(u64) << g.lt_row), (cudaStream_t)k.stream>>>(p);
