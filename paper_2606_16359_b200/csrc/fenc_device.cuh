@@ -128,8 +128,13 @@ DEVI ulonglong2 tw_load(const ulonglong2 *p) {
   if constexpr (TWS != 0) return *p;
   else return __ldg(p);
 }
-template <bool FWD, bool LAZY, int PW, int SLO, int SHI, int F64, bool FIRST = true, bool LAST = true, int TWS = 0>  // F64: 0 integer, 1 fp64 narrow (q < 2^45), 2 fp64 wide
-DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid, u64 f64) {
+// REGIN (first round only): the round's eight inputs come from registers, vin[k] = element ebase + (k << PW) of the tile
+// (round_ebase<PW>(tid)), instead of shared memory: a kernel that loads the tile in that order skips the fill's stores,
+// the round's loads and one barrier per tile.
+template <int PW>
+DEVI int round_ebase(int tid) { return ((tid >> PW) << (PW + 3)) | (tid & ((1 << PW) - 1)); }
+template <bool FWD, bool LAZY, int PW, int SLO, int SHI, int F64, bool FIRST = true, bool LAST = true, int TWS = 0, bool REGIN = false>  // F64: 0 integer, 1 fp64 narrow (q < 2^45), 2 fp64 wide
+DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid, u64 f64, const u64 *vin = nullptr) {
   const int ebase = ((tid >> PW) << (PW + 3)) | (tid & ((1 << PW) - 1));
   const int gpw = G.gbit(PW);
   const u32 nj = (1u << G.logN) + G.gidx(ebase);
@@ -168,7 +173,7 @@ DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 
     double x[8];
 #pragma unroll
     for (int k = 0; k < 8; k++) {
-      const u64 v = sm[sbase ^ swz(k << PW)];
+      const u64 v = (REGIN && FIRST) ? vin[k] : sm[sbase ^ swz(k << PW)];
       x[k] = FIRST ? __dadd_rn(__hiloint2double((int)((u32)(v >> 32) | 0x43300000u), (int)(u32)v), in_off) : __longlong_as_double((long long)v);
     }
     int done = 0;
@@ -211,7 +216,7 @@ DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 
   } else {
   u64 x[8];
 #pragma unroll
-  for (int k = 0; k < 8; k++) x[k] = sm[sbase ^ swz(k << PW)];
+  for (int k = 0; k < 8; k++) x[k] = (REGIN && FIRST) ? vin[k] : sm[sbase ^ swz(k << PW)];
 #pragma unroll
   for (int ss = 0; ss < 3; ss++) {
     const int s = FWD ? 2 - ss : ss;
@@ -244,18 +249,28 @@ DEVI void tile_sync(int bar) {
   if constexpr (GRP) asm volatile("bar.sync %0, 128;" ::"r"(bar) : "memory");
   else __syncthreads();
 }
-template <bool FWD, bool LAZY, int LT, int LO, int NB, int DONE, int F64 = 0, bool GRP = false, int TWS = 0>
-DEVI void tile_rounds_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid, u64 f64 = 0, int bar = 0) {
+struct NoAfter { DEVI void operator()() const {} };
+// AF: called by every thread right after the first round (a REGIN caller requests the next tile into the registers the
+// round has just consumed)
+template <bool FWD, bool LAZY, int LT, int LO, int NB, int DONE, int F64 = 0, bool GRP = false, int TWS = 0, bool REGIN = false, class AF = NoAfter>
+DEVI void tile_rounds_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid, u64 f64 = 0, int bar = 0, const u64 *vin = nullptr, AF af = AF()) {
   if constexpr (DONE < NB) {
     constexpr int take = NB - DONE < 3 ? NB - DONE : 3;
     constexpr int cur = FWD ? LO + NB - DONE : LO + DONE;         // FWD: exclusive top; INV: inclusive bottom
     constexpr int p = FWD ? cur - take : cur;
     constexpr int pw = p < LT - 3 ? p : LT - 3;
-    if (tid < (1 << (LT - 3))) tile_round_ct<FWD, LAZY, pw, p - pw, p - pw + take, F64, DONE == 0, (DONE + take >= NB), TWS>(sm, G, tw, q, q2, tid, f64);
+    if (tid < (1 << (LT - 3))) tile_round_ct<FWD, LAZY, pw, p - pw, p - pw + take, F64, DONE == 0, (DONE + take >= NB), TWS, REGIN>(sm, G, tw, q, q2, tid, f64, vin);
+    if constexpr (DONE == 0) af();
     tile_sync<GRP>(bar);
-    tile_rounds_ct<FWD, LAZY, LT, LO, NB, DONE + take, F64, GRP, TWS>(sm, G, tw, q, q2, tid, f64, bar);
+    tile_rounds_ct<FWD, LAZY, LT, LO, NB, DONE + take, F64, GRP, TWS, false>(sm, G, tw, q, q2, tid, f64, bar);
   }
 }
+// window position of the FIRST round of a compile-time schedule (the order a REGIN caller loads the tile in)
+template <bool FWD, int LT, int LO, int NB>
+struct FirstRound {
+  static constexpr int take = NB < 3 ? NB : 3, p = FWD ? LO + NB - take : LO;
+  static constexpr int pw = p < LT - 3 ? p : LT - 3;
+};
 
 // runtime round (toy ring degrees and any geometry without a compile-time instance)
 template <bool FWD, bool F64>
@@ -338,10 +353,10 @@ DEVI TileGeo row_slab_geo() { return TileGeo{LT, LT, 0, LT, 0}; }
 // GEO selects the schedule: 0 = runtime (any lo/nb), 1 = row pass of 2048-element tiles with 8 stages,
 // 4..8 = column pass with GEO stages over tiles of 2^(GEO+4) elements (16 columns).
 // Every thread of the block must call this (it synchronises).  Outputs: forward < 33q (use fullred), inverse < 2q.
-template <bool FWD, int GEO, int TWS = 0>
-DEVI void tile_transform(u64 *sm, const TileGeo &G, int lo, int nb, const ShoupC *tw, u64 q, int tid, u64 f64) {
+template <bool FWD, int GEO, int TWS = 0, bool REGIN = false, class AF = NoAfter>
+DEVI void tile_transform(u64 *sm, const TileGeo &G, int lo, int nb, const ShoupC *tw, u64 q, int tid, u64 f64, const u64 *vin = nullptr, AF af = AF()) {
   const u64 q2 = q + q;
-  static_assert(!(TWS && GEO == 0), "twiddle slabs exist for the compile-time schedules only");
+  static_assert(!((TWS || REGIN) && GEO == 0), "twiddle slabs and register inputs exist for the compile-time schedules only");
   if constexpr (GEO == 0) {
     const bool active = tid < (1 << (G.lt - 3));
     if (FWD) {
@@ -366,9 +381,9 @@ DEVI void tile_transform(u64 *sm, const TileGeo &G, int lo, int nb, const ShoupC
     }
   } else {
     constexpr int LT = GEO == 1 ? FENC_ROW_LT : GEO + 4, LO = GEO == 1 ? 0 : 4, NB = GEO == 1 ? 8 : GEO;
-    if (f64 && q < (1ull << FENC_F64_MAX_BITS)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 1, false, TWS>(sm, G, tw, q, q2, tid, f64);
-    else if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 2, false, TWS>(sm, G, tw, q, q2, tid, f64);
-    else if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 0, false, TWS>(sm, G, tw, q, q2, tid);
-    else tile_rounds_ct<FWD, false, LT, LO, NB, 0, 0, false, TWS>(sm, G, tw, q, q2, tid);
+    if (f64 && q < (1ull << FENC_F64_MAX_BITS)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 1, false, TWS, REGIN, AF>(sm, G, tw, q, q2, tid, f64, 0, vin, af);
+    else if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 2, false, TWS, REGIN, AF>(sm, G, tw, q, q2, tid, f64, 0, vin, af);
+    else if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 0, false, TWS, REGIN, AF>(sm, G, tw, q, q2, tid, 0, 0, vin, af);
+    else tile_rounds_ct<FWD, false, LT, LO, NB, 0, 0, false, TWS, REGIN, AF>(sm, G, tw, q, q2, tid, 0, 0, vin, af);
   }
 }

@@ -492,12 +492,17 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? 6 : 4) ntt_ro
   const ModConst mc = p.mods[rd.mod];
   ShoupC *slab = reinterpret_cast<ShoupC *>(sm + T);
   u64 v[8];
+  // SLAB: the tile is loaded in the order of the transform's first round (element round_ebase(tid) + (i << PW0): runs of
+  // 32 consecutive words per warp and i), which takes it from the registers: no fill, one barrier less per tile, and the
+  // next tile is requested into the same registers right behind that round
+  constexpr int PW0 = FirstRound<true, FENC_ROW_LT, 0, 8>::pw;
+  const int eb0 = round_ebase<PW0>(tid);
   auto request = [&](int k) {
     TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, SLAB ? blockIdx.x : blockIdx.x * TPB + k};
     const u64 *src = p.src + (size_t)(SLAB ? b0 + k : b0) * p.src_bstride + src_off;
 #pragma unroll
     for (int i = 0; i < 8; i++) {
-      const int e = tid + i * nth;
+      const int e = SLAB ? eb0 + (i << PW0) : tid + i * nth;
       if (e < T) v[i] = src[G.gidx(e)];
     }
   };
@@ -507,16 +512,23 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? 6 : 4) ntt_ro
   for (int k = 0; k < n_it; k++) {
     TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, SLAB ? blockIdx.x : blockIdx.x * TPB + k};
     u64 *dst = p.dst + (size_t)(SLAB ? b0 + k : b0) * p.dst_bstride + dst_off;
+    if constexpr (SLAB) {
+      if (k == 0) {
+        tw_slab_wait();
+        __syncthreads();
+      }
+      auto next = [&]() { if (k + 1 < n_it) request(k + 1); };
+      tile_transform<true, GEO, 2, true>(sm, row_slab_geo<FENC_ROW_LT>(), 0, p.g.brow, slab, mc.q, tid, mc.f64, v, next);
+    } else {
 #pragma unroll
     for (int i = 0; i < 8; i++) {
       const int e = tid + i * nth;
       if (e < T) sm[swz(e)] = v[i];
     }
-    if (SLAB && k == 0) tw_slab_wait();
     __syncthreads();
     if (k + 1 < n_it) request(k + 1);
-    if constexpr (SLAB) tile_transform<true, GEO, 2>(sm, row_slab_geo<FENC_ROW_LT>(), 0, p.g.brow, slab, mc.q, tid, mc.f64);
-    else tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, mc.q, tid, mc.f64);
+    tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, mc.q, tid, mc.f64);
+    }
     tile_drain(sm, T, tid, nth, [&](int e, u64 x) { dst[G.gidx(e)] = fullred(x, mc.q, mc.qbar); });
     if (k + 1 < n_it) __syncthreads();  // every thread has read its results before the next tile overwrites them
   }
@@ -796,12 +808,14 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, 4) ntt_rows_divide_kerne
   const int n_it = SLAB ? min(p.bpb, p.n_batch - b0) : TPB;
   ShoupC *slab = reinterpret_cast<ShoupC *>(sm + T);
   u64 v[8];
+  constexpr int PW0 = FirstRound<true, FENC_ROW_LT, 0, 8>::pw;  // SLAB: tile loaded in the first round's order (ntt_rowpass_kernel)
+  const int eb0 = round_ebase<PW0>(tid);
   auto request = [&](int k) {  // iteration k's tile of the temp
     TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, SLAB ? blockIdx.x : blockIdx.x * TPB + k};
     const u64 *src = p.tmp + (size_t)(SLAB ? b0 + k : b0) * p.tmp_bstride + (size_t)rd.src_row * N;
 #pragma unroll
     for (int i = 0; i < 8; i++) {
-      const int e = tid + i * nth;
+      const int e = SLAB ? eb0 + (i << PW0) : tid + i * nth;
       if (e < T) v[i] = src[G.gidx(e)];
     }
   };
@@ -819,13 +833,19 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, 4) ntt_rows_divide_kerne
   for (int k = 0; k < n_it; k++) {
     const int b = SLAB ? b0 + k : b0;
     TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, SLAB ? blockIdx.x : blockIdx.x * TPB + k};
+    if constexpr (SLAB) {
+      if (k == 0) {
+        tw_slab_wait();
+        __syncthreads();  // slab and item descriptors are in place
+      }
+    } else {
 #pragma unroll
-    for (int i = 0; i < 8; i++) {
-      const int e = tid + i * nth;
-      if (e < T) sm[swz(e)] = v[i];
+      for (int i = 0; i < 8; i++) {
+        const int e = tid + i * nth;
+        if (e < T) sm[swz(e)] = v[i];
+      }
+      __syncthreads();
     }
-    if (SLAB && k == 0) tw_slab_wait();
-    __syncthreads();
     const BatchItem it = SLAB ? s_items[k] : p.items[b0];
     const u64 *minuend = (p.from_items ? it.sub_in : p.acc + (size_t)b * p.acc_bstride) + (size_t)rd.aux2 * N;
     const u64 *addend = rd.aux == 0 ? it.add0 : it.add1;
@@ -840,9 +860,13 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, 4) ntt_rows_divide_kerne
       mi[i] = __ldg(minuend + j);
       ad[i] = addend ? __ldg(addend + galois_src(j, gal, logN)) : 0;
     }
-    if (k + 1 < n_it) request(k + 1);
-    if constexpr (SLAB) tile_transform<true, GEO, 2>(sm, row_slab_geo<FENC_ROW_LT>(), 0, p.g.brow, slab, q, tid, mq.f64);
-    else tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid, mq.f64);
+    if constexpr (SLAB) {
+      auto next = [&]() { if (k + 1 < n_it) request(k + 1); };
+      tile_transform<true, GEO, 2, true>(sm, row_slab_geo<FENC_ROW_LT>(), 0, p.g.brow, slab, q, tid, mq.f64, v, next);
+    } else {
+      if (k + 1 < n_it) request(k + 1);
+      tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid, mq.f64);
+    }
 #pragma unroll
     for (int i = 0; i < 8; i++) {
       const int e = tid + i * nth;

@@ -80,3 +80,20 @@ def test_column_pass_twiddles_fit_the_staged_256_entries():
                 for s in stages:
                     for i in range(1 << (2 - s)):
                         assert 1 <= (nj >> (gpw + s + 1)) + i <= 255
+
+
+def test_first_round_order_covers_the_tile_in_coalesced_runs():
+    """REGIN (row kernels, slab form): thread tid loads element round_ebase<PW0>(tid) + (i << PW0), PW0 = 5 for the forward
+    row pass -- every element of the tile exactly once, 32 consecutive words per warp and i, and exactly the elements the
+    first round (window PW0) gives that thread."""
+    PW0 = ROUNDS_FWD[0][0]
+    seen = set()
+    for tid in range(NT8):
+        eb = ((tid >> PW0) << (PW0 + 3)) | (tid & ((1 << PW0) - 1))
+        for i in range(8):
+            seen.add(eb + (i << PW0))
+    assert seen == set(range(T))
+    for warp in range(NT8 // 32):
+        for i in range(8):
+            run = [(((t >> PW0) << (PW0 + 3)) | (t & ((1 << PW0) - 1))) + (i << PW0) for t in range(32 * warp, 32 * warp + 32)]
+            assert run == list(range(run[0], run[0] + 32))
