@@ -309,13 +309,13 @@ DEVI void tile_round_rt(u64 *sm, const TileGeo &G, int pw, int s_lo, int s_hi, c
 
 // compile-time schedule over active tile bits [LO, LO+NB) of a 2^LT-element tile; picks the lazy forward butterflies
 // for q < 2^58.  Every thread of the block must call this (it synchronises).
-template <bool FWD, int LT, int LO, int NB, bool GRP = false, int TWS = 0>
-DEVI void tile_transform_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, int tid, u64 f64, int bar = 0) {
+template <bool FWD, int LT, int LO, int NB, bool GRP = false, int TWS = 0, bool REGIN = false>
+DEVI void tile_transform_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, int tid, u64 f64, int bar = 0, const u64 *vin = nullptr) {
   const u64 q2 = q + q;
-  if (f64 && q < (1ull << FENC_F64_MAX_BITS)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 1, GRP, TWS>(sm, G, tw, q, q2, tid, f64, bar);
-  else if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 2, GRP, TWS>(sm, G, tw, q, q2, tid, f64, bar);
-  else if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 0, GRP, TWS>(sm, G, tw, q, q2, tid, 0, bar);
-  else tile_rounds_ct<FWD, false, LT, LO, NB, 0, 0, GRP, TWS>(sm, G, tw, q, q2, tid, 0, bar);
+  if (f64 && q < (1ull << FENC_F64_MAX_BITS)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 1, GRP, TWS, REGIN>(sm, G, tw, q, q2, tid, f64, bar, vin);
+  else if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 2, GRP, TWS, REGIN>(sm, G, tw, q, q2, tid, f64, bar, vin);
+  else if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 0, GRP, TWS, REGIN>(sm, G, tw, q, q2, tid, 0, bar, vin);
+  else tile_rounds_ct<FWD, false, LT, LO, NB, 0, 0, GRP, TWS, REGIN>(sm, G, tw, q, q2, tid, 0, bar, vin);
 }
 
 // The twiddles of a ROW pass over the 2^LT contiguous coefficients of tile `tile`, copied to shared memory in heap order:

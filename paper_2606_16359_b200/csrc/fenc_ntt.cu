@@ -327,11 +327,12 @@ __global__ void __launch_bounds__(128 * NG, NG == 1 ? 5 : (NG == 2 ? 2 : 1)) con
 #pragma unroll
       for (int i = 0; i < 8; i++) v[i] = addmod(shoup_mul(v[i], pt.c, pt.cs, mc.q), fullred(outl[i], mc.q, mc.qbar), mc.q);
     }
-#pragma unroll
-    for (int i = 0; i < 8; i++) W[swz(tid + i * NTH)] = v[i];
+    // the converted values go straight into the first forward round: its window sits on the top three tile bits, so the
+    // elements it gives thread tid are tid + i NTH, the ones this thread has just produced
+    static_assert(FirstRound<true, LT, LC, BCOL>::pw == LT - 3, "first forward round over the top tile bits");
     cp_async_wait_all();
-    tile_sync<GRP>(bar);
-    tile_transform_ct<true, LT, LC, BCOL, GRP, 1>(W, G, twb, mc.q, tid, mc.f64, bar);
+    tile_sync<GRP>(bar);  // the twiddles are in place
+    tile_transform_ct<true, LT, LC, BCOL, GRP, 1, true>(W, G, twb, mc.q, tid, mc.f64, bar, v);
     u64 *dst = p.tmp + (size_t)b * p.tmp_bstride + (size_t)rd.dst_row * N;
     tile_drain(W, T, tid, NTH, [&](int e, u64 v) { dst[G.gidx(e)] = v; });  // lazy, below 33q
     tile_sync<GRP>(bar);
