@@ -133,8 +133,10 @@ DEVI ulonglong2 tw_load(const ulonglong2 *p) {
 // the round's loads and one barrier per tile.
 template <int PW>
 DEVI int round_ebase(int tid) { return ((tid >> PW) << (PW + 3)) | (tid & ((1 << PW) - 1)); }
-template <bool FWD, bool LAZY, int PW, int SLO, int SHI, int F64, bool FIRST = true, bool LAST = true, int TWS = 0, bool REGIN = false>  // F64: 0 integer, 1 fp64 narrow (q < 2^45), 2 fp64 wide
-DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid, u64 f64, const u64 *vin = nullptr) {
+// REGOUT (last round only): the round's eight results stay in registers, vout[k] = element ebase + (k << PW), in the
+// form the round would have stored (unsigned lazy words); the caller drains them itself.
+template <bool FWD, bool LAZY, int PW, int SLO, int SHI, int F64, bool FIRST = true, bool LAST = true, int TWS = 0, bool REGIN = false, bool REGOUT = false>  // F64: 0 integer, 1 fp64 narrow (q < 2^45), 2 fp64 wide
+DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid, u64 f64, const u64 *vin = nullptr, u64 *vout = nullptr) {
   const int ebase = ((tid >> PW) << (PW + 3)) | (tid & ((1 << PW) - 1));
   const int gpw = G.gbit(PW);
   const u32 nj = (1u << G.logN) + G.gidx(ebase);
@@ -208,7 +210,11 @@ DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 
       // makes them non-negative and keeps them below 2^52; reduced values (+ q) land in (0, 2q)
       const double off = red ? __dadd_rn(fm.q, 4503599627370496.0) : __fma_rn(16.0, fm.q, 4503599627370496.0);
 #pragma unroll
-      for (int k = 0; k < 8; k++) sm[sbase ^ swz(k << PW)] = d2u_off(red ? reduce_dd(x[k], fm) : x[k], off);
+      for (int k = 0; k < 8; k++) {
+        const u64 r = d2u_off(red ? reduce_dd(x[k], fm) : x[k], off);
+        if (REGOUT) vout[k] = r;
+        else sm[sbase ^ swz(k << PW)] = r;
+      }
     } else {
 #pragma unroll
       for (int k = 0; k < 8; k++) sm[sbase ^ swz(k << PW)] = (u64)__double_as_longlong(red ? reduce_dd(x[k], fm) : x[k]);
@@ -239,7 +245,10 @@ DEVI void tile_round_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 
     }
   }
 #pragma unroll
-  for (int k = 0; k < 8; k++) sm[sbase ^ swz(k << PW)] = x[k];
+  for (int k = 0; k < 8; k++) {
+    if (REGOUT && LAST) vout[k] = x[k];
+    else sm[sbase ^ swz(k << PW)] = x[k];
+  }
   }
 }
 
@@ -252,19 +261,27 @@ DEVI void tile_sync(int bar) {
 struct NoAfter { DEVI void operator()() const {} };
 // AF: called by every thread right after the first round (a REGIN caller requests the next tile into the registers the
 // round has just consumed)
-template <bool FWD, bool LAZY, int LT, int LO, int NB, int DONE, int F64 = 0, bool GRP = false, int TWS = 0, bool REGIN = false, class AF = NoAfter>
-DEVI void tile_rounds_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid, u64 f64 = 0, int bar = 0, const u64 *vin = nullptr, AF af = AF()) {
+template <bool FWD, bool LAZY, int LT, int LO, int NB, int DONE, int F64 = 0, bool GRP = false, int TWS = 0, bool REGIN = false, class AF = NoAfter, bool REGOUT = false>
+DEVI void tile_rounds_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, u64 q2, int tid, u64 f64 = 0, int bar = 0, const u64 *vin = nullptr, AF af = AF(), u64 *vout = nullptr) {
   if constexpr (DONE < NB) {
     constexpr int take = NB - DONE < 3 ? NB - DONE : 3;
     constexpr int cur = FWD ? LO + NB - DONE : LO + DONE;         // FWD: exclusive top; INV: inclusive bottom
     constexpr int p = FWD ? cur - take : cur;
     constexpr int pw = p < LT - 3 ? p : LT - 3;
-    if (tid < (1 << (LT - 3))) tile_round_ct<FWD, LAZY, pw, p - pw, p - pw + take, F64, DONE == 0, (DONE + take >= NB), TWS, REGIN>(sm, G, tw, q, q2, tid, f64, vin);
+    constexpr bool last = DONE + take >= NB;
+    if (tid < (1 << (LT - 3))) tile_round_ct<FWD, LAZY, pw, p - pw, p - pw + take, F64, DONE == 0, last, TWS, REGIN, REGOUT>(sm, G, tw, q, q2, tid, f64, vin, vout);
     if constexpr (DONE == 0) af();
-    tile_sync<GRP>(bar);
-    tile_rounds_ct<FWD, LAZY, LT, LO, NB, DONE + take, F64, GRP, TWS, false>(sm, G, tw, q, q2, tid, f64, bar);
+    if constexpr (!(REGOUT && last)) tile_sync<GRP>(bar);  // (a REGOUT caller synchronises before the tile is written again)
+    tile_rounds_ct<FWD, LAZY, LT, LO, NB, DONE + take, F64, GRP, TWS, false, NoAfter, REGOUT>(sm, G, tw, q, q2, tid, f64, bar, nullptr, NoAfter(), vout);
   }
 }
+// window position of the LAST round of a compile-time schedule (the order a REGOUT caller drains in)
+template <bool FWD, int LT, int LO, int NB>
+struct LastRound {
+  static constexpr int rem = NB % 3 == 0 ? 3 : NB % 3;                 // stages of the last round
+  static constexpr int p = FWD ? LO : LO + NB - rem;
+  static constexpr int pw = p < LT - 3 ? p : LT - 3;
+};
 // window position of the FIRST round of a compile-time schedule (the order a REGIN caller loads the tile in)
 template <bool FWD, int LT, int LO, int NB>
 struct FirstRound {
@@ -309,13 +326,13 @@ DEVI void tile_round_rt(u64 *sm, const TileGeo &G, int pw, int s_lo, int s_hi, c
 
 // compile-time schedule over active tile bits [LO, LO+NB) of a 2^LT-element tile; picks the lazy forward butterflies
 // for q < 2^58.  Every thread of the block must call this (it synchronises).
-template <bool FWD, int LT, int LO, int NB, bool GRP = false, int TWS = 0, bool REGIN = false>
-DEVI void tile_transform_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, int tid, u64 f64, int bar = 0, const u64 *vin = nullptr) {
+template <bool FWD, int LT, int LO, int NB, bool GRP = false, int TWS = 0, bool REGIN = false, bool REGOUT = false>
+DEVI void tile_transform_ct(u64 *sm, const TileGeo &G, const ShoupC *tw, u64 q, int tid, u64 f64, int bar = 0, const u64 *vin = nullptr, u64 *vout = nullptr) {
   const u64 q2 = q + q;
-  if (f64 && q < (1ull << FENC_F64_MAX_BITS)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 1, GRP, TWS, REGIN>(sm, G, tw, q, q2, tid, f64, bar, vin);
-  else if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 2, GRP, TWS, REGIN>(sm, G, tw, q, q2, tid, f64, bar, vin);
-  else if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 0, GRP, TWS, REGIN>(sm, G, tw, q, q2, tid, 0, bar, vin);
-  else tile_rounds_ct<FWD, false, LT, LO, NB, 0, 0, GRP, TWS, REGIN>(sm, G, tw, q, q2, tid, 0, bar, vin);
+  if (f64 && q < (1ull << FENC_F64_MAX_BITS)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 1, GRP, TWS, REGIN, NoAfter, REGOUT>(sm, G, tw, q, q2, tid, f64, bar, vin, NoAfter(), vout);
+  else if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 2, GRP, TWS, REGIN, NoAfter, REGOUT>(sm, G, tw, q, q2, tid, f64, bar, vin, NoAfter(), vout);
+  else if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 0, GRP, TWS, REGIN, NoAfter, REGOUT>(sm, G, tw, q, q2, tid, 0, bar, vin, NoAfter(), vout);
+  else tile_rounds_ct<FWD, false, LT, LO, NB, 0, 0, GRP, TWS, REGIN, NoAfter, REGOUT>(sm, G, tw, q, q2, tid, 0, bar, vin, NoAfter(), vout);
 }
 
 // The twiddles of a ROW pass over the 2^LT contiguous coefficients of tile `tile`, copied to shared memory in heap order:
@@ -353,8 +370,8 @@ DEVI TileGeo row_slab_geo() { return TileGeo{LT, LT, 0, LT, 0}; }
 // GEO selects the schedule: 0 = runtime (any lo/nb), 1 = row pass of 2048-element tiles with 8 stages,
 // 4..8 = column pass with GEO stages over tiles of 2^(GEO+4) elements (16 columns).
 // Every thread of the block must call this (it synchronises).  Outputs: forward < 33q (use fullred), inverse < 2q.
-template <bool FWD, int GEO, int TWS = 0, bool REGIN = false, class AF = NoAfter>
-DEVI void tile_transform(u64 *sm, const TileGeo &G, int lo, int nb, const ShoupC *tw, u64 q, int tid, u64 f64, const u64 *vin = nullptr, AF af = AF()) {
+template <bool FWD, int GEO, int TWS = 0, bool REGIN = false, class AF = NoAfter, bool REGOUT = false>
+DEVI void tile_transform(u64 *sm, const TileGeo &G, int lo, int nb, const ShoupC *tw, u64 q, int tid, u64 f64, const u64 *vin = nullptr, AF af = AF(), u64 *vout = nullptr) {
   const u64 q2 = q + q;
   static_assert(!((TWS || REGIN) && GEO == 0), "twiddle slabs and register inputs exist for the compile-time schedules only");
   if constexpr (GEO == 0) {
@@ -381,9 +398,9 @@ DEVI void tile_transform(u64 *sm, const TileGeo &G, int lo, int nb, const ShoupC
     }
   } else {
     constexpr int LT = GEO == 1 ? FENC_ROW_LT : GEO + 4, LO = GEO == 1 ? 0 : 4, NB = GEO == 1 ? 8 : GEO;
-    if (f64 && q < (1ull << FENC_F64_MAX_BITS)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 1, false, TWS, REGIN, AF>(sm, G, tw, q, q2, tid, f64, 0, vin, af);
-    else if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 2, false, TWS, REGIN, AF>(sm, G, tw, q, q2, tid, f64, 0, vin, af);
-    else if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 0, false, TWS, REGIN, AF>(sm, G, tw, q, q2, tid, 0, 0, vin, af);
-    else tile_rounds_ct<FWD, false, LT, LO, NB, 0, 0, false, TWS, REGIN, AF>(sm, G, tw, q, q2, tid, 0, 0, vin, af);
+    if (f64 && q < (1ull << FENC_F64_MAX_BITS)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 1, false, TWS, REGIN, AF, REGOUT>(sm, G, tw, q, q2, tid, f64, 0, vin, af, vout);
+    else if (f64) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 2, false, TWS, REGIN, AF, REGOUT>(sm, G, tw, q, q2, tid, f64, 0, vin, af, vout);
+    else if (FWD && q < (1ull << 58)) tile_rounds_ct<FWD, true, LT, LO, NB, 0, 0, false, TWS, REGIN, AF, REGOUT>(sm, G, tw, q, q2, tid, 0, 0, vin, af, vout);
+    else tile_rounds_ct<FWD, false, LT, LO, NB, 0, 0, false, TWS, REGIN, AF, REGOUT>(sm, G, tw, q, q2, tid, 0, 0, vin, af, vout);
   }
 }

@@ -332,10 +332,15 @@ __global__ void __launch_bounds__(128 * NG, NG == 1 ? 5 : (NG == 2 ? 2 : 1)) con
     static_assert(FirstRound<true, LT, LC, BCOL>::pw == LT - 3, "first forward round over the top tile bits");
     cp_async_wait_all();
     tile_sync<GRP>(bar);  // the twiddles are in place
-    tile_transform_ct<true, LT, LC, BCOL, GRP, 1, true>(W, G, twb, mc.q, tid, mc.f64, bar, v);
+    // ... and the last round's results leave from registers (same 32-byte runs per row as a drain through shared memory)
+    constexpr int PWL = LastRound<true, LT, LC, BCOL>::pw;
+    u64 r[8];
+    tile_transform_ct<true, LT, LC, BCOL, GRP, 1, true, true>(W, G, twb, mc.q, tid, mc.f64, bar, v, r);
     u64 *dst = p.tmp + (size_t)b * p.tmp_bstride + (size_t)rd.dst_row * N;
-    tile_drain(W, T, tid, NTH, [&](int e, u64 v) { dst[G.gidx(e)] = v; });  // lazy, below 33q
-    tile_sync<GRP>(bar);
+    const int ebl = round_ebase<PWL>(tid);
+#pragma unroll
+    for (int k = 0; k < 8; k++) dst[G.gidx(ebl + (k << PWL))] = r[k];  // lazy, below 33q
+    tile_sync<GRP>(bar);  // every thread is done with W before the next target's first round writes it
   }
 }
 
@@ -519,7 +524,14 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? 6 : 4) ntt_ro
         __syncthreads();
       }
       auto next = [&]() { if (k + 1 < n_it) request(k + 1); };
-      tile_transform<true, GEO, 2, true>(sm, row_slab_geo<FENC_ROW_LT>(), 0, p.g.brow, slab, mc.q, tid, mc.f64, v, next);
+      // the last round (window on the lowest bits) leaves its eight consecutive results in registers: 64 bytes per thread,
+      // stored as four 16-byte words
+      static_assert(LastRound<true, FENC_ROW_LT, 0, 8>::pw == 0, "last forward row round over the lowest tile bits");
+      u64 r[8];
+      tile_transform<true, GEO, 2, true, decltype(next), true>(sm, row_slab_geo<FENC_ROW_LT>(), 0, p.g.brow, slab, mc.q, tid, mc.f64, v, next, r);
+      ulonglong2 *d2 = reinterpret_cast<ulonglong2 *>(dst + G.gidx(8 * tid));
+#pragma unroll
+      for (int i = 0; i < 4; i++) d2[i] = make_ulonglong2(fullred(r[2 * i], mc.q, mc.qbar), fullred(r[2 * i + 1], mc.q, mc.qbar));
     } else {
 #pragma unroll
     for (int i = 0; i < 8; i++) {
@@ -529,9 +541,9 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? 6 : 4) ntt_ro
     __syncthreads();
     if (k + 1 < n_it) request(k + 1);
     tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, mc.q, tid, mc.f64);
-    }
     tile_drain(sm, T, tid, nth, [&](int e, u64 x) { dst[G.gidx(e)] = fullred(x, mc.q, mc.qbar); });
-    if (k + 1 < n_it) __syncthreads();  // every thread has read its results before the next tile overwrites them
+    }
+    if (k + 1 < n_it) __syncthreads();  // every thread is done with the tile before the next one overwrites it
   }
 }
 // launch of the forward row pass over (rows x batch), slab form for batches
