@@ -866,27 +866,37 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, 4) ntt_rows_divide_kerne
     u64 *dst = it.out + (size_t)rd.dst_row * N;
     const u32 gal = it.g;
     // epilogue operands of this tile and the words of the next tile are fetched BEFORE the transform: their latency hides behind it
-    u64 mi[8], ad[8];
+    // SLAB: the last round keeps its results in registers (eight consecutive coefficients per thread), so the epilogue's
+    // operands are fetched in that order (16-byte loads) and the output leaves as four 16-byte stores
+    u64 mi[8], ad[8], xr[8];
 #pragma unroll
     for (int i = 0; i < 8; i++) {
-      const u32 j = G.gidx((tid + i * nth) & (T - 1));
-      mi[i] = __ldg(minuend + j);
+      const u32 j = G.gidx(SLAB ? 8 * tid + i : (tid + i * nth) & (T - 1));
+      if (!SLAB) mi[i] = __ldg(minuend + j);
       ad[i] = addend ? __ldg(addend + galois_src(j, gal, logN)) : 0;
     }
     if constexpr (SLAB) {
+      const ulonglong2 *m2p = reinterpret_cast<const ulonglong2 *>(minuend + G.gidx(8 * tid));
+#pragma unroll
+      for (int i = 0; i < 4; i++) {
+        const ulonglong2 m = __ldg(m2p + i);
+        mi[2 * i] = m.x, mi[2 * i + 1] = m.y;
+      }
       auto next = [&]() { if (k + 1 < n_it) request(k + 1); };
-      tile_transform<true, GEO, 2, true>(sm, row_slab_geo<FENC_ROW_LT>(), 0, p.g.brow, slab, q, tid, mq.f64, v, next);
+      tile_transform<true, GEO, 2, true, decltype(next), true>(sm, row_slab_geo<FENC_ROW_LT>(), 0, p.g.brow, slab, q, tid, mq.f64, v, next, xr);
     } else {
       if (k + 1 < n_it) request(k + 1);
       tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, q, tid, mq.f64);
     }
+    u64 res[8];
 #pragma unroll
     for (int i = 0; i < 8; i++) {
-      const int e = tid + i * nth;
+      const int e = SLAB ? 8 * tid + i : tid + i * nth;
       if (e < T) {
         // fp64 rows: X mod q as v - rint(v/q) q + q in (0, 2q) on the FP64 pipe; the Shoup multiply takes any 64-bit input
         const bool fp = mq.f64 != 0;
-        const u64 x = fp ? d2u_off(reduce_dd(u2d52(sm[swz(e)]), fm), fm.q + 4503599627370496.0) : fullred(sm[swz(e)], q, mq.qbar);
+        const u64 xv = SLAB ? xr[i] : sm[swz(e)];
+        const u64 x = fp ? d2u_off(reduce_dd(u2d52(xv), fm), fm.q + 4503599627370496.0) : fullred(xv, q, mq.qbar);
         u64 r;
         if (MERGED) {
           const ShoupC m2 = p.mul2[rd.mod];
@@ -896,8 +906,14 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, 4) ntt_rows_divide_kerne
           r = shoup_mul(fp ? mi[i] + 2 * q - x : submod(mi[i], x, q), mc.c, mc.cs, q);
           r = addmod(r, ad[i], q);
         }
-        dst[G.gidx(e)] = r;
+        if (SLAB) res[i] = r;
+        else dst[G.gidx(e)] = r;
       }
+    }
+    if constexpr (SLAB) {
+      ulonglong2 *d2 = reinterpret_cast<ulonglong2 *>(dst + G.gidx(8 * tid));
+#pragma unroll
+      for (int i = 0; i < 4; i++) d2[i] = make_ulonglong2(res[2 * i], res[2 * i + 1]);
     }
     if (k + 1 < n_it) __syncthreads();
   }
