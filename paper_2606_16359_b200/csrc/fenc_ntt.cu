@@ -498,9 +498,10 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? 6 : 4) ntt_ro
   const ModConst mc = p.mods[rd.mod];
   ShoupC *slab = reinterpret_cast<ShoupC *>(sm + T);
   u64 v[8];
-  // SLAB: the tile is loaded in the order of the transform's first round (element round_ebase(tid) + (i << PW0): runs of
-  // 32 consecutive words per warp and i), which takes it from the registers: no fill, one barrier less per tile, and the
-  // next tile is requested into the same registers right behind that round
+  // REG (compile-time row geometry, slab form or not): the tile is loaded in the order of the transform's first round
+  // (element round_ebase(tid) + (i << PW0): runs of 32 consecutive words per warp and i), which takes it from the registers:
+  // no fill, one barrier less per tile, and the next tile is requested into the same registers right behind that round
+  constexpr bool REG = GEO == 1;
   constexpr int PW0 = FirstRound<true, FENC_ROW_LT, 0, 8>::pw;
   const int eb0 = round_ebase<PW0>(tid);
   auto request = [&](int k) {
@@ -508,7 +509,7 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? 6 : 4) ntt_ro
     const u64 *src = p.src + (size_t)(SLAB ? b0 + k : b0) * p.src_bstride + src_off;
 #pragma unroll
     for (int i = 0; i < 8; i++) {
-      const int e = SLAB ? eb0 + (i << PW0) : tid + i * nth;
+      const int e = REG ? eb0 + (i << PW0) : tid + i * nth;
       if (e < T) v[i] = src[G.gidx(e)];
     }
   };
@@ -518,8 +519,8 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? 6 : 4) ntt_ro
   for (int k = 0; k < n_it; k++) {
     TileGeo G{p.g.lt_row, p.g.lt_row, 0, p.g.logN, SLAB ? blockIdx.x : blockIdx.x * TPB + k};
     u64 *dst = p.dst + (size_t)(SLAB ? b0 + k : b0) * p.dst_bstride + dst_off;
-    if constexpr (SLAB) {
-      if (k == 0) {
+    if constexpr (REG) {
+      if (SLAB && k == 0) {
         tw_slab_wait();
         __syncthreads();
       }
@@ -528,7 +529,8 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? 6 : 4) ntt_ro
       // stored as four 16-byte words
       static_assert(LastRound<true, FENC_ROW_LT, 0, 8>::pw == 0, "last forward row round over the lowest tile bits");
       u64 r[8];
-      tile_transform<true, GEO, 2, true, decltype(next), true>(sm, row_slab_geo<FENC_ROW_LT>(), 0, p.g.brow, slab, mc.q, tid, mc.f64, v, next, r);
+      if constexpr (SLAB) tile_transform<true, GEO, 2, true, decltype(next), true>(sm, row_slab_geo<FENC_ROW_LT>(), 0, p.g.brow, slab, mc.q, tid, mc.f64, v, next, r);
+      else tile_transform<true, GEO, 0, true, decltype(next), true>(sm, G, 0, p.g.brow, p.tw + (size_t)rd.mod * N, mc.q, tid, mc.f64, v, next, r);
       ulonglong2 *d2 = reinterpret_cast<ulonglong2 *>(dst + G.gidx(8 * tid));
 #pragma unroll
       for (int i = 0; i < 4; i++) d2[i] = make_ulonglong2(fullred(r[2 * i], mc.q, mc.qbar), fullred(r[2 * i + 1], mc.q, mc.qbar));
