@@ -9,6 +9,11 @@
 // The first touch of a forward transform and the last touch of either direction carry the fused work; for ring degrees
 // >= 2^12 the inverse column pass, the base conversion and the forward column pass of a key switch are ONE kernel
 // (convert_cols_kernel) that keeps the converted limbs in shared memory.
+// What the kernels stage in shared memory beside the tile (round 2, profiles/r02_late_captures.md): the row passes keep one
+// tile position per block over several batch items with that position's twiddles ("slab") and the items' descriptors; the
+// fused column kernel its targets' descriptors, each target's forward twiddles and base-conversion constants (cp.async);
+// the key inner product its digit's key words.  Where the load / store order allows, the first and the last round of a
+// transform work on registers (REGIN / REGOUT in fenc_device.cuh) instead of a fill / drain through shared memory.
 #include "fenc_device.cuh"
 
 // geometry dispatch: row kernels GEO in {0,1}; column kernels GEO in {0,4..8} (fenc_device.cuh tile_transform)
