@@ -651,6 +651,10 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? KEYMAC_BLOCKS
     cp_async_commit();
   };
   request(0);
+  // compile-time row geometry: the beta transforms of the block share tile position and modulus, so their twiddles are
+  // copied to shared memory once (the slab of the row passes, behind the tiles and the key words)
+  ShoupC *slab = reinterpret_cast<ShoupC *>(sm_all + 4 * (size_t)T);
+  if constexpr (GEO == 1) tw_slab_fill<FENC_ROW_LT>(slab, p.tw + (size_t)mod * N, p.g.logN, (u32)tile, tid, nth);
   for (int j = 0; j < p.beta; j++) {
     const int ti = p.tmp_index[j * p.E + t];
     const u64 *kb = it.evk + ((size_t)(j * 2 + 0) * p.A + mod) * N;
@@ -675,7 +679,10 @@ __global__ void __launch_bounds__(GEO == 1 ? 128 : 256, GEO == 1 ? KEYMAC_BLOCKS
       }
       cp_async_commit();
     }
-    if (ti >= 0) tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)mod * N, mc.q, tid, mc.f64);
+    if (ti >= 0) {
+      if constexpr (GEO == 1) tile_transform<true, GEO, 2>(sm, row_slab_geo<FENC_ROW_LT>(), 0, p.g.brow, slab, mc.q, tid, mc.f64);
+      else tile_transform<true, GEO>(sm, G, 0, p.g.brow, p.tw + (size_t)mod * N, mc.q, tid, mc.f64);
+    }
     if constexpr (KEYS) cp_async_wait_all();  // (the next digit's tile has had the transform's time as well)
     // the key words (and, inside the digit, the permuted input words) of 4 elements are loaded together, then used
 #pragma unroll
@@ -727,7 +734,14 @@ int k_ntt_rows_keymac(const KCtx &k, const BatchItem *items, int L, int E, int b
   // algorithmic bytes: ModUp temp + the switched polynomial read once, accumulators written once, each key once
   PROF(k, K_KEYMAC, 8.0 * k.N * (((double)n_up + L + 2.0 * E) * n_batch + 2.0 * beta * E * n_distinct_keys),
        HALF_N(k) * g.brow * n_up * n_batch);
-  if (g.logN >= 12) ntt_rows_keymac_kernel<8, 1><<<grid, nth, 4 * (sizeof(u64) << g.lt_row), (cudaStream_t)k.stream>>>(p);  // two tiles + the key words
+  if (g.logN >= 12) {  // two tiles + the key words + the twiddle slab: 48 KiB
+    static bool attr_set = false;
+    if (!attr_set) {
+      cudaFuncSetAttribute(ntt_rows_keymac_kernel<8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(6 * (sizeof(u64) << FENC_ROW_LT)));
+      attr_set = true;
+    }
+    ntt_rows_keymac_kernel<8, 1><<<grid, nth, 6 * (sizeof(u64) << g.lt_row), (cudaStream_t)k.stream>>>(p);
+  }
   else if (ept <= 1) ntt_rows_keymac_kernel<1, 0><<<grid, nth, 2 * (sizeof(u64) << g.lt_row), (cudaStream_t)k.stream>>>(p);
   else if (ept <= 4) ntt_rows_keymac_kernel<4, 0><<<grid, nth, 2 * (sizeof(u64) << g.lt_row), (cudaStream_t)k.stream>>>(p);
   else ntt_rows_keymac_kernel<8, 0><<<grid, nth, 2 * (sizeof(u64) << g.lt_row), (cudaStream_t)k.stream>>>(p);
